@@ -1,0 +1,157 @@
+/*
+ * ccsd.h -- C ABI of the B200-native complex spinor-basis CCSD hot path (arXiv 2103.08473, "ExaCorr").
+ *
+ * What the library computes: one iteration of the CCSD amplitude equations in complex (spinor) algebra,
+ * Appendix 7.1 of the paper (eqs 22-33): tau (eq 23), the Fock-like intermediates
+ * H^a_c/G^a_c, H^k_i/G^k_i, H^k_c (eqs 24-28), the particle-hole intermediate H^{ak}_{ci} (eq 29), C^{kb}_{ij}
+ * (eq 30), the hole-hole intermediate A^{kl}_{ij} (eq 31), the doubles residual S^{ab}_{ij} (eq 32: ring,
+ * hole-hole ladder, particle-particle ladder and the small terms) and the singles residual S^a_i (eq 33);
+ * followed by the denominator ("Jacobi") update with DIIS and the correlation
+ * energy (eq 9; contraction string PAPER.md:178-182).  Inputs are those of eq 5: the
+ * one-electron matrix h_pq and the two-electron integrals in factorised (Cholesky-type) form.
+ * Reading of the paper's notation: DESIGN.md "Readings of the paper".
+ *
+ * Conventions for EVERY entry point
+ *  - ccsd_c128 is an interleaved (re, im) pair of doubles, 16-byte aligned: binary compatible with
+ *    torch.complex128 / numpy.complex128 / CUDA double2.
+ *  - All tensor pointers are DEVICE pointers unless the comment says HOST.  Row-major, last index fastest.
+ *  - Spinors are ordered occupied first: o = nocc, v = nvir, n = o + v.  oo = o(o-1)/2, vv = v(v-1)/2.
+ *    A packed pair (x<y) of a dimension of size m has index  x*m - x(x+1)/2 + (y-x-1)  (row-major strict upper
+ *    triangle, the order of numpy.triu_indices(m, 1)).
+ *  - Canonical layouts at the boundary:  t1, S1 [i][a];  t2, tau, S2 [(i<j)][(a<b)];  <ab||cd> [(a<b)][(c<d)];
+ *    Hvv, Gvv [a][c];  Hoo, Goo [k][i];  Hov [k][c];  Hvovo [a][k][c][i];  C [k][b][(i<j)];  A [(k<l)][(i<j)].
+ *  - Ownership: the caller owns every buffer including `workspace`; the library never allocates or frees device
+ *    memory and never creates streams.  All work is enqueued on the caller's `cuda_stream` (a cudaStream_t).
+ *  - Errors: every call returns a CCSD_* status; nothing is thrown or printed.  There is no CPU fallback: without
+ *    a CUDA device every compute entry point returns CCSD_ECUDA.
+ */
+#ifndef CCSD_B200_H
+#define CCSD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ccsd_ctx ccsd_ctx; /* opaque, host-side handle */
+typedef struct { double re, im; } ccsd_c128;
+
+enum { CCSD_OK = 0, CCSD_EINVAL = 1, CCSD_ENOMEM = 2, CCSD_ECUDA = 3, CCSD_ESTATE = 4, CCSD_ESINGULAR = 5 };
+
+typedef struct {
+    int ndiis;          /* DIIS subspace size; 0 = plain Jacobi; default 6 (reading G13) */
+    double level_shift; /* added to the virtual orbital energies in the denominators; default 0 */
+    int gemm_mode;      /* 0 = auto (FP64 tensor-core DMMA kernels where the shape allows), 1 = force the simple
+                           FP64-FMA kernels (on-device debugging reference) */
+    int ccd;            /* 1 = CCD: t1 is kept at zero */
+} ccsd_options;
+
+/* Fill *opts with the defaults above. */
+void ccsd_default_options(ccsd_options* opts);
+
+/* Bytes of device workspace ccsd_init needs for (nocc, nvir, naux).  HOST out-pointer. */
+int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes);
+
+/*
+ * Set up a calculation: builds the Fock matrix f = h + sum_i <pi||qi>, the six
+ * antisymmetrised integral classes <pq||rs> = (pr|qs) - (ps|qr) with (pq|rs) = sum_L B[L][p][q] B[L][r][s], the
+ * orbital-energy denominators and the MP2 starting amplitudes ("iteration 0").
+ *   h  [n][n]         bare one-electron matrix of eq 5, Hermitian
+ *   B  [naux][n][n]   factor of the two-electron integrals, every B[L] Hermitian
+ *   workspace         at least ccsd_workspace_bytes() bytes, 256-byte aligned; must stay alive until ccsd_destroy
+ * h and B may be released after the call returns (the call synchronises the stream).
+ * Errors: CCSD_EINVAL (bad sizes / null pointers / workspace too small), CCSD_ECUDA.
+ */
+int ccsd_init(ccsd_ctx** ctx, const ccsd_c128* h, const ccsd_c128* B, int nocc, int nvir, int naux,
+              const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * One CCSD iteration at the current amplitudes: eqs 23-33, t <- t + S/D, DIIS extrapolation.
+ * HOST outputs: correlation energy (Re, Im) of the NEW amplitudes and ||S/D||_2 over the unique amplitudes of the
+ * residual just evaluated.  Synchronises the stream (one small device->host copy).
+ * Errors: CCSD_ESTATE (no context), CCSD_ESINGULAR (DIIS system singular even with one vector), CCSD_ECUDA.
+ */
+int ccsd_iterate(ccsd_ctx* ctx, double* e_re, double* e_im, double* step_norm);
+
+/* E_corr = sum f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij} of the current amplitudes (eq 9).  HOST outputs. */
+int ccsd_energy(ccsd_ctx* ctx, double* e_re, double* e_im);
+
+/* Evaluate eqs 23-33 at the current amplitudes WITHOUT updating them (fills the tensors ccsd_get_tensor returns). */
+int ccsd_residual(ccsd_ctx* ctx);
+
+/* Copy the current amplitudes out / in (device pointers): t1 [o][v], t2p [(i<j)][(a<b)].  Asynchronous. */
+int ccsd_get_amplitudes(ccsd_ctx* ctx, ccsd_c128* t1, ccsd_c128* t2p);
+int ccsd_set_amplitudes(ccsd_ctx* ctx, const ccsd_c128* t1, const ccsd_c128* t2p, int reset_diis);
+
+/* Tensor ids for ccsd_get_tensor; canonical layouts as listed at the top.  S2_* are the eight terms of eq 32. */
+enum {
+    CCSD_T_FOCK = 0,   /* [n][n] */
+    CCSD_T_VVVV = 1,   /* [(a<b)][(c<d)] */
+    CCSD_T_VOVV = 2,   /* [a][k][(c<d)] */
+    CCSD_T_VOVO = 3,   /* [a][k][c][i] */
+    CCSD_T_OOVV = 4,   /* [(k<l)][(c<d)] */
+    CCSD_T_OOOV = 5,   /* [(k<l)][i][c] */
+    CCSD_T_OOOO = 6,   /* [(k<l)][(i<j)] */
+    CCSD_T_TAU = 10, CCSD_T_HVV = 11, CCSD_T_GVV = 12, CCSD_T_HOO = 13, CCSD_T_GOO = 14, CCSD_T_HOV = 15,
+    CCSD_T_HVOVO = 16, CCSD_T_C = 17, CCSD_T_A = 18, CCSD_T_S1 = 19, CCSD_T_S2 = 20,
+    CCSD_T_S2_RING = 30, CCSD_T_S2_GOO = 31, CCSD_T_S2_VDAG_T1 = 32, CCSD_T_S2_GVV = 33, CCSD_T_S2_C_T1 = 34,
+    CCSD_T_S2_HH_LADDER = 35, CCSD_T_S2_PP_LADDER = 36, CCSD_T_S2_DRIVER = 37
+};
+/* Number of ccsd_c128 elements of tensor `tensor_id` (HOST out-pointer). */
+int ccsd_tensor_elems(ccsd_ctx* ctx, int tensor_id, size_t* elems);
+/* Copy tensor `tensor_id` into out (device).  Intermediates, S1, S2 are those of the last ccsd_residual/iterate;
+ * the S2_* ids re-evaluate that single term of eq 32 from the stored intermediates.  Asynchronous. */
+int ccsd_get_tensor(ccsd_ctx* ctx, int tensor_id, ccsd_c128* out);
+
+int ccsd_destroy(ccsd_ctx* ctx);
+
+/*
+ * Standalone contractions on caller-supplied tensors (per-term parity and timing; BASELINE config 4).
+ *   CCSD_TERM_PP_LADDER (eq 32; string form PAPER.md:176):
+ *        in[0] = tau [(i<j)][(c<d)], in[1] = W [(a<b)][(c<d)];  out [(i<j)][(a<b)] = sum_{c<d} W tau
+ *   CCSD_TERM_HH_LADDER (eq 32): in[0] = A [(k<l)][(i<j)], in[1] = tau [(k<l)][(a<b)];
+ *        out [(i<j)][(a<b)] = sum_{k<l} A tau
+ *   CCSD_TERM_RING (eq 32 first line): in[0] = Hvovo [a][k][c][i], in[1] = t2 [(i<j)][(a<b)];
+ *        out [(i<j)][(a<b)] = P-_ij P-_ab sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b]
+ *   CCSD_TERM_TAU (eq 23): in[0] = t1 [i][a], in[1] = t2 [(i<j)][(a<b)]; out = tau packed
+ * accumulate != 0 adds into out.  workspace: ccsd_contract_workspace_bytes() bytes.  Asynchronous on the stream.
+ */
+enum { CCSD_TERM_PP_LADDER = 0, CCSD_TERM_HH_LADDER = 1, CCSD_TERM_RING = 2, CCSD_TERM_TAU = 3 };
+int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes);
+int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd_c128* out, int accumulate,
+                  const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Generic complex GEMM used by every contraction above ("NT" form, both operands K-contiguous):
+ *   C[m*csm + n*csn] (+)= alpha * sum_k A[m*lda + k] * B[n*ldb + k]
+ * mode: 0 auto, 1 simple FMA kernel, 2 force the DMMA tensor-core kernel (CCSD_EINVAL if K % 4 != 0).
+ */
+int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
+                  ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
+                  void* cuda_stream);
+
+/*
+ * Tensor transposition ("A(a,c,b,d)+=B(a,b,c,d)"):  out[permuted index] = in[index]
+ * (conj != 0: complex conjugate).  dims = extents of `in`; out dimension d is in dimension perm[d].
+ */
+int ccsd_transpose(const ccsd_c128* in, ccsd_c128* out, const int64_t dims[4], const int perm[4], int conj,
+                   void* cuda_stream);
+
+/* Per-step device times (ms, CUDA events) of the last ccsd_iterate/ccsd_residual when timing was enabled. */
+enum { CCSD_NSTEPS = 16 };
+int ccsd_enable_step_timing(ccsd_ctx* ctx, int enable);
+int ccsd_get_step_times(ccsd_ctx* ctx, float ms[CCSD_NSTEPS]);
+const char* ccsd_step_name(int step);
+/* Kernel launches issued by the library since the last reset (all contexts, this process). */
+long long ccsd_launch_count(int reset);
+
+const char* ccsd_strerror(int status);
+/* Last CUDA error string seen by the library on this thread ("" if none). */
+const char* ccsd_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CCSD_B200_H */

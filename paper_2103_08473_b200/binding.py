@@ -1,0 +1,277 @@
+"""ctypes binding of include/ccsd.h (argument marshalling only; same names as the C entry points)."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+STATUS = {0: "CCSD_OK", 1: "CCSD_EINVAL", 2: "CCSD_ENOMEM", 3: "CCSD_ECUDA", 4: "CCSD_ESTATE", 5: "CCSD_ESINGULAR"}
+TENSOR_IDS = {"fock": 0, "vvvv": 1, "vovv": 2, "vovo": 3, "oovv": 4, "ooov": 5, "oooo": 6, "tau": 10, "Hvv": 11,
+              "Gvv": 12, "Hoo": 13, "Goo": 14, "Hov": 15, "Hvovo": 16, "C": 17, "A": 18, "S1": 19, "S2": 20,
+              "S2_ring": 30, "S2_goo": 31, "S2_vdag_t1": 32, "S2_gvv": 33, "S2_c_t1": 34, "S2_hh_ladder": 35,
+              "S2_pp_ladder": 36, "S2_driver": 37}
+TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3}
+NSTEPS = 16
+
+# every symbol include/ccsd.h declares
+EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_iterate", "ccsd_energy", "ccsd_residual",
+           "ccsd_get_amplitudes", "ccsd_set_amplitudes", "ccsd_tensor_elems", "ccsd_get_tensor", "ccsd_destroy",
+           "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_transpose",
+           "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count", "ccsd_strerror",
+           "ccsd_last_cuda_error"]
+
+
+class CCSDError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        lib = load_library()
+        msg = lib.ccsd_strerror(status).decode()
+        cuda = lib.ccsd_last_cuda_error().decode()
+        super().__init__(f"{where}: {STATUS.get(status, status)} ({msg}){' [' + cuda + ']' if cuda else ''}")
+        self.status = status
+
+
+class Options(ctypes.Structure):
+    _fields_ = [("ndiis", ctypes.c_int), ("level_shift", ctypes.c_double), ("gemm_mode", ctypes.c_int),
+                ("ccd", ctypes.c_int)]
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, "libccsd_b200.so")
+
+
+def load_library():
+    """dlopen the in-tree CUDA library; fails loudly if it has not been built (no fallback)."""
+    global _LIB
+    if _LIB is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: run `python -m paper_2103_08473_b200.build` (needs nvcc); "
+                              "there is no CPU fallback")
+        lib = ctypes.CDLL(path)
+        vp, i64, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double
+        lib.ccsd_default_options.argtypes = [ctypes.POINTER(Options)]
+        lib.ccsd_default_options.restype = None
+        lib.ccsd_workspace_bytes.argtypes = [ctypes.c_int] * 3 + [ctypes.POINTER(Options), ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_init.argtypes = [ctypes.POINTER(vp), vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                  ctypes.POINTER(Options), vp, ctypes.c_size_t, vp]
+        lib.ccsd_iterate.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
+        lib.ccsd_energy.argtypes = [vp] + [ctypes.POINTER(dbl)] * 2
+        lib.ccsd_residual.argtypes = [vp]
+        lib.ccsd_get_amplitudes.argtypes = [vp, vp, vp]
+        lib.ccsd_set_amplitudes.argtypes = [vp, vp, vp, ctypes.c_int]
+        lib.ccsd_tensor_elems.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_get_tensor.argtypes = [vp, ctypes.c_int, vp]
+        lib.ccsd_destroy.argtypes = [vp]
+        lib.ccsd_contract_workspace_bytes.argtypes = [ctypes.c_int] * 3 + [ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_contract.argtypes = [ctypes.c_int] * 3 + [ctypes.POINTER(vp), vp, ctypes.c_int,
+                                                            ctypes.POINTER(Options), vp, ctypes.c_size_t, vp]
+        lib.ccsd_zgemm_nt.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
+                                      ctypes.c_int, vp]
+        lib.ccsd_transpose.argtypes = [vp, vp, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_int), ctypes.c_int, vp]
+        lib.ccsd_enable_step_timing.argtypes = [vp, ctypes.c_int]
+        lib.ccsd_get_step_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+        lib.ccsd_step_name.argtypes = [ctypes.c_int]
+        lib.ccsd_step_name.restype = ctypes.c_char_p
+        lib.ccsd_launch_count.argtypes = [ctypes.c_int]
+        lib.ccsd_launch_count.restype = ctypes.c_longlong
+        lib.ccsd_strerror.argtypes = [ctypes.c_int]
+        lib.ccsd_strerror.restype = ctypes.c_char_p
+        lib.ccsd_last_cuda_error.restype = ctypes.c_char_p
+        _LIB = lib
+    return _LIB
+
+
+def _step_names():
+    lib = load_library()
+    return [lib.ccsd_step_name(k).decode() for k in range(NSTEPS)]
+
+
+class _LazyNames(list):
+    def _fill(self):
+        if not len(self):
+            self.extend(_step_names())
+
+    def __iter__(self):
+        self._fill()
+        return super().__iter__()
+
+    def __getitem__(self, k):
+        self._fill()
+        return super().__getitem__(k)
+
+
+STEP_NAMES = _LazyNames()
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise CCSDError(status, where)
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2103_08473_b200 needs a CUDA device (B200); there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(torch):
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev_c128(torch, x):
+    """host numpy / torch tensor -> contiguous complex128 CUDA tensor (marshalling only)."""
+    if not isinstance(x, torch.Tensor):
+        x = torch.from_numpy(x)
+    return x.to(device="cuda", dtype=torch.complex128).contiguous()
+
+
+def launch_count(reset: bool = False) -> int:
+    return int(load_library().ccsd_launch_count(1 if reset else 0))
+
+
+def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False) -> Options:
+    return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)))
+
+
+class CCSD:
+    """ccsd_init / ccsd_iterate / ccsd_energy / ccsd_get_* on device tensors.
+
+    h [n][n] and B [naux][n][n] may be numpy arrays (copied host->device here) or CUDA complex128 tensors.
+    """
+
+    def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
+                 ccd: bool = False):
+        torch = _torch()
+        lib = load_library()
+        self._lib, self._torch = lib, torch
+        self.nocc, self.nvir, self.n = int(nocc), int(nvir), int(nocc + nvir)
+        self.oo = self.nocc * (self.nocc - 1) // 2
+        self.vv = self.nvir * (self.nvir - 1) // 2
+        h_d, B_d = _dev_c128(torch, h), _dev_c128(torch, B)
+        self.naux = int(B_d.shape[0])
+        assert tuple(h_d.shape) == (self.n, self.n) and tuple(B_d.shape) == (self.naux, self.n, self.n)
+        self._opts = _options(ndiis, level_shift, gemm_mode, ccd)
+        nbytes = ctypes.c_size_t(0)
+        _check(lib.ccsd_workspace_bytes(self.nocc, self.nvir, self.naux, ctypes.byref(self._opts),
+                                        ctypes.byref(nbytes)), "ccsd_workspace_bytes")
+        self.workspace_bytes = int(nbytes.value)
+        self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device="cuda")
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        self._ctx = ctypes.c_void_p(None)
+        _check(lib.ccsd_init(ctypes.byref(self._ctx), h_d.data_ptr(), B_d.data_ptr(), self.nocc, self.nvir, self.naux,
+                             ctypes.byref(self._opts), base, self.workspace_bytes, _stream_ptr(torch)), "ccsd_init")
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._lib.ccsd_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p(None)
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def iterate(self):
+        """One CCSD iteration -> (complex E_corr of the new amplitudes, ||S/D||_2)."""
+        er, ei, sn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        st = self._lib.ccsd_iterate(self._ctx, ctypes.byref(er), ctypes.byref(ei), ctypes.byref(sn))
+        if st not in (0, 5):
+            _check(st, "ccsd_iterate")
+        return complex(er.value, ei.value), sn.value
+
+    def energy(self) -> complex:
+        er, ei = ctypes.c_double(), ctypes.c_double()
+        _check(self._lib.ccsd_energy(self._ctx, ctypes.byref(er), ctypes.byref(ei)), "ccsd_energy")
+        return complex(er.value, ei.value)
+
+    def residual(self):
+        _check(self._lib.ccsd_residual(self._ctx), "ccsd_residual")
+
+    def get_amplitudes(self):
+        torch = self._torch
+        t1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
+        t2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
+        _check(self._lib.ccsd_get_amplitudes(self._ctx, t1.data_ptr(), t2p.data_ptr()), "ccsd_get_amplitudes")
+        return t1, t2p
+
+    def set_amplitudes(self, t1, t2p, reset_diis: bool = True):
+        torch = self._torch
+        t1_d, t2_d = _dev_c128(torch, t1), _dev_c128(torch, t2p)
+        assert tuple(t1_d.shape) == (self.nocc, self.nvir) and tuple(t2_d.shape) == (self.oo, self.vv)
+        _check(self._lib.ccsd_set_amplitudes(self._ctx, t1_d.data_ptr(), t2_d.data_ptr(), int(reset_diis)),
+               "ccsd_set_amplitudes")
+        torch.cuda.current_stream().synchronize()
+
+    def get_tensor(self, name: str):
+        torch = self._torch
+        tid = TENSOR_IDS[name]
+        ne = ctypes.c_size_t(0)
+        _check(self._lib.ccsd_tensor_elems(self._ctx, tid, ctypes.byref(ne)), "ccsd_tensor_elems")
+        out = torch.empty(int(ne.value), dtype=torch.complex128, device="cuda")
+        _check(self._lib.ccsd_get_tensor(self._ctx, tid, out.data_ptr()), f"ccsd_get_tensor({name})")
+        return out
+
+    def enable_step_timing(self, enable: bool = True):
+        _check(self._lib.ccsd_enable_step_timing(self._ctx, int(enable)), "ccsd_enable_step_timing")
+
+    def step_times(self):
+        arr = (ctypes.c_float * NSTEPS)()
+        _check(self._lib.ccsd_get_step_times(self._ctx, arr), "ccsd_get_step_times")
+        return {n: float(arr[k]) for k, n in enumerate(STEP_NAMES)}
+
+
+def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool = False, gemm_mode: int = 0):
+    """ccsd_contract on CUDA tensors; returns out [(i<j)][(a<b)]."""
+    torch = _torch()
+    lib = load_library()
+    tid = TERM_IDS[term]
+    oo, vv = nocc * (nocc - 1) // 2, nvir * (nvir - 1) // 2
+    ins = [_dev_c128(torch, x) for x in inputs]
+    if out is None:
+        out = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
+    nbytes = ctypes.c_size_t(0)
+    _check(lib.ccsd_contract_workspace_bytes(tid, nocc, nvir, ctypes.byref(nbytes)), "ccsd_contract_workspace_bytes")
+    ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    arr = (ctypes.c_void_p * len(ins))(*[x.data_ptr() for x in ins])
+    opts = _options(gemm_mode=gemm_mode)
+    _check(lib.ccsd_contract(tid, nocc, nvir, arr, out.data_ptr(), int(accumulate), ctypes.byref(opts), base,
+                             int(nbytes.value), _stream_ptr(torch)), f"ccsd_contract({term})")
+    torch.cuda.current_stream().synchronize()   # ws / ins must outlive the enqueued kernels
+    return out
+
+
+def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False):
+    """C[m][n] (+)= alpha * sum_k A[m][k] B[n][k]; transposed_out stores C as [n][m]."""
+    torch = _torch()
+    lib = load_library()
+    A, B = _dev_c128(torch, A), _dev_c128(torch, B)
+    M, K = A.shape
+    N = B.shape[0]
+    assert B.shape[1] == K
+    if C is None:
+        C = torch.zeros((N, M) if transposed_out else (M, N), dtype=torch.complex128, device="cuda")
+    csm, csn = (1, M) if transposed_out else (N, 1)
+    alpha = complex(alpha)
+    _check(lib.ccsd_zgemm_nt(M, N, K, A.data_ptr(), K, B.data_ptr(), K, C.data_ptr(), csm, csn, alpha.real, alpha.imag,
+                             int(accumulate), mode, _stream_ptr(torch)), "ccsd_zgemm_nt")
+    torch.cuda.current_stream().synchronize()
+    return C
+
+
+def transpose(x, perm, conj: bool = False):
+    """4-index transposition out[...perm...] = x (ccsd_transpose); x is a 4-d CUDA complex128 tensor."""
+    torch = _torch()
+    lib = load_library()
+    x = _dev_c128(torch, x)
+    assert x.dim() == 4 and sorted(perm) == [0, 1, 2, 3]
+    dims = (ctypes.c_int64 * 4)(*x.shape)
+    pr = (ctypes.c_int * 4)(*perm)
+    out = torch.empty([x.shape[p] for p in perm], dtype=torch.complex128, device="cuda")
+    _check(lib.ccsd_transpose(x.data_ptr(), out.data_ptr(), dims, pr, int(conj), _stream_ptr(torch)), "ccsd_transpose")
+    return out

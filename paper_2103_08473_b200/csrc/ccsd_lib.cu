@@ -1,0 +1,1353 @@
+// B200-native complex spinor-basis CCSD hot path: C ABI + host-side iteration driver.
+// Equations: arXiv 2103.08473 Appendix 7.1 (eqs 22-33) in the reading of DESIGN.md.
+// Every step runs in CUDA kernels of this library; there is no CPU fallback and no code shared with oracle/.
+//
+// Design (DESIGN.md "Data layout" / "Kernels"): every contraction of eqs 24-33 is brought to ONE form,
+//     C[m][n] (+)= alpha * sum_k A[m][k] * B[n][k]          ("NT": both operands K-contiguous)
+// by keeping the constant integral classes resident in HBM in every operand layout they are needed in (180 GB
+// part: redundancy is cheap) and by re-laying-out the amplitudes once per iteration with bandwidth-bound fill /
+// transpose kernels.  The GEMM is the FP64 tensor-core (DMMA) kernel of gemm_dmma.cuh.
+#include "../../include/ccsd.h"
+#include "common.cuh"
+#include "fill.cuh"
+#include "gemm_simple.cuh"
+#include "gemm_dmma.cuh"
+#include "transpose.cuh"
+#include "reduce.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+thread_local char g_cuda_err[256] = "";
+long long g_launches = 0;
+
+// ---------------------------------------------------------------------------------------------------------------
+// GEMM front end
+// ---------------------------------------------------------------------------------------------------------------
+struct Env {
+    cudaStream_t st;
+    int gemm_mode;          // 0 auto, 1 simple only, 2 force dmma
+    c128* partial;          // split-K scratch
+    int64_t partial_elems;
+};
+
+static GemmParams gp(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda, const c128* B, int64_t ldb, c128* C,
+                     int64_t csm, int64_t csn, double alpha, int acc)
+{
+    GemmParams p;
+    memset(&p, 0, sizeof(p));
+    p.M = M; p.N = N; p.K = K;
+    p.A = A; p.sam = lda; p.sak = 1;
+    p.B = B; p.sbn = ldb; p.sbk = 1;
+    p.C = C; p.csm = csm; p.csn = csn;
+    p.alpha = mk(alpha, 0.0); p.accumulate = acc;
+    p.batch = 1; p.ksplit = 1; p.kchunk = K;
+    return p;
+}
+
+static int run_gemm(const Env& env, GemmParams p)
+{
+    if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return CCSD_OK;
+    if (p.K <= 0) return p.accumulate ? CCSD_OK : CCSD_EINVAL;
+    bool dmma_ok = dmma_supported(p);
+    if (env.gemm_mode == 2 && !dmma_ok) return CCSD_EINVAL;
+    bool use_dmma = (env.gemm_mode == 2) || (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p));
+    // split-K when the output has too few tiles to fill the machine
+    const int bm = use_dmma ? DMMA_BM : SG_BM, bn = use_dmma ? dmma_bn_for(p.N) : SG_BN;
+    int64_t tiles = ((p.M + bm - 1) / bm) * ((p.N + bn - 1) / bn) * p.batch;
+    p.ksplit = 1; p.kchunk = p.K; p.partial = nullptr;
+    if (env.partial && tiles < 148 && p.K >= 2048) {
+        int64_t want = (2 * 148 + tiles - 1) / tiles;
+        int64_t maxk = p.K / 512;
+        int64_t cap = env.partial_elems / (p.M * p.N * p.batch);
+        int64_t ks = want < maxk ? want : maxk;
+        if (ks > cap) ks = cap;
+        if (ks > 1) {
+            int64_t chunk = round_up((p.K + ks - 1) / ks, 16);
+            p.ksplit = (int)((p.K + chunk - 1) / chunk);
+            p.kchunk = chunk;
+            p.partial = env.partial;
+        }
+    }
+    if (use_dmma) {
+        CCSD_TRY(launch_gemm_dmma(env.st, p));
+    } else {
+        dim3 grid((unsigned)((p.N + SG_BN - 1) / SG_BN), (unsigned)((p.M + SG_BM - 1) / SG_BM), (unsigned)(p.batch * p.ksplit));
+        gemm_simple_kernel<<<grid, SG_T * SG_T, 0, env.st>>>(p);
+        g_launches++;
+    }
+    if (p.ksplit > 1) {
+        int64_t tot = p.M * p.N * p.batch;
+        splitk_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, env.st>>>(p);
+        g_launches++;
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+static int run_gemv(const Env& env, int64_t M, int64_t K, const c128* A, int64_t lda, const c128* x, c128* y, int64_t sy,
+                    double alpha, int acc)
+{
+    if (M <= 0) return CCSD_OK;
+    gemv_kernel<<<(unsigned)((M + 7) / 8), 256, 0, env.st>>>(M, K, A, lda, x, y, sy, mk(alpha, 0.0), acc);
+    g_launches++;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+static void dcopy(cudaStream_t st, c128* dst, const c128* src, int64_t elems)
+{
+    if (elems > 0) cudaMemcpyAsync(dst, src, (size_t)elems * sizeof(c128), cudaMemcpyDeviceToDevice, st);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// context
+// ---------------------------------------------------------------------------------------------------------------
+static const char* k_step_names[CCSD_NSTEPS] = {"prep_permute", "fock_like", "Hvovo_linear", "Hvovo_quad", "C_ovoo",
+                                                "A_oooo", "pp_ladder", "hh_ladder+Goo", "ring_gemm", "ring_antisym",
+                                                "Vdag_t1", "Gvv_t2", "C_t1", "S1", "update_diis", "energy"};
+
+struct ccsd_ctx {
+    int o, v, n, L, Lp;
+    int64_t oo, vv, ov, oop, nvec;
+    ccsd_options opt;
+    cudaStream_t st;
+    Env env;
+    // tables
+    int2 *po, *pv;
+    double* eps;
+    // constants
+    c128 *f, *W, *Vvovv_p, *Vvovv_u, *VvovvT, *Voovv_p, *G1, *Voovv_c, *Voovv_ou, *Vvovo_m, *Vvovo_c, *Vooov_p,
+        *Vooov_b, *Vooov_cc, *Vooov_d, *Vooov_e, *Voooo_p;
+    // init temporaries
+    c128 *Boo, *Bov, *Bvo, *Bvv, *Jovov, *Jvoov, *Jvvoo, *Jvvov, *Jooov, *Joooo, *Jslab, *JslabT;
+    int na_slab;
+    // amplitudes and per-iteration tensors
+    c128 *t1, *t2p, *t1T, *S1, *S2p, *taup, *TT, *AG, *Xm, *T2r, *tauc, *tauou, *t2hu;
+    c128 *Hvv, *Gvv, *Hoo, *Goo, *Hov, *HovT, *HF, *inner, *Hm, *Cm, *Cm2, *Am, *tmp_ov;
+    c128 *Xr, *P, *Qm, *Rr, *Y, *Z;
+    c128* partial;
+    int64_t partial_elems;
+    // DIIS
+    c128 *diis_u, *diis_e;  // [ndiis][nvec]
+    double* red;            // device reduction outputs (>= 16 doubles)
+    double* red_host;       // pinned host mirror
+    int diis_count;         // vectors stored so far (<= ndiis)
+    int diis_next;          // slot to overwrite next
+    std::vector<int> diis_order;       // slots, oldest first
+    std::vector<double> gram;          // [ndiis][ndiis] by slot
+    // timing
+    int timing;
+    cudaEvent_t ev[CCSD_NSTEPS + 1];
+    float step_ms[CCSD_NSTEPS];
+    bool have_residual;
+};
+
+struct Carver {
+    char* base;
+    size_t off;
+    template <class T>
+    T* take(int64_t elems)
+    {
+        size_t bytes = ((size_t)(elems > 0 ? elems : 1) * sizeof(T) + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += bytes;
+        return p;
+    }
+};
+
+static void carve(ccsd_ctx* c, char* base, size_t* total)
+{
+    Carver w{base, 0};
+    const int64_t o = c->o, v = c->v, n = c->n, Lp = c->Lp, oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
+    c->po = w.take<int2>(oo);
+    c->pv = w.take<int2>(vv);
+    c->eps = w.take<double>(n);
+    c->f = w.take<c128>(n * n);
+    c->W = w.take<c128>(vv * vv);
+    c->Vvovv_p = w.take<c128>(v * o * vv);
+    c->Vvovv_u = w.take<c128>(v * v * o * v);
+    c->VvovvT = w.take<c128>(o * vv * v);
+    c->Voovv_p = w.take<c128>(oo * vv);
+    c->G1 = w.take<c128>(ov * ov);
+    c->Voovv_c = w.take<c128>(v * oo * v);
+    c->Voovv_ou = w.take<c128>(o * o * vv);
+    c->Vvovo_m = w.take<c128>(ov * ov);
+    c->Vvovo_c = w.take<c128>(ov * ov);
+    c->Vooov_p = w.take<c128>(oo * ov);
+    c->Vooov_b = w.take<c128>(o * ov * o);
+    c->Vooov_cc = w.take<c128>(ov * oo);
+    c->Vooov_d = w.take<c128>(o * o * ov);
+    c->Vooov_e = w.take<c128>(o * oo * v);
+    c->Voooo_p = w.take<c128>(oo * oo);
+    // init temporaries
+    c->Boo = w.take<c128>(o * o * Lp);
+    c->Bov = w.take<c128>(ov * Lp);
+    c->Bvo = w.take<c128>(ov * Lp);
+    c->Bvv = w.take<c128>(v * v * Lp);
+    c->Jovov = w.take<c128>(ov * ov);
+    c->Jvoov = w.take<c128>(ov * ov);
+    c->Jvvoo = w.take<c128>(v * v * o * o);
+    c->Jvvov = w.take<c128>(v * v * ov);
+    c->Jooov = w.take<c128>(o * o * ov);
+    c->Joooo = w.take<c128>(o * o * o * o);
+    {
+        double per_a = (double)v * v * v * 16.0;
+        int na = (int)(1.5e9 / (per_a > 1 ? per_a : 1));
+        if (na < 1) na = 1;
+        if (na > v) na = (int)v;
+        c->na_slab = na;
+        c->Jslab = w.take<c128>((int64_t)na * v * v * v);
+        c->JslabT = w.take<c128>((int64_t)na * v * v * v);
+    }
+    // amplitudes, residuals, operands
+    c->t1 = w.take<c128>(ov);
+    c->t2p = w.take<c128>(oo * vv);
+    c->t1T = w.take<c128>(ov);
+    c->S1 = w.take<c128>(ov);
+    c->S2p = w.take<c128>(oo * vv);
+    c->taup = w.take<c128>(oo * vv);
+    c->TT = w.take<c128>(vv * 2 * oop);
+    c->AG = w.take<c128>(oo * 2 * oop);
+    c->Xm = w.take<c128>(ov * ov);
+    c->T2r = w.take<c128>(ov * ov);
+    c->tauc = w.take<c128>(v * oo * v);
+    c->tauou = w.take<c128>(o * o * vv);
+    c->t2hu = w.take<c128>(oo * v * v);
+    c->Hvv = w.take<c128>(v * v);
+    c->Gvv = w.take<c128>(v * v);
+    c->Hoo = w.take<c128>(o * o);
+    c->Goo = w.take<c128>(o * o);
+    c->Hov = w.take<c128>(ov);
+    c->HovT = w.take<c128>(ov);
+    c->HF = w.take<c128>(ov);
+    c->inner = w.take<c128>(o * o);
+    c->Hm = w.take<c128>(ov * ov);
+    c->Cm = w.take<c128>(ov * oo);
+    c->Cm2 = w.take<c128>(ov * oo);
+    c->Am = w.take<c128>(oo * oo);
+    c->tmp_ov = w.take<c128>(ov);
+    c->Xr = w.take<c128>(ov * ov);
+    c->P = w.take<c128>(o * o * vv);
+    c->Qm = w.take<c128>(oo * v * v);
+    c->Rr = w.take<c128>(v * oo * v);
+    c->Y = w.take<c128>(ov * o * o);
+    c->Z = w.take<c128>(oo * o * o);
+    c->partial_elems = 16 * 1024 * 1024;  // 256 MB of split-K partials
+    c->partial = w.take<c128>(c->partial_elems);
+    c->nvec = ov + oo * vv;
+    int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
+    c->diis_u = w.take<c128>((int64_t)nd * c->nvec);
+    c->diis_e = w.take<c128>((int64_t)nd * c->nvec);
+    c->red = w.take<double>(64);
+    *total = w.off;
+}
+
+static int check_sizes(int nocc, int nvir, int naux)
+{
+    if (nocc < 2 || nvir < 2 || naux < 1) return CCSD_EINVAL;
+    if (nocc > 4096 || nvir > 8192) return CCSD_EINVAL;
+    return CCSD_OK;
+}
+
+static void setup_dims(ccsd_ctx* c, int nocc, int nvir, int naux, const ccsd_options* opts)
+{
+    c->o = nocc; c->v = nvir; c->n = nocc + nvir; c->L = naux; c->Lp = (int)round_up(naux, 4);
+    c->oo = (int64_t)nocc * (nocc - 1) / 2;
+    c->vv = (int64_t)nvir * (nvir - 1) / 2;
+    c->ov = (int64_t)nocc * nvir;
+    c->oop = round_up(c->oo > 0 ? c->oo : 1, 4);
+    if (opts) c->opt = *opts; else ccsd_default_options(&c->opt);
+    if (c->opt.ndiis < 0) c->opt.ndiis = 0;
+    if (c->opt.ndiis > 12) c->opt.ndiis = 12;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// integral-class functors over the chemists'-notation blocks J (eq 6 PAPER.md:71 reading G1):
+//   <pq||rs> = (pr|qs) - (ps|qr)
+// ---------------------------------------------------------------------------------------------------------------
+struct GOovv {  // <kl||cd> = (kc|ld) - (kd|lc)
+    const c128* J; int64_t o, v;
+    __device__ c128 operator()(int k, int l, int c, int d) const
+    {
+        int64_t ov = o * v;
+        return csub(J[(k * v + c) * ov + l * v + d], J[(k * v + d) * ov + l * v + c]);
+    }
+};
+struct GVovo {  // <ak||ci> = (ac|ki) - (ai|kc)
+    const c128 *Jvvoo, *Jvoov; int64_t o, v;
+    __device__ c128 operator()(int a, int k, int c, int i) const
+    {
+        return csub(Jvvoo[(a * v + c) * o * o + k * o + i], Jvoov[(a * o + i) * o * v + k * v + c]);
+    }
+};
+struct GVovv {  // <ak||cd> = (ac|kd) - (ad|kc)
+    const c128* J; int64_t o, v;
+    __device__ c128 operator()(int a, int k, int c, int d) const
+    {
+        int64_t ov = o * v;
+        return csub(J[(a * v + c) * ov + k * v + d], J[(a * v + d) * ov + k * v + c]);
+    }
+};
+struct GOoov {  // <kl||ic> = (ki|lc) - (kc|li)
+    const c128* J; int64_t o, v;
+    __device__ c128 operator()(int k, int l, int i, int c) const
+    {
+        int64_t ov = o * v;
+        return csub(J[(k * o + i) * ov + l * v + c], J[(l * o + i) * ov + k * v + c]);
+    }
+};
+struct GOooo {  // <kl||ij> = (ki|lj) - (kj|li)
+    const c128* J; int64_t o;
+    __device__ c128 operator()(int k, int l, int i, int j) const
+    {
+        int64_t o2 = o * o;
+        return csub(J[(k * o + i) * o2 + l * o + j], J[(k * o + j) * o2 + l * o + i]);
+    }
+};
+
+__global__ void eps_kernel(const c128* f, double* eps, int n, int o, double shift)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) eps[p] = f[(int64_t)p * n + p].x + (p >= o ? shift : 0.0);
+}
+
+// Bxy[(p,q)][l] = B[l][p][q], auxiliary index fastest and zero-padded to Lp
+static void bblock(cudaStream_t st, c128* out, const c128* B, int n, int L, int Lp, int p0, int np, int q0, int nq)
+{
+    launch_fill(st, out, (int64_t)np * nq, Lp, Lp, 0, [=] __device__(int64_t row, int64_t l) {
+        if (l >= L) return mk(0.0, 0.0);
+        int64_t p = p0 + row / nq, q = q0 + row % nq;
+        return B[l * (int64_t)n * n + p * n + q];
+    });
+}
+
+static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const int o = c->o, v = c->v, n = c->n, L = c->L, Lp = c->Lp;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    const int2 *po = c->po, *pv = c->pv;
+
+    if (oo > 0) { pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(c->po, o); g_launches++; }
+    if (vv > 0) { pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(c->pv, v); g_launches++; }
+
+    // Fock matrix f = h + sum_i <pi||qi>
+    launch_fill(st, c->f, n, n, n, 0, [=] __device__(int64_t p, int64_t q) {
+        c128 s = h[p * n + q];
+        for (int l = 0; l < L; l++) {
+            const c128* Bl = B + (int64_t)l * n * n;
+            c128 d = mk(0.0, 0.0), x = mk(0.0, 0.0);
+            for (int i = 0; i < o; i++) {
+                d = cadd(d, Bl[(int64_t)i * n + i]);
+                cfma(x, Bl[p * n + i], Bl[(int64_t)i * n + q]);
+            }
+            cfma(s, Bl[p * n + q], d);
+            s = csub(s, x);
+        }
+        return s;
+    });
+    eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(c->f, c->eps, n, o, c->opt.level_shift);
+    g_launches++;
+
+    // B blocks with the auxiliary index fastest (zero-padded to a multiple of 4): Bxy[(p,q)][l] = B[l][p][q]
+    bblock(st, c->Boo, B, n, L, Lp, 0, o, 0, o);
+    bblock(st, c->Bov, B, n, L, Lp, 0, o, o, v);
+    bblock(st, c->Bvo, B, n, L, Lp, o, v, 0, o);
+    bblock(st, c->Bvv, B, n, L, Lp, o, v, o, v);
+
+    // chemists' blocks (pq|rs) = sum_L B[L,p,q] B[L,r,s]  as NT GEMMs over the auxiliary index
+    CCSD_TRY(run_gemm(env, gp(ov, ov, Lp, c->Bov, Lp, c->Bov, Lp, c->Jovov, ov, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp(ov, ov, Lp, c->Bvo, Lp, c->Bov, Lp, c->Jvoov, ov, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp((int64_t)v * v, (int64_t)o * o, Lp, c->Bvv, Lp, c->Boo, Lp, c->Jvvoo, (int64_t)o * o, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp((int64_t)v * v, ov, Lp, c->Bvv, Lp, c->Bov, Lp, c->Jvvov, ov, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp((int64_t)o * o, ov, Lp, c->Boo, Lp, c->Bov, Lp, c->Jooov, ov, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp((int64_t)o * o, (int64_t)o * o, Lp, c->Boo, Lp, c->Boo, Lp, c->Joooo, (int64_t)o * o, 1, 1.0, 0)));
+
+    GOovv goovv{c->Jovov, o, v};
+    GVovo gvovo{c->Jvvoo, c->Jvoov, o, v};
+    GVovv gvovv{c->Jvvov, o, v};
+    GOoov gooov{c->Jooov, o, v};
+    GOooo goooo{c->Joooo, o};
+
+    // <kl||cd> in four operand layouts
+    launch_fill(st, c->Voovv_p, oo, vv, vv, 0, [=] __device__(int64_t KL, int64_t CD) {
+        int2 kl = po[KL], cd = pv[CD];
+        return goovv(kl.x, kl.y, cd.x, cd.y);
+    });
+    launch_fill(st, c->G1, ov, ov, ov, 0, [=] __device__(int64_t ck, int64_t ld) {
+        int cc = ck / o, k = ck % o, l = ld / v, d = ld % v;
+        return goovv(k, l, cc, d);
+    });
+    launch_fill(st, c->Voovv_c, v, oo * v, oo * v, 0, [=] __device__(int64_t cc, int64_t col) {
+        int2 kl = po[col / v];
+        int d = col % v;
+        return goovv(kl.x, kl.y, (int)cc, d);
+    });
+    launch_fill(st, c->Voovv_ou, (int64_t)o * o, vv, vv, 0, [=] __device__(int64_t row, int64_t CD) {
+        int2 cd = pv[CD];
+        return goovv((int)(row / o), (int)(row % o), cd.x, cd.y);
+    });
+    // <ak||ci>
+    launch_fill(st, c->Vvovo_m, ov, ov, ov, 0, [=] __device__(int64_t ai, int64_t ck) {
+        int a = ai / o, i = ai % o, cc = ck / o, k = ck % o;
+        return gvovo(a, k, cc, i);
+    });
+    launch_fill(st, c->Vvovo_c, ov * o, v, v, 0, [=] __device__(int64_t row, int64_t cc) {
+        int i = row % o, k = (row / o) % o, b = row / ((int64_t)o * o);
+        return gvovo(b, k, (int)cc, i);
+    });
+    // <ak||cd>
+    launch_fill(st, c->Vvovv_p, ov, vv, vv, 0, [=] __device__(int64_t ak, int64_t CD) {
+        int2 cd = pv[CD];
+        return gvovv((int)(ak / o), (int)(ak % o), cd.x, cd.y);
+    });
+    launch_fill(st, c->Vvovv_u, (int64_t)v * v, ov, ov, 0, [=] __device__(int64_t ac, int64_t kd) {
+        return gvovv((int)(ac / v), (int)(kd / v), (int)(ac % v), (int)(kd % v));
+    });
+    launch_fill(st, c->VvovvT, o * vv, v, v, 0, [=] __device__(int64_t row, int64_t cc) {
+        int j = row / vv;
+        int2 ab = pv[row % vv];
+        return cconj(gvovv((int)cc, j, ab.x, ab.y));
+    });
+    // <kl||ic>
+    launch_fill(st, c->Vooov_p, oo, ov, ov, 0, [=] __device__(int64_t KL, int64_t ic) {
+        int2 kl = po[KL];
+        return gooov(kl.x, kl.y, (int)(ic / v), (int)(ic % v));
+    });
+    launch_fill(st, c->Vooov_b, (int64_t)o * ov, o, o, 0, [=] __device__(int64_t row, int64_t l) {
+        int k = row % o, cc = (row / o) % v, i = row / ((int64_t)o * v);
+        return gooov(k, (int)l, i, cc);
+    });
+    launch_fill(st, c->Vooov_cc, ov, oo, oo, 0, [=] __device__(int64_t bk, int64_t IJ) {
+        int2 ij = po[IJ];
+        return cconj(gooov(ij.x, ij.y, (int)(bk % o), (int)(bk / o)));
+    });
+    launch_fill(st, c->Vooov_d, (int64_t)o * o, ov, ov, 0, [=] __device__(int64_t ki, int64_t lc) {
+        return gooov((int)(ki / o), (int)(lc / v), (int)(ki % o), (int)(lc % v));
+    });
+    launch_fill(st, c->Vooov_e, o, oo * v, oo * v, 0, [=] __device__(int64_t i, int64_t col) {
+        int2 kl = po[col / v];
+        return gooov(kl.x, kl.y, (int)i, (int)(col % v));
+    });
+    // <kl||ij>
+    launch_fill(st, c->Voooo_p, oo, oo, oo, 0, [=] __device__(int64_t KL, int64_t IJ) {
+        int2 kl = po[KL], ij = po[IJ];
+        return goooo(kl.x, kl.y, ij.x, ij.y);
+    });
+
+    // <ab||cd> = (ac|bd) - (ad|bc), packed, built in slabs of the first virtual index so that the v^4 staging
+    // tensor is never materialised.  For a in [a0, a0+na):
+    //   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
+    //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
+    //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
+    const int64_t v2 = (int64_t)v * v;
+    for (int a0 = 0; a0 < v && vv > 0; a0 += c->na_slab) {
+        if (a0 > v - 2) break;
+        int na = (a0 + c->na_slab <= v) ? c->na_slab : v - a0;
+        int64_t rows = (int64_t)na * v;
+        CCSD_TRY(run_gemm(env, gp(rows, v2, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv, Lp, c->Jslab, v2, 1, 1.0, 0)));
+        CCSD_TRY(launch_transpose2d(st, c->Jslab, c->JslabT, rows, v2, 0));
+        // rows of W owned by this slab: pairs (a,b), a in [a0, a0+na), b > a -> a contiguous packed range
+        int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
+        int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
+        const c128 *J = c->Jslab, *JT = c->JslabT;
+        launch_fill(st, c->W + r0 * vv, r1 - r0, vv, vv, 0, [=] __device__(int64_t r, int64_t CD) {
+            int2 ab = pv[r0 + r], cd = pv[CD];
+            int64_t al = ab.x - a0;
+            c128 x = J[(al * v + cd.x) * v2 + (int64_t)ab.y * v + cd.y];
+            c128 y = JT[((int64_t)ab.y * v + cd.x) * rows + al * v + cd.y];
+            return csub(x, y);
+        });
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// MP2 start: t1 = f_ai / D^a_i, t2 = <ab||ij> / D^ab_ij
+static void mp2_guess(ccsd_ctx* c)
+{
+    const int o = c->o, v = c->v, n = c->n;
+    const int64_t vv = c->vv;
+    const c128 *f = c->f, *V = c->Voovv_p;
+    const double* eps = c->eps;
+    const int2 *po = c->po, *pv = c->pv;
+    const int ccd = c->opt.ccd;
+    launch_fill(c->st, c->t1, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
+        if (ccd) return mk(0.0, 0.0);
+        double d = eps[i] - eps[o + a];
+        c128 x = cconj(f[i * n + o + a]);
+        return mk(x.x / d, x.y / d);
+    });
+    launch_fill(c->st, c->t2p, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ij = po[IJ], ab = pv[AB];
+        double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
+        c128 x = cconj(V[IJ * vv + AB]);
+        return mk(x.x / d, x.y / d);
+    });
+    c->diis_count = 0; c->diis_next = 0; c->diis_order.clear();
+    c->have_residual = false;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// one residual evaluation, eqs 23-33
+// ---------------------------------------------------------------------------------------------------------------
+static void tick(ccsd_ctx* c, int k)
+{
+    if (c->timing) cudaEventRecord(c->ev[k], c->st);
+}
+
+// eq 23 on packed storage: tau = t2 + t1[i,a] t1[j,b] - t1[j,a] t1[i,b]
+static void build_tau(cudaStream_t st, c128* taup, const c128* t1, const c128* t2p, int o, int v, const int2* po,
+                      const int2* pv)
+{
+    const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2;
+    launch_fill(st, taup, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ij = po[IJ], ab = pv[AB];
+        c128 x = t2p[IJ * vv + AB];
+        cfma(x, t1[ij.x * v + ab.x], t1[ij.y * v + ab.y]);
+        c128 y = cmul(t1[ij.y * v + ab.x], t1[ij.x * v + ab.y]);
+        return csub(x, y);
+    });
+}
+
+static int prep_operands(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
+    const int2 *po = c->po, *pv = c->pv;
+    const c128 *t1 = c->t1, *t2p = c->t2p, *taup = c->taup;
+    build_tau(st, c->taup, t1, t2p, o, v, po, pv);
+    launch_fill(st, c->t1T, v, o, o, 0, [=] __device__(int64_t a, int64_t i) { return t1[i * v + a]; });
+    // TT[(a<b)][0:oo) = tau^T, TT[(a<b)][oop:oop+oo) = t2^T   (K-contiguous operands of the hh-ladder and Goo terms)
+    CCSD_TRY(launch_transpose2d_ld(st, c->taup, vv, c->TT, 2 * oop, oo, vv, 0));
+    CCSD_TRY(launch_transpose2d_ld(st, c->t2p, vv, c->TT + oop, 2 * oop, oo, vv, 0));
+    // Xm[(a,i)][(l,d)] = 1/2 t2[l,i,a,d] + t1[l,a] t1[i,d]      (eq 29 operand)
+    launch_fill(st, c->Xm, ov, ov, ov, 0, [=] __device__(int64_t ai, int64_t ld) {
+        int a = ai / o, i = ai % o, l = ld / v, d = ld % v;
+        c128 x = cscale(0.5, t2_at(t2p, l, i, a, d, o, v, vv));
+        cfma(x, t1[l * v + a], t1[i * v + d]);
+        return x;
+    });
+    // T2r[(j,b)][(c,k)] = t2[j,k,c,b]                            (eq 32 ring operand)
+    launch_fill(st, c->T2r, ov, ov, ov, 0, [=] __device__(int64_t jb, int64_t ck) {
+        int j = jb / v, b = jb % v, cc = ck / o, k = ck % o;
+        return t2_at(t2p, j, k, cc, b, o, v, vv);
+    });
+    // tauc[a][(k<l, d)] = tau[k,l,d,a]
+    launch_fill(st, c->tauc, v, oo * v, oo * v, 0, [=] __device__(int64_t a, int64_t col) {
+        int64_t KL = col / v;
+        int d = col % v;
+        return asym_col(taup, KL, vv, d, (int)a, v);
+    });
+    // tauou[(i,l)][(c<d)] = tau[i,l,c,d]
+    launch_fill(st, c->tauou, (int64_t)o * o, vv, vv, 0, [=] __device__(int64_t il, int64_t CD) {
+        int i = il / o, l = il % o;
+        if (i == l) return mk(0.0, 0.0);
+        if (i < l) return taup[pair_idx(i, l, o) * vv + CD];
+        return cneg(taup[pair_idx(l, i, o) * vv + CD]);
+    });
+    // t2hu[(i<j, b)][c] = t2[i,j,b,c]
+    launch_fill(st, c->t2hu, oo * v, v, v, 0, [=] __device__(int64_t row, int64_t cc) {
+        int64_t IJ = row / v;
+        int b = row % v;
+        return asym_col(t2p, IJ, vv, b, (int)cc, v);
+    });
+    return CCSD_OK;
+}
+
+static int fock_like(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const int o = c->o, v = c->v, n = c->n;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    const c128* f = c->f;
+    // eq 28: Hov[k,c] = f[k,c] + sum_{ld} <kl||cd> t1[l,d]            (HovT[(c,k)])
+    launch_fill(st, c->HovT, v, o, o, 0, [=] __device__(int64_t cc, int64_t k) { return f[k * n + o + cc]; });
+    CCSD_TRY(run_gemv(env, ov, ov, c->G1, ov, c->t1, c->HovT, 1, 1.0, 1));
+    const c128* HovT = c->HovT;
+    launch_fill(st, c->Hov, o, v, v, 0, [=] __device__(int64_t k, int64_t cc) { return HovT[cc * o + k]; });
+    // eq 24: Hvv[a,c] = f[a,c] + sum_{k<l,d} <kl||cd> tau[k,l,d,a]
+    launch_fill(st, c->Hvv, v, v, v, 0, [=] __device__(int64_t a, int64_t cc) { return f[(o + a) * n + o + cc]; });
+    CCSD_TRY(run_gemm(env, gp(v, v, oo * v, c->tauc, oo * v, c->Voovv_c, oo * v, c->Hvv, v, 1, 1.0, 1)));
+    // eq 25: Gvv = Hvv + sum_{kd} <ak||cd> t1[k,d] - sum_k f[k,c] t1[k,a]
+    dcopy(st, c->Gvv, c->Hvv, (int64_t)v * v);
+    CCSD_TRY(run_gemv(env, (int64_t)v * v, ov, c->Vvovv_u, ov, c->t1, c->Gvv, 1, 1.0, 1));
+    {
+        GemmParams p = gp(v, v, o, c->t1T, o, f + o, 1, c->Gvv, v, 1, -1.0, 1);
+        p.sbn = 1; p.sbk = n;  // B[c][k] = f[k][o+c]
+        CCSD_TRY(run_gemm(env, p));
+    }
+    // eq 26: Hoo[k,i] = -f[k,i] + sum_{l, c<d} <kl||cd> tau[l,i,c,d]   (tau[l,i] = -tauou[(i,l)])
+    launch_fill(st, c->Hoo, o, o, o, 0, [=] __device__(int64_t k, int64_t i) { return cneg(f[k * n + i]); });
+    CCSD_TRY(run_gemm(env, gp(o, o, o * vv, c->Voovv_ou, o * vv, c->tauou, o * vv, c->Hoo, o, 1, -1.0, 1)));
+    // eq 27: Goo = Hoo - sum_{lc} <kl||ic> t1[l,c] - sum_c f[k,c] t1[i,c]
+    dcopy(st, c->Goo, c->Hoo, (int64_t)o * o);
+    CCSD_TRY(run_gemv(env, (int64_t)o * o, ov, c->Vooov_d, ov, c->t1, c->Goo, 1, -1.0, 1));
+    CCSD_TRY(run_gemm(env, gp(o, o, v, f + o, n, c->t1, v, c->Goo, o, 1, -1.0, 1)));
+    return CCSD_OK;
+}
+
+static int build_Hvovo(ccsd_ctx* c)
+{
+    const Env& env = c->env;
+    const int o = c->o, v = c->v;
+    const int64_t ov = c->ov;
+    // eq 29, stored as Hm[(a,i)][(c,k)]
+    dcopy(c->st, c->Hm, c->Vvovo_m, ov * ov);
+    {   // + sum_d <ak||cd> t1[i,d]        batched over a: C_a[(c,k)][i]
+        GemmParams p = gp(ov, o, v, c->Vvovv_u, v, c->t1, v, c->Hm, 1, ov, 1.0, 1);
+        p.batch = v; p.bsA = ov * v; p.bsB = 0; p.bsC = (int64_t)o * ov;
+        CCSD_TRY(run_gemm(env, p));
+    }
+    // - sum_l <kl||ic> t1[l,a]            C[a][(i,c,k)]
+    CCSD_TRY(run_gemm(env, gp(v, (int64_t)o * ov, o, c->t1T, o, c->Vooov_b, o, c->Hm, (int64_t)o * ov, 1, -1.0, 1)));
+    tick(c, 3);
+    // + sum_{ld} <kl||cd> (1/2 t2[l,i,a,d] + t1[l,a] t1[i,d])       (ov x ov x ov)
+    CCSD_TRY(run_gemm(env, gp(ov, ov, ov, c->Xm, ov, c->G1, ov, c->Hm, ov, 1, 1.0, 1)));
+    return CCSD_OK;
+}
+
+static int build_C(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    const int2* po = c->po;
+    // eq 30, stored as Cm[(b,k)][(i<j)]
+    dcopy(st, c->Cm, c->Vooov_cc, ov * oo);
+    CCSD_TRY(run_gemm(env, gp(ov * o, o, v, c->Vvovo_c, v, c->t1, v, c->Y, o, 1, 1.0, 0)));
+    const c128* Y = c->Y;
+    launch_fill(st, c->Cm, ov, oo, oo, 1, [=] __device__(int64_t bk, int64_t IJ) {
+        int2 ij = po[IJ];
+        return csub(Y[(bk * o + ij.x) * o + ij.y], Y[(bk * o + ij.y) * o + ij.x]);
+    });
+    CCSD_TRY(run_gemm(env, gp(ov, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1)));
+    return CCSD_OK;
+}
+
+static int build_A(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo, vv = c->vv;
+    const int2* po = c->po;
+    // eq 31, stored as Am[(k<l)][(i<j)]
+    dcopy(st, c->Am, c->Voooo_p, oo * oo);
+    CCSD_TRY(run_gemm(env, gp(oo * o, o, v, c->Vooov_p, v, c->t1, v, c->Z, o, 1, 1.0, 0)));
+    const c128* Z = c->Z;
+    launch_fill(st, c->Am, oo, oo, oo, 1, [=] __device__(int64_t KL, int64_t IJ) {
+        int2 ij = po[IJ];
+        return csub(Z[(KL * o + ij.x) * o + ij.y], Z[(KL * o + ij.y) * o + ij.x]);
+    });
+    CCSD_TRY(run_gemm(env, gp(oo, oo, vv, c->Voovv_p, vv, c->taup, vv, c->Am, oo, 1, 1.0, 1)));
+    return CCSD_OK;
+}
+
+// ---- the eight terms of eq 32; each ADDS into S[(i<j)][(a<b)] ---------------------------------------------------
+static int s2_driver(ccsd_ctx* c, c128* S)
+{
+    const c128* V = c->Voovv_p;
+    const int64_t vv = c->vv;
+    launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) { return cconj(V[IJ * vv + AB]); });
+    return CCSD_OK;
+}
+static int s2_pp_ladder(ccsd_ctx* c, c128* S)
+{   // sum_{c<d} <ab||cd> tau[i,j,c,d]      M = (a<b), N = (i<j), K = (c<d)
+    return run_gemm(c->env, gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1));
+}
+static void fill_AG_hh(ccsd_ctx* c)
+{   // AG[(i<j)][(k<l)] = A[k,l,i,j]
+    const c128* Am = c->Am;
+    const int64_t oo = c->oo;
+    launch_fill(c->st, c->AG, oo, oo, 2 * c->oop, 0, [=] __device__(int64_t IJ, int64_t KL) { return Am[KL * oo + IJ]; });
+}
+static void fill_AG_goo(ccsd_ctx* c)
+{   // Ghat[(i<j)][(k<l)] = d_ik Goo[l,j] - d_il Goo[k,j] - d_jk Goo[l,i] + d_jl Goo[k,i]
+    //   == P-_ji sum_m Goo[m,j] t2[i,m,a,b] written on packed pairs (reading G7 of eq 32)
+    const c128* Goo = c->Goo;
+    const int o = c->o;
+    const int2* po = c->po;
+    launch_fill(c->st, c->AG + c->oop, c->oo, c->oo, 2 * c->oop, 0, [=] __device__(int64_t IJ, int64_t KL) {
+        int2 ij = po[IJ], kl = po[KL];
+        c128 s = mk(0.0, 0.0);
+        if (ij.x == kl.x) s = cadd(s, Goo[kl.y * o + ij.y]);
+        if (ij.x == kl.y) s = csub(s, Goo[kl.x * o + ij.y]);
+        if (ij.y == kl.x) s = csub(s, Goo[kl.y * o + ij.x]);
+        if (ij.y == kl.y) s = cadd(s, Goo[kl.x * o + ij.x]);
+        return s;
+    });
+}
+static int s2_hh_ladder(ccsd_ctx* c, c128* S)
+{   // sum_{k<l} A[k,l,i,j] tau[k,l,a,b]
+    fill_AG_hh(c);
+    return run_gemm(c->env, gp(c->vv, c->oo, c->oop, c->TT, 2 * c->oop, c->AG, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+}
+static int s2_goo(ccsd_ctx* c, c128* S)
+{
+    fill_AG_goo(c);
+    return run_gemm(c->env, gp(c->vv, c->oo, c->oop, c->TT + c->oop, 2 * c->oop, c->AG + c->oop, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+}
+static int s2_hh_and_goo(ccsd_ctx* c, c128* S)
+{   // both in one GEMM with K = [ (k<l) of tau | (k<l) of t2 ]
+    fill_AG_hh(c);
+    fill_AG_goo(c);
+    return run_gemm(c->env, gp(c->vv, c->oo, 2 * c->oop, c->TT, 2 * c->oop, c->AG, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+}
+static int s2_ring(ccsd_ctx* c, c128* S)
+{   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)];  S += P-_ij P-_ab X
+    const int o = c->o, v = c->v;
+    const int64_t ov = c->ov, vv = c->vv;
+    CCSD_TRY(run_gemm(c->env, gp(ov, ov, ov, c->Hm, ov, c->T2r, ov, c->Xr, ov, 1, 1.0, 0)));
+    tick(c, 9);
+    const c128* Xr = c->Xr;
+    const int2 *po = c->po, *pv = c->pv;
+    launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ij = po[IJ], ab = pv[AB];
+        int64_t i = ij.x, j = ij.y, a = ab.x, b = ab.y;
+        c128 s = Xr[((a * o + i) * o + j) * v + b];
+        s = csub(s, Xr[((a * o + j) * o + i) * v + b]);
+        s = csub(s, Xr[((b * o + i) * o + j) * v + a]);
+        s = cadd(s, Xr[((b * o + j) * o + i) * v + a]);
+        return s;
+    });
+    return CCSD_OK;
+}
+static int s2_vdag_t1(ccsd_ctx* c, c128* S)
+{   // sum_c conj(<cj||ab>) t1[i,c] - (i<->j):   P[i][(j,a<b)]
+    const int o = c->o, v = c->v;
+    const int64_t vv = c->vv;
+    CCSD_TRY(run_gemm(c->env, gp(o * vv, o, v, c->VvovvT, v, c->t1, v, c->P, 1, o * vv, 1.0, 0)));
+    const c128* P = c->P;
+    const int2* po = c->po;
+    launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ij = po[IJ];
+        return csub(P[((int64_t)ij.x * o + ij.y) * vv + AB], P[((int64_t)ij.y * o + ij.x) * vv + AB]);
+    });
+    return CCSD_OK;
+}
+static int s2_gvv(ccsd_ctx* c, c128* S)
+{   // sum_c Gvv[a,c] t2[i,j,c,b] - Gvv[b,c] t2[i,j,c,a];   Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]
+    const int v = c->v;
+    const int64_t vv = c->vv, oo = c->oo;
+    CCSD_TRY(run_gemm(c->env, gp(oo * v, v, v, c->t2hu, v, c->Gvv, v, c->Qm, v, 1, 1.0, 0)));
+    const c128* Qm = c->Qm;
+    const int2* pv = c->pv;
+    launch_fill(c->st, S, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ab = pv[AB];
+        return csub(Qm[(IJ * v + ab.x) * v + ab.y], Qm[(IJ * v + ab.y) * v + ab.x]);
+    });
+    return CCSD_OK;
+}
+static int s2_c_t1(ccsd_ctx* c, c128* S)
+{   // sum_k C[k,a,i,j] t1[k,b] - C[k,b,i,j] t1[k,a];   Rr[(a,i<j)][b] = sum_k C[k,a,i,j] t1[k,b]
+    const int o = c->o, v = c->v;
+    const int64_t vv = c->vv, oo = c->oo;
+    const c128* Cm = c->Cm;
+    launch_fill(c->st, c->Cm2, v * oo, o, o, 0, [=] __device__(int64_t row, int64_t k) {
+        int64_t a = row / oo, IJ = row % oo;
+        return Cm[(a * o + k) * oo + IJ];
+    });
+    CCSD_TRY(run_gemm(c->env, gp(v * oo, v, o, c->Cm2, o, c->t1T, o, c->Rr, v, 1, 1.0, 0)));
+    const c128* Rr = c->Rr;
+    const int2* pv = c->pv;
+    launch_fill(c->st, S, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+        int2 ab = pv[AB];
+        return csub(Rr[((int64_t)ab.x * oo + IJ) * v + ab.y], Rr[((int64_t)ab.y * oo + IJ) * v + ab.x]);
+    });
+    return CCSD_OK;
+}
+
+static int build_S1(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const int o = c->o, v = c->v, n = c->n;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    const c128* f = c->f;
+    // eq 33
+    launch_fill(st, c->S1, o, v, v, 0, [=] __device__(int64_t i, int64_t a) { return cconj(f[i * n + o + a]); });
+    CCSD_TRY(run_gemm(env, gp(o, v, v, c->t1, v, c->Hvv, v, c->S1, v, 1, 1.0, 1)));                  // Hvv[a,c] t1[i,c]
+    {
+        GemmParams p = gp(o, v, o, c->Hoo, 1, c->t1, 1, c->S1, v, 1, 1.0, 1);                         // Hoo[k,i] t1[k,a]
+        p.sam = 1; p.sak = o; p.sbn = 1; p.sbk = v;
+        CCSD_TRY(run_gemm(env, p));
+    }
+    CCSD_TRY(run_gemv(env, ov, ov, c->T2r, ov, c->HovT, c->S1, 1, -1.0, 1));                          // Hov[k,c] t2[i,k,a,c]
+    const c128* Hov = c->Hov;
+    launch_fill(st, c->HF, o, v, v, 0, [=] __device__(int64_t k, int64_t cc) {
+        c128 x = f[k * n + o + cc];
+        return mk(Hov[k * v + cc].x - 2.0 * x.x, Hov[k * v + cc].y - 2.0 * x.y);
+    });
+    CCSD_TRY(run_gemm(env, gp(o, o, v, c->HF, v, c->t1, v, c->inner, o, 1, 1.0, 0)));                 // inner[k][i]
+    {
+        GemmParams p = gp(o, v, o, c->inner, 1, c->t1, 1, c->S1, v, 1, 1.0, 1);
+        p.sam = 1; p.sak = o; p.sbn = 1; p.sbk = v;
+        CCSD_TRY(run_gemm(env, p));
+    }
+    CCSD_TRY(run_gemm(env, gp(v, o, o * vv, c->Vvovv_p, o * vv, c->tauou, o * vv, c->S1, 1, v, 1.0, 1)));  // <ak||cd> tau[i,k,c,d]
+    CCSD_TRY(run_gemm(env, gp(o, v, oo * v, c->Vooov_e, oo * v, c->tauc, oo * v, c->S1, v, 1, 1.0, 1)));   // <kl||ic> tau[k,l,c,a]
+    CCSD_TRY(run_gemv(env, ov, ov, c->Vvovo_m, ov, c->t1T, c->tmp_ov, 1, 1.0, 0));                         // <ak||ci> t1[k,c]
+    const c128* tmp = c->tmp_ov;
+    launch_fill(st, c->S1, o, v, v, 1, [=] __device__(int64_t i, int64_t a) { return cneg(tmp[a * o + i]); });
+    return CCSD_OK;
+}
+
+static int residual(ccsd_ctx* c)
+{
+    tick(c, 0);
+    CCSD_TRY(prep_operands(c));
+    tick(c, 1);
+    CCSD_TRY(fock_like(c));
+    tick(c, 2);
+    CCSD_TRY(build_Hvovo(c));   // ticks 3 inside
+    tick(c, 4);
+    CCSD_TRY(build_C(c));
+    tick(c, 5);
+    CCSD_TRY(build_A(c));
+    tick(c, 6);
+    cudaMemsetAsync(c->S2p, 0, (size_t)(c->oo * c->vv) * sizeof(c128), c->st);
+    CCSD_TRY(s2_driver(c, c->S2p));
+    CCSD_TRY(s2_pp_ladder(c, c->S2p));
+    tick(c, 7);
+    CCSD_TRY(s2_hh_and_goo(c, c->S2p));
+    tick(c, 8);
+    CCSD_TRY(s2_ring(c, c->S2p));  // ticks 9 inside
+    tick(c, 10);
+    CCSD_TRY(s2_vdag_t1(c, c->S2p));
+    tick(c, 11);
+    CCSD_TRY(s2_gvv(c, c->S2p));
+    tick(c, 12);
+    CCSD_TRY(s2_c_t1(c, c->S2p));
+    tick(c, 13);
+    CCSD_TRY(build_S1(c));
+    tick(c, 14);
+    c->have_residual = true;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// energy, update, DIIS
+// ---------------------------------------------------------------------------------------------------------------
+static int energy_async(ccsd_ctx* c, double* red_out /* device, 2 doubles */)
+{
+    build_tau(c->st, c->taup, c->t1, c->t2p, c->o, c->v, c->po, c->pv);
+    CCSD_CUDA_TRY(cudaMemsetAsync(red_out, 0, 2 * sizeof(double), c->st));
+    // E = sum_ia f[i,a] t1[i,a] + sum_{i<j,a<b} <ij||ab> tau   (eq 9; reading G11)
+    launch_energy(c->st, c->f, c->n, c->o, c->v, c->t1, c->Voovv_p, c->taup, c->oo * c->vv, red_out);
+    return CCSD_OK;
+}
+
+static int solve_small(std::vector<double>& A, std::vector<double>& b, int m)
+{   // Gaussian elimination with partial pivoting, in place; returns non-zero if singular
+    for (int col = 0; col < m; col++) {
+        int piv = col;
+        for (int r = col + 1; r < m; r++)
+            if (fabs(A[r * m + col]) > fabs(A[piv * m + col])) piv = r;
+        if (fabs(A[piv * m + col]) < 1e-300 || !std::isfinite(A[piv * m + col])) return 1;
+        if (piv != col) {
+            for (int k = 0; k < m; k++) std::swap(A[col * m + k], A[piv * m + k]);
+            std::swap(b[col], b[piv]);
+        }
+        for (int r = col + 1; r < m; r++) {
+            double fct = A[r * m + col] / A[col * m + col];
+            for (int k = col; k < m; k++) A[r * m + k] -= fct * A[col * m + k];
+            b[r] -= fct * b[col];
+        }
+    }
+    for (int r = m - 1; r >= 0; r--) {
+        double s = b[r];
+        for (int k = r + 1; k < m; k++) s -= A[r * m + k] * b[k];
+        b[r] = s / A[r * m + r];
+        if (!std::isfinite(b[r])) return 1;
+    }
+    return 0;
+}
+
+extern "C" {
+
+void ccsd_default_options(ccsd_options* opts)
+{
+    if (!opts) return;
+    opts->ndiis = 6;
+    opts->level_shift = 0.0;
+    opts->gemm_mode = 0;
+    opts->ccd = 0;
+}
+
+int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
+{
+    if (!bytes) return CCSD_EINVAL;
+    CCSD_TRY(check_sizes(nocc, nvir, naux));
+    ccsd_ctx tmp;
+    setup_dims(&tmp, nocc, nvir, naux, opts);
+    carve(&tmp, nullptr, bytes);
+    return CCSD_OK;
+}
+
+int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, int nvir, int naux,
+              const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out || !h || !B || !workspace) return CCSD_EINVAL;
+    CCSD_TRY(check_sizes(nocc, nvir, naux));
+    if (reinterpret_cast<uintptr_t>(workspace) % 256 != 0) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    ccsd_ctx* c = new (std::nothrow) ccsd_ctx();
+    if (!c) return CCSD_ENOMEM;
+    setup_dims(c, nocc, nvir, naux, opts);
+    size_t need = 0;
+    carve(c, nullptr, &need);
+    if (workspace_bytes < need) { delete c; return CCSD_EINVAL; }
+    carve(c, static_cast<char*>(workspace), &need);
+    c->st = static_cast<cudaStream_t>(cuda_stream);
+    c->env = Env{c->st, c->opt.gemm_mode, c->partial, c->partial_elems};
+    c->timing = 0;
+    c->red_host = nullptr;
+    c->gram.assign(13 * 13, 0.0);
+    for (int k = 0; k <= CCSD_NSTEPS; k++) c->ev[k] = nullptr;
+    if (cudaMallocHost(&c->red_host, 64 * sizeof(double)) != cudaSuccess) { delete c; return CCSD_ECUDA; }
+    // zero the padded operand buffers once (pads must stay zero)
+    cudaMemsetAsync(c->TT, 0, (size_t)(c->vv * 2 * c->oop) * sizeof(c128), c->st);
+    cudaMemsetAsync(c->AG, 0, (size_t)(c->oo * 2 * c->oop) * sizeof(c128), c->st);
+    int s = build_constants(c, reinterpret_cast<const c128*>(h), reinterpret_cast<const c128*>(B));
+    if (s == CCSD_OK) mp2_guess(c);
+    if (s == CCSD_OK && cudaStreamSynchronize(c->st) != cudaSuccess) s = CCSD_ECUDA;
+    if (s == CCSD_OK) {
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (init)", cudaGetErrorString(e)); s = CCSD_ECUDA; }
+    }
+    if (s != CCSD_OK) { cudaFreeHost(c->red_host); delete c; return s; }
+    *out = c;
+    return CCSD_OK;
+}
+
+int ccsd_destroy(ccsd_ctx* c)
+{
+    if (!c) return CCSD_ESTATE;
+    for (int k = 0; k <= CCSD_NSTEPS; k++)
+        if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    if (c->red_host) cudaFreeHost(c->red_host);
+    delete c;
+    return CCSD_OK;
+}
+
+int ccsd_energy(ccsd_ctx* c, double* e_re, double* e_im)
+{
+    if (!c) return CCSD_ESTATE;
+    CCSD_TRY(energy_async(c, c->red));
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host, c->red, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    if (e_re) *e_re = c->red_host[0];
+    if (e_im) *e_im = c->red_host[1];
+    return CCSD_OK;
+}
+
+int ccsd_residual(ccsd_ctx* c)
+{
+    if (!c) return CCSD_ESTATE;
+    return residual(c);
+}
+
+int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
+{
+    if (!c) return CCSD_ESTATE;
+    CCSD_TRY(residual(c));
+    const int o = c->o, v = c->v;
+    const int64_t vv = c->vv, ov = c->ov, nvec = c->nvec;
+    const int nd = c->opt.ndiis;
+    const int slot = nd > 0 ? c->diis_next : 0;
+    c128* U = c->diis_u + (int64_t)slot * nvec;
+    c128* E = c->diis_e + (int64_t)slot * nvec;
+    {   // Jacobi step (reading G12): e = S/D, u = t + e
+        const c128 *S1 = c->S1, *S2 = c->S2p, *t1 = c->t1, *t2p = c->t2p;
+        const double* eps = c->eps;
+        const int2 *po = c->po, *pv = c->pv;
+        const int ccd = c->opt.ccd;
+        launch_fill(c->st, E, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
+            if (ccd) { U[i * v + a] = mk(0.0, 0.0); return mk(0.0, 0.0); }
+            double d = eps[i] - eps[o + a];
+            c128 e = mk(S1[i * v + a].x / d, S1[i * v + a].y / d);
+            U[i * v + a] = cadd(t1[i * v + a], e);
+            return e;
+        });
+        c128 *E2 = E + ov, *U2 = U + ov;
+        launch_fill(c->st, E2, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+            int2 ij = po[IJ], ab = pv[AB];
+            double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
+            c128 s = S2[IJ * vv + AB];
+            c128 e = mk(s.x / d, s.y / d);
+            U2[IJ * vv + AB] = cadd(t2p[IJ * vv + AB], e);
+            return e;
+        });
+    }
+    // Gram row of the new error vector against every stored one: Re <e_new | e_l>
+    std::vector<int> order = c->diis_order;
+    if (nd > 0) {
+        // the slot being overwritten leaves the subspace
+        for (size_t k = 0; k < order.size(); k++)
+            if (order[k] == slot) { order.erase(order.begin() + k); break; }
+        order.push_back(slot);
+    } else {
+        order.assign(1, 0);
+    }
+    const int m = (int)order.size();
+    CCSD_CUDA_TRY(cudaMemsetAsync(c->red, 0, 16 * sizeof(double), c->st));
+    for (int k = 0; k < m; k++)
+        launch_redot(c->st, E, c->diis_e + (int64_t)order[k] * nvec, nvec, c->red + k);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host, c->red, 16 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    for (int k = 0; k < m; k++) {
+        c->gram[slot * 13 + order[k]] = c->red_host[k];
+        c->gram[order[k] * 13 + slot] = c->red_host[k];
+    }
+    double snorm = sqrt(c->red_host[m - 1] > 0 ? c->red_host[m - 1] : 0.0);
+    int status = CCSD_OK;
+    // DIIS (reading G13): bordered Pulay system on the last m pairs, real coefficients
+    std::vector<double> coef(m, 0.0);
+    int mm = m;
+    if (nd > 0 && m >= 2) {
+        for (;;) {
+            int dim = mm + 1;
+            std::vector<double> A(dim * dim, 0.0), rhs(dim, 0.0);
+            for (int a = 0; a < mm; a++)
+                for (int b = 0; b < mm; b++) A[a * dim + b] = c->gram[order[m - mm + a] * 13 + order[m - mm + b]];
+            for (int a = 0; a < mm; a++) { A[a * dim + mm] = -1.0; A[mm * dim + a] = -1.0; }
+            rhs[mm] = -1.0;
+            if (solve_small(A, rhs, dim) == 0) {
+                for (int a = 0; a < mm; a++) coef[m - mm + a] = rhs[a];
+                break;
+            }
+            mm--;
+            if (mm < 1) { status = CCSD_ESINGULAR; coef.assign(m, 0.0); coef[m - 1] = 1.0; break; }
+        }
+    } else {
+        coef[m - 1] = 1.0;
+    }
+    // t = sum_l coef_l u_l
+    {
+        DiisCombo combo;
+        combo.m = m;
+        for (int k = 0; k < m; k++) { combo.c[k] = coef[k]; combo.u[k] = c->diis_u + (int64_t)order[k] * nvec; }
+        launch_combine(c->st, combo, c->t1, c->t2p, ov, nvec);
+    }
+    if (nd > 0) {
+        c->diis_order = order;
+        c->diis_next = (slot + 1) % nd;
+        if (c->diis_count < nd) c->diis_count++;
+    }
+    tick(c, 15);
+    CCSD_TRY(energy_async(c, c->red + 32));
+    tick(c, 16);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 32, c->red + 32, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    if (e_re) *e_re = c->red_host[32];
+    if (e_im) *e_im = c->red_host[33];
+    if (step_norm) *step_norm = snorm;
+    if (c->timing) {
+        for (int k = 0; k < CCSD_NSTEPS; k++) cudaEventElapsedTime(&c->step_ms[k], c->ev[k], c->ev[k + 1]);
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return status;
+}
+
+int ccsd_get_amplitudes(ccsd_ctx* c, ccsd_c128* t1, ccsd_c128* t2p)
+{
+    if (!c) return CCSD_ESTATE;
+    if (t1) dcopy(c->st, reinterpret_cast<c128*>(t1), c->t1, c->ov);
+    if (t2p) dcopy(c->st, reinterpret_cast<c128*>(t2p), c->t2p, c->oo * c->vv);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_set_amplitudes(ccsd_ctx* c, const ccsd_c128* t1, const ccsd_c128* t2p, int reset_diis)
+{
+    if (!c) return CCSD_ESTATE;
+    if (t1) dcopy(c->st, c->t1, reinterpret_cast<const c128*>(t1), c->ov);
+    if (t2p) dcopy(c->st, c->t2p, reinterpret_cast<const c128*>(t2p), c->oo * c->vv);
+    if (reset_diis) { c->diis_count = 0; c->diis_next = 0; c->diis_order.clear(); }
+    c->have_residual = false;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_tensor_elems(ccsd_ctx* c, int id, size_t* elems)
+{
+    if (!c || !elems) return CCSD_ESTATE;
+    const int64_t o = c->o, v = c->v, n = c->n, oo = c->oo, vv = c->vv, ov = c->ov;
+    int64_t e = -1;
+    switch (id) {
+    case CCSD_T_FOCK: e = n * n; break;
+    case CCSD_T_VVVV: e = vv * vv; break;
+    case CCSD_T_VOVV: e = ov * vv; break;
+    case CCSD_T_VOVO: e = ov * ov; break;
+    case CCSD_T_OOVV: e = oo * vv; break;
+    case CCSD_T_OOOV: e = oo * ov; break;
+    case CCSD_T_OOOO: e = oo * oo; break;
+    case CCSD_T_TAU: e = oo * vv; break;
+    case CCSD_T_HVV: case CCSD_T_GVV: e = v * v; break;
+    case CCSD_T_HOO: case CCSD_T_GOO: e = o * o; break;
+    case CCSD_T_HOV: e = ov; break;
+    case CCSD_T_HVOVO: e = ov * ov; break;
+    case CCSD_T_C: e = ov * oo; break;
+    case CCSD_T_A: e = oo * oo; break;
+    case CCSD_T_S1: e = ov; break;
+    case CCSD_T_S2: e = oo * vv; break;
+    default:
+        if (id >= CCSD_T_S2_RING && id <= CCSD_T_S2_DRIVER) e = oo * vv;
+    }
+    if (e < 0) return CCSD_EINVAL;
+    *elems = (size_t)e;
+    return CCSD_OK;
+}
+
+int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
+{
+    if (!c || !out_) return CCSD_ESTATE;
+    c128* out = reinterpret_cast<c128*>(out_);
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    cudaStream_t st = c->st;
+    if (id >= CCSD_T_TAU && !c->have_residual) return CCSD_ESTATE;
+    switch (id) {
+    case CCSD_T_FOCK: dcopy(st, out, c->f, (int64_t)c->n * c->n); break;
+    case CCSD_T_VVVV: dcopy(st, out, c->W, vv * vv); break;
+    case CCSD_T_VOVV: dcopy(st, out, c->Vvovv_p, ov * vv); break;
+    case CCSD_T_VOVO: {
+        const c128* V = c->Vvovo_m;  // [(a,i)][(c,k)] -> [a][k][c][i]
+        launch_fill(st, out, ov, ov, ov, 0, [=] __device__(int64_t ak, int64_t ci) {
+            int64_t a = ak / o, k = ak % o, cc = ci / o, i = ci % o;
+            return V[(a * o + i) * ov + cc * o + k];
+        });
+        break;
+    }
+    case CCSD_T_OOVV: dcopy(st, out, c->Voovv_p, oo * vv); break;
+    case CCSD_T_OOOV: dcopy(st, out, c->Vooov_p, oo * ov); break;
+    case CCSD_T_OOOO: dcopy(st, out, c->Voooo_p, oo * oo); break;
+    case CCSD_T_TAU: dcopy(st, out, c->taup, oo * vv); break;
+    case CCSD_T_HVV: dcopy(st, out, c->Hvv, (int64_t)v * v); break;
+    case CCSD_T_GVV: dcopy(st, out, c->Gvv, (int64_t)v * v); break;
+    case CCSD_T_HOO: dcopy(st, out, c->Hoo, (int64_t)o * o); break;
+    case CCSD_T_GOO: dcopy(st, out, c->Goo, (int64_t)o * o); break;
+    case CCSD_T_HOV: dcopy(st, out, c->Hov, ov); break;
+    case CCSD_T_HVOVO: {
+        const c128* H = c->Hm;
+        launch_fill(st, out, ov, ov, ov, 0, [=] __device__(int64_t ak, int64_t ci) {
+            int64_t a = ak / o, k = ak % o, cc = ci / o, i = ci % o;
+            return H[(a * o + i) * ov + cc * o + k];
+        });
+        break;
+    }
+    case CCSD_T_C: {
+        const c128* Cm = c->Cm;  // [(b,k)][I] -> [k][b][I]
+        launch_fill(st, out, ov, oo, oo, 0, [=] __device__(int64_t kb, int64_t IJ) {
+            int64_t k = kb / v, b = kb % v;
+            return Cm[(b * o + k) * oo + IJ];
+        });
+        break;
+    }
+    case CCSD_T_A: dcopy(st, out, c->Am, oo * oo); break;
+    case CCSD_T_S1: dcopy(st, out, c->S1, ov); break;
+    case CCSD_T_S2: dcopy(st, out, c->S2p, oo * vv); break;
+    default: {
+        if (id < CCSD_T_S2_RING || id > CCSD_T_S2_DRIVER) return CCSD_EINVAL;
+        CCSD_CUDA_TRY(cudaMemsetAsync(out, 0, (size_t)(oo * vv) * sizeof(c128), st));
+        int saved = c->timing;
+        c->timing = 0;
+        int s = CCSD_OK;
+        switch (id) {
+        case CCSD_T_S2_RING: s = s2_ring(c, out); break;
+        case CCSD_T_S2_GOO: s = s2_goo(c, out); break;
+        case CCSD_T_S2_VDAG_T1: s = s2_vdag_t1(c, out); break;
+        case CCSD_T_S2_GVV: s = s2_gvv(c, out); break;
+        case CCSD_T_S2_C_T1: s = s2_c_t1(c, out); break;
+        case CCSD_T_S2_HH_LADDER: s = s2_hh_ladder(c, out); break;
+        case CCSD_T_S2_PP_LADDER: s = s2_pp_ladder(c, out); break;
+        case CCSD_T_S2_DRIVER: s = s2_driver(c, out); break;
+        }
+        c->timing = saved;
+        CCSD_TRY(s);
+    }
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// ---- standalone contractions ----------------------------------------------------------------------------------
+int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
+{
+    if (!bytes || nocc < 1 || nvir < 1) return CCSD_EINVAL;
+    const int64_t o = nocc, v = nvir, oo = o * (o - 1) / 2, vv = v * (v - 1) / 2, ov = o * v, oop = round_up(oo > 0 ? oo : 1, 4);
+    Carver w{nullptr, 0};
+    w.take<int2>(oo); w.take<int2>(vv);
+    switch (term) {
+    case CCSD_TERM_PP_LADDER: break;
+    case CCSD_TERM_TAU: break;
+    case CCSD_TERM_HH_LADDER: w.take<c128>(vv * oop); w.take<c128>(oo * oop); break;
+    case CCSD_TERM_RING: w.take<c128>(ov * ov); w.take<c128>(ov * ov); w.take<c128>(ov * ov); break;
+    default: return CCSD_EINVAL;
+    }
+    *bytes = w.off;
+    return CCSD_OK;
+}
+
+int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccsd_c128* out_, int accumulate,
+                  const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!in_ || !out_ || nocc < 1 || nvir < 1) return CCSD_EINVAL;
+    size_t need = 0;
+    CCSD_TRY(ccsd_contract_workspace_bytes(term, nocc, nvir, &need));
+    if (need > 0 && (!workspace || workspace_bytes < need || reinterpret_cast<uintptr_t>(workspace) % 256)) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int o = nocc, v = nvir;
+    const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2, ov = (int64_t)o * v, oop = round_up(oo > 0 ? oo : 1, 4);
+    Env env{st, opts ? opts->gemm_mode : 0, nullptr, 0};
+    c128* out = reinterpret_cast<c128*>(out_);
+    const c128* in0 = reinterpret_cast<const c128*>(in_[0]);
+    const c128* in1 = reinterpret_cast<const c128*>(in_[1]);
+    if (!in0 || !in1) return CCSD_EINVAL;
+    Carver w{static_cast<char*>(workspace), 0};
+    int2* po = w.take<int2>(oo);
+    int2* pv = w.take<int2>(vv);
+    if (oo == 0 || vv == 0) return CCSD_OK;
+    switch (term) {
+    case CCSD_TERM_PP_LADDER:
+        // out[(i<j)][(a<b)] (+)= sum_{c<d} W[(a<b)][(c<d)] tau[(i<j)][(c<d)]
+        return run_gemm(env, gp(vv, oo, vv, in1, vv, in0, vv, out, 1, vv, 1.0, accumulate));
+    case CCSD_TERM_TAU: {
+        pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(po, o);
+        pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(pv, v);
+        g_launches += 2;
+        if (accumulate) return CCSD_EINVAL;
+        build_tau(st, out, in0, in1, o, v, po, pv);
+        CCSD_CUDA_TRY(cudaGetLastError());
+        return CCSD_OK;
+    }
+    case CCSD_TERM_HH_LADDER: {
+        c128* TT = w.take<c128>(vv * oop);
+        c128* AT = w.take<c128>(oo * oop);
+        CCSD_CUDA_TRY(cudaMemsetAsync(TT, 0, (size_t)(vv * oop) * sizeof(c128), st));
+        CCSD_CUDA_TRY(cudaMemsetAsync(AT, 0, (size_t)(oo * oop) * sizeof(c128), st));
+        CCSD_TRY(launch_transpose2d_ld(st, in1, vv, TT, oop, oo, vv, 0));
+        CCSD_TRY(launch_transpose2d_ld(st, in0, oo, AT, oop, oo, oo, 0));
+        return run_gemm(env, gp(vv, oo, oop, TT, oop, AT, oop, out, 1, vv, 1.0, accumulate));
+    }
+    case CCSD_TERM_RING: {
+        pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(po, o);
+        pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(pv, v);
+        g_launches += 2;
+        c128* Hm = w.take<c128>(ov * ov);
+        c128* T2r = w.take<c128>(ov * ov);
+        c128* Xr = w.take<c128>(ov * ov);
+        launch_fill(st, Hm, ov, ov, ov, 0, [=] __device__(int64_t ai, int64_t ck) {   // Hvovo[a][k][c][i] -> [(a,i)][(c,k)]
+            int64_t a = ai / o, i = ai % o, cc = ck / o, k = ck % o;
+            return in0[((a * o + k) * v + cc) * o + i];
+        });
+        launch_fill(st, T2r, ov, ov, ov, 0, [=] __device__(int64_t jb, int64_t ck) {
+            int j = jb / v, b = jb % v, cc = ck / o, k = ck % o;
+            return t2_at(in1, j, k, cc, b, o, v, vv);
+        });
+        CCSD_TRY(run_gemm(env, gp(ov, ov, ov, Hm, ov, T2r, ov, Xr, ov, 1, 1.0, 0)));
+        launch_fill(st, out, oo, vv, vv, accumulate ? 1 : 0, [=] __device__(int64_t IJ, int64_t AB) {
+            int2 ij = po[IJ], ab = pv[AB];
+            int64_t i = ij.x, j = ij.y, a = ab.x, b = ab.y;
+            c128 s = Xr[((a * o + i) * o + j) * v + b];
+            s = csub(s, Xr[((a * o + j) * o + i) * v + b]);
+            s = csub(s, Xr[((b * o + i) * o + j) * v + a]);
+            s = cadd(s, Xr[((b * o + j) * o + i) * v + a]);
+            return s;
+        });
+        CCSD_CUDA_TRY(cudaGetLastError());
+        return CCSD_OK;
+    }
+    default: return CCSD_EINVAL;
+    }
+}
+
+int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
+                  ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
+                  void* cuda_stream)
+{
+    if (!A || !B || !C || M < 0 || N < 0 || K < 0 || mode < 0 || mode > 2) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    Env env{static_cast<cudaStream_t>(cuda_stream), mode, nullptr, 0};
+    GemmParams p = gp(M, N, K, reinterpret_cast<const c128*>(A), lda, reinterpret_cast<const c128*>(B), ldb,
+                      reinterpret_cast<c128*>(C), csm, csn, 1.0, accumulate);
+    p.alpha = mk(alpha_re, alpha_im);
+    return run_gemm(env, p);
+}
+
+int ccsd_transpose(const ccsd_c128* in, ccsd_c128* out, const int64_t dims[4], const int perm[4], int conj, void* cuda_stream)
+{
+    if (!in || !out || !dims || !perm) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    return launch_transpose4d(static_cast<cudaStream_t>(cuda_stream), reinterpret_cast<const c128*>(in),
+                              reinterpret_cast<c128*>(out), dims, perm, conj);
+}
+
+int ccsd_enable_step_timing(ccsd_ctx* c, int enable)
+{
+    if (!c) return CCSD_ESTATE;
+    if (enable && !c->ev[0])
+        for (int k = 0; k <= CCSD_NSTEPS; k++) CCSD_CUDA_TRY(cudaEventCreate(&c->ev[k]));
+    c->timing = enable ? 1 : 0;
+    return CCSD_OK;
+}
+
+int ccsd_get_step_times(ccsd_ctx* c, float ms[CCSD_NSTEPS])
+{
+    if (!c || !ms) return CCSD_ESTATE;
+    for (int k = 0; k < CCSD_NSTEPS; k++) ms[k] = c->step_ms[k];
+    return CCSD_OK;
+}
+
+const char* ccsd_step_name(int step) { return (step >= 0 && step < CCSD_NSTEPS) ? k_step_names[step] : ""; }
+
+long long ccsd_launch_count(int reset)
+{
+    long long r = g_launches;
+    if (reset) g_launches = 0;
+    return r;
+}
+
+const char* ccsd_strerror(int s)
+{
+    switch (s) {
+    case CCSD_OK: return "ok";
+    case CCSD_EINVAL: return "invalid argument";
+    case CCSD_ENOMEM: return "out of host memory";
+    case CCSD_ECUDA: return "CUDA error";
+    case CCSD_ESTATE: return "invalid state or handle";
+    case CCSD_ESINGULAR: return "singular DIIS system";
+    default: return "unknown status";
+    }
+}
+
+const char* ccsd_last_cuda_error(void) { return g_cuda_err; }
+
+}  // extern "C"
