@@ -1,0 +1,427 @@
+#!/usr/bin/env python
+"""Benchmark of the B200-native complex CCSD hot path (BASELINE.json metric: CCSD s/iteration and pp-ladder FP64
+TFLOP/s as % of the B200 FP64 peak, 1 GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3|cfg2|cfg1|cfg0] [--no-sweep]
+    python bench.py --impl reference ...        # the CPU oracle, timed on the host cores (bounded sample)
+
+One "step" = one ccsd_iterate: the whole hot path (eqs 23-33, Jacobi + DIIS update, energy) on one set of synthetic
+inputs (ccsd_inputs.py, recipe in DESIGN.md).  `value` is measured with the tensors resident in HBM; `e2e` adds the
+host->device copy of the amplitudes from pinned memory and the device->host copy of the new amplitudes + energy
+every step.  The path does not shard (north_star: one GPU, no collectives): N > 1 runs N independent replicas.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import ccsd_inputs as ci  # noqa: E402
+
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of gemm_dmma_kernel<8> at cfg3, from
+# profiles/r01_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
+NCU_TRAFFIC_BYTES = {"cfg3": None}
+
+
+def flops_per_iteration(o: int, v: int) -> dict:
+    """Algorithmic work of the GEMM-view steps (8 real flop per complex MAC, packed index ranges): DESIGN.md table."""
+    oo, vv, ov = o * (o - 1) // 2, v * (v - 1) // 2, o * v
+    f = {
+        "pp_ladder": 8 * oo * vv * vv,
+        "Hvovo_quad": 8 * ov ** 3,
+        "ring_gemm": 8 * ov ** 3,
+        "C_ovoo": 8 * ov * oo * vv + 8 * ov * o * o * v,
+        "A_oooo": 8 * oo * oo * vv + 8 * oo * o * o * v,
+        "hh_ladder+Goo": 8 * oo * oo * vv,            # algorithmic: hh-ladder oo^2 vv (+ Goo term o*oo*vv*... small)
+        "fock_like": 8 * (v * v * oo * v + o * o * o * vv + 2 * ov * ov),
+        "Hvovo_linear": 8 * (v * ov * o * v + v * o * ov * o),
+        "Vdag_t1": 8 * o * vv * o * v,
+        "Gvv_t2": 8 * oo * v * v * v,
+        "C_t1": 8 * v * oo * v * o,
+        "S1": 8 * (v * o * o * vv + o * v * oo * v + 2 * ov * ov),
+    }
+    f["total"] = sum(f.values())
+    return f
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, power, reasons = [], [], [], set()
+        for t, line in self.rows:
+            if t < t0 or t > t1 + 0.1:
+                continue
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "MEASURED_PEAKS.json (of measured)"}
+    return {"hbm_gbs": 6650.0, "source": "fallback of B200_PROFILING.md (of fallback)"}
+
+
+# -------------------------------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference)
+# -------------------------------------------------------------------------------------------------------------------
+def oracle_sample_seconds_per_iteration(cfg: str, budget_s: float = 12.0) -> dict:
+    """Time the oracle, as it stands, on a bounded sample of the workload and scale to s/iteration.
+
+    cfg0 / cfg1: one real oracle iteration (restricted-sum mode).  cfg2 / cfg3: the oracle's explicit pp-ladder loop
+    (oracle_pp_ladder_samples) on `nrow` rows of a synthetic W[(a<b)][(c<d)] against every row of tau[(i<j)][(c<d)]
+    of the real shape; the measured complex-MAC rate is scaled to the algorithmic work of the whole iteration.
+    """
+    from oracle import ccsd_oracle as orc
+    o, v, L, seed = ci.CONFIGS[cfg]
+    cores = orc.num_threads()
+    if cfg in ("cfg0", "cfg0_2e", "cfg1"):
+        inp = ci.make_config(cfg)
+        oc = orc.OracleCCSD(inp.h, inp.B, o, v, restricted=True)
+        t0 = time.perf_counter()
+        oc.iterate()
+        dt = time.perf_counter() - t0
+        return {"value": dt, "unit": "s/iteration", "cores": cores, "kind": "oracle",
+                "sample": f"one full oracle iteration of {cfg} (restricted-sum loops)"}
+    oo, vv = ci.pair_count(o), ci.pair_count(v)
+    rng = np.random.default_rng(seed)
+    tau = (rng.standard_normal((oo, vv)) + 1j * rng.standard_normal((oo, vv))) * 0.01 / np.sqrt(2)
+    rate = None
+    nrow = 64
+    while True:
+        W = (rng.standard_normal((nrow, vv)) + 1j * rng.standard_normal((nrow, vv))) * 5e-3 / np.sqrt(2)
+        ij, ab = np.meshgrid(np.arange(oo), np.arange(nrow), indexing="ij")
+        t0 = time.perf_counter()
+        orc.pp_ladder_samples(tau, W, ij.ravel(), ab.ravel())
+        dt = time.perf_counter() - t0
+        rate = oo * nrow * vv / dt            # complex MAC / s
+        if dt > budget_s / 3 or nrow >= 8192:
+            break
+        nrow = int(min(8192, nrow * 8, max(nrow * 2, nrow * (budget_s * 0.6) / max(dt, 1e-3))))
+    total_cmac = flops_per_iteration(o, v)["total"] / 8.0
+    return {"value": total_cmac / rate, "unit": "s/iteration", "cores": cores, "kind": "oracle",
+            "sample": f"oracle pp-ladder loop on {nrow} of {vv} W rows x all {oo} tau rows ({dt:.1f} s, "
+                      f"{8 * rate * 1e-9:.1f} GFLOP/s), scaled to the {total_cmac * 8e-12:.2f} TFLOP of one {cfg} iteration"}
+
+
+def run_reference(args) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    info = None
+    for _ in range(max(1, args.warmup if args.warmup < 2 else 1)):
+        oracle_sample_seconds_per_iteration(args.config, budget_s=3.0)
+    for _ in range(max(1, min(args.steps, 3))):
+        info = oracle_sample_seconds_per_iteration(args.config, budget_s=8.0)
+        vals.append(info["value"])
+    v = statistics.median(vals)
+    o, vv_, L, _ = ci.CONFIGS[args.config]
+    info["value"] = v
+    line = {"impl": "reference", "metric": "ccsd_seconds_per_iteration", "value": v, "unit": "s/iteration",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": v * 1e3,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
+            "data": "synthetic", "config": {"workload": f"{args.config}: nocc={o} nvir={vv_} naux={L}"},
+            "cpu_baseline": info,
+            "e2e": {"value": v, "unit": "s/iteration", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# -------------------------------------------------------------------------------------------------------------------
+# GPU arm
+# -------------------------------------------------------------------------------------------------------------------
+def time_events(torch, fn, reps, warmup):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    return ts
+
+
+def ladder_sweep(torch, pkg, peak_tflops, reps=5, warmup=3):
+    """BASELINE config 4: isolated pp-ladder R[(i<j)][(a<b)] = sum_{c<d} W tau per shape, with sampled parity."""
+    from oracle.ccsd_oracle import pp_ladder_samples
+    out = []
+    for k, (o, v) in enumerate(ci.LADDER_SWEEP):
+        oo, vv = ci.pair_count(o), ci.pair_count(v)
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(ci.LADDER_SEED0 + k)
+        W = torch.view_as_complex(torch.randn((vv, vv, 2), generator=gen, device="cuda", dtype=torch.float64))
+        W.mul_(5e-3 / np.sqrt(2))
+        tau = torch.view_as_complex(torch.randn((oo, vv, 2), generator=gen, device="cuda", dtype=torch.float64))
+        tau.mul_(0.01 / np.sqrt(2))
+        R = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
+        ts = time_events(torch, lambda: pkg.contract("pp_ladder", o, v, [tau, W], out=R), reps, warmup)
+        t = statistics.median(ts)
+        # sampled parity against the oracle (inputs come from torch's RNG, not from the CUDA path)
+        rng = np.random.default_rng(k)
+        ij = rng.integers(0, oo, 64); ab = rng.integers(0, vv, 64)
+        Wrows = W[torch.from_numpy(np.unique(ab)).cuda()].cpu().numpy()
+        remap = {a: i for i, a in enumerate(np.unique(ab))}
+        ref = pp_ladder_samples(tau.cpu().numpy(), Wrows, ij, np.array([remap[a] for a in ab]))
+        got = R[torch.from_numpy(ij).cuda(), torch.from_numpy(ab).cuda()].cpu().numpy()
+        err = float(np.abs(got - ref).max() / np.abs(ref).max())
+        tf = 8.0 * oo * vv * vv / (t * 1e-3) * 1e-12
+        out.append({"nocc": o, "nvir": v, "ms": round(t, 3), "tflops": round(tf, 2),
+                    "frac_fp64_peak": round(tf / peak_tflops, 4), "sampled_rel_err": err})
+        del W, tau, R
+        torch.cuda.empty_cache()
+    return out
+
+
+def transpose_bench(torch, pkg, hbm_gbs, o, v):
+    """Transposition GB/s (read + write bytes) on o^2 v^2-shaped complex128 tensors."""
+    x = torch.view_as_complex(torch.randn((o, o, v, v, 2), device="cuda", dtype=torch.float64))
+    nbytes = 2 * x.numel() * 16
+    res = {}
+    for name, perm in (("ijab->abij", [2, 3, 0, 1]), ("ijab->iajb", [0, 2, 1, 3]), ("ijab->jiba", [1, 0, 3, 2])):
+        ts = time_events(torch, lambda: pkg.transpose(x, perm), 5, 3)
+        gbs = nbytes / (statistics.median(ts) * 1e-3) * 1e-9
+        res[name] = {"gbs": round(gbs, 1), "frac_hbm": round(gbs / hbm_gbs, 3)}
+    return res
+
+
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+    import paper_2103_08473_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = args.config
+    o, v, L, seed = ci.CONFIGS[cfg]
+    oo, vv, ov = ci.pair_count(o), ci.pair_count(v), o * v
+    if args.only_ladder:
+        # profiling aid: just the pp-ladder launch of this workload's shape (same kernel, same launch configuration
+        # as inside ccsd_iterate), W warm-ups + K timed launches
+        pkg.load_library()
+        gen = torch.Generator(device="cuda"); gen.manual_seed(seed)
+        W = torch.view_as_complex(torch.randn((vv, vv, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(5e-3 / np.sqrt(2))
+        tau = torch.view_as_complex(torch.randn((oo, vv, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(0.01 / np.sqrt(2))
+        R = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
+        ts = time_events(torch, lambda: pkg.contract("pp_ladder", o, v, [tau, W], out=R), args.steps, args.warmup)
+        t = statistics.median(ts)
+        print(json.dumps({"metric": "pp_ladder_tflops", "value": 8.0 * oo * vv * vv / (t * 1e-3) * 1e-12, "unit": "TFLOP/s",
+                          "ms_per_launch": t, "config": {"workload": f"{cfg} pp-ladder {vv}x{oo}x{vv}"}}))
+        return
+    inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
+    pkg.load_library()
+    pkg.launch_count(reset=True)
+    t0 = time.perf_counter()
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    torch.cuda.synchronize()
+    init_s = time.perf_counter() - t0
+    e_mp2 = solver.energy()
+    peak = pkg.measure_fp64_peak(8) if rank == 0 else FP64_NOMINAL_TFLOPS
+    peaks = measured_peaks()
+    solver.enable_step_timing(True)
+
+    # ---- device-resident timing: W warm-up iterations, then exactly K timed iterations --------------------------
+    for _ in range(args.warmup):
+        solver.iterate()
+    barrier()
+    launches0 = pkg.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    step_acc = {}
+    t_wall0 = time.time()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    energies = []
+    for _ in range(args.steps):
+        e, sn = solver.iterate()
+        energies.append((e, sn))
+        for k, x in solver.step_times().items():
+            step_acc.setdefault(k, []).append(x)
+    e1.record()
+    barrier()
+    t_wall1 = time.time()
+    ms_total = e0.elapsed_time(e1)
+    launches = pkg.launch_count() - launches0
+    clocks = sampler.stop(t_wall0, t_wall1)
+    if world > 1:
+        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_per_step = ms_total / args.steps
+
+    # ---- end to end: amplitudes travel host(pinned) -> device -> host every step ----------------------------------
+    t1_d, t2_d = solver.get_amplitudes()
+    t1_h = torch.empty(t1_d.shape, dtype=torch.complex128).pin_memory()
+    t2_h = torch.empty(t2_d.shape, dtype=torch.complex128).pin_memory()
+    t1_h.copy_(t1_d); t2_h.copy_(t2_d)
+
+    def e2e_step():
+        t1_d.copy_(t1_h, non_blocking=True)
+        t2_d.copy_(t2_h, non_blocking=True)
+        solver.set_amplitudes(t1_d, t2_d, reset_diis=False)
+        e, sn = solver.iterate()
+        a1, a2 = solver.get_amplitudes()
+        t1_h.copy_(a1, non_blocking=True)
+        t2_h.copy_(a2, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    e2e_step()
+    barrier()
+    tw = time.perf_counter()
+    nsteps_e2e = max(1, min(args.steps, 5))
+    for _ in range(nsteps_e2e):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - tw) / nsteps_e2e
+    if world > 1:
+        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    nvec_bytes = (ov + oo * vv) * 16
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the DMMA GEMM, measured on the pp-ladder launch) ------------------------
+    fl = flops_per_iteration(o, v)
+    steps_med = {k: statistics.median(x) for k, x in step_acc.items()}
+    pp_ms = steps_med["pp_ladder"]
+    pp_tflops = fl["pp_ladder"] / (pp_ms * 1e-3) * 1e-12
+    terms = {}
+    for k, ms in steps_med.items():
+        ent = {"ms": round(ms, 3)}
+        if k in fl and ms > 0:
+            ent["tflops"] = round(fl[k] / (ms * 1e-3) * 1e-12, 2)
+        terms[k] = ent
+    gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
+    gemm_ms = sum(steps_med[k] for k in gemm_steps)
+    roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<NI> (FP64 DMMA.8x8x4), pp-ladder launch",
+                "achieved": round(pp_tflops, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
+                "frac": round(pp_tflops / peak, 4), "traffic": NCU_TRAFFIC_BYTES.get(cfg),
+                "peak_source": "DMMA.8x8x4 issue-rate microbenchmark measured in this run (ccsd_measure_fp64_peak); "
+                               f"nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = {FP64_NOMINAL_TFLOPS:.1f}; "
+                               "MEASURED_PEAKS.json has no FP64 entry",
+                "flops_per_launch": fl["pp_ladder"], "launch_ms": round(pp_ms, 3),
+                "share_of_step": round(pp_ms / ms_per_step, 4),
+                "three_big_gemms": {"ms": round(gemm_ms, 3), "share_of_step": round(gemm_ms / ms_per_step, 4),
+                                    "tflops": round(sum(fl[k] for k in gemm_steps) / (gemm_ms * 1e-3) * 1e-12, 2)}}
+
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
+    transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
+    cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
+
+    line = {
+        "metric": "ccsd_seconds_per_iteration", "value": ms_per_step * 1e-3, "unit": "s/iteration",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
+        "data": "synthetic",
+        "config": {"workload": f"{cfg}: nocc={o} nvir={v} naux={L} complex128, DIIS(6), antisymmetry-packed "
+                               f"<ab||cd> {vv}x{vv}", "replicas": world, "l2": "inputs larger than L2 (packed <ab||cd> "
+                               f"= {vv * vv * 16 / 2 ** 30:.2f} GiB vs 126 MB L2); no flush needed",
+                   "init_seconds": round(init_s, 3)},
+        "iteration_tflops": round(fl["total"] / (ms_per_step * 1e-3) * 1e-12, 2),
+        "iteration_frac_fp64_peak": round(fl["total"] / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
+        "pp_ladder_tflops": round(pp_tflops, 2), "pp_ladder_frac_fp64_peak": round(pp_tflops / peak, 4),
+        "roofline": roofline, "terms": terms,
+        "e2e": {"value": e2e_s, "unit": "s/iteration", "h2d_bytes_per_step": nvec_bytes,
+                "d2h_bytes_per_step": nvec_bytes + 24},
+        "gpu_launches": launches, "clocks": clocks,
+        "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
+                     "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
+        "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -147,6 +147,13 @@ const char* ccsd_step_name(int step);
 /* Kernel launches issued by the library since the last reset (all contexts, this process). */
 long long ccsd_launch_count(int reset);
 
+/*
+ * FP64 tensor-pipe yardstick: times a register-resident DMMA.8x8x4 (mma.sync.m8n8k4.f64) issue loop with no memory
+ * traffic and returns the best of `launches` (~1 ms each) in TFLOP/s (HOST out-pointer).  device_scratch: >= 8 bytes.
+ * This is the denominator of the "fraction of FP64 peak" numbers (148 SMs x 64 FMA/clk x 2 x SM clock).
+ */
+int ccsd_measure_fp64_peak(double* tflops, double* device_scratch, int launches, void* cuda_stream);
+
 const char* ccsd_strerror(int status);
 /* Last CUDA error string seen by the library on this thread ("" if none). */
 const char* ccsd_last_cuda_error(void);

@@ -273,7 +273,8 @@ def pp_ladder_samples(taup: np.ndarray, W: np.ndarray, ij: np.ndarray, ab: np.nd
     ij = np.ascontiguousarray(ij, dtype=np.int64)
     ab = np.ascontiguousarray(ab, dtype=np.int64)
     out = np.zeros(len(ij), dtype=C128)
-    lib().oracle_pp_ladder_samples(ctypes.c_long(taup.shape[0]), ctypes.c_long(W.shape[0]), _p(taup), _p(W),
+    assert taup.shape[1] == W.shape[1]
+    lib().oracle_pp_ladder_samples(ctypes.c_long(taup.shape[0]), ctypes.c_long(W.shape[1]), _p(taup), _p(W),
                                    len(ij), _p(ij), _p(ab), _p(out))
     return out
 

@@ -19,7 +19,8 @@ NSTEPS = 16
 EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_iterate", "ccsd_energy", "ccsd_residual",
            "ccsd_get_amplitudes", "ccsd_set_amplitudes", "ccsd_tensor_elems", "ccsd_get_tensor", "ccsd_destroy",
            "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_transpose",
-           "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count", "ccsd_strerror",
+           "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
+           "ccsd_measure_fp64_peak", "ccsd_strerror",
            "ccsd_last_cuda_error"]
 
 
@@ -76,6 +77,7 @@ def load_library():
         lib.ccsd_step_name.restype = ctypes.c_char_p
         lib.ccsd_launch_count.argtypes = [ctypes.c_int]
         lib.ccsd_launch_count.restype = ctypes.c_longlong
+        lib.ccsd_measure_fp64_peak.argtypes = [ctypes.POINTER(dbl), vp, ctypes.c_int, vp]
         lib.ccsd_strerror.argtypes = [ctypes.c_int]
         lib.ccsd_strerror.restype = ctypes.c_char_p
         lib.ccsd_last_cuda_error.restype = ctypes.c_char_p
@@ -130,6 +132,17 @@ def _dev_c128(torch, x):
 
 def launch_count(reset: bool = False) -> int:
     return int(load_library().ccsd_launch_count(1 if reset else 0))
+
+
+def measure_fp64_peak(launches: int = 10) -> float:
+    """DMMA.8x8x4 issue-rate yardstick in TFLOP/s (ccsd_measure_fp64_peak)."""
+    torch = _torch()
+    lib = load_library()
+    scratch = torch.zeros(8, dtype=torch.float64, device="cuda")
+    out = ctypes.c_double(0.0)
+    _check(lib.ccsd_measure_fp64_peak(ctypes.byref(out), scratch.data_ptr(), int(launches), _stream_ptr(torch)),
+           "ccsd_measure_fp64_peak")
+    return float(out.value)
 
 
 def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False) -> Options:

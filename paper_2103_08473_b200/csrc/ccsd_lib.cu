@@ -14,6 +14,7 @@
 #include "gemm_dmma.cuh"
 #include "transpose.cuh"
 #include "reduce.cuh"
+#include "peak.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -55,21 +56,29 @@ static int run_gemm(const Env& env, GemmParams p)
     bool dmma_ok = dmma_supported(p);
     if (env.gemm_mode == 2 && !dmma_ok) return CCSD_EINVAL;
     bool use_dmma = (env.gemm_mode == 2) || (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p));
-    // split-K when the output has too few tiles to fill the machine
+    // split-K chosen against wave quantisation on the 148 SMs: minimise  waves(ks) * (K/ks + pipeline overhead)
     const int bm = use_dmma ? DMMA_BM : SG_BM, bn = use_dmma ? dmma_bn_for(p.N) : SG_BN;
-    int64_t tiles = ((p.M + bm - 1) / bm) * ((p.N + bn - 1) / bn) * p.batch;
+    const int64_t tiles = ((p.M + bm - 1) / bm) * ((p.N + bn - 1) / bn) * p.batch;
     p.ksplit = 1; p.kchunk = p.K; p.partial = nullptr;
-    if (env.partial && tiles < 148 && p.K >= 2048) {
-        int64_t want = (2 * 148 + tiles - 1) / tiles;
-        int64_t maxk = p.K / 512;
-        int64_t cap = env.partial_elems / (p.M * p.N * p.batch);
-        int64_t ks = want < maxk ? want : maxk;
-        if (ks > cap) ks = cap;
-        if (ks > 1) {
-            int64_t chunk = round_up((p.K + ks - 1) / ks, 16);
+    if (env.partial && p.K >= 512) {
+        const int64_t cap = env.partial_elems / (p.M * p.N * p.batch);
+        const double overhead = 96.0;   // pipeline fill + epilogue, in units of k
+        double best = 1e300;
+        int best_ks = 1;
+        for (int ks = 1; ks <= 592 && ks <= cap && (ks == 1 || p.K / ks >= 256); ks++) {
+            if (ks > 16 && tiles * ks > 2 * 592) break;   // deep splits only for skinny outputs
+            const int64_t chunk = round_up((p.K + ks - 1) / ks, 16);
+            const int64_t nsplit = (p.K + chunk - 1) / chunk;
+            const int64_t waves = (tiles * nsplit + 147) / 148;
+            double cost = (double)waves * ((double)chunk + overhead) * (ks > 1 ? 1.02 : 1.0);
+            if (cost < best * 0.97) { best = cost; best_ks = ks; }
+        }
+        if (best_ks > 1) {
+            const int64_t chunk = round_up((p.K + best_ks - 1) / best_ks, 16);
             p.ksplit = (int)((p.K + chunk - 1) / chunk);
             p.kchunk = chunk;
             p.partial = env.partial;
+            if (p.ksplit <= 1) { p.ksplit = 1; p.kchunk = p.K; p.partial = nullptr; }
         }
     }
     if (use_dmma) {
@@ -236,7 +245,9 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Rr = w.take<c128>(v * oo * v);
     c->Y = w.take<c128>(ov * o * o);
     c->Z = w.take<c128>(oo * o * o);
-    c->partial_elems = 16 * 1024 * 1024;  // 256 MB of split-K partials
+    c->partial_elems = 16 * 1024 * 1024;  // split-K partials: >= 256 MB and >= 4 copies of the largest split-K output
+    if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
+    if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
     c->partial = w.take<c128>(c->partial_elems);
     c->nvec = ov + oo * vv;
     int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
@@ -813,9 +824,9 @@ static int residual(ccsd_ctx* c)
     CCSD_TRY(build_C(c));
     tick(c, 5);
     CCSD_TRY(build_A(c));
-    tick(c, 6);
     cudaMemsetAsync(c->S2p, 0, (size_t)(c->oo * c->vv) * sizeof(c128), c->st);
     CCSD_TRY(s2_driver(c, c->S2p));
+    tick(c, 6);
     CCSD_TRY(s2_pp_ladder(c, c->S2p));
     tick(c, 7);
     CCSD_TRY(s2_hh_and_goo(c, c->S2p));
@@ -1186,6 +1197,12 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
 }
 
 // ---- standalone contractions ----------------------------------------------------------------------------------
+static int64_t contract_partial_elems(int term, int64_t oo, int64_t vv, int64_t ov)
+{
+    if (term == CCSD_TERM_TAU) return 0;
+    return 8 * (term == CCSD_TERM_RING ? ov * ov : oo * vv);
+}
+
 int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
 {
     if (!bytes || nocc < 1 || nvir < 1) return CCSD_EINVAL;
@@ -1199,6 +1216,7 @@ int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
     case CCSD_TERM_RING: w.take<c128>(ov * ov); w.take<c128>(ov * ov); w.take<c128>(ov * ov); break;
     default: return CCSD_EINVAL;
     }
+    w.take<c128>(contract_partial_elems(term, oo, vv, ov));
     *bytes = w.off;
     return CCSD_OK;
 }
@@ -1219,6 +1237,13 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
     const int o = nocc, v = nvir;
     const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2, ov = (int64_t)o * v, oop = round_up(oo > 0 ? oo : 1, 4);
     Env env{st, opts ? opts->gemm_mode : 0, nullptr, 0};
+    {   // split-K partials live at the end of the workspace (same carving order as ccsd_contract_workspace_bytes)
+        size_t all = 0;
+        ccsd_contract_workspace_bytes(term, nocc, nvir, &all);
+        int64_t pe = contract_partial_elems(term, oo, vv, ov);
+        size_t pbytes = ((size_t)(pe > 0 ? pe : 1) * sizeof(c128) + 255) & ~(size_t)255;
+        if (pe > 0) { env.partial = reinterpret_cast<c128*>(static_cast<char*>(workspace) + (all - pbytes)); env.partial_elems = pe; }
+    }
     c128* out = reinterpret_cast<c128*>(out_);
     const c128* in0 = reinterpret_cast<const c128*>(in_[0]);
     const c128* in1 = reinterpret_cast<const c128*>(in_[1]);
@@ -1324,6 +1349,17 @@ int ccsd_get_step_times(ccsd_ctx* c, float ms[CCSD_NSTEPS])
     if (!c || !ms) return CCSD_ESTATE;
     for (int k = 0; k < CCSD_NSTEPS; k++) ms[k] = c->step_ms[k];
     return CCSD_OK;
+}
+
+int ccsd_measure_fp64_peak(double* tflops, double* device_scratch, int launches, void* cuda_stream)
+{
+    if (!tflops || !device_scratch || launches < 1) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    return measure_fp64_peak(static_cast<cudaStream_t>(cuda_stream), device_scratch, launches, tflops);
 }
 
 const char* ccsd_step_name(int step) { return (step >= 0 && step < CCSD_NSTEPS) ? k_step_names[step] : ""; }
