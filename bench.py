@@ -238,6 +238,20 @@ def transpose_bench(torch, pkg, hbm_gbs, o, v):
     return res
 
 
+def max_over_ranks(value: float, dist, device="cuda") -> float:
+    """Multi-GPU numbers are the MAX over ranks (replicas-only path: no data-path collective exists)."""
+    import torch
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def is_reporting_rank() -> bool:
+    return int(os.environ.get("RANK", "0")) == 0
+
+
 def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
@@ -310,10 +324,7 @@ def run_ours(args) -> None:
     ms_total = e0.elapsed_time(e1)
     launches = pkg.launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1)
-    if world > 1:
-        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(ms_total, dist if world > 1 else None)
     ms_per_step = ms_total / args.steps
 
     # ---- end to end: amplitudes travel host(pinned) -> device -> host every step ----------------------------------
@@ -340,13 +351,10 @@ def run_ours(args) -> None:
         e2e_step()
     barrier()
     e2e_s = (time.perf_counter() - tw) / nsteps_e2e
-    if world > 1:
-        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = max_over_ranks(e2e_s, dist if world > 1 else None)
     nvec_bytes = (ov + oo * vv) * 16
 
-    if rank != 0:
+    if not is_reporting_rank():
         if world > 1:
             dist.destroy_process_group()
         return

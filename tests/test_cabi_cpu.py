@@ -1,0 +1,102 @@
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol include/ccsd.h declares, its host
+logic (sizes, defaults, error codes) behaves, and nothing computes without a GPU (no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2103_08473_b200 import build
+    build.build()                       # nvcc cross-compiles for sm_100a without a GPU
+    import paper_2103_08473_b200 as pkg
+    return pkg.load_library()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "ccsd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ccsd_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_symbols()
+    assert len(names) >= 20
+    for n in names:
+        assert hasattr(lib, n), n
+    from paper_2103_08473_b200.binding import EXPORTS
+    assert sorted(EXPORTS) == names
+
+
+def test_defaults_and_strerror(lib):
+    from paper_2103_08473_b200.binding import Options
+    o = Options()
+    lib.ccsd_default_options(ctypes.byref(o))
+    assert (o.ndiis, o.level_shift, o.gemm_mode, o.ccd) == (6, 0.0, 0, 0)
+    assert lib.ccsd_strerror(0) == b"ok"
+    assert b"CUDA" in lib.ccsd_strerror(3)
+    assert lib.ccsd_step_name(6) == b"pp_ladder" and lib.ccsd_step_name(99) == b""
+
+
+def test_workspace_bytes_scales_and_validates(lib):
+    n = ctypes.c_size_t(0)
+    assert lib.ccsd_workspace_bytes(4, 16, 60, None, ctypes.byref(n)) == 0
+    small = n.value
+    assert lib.ccsd_workspace_bytes(34, 224, 774, None, ctypes.byref(n)) == 0
+    big = n.value
+    vv = 224 * 223 // 2
+    assert big > vv * vv * 16 and big < 80 * 2 ** 30      # holds packed <ab||cd>; fits a 180 GB part with room
+    assert small < big
+    assert lib.ccsd_workspace_bytes(1, 16, 60, None, ctypes.byref(n)) == 1      # CCSD_EINVAL
+    assert lib.ccsd_workspace_bytes(4, 16, 0, None, ctypes.byref(n)) == 1
+    assert lib.ccsd_workspace_bytes(4, 16, 60, None, None) == 1
+    assert lib.ccsd_contract_workspace_bytes(0, 4, 16, ctypes.byref(n)) == 0
+    assert lib.ccsd_contract_workspace_bytes(7, 4, 16, ctypes.byref(n)) == 1
+
+
+def test_null_handles_are_rejected(lib):
+    assert lib.ccsd_iterate(None, None, None, None) == 4     # CCSD_ESTATE
+    assert lib.ccsd_energy(None, None, None) == 4
+    assert lib.ccsd_destroy(None) == 4
+    assert lib.ccsd_get_tensor(None, 0, None) == 4
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device the compute entry points fail loudly instead of computing on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    buf = (ctypes.c_double * 64)()
+    p = ctypes.cast(buf, ctypes.c_void_p)
+    assert lib.ccsd_zgemm_nt(2, 2, 2, p, 2, p, 2, p, 2, 1, 1.0, 0.0, 0, 0, None) == 3       # CCSD_ECUDA
+    ctx = ctypes.c_void_p(None)
+    ws = ctypes.c_void_p(256 * 1024)
+    assert lib.ccsd_init(ctypes.byref(ctx), p, p, 2, 2, 1, None, ws, 1 << 40, None) == 3
+    assert not ctx.value
+    import paper_2103_08473_b200 as pkg
+    with pytest.raises(RuntimeError):
+        pkg.zgemm_nt([[1.0]], [[1.0]])
+    import numpy as np
+    with pytest.raises(RuntimeError):
+        pkg.CCSD(np.eye(4), np.zeros((1, 4, 4)), 2, 2)
+
+
+def test_product_does_not_import_oracle():
+    """The product path shares no code with the oracle and never routes through it."""
+    pkg_dir = os.path.join(ROOT, "paper_2103_08473_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.replace("shares nothing with oracle/", "").replace(
+                    "no code shared with oracle/", "") or f in ("ccsd_lib.cu", "common.cuh"), f
+                assert "import oracle" not in text and "from oracle" not in text, f
+    for f in ("ccsd_oracle.py", "ccsd_oracle.c"):
+        text = open(os.path.join(ROOT, "oracle", f)).read()
+        assert not re.search(r"^\s*(import|from)\s+paper_2103_08473_b200", text, flags=re.M), f
+        assert not re.search(r"#\s*include\s*[<\"].*ccsd\.h", text), f
+        assert "csrc" not in text, f
