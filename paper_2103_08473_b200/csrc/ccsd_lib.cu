@@ -30,7 +30,7 @@ long long g_launches = 0;
 // ---------------------------------------------------------------------------------------------------------------
 struct Env {
     cudaStream_t st;
-    int gemm_mode;          // 0 auto, 1 simple only, 2 force dmma
+    int gemm_mode;          // 0 auto, 1 simple only, 2 DMMA 4M, 3 DMMA 3M, 100+v explicit variant
     c128* partial;          // split-K scratch
     int64_t partial_elems;
 };
@@ -54,10 +54,17 @@ static int run_gemm(const Env& env, GemmParams p)
     if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return CCSD_OK;
     if (p.K <= 0) return p.accumulate ? CCSD_OK : CCSD_EINVAL;
     bool dmma_ok = dmma_supported(p);
-    if (env.gemm_mode == 2 && !dmma_ok) return CCSD_EINVAL;
-    bool use_dmma = (env.gemm_mode == 2) || (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p));
+    // gemm_mode: 0 auto, 1 simple FMA kernel, 2 DMMA 4M, 3 DMMA 3M, 100+v explicit DMMA variant v (tuning)
+    int variant = -1;
+    if (env.gemm_mode >= 100) variant = env.gemm_mode - 100;
+    else if (env.gemm_mode == 2) variant = dmma_pick(p.N, false);
+    else if (env.gemm_mode == 3) variant = dmma_pick(p.N, true);
+    else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p)) variant = dmma_pick(p.N, CCSD_DEFAULT_3M != 0);
+    if (variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
+    if (variant >= 0 && !dmma_ok) return CCSD_EINVAL;
+    const bool use_dmma = variant >= 0;
     // split-K chosen against wave quantisation on the 148 SMs: minimise  waves(ks) * (K/ks + pipeline overhead)
-    const int bm = use_dmma ? DMMA_BM : SG_BM, bn = use_dmma ? dmma_bn_for(p.N) : SG_BN;
+    const int bm = use_dmma ? k_dmma_variants[variant].bm : SG_BM, bn = use_dmma ? k_dmma_variants[variant].bn : SG_BN;
     const int64_t tiles = ((p.M + bm - 1) / bm) * ((p.N + bn - 1) / bn) * p.batch;
     p.ksplit = 1; p.kchunk = p.K; p.partial = nullptr;
     if (env.partial && p.K >= 512) {
@@ -82,7 +89,7 @@ static int run_gemm(const Env& env, GemmParams p)
         }
     }
     if (use_dmma) {
-        CCSD_TRY(launch_gemm_dmma(env.st, p));
+        CCSD_TRY(launch_gemm_dmma(env.st, p, variant));
     } else {
         dim3 grid((unsigned)((p.N + SG_BN - 1) / SG_BN), (unsigned)((p.M + SG_BM - 1) / SG_BM), (unsigned)(p.batch * p.ksplit));
         gemm_simple_kernel<<<grid, SG_T * SG_T, 0, env.st>>>(p);
@@ -1310,7 +1317,7 @@ int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t l
                   ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
                   void* cuda_stream)
 {
-    if (!A || !B || !C || M < 0 || N < 0 || K < 0 || mode < 0 || mode > 2) return CCSD_EINVAL;
+    if (!A || !B || !C || M < 0 || N < 0 || K < 0 || mode < 0 || (mode > 3 && mode < 100)) return CCSD_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");

@@ -20,11 +20,24 @@
 #include <cuda.h>
 #include "gemm_simple.cuh"
 
-constexpr int DMMA_BM = 128;        // CTA tile rows (A operand)
 constexpr int DMMA_BKG = 4;         // k-groups (of 4 complex) per pipeline stage -> BK = 16 complex
 constexpr int DMMA_STAGES = 4;
-constexpr int DMMA_CONSUMER_WARPS = 8;
-constexpr int DMMA_THREADS = (DMMA_CONSUMER_WARPS + 1) * 32;
+
+// Tile configuration.  NWM x NWN consumer warps; every warp owns MI x NJ fragment pairs.  An A fragment is 8 rows
+// x 4 complex k; a B fragment is 4 complex columns (4M: 8 real columns = re/im interleaved) or 8 complex columns (3M).
+template <int NWM_, int NWN_, int MI_, int NJ_, bool M3_>
+struct DmmaCfg {
+    static constexpr int NWM = NWM_, NWN = NWN_, MI = MI_, NJ = NJ_;
+    static constexpr bool M3 = M3_;
+    static constexpr int NB = M3_ ? 8 : 4;                       // complex columns per B fragment
+    static constexpr int BM = NWM_ * MI_ * 8, BN = NWN_ * NJ_ * NB;
+    static constexpr int WARPS = NWM_ * NWN_, THREADS = (WARPS + 1) * 32;
+    static constexpr int A_KG = BM * 64, B_KG = BN * 64;           // bytes per k-group
+    static constexpr int A_STAGE = DMMA_BKG * A_KG, B_STAGE = DMMA_BKG * B_KG, STAGE = A_STAGE + B_STAGE;
+    static constexpr int SMEM = DMMA_STAGES * STAGE + 2 * DMMA_STAGES * 8;
+    static_assert(BM <= 256 && BN <= 256, "TMA box dimension limit");
+    static_assert(SMEM <= 227 * 1024, "shared memory");
+};
 
 struct DmmaArgs {
     int64_t M, N, K;
@@ -71,22 +84,26 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
+// x with its sign bit XORed by `mask` (0 or 0x80000000): a negation on the integer pipe, so that the FP64 pipe
+// (shared by DMMA and DADD) sees nothing but DMMAs
+__device__ __forceinline__ double dsignflip(double x, unsigned mask)
+{
+    return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
 
-template <int NI>
-__global__ void __launch_bounds__(DMMA_THREADS, 1)
+template <class Cfg>
+__global__ void __launch_bounds__(Cfg::THREADS, 1)
 gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, DmmaArgs p)
 {
-    constexpr int BN = 8 * NI;
-    constexpr int A_KG = DMMA_BM * 64, B_KG = BN * 64;                 // bytes per k-group
-    constexpr int A_STAGE = DMMA_BKG * A_KG, B_STAGE = DMMA_BKG * B_KG;
-    constexpr int STAGE = A_STAGE + B_STAGE;
+    constexpr int MI = Cfg::MI, NJ = Cfg::NJ, NB = Cfg::NB;
+    constexpr int A_KG = Cfg::A_KG, B_KG = Cfg::B_KG, A_STAGE = Cfg::A_STAGE, STAGE = Cfg::STAGE;
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + DMMA_STAGES * STAGE);
     uint64_t* empty = full + DMMA_STAGES;
 
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int bz = blockIdx.z / p.ksplit, split = blockIdx.z % p.ksplit;
-    const int64_t m0 = (int64_t)blockIdx.y * DMMA_BM, n0 = (int64_t)blockIdx.x * BN;
+    const int64_t m0 = (int64_t)blockIdx.y * Cfg::BM, n0 = (int64_t)blockIdx.x * Cfg::BN;
     const int64_t kbeg = (int64_t)split * p.kchunk;
     const int64_t kend = (kbeg + p.kchunk < p.K) ? kbeg + p.kchunk : p.K;
     const int kt = (int)((kend - kbeg + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG));
@@ -94,13 +111,13 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     if (threadIdx.x == 0) {
         for (int s = 0; s < DMMA_STAGES; s++) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], DMMA_CONSUMER_WARPS);
+            mbar_init(&empty[s], Cfg::WARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (warp == DMMA_CONSUMER_WARPS) {
+    if (warp == Cfg::WARPS) {
         // ===== TMA producer =====
         if (lane == 0) {
             const int cA = p.batchA ? bz : 0, cB = p.batchB ? bz : 0;
@@ -122,61 +139,129 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         return;
     }
 
-    // ===== DMMA consumers: warp tile 32 rows x 4*NI complex columns =====
+    // ===== DMMA consumers: warp tile (8 MI) rows x (NB NJ) complex columns =====
     const int g = lane >> 2, q = lane & 3;
-    const int wm = warp & 3, wn = warp >> 2;
-    const bool odd = g & 1;
-    double acc[4][NI][2];
-#pragma unroll
-    for (int mi = 0; mi < 4; mi++)
-#pragma unroll
-        for (int nj = 0; nj < NI; nj++) { acc[mi][nj][0] = 0.0; acc[mi][nj][1] = 0.0; }
+    const int wm = warp % Cfg::NWM, wn = warp / Cfg::NWM;
+    const int a_off = (wm * MI * 8 + g) * 64 + q * 16;
 
-    const int a_off = (wm * 32 + g) * 64 + q * 16;
-    const int b_off = (wn * 4 * NI + (g >> 1)) * 64 + q * 16;
+    if constexpr (!Cfg::M3) {
+        // ---- 4M: two DMMAs per (A fragment, B fragment) pair; accumulator pair = (Re, Im) of one complex output ----
+        const bool odd = g & 1;
+        const unsigned negmask = odd ? 0u : 0x80000000u;
+        double acc[MI][NJ][2];
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++)
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++) { acc[mi][nj][0] = 0.0; acc[mi][nj][1] = 0.0; }
+        const int b_off = (wn * NJ * 4 + (g >> 1)) * 64 + q * 16;
 
-    for (int it = 0; it < kt; it++) {
-        const int s = it % DMMA_STAGES;
-        mbar_wait(&full[s], (it / DMMA_STAGES) & 1);
-        const unsigned char* sa = smem + s * STAGE + a_off;
-        const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off;
+        for (int it = 0; it < kt; it++) {
+            const int s = it % DMMA_STAGES;
+            mbar_wait(&full[s], (it / DMMA_STAGES) & 1);
+            const unsigned char* sa = smem + s * STAGE + a_off;
+            const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off;
 #pragma unroll
-        for (int kg = 0; kg < DMMA_BKG; kg++) {
-            double2 a[4];
+            for (int kg = 0; kg < DMMA_BKG; kg++) {
+                double2 a[MI];
 #pragma unroll
-            for (int mi = 0; mi < 4; mi++) a[mi] = *reinterpret_cast<const double2*>(sa + kg * A_KG + mi * 8 * 64);
+                for (int mi = 0; mi < MI; mi++) a[mi] = *reinterpret_cast<const double2*>(sa + kg * A_KG + mi * 8 * 64);
 #pragma unroll
-            for (int nj = 0; nj < NI; nj++) {
-                const double2 b = *reinterpret_cast<const double2*>(sb + kg * B_KG + nj * 4 * 64);
-                const double b1 = odd ? b.y : b.x;
-                const double b2 = odd ? b.x : -b.y;
+                for (int nj = 0; nj < NJ; nj++) {
+                    const double2 b = *reinterpret_cast<const double2*>(sb + kg * B_KG + nj * 4 * 64);
+                    const double b1 = odd ? b.y : b.x;                          // Re column: Re B, Im column: Im B
+                    const double b2 = dsignflip(odd ? b.x : b.y, negmask);      // Re column: -Im B, Im column: Re B
 #pragma unroll
-                for (int mi = 0; mi < 4; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].x, b1);
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].x, b1);
 #pragma unroll
-                for (int mi = 0; mi < 4; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].y, b2);
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].y, b2);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+
+        // epilogue: lane (g,q) owns C[m][n] = (acc[..][0], acc[..][1])
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++) {
+            const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
+            if (m >= p.M) continue;
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++) {
+                const int64_t n = n0 + wn * NJ * 4 + nj * 4 + q;
+                if (n >= p.N) continue;
+                c128 r = mk(acc[mi][nj][0], acc[mi][nj][1]);
+                if (p.ksplit > 1) {
+                    p.partial[((int64_t)blockIdx.z * p.M + m) * p.N + n] = r;
+                } else {
+                    c128* c = p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn;
+                    r = cmul(p.alpha, r);
+                    *c = p.accumulate ? cadd(*c, r) : r;
+                }
             }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[s]);
-    }
+    } else {
+        // ---- 3M (Karatsuba): three real products per complex MAC instead of four ----
+        //   P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi);   Re = P1 - P2,  Im = P3 - P1 - P2
+        // One DMMA each per (A fragment, B fragment) pair, the B fragment now spanning 8 complex columns: lane (g,q)
+        // feeds B[n0 + g][k0 + q] and owns, in each of the three accumulators, the outputs (row g, columns 2q, 2q+1).
+        double p1[MI][NJ][2], p2[MI][NJ][2], p3[MI][NJ][2];
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++)
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) { p1[mi][nj][e] = 0.0; p2[mi][nj][e] = 0.0; p3[mi][nj][e] = 0.0; }
+        const int b_off = (wn * NJ * 8 + g) * 64 + q * 16;
 
-    // ===== epilogue: lane (g,q) owns C[m][n] = (acc[..][0], acc[..][1]) =====
+        for (int it = 0; it < kt; it++) {
+            const int s = it % DMMA_STAGES;
+            mbar_wait(&full[s], (it / DMMA_STAGES) & 1);
+            const unsigned char* sa = smem + s * STAGE + a_off;
+            const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off;
 #pragma unroll
-    for (int mi = 0; mi < 4; mi++) {
-        const int64_t m = m0 + wm * 32 + mi * 8 + g;
-        if (m >= p.M) continue;
+            for (int kg = 0; kg < DMMA_BKG; kg++) {
+                double2 a[MI];
+                double as[MI];
 #pragma unroll
-        for (int nj = 0; nj < NI; nj++) {
-            const int64_t n = n0 + wn * 4 * NI + nj * 4 + q;
-            if (n >= p.N) continue;
-            c128 r = mk(acc[mi][nj][0], acc[mi][nj][1]);
-            if (p.ksplit > 1) {
-                p.partial[((int64_t)blockIdx.z * p.M + m) * p.N + n] = r;
-            } else {
-                c128* c = p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn;
-                r = cmul(p.alpha, r);
-                *c = p.accumulate ? cadd(*c, r) : r;
+                for (int mi = 0; mi < MI; mi++) {
+                    a[mi] = *reinterpret_cast<const double2*>(sa + kg * A_KG + mi * 8 * 64);
+                    as[mi] = a[mi].x + a[mi].y;
+                }
+#pragma unroll
+                for (int nj = 0; nj < NJ; nj++) {
+                    const double2 b = *reinterpret_cast<const double2*>(sb + kg * B_KG + nj * 8 * 64);
+                    const double bs = b.x + b.y;
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(p1[mi][nj][0], p1[mi][nj][1], a[mi].x, b.x);
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(p2[mi][nj][0], p2[mi][nj][1], a[mi].y, b.y);
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(p3[mi][nj][0], p3[mi][nj][1], as[mi], bs);
+                }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++) {
+            const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
+            if (m >= p.M) continue;
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int64_t n = n0 + wn * NJ * 8 + nj * 8 + 2 * q + e;
+                    if (n >= p.N) continue;
+                    c128 r = mk(p1[mi][nj][e] - p2[mi][nj][e], p3[mi][nj][e] - p1[mi][nj][e] - p2[mi][nj][e]);
+                    if (p.ksplit > 1) {
+                        p.partial[((int64_t)blockIdx.z * p.M + m) * p.N + n] = r;
+                    } else {
+                        c128* c = p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn;
+                        r = cmul(p.alpha, r);
+                        *c = p.accumulate ? cadd(*c, r) : r;
+                    }
+                }
         }
     }
 }
@@ -233,7 +318,7 @@ static inline bool dmma_supported(const GemmParams& p)
     if (p.sam * 16 >= (1LL << 40) || p.sbn * 16 >= (1LL << 40)) return false;
     if (p.batch > 1 && ((p.bsA != 0 && p.bsA * 16 >= (1LL << 40)) || (p.bsB != 0 && p.bsB * 16 >= (1LL << 40)))) return false;
     if ((reinterpret_cast<uintptr_t>(p.A) | reinterpret_cast<uintptr_t>(p.B)) & 15) return false;
-    if ((p.M + DMMA_BM - 1) / DMMA_BM > 65535) return false;
+    if ((p.M + 127) / 128 > 65535) return false;
     if ((int64_t)p.batch * 64 > 65535) return false;
     return true;
 }
@@ -241,39 +326,63 @@ static inline bool dmma_worthwhile(const GemmParams& p)
 {
     return (double)p.M * (double)p.N * (double)p.K * p.batch >= 2.0e5;
 }
-// column-tile width (complex) in {32,40,48,56,64} that wastes the fewest padded columns; ties -> wider
-static inline int dmma_bn_for(int64_t N)
-{
-    int best = 64;
-    int64_t bestpad = ((N + 63) / 64) * 64;
-    for (int bn = 56; bn >= 32; bn -= 8) {
-        int64_t pad = ((N + bn - 1) / bn) * bn;
-        if (pad < bestpad) { bestpad = pad; best = bn; }
-    }
-    return best;
-}
 
-template <int NI>
-static int launch_dmma_t(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const DmmaArgs& a, dim3 grid)
+template <class Cfg>
+static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const DmmaArgs& a, dim3 grid)
 {
-    constexpr int BN = 8 * NI;
-    constexpr int smem = DMMA_STAGES * DMMA_BKG * (DMMA_BM + BN) * 64 + 2 * DMMA_STAGES * 8;
     static bool configured = false;
     if (!configured) {
-        CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
         configured = true;
     }
-    gemm_dmma_kernel<NI><<<grid, DMMA_THREADS, smem, st>>>(mA, mB, a);
+    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mA, mB, a);
     g_launches++;
     return CCSD_OK;
 }
 
-static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p)
+// The kernel variants that are compiled.  Families: "4M" (variants 0-4) and "3M" (variants 5-7) are the two shipping
+// families, column-tile width chosen per launch; the rest are tuning variants reachable through gemm_mode >= 100.
+struct DmmaVariant {
+    int bm, bn;
+    bool m3;
+    int (*launch)(cudaStream_t, const CUtensorMap&, const CUtensorMap&, const DmmaArgs&, dim3);
+};
+#define DMMA_V(nwm, nwn, mi, nj, m3) \
+    {DmmaCfg<nwm, nwn, mi, nj, m3>::BM, DmmaCfg<nwm, nwn, mi, nj, m3>::BN, m3, &launch_dmma_cfg<DmmaCfg<nwm, nwn, mi, nj, m3>>}
+static const DmmaVariant k_dmma_variants[] = {
+    DMMA_V(4, 2, 4, 4, false), DMMA_V(4, 2, 4, 5, false), DMMA_V(4, 2, 4, 6, false), DMMA_V(4, 2, 4, 7, false),
+    DMMA_V(4, 2, 4, 8, false),                                       // 0-4: 4M, 128 x {32,40,48,56,64}, 8 warps
+    DMMA_V(4, 2, 4, 2, true), DMMA_V(4, 2, 4, 3, true), DMMA_V(4, 2, 4, 4, true),   // 5-7: 3M, 128 x {32,48,64}, 8 warps
+    DMMA_V(4, 4, 4, 4, false),                                       // 8: 4M 128 x 64, 16 warps
+    DMMA_V(4, 3, 4, 2, true),                                        // 9: 3M 128 x 48, 12 warps
+    DMMA_V(4, 3, 4, 5, false),                                       // 10: 4M 128 x 60, 12 warps
+};
+#undef DMMA_V
+constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_variants[0]));
+#ifndef CCSD_DEFAULT_3M
+#define CCSD_DEFAULT_3M 1
+#endif
+
+// variant of a family (3M or 4M) whose column-tile width wastes the fewest padded columns; ties -> wider
+static inline int dmma_pick(int64_t N, bool m3)
 {
-    const int bn = dmma_bn_for(p.N);
+    const int lo = m3 ? 5 : 0, hi = m3 ? 5 : 4;   // 3M: the 128 x 32 tile only (wider 3M tiles spill at 168 registers)
+    int best = hi;
+    int64_t bestpad = round_up(N, k_dmma_variants[hi].bn);
+    for (int v = hi - 1; v >= lo; v--) {
+        int64_t pad = round_up(N, k_dmma_variants[v].bn);
+        if (pad < bestpad) { bestpad = pad; best = v; }
+    }
+    return best;
+}
+
+static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
+{
+    if (variant < 0 || variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
+    const DmmaVariant& V = k_dmma_variants[variant];
     CUtensorMap mA, mB;
-    CCSD_TRY(make_operand_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, DMMA_BM));
-    CCSD_TRY(make_operand_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, bn));
+    CCSD_TRY(make_operand_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
+    CCSD_TRY(make_operand_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
     DmmaArgs a;
     a.M = p.M; a.N = p.N; a.K = p.K;
     a.C = p.C; a.csm = p.csm; a.csn = p.csn; a.bsC = p.bsC;
@@ -281,12 +390,6 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p)
     a.batchA = (p.batch > 1 && p.bsA != 0) ? 1 : 0;
     a.batchB = (p.batch > 1 && p.bsB != 0) ? 1 : 0;
     a.ksplit = p.ksplit; a.kchunk = p.kchunk; a.partial = p.partial;
-    dim3 grid((unsigned)((p.N + bn - 1) / bn), (unsigned)((p.M + DMMA_BM - 1) / DMMA_BM), (unsigned)(p.batch * p.ksplit));
-    switch (bn) {
-    case 32: return launch_dmma_t<4>(st, mA, mB, a, grid);
-    case 40: return launch_dmma_t<5>(st, mA, mB, a, grid);
-    case 48: return launch_dmma_t<6>(st, mA, mB, a, grid);
-    case 56: return launch_dmma_t<7>(st, mA, mB, a, grid);
-    default: return launch_dmma_t<8>(st, mA, mB, a, grid);
-    }
+    dim3 grid((unsigned)((p.N + V.bn - 1) / V.bn), (unsigned)((p.M + V.bm - 1) / V.bm), (unsigned)(p.batch * p.ksplit));
+    return V.launch(st, mA, mB, a, grid);
 }
