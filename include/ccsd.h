@@ -43,8 +43,10 @@ enum { CCSD_OK = 0, CCSD_EINVAL = 1, CCSD_ENOMEM = 2, CCSD_ECUDA = 3, CCSD_ESTAT
 typedef struct {
     int ndiis;          /* DIIS subspace size; 0 = plain Jacobi; default 6 (reading G13) */
     double level_shift; /* added to the virtual orbital energies in the denominators; default 0 */
-    int gemm_mode;      /* 0 = auto (FP64 tensor-core DMMA kernels where the shape allows), 1 = force the simple
-                           FP64-FMA kernels (on-device debugging reference) */
+    int gemm_mode;      /* 0 = auto (FP64 tensor-core DMMA kernels where the shape allows; complex arithmetic by the
+                           3M scheme, chosen by measurement), 1 = force the simple FP64-FMA kernels
+                           (on-device debugging reference), 2 = DMMA kernels with 4M complex arithmetic,
+                           3 = DMMA kernels with 3M; 100+v = one fixed tile variant v (tuning only) */
     int ccd;            /* 1 = CCD: t1 is kept at zero */
 } ccsd_options;
 
@@ -116,9 +118,14 @@ int ccsd_destroy(ccsd_ctx* ctx);
  *   CCSD_TERM_RING (eq 32 first line): in[0] = Hvovo [a][k][c][i], in[1] = t2 [(i<j)][(a<b)];
  *        out [(i<j)][(a<b)] = P-_ij P-_ab sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b]
  *   CCSD_TERM_TAU (eq 23): in[0] = t1 [i][a], in[1] = t2 [(i<j)][(a<b)]; out = tau packed
+ *   CCSD_TERM_PP_LADDER_PLANES: CCSD_TERM_PP_LADDER with the operands' 3M "sum planes" supplied by the caller, the way
+ *        ccsd_iterate runs it (the plane of the constant W is built once, by ccsd_init / ccsd_sum_plane):
+ *        in[2] = (double*) plane of tau [(i<j)][(c<d)], in[3] = (double*) plane of W [(a<b)][(c<d)], plane = Re + Im.
+ *        Same result as CCSD_TERM_PP_LADDER up to rounding.
  * accumulate != 0 adds into out.  workspace: ccsd_contract_workspace_bytes() bytes.  Asynchronous on the stream.
  */
-enum { CCSD_TERM_PP_LADDER = 0, CCSD_TERM_HH_LADDER = 1, CCSD_TERM_RING = 2, CCSD_TERM_TAU = 3 };
+enum { CCSD_TERM_PP_LADDER = 0, CCSD_TERM_HH_LADDER = 1, CCSD_TERM_RING = 2, CCSD_TERM_TAU = 3,
+       CCSD_TERM_PP_LADDER_PLANES = 4 };
 int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes);
 int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd_c128* out, int accumulate,
                   const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -126,11 +133,23 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd
 /*
  * Generic complex GEMM used by every contraction above ("NT" form, both operands K-contiguous):
  *   C[m*csm + n*csn] (+)= alpha * sum_k A[m*lda + k] * B[n*ldb + k]
- * mode: 0 auto, 1 simple FMA kernel, 2 force the DMMA tensor-core kernel (CCSD_EINVAL if K % 4 != 0).
+ * mode: as ccsd_options.gemm_mode (0 auto, 1 simple FMA kernel, 2 DMMA 4M, 3 DMMA 3M, 100+v tile variant v).
  */
 int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
                   ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
                   void* cuda_stream);
+
+/*
+ * 3M operand "sum plane": out[i] = Re in[i] + Im in[i], i < n.  The 3M complex GEMM (three real products per complex
+ * MAC: Ar Br, Ai Bi, (Ar + Ai)(Br + Bi)) reads these sums through TMA instead of forming them on the FP64 pipe.
+ */
+int ccsd_sum_plane(const ccsd_c128* in, double* out, int64_t n, void* cuda_stream);
+/* ccsd_zgemm_nt on the 3M kernels with the operands' sum planes As[m*lda + k], Bs[n*ldb + k] supplied (mode 0, 3 or
+ * 100+v).  The planes are used when lda and ldb are even and the planes 16-byte aligned (TMA rows); otherwise the
+ * kernel forms the sums itself.  Same result as ccsd_zgemm_nt up to rounding. */
+int ccsd_zgemm_nt_planes(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const double* As,
+                         const ccsd_c128* B, int64_t ldb, const double* Bs, ccsd_c128* C, int64_t csm, int64_t csn,
+                         double alpha_re, double alpha_im, int accumulate, int mode, void* cuda_stream);
 
 /*
  * Tensor transposition ("A(a,c,b,d)+=B(a,b,c,d)"):  out[permuted index] = in[index]
@@ -138,6 +157,11 @@ int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t l
  */
 int ccsd_transpose(const ccsd_c128* in, ccsd_c128* out, const int64_t dims[4], const int perm[4], int conj,
                    void* cuda_stream);
+
+/* Real flops the DMMA GEMM kernels EXECUTE per complex multiply-add under `opts` (NULL = defaults): 8 for the 4M
+ * scheme, 6 for 3M.  Algorithmic rates are always quoted on the 8-flop (ZGEMM) convention; the fraction of the FP64
+ * peak must be computed from the executed flops so that it cannot exceed 1. */
+int ccsd_real_flops_per_cmac(const ccsd_options* opts);
 
 /* Per-step device times (ms, CUDA events) of the last ccsd_iterate/ccsd_residual when timing was enabled. */
 enum { CCSD_NSTEPS = 16 };

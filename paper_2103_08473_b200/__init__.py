@@ -5,7 +5,7 @@ for device memory and streams.  There is no CPU fallback: without the built libr
 compute entry points raise.
 """
 from .binding import (CCSD, CCSDError, TENSOR_IDS, TERM_IDS, STEP_NAMES, contract, launch_count, lib_path, load_library,
-                      measure_fp64_peak, transpose, zgemm_nt)
+                      measure_fp64_peak, real_flops_per_cmac, sum_plane, transpose, zgemm_nt)
 
 __all__ = ["CCSD", "CCSDError", "TENSOR_IDS", "TERM_IDS", "STEP_NAMES", "contract", "launch_count", "lib_path",
-           "load_library", "measure_fp64_peak", "transpose", "zgemm_nt"]
+           "load_library", "measure_fp64_peak", "real_flops_per_cmac", "sum_plane", "transpose", "zgemm_nt"]

@@ -12,15 +12,15 @@ TENSOR_IDS = {"fock": 0, "vvvv": 1, "vovv": 2, "vovo": 3, "oovv": 4, "ooov": 5, 
               "Gvv": 12, "Hoo": 13, "Goo": 14, "Hov": 15, "Hvovo": 16, "C": 17, "A": 18, "S1": 19, "S2": 20,
               "S2_ring": 30, "S2_goo": 31, "S2_vdag_t1": 32, "S2_gvv": 33, "S2_c_t1": 34, "S2_hh_ladder": 35,
               "S2_pp_ladder": 36, "S2_driver": 37}
-TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3}
+TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3, "pp_ladder_planes": 4}
 NSTEPS = 16
 
 # every symbol include/ccsd.h declares
 EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_iterate", "ccsd_energy", "ccsd_residual",
            "ccsd_get_amplitudes", "ccsd_set_amplitudes", "ccsd_tensor_elems", "ccsd_get_tensor", "ccsd_destroy",
-           "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_transpose",
+           "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_zgemm_nt_planes", "ccsd_sum_plane", "ccsd_transpose",
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
-           "ccsd_measure_fp64_peak", "ccsd_strerror",
+           "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error"]
 
 
@@ -70,6 +70,9 @@ def load_library():
                                                             ctypes.POINTER(Options), vp, ctypes.c_size_t, vp]
         lib.ccsd_zgemm_nt.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
                                       ctypes.c_int, vp]
+        lib.ccsd_sum_plane.argtypes = [vp, vp, i64, vp]
+        lib.ccsd_zgemm_nt_planes.argtypes = [i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, i64, dbl, dbl, ctypes.c_int,
+                                             ctypes.c_int, vp]
         lib.ccsd_transpose.argtypes = [vp, vp, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_int), ctypes.c_int, vp]
         lib.ccsd_enable_step_timing.argtypes = [vp, ctypes.c_int]
         lib.ccsd_get_step_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -78,6 +81,7 @@ def load_library():
         lib.ccsd_launch_count.argtypes = [ctypes.c_int]
         lib.ccsd_launch_count.restype = ctypes.c_longlong
         lib.ccsd_measure_fp64_peak.argtypes = [ctypes.POINTER(dbl), vp, ctypes.c_int, vp]
+        lib.ccsd_real_flops_per_cmac.argtypes = [ctypes.POINTER(Options)]
         lib.ccsd_strerror.argtypes = [ctypes.c_int]
         lib.ccsd_strerror.restype = ctypes.c_char_p
         lib.ccsd_last_cuda_error.restype = ctypes.c_char_p
@@ -132,6 +136,12 @@ def _dev_c128(torch, x):
 
 def launch_count(reset: bool = False) -> int:
     return int(load_library().ccsd_launch_count(1 if reset else 0))
+
+
+def real_flops_per_cmac(gemm_mode: int = 0) -> int:
+    """8 (4M) or 6 (3M): real flops the DMMA GEMMs execute per complex multiply-add (ccsd_real_flops_per_cmac)."""
+    opts = _options(gemm_mode=gemm_mode)
+    return int(load_library().ccsd_real_flops_per_cmac(ctypes.byref(opts)))
 
 
 def measure_fp64_peak(launches: int = 10) -> float:
@@ -244,7 +254,8 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
     lib = load_library()
     tid = TERM_IDS[term]
     oo, vv = nocc * (nocc - 1) // 2, nvir * (nvir - 1) // 2
-    ins = [_dev_c128(torch, x) for x in inputs]
+    # the sum planes of "pp_ladder_planes" (inputs[2:]) are real float64 CUDA tensors made by sum_plane()
+    ins = [_dev_c128(torch, x) for x in inputs[:2]] + list(inputs[2:])
     if out is None:
         out = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
     nbytes = ctypes.c_size_t(0)
@@ -259,8 +270,10 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
     return out
 
 
-def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False):
-    """C[m][n] (+)= alpha * sum_k A[m][k] B[n][k]; transposed_out stores C as [n][m]."""
+def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False,
+             planes=None):
+    """C[m][n] (+)= alpha * sum_k A[m][k] B[n][k]; transposed_out stores C as [n][m].
+    planes = (As, Bs): float64 CUDA sum planes of A and B (sum_plane()) -> ccsd_zgemm_nt_planes."""
     torch = _torch()
     lib = load_library()
     A, B = _dev_c128(torch, A), _dev_c128(torch, B)
@@ -271,10 +284,28 @@ def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode:
         C = torch.zeros((N, M) if transposed_out else (M, N), dtype=torch.complex128, device="cuda")
     csm, csn = (1, M) if transposed_out else (N, 1)
     alpha = complex(alpha)
+    if planes is not None:
+        As, Bs = planes
+        assert As.shape == A.shape and Bs.shape == B.shape and As.dtype == torch.float64 and Bs.dtype == torch.float64
+        _check(lib.ccsd_zgemm_nt_planes(M, N, K, A.data_ptr(), K, As.data_ptr(), B.data_ptr(), K, Bs.data_ptr(),
+                                        C.data_ptr(), csm, csn, alpha.real, alpha.imag, int(accumulate), mode,
+                                        _stream_ptr(torch)), "ccsd_zgemm_nt_planes")
+        torch.cuda.current_stream().synchronize()
+        return C
     _check(lib.ccsd_zgemm_nt(M, N, K, A.data_ptr(), K, B.data_ptr(), K, C.data_ptr(), csm, csn, alpha.real, alpha.imag,
                              int(accumulate), mode, _stream_ptr(torch)), "ccsd_zgemm_nt")
     torch.cuda.current_stream().synchronize()
     return C
+
+
+def sum_plane(x):
+    """3M operand sum plane Re x + Im x of a complex128 CUDA tensor (ccsd_sum_plane); same shape, float64."""
+    torch = _torch()
+    lib = load_library()
+    x = _dev_c128(torch, x)
+    out = torch.empty(x.shape, dtype=torch.float64, device="cuda")
+    _check(lib.ccsd_sum_plane(x.data_ptr(), out.data_ptr(), x.numel(), _stream_ptr(torch)), "ccsd_sum_plane")
+    return out
 
 
 def transpose(x, perm, conj: bool = False):

@@ -49,6 +49,12 @@ static GemmParams gp(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
     return p;
 }
 
+static GemmParams with_planes(GemmParams p, const double* As, const double* Bs)
+{
+    p.As = As; p.Bs = Bs;
+    return p;
+}
+
 static int run_gemm(const Env& env, GemmParams p)
 {
     if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return CCSD_OK;
@@ -56,10 +62,14 @@ static int run_gemm(const Env& env, GemmParams p)
     bool dmma_ok = dmma_supported(p);
     // gemm_mode: 0 auto, 1 simple FMA kernel, 2 DMMA 4M, 3 DMMA 3M, 100+v explicit DMMA variant v (tuning)
     int variant = -1;
+    // sum planes are staged by TMA: 16-byte aligned rows, i.e. even leading dimensions
+    const bool planes_ok = p.As && p.Bs && p.sam % 2 == 0 && p.sbn % 2 == 0 && (p.batch == 1 || (p.bsA % 2 == 0 && p.bsB % 2 == 0)) &&
+                           ((reinterpret_cast<uintptr_t>(p.As) | reinterpret_cast<uintptr_t>(p.Bs)) & 15) == 0;
     if (env.gemm_mode >= 100) variant = env.gemm_mode - 100;
     else if (env.gemm_mode == 2) variant = dmma_pick(p.N, false);
-    else if (env.gemm_mode == 3) variant = dmma_pick(p.N, true);
-    else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p)) variant = dmma_pick(p.N, CCSD_DEFAULT_3M != 0);
+    else if (env.gemm_mode == 3) variant = dmma_pick(p.N, true, planes_ok);
+    else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p))
+        variant = dmma_pick(p.N, CCSD_DEFAULT_3M != 0, CCSD_DEFAULT_3M != 0 && planes_ok);
     if (variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
     if (variant >= 0 && !dmma_ok) return CCSD_EINVAL;
     const bool use_dmma = variant >= 0;
@@ -147,6 +157,9 @@ struct ccsd_ctx {
     c128 *Xr, *P, *Qm, *Rr, *Y, *Z;
     c128* partial;
     int64_t partial_elems;
+    // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
+    bool planes;
+    double *Ws, *Vvovv_ps, *Voovv_ps, *G1s, *taups, *Xms, *T2rs, *Hms;
     // DIIS
     c128 *diis_u, *diis_e;  // [ndiis][nvec]
     double* red;            // device reduction outputs (>= 16 doubles)
@@ -256,6 +269,18 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
     if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
     c->partial = w.take<c128>(c->partial_elems);
+    c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
+    c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
+    if (c->planes) {
+        c->Ws = w.take<double>(vv * vv);
+        c->Vvovv_ps = w.take<double>(ov * vv);
+        c->Voovv_ps = w.take<double>(oo * vv);
+        c->G1s = w.take<double>(ov * ov);
+        c->taups = w.take<double>(oo * vv);
+        c->Xms = w.take<double>(ov * ov);
+        c->T2rs = w.take<double>(ov * ov);
+        c->Hms = w.take<double>(ov * ov);
+    }
     c->nvec = ov + oo * vv;
     int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
     c->diis_u = w.take<c128>((int64_t)nd * c->nvec);
@@ -482,6 +507,12 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
             return csub(x, y);
         });
     }
+    if (c->planes) {   // sum planes of the constant operands of the large GEMMs (3M, gemm_dmma.cuh)
+        launch_sum_plane(st, c->W, c->Ws, vv * vv);
+        launch_sum_plane(st, c->Vvovv_p, c->Vvovv_ps, ov * vv);
+        launch_sum_plane(st, c->Voovv_p, c->Voovv_ps, oo * vv);
+        launch_sum_plane(st, c->G1, c->G1s, ov * ov);
+    }
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -520,8 +551,9 @@ static void tick(ccsd_ctx* c, int k)
 }
 
 // eq 23 on packed storage: tau = t2 + t1[i,a] t1[j,b] - t1[j,a] t1[i,b]
+// (plane != null: also its 3M sum plane, so that the two can never be out of step)
 static void build_tau(cudaStream_t st, c128* taup, const c128* t1, const c128* t2p, int o, int v, const int2* po,
-                      const int2* pv)
+                      const int2* pv, double* plane)
 {
     const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2;
     launch_fill(st, taup, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
@@ -529,7 +561,9 @@ static void build_tau(cudaStream_t st, c128* taup, const c128* t1, const c128* t
         c128 x = t2p[IJ * vv + AB];
         cfma(x, t1[ij.x * v + ab.x], t1[ij.y * v + ab.y]);
         c128 y = cmul(t1[ij.y * v + ab.x], t1[ij.x * v + ab.y]);
-        return csub(x, y);
+        x = csub(x, y);
+        if (plane) plane[IJ * vv + AB] = x.x + x.y;
+        return x;
     });
 }
 
@@ -540,7 +574,8 @@ static int prep_operands(ccsd_ctx* c)
     const int64_t oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
     const int2 *po = c->po, *pv = c->pv;
     const c128 *t1 = c->t1, *t2p = c->t2p, *taup = c->taup;
-    build_tau(st, c->taup, t1, t2p, o, v, po, pv);
+    build_tau(st, c->taup, t1, t2p, o, v, po, pv, c->taups);
+    double *Xms = c->Xms, *T2rs = c->T2rs;
     launch_fill(st, c->t1T, v, o, o, 0, [=] __device__(int64_t a, int64_t i) { return t1[i * v + a]; });
     // TT[(a<b)][0:oo) = tau^T, TT[(a<b)][oop:oop+oo) = t2^T   (K-contiguous operands of the hh-ladder and Goo terms)
     CCSD_TRY(launch_transpose2d_ld(st, c->taup, vv, c->TT, 2 * oop, oo, vv, 0));
@@ -550,12 +585,15 @@ static int prep_operands(ccsd_ctx* c)
         int a = ai / o, i = ai % o, l = ld / v, d = ld % v;
         c128 x = cscale(0.5, t2_at(t2p, l, i, a, d, o, v, vv));
         cfma(x, t1[l * v + a], t1[i * v + d]);
+        if (Xms) Xms[ai * ov + ld] = x.x + x.y;
         return x;
     });
     // T2r[(j,b)][(c,k)] = t2[j,k,c,b]                            (eq 32 ring operand)
     launch_fill(st, c->T2r, ov, ov, ov, 0, [=] __device__(int64_t jb, int64_t ck) {
         int j = jb / v, b = jb % v, cc = ck / o, k = ck % o;
-        return t2_at(t2p, j, k, cc, b, o, v, vv);
+        c128 x = t2_at(t2p, j, k, cc, b, o, v, vv);
+        if (T2rs) T2rs[jb * ov + ck] = x.x + x.y;
+        return x;
     });
     // tauc[a][(k<l, d)] = tau[k,l,d,a]
     launch_fill(st, c->tauc, v, oo * v, oo * v, 0, [=] __device__(int64_t a, int64_t col) {
@@ -628,7 +666,8 @@ static int build_Hvovo(ccsd_ctx* c)
     CCSD_TRY(run_gemm(env, gp(v, (int64_t)o * ov, o, c->t1T, o, c->Vooov_b, o, c->Hm, (int64_t)o * ov, 1, -1.0, 1)));
     tick(c, 3);
     // + sum_{ld} <kl||cd> (1/2 t2[l,i,a,d] + t1[l,a] t1[i,d])       (ov x ov x ov)
-    CCSD_TRY(run_gemm(env, gp(ov, ov, ov, c->Xm, ov, c->G1, ov, c->Hm, ov, 1, 1.0, 1)));
+    CCSD_TRY(run_gemm(env, with_planes(gp(ov, ov, ov, c->Xm, ov, c->G1, ov, c->Hm, ov, 1, 1.0, 1), c->Xms, c->G1s)));
+    if (c->planes) launch_sum_plane(c->st, c->Hm, c->Hms, ov * ov);   // operand of the ring GEMM
     return CCSD_OK;
 }
 
@@ -647,7 +686,7 @@ static int build_C(ccsd_ctx* c)
         int2 ij = po[IJ];
         return csub(Y[(bk * o + ij.x) * o + ij.y], Y[(bk * o + ij.y) * o + ij.x]);
     });
-    CCSD_TRY(run_gemm(env, gp(ov, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1)));
+    CCSD_TRY(run_gemm(env, with_planes(gp(ov, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), c->Vvovv_ps, c->taups)));
     return CCSD_OK;
 }
 
@@ -666,7 +705,7 @@ static int build_A(ccsd_ctx* c)
         int2 ij = po[IJ];
         return csub(Z[(KL * o + ij.x) * o + ij.y], Z[(KL * o + ij.y) * o + ij.x]);
     });
-    CCSD_TRY(run_gemm(env, gp(oo, oo, vv, c->Voovv_p, vv, c->taup, vv, c->Am, oo, 1, 1.0, 1)));
+    CCSD_TRY(run_gemm(env, with_planes(gp(oo, oo, vv, c->Voovv_p, vv, c->taup, vv, c->Am, oo, 1, 1.0, 1), c->Voovv_ps, c->taups)));
     return CCSD_OK;
 }
 
@@ -680,7 +719,7 @@ static int s2_driver(ccsd_ctx* c, c128* S)
 }
 static int s2_pp_ladder(ccsd_ctx* c, c128* S)
 {   // sum_{c<d} <ab||cd> tau[i,j,c,d]      M = (a<b), N = (i<j), K = (c<d)
-    return run_gemm(c->env, gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1));
+    return run_gemm(c->env, with_planes(gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
 static void fill_AG_hh(ccsd_ctx* c)
 {   // AG[(i<j)][(k<l)] = A[k,l,i,j]
@@ -724,7 +763,7 @@ static int s2_ring(ccsd_ctx* c, c128* S)
 {   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)];  S += P-_ij P-_ab X
     const int o = c->o, v = c->v;
     const int64_t ov = c->ov, vv = c->vv;
-    CCSD_TRY(run_gemm(c->env, gp(ov, ov, ov, c->Hm, ov, c->T2r, ov, c->Xr, ov, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(c->env, with_planes(gp(ov, ov, ov, c->Hm, ov, c->T2r, ov, c->Xr, ov, 1, 1.0, 0), c->Hms, c->T2rs)));
     tick(c, 9);
     const c128* Xr = c->Xr;
     const int2 *po = c->po, *pv = c->pv;
@@ -858,7 +897,7 @@ static int residual(ccsd_ctx* c)
 // ---------------------------------------------------------------------------------------------------------------
 static int energy_async(ccsd_ctx* c, double* red_out /* device, 2 doubles */)
 {
-    build_tau(c->st, c->taup, c->t1, c->t2p, c->o, c->v, c->po, c->pv);
+    build_tau(c->st, c->taup, c->t1, c->t2p, c->o, c->v, c->po, c->pv, c->taups);
     CCSD_CUDA_TRY(cudaMemsetAsync(red_out, 0, 2 * sizeof(double), c->st));
     // E = sum_ia f[i,a] t1[i,a] + sum_{i<j,a<b} <ij||ab> tau   (eq 9; reading G11)
     launch_energy(c->st, c->f, c->n, c->o, c->v, c->t1, c->Voovv_p, c->taup, c->oo * c->vv, red_out);
@@ -1218,6 +1257,7 @@ int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
     w.take<int2>(oo); w.take<int2>(vv);
     switch (term) {
     case CCSD_TERM_PP_LADDER: break;
+    case CCSD_TERM_PP_LADDER_PLANES: break;
     case CCSD_TERM_TAU: break;
     case CCSD_TERM_HH_LADDER: w.take<c128>(vv * oop); w.take<c128>(oo * oop); break;
     case CCSD_TERM_RING: w.take<c128>(ov * ov); w.take<c128>(ov * ov); w.take<c128>(ov * ov); break;
@@ -1263,12 +1303,18 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
     case CCSD_TERM_PP_LADDER:
         // out[(i<j)][(a<b)] (+)= sum_{c<d} W[(a<b)][(c<d)] tau[(i<j)][(c<d)]
         return run_gemm(env, gp(vv, oo, vv, in1, vv, in0, vv, out, 1, vv, 1.0, accumulate));
+    case CCSD_TERM_PP_LADDER_PLANES: {
+        const double* taus = reinterpret_cast<const double*>(in_[2]);
+        const double* Ws = reinterpret_cast<const double*>(in_[3]);
+        if (!taus || !Ws) return CCSD_EINVAL;
+        return run_gemm(env, with_planes(gp(vv, oo, vv, in1, vv, in0, vv, out, 1, vv, 1.0, accumulate), Ws, taus));
+    }
     case CCSD_TERM_TAU: {
         pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(po, o);
         pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(pv, v);
         g_launches += 2;
         if (accumulate) return CCSD_EINVAL;
-        build_tau(st, out, in0, in1, o, v, po, pv);
+        build_tau(st, out, in0, in1, o, v, po, pv, nullptr);
         CCSD_CUDA_TRY(cudaGetLastError());
         return CCSD_OK;
     }
@@ -1330,6 +1376,37 @@ int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t l
     return run_gemm(env, p);
 }
 
+int ccsd_zgemm_nt_planes(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const double* As,
+                         const ccsd_c128* B, int64_t ldb, const double* Bs, ccsd_c128* C, int64_t csm, int64_t csn,
+                         double alpha_re, double alpha_im, int accumulate, int mode, void* cuda_stream)
+{
+    if (!A || !B || !C || !As || !Bs || M < 0 || N < 0 || K < 0) return CCSD_EINVAL;
+    if (!(mode == 0 || mode == 3 || mode >= 100)) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    Env env{static_cast<cudaStream_t>(cuda_stream), mode, nullptr, 0};
+    GemmParams p = gp(M, N, K, reinterpret_cast<const c128*>(A), lda, reinterpret_cast<const c128*>(B), ldb,
+                      reinterpret_cast<c128*>(C), csm, csn, 1.0, accumulate);
+    p.alpha = mk(alpha_re, alpha_im);
+    return run_gemm(env, with_planes(p, As, Bs));
+}
+
+int ccsd_sum_plane(const ccsd_c128* in, double* out, int64_t n, void* cuda_stream)
+{
+    if (!in || !out || n < 0) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    launch_sum_plane(static_cast<cudaStream_t>(cuda_stream), reinterpret_cast<const c128*>(in), out, n);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
 int ccsd_transpose(const ccsd_c128* in, ccsd_c128* out, const int64_t dims[4], const int perm[4], int conj, void* cuda_stream)
 {
     if (!in || !out || !dims || !perm) return CCSD_EINVAL;
@@ -1367,6 +1444,14 @@ int ccsd_measure_fp64_peak(double* tflops, double* device_scratch, int launches,
         return CCSD_ECUDA;
     }
     return measure_fp64_peak(static_cast<cudaStream_t>(cuda_stream), device_scratch, launches, tflops);
+}
+
+int ccsd_real_flops_per_cmac(const ccsd_options* opts)
+{
+    const int mode = opts ? opts->gemm_mode : 0;
+    if (mode >= 100 && mode - 100 < DMMA_NVARIANTS) return k_dmma_variants[mode - 100].m3 ? 6 : 8;
+    if (mode == 3 || (mode == 0 && CCSD_DEFAULT_3M != 0)) return 6;
+    return 8;
 }
 
 const char* ccsd_step_name(int step) { return (step >= 0 && step < CCSD_NSTEPS) ? k_step_names[step] : ""; }

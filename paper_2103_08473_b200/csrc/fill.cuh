@@ -35,6 +35,31 @@ static inline void launch_fill(cudaStream_t st, c128* out, int64_t rows, int64_t
     g_launches++;
 }
 
+// 3M "sum plane" of a complex buffer: out[i] = Re in[i] + Im in[i]  (gemm_dmma.cuh, DmmaCfg::PL).  Streaming:
+// 32 bytes read + 16 bytes written per thread and step.
+__global__ void __launch_bounds__(256) sum_plane_kernel(const c128* __restrict__ in, double* __restrict__ out, int64_t n)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x * 2;
+    for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n; i += stride) {
+        if (i + 1 < n) {
+            const c128 x = in[i], y = in[i + 1];
+            *reinterpret_cast<double2*>(out + i) = make_double2(x.x + x.y, y.x + y.y);
+        } else {
+            const c128 x = in[i];
+            out[i] = x.x + x.y;
+        }
+    }
+}
+static inline void launch_sum_plane(cudaStream_t st, const c128* in, double* out, int64_t n)
+{
+    if (n <= 0) return;
+    int64_t blocks = (n / 2 + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks < 1) blocks = 1;
+    sum_plane_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, n);
+    g_launches++;
+}
+
 // pair table: tab[p] = (x, y) with x<y, p = pair_idx(x, y, m)
 __global__ void pair_table_kernel(int2* tab, int m)
 {

@@ -21,21 +21,31 @@
 #include "gemm_simple.cuh"
 
 constexpr int DMMA_BKG = 4;         // k-groups (of 4 complex) per pipeline stage -> BK = 16 complex
-constexpr int DMMA_STAGES = 4;
 
-// Tile configuration.  NWM x NWN consumer warps; every warp owns MI x NJ fragment pairs.  An A fragment is 8 rows
-// x 4 complex k; a B fragment is 4 complex columns (4M: 8 real columns = re/im interleaved) or 8 complex columns (3M).
-template <int NWM_, int NWN_, int MI_, int NJ_, bool M3_>
+// Tile configuration.  NWM x NWN warps, all of them DMMA consumers (no dedicated producer warp: with 8 warps = 2 per
+// SM sub-partition every thread may use 255 registers; a ninth warp would cap them at 168).  Every warp owns MI x NJ
+// fragment pairs.  An A fragment is 8 rows x 4 complex k; a B fragment is 4 complex columns (4M: 8 real columns =
+// re/im interleaved) or 8 complex columns (3M).
+// PL (3M only): the sums Ar + Ai / Br + Bi come from precomputed real "sum planes" (TMA-staged beside the complex
+// tiles) instead of DADDs in the main loop: DADD shares the FP64 pipe with DMMA and every DADD between DMMAs costs
+// far more than its two issue cycles (measured: 5 % of the kernel).
+template <int NWM_, int NWN_, int MI_, int NJ_, bool M3_, bool PL_ = false>
 struct DmmaCfg {
     static constexpr int NWM = NWM_, NWN = NWN_, MI = MI_, NJ = NJ_;
-    static constexpr bool M3 = M3_;
+    static constexpr bool M3 = M3_, PL = PL_;
+    static_assert(!PL_ || M3_, "sum planes belong to the 3M scheme");
     static constexpr int NB = M3_ ? 8 : 4;                       // complex columns per B fragment
     static constexpr int BM = NWM_ * MI_ * 8, BN = NWN_ * NJ_ * NB;
-    static constexpr int WARPS = NWM_ * NWN_, THREADS = (WARPS + 1) * 32;
-    static constexpr int A_KG = BM * 64, B_KG = BN * 64;           // bytes per k-group
-    static constexpr int A_STAGE = DMMA_BKG * A_KG, B_STAGE = DMMA_BKG * B_KG, STAGE = A_STAGE + B_STAGE;
-    static constexpr int SMEM = DMMA_STAGES * STAGE + 2 * DMMA_STAGES * 8;
+    static constexpr int WARPS = NWM_ * NWN_, THREADS = WARPS * 32;
+    static constexpr int A_KG = BM * 64, B_KG = BN * 64;           // bytes per k-group (complex tiles)
+    static constexpr int AS_KG = BM * 32, BS_KG = BN * 32;         // bytes per k-group (sum planes)
+    static constexpr int A_STAGE = DMMA_BKG * A_KG, B_STAGE = DMMA_BKG * B_KG;
+    static constexpr int P_STAGE = PL_ ? DMMA_BKG * (AS_KG + BS_KG) : 0;
+    static constexpr int STAGE = A_STAGE + B_STAGE + P_STAGE;
+    static constexpr int STAGES = (220 * 1024 / STAGE) > 6 ? 6 : (220 * 1024 / STAGE);
+    static constexpr int SMEM = STAGES * STAGE + 2 * STAGES * 8;
     static_assert(BM <= 256 && BN <= 256, "TMA box dimension limit");
+    static_assert(STAGES >= 3, "pipeline needs >= 3 stages");
     static_assert(SMEM <= 227 * 1024, "shared memory");
 };
 
@@ -93,13 +103,14 @@ __device__ __forceinline__ double dsignflip(double x, unsigned mask)
 
 template <class Cfg>
 __global__ void __launch_bounds__(Cfg::THREADS, 1)
-gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, DmmaArgs p)
+gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                 const __grid_constant__ CUtensorMap mapAs, const __grid_constant__ CUtensorMap mapBs, DmmaArgs p)
 {
-    constexpr int MI = Cfg::MI, NJ = Cfg::NJ, NB = Cfg::NB;
+    constexpr int MI = Cfg::MI, NJ = Cfg::NJ, S = Cfg::STAGES, D = Cfg::STAGES - 2;
     constexpr int A_KG = Cfg::A_KG, B_KG = Cfg::B_KG, A_STAGE = Cfg::A_STAGE, STAGE = Cfg::STAGE;
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem + DMMA_STAGES * STAGE);
-    uint64_t* empty = full + DMMA_STAGES;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + S * STAGE);
+    uint64_t* empty = full + S;
 
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int bz = blockIdx.z / p.ksplit, split = blockIdx.z % p.ksplit;
@@ -107,89 +118,162 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     const int64_t kbeg = (int64_t)split * p.kchunk;
     const int64_t kend = (kbeg + p.kchunk < p.K) ? kbeg + p.kchunk : p.K;
     const int kt = (int)((kend - kbeg + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG));
+    const int cA = p.batchA ? bz : 0, cB = p.batchB ? bz : 0;
+
+    // TMA for k-iteration L into stage L % S (one elected lane).  It is issued D = S - 2 iterations ahead, so the
+    // stage it overwrites was released by every warp at least one whole iteration ago: the wait never spins long.
+    auto issue = [&](int L) {
+        const int s = L % S;
+        if (L >= S) mbar_wait(&empty[s], ((L / S) & 1) ^ 1);
+        mbar_expect_tx(&full[s], STAGE);
+        unsigned char* sa = smem + s * STAGE;
+        unsigned char* sb = sa + A_STAGE;
+        const int64_t k0 = kbeg + (int64_t)L * 4 * DMMA_BKG;
+#pragma unroll
+        for (int kg = 0; kg < DMMA_BKG; kg++) {
+            const int cd = (int)((k0 + 4 * kg) * 2);   // coordinate in doubles
+            tma_load_3d(sa + kg * A_KG, &mapA, cd, (int)m0, cA, &full[s]);
+            tma_load_3d(sb + kg * B_KG, &mapB, cd, (int)n0, cB, &full[s]);
+            if constexpr (Cfg::PL) {
+                unsigned char* sp = sb + Cfg::B_STAGE;
+                tma_load_3d(sp + kg * Cfg::AS_KG, &mapAs, cd / 2, (int)m0, cA, &full[s]);
+                tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, &mapBs, cd / 2, (int)n0, cB, &full[s]);
+            }
+        }
+    };
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < DMMA_STAGES; s++) {
+        for (int s = 0; s < S; s++) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], Cfg::WARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    if (threadIdx.x == 0)
+        for (int L = 0; L < D && L < kt; L++) issue(L);
 
-    if (warp == Cfg::WARPS) {
-        // ===== TMA producer =====
-        if (lane == 0) {
-            const int cA = p.batchA ? bz : 0, cB = p.batchB ? bz : 0;
-            for (int it = 0; it < kt; it++) {
-                const int s = it % DMMA_STAGES;
-                if (it >= DMMA_STAGES) mbar_wait(&empty[s], ((it / DMMA_STAGES) & 1) ^ 1);
-                mbar_expect_tx(&full[s], STAGE);
-                unsigned char* sa = smem + s * STAGE;
-                unsigned char* sb = sa + A_STAGE;
-                const int64_t k0 = kbeg + (int64_t)it * 4 * DMMA_BKG;
-#pragma unroll
-                for (int kg = 0; kg < DMMA_BKG; kg++) {
-                    const int cd = (int)((k0 + 4 * kg) * 2);   // coordinate in doubles
-                    tma_load_3d(sa + kg * A_KG, &mapA, cd, (int)m0, cA, &full[s]);
-                    tma_load_3d(sb + kg * B_KG, &mapB, cd, (int)n0, cB, &full[s]);
-                }
-            }
-        }
-        return;
-    }
-
-    // ===== DMMA consumers: warp tile (8 MI) rows x (NB NJ) complex columns =====
+    // warp tile (8 MI) rows x (NB NJ) complex columns; lane (g,q) loads ONE complex A element per A fragment and ONE
+    // complex B element per B fragment and k-group.  Fragment loads run one k-group ahead of the DMMAs (also across
+    // stage boundaries), so neither the shared-memory latency nor the barrier wait is exposed.
     const int g = lane >> 2, q = lane & 3;
     const int wm = warp % Cfg::NWM, wn = warp / Cfg::NWM;
     const int a_off = (wm * MI * 8 + g) * 64 + q * 16;
+    const int b_off = Cfg::M3 ? (wn * NJ * 8 + g) * 64 + q * 16 : (wn * NJ * 4 + (g >> 1)) * 64 + q * 16;
+    constexpr int B_ROWS = Cfg::M3 ? 8 : 4;   // rows of the B tile per B fragment
 
-    if constexpr (!Cfg::M3) {
-        // ---- 4M: two DMMAs per (A fragment, B fragment) pair; accumulator pair = (Re, Im) of one complex output ----
-        const bool odd = g & 1;
-        const unsigned negmask = odd ? 0u : 0x80000000u;
-        double acc[MI][NJ][2];
+    double2 an[MI], bn[NJ];
+    double asn[Cfg::PL ? MI : 1], bsn[Cfg::PL ? NJ : 1];
+    const int as_off = (wm * MI * 8 + g) * 32 + q * 8, bs_off = (wn * NJ * 8 + g) * 32 + q * 8;
+    auto load_frags = [&](int s, int kg) {
+        const unsigned char* sa = smem + s * STAGE + a_off + kg * A_KG;
+        const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off + kg * B_KG;
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++) an[mi] = *reinterpret_cast<const double2*>(sa + mi * 8 * 64);
+#pragma unroll
+        for (int nj = 0; nj < NJ; nj++) bn[nj] = *reinterpret_cast<const double2*>(sb + nj * B_ROWS * 64);
+        if constexpr (Cfg::PL) {
+            const unsigned char* sp = smem + s * STAGE + A_STAGE + Cfg::B_STAGE;
+            const unsigned char* sas = sp + as_off + kg * Cfg::AS_KG;
+            const unsigned char* sbs = sp + DMMA_BKG * Cfg::AS_KG + bs_off + kg * Cfg::BS_KG;
+#pragma unroll
+            for (int mi = 0; mi < MI; mi++) asn[mi] = *reinterpret_cast<const double*>(sas + mi * 8 * 32);
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++) bsn[nj] = *reinterpret_cast<const double*>(sbs + nj * 8 * 32);
+        }
+    };
+
+    // accumulators: 4M: (Re, Im) of C[row g][col q] per fragment pair;  3M: P1, P2, P3 of C[row g][cols 2q, 2q+1]
+    constexpr int NACC = Cfg::M3 ? 3 : 1;
+    double acc[NACC][MI][NJ][2];
+#pragma unroll
+    for (int t = 0; t < NACC; t++)
 #pragma unroll
         for (int mi = 0; mi < MI; mi++)
 #pragma unroll
-            for (int nj = 0; nj < NJ; nj++) { acc[mi][nj][0] = 0.0; acc[mi][nj][1] = 0.0; }
-        const int b_off = (wn * NJ * 4 + (g >> 1)) * 64 + q * 16;
+            for (int nj = 0; nj < NJ; nj++) { acc[t][mi][nj][0] = 0.0; acc[t][mi][nj][1] = 0.0; }
+    const bool odd = g & 1;
+    const unsigned negmask = odd ? 0u : 0x80000000u;
 
-        for (int it = 0; it < kt; it++) {
-            const int s = it % DMMA_STAGES;
-            mbar_wait(&full[s], (it / DMMA_STAGES) & 1);
-            const unsigned char* sa = smem + s * STAGE + a_off;
-            const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off;
+    if (kt > 0) {
+        mbar_wait(&full[0], 0);
+        load_frags(0, 0);
+    }
+    for (int it = 0; it < kt; it++) {
+        const int s = it % S;
+        if (it + D < kt && warp == it % Cfg::WARPS) {      // producer duty rotates over the warps
+            if (lane == 0) issue(it + D);
+            __syncwarp();
+        }
 #pragma unroll
-            for (int kg = 0; kg < DMMA_BKG; kg++) {
-                double2 a[MI];
+        for (int kg = 0; kg < DMMA_BKG; kg++) {
+            double2 a[MI], b[NJ];
+            double as[MI], bs[NJ];
 #pragma unroll
-                for (int mi = 0; mi < MI; mi++) a[mi] = *reinterpret_cast<const double2*>(sa + kg * A_KG + mi * 8 * 64);
+            for (int mi = 0; mi < MI; mi++) { a[mi] = an[mi]; if constexpr (Cfg::PL) as[mi] = asn[mi]; }
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++) { b[nj] = bn[nj]; if constexpr (Cfg::PL) bs[nj] = bsn[nj]; }
+            if (kg + 1 < DMMA_BKG) {
+                load_frags(s, kg + 1);
+            } else if (it + 1 < kt) {
+                mbar_wait(&full[(it + 1) % S], ((it + 1) / S) & 1);
+                load_frags((it + 1) % S, 0);
+            }
+            if constexpr (!Cfg::M3) {
+                // 4M: DMMA #1 (Re A) x (Re column: Re B | Im column: Im B); DMMA #2 (Im A) x (-Im B | Re B)
 #pragma unroll
                 for (int nj = 0; nj < NJ; nj++) {
-                    const double2 b = *reinterpret_cast<const double2*>(sb + kg * B_KG + nj * 4 * 64);
-                    const double b1 = odd ? b.y : b.x;                          // Re column: Re B, Im column: Im B
-                    const double b2 = dsignflip(odd ? b.x : b.y, negmask);      // Re column: -Im B, Im column: Re B
+                    const double b1 = odd ? b[nj].y : b[nj].x;
+                    const double b2 = dsignflip(odd ? b[nj].x : b[nj].y, negmask);
 #pragma unroll
-                    for (int mi = 0; mi < MI; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].x, b1);
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[0][mi][nj][0], acc[0][mi][nj][1], a[mi].x, b1);
 #pragma unroll
-                    for (int mi = 0; mi < MI; mi++) dmma884(acc[mi][nj][0], acc[mi][nj][1], a[mi].y, b2);
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[0][mi][nj][0], acc[0][mi][nj][1], a[mi].y, b2);
+                }
+            } else {
+                // 3M (Karatsuba): P1 = Ar Br, P2 = Ai Bi, P3 = (Ar + Ai)(Br + Bi); Re = P1 - P2, Im = P3 - P1 - P2
+                if constexpr (!Cfg::PL) {
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) as[mi] = a[mi].x + a[mi].y;
+#pragma unroll
+                    for (int nj = 0; nj < NJ; nj++) bs[nj] = b[nj].x + b[nj].y;
+                }
+#pragma unroll
+                for (int nj = 0; nj < NJ; nj++) {
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[0][mi][nj][0], acc[0][mi][nj][1], a[mi].x, b[nj].x);
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[1][mi][nj][0], acc[1][mi][nj][1], a[mi].y, b[nj].y);
+#pragma unroll
+                    for (int mi = 0; mi < MI; mi++) dmma884(acc[2][mi][nj][0], acc[2][mi][nj][1], as[mi], bs[nj]);
                 }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);
+    }
 
-        // epilogue: lane (g,q) owns C[m][n] = (acc[..][0], acc[..][1])
+    // ===== epilogue =====
+    constexpr int NE = Cfg::M3 ? 2 : 1;
 #pragma unroll
-        for (int mi = 0; mi < MI; mi++) {
-            const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
-            if (m >= p.M) continue;
+    for (int mi = 0; mi < MI; mi++) {
+        const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
+        if (m >= p.M) continue;
 #pragma unroll
-            for (int nj = 0; nj < NJ; nj++) {
-                const int64_t n = n0 + wn * NJ * 4 + nj * 4 + q;
+        for (int nj = 0; nj < NJ; nj++)
+#pragma unroll
+            for (int e = 0; e < NE; e++) {
+                int64_t n;
+                c128 r;
+                if constexpr (Cfg::M3) {
+                    n = n0 + wn * NJ * 8 + nj * 8 + 2 * q + e;
+                    r = mk(acc[0][mi][nj][e] - acc[NACC - 2][mi][nj][e],
+                           acc[NACC - 1][mi][nj][e] - acc[0][mi][nj][e] - acc[NACC - 2][mi][nj][e]);
+                } else {
+                    n = n0 + wn * NJ * 4 + nj * 4 + q;
+                    r = mk(acc[0][mi][nj][0], acc[0][mi][nj][1]);
+                }
                 if (n >= p.N) continue;
-                c128 r = mk(acc[mi][nj][0], acc[mi][nj][1]);
                 if (p.ksplit > 1) {
                     p.partial[((int64_t)blockIdx.z * p.M + m) * p.N + n] = r;
                 } else {
@@ -198,71 +282,6 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                     *c = p.accumulate ? cadd(*c, r) : r;
                 }
             }
-        }
-    } else {
-        // ---- 3M (Karatsuba): three real products per complex MAC instead of four ----
-        //   P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi);   Re = P1 - P2,  Im = P3 - P1 - P2
-        // One DMMA each per (A fragment, B fragment) pair, the B fragment now spanning 8 complex columns: lane (g,q)
-        // feeds B[n0 + g][k0 + q] and owns, in each of the three accumulators, the outputs (row g, columns 2q, 2q+1).
-        double p1[MI][NJ][2], p2[MI][NJ][2], p3[MI][NJ][2];
-#pragma unroll
-        for (int mi = 0; mi < MI; mi++)
-#pragma unroll
-            for (int nj = 0; nj < NJ; nj++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) { p1[mi][nj][e] = 0.0; p2[mi][nj][e] = 0.0; p3[mi][nj][e] = 0.0; }
-        const int b_off = (wn * NJ * 8 + g) * 64 + q * 16;
-
-        for (int it = 0; it < kt; it++) {
-            const int s = it % DMMA_STAGES;
-            mbar_wait(&full[s], (it / DMMA_STAGES) & 1);
-            const unsigned char* sa = smem + s * STAGE + a_off;
-            const unsigned char* sb = smem + s * STAGE + A_STAGE + b_off;
-#pragma unroll
-            for (int kg = 0; kg < DMMA_BKG; kg++) {
-                double2 a[MI];
-                double as[MI];
-#pragma unroll
-                for (int mi = 0; mi < MI; mi++) {
-                    a[mi] = *reinterpret_cast<const double2*>(sa + kg * A_KG + mi * 8 * 64);
-                    as[mi] = a[mi].x + a[mi].y;
-                }
-#pragma unroll
-                for (int nj = 0; nj < NJ; nj++) {
-                    const double2 b = *reinterpret_cast<const double2*>(sb + kg * B_KG + nj * 8 * 64);
-                    const double bs = b.x + b.y;
-#pragma unroll
-                    for (int mi = 0; mi < MI; mi++) dmma884(p1[mi][nj][0], p1[mi][nj][1], a[mi].x, b.x);
-#pragma unroll
-                    for (int mi = 0; mi < MI; mi++) dmma884(p2[mi][nj][0], p2[mi][nj][1], a[mi].y, b.y);
-#pragma unroll
-                    for (int mi = 0; mi < MI; mi++) dmma884(p3[mi][nj][0], p3[mi][nj][1], as[mi], bs);
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
-        }
-
-#pragma unroll
-        for (int mi = 0; mi < MI; mi++) {
-            const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
-            if (m >= p.M) continue;
-#pragma unroll
-            for (int nj = 0; nj < NJ; nj++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                    const int64_t n = n0 + wn * NJ * 8 + nj * 8 + 2 * q + e;
-                    if (n >= p.N) continue;
-                    c128 r = mk(p1[mi][nj][e] - p2[mi][nj][e], p3[mi][nj][e] - p1[mi][nj][e] - p2[mi][nj][e]);
-                    if (p.ksplit > 1) {
-                        p.partial[((int64_t)blockIdx.z * p.M + m) * p.N + n] = r;
-                    } else {
-                        c128* c = p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn;
-                        r = cmul(p.alpha, r);
-                        *c = p.accumulate ? cadd(*c, r) : r;
-                    }
-                }
-        }
     }
 }
 
@@ -309,6 +328,27 @@ static int make_operand_map(CUtensorMap* map, const c128* base, int64_t rows, in
     return CCSD_OK;
 }
 
+// rows x K real sum plane (same leading dimension / batch stride, in elements, as the complex operand it belongs to)
+static int make_plane_map(CUtensorMap* map, const double* base, int64_t rows, int64_t K, int64_t ld, int nb, int64_t bs,
+                          int box_rows)
+{
+    PFN_encodeTiled enc = get_encode_fn();
+    if (!enc) { snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled unavailable"); return CCSD_ECUDA; }
+    cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)rows, (cuuint64_t)(nb > 0 ? nb : 1)};
+    cuuint64_t strides[2] = {(cuuint64_t)(ld * 8), (cuuint64_t)((nb > 1 && bs > 0) ? bs * 8 : ld * 8)};
+    cuuint32_t box[3] = {4, (cuuint32_t)box_rows, 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled (plane) failed (%d): rows=%lld K=%lld ld=%lld", (int)r,
+                 (long long)rows, (long long)K, (long long)ld);
+        return CCSD_ECUDA;
+    }
+    return CCSD_OK;
+}
+
 static inline bool dmma_supported(const GemmParams& p)
 {
     if (p.sak != 1 || p.sbk != 1) return false;
@@ -328,14 +368,15 @@ static inline bool dmma_worthwhile(const GemmParams& p)
 }
 
 template <class Cfg>
-static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const DmmaArgs& a, dim3 grid)
+static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const CUtensorMap& mAs,
+                           const CUtensorMap& mBs, const DmmaArgs& a, dim3 grid)
 {
     static bool configured = false;
     if (!configured) {
         CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
         configured = true;
     }
-    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mA, mB, a);
+    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mA, mB, mAs, mBs, a);
     g_launches++;
     return CCSD_OK;
 }
@@ -344,11 +385,13 @@ static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtenso
 // families, column-tile width chosen per launch; the rest are tuning variants reachable through gemm_mode >= 100.
 struct DmmaVariant {
     int bm, bn;
-    bool m3;
-    int (*launch)(cudaStream_t, const CUtensorMap&, const CUtensorMap&, const DmmaArgs&, dim3);
+    bool m3, planes;
+    int (*launch)(cudaStream_t, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&,
+                  const DmmaArgs&, dim3);
 };
-#define DMMA_V(nwm, nwn, mi, nj, m3) \
-    {DmmaCfg<nwm, nwn, mi, nj, m3>::BM, DmmaCfg<nwm, nwn, mi, nj, m3>::BN, m3, &launch_dmma_cfg<DmmaCfg<nwm, nwn, mi, nj, m3>>}
+#define DMMA_V(nwm, nwn, mi, nj, m3, ...) \
+    {DmmaCfg<nwm, nwn, mi, nj, m3, ##__VA_ARGS__>::BM, DmmaCfg<nwm, nwn, mi, nj, m3, ##__VA_ARGS__>::BN, m3, \
+     DmmaCfg<nwm, nwn, mi, nj, m3, ##__VA_ARGS__>::PL, &launch_dmma_cfg<DmmaCfg<nwm, nwn, mi, nj, m3, ##__VA_ARGS__>>}
 static const DmmaVariant k_dmma_variants[] = {
     DMMA_V(4, 2, 4, 4, false), DMMA_V(4, 2, 4, 5, false), DMMA_V(4, 2, 4, 6, false), DMMA_V(4, 2, 4, 7, false),
     DMMA_V(4, 2, 4, 8, false),                                       // 0-4: 4M, 128 x {32,40,48,56,64}, 8 warps
@@ -356,6 +399,7 @@ static const DmmaVariant k_dmma_variants[] = {
     DMMA_V(4, 4, 4, 4, false),                                       // 8: 4M 128 x 64, 16 warps
     DMMA_V(4, 3, 4, 2, true),                                        // 9: 3M 128 x 48, 12 warps
     DMMA_V(4, 3, 4, 5, false),                                       // 10: 4M 128 x 60, 12 warps
+    DMMA_V(4, 2, 4, 2, true, true), DMMA_V(4, 2, 4, 3, true, true),  // 11-12: 3M with sum planes, 128 x {32,48}
 };
 #undef DMMA_V
 constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_variants[0]));
@@ -363,15 +407,19 @@ constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_var
 #define CCSD_DEFAULT_3M 1
 #endif
 
-// variant of a family (3M or 4M) whose column-tile width wastes the fewest padded columns; ties -> wider
-static inline int dmma_pick(int64_t N, bool m3)
+// variant of a family (4M, 3M, 3M with sum planes) with the lowest estimated cost: padded columns x the measured
+// relative cost per column of that tile width (narrow tiles re-read the A tile more often and, for 3M, spend a larger
+// share of the FP64 pipe on the sums; cfg3 (ov)^3 GEMM: 128x32 vs 128x48 = 1.037 without planes, 1.019 with)
+static inline int dmma_pick(int64_t N, bool m3, bool planes = false)
 {
-    const int lo = m3 ? 5 : 0, hi = m3 ? 5 : 4;   // 3M: the 128 x 32 tile only (wider 3M tiles spill at 168 registers)
-    int best = hi;
-    int64_t bestpad = round_up(N, k_dmma_variants[hi].bn);
-    for (int v = hi - 1; v >= lo; v--) {
-        int64_t pad = round_up(N, k_dmma_variants[v].bn);
-        if (pad < bestpad) { bestpad = pad; best = v; }
+    const int lo = planes ? 11 : (m3 ? 5 : 0), hi = planes ? 12 : (m3 ? 6 : 4);
+    int best = -1;
+    double bestcost = 0.0;
+    for (int v = hi; v >= lo; v--) {
+        const int bn = k_dmma_variants[v].bn;
+        const double rel = planes ? (bn == 32 ? 1.019 : 1.0) : m3 ? (bn == 32 ? 1.037 : 1.0) : 1.0 + 0.01 * (64 - bn) / 8.0;
+        const double cost = (double)round_up(N, bn) * rel;
+        if (best < 0 || cost < bestcost) { best = v; bestcost = cost; }
     }
     return best;
 }
@@ -383,6 +431,12 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     CUtensorMap mA, mB;
     CCSD_TRY(make_operand_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
     CCSD_TRY(make_operand_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
+    CUtensorMap mAs = mA, mBs = mB;   // unused unless the variant stages sum planes
+    if (V.planes) {
+        if (!p.As || !p.Bs) return CCSD_EINVAL;
+        CCSD_TRY(make_plane_map(&mAs, p.As, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
+        CCSD_TRY(make_plane_map(&mBs, p.Bs, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
+    }
     DmmaArgs a;
     a.M = p.M; a.N = p.N; a.K = p.K;
     a.C = p.C; a.csm = p.csm; a.csn = p.csn; a.bsC = p.bsC;
@@ -391,5 +445,5 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     a.batchB = (p.batch > 1 && p.bsB != 0) ? 1 : 0;
     a.ksplit = p.ksplit; a.kchunk = p.kchunk; a.partial = p.partial;
     dim3 grid((unsigned)((p.N + V.bn - 1) / V.bn), (unsigned)((p.M + V.bm - 1) / V.bm), (unsigned)(p.batch * p.ksplit));
-    return V.launch(st, mA, mB, a, grid);
+    return V.launch(st, mA, mB, mAs, mBs, a, grid);
 }

@@ -13,6 +13,7 @@ struct GemmParams {
     int batch; int64_t bsA, bsB, bsC;  // batch strides (elements)
     int ksplit; int64_t kchunk;        // split-K: slice s covers k in [s*kchunk, min(K,(s+1)*kchunk))
     c128* partial;                     // ksplit > 1: partial[(b*ksplit + s)][m][n] (dense M x N), reduced afterwards
+    const double *As, *Bs;             // optional 3M sum planes  As[m*sam + k] = Re A + Im A  (DMMA kernel only)
 };
 
 constexpr int SG_BM = 64, SG_BN = 64, SG_BK = 8, SG_T = 16;

@@ -182,6 +182,15 @@ def test_contract_terms(gpu, o, v):
     assert _rel(got.ravel(), ref["tau"]) < REL_TOL
     got = gpu.contract("pp_ladder", o, v, [tau, ref["vvvv"].reshape(vv, vv)]).cpu().numpy()
     assert _rel(got.ravel(), ref["S2_pp_ladder"]) < REL_TOL
+    # the same contraction on the 4M kernels, the 3M kernels, and 3M with caller-supplied sum planes (as ccsd_iterate runs it)
+    W = ref["vvvv"].reshape(vv, vv)
+    for mode in (2, 3):
+        got = gpu.contract("pp_ladder", o, v, [tau, W], gemm_mode=mode).cpu().numpy()
+        assert _rel(got.ravel(), ref["S2_pp_ladder"]) < REL_TOL, mode
+    taus, Ws = gpu.sum_plane(tau), gpu.sum_plane(W)
+    assert np.array_equal(taus.cpu().numpy(), tau.real + tau.imag)
+    got = gpu.contract("pp_ladder_planes", o, v, [tau, W, taus, Ws]).cpu().numpy()
+    assert _rel(got.ravel(), ref["S2_pp_ladder"]) < REL_TOL
     got = gpu.contract("hh_ladder", o, v, [ref["A"].reshape(oo, oo), tau]).cpu().numpy()
     assert _rel(got.ravel(), ref["S2_hh_ladder"]) < REL_TOL
     got = gpu.contract("ring", o, v, [ref["Hvovo"].reshape(v, o, v, o), t2p]).cpu().numpy()
@@ -194,7 +203,7 @@ def test_contract_terms(gpu, o, v):
 
 
 @pytest.mark.parametrize("M,N,K", [(1, 1, 1), (37, 53, 29), (130, 70, 260), (64, 64, 64), (300, 9, 1000), (5, 700, 36)])
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 def test_zgemm_nt_matches_oracle_samples(gpu, M, N, K, mode):
     from oracle.ccsd_oracle import nt_samples
     rng = np.random.default_rng(M * 1000 + N + K)
@@ -206,6 +215,21 @@ def test_zgemm_nt_matches_oracle_samples(gpu, M, N, K, mode):
     assert _rel(C, ref) < REL_TOL
     Ct = gpu.zgemm_nt(A, B, alpha=0.5 - 0.25j, mode=mode, transposed_out=True).cpu().numpy()
     assert _rel(Ct.T, ref) < REL_TOL
+
+
+@pytest.mark.parametrize("M,N,K", [(37, 53, 30), (130, 70, 260), (300, 9, 1002), (5, 700, 36), (129, 49, 18)])
+@pytest.mark.parametrize("mode", [0, 111, 112])
+def test_zgemm_nt_with_sum_planes(gpu, M, N, K, mode):
+    """The 3M kernels reading caller-supplied sum planes (even K = leading dimension, ragged everything else)."""
+    from oracle.ccsd_oracle import nt_samples
+    rng = np.random.default_rng(M * 1000 + N + K)
+    A = rng.standard_normal((M, K)) + 1j * rng.standard_normal((M, K))
+    B = rng.standard_normal((N, K)) + 1j * rng.standard_normal((N, K))
+    As, Bs = gpu.sum_plane(A), gpu.sum_plane(B)
+    C = gpu.zgemm_nt(A, B, alpha=-0.75 + 0.5j, mode=mode, planes=(As, Bs)).cpu().numpy()
+    ms, ns = np.meshgrid(np.arange(M), np.arange(N), indexing="ij")
+    ref = (-0.75 + 0.5j) * nt_samples(A, B, ms.ravel(), ns.ravel()).reshape(M, N)
+    assert _rel(C, ref) < REL_TOL
 
 
 @pytest.mark.parametrize("dims", [(3, 5, 7, 9), (34, 33, 2, 65), (1, 1, 40, 40), (8, 8, 8, 8)])
