@@ -239,7 +239,8 @@ def transpose_bench(torch, pkg, hbm_gbs, o, v):
     x = torch.view_as_complex(torch.randn((o, o, v, v, 2), device="cuda", dtype=torch.float64))
     nbytes = 2 * x.numel() * 16
     res = {}
-    for name, perm in (("ijab->abij", [2, 3, 0, 1]), ("ijab->iajb", [0, 2, 1, 3]), ("ijab->jiba", [1, 0, 3, 2])):
+    for name, perm in (("ijab->abij", [2, 3, 0, 1]), ("ijab->iajb", [0, 2, 1, 3]), ("ijab->jiba", [1, 0, 3, 2]),
+                       ("ijab->baji", [3, 2, 1, 0]), ("ijab->aibj", [2, 0, 3, 1]), ("ijab->ibaj", [0, 3, 2, 1])):
         ts = time_events(torch, lambda: pkg.transpose(x, perm), 5, 3)
         gbs = nbytes / (statistics.median(ts) * 1e-3) * 1e-9
         res[name] = {"gbs": round(gbs, 1), "frac_hbm": round(gbs / hbm_gbs, 3)}

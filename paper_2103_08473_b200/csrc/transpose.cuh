@@ -44,23 +44,42 @@ __global__ void __launch_bounds__(256) transpose4_kernel(const c128* __restrict_
     }
 }
 
-// Fastest index preserved: plain strided row copy.  rows enumerate the three slow input dims.
+// Fastest index preserved: the tensor is a set of contiguous rows of nx elements that are re-ordered.  The kernel
+// walks the OUTPUT linearly (perfectly coalesced 16-byte stores, 8 independent 16-byte loads in flight per thread) and
+// decomposes the output row index into the (up to three) slow output dims to find the input row.
 struct Cp4 {
-    int64_t nx, n0, n1, n2;
-    int64_t i0, i1, i2, o0, o1, o2;
+    int64_t nx, total;             // row length, total elements
+    unsigned n1, n2;               // extents of the two fastest slow OUTPUT dims (n0 is implied)
+    int64_t i0, i1, i2;            // input strides of the slow output dims
     int conj;
 };
+constexpr int CP_UNROLL = 8;
 __global__ void __launch_bounds__(256) copy4_kernel(const c128* __restrict__ in, c128* __restrict__ out, Cp4 t)
 {
-    int64_t row = (int64_t)blockIdx.x * blockDim.y + threadIdx.y;
-    if (row >= t.n0 * t.n1 * t.n2) return;
-    int64_t a2 = row % t.n2, a1 = (row / t.n2) % t.n1, a0 = row / (t.n2 * t.n1);
-    const c128* src = in + a0 * t.i0 + a1 * t.i1 + a2 * t.i2;
-    c128* dst = out + a0 * t.o0 + a1 * t.o1 + a2 * t.o2;
-    for (int64_t x = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; x < t.nx; x += (int64_t)gridDim.y * blockDim.x) {
-        c128 val = src[x];
-        if (t.conj) val.y = -val.y;
-        dst[x] = val;
+    const int64_t base = (int64_t)blockIdx.x * (256 * CP_UNROLL);
+    // 64-bit division once per block; everything below is 32-bit relative to the block's first row
+    const int64_t row0 = base / t.nx;
+    const unsigned x0 = (unsigned)(base - row0 * t.nx), nx = (unsigned)t.nx;
+    c128 val[CP_UNROLL];
+#pragma unroll
+    for (int k = 0; k < CP_UNROLL; k++) {
+        const unsigned off = x0 + threadIdx.x + 256u * k;
+        if (base + threadIdx.x + 256 * k < t.total) {
+            const int64_t row = row0 + off / nx;
+            const unsigned x = off % nx;
+            const int64_t a2 = row % t.n2, r1 = row / t.n2;
+            const int64_t a1 = r1 % t.n1, a0 = r1 / t.n1;
+            val[k] = in[a0 * t.i0 + a1 * t.i1 + a2 * t.i2 + x];
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < CP_UNROLL; k++) {
+        const int64_t e = base + threadIdx.x + 256 * k;
+        if (e < t.total) {
+            c128 w = val[k];
+            if (t.conj) w.y = -w.y;
+            out[e] = w;
+        }
     }
 }
 
@@ -86,7 +105,9 @@ static inline int launch_transpose2d(cudaStream_t st, const c128* in, c128* out,
     return launch_transpose2d_ld(st, in, cols, out, rows, rows, cols, conj);
 }
 
-// out dimension q is input dimension perm[q]
+// out dimension q is input dimension perm[q].  Extent-1 dims are dropped and input dims that stay adjacent (in the same
+// order) in the output are merged first, so that e.g. ijab -> abij runs as ONE 2-d transposition (ij) x (ab) with full
+// tiles instead of o x v ragged ones.
 static inline int launch_transpose4d(cudaStream_t st, const c128* in, c128* out, const int64_t d[4], const int perm[4], int conj)
 {
     int seen[4] = {0, 0, 0, 0};
@@ -95,35 +116,67 @@ static inline int launch_transpose4d(cudaStream_t st, const c128* in, c128* out,
         seen[perm[q]] = 1;
         if (d[q] < 0) return CCSD_EINVAL;
     }
-    if (d[0] * d[1] * d[2] * d[3] == 0) return CCSD_OK;
-    int64_t is[4] = {d[1] * d[2] * d[3], d[2] * d[3], d[3], 1};
-    int64_t od[4], os[4], os_of_in[4];
-    for (int q = 0; q < 4; q++) od[q] = d[perm[q]];
-    os[3] = 1; os[2] = od[3]; os[1] = od[2] * od[3]; os[0] = od[1] * od[2] * od[3];
-    for (int q = 0; q < 4; q++) os_of_in[perm[q]] = os[q];
-    if (perm[3] == 3) {
+    const int64_t total = d[0] * d[1] * d[2] * d[3];
+    if (total == 0) return CCSD_OK;
+    // rank of every non-trivial input dim in the output order
+    int orank[4] = {-1, -1, -1, -1}, nout = 0;
+    for (int q = 0; q < 4; q++)
+        if (d[perm[q]] > 1) orank[perm[q]] = nout++;
+    // groups of merged dims, in input order
+    int ng = 0, grank[4];
+    int64_t gext[4];
+    for (int q = 0, prev = -1; q < 4; q++) {
+        if (d[q] <= 1) continue;
+        if (prev >= 0 && orank[q] == orank[prev] + 1) {
+            gext[ng - 1] *= d[q];
+        } else {
+            gext[ng] = d[q]; grank[ng] = orank[q]; ng++;
+        }
+        prev = q;
+    }
+    if (ng == 0) { ng = 1; gext[0] = 1; grank[0] = 0; }
+    // input strides (groups are in input order) and the groups in output order
+    int64_t gis[4], gos[4];
+    gis[ng - 1] = 1;
+    for (int k = ng - 2; k >= 0; k--) gis[k] = gis[k + 1] * gext[k + 1];
+    int order[4];   // order[r] = group that is r-th in the output
+    for (int r = 0; r < ng; r++) {
+        int best = -1;
+        for (int k = 0; k < ng; k++) {
+            bool used = false;
+            for (int rr = 0; rr < r; rr++) used |= (order[rr] == k);
+            if (!used && (best < 0 || grank[k] < grank[best])) best = k;
+        }
+        order[r] = best;
+    }
+    gos[order[ng - 1]] = 1;
+    for (int r = ng - 2; r >= 0; r--) gos[order[r]] = gos[order[r + 1]] * gext[order[r + 1]];
+
+    if (order[ng - 1] == ng - 1) {
+        // fastest group preserved: re-ordered contiguous rows
         Cp4 t;
-        t.nx = d[3]; t.n0 = d[0]; t.n1 = d[1]; t.n2 = d[2];
-        t.i0 = is[0]; t.i1 = is[1]; t.i2 = is[2];
-        t.o0 = os_of_in[0]; t.o1 = os_of_in[1]; t.o2 = os_of_in[2];
-        t.conj = conj;
-        int bx = 1;
-        while (bx < 256 && bx < d[3]) bx <<= 1;
-        int by = 256 / bx;
-        int64_t rows = d[0] * d[1] * d[2];
-        int64_t gy = (d[3] + bx - 1) / bx;
-        if (gy > 64) gy = 64;
-        dim3 grid((unsigned)((rows + by - 1) / by), (unsigned)gy), block(bx, by);
-        copy4_kernel<<<grid, block, 0, st>>>(in, out, t);
+        t.nx = gext[ng - 1]; t.total = total; t.conj = conj;
+        int64_t ext[3] = {1, 1, 1}, ist[3] = {0, 0, 0};   // slow output dims, right-aligned
+        for (int r = ng - 2, s = 2; r >= 0; r--, s--) { ext[s] = gext[order[r]]; ist[s] = gis[order[r]]; }
+        if (ext[1] > 0xffffffffLL || ext[2] > 0xffffffffLL || t.nx > 0x7fffffffLL) return CCSD_EINVAL;
+        t.n1 = (unsigned)ext[1]; t.n2 = (unsigned)ext[2];
+        t.i0 = ist[0]; t.i1 = ist[1]; t.i2 = ist[2];
+        const int64_t blocks = (total + 256 * CP_UNROLL - 1) / (256 * CP_UNROLL);
+        if (blocks > 0x7fffffffLL) return CCSD_EINVAL;
+        copy4_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, t);
     } else {
-        int p = perm[3];           // input dim that becomes fastest in the output
-        int r[2], nr = 0;
-        for (int q = 0; q < 3; q++)
-            if (q != p) r[nr++] = q;
+        const int gx = ng - 1, gy = order[ng - 1];   // x: input-fastest group, y: output-fastest group
         Tr4 t;
-        t.nx = d[3]; t.ny = d[p]; t.n1 = d[r[0]]; t.n2 = d[r[1]];
-        t.iy = is[p]; t.i1 = is[r[0]]; t.i2 = is[r[1]];
-        t.ox = os_of_in[3]; t.o1 = os_of_in[r[0]]; t.o2 = os_of_in[r[1]];
+        t.nx = gext[gx]; t.ny = gext[gy];
+        t.iy = gis[gy]; t.ox = gos[gx];
+        t.n1 = 1; t.n2 = 1; t.i1 = t.i2 = t.o1 = t.o2 = 0;
+        int nr = 0;
+        for (int k = 0; k < ng; k++) {
+            if (k == gx || k == gy) continue;
+            if (nr == 0) { t.n1 = gext[k]; t.i1 = gis[k]; t.o1 = gos[k]; }
+            else { t.n2 = gext[k]; t.i2 = gis[k]; t.o2 = gos[k]; }
+            nr++;
+        }
         t.conj = conj;
         int64_t blocks = ((t.nx + TR_TILE - 1) / TR_TILE) * ((t.ny + TR_TILE - 1) / TR_TILE) * t.n1 * t.n2;
         if (blocks > 0x7fffffffLL) return CCSD_EINVAL;
