@@ -288,3 +288,60 @@ def nt_samples(A: np.ndarray, B: np.ndarray, ms, ns, conjB: bool = False) -> np.
     lib().oracle_nt_samples(ctypes.c_long(A.shape[1]), _p(A), ctypes.c_long(A.shape[1]), _p(B),
                             ctypes.c_long(B.shape[1]), int(conjB), len(ms), _p(ms), _p(ns), _p(out))
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# single-element evaluators straight from the factorised integrals (full-size spot checks at cfg2/cfg3, where the
+# unpacked <ab||cd> of OracleCCSD would need v^4 * 16 bytes).  Each is the definition written out for one element.
+# ---------------------------------------------------------------------------------------------------------------
+def g_samples(B: np.ndarray, p, q, r, s) -> np.ndarray:
+    """<pq||rs> = (pr|qs) - (ps|qr) with (pq|rs) = sum_L B[L,p,q] B[L,r,s]  (eq 6 PAPER.md:71 in
+    reading G1) at sampled index quadruples (absolute spinor indices)."""
+    p, q, r, s = (np.asarray(x, dtype=np.int64) for x in (p, q, r, s))
+    out = np.zeros(len(p), dtype=C128)
+    for n in range(len(p)):
+        out[n] = np.sum(B[:, p[n], r[n]] * B[:, q[n], s[n]]) - np.sum(B[:, p[n], s[n]] * B[:, q[n], r[n]])
+    return out
+
+
+def vvvv_row_packed(B: np.ndarray, nocc: int, a: int, b: int) -> np.ndarray:
+    """Row (a<b) of <ab||cd>, all c<d in packed order: (ac|bd) - (ad|bc), the sum over L as one matrix product."""
+    o = nocc
+    Ba, Bb = B[:, o + a, o:], B[:, o + b, o:]            # [L][c], [L][d]
+    J = Ba.T @ Bb                                          # J[c][d] = (ac|bd)
+    K = J.T                                                # K[c][d] = (ad|bc)
+    c, d = np.triu_indices(B.shape[1] - o, 1)
+    return (J - K)[c, d]
+
+
+def tau_row_packed(t1: np.ndarray, t2p_row: np.ndarray, i: int, j: int) -> np.ndarray:
+    """Row (i<j) of tau = t2 + t1[i,a] t1[j,b] - t1[j,a] t1[i,b] (eq 23), all a<b packed."""
+    a, b = np.triu_indices(t1.shape[1], 1)
+    return t2p_row + t1[i, a] * t1[j, b] - t1[j, a] * t1[i, b]
+
+
+def pp_ladder_samples_from_B(B: np.ndarray, nocc: int, t1: np.ndarray, t2p: np.ndarray, ij, ab) -> np.ndarray:
+    """1/2 sum_cd <ab||cd> tau^cd_ij = sum_{c<d} (eq 32 last line) at sampled packed (ij, ab) pairs,
+    from the factorised integrals and the amplitudes (t2p packed [(i<j)][(a<b)])."""
+    o, v = nocc, B.shape[1] - nocc
+    io, jo = np.triu_indices(o, 1)
+    av, bv = np.triu_indices(v, 1)
+    out = np.zeros(len(ij), dtype=C128)
+    for n, (IJ, AB) in enumerate(zip(ij, ab)):
+        w = vvvv_row_packed(B, o, int(av[AB]), int(bv[AB]))
+        tau = tau_row_packed(t1, t2p[IJ], int(io[IJ]), int(jo[IJ]))
+        out[n] = np.sum(w * tau)
+    return out
+
+
+def hov_samples_from_B(B: np.ndarray, f: np.ndarray, nocc: int, t1: np.ndarray, ks, cs) -> np.ndarray:
+    """H^k_c = f_kc + sum_ld <kl||cd> t^d_l (eq 28) at sampled (k, c)."""
+    o = nocc
+    out = np.zeros(len(ks), dtype=C128)
+    Bov = B[:, :o, o:]                                      # [L][l][d]
+    for n, (k, c) in enumerate(zip(ks, cs)):
+        # (kc|ld) - (kd|lc)
+        coul = np.einsum("L,Lld->ld", B[:, k, o + c], Bov)
+        exch = np.einsum("Ld,Ll->ld", B[:, k, o:], B[:, :o, o + c])
+        out[n] = f[k, o + c] + np.sum((coul - exch) * t1)
+    return out

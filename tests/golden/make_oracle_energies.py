@@ -26,16 +26,22 @@ def main():
              "# written by tests/golden/make_oracle_energies.py (oracle/ only, restricted-sum mode, DIIS(6))",
              f"# host threads: {num_threads()}",
              "# iteration  Re(E)  Im(E)  ||S/D||_2 of the residual evaluated in that iteration (nan for the MP2 start)"]
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"oracle_lockstep_{cfg}.txt")
+
+    def flush():   # rewritten after every iteration: a long run that is cut short still leaves its finished lines
+        with open(path, "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+
     e = oc.energy()
     lines.append(f"0 {e.real!r} {e.imag!r} nan")
     print(lines[-1], f"(setup {time.time() - t0:.0f} s)", flush=True)
+    flush()
     for it in range(1, niter + 1):
         t1 = time.time()
         e, sn = oc.iterate()
         lines.append(f"{it} {e.real!r} {e.imag!r} {sn!r}")
         print(lines[-1], f"({time.time() - t1:.0f} s)", flush=True)
-    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), f"oracle_lockstep_{cfg}.txt"), "w") as fh:
-        fh.write("\n".join(lines) + "\n")
+        flush()
 
 
 if __name__ == "__main__":

@@ -1,0 +1,164 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The plain-loop oracle needs minutes to hours per iteration at these sizes, so the comparisons are
+  * lock-step energies against files written by tests/golden/make_oracle_energies.py (oracle/ only, run on the CPU),
+  * sampled outputs the oracle evaluates one by one from the factorised integrals (oracle.*_samples_from_B),
+  * properties that hold at any size (Hermiticity / antisymmetry of the integral classes, residual antisymmetry).
+Tolerances: BASELINE.json north_star (1e-10 Eh on energies, 1e-12 relative max-abs per contraction output).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import ccsd_inputs as ci
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+REL_TOL = 1e-12
+E_TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2103_08473_b200 as lib
+    lib.load_library()
+    return lib
+
+
+def _read_golden(cfg):
+    path = os.path.join(GOLDEN, f"oracle_lockstep_{cfg}.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated")
+    rows = []
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            it, re, im, sn = line.split()
+            rows.append((int(it), complex(float(re), float(im)), float(sn)))
+    return rows
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2", "cfg3"])
+def test_lockstep_energies_against_oracle_golden(gpu, cfg):
+    """ccsd_init + N x ccsd_iterate from the MP2 start, DIIS(6): E after every iteration and ||S/D||_2 against the
+    CPU oracle's own run (every line of the golden file; cfg3 holds as many iterations as the oracle could afford)."""
+    rows = _read_golden(cfg)
+    inp = ci.make_config(cfg)
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, ndiis=6)
+    assert rows[0][0] == 0
+    e = gc.energy()
+    assert abs(e - rows[0][1]) < E_TOL, (e, rows[0][1])
+    for it, e_ref, sn_ref in rows[1:]:
+        e, sn = gc.iterate()
+        assert abs(e - e_ref) < E_TOL, (cfg, it, e, e_ref)
+        assert abs(sn - sn_ref) < 1e-9 * max(1.0, sn_ref), (cfg, it, sn, sn_ref)
+    gc.close()
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg3"])
+def test_fullsize_sampled_integrals_ladder_and_properties(gpu, cfg):
+    """Sampled <ab||cd>, <ak||cd>, <kl||cd>, H^k_c and pp-ladder outputs against the oracle's single-element
+    evaluators, at seeded random amplitudes CN(0, 0.01^2); plus Hermiticity of <ab||cd> across the whole tensor."""
+    import torch
+    from oracle import ccsd_oracle as orc
+    inp = ci.make_config(cfg)
+    o, v = inp.nocc, inp.nvir
+    oo, vv = ci.pair_count(o), ci.pair_count(v)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    rng = np.random.default_rng(12345)
+    av, bv = np.triu_indices(v, 1)
+    io, jo = np.triu_indices(o, 1)
+    ns = 48
+    # ---- integral classes (step I2) ----
+    W = gc.get_tensor("vvvv").view(vv, vv)
+    AB, CD = rng.integers(0, vv, ns), rng.integers(0, vv, ns)
+    AB[:4] = [0, vv - 1, 0, vv - 1]; CD[:4] = [0, vv - 1, vv - 1, 0]          # corners of the packed matrix
+    got = W[torch.from_numpy(AB).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
+    ref = orc.g_samples(inp.B, o + av[AB], o + bv[AB], o + av[CD], o + bv[CD])
+    scale = np.abs(ref).max()
+    assert np.abs(got - ref).max() <= REL_TOL * scale
+    # Hermiticity <ab||cd> = conj <cd||ab> over the whole tensor, slab by slab (a property at any size)
+    worst = 0.0
+    step = 2048
+    for r0 in range(0, vv, step):
+        blk = W[r0:r0 + step, :]
+        blkT = W[:, r0:r0 + step].transpose(0, 1).conj()
+        worst = max(worst, float((blk - blkT).abs().max()))
+    assert worst <= 1e-15 * 10 + REL_TOL * scale
+    del W
+    X = gc.get_tensor("vovv").view(v, o, vv)
+    a, k = rng.integers(0, v, ns), rng.integers(0, o, ns)
+    got = X[torch.from_numpy(a).cuda(), torch.from_numpy(k).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
+    ref = orc.g_samples(inp.B, o + a, k, o + av[CD], o + bv[CD])
+    assert np.abs(got - ref).max() <= REL_TOL * np.abs(ref).max()
+    del X
+    Y = gc.get_tensor("oovv").view(oo, vv)
+    KL = rng.integers(0, oo, ns)
+    got = Y[torch.from_numpy(KL).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
+    ref = orc.g_samples(inp.B, io[KL], jo[KL], o + av[CD], o + bv[CD])
+    assert np.abs(got - ref).max() <= REL_TOL * np.abs(ref).max()
+    del Y
+    torch.cuda.empty_cache()
+    # ---- one residual at seeded random amplitudes ----
+    t1, t2p = ci.random_amplitudes(o, v, 7, 0.01)
+    gc.set_amplitudes(t1, t2p)
+    gc.residual()
+    f = gc.get_tensor("fock").view(o + v, o + v).cpu().numpy()
+    # tau (eq 23): sampled rows
+    tau = gc.get_tensor("tau").view(oo, vv)
+    for IJ in (0, oo - 1, int(rng.integers(0, oo))):
+        ref = orc.tau_row_packed(t1, t2p[IJ], int(io[IJ]), int(jo[IJ]))
+        assert np.abs(tau[IJ].cpu().numpy() - ref).max() <= REL_TOL * np.abs(ref).max()
+    del tau
+    # H^k_c (eq 28)
+    ks, cs = rng.integers(0, o, 16), rng.integers(0, v, 16)
+    got = gc.get_tensor("Hov").view(o, v).cpu().numpy()[ks, cs]
+    ref = orc.hov_samples_from_B(inp.B, f, o, t1, ks, cs)
+    assert np.abs(got - ref).max() <= REL_TOL * np.abs(ref).max()
+    # pp-ladder (eq 32 last line), the bench's roofline launch: sampled outputs incl. the ragged last tiles
+    R = gc.get_tensor("S2_pp_ladder").view(oo, vv)
+    nl = 24
+    IJ, AB = rng.integers(0, oo, nl), rng.integers(0, vv, nl)
+    IJ[:4] = [0, oo - 1, 0, oo - 1]; AB[:4] = [0, vv - 1, vv - 1, 0]
+    got = R[torch.from_numpy(IJ).cuda(), torch.from_numpy(AB).cuda()].cpu().numpy()
+    ref = orc.pp_ladder_samples_from_B(inp.B, o, t1, t2p, IJ, AB)
+    assert np.abs(got - ref).max() <= REL_TOL * float(R.abs().max())
+    del R
+    gc.close()
+
+
+@pytest.mark.parametrize("k", range(len(ci.LADDER_SWEEP)))
+def test_cfg4_isolated_ladder_sampled(gpu, k):
+    """BASELINE config 4: the isolated pp-ladder at every sweep shape, launched as bench.py launches it (3M kernels with
+    sum planes), on sampled outputs the oracle computes one by one."""
+    import torch
+    from oracle.ccsd_oracle import pp_ladder_samples
+    o, v = ci.LADDER_SWEEP[k]
+    oo, vv = ci.pair_count(o), ci.pair_count(v)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(ci.LADDER_SEED0 + k)
+    W = torch.view_as_complex(torch.randn((vv, vv, 2), generator=gen, device="cuda", dtype=torch.float64))
+    W.mul_(5e-3 / np.sqrt(2))
+    tau = torch.view_as_complex(torch.randn((oo, vv, 2), generator=gen, device="cuda", dtype=torch.float64))
+    tau.mul_(0.01 / np.sqrt(2))
+    R = gpu.contract("pp_ladder_planes", o, v, [tau, W, gpu.sum_plane(tau), gpu.sum_plane(W)])
+    rng = np.random.default_rng(k)
+    ns = 64
+    ij, ab = rng.integers(0, oo, ns), rng.integers(0, vv, ns)
+    ij[:4] = [0, oo - 1, 0, oo - 1]; ab[:4] = [0, vv - 1, vv - 1, 0]
+    uab = np.unique(ab)
+    remap = {a: i for i, a in enumerate(uab)}
+    Wrows = W[torch.from_numpy(uab).cuda()].cpu().numpy()
+    ref = pp_ladder_samples(tau.cpu().numpy(), Wrows, ij, np.array([remap[a] for a in ab]))
+    got = R[torch.from_numpy(ij).cuda(), torch.from_numpy(ab).cuda()].cpu().numpy()
+    assert np.abs(got - ref).max() <= REL_TOL * float(R.abs().max())
+    # the 4M kernels give the same numbers (what differs is rounding only)
+    if vv <= 20000:
+        R4 = gpu.contract("pp_ladder", o, v, [tau, W], gemm_mode=2)
+        assert float((R4 - R).abs().max()) <= REL_TOL * float(R.abs().max())

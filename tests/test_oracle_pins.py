@@ -232,3 +232,27 @@ def test_p9_soft_reference_energies_from_survey():
             assert abs(e.real - re_) < 2e-13, (cfg, key, e)
             if im_ is not None:
                 assert abs(e.imag - im_) < max(2e-13, 5e-3 * abs(im_)), (cfg, key, e)
+
+
+def test_sampled_evaluators_from_B_equal_the_plain_loop_oracle():
+    """The single-element evaluators used for the full-size (cfg2/cfg3) spot checks are pinned to the explicit-loop
+    oracle on a small ragged system: <pq||rs> samples, the pp-ladder of eq 32 and H^k_c of eq 28."""
+    from oracle import ccsd_oracle as orc
+    o, v, L = 5, 11, 20
+    inp = ci.make_inputs(o, v, L, seed=3, b_scale=0.1, f_offdiag=0.05)
+    oc = orc.OracleCCSD(inp.h, inp.B, o, v)
+    t1, t2p = ci.random_amplitudes(o, v, 1, 0.1)
+    oc.set_amplitudes(t1, orc.unpack_t2(t2p, o, v))
+    oc.residual()
+    rng = np.random.default_rng(0)
+    ref = orc.pack_t2(oc.s2_term("pp_ladder"))
+    ij, ab = rng.integers(0, ref.shape[0], 25), rng.integers(0, ref.shape[1], 25)
+    got = orc.pp_ladder_samples_from_B(inp.B, o, t1, t2p, ij, ab)
+    assert np.abs(got - ref[ij, ab]).max() < 1e-14 * max(1.0, np.abs(ref).max())
+    ks, cs = rng.integers(0, o, 12), rng.integers(0, v, 12)
+    assert np.abs(orc.hov_samples_from_B(inp.B, oc.f, o, t1, ks, cs) - oc.Hov[ks, cs]).max() < 1e-14
+    a, b, c, d = rng.integers(0, v, (4, 30))
+    assert np.abs(orc.g_samples(inp.B, o + a, o + b, o + c, o + d) - oc.vvvv[a, b, c, d]).max() < 1e-15
+    k, l = rng.integers(0, o, (2, 30))
+    assert np.abs(orc.g_samples(inp.B, k, l, o + c, o + d) - oc.oovv[k, l, c, d]).max() < 1e-15
+    assert np.abs(orc.g_samples(inp.B, o + a, k, o + c, o + d) - oc.vovv[a, k, c, d]).max() < 1e-15
