@@ -48,6 +48,9 @@ typedef struct {
                            (on-device debugging reference), 2 = DMMA kernels with 4M complex arithmetic,
                            3 = DMMA kernels with 3M; 100+v = one fixed tile variant v (tuning only) */
     int ccd;            /* 1 = CCD: t1 is kept at zero */
+    int cc2;            /* 1 = CC2 (Appendix 7.2 eqs 34-38): singles equations of CCSD,
+                           doubles equations <Phi_ij^ab| exp(-T1) H exp(T1) + [F, T2] |Phi_0>; ccsd_get_tensor then returns
+                           tau, C, A at t2 = 0, GVV = f_vv, GOO = -f_oo, and S2_GVV / S2_GOO the two Fock terms */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */

@@ -551,14 +551,14 @@ static void tick(ccsd_ctx* c, int k)
 }
 
 // eq 23 on packed storage: tau = t2 + t1[i,a] t1[j,b] - t1[j,a] t1[i,b]
-// (plane != null: also its 3M sum plane, so that the two can never be out of step)
+// (plane != null: also its 3M sum plane, so that the two can never be out of step; t2p == null: t2 = 0, the CC2 operand)
 static void build_tau(cudaStream_t st, c128* taup, const c128* t1, const c128* t2p, int o, int v, const int2* po,
                       const int2* pv, double* plane)
 {
     const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2;
     launch_fill(st, taup, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
         int2 ij = po[IJ], ab = pv[AB];
-        c128 x = t2p[IJ * vv + AB];
+        c128 x = t2p ? t2p[IJ * vv + AB] : mk(0.0, 0.0);
         cfma(x, t1[ij.x * v + ab.x], t1[ij.y * v + ab.y]);
         c128 y = cmul(t1[ij.y * v + ab.x], t1[ij.x * v + ab.y]);
         x = csub(x, y);
@@ -892,6 +892,57 @@ static int residual(ccsd_ctx* c)
     return CCSD_OK;
 }
 
+// CC2 (Appendix 7.2, eqs 34-38).  "The T1 amplitude equations in 7.1 are unchanged":
+// S1 is eq 33 at the full (t1, t2).  The doubles equation 34 is <Phi_ij^ab| exp(-T1) H exp(T1) + [F, T2] |Phi_0>, i.e.
+// eq 32 evaluated with t2 -> 0 in every operand (tau -> P-(t1 t1); the ring, G.t2 terms vanish; H^{ak}_{ci} is not
+// needed) plus the two Fock terms, which have the form of the G.t2 terms of eq 32 with G^a_c -> f_ac, G^k_i -> -f_ki:
+//   W^{ab}_{ef}CC2 (x) t1 t1  = pp-ladder(tau0) + the <bk||cd> tau0 part of C;  W^{mn}_{ij}CC2 = A(tau0) of eq 31 (up to the
+//   factor of the quartic term shared between eqs 35 and 36);  W^{ab}_{ej}, W^{mb}_{ij} = V-dagger.t1 and the rest of C.t1.
+// The oracle evaluates eqs 34-38 literally; the two agree to rounding (tests/test_gpu_cc2.py).
+static int residual_cc2(ccsd_ctx* c)
+{
+    cudaStream_t st = c->st;
+    const int o = c->o, v = c->v, n = c->n;
+    tick(c, 0);
+    CCSD_TRY(prep_operands(c));
+    tick(c, 1);
+    CCSD_TRY(fock_like(c));
+    tick(c, 2);
+    tick(c, 3);
+    CCSD_TRY(build_S1(c));                      // eq 33, full tau (timed under "Hvovo_quad"'s slot: see ccsd_step_name)
+    tick(c, 4);
+    // doubles: operands with t2 = 0
+    build_tau(st, c->taup, c->t1, nullptr, o, v, c->po, c->pv, c->taups);
+    CCSD_TRY(launch_transpose2d_ld(st, c->taup, c->vv, c->TT, 2 * c->oop, c->oo, c->vv, 0));
+    const c128* f = c->f;
+    launch_fill(st, c->Gvv, v, v, v, 0, [=] __device__(int64_t a, int64_t cc) { return f[(o + a) * n + o + cc]; });
+    launch_fill(st, c->Goo, o, o, o, 0, [=] __device__(int64_t k, int64_t i) { return cneg(f[k * n + i]); });
+    CCSD_TRY(build_C(c));
+    tick(c, 5);
+    CCSD_TRY(build_A(c));
+    cudaMemsetAsync(c->S2p, 0, (size_t)(c->oo * c->vv) * sizeof(c128), st);
+    CCSD_TRY(s2_driver(c, c->S2p));
+    tick(c, 6);
+    CCSD_TRY(s2_pp_ladder(c, c->S2p));
+    tick(c, 7);
+    CCSD_TRY(s2_hh_and_goo(c, c->S2p));         // hh-ladder of tau0 and -f_oo . t2
+    tick(c, 8);
+    tick(c, 9);
+    tick(c, 10);
+    CCSD_TRY(s2_vdag_t1(c, c->S2p));
+    tick(c, 11);
+    CCSD_TRY(s2_gvv(c, c->S2p));                // f_vv . t2
+    tick(c, 12);
+    CCSD_TRY(s2_c_t1(c, c->S2p));
+    tick(c, 13);
+    tick(c, 14);
+    c->have_residual = true;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+static int residual_any(ccsd_ctx* c) { return c->opt.cc2 ? residual_cc2(c) : residual(c); }
+
 // ---------------------------------------------------------------------------------------------------------------
 // energy, update, DIIS
 // ---------------------------------------------------------------------------------------------------------------
@@ -939,6 +990,7 @@ void ccsd_default_options(ccsd_options* opts)
     opts->level_shift = 0.0;
     opts->gemm_mode = 0;
     opts->ccd = 0;
+    opts->cc2 = 0;
 }
 
 int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
@@ -1015,13 +1067,13 @@ int ccsd_energy(ccsd_ctx* c, double* e_re, double* e_im)
 int ccsd_residual(ccsd_ctx* c)
 {
     if (!c) return CCSD_ESTATE;
-    return residual(c);
+    return residual_any(c);
 }
 
 int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
 {
     if (!c) return CCSD_ESTATE;
-    CCSD_TRY(residual(c));
+    CCSD_TRY(residual_any(c));
     const int o = c->o, v = c->v;
     const int64_t vv = c->vv, ov = c->ov, nvec = c->nvec;
     const int nd = c->opt.ndiis;
