@@ -247,6 +247,22 @@ def transpose_bench(torch, pkg, hbm_gbs, o, v):
     return res
 
 
+def cc2_bench(torch, pkg, inp, o, v, steps=5, warmup=3):
+    """NEXT-1 row of SURVEY 8(f): the CC2 iteration on the same workload, device-resident."""
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, cc2=True)
+    solver.enable_step_timing(True)
+    ts = time_events(torch, solver.iterate, steps, warmup)
+    st = solver.step_times()
+    e, sn = solver.iterate()
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    return {"s_per_iteration": round(statistics.median(ts) * 1e-3, 6), "steps": steps, "warmup": warmup,
+            "pp_ladder_ms": round(st["pp_ladder"], 3), "C_ovoo_ms": round(st["C_ovoo"], 3),
+            "E_last": [e.real, e.imag], "step_norm_last": sn,
+            "note": "eq 34 evaluated as eq 32 at t2 = 0 plus the two Fock terms; singles by eq 33"}
+
+
 def max_over_ranks(value: float, dist, device="cuda") -> float:
     """Multi-GPU numbers are the MAX over ranks (replicas-only path: no data-path collective exists)."""
     import torch
@@ -406,6 +422,7 @@ def run_ours(args) -> None:
     solver.close()
     del solver
     torch.cuda.empty_cache()
+    cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
     cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
@@ -429,7 +446,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:
