@@ -113,6 +113,27 @@ int ccsd_get_tensor(ccsd_ctx* ctx, int tensor_id, ccsd_c128* out);
 int ccsd_destroy(ccsd_ctx* ctx);
 
 /*
+ * Perturbative triples corrections at the CURRENT amplitudes (Appendix 7.3, eqs 39-44):
+ *   E(+T)  = sum conj(Wbar) Wbar / (36 D)            (eq 39)      Wbar = W^abc + W^bca + W^cab, W of eq 40
+ *   E((T)) = E(+T) + sum conj(Zbar) Wbar / (36 D)    (eq 41)      Z of eq 42
+ *   E(-T)  = E(+T) + sum conj(Ybar) Wbar / 36        (eq 43)      Y of eq 44
+ * with D = eps_i + eps_j + eps_k - eps_a - eps_b - eps_c and the sums over all i,j,k,a,b,c (evaluated over the unique
+ * i<j<k, a<b<c).  Reading of the printed equations for complex amplitudes: DESIGN.md G22.
+ * HOST outputs, (Re, Im) each.  workspace: device, 256-byte aligned, ccsd_triples_workspace_bytes() bytes, used only
+ * during the call.  Needs nocc >= 3 and nvir >= 3 (CCSD_EINVAL otherwise).  Synchronises the stream.
+ * With step timing enabled ccsd_get_triples_times returns the summed device times (ms) of {0: the W GEMM launches,
+ * 1: the energy kernels} of the last call.
+ */
+int ccsd_triples_workspace_bytes(ccsd_ctx* ctx, size_t* bytes);
+int ccsd_triples(ccsd_ctx* ctx, double e_plus_t[2], double e_par_t[2], double e_minus_t[2], void* workspace,
+                 size_t workspace_bytes);
+int ccsd_get_triples_times(ccsd_ctx* ctx, float ms[2]);
+/* Per-term parity hook: the dense, fully antisymmetric blocks Wbar, Zbar, Ybar [a][b][c] (nvir^3 elements each, device;
+ * NULL = skip) of one occupied triple i<j<k.  Asynchronous on the stream after an initial synchronisation. */
+int ccsd_triples_block(ccsd_ctx* ctx, int i, int j, int k, ccsd_c128* Wbar, ccsd_c128* Zbar, ccsd_c128* Ybar,
+                       void* workspace, size_t workspace_bytes);
+
+/*
  * Standalone contractions on caller-supplied tensors (per-term parity and timing; BASELINE config 4).
  *   CCSD_TERM_PP_LADDER (eq 32; string form PAPER.md:176):
  *        in[0] = tau [(i<j)][(c<d)], in[1] = W [(a<b)][(c<d)];  out [(i<j)][(a<b)] = sum_{c<d} W tau

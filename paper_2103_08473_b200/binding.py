@@ -21,7 +21,8 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_zgemm_nt_planes", "ccsd_sum_plane", "ccsd_transpose",
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
-           "ccsd_last_cuda_error"]
+           "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
+           "ccsd_triples_block"]
 
 
 class CCSDError(RuntimeError):
@@ -85,6 +86,10 @@ def load_library():
         lib.ccsd_strerror.argtypes = [ctypes.c_int]
         lib.ccsd_strerror.restype = ctypes.c_char_p
         lib.ccsd_last_cuda_error.restype = ctypes.c_char_p
+        lib.ccsd_triples_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_triples.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3 + [vp, ctypes.c_size_t]
+        lib.ccsd_get_triples_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+        lib.ccsd_triples_block.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, ctypes.c_size_t]
         _LIB = lib
     return _LIB
 
@@ -237,6 +242,38 @@ class CCSD:
         _check(self._lib.ccsd_tensor_elems(self._ctx, tid, ctypes.byref(ne)), "ccsd_tensor_elems")
         out = torch.empty(int(ne.value), dtype=torch.complex128, device="cuda")
         _check(self._lib.ccsd_get_tensor(self._ctx, tid, out.data_ptr()), f"ccsd_get_tensor({name})")
+        return out
+
+    def _triples_workspace(self):
+        torch = self._torch
+        nbytes = ctypes.c_size_t(0)
+        _check(self._lib.ccsd_triples_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_triples_workspace_bytes")
+        ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")
+        return ws, (ws.data_ptr() + 255) // 256 * 256, int(nbytes.value)
+
+    def triples(self) -> dict:
+        """+T / (T) / -T corrections at the current amplitudes (ccsd_triples): {"+T": E, "(T)": E, "-T": E} (complex)."""
+        ws, base, nbytes = self._triples_workspace()
+        a, b, c = (ctypes.c_double * 2)(), (ctypes.c_double * 2)(), (ctypes.c_double * 2)()
+        _check(self._lib.ccsd_triples(self._ctx, a, b, c, base, nbytes), "ccsd_triples")
+        del ws
+        return {"+T": complex(a[0], a[1]), "(T)": complex(b[0], b[1]), "-T": complex(c[0], c[1])}
+
+    def triples_times(self) -> dict:
+        arr = (ctypes.c_float * 2)()
+        _check(self._lib.ccsd_get_triples_times(self._ctx, arr), "ccsd_get_triples_times")
+        return {"w_gemm_ms": float(arr[0]), "energy_ms": float(arr[1])}
+
+    def triples_block(self, i: int, j: int, k: int):
+        """Dense Wbar, Zbar, Ybar [a][b][c] of one occupied triple i<j<k (ccsd_triples_block)."""
+        torch = self._torch
+        ws, base, nbytes = self._triples_workspace()
+        v = self.nvir
+        out = [torch.empty((v, v, v), dtype=torch.complex128, device="cuda") for _ in range(3)]
+        _check(self._lib.ccsd_triples_block(self._ctx, int(i), int(j), int(k), out[0].data_ptr(), out[1].data_ptr(),
+                                            out[2].data_ptr(), base, nbytes), "ccsd_triples_block")
+        torch.cuda.current_stream().synchronize()
+        del ws
         return out
 
     def enable_step_timing(self, enable: bool = True):

@@ -12,6 +12,7 @@
 #include "fill.cuh"
 #include "gemm_simple.cuh"
 #include "gemm_dmma.cuh"
+#include "triples.cuh"
 #include "transpose.cuh"
 #include "reduce.cuh"
 #include "peak.cuh"
@@ -172,6 +173,7 @@ struct ccsd_ctx {
     int timing;
     cudaEvent_t ev[CCSD_NSTEPS + 1];
     float step_ms[CCSD_NSTEPS];
+    float trip_ms[2];
     bool have_residual;
 };
 
@@ -1291,6 +1293,246 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
     }
     }
     CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// ---- perturbative triples (Appendix 7.3; kernels in triples.cuh) ------------------------------
+struct TripWs {
+    c128 *t2u, *t2T, *Uo, *Mbuf;
+    double *t2us, *t2Ts, *Uos, *Vs, *partials, *acc;
+    int4* ijk;
+    int nb, op;
+    int64_t ntrip;
+    bool planes;
+};
+static void trip_carve(const ccsd_ctx* c, char* base, TripWs* w, size_t* total)
+{
+    Carver cv{base, 0};
+    const int64_t o = c->o, v = c->v, vv = c->vv;
+    w->op = (int)round_up(o, 2);
+    w->ntrip = o * (o - 1) * (o - 2) / 6;
+    int64_t nb = ((int64_t)1 << 30) / (vv * v * 16 > 0 ? vv * v * 16 : 1);
+    if (nb < 1) nb = 1;
+    if (nb > 256) nb = 256;
+    if (nb > w->ntrip) nb = w->ntrip > 0 ? w->ntrip : 1;
+    w->nb = (int)nb;
+    w->planes = c->planes && v % 2 == 0;
+    w->t2u = cv.take<c128>(o * o * v * v);
+    w->t2T = cv.take<c128>(o * vv * w->op);
+    w->Uo = cv.take<c128>(o * o * v * w->op);
+    w->Mbuf = cv.take<c128>(nb * vv * v);
+    w->t2us = cv.take<double>(o * o * v * v);
+    w->t2Ts = cv.take<double>(o * vv * w->op);
+    w->Uos = cv.take<double>(o * o * v * w->op);
+    w->Vs = cv.take<double>(o * vv * v);
+    w->partials = cv.take<double>(nb * v * 5);
+    w->acc = cv.take<double>(8);
+    w->ijk = cv.take<int4>(w->ntrip > 0 ? w->ntrip : 1);
+    *total = cv.off;
+}
+
+// operands of the segmented GEMM (triples.cuh) from the current amplitudes and the stored integral classes
+static int trip_prepare(ccsd_ctx* c, const TripWs& w)
+{
+    cudaStream_t st = c->st;
+    const int o = c->o, v = c->v, op = w.op;
+    const int64_t vv = c->vv;
+    const c128 *t2p = c->t2p, *Vooov = c->Vooov_p;
+    double *t2us = w.planes ? w.t2us : nullptr, *t2Ts = w.planes ? w.t2Ts : nullptr, *Uos = w.planes ? w.Uos : nullptr;
+    // t2u[(z,y)][c][e] = t2[z,y,e,c]
+    launch_fill(st, w.t2u, (int64_t)o * o * v, v, v, 0, [=] __device__(int64_t row, int64_t e) {
+        const int64_t zy = row / v;
+        const int cc = (int)(row % v), z = (int)(zy / o), y = (int)(zy % o);
+        c128 x = t2_at(t2p, z, y, (int)e, cc, o, v, vv);
+        if (t2us) t2us[row * v + e] = x.x + x.y;
+        return x;
+    });
+    // t2T[z][(a<b)][m] = t2[z,m,a,b]   (pad m >= o: zero)
+    launch_fill(st, w.t2T, (int64_t)o * vv, op, op, 0, [=] __device__(int64_t row, int64_t m) {
+        const int z = (int)(row / vv);
+        const int64_t AB = row % vv;
+        c128 x = mk(0.0, 0.0);
+        if (m < o && m != z) {
+            x = z < m ? t2p[pair_idx(z, (int)m, o) * vv + AB] : cneg(t2p[pair_idx((int)m, z, o) * vv + AB]);
+        }
+        if (t2Ts) t2Ts[row * op + m] = x.x + x.y;
+        return x;
+    });
+    // Uo[(x,y)][c][m] = <cm||xy> = -conj <xy||mc>   (dagger of the stored class <kl||ic>, reading G5)
+    launch_fill(st, w.Uo, (int64_t)o * o * v, op, op, 0, [=] __device__(int64_t row, int64_t m) {
+        const int64_t xy = row / v;
+        const int cc = (int)(row % v), x = (int)(xy / o), y = (int)(xy % o);
+        c128 r = mk(0.0, 0.0);
+        if (m < o && x != y) {
+            const int64_t P = x < y ? pair_idx(x, y, o) : pair_idx(y, x, o);
+            c128 g = Vooov[(P * o + m) * v + cc];          // <xy||mc> for x<y
+            r = x < y ? mk(-g.x, g.y) : mk(g.x, -g.y);      // -conj(g), sign flipped for x>y
+        }
+        if (Uos) Uos[row * op + m] = r.x + r.y;
+        return r;
+    });
+    if (w.planes) launch_sum_plane(st, c->VvovvT, w.Vs, (int64_t)o * vv * v);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+static int trip_loader(ccsd_ctx* c, const TripWs& w, const TripVariant& V, TripLoader* ld)
+{
+    const int o = c->o, v = c->v, op = w.op;
+    const int64_t vv = c->vv;
+    // A = VvovvT[x][(a<b)][e] = conj <ex||ab> = -<ab||xe>; the sign is absorbed by B = t2[z,y,e,c] = -t2[y,z,e,c]
+    CCSD_TRY(make_operand_map(&ld->PA, c->VvovvT, vv, v, v, o, vv * v, V.bm));
+    CCSD_TRY(make_operand_map(&ld->PB, w.t2u, v, v, v, o * o, (int64_t)v * v, V.bn));
+    CCSD_TRY(make_operand_map(&ld->HA, w.t2T, vv, o, op, o, vv * op, V.bm));
+    CCSD_TRY(make_operand_map(&ld->HB, w.Uo, v, o, op, o * o, (int64_t)v * op, V.bn));
+    ld->PAs = ld->PA; ld->PBs = ld->PB; ld->HAs = ld->HA; ld->HBs = ld->HB;
+    if (V.planes) {
+        CCSD_TRY(make_plane_map(&ld->PAs, w.Vs, vv, v, v, o, vv * v, V.bm));
+        CCSD_TRY(make_plane_map(&ld->PBs, w.t2us, v, v, v, o * o, (int64_t)v * v, V.bn));
+        CCSD_TRY(make_plane_map(&ld->HAs, w.t2Ts, vv, o, op, o, vv * op, V.bm));
+        CCSD_TRY(make_plane_map(&ld->HBs, w.Uos, v, o, op, o * o, (int64_t)v * op, V.bn));
+    }
+    ld->ijk = w.ijk;
+    ld->o = o;
+    ld->tp = (v + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG);
+    ld->th = (o + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG);
+    return CCSD_OK;
+}
+
+static const TripVariant& trip_variant(const ccsd_ctx* c, const TripWs& w)
+{
+    // column-tile width by padded columns x relative cost, as dmma_pick
+    const int v = c->v;
+    const double c32 = (double)round_up(v, 32) * (w.planes ? 1.019 : 1.037), c48 = (double)round_up(v, 48);
+    const int idx = (w.planes ? 2 : 0) + (c48 < c32 ? 1 : 0);
+    return k_trip_variants[idx];
+}
+
+static int trip_gemm(ccsd_ctx* c, const TripWs& w, const TripLoader& ld0, const TripVariant& V, int64_t first, int count)
+{
+    TripLoader ld = ld0;
+    ld.ijk = w.ijk + first;
+    DmmaArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = c->vv; a.N = c->v; a.K = 3 * ((int64_t)c->v + c->o);
+    a.C = w.Mbuf; a.csm = c->v; a.csn = 1; a.bsC = c->vv * c->v;
+    a.alpha = mk(1.0, 0.0); a.accumulate = 0;
+    a.batchA = a.batchB = 1; a.ksplit = 1; a.kchunk = a.K; a.partial = nullptr;
+    dim3 grid((unsigned)((c->v + V.bn - 1) / V.bn), (unsigned)((c->vv + V.bm - 1) / V.bm), (unsigned)count);
+    return V.launch(c->st, ld, a, grid);
+}
+
+static TripData trip_data(const ccsd_ctx* c)
+{
+    TripData d;
+    d.t1 = c->t1; d.t2p = c->t2p; d.Voovv_p = c->Voovv_p; d.f = c->f; d.eps = c->eps;
+    d.o = c->o; d.v = c->v; d.n = c->n; d.vv = c->vv;
+    return d;
+}
+
+int ccsd_triples_workspace_bytes(ccsd_ctx* c, size_t* bytes)
+{
+    if (!c || !bytes) return CCSD_ESTATE;
+    TripWs w;
+    trip_carve(c, nullptr, &w, bytes);
+    return CCSD_OK;
+}
+
+int ccsd_triples(ccsd_ctx* c, double e_plus_t[2], double e_par_t[2], double e_minus_t[2], void* workspace,
+                 size_t workspace_bytes)
+{
+    if (!c) return CCSD_ESTATE;
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0) return CCSD_EINVAL;
+    if (c->o < 3 || c->v < 3) return CCSD_EINVAL;
+    TripWs w;
+    size_t need = 0;
+    trip_carve(c, nullptr, &w, &need);
+    if (workspace_bytes < need) return CCSD_EINVAL;
+    trip_carve(c, static_cast<char*>(workspace), &w, &need);
+    cudaStream_t st = c->st;
+    const int o = c->o, v = c->v;
+    {   // unique occupied triples i<j<k, lexicographic: consecutive triples share the i and j slices of <ab||xe> in L2
+        std::vector<int4> h((size_t)w.ntrip);
+        size_t x = 0;
+        for (int i = 0; i < o; i++)
+            for (int j = i + 1; j < o; j++)
+                for (int k = j + 1; k < o; k++) h[x++] = make_int4(i, j, k, 0);
+        CCSD_CUDA_TRY(cudaMemcpyAsync(w.ijk, h.data(), h.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
+        CCSD_CUDA_TRY(cudaStreamSynchronize(st));   // h goes out of scope
+    }
+    CCSD_TRY(trip_prepare(c, w));
+    const TripVariant& V = trip_variant(c, w);
+    TripLoader ld;
+    CCSD_TRY(trip_loader(c, w, V, &ld));
+    const TripData d = trip_data(c);
+    CCSD_CUDA_TRY(cudaMemsetAsync(w.acc, 0, 8 * sizeof(double), st));
+    cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+    float gemm_ms = 0.f, energy_ms = 0.f;
+    if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
+    for (int64_t first = 0; first < w.ntrip; first += w.nb) {
+        const int count = (int)((w.ntrip - first < w.nb) ? w.ntrip - first : w.nb);
+        if (c->timing) cudaEventRecord(e0, st);
+        CCSD_TRY(trip_gemm(c, w, ld, V, first, count));
+        if (c->timing) cudaEventRecord(e1, st);
+        trip_energy_kernel<<<dim3((unsigned)v, (unsigned)count), TRIP_THREADS, 0, st>>>(d, w.Mbuf, c->vv * v, w.ijk + first, w.partials);
+        trip_reduce_kernel<<<1, 256, 0, st>>>(w.partials, (int64_t)count * v, w.acc);
+        g_launches += 2;
+        if (c->timing) {
+            cudaEventRecord(e2, st);
+            CCSD_CUDA_TRY(cudaEventSynchronize(e2));
+            float a = 0.f, b = 0.f;
+            cudaEventElapsedTime(&a, e0, e1);
+            cudaEventElapsedTime(&b, e1, e2);
+            gemm_ms += a; energy_ms += b;
+        }
+    }
+    if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
+    c->trip_ms[0] = gemm_ms; c->trip_ms[1] = energy_ms;
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 40, w.acc, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(st));
+    CCSD_CUDA_TRY(cudaGetLastError());
+    const double* r = c->red_host + 40;
+    if (e_plus_t) { e_plus_t[0] = r[0]; e_plus_t[1] = 0.0; }
+    if (e_par_t) { e_par_t[0] = r[0] + r[1]; e_par_t[1] = r[2]; }
+    if (e_minus_t) { e_minus_t[0] = r[0] + r[3]; e_minus_t[1] = r[4]; }
+    return CCSD_OK;
+}
+
+int ccsd_triples_block(ccsd_ctx* c, int i, int j, int k, ccsd_c128* Wbar, ccsd_c128* Zbar, ccsd_c128* Ybar, void* workspace,
+                       size_t workspace_bytes)
+{
+    if (!c) return CCSD_ESTATE;
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0) return CCSD_EINVAL;
+    if (c->o < 3 || c->v < 3 || !(0 <= i && i < j && j < k && k < c->o)) return CCSD_EINVAL;
+    TripWs w;
+    size_t need = 0;
+    trip_carve(c, nullptr, &w, &need);
+    if (workspace_bytes < need) return CCSD_EINVAL;
+    trip_carve(c, static_cast<char*>(workspace), &w, &need);
+    cudaStream_t st = c->st;
+    const int4 t = make_int4(i, j, k, 0);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(w.ijk, &t, sizeof(int4), cudaMemcpyHostToDevice, st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(st));
+    CCSD_TRY(trip_prepare(c, w));
+    const TripVariant& V = trip_variant(c, w);
+    TripLoader ld;
+    CCSD_TRY(trip_loader(c, w, V, &ld));
+    CCSD_TRY(trip_gemm(c, w, ld, V, 0, 1));
+    const size_t bytes = (size_t)c->v * c->v * c->v * sizeof(c128);
+    if (Wbar) CCSD_CUDA_TRY(cudaMemsetAsync(Wbar, 0, bytes, st));
+    if (Zbar) CCSD_CUDA_TRY(cudaMemsetAsync(Zbar, 0, bytes, st));
+    if (Ybar) CCSD_CUDA_TRY(cudaMemsetAsync(Ybar, 0, bytes, st));
+    trip_dense_kernel<<<(unsigned)c->v, TRIP_THREADS, 0, st>>>(trip_data(c), w.Mbuf, i, j, k, reinterpret_cast<c128*>(Wbar),
+                                                            reinterpret_cast<c128*>(Zbar), reinterpret_cast<c128*>(Ybar));
+    g_launches++;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_get_triples_times(ccsd_ctx* c, float ms[2])
+{
+    if (!c || !ms) return CCSD_ESTATE;
+    ms[0] = c->trip_ms[0]; ms[1] = c->trip_ms[1];
     return CCSD_OK;
 }
 

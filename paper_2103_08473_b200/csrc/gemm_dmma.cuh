@@ -101,10 +101,43 @@ __device__ __forceinline__ double dsignflip(double x, unsigned mask)
     return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
 
-template <class Cfg>
+// Operand loaders: what one k-iteration (16 complex k) of one CTA stages into shared memory.  The loader is a
+// __grid_constant__ kernel parameter (the tensor maps must live in parameter space for TMA).
+//   setup(p, bz, split, st) -> number of k-iterations of this CTA;   load<Cfg>(st, L, stage, bar, m0, n0) issues the
+//   TMA copies of k-iteration L (exactly Cfg::STAGE bytes; out-of-range rows / k are zero-filled by TMA).
+struct PlainLoader {   // C = A B^T with both operands K-contiguous, optional batch coordinate, split-K
+    CUtensorMap mapA, mapB, mapAs, mapBs;
+    struct State { int64_t kbeg; int cA, cB; };
+    __device__ __forceinline__ int setup(const DmmaArgs& p, int bz, int split, State& st) const
+    {
+        st.kbeg = (int64_t)split * p.kchunk;
+        const int64_t kend = (st.kbeg + p.kchunk < p.K) ? st.kbeg + p.kchunk : p.K;
+        st.cA = p.batchA ? bz : 0;
+        st.cB = p.batchB ? bz : 0;
+        return (int)((kend - st.kbeg + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG));
+    }
+    template <class Cfg>
+    __device__ __forceinline__ void load(const State& st, int L, unsigned char* sa, uint64_t* bar, int m0, int n0) const
+    {
+        unsigned char* sb = sa + Cfg::A_STAGE;
+        const int64_t k0 = st.kbeg + (int64_t)L * 4 * DMMA_BKG;
+#pragma unroll
+        for (int kg = 0; kg < DMMA_BKG; kg++) {
+            const int cd = (int)((k0 + 4 * kg) * 2);   // coordinate in doubles
+            tma_load_3d(sa + kg * Cfg::A_KG, &mapA, cd, m0, st.cA, bar);
+            tma_load_3d(sb + kg * Cfg::B_KG, &mapB, cd, n0, st.cB, bar);
+            if constexpr (Cfg::PL) {
+                unsigned char* sp = sb + Cfg::B_STAGE;
+                tma_load_3d(sp + kg * Cfg::AS_KG, &mapAs, cd / 2, m0, st.cA, bar);
+                tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, &mapBs, cd / 2, n0, st.cB, bar);
+            }
+        }
+    }
+};
+
+template <class Cfg, class Loader>
 __global__ void __launch_bounds__(Cfg::THREADS, 1)
-gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
-                 const __grid_constant__ CUtensorMap mapAs, const __grid_constant__ CUtensorMap mapBs, DmmaArgs p)
+gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
 {
     constexpr int MI = Cfg::MI, NJ = Cfg::NJ, S = Cfg::STAGES, D = Cfg::STAGES - 2;
     constexpr int A_KG = Cfg::A_KG, B_KG = Cfg::B_KG, A_STAGE = Cfg::A_STAGE, STAGE = Cfg::STAGE;
@@ -115,10 +148,8 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int bz = blockIdx.z / p.ksplit, split = blockIdx.z % p.ksplit;
     const int64_t m0 = (int64_t)blockIdx.y * Cfg::BM, n0 = (int64_t)blockIdx.x * Cfg::BN;
-    const int64_t kbeg = (int64_t)split * p.kchunk;
-    const int64_t kend = (kbeg + p.kchunk < p.K) ? kbeg + p.kchunk : p.K;
-    const int kt = (int)((kend - kbeg + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG));
-    const int cA = p.batchA ? bz : 0, cB = p.batchB ? bz : 0;
+    typename Loader::State lst;
+    const int kt = ld.setup(p, bz, split, lst);
 
     // TMA for k-iteration L into stage L % S (one elected lane).  It is issued D = S - 2 iterations ahead, so the
     // stage it overwrites was released by every warp at least one whole iteration ago: the wait never spins long.
@@ -126,20 +157,7 @@ gemm_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         const int s = L % S;
         if (L >= S) mbar_wait(&empty[s], ((L / S) & 1) ^ 1);
         mbar_expect_tx(&full[s], STAGE);
-        unsigned char* sa = smem + s * STAGE;
-        unsigned char* sb = sa + A_STAGE;
-        const int64_t k0 = kbeg + (int64_t)L * 4 * DMMA_BKG;
-#pragma unroll
-        for (int kg = 0; kg < DMMA_BKG; kg++) {
-            const int cd = (int)((k0 + 4 * kg) * 2);   // coordinate in doubles
-            tma_load_3d(sa + kg * A_KG, &mapA, cd, (int)m0, cA, &full[s]);
-            tma_load_3d(sb + kg * B_KG, &mapB, cd, (int)n0, cB, &full[s]);
-            if constexpr (Cfg::PL) {
-                unsigned char* sp = sb + Cfg::B_STAGE;
-                tma_load_3d(sp + kg * Cfg::AS_KG, &mapAs, cd / 2, (int)m0, cA, &full[s]);
-                tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, &mapBs, cd / 2, (int)n0, cB, &full[s]);
-            }
-        }
+        ld.template load<Cfg>(lst, L, smem + s * STAGE, &full[s], (int)m0, (int)n0);
     };
 
     if (threadIdx.x == 0) {
@@ -373,10 +391,12 @@ static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtenso
 {
     static bool configured = false;
     if (!configured) {
-        CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
+        CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg, PlainLoader>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
         configured = true;
     }
-    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(mA, mB, mAs, mBs, a);
+    PlainLoader ld;
+    ld.mapA = mA; ld.mapB = mB; ld.mapAs = mAs; ld.mapBs = mBs;
+    gemm_dmma_kernel<Cfg, PlainLoader><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(ld, a);
     g_launches++;
     return CCSD_OK;
 }

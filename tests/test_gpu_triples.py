@@ -1,0 +1,117 @@
+"""GPU parity of the perturbative triples (Appendix 7.3) against the triples oracle.
+
+Per-term: the dense blocks Wbar, Zbar, Ybar [a][b][c] of sampled occupied triples, element by element (1e-12 relative
+max-abs).  Energies: E(+T), E((T)), E(-T) (Re and Im) within 1e-10 Eh at seeded random amplitudes and at the oracle's
+CCSD iterate.  Shapes: cfg0, a ragged one (several DMMA tiles with tails in every dimension, odd nvir -> the kernel
+variant without sum planes), cfg1 (sampled blocks live, energies against tests/golden/oracle_triples_cfg1.txt).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import ccsd_inputs as ci
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-12
+E_TOL = 1e-10
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2103_08473_b200 as lib
+    lib.load_library()
+    return lib
+
+
+def _rel(a, b):
+    scale = np.abs(b).max()
+    return np.abs(np.asarray(a) - np.asarray(b)).max() / (scale if scale > 0 else 1.0)
+
+
+def _pair(cfg):
+    from oracle.ccsd_oracle import OracleCCSD
+    if cfg == "ragged":
+        inp = ci.make_inputs(7, 29, 37, seed=4711)
+    elif cfg == "ragged_even":
+        inp = ci.make_inputs(5, 38, 30, seed=4712)
+    else:
+        inp = ci.make_config(cfg)
+    oc = OracleCCSD(inp.h, inp.B, inp.nocc, inp.nvir, restricted=inp.nvir > 40)
+    return inp, oc
+
+
+@pytest.mark.parametrize("cfg,scale,triples", [
+    ("cfg0", 0.2, [(0, 1, 2), (0, 1, 3), (1, 2, 3)]),
+    ("ragged", 0.05, [(0, 1, 2), (1, 3, 6), (4, 5, 6)]),
+    ("ragged_even", 0.05, [(0, 2, 4), (2, 3, 4)]),
+    ("cfg1", 0.01, [(0, 1, 2), (3, 9, 15), (13, 14, 15)]),
+])
+def test_triples_blocks_match_oracle(gpu, cfg, scale, triples):
+    from oracle.ccsd_oracle import unpack_t2
+    from oracle.triples_oracle import OracleTriples
+    inp, oc = _pair(cfg)
+    o, v = inp.nocc, inp.nvir
+    t1, t2p = ci.random_amplitudes(o, v, 33, scale)
+    ot = OracleTriples(oc, t1=t1, t2=unpack_t2(t2p, o, v))
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc.set_amplitudes(t1, t2p)
+    for (i, j, k) in triples:
+        Wg, Zg, Yg = (x.cpu().numpy() for x in gc.triples_block(i, j, k))
+        assert _rel(Wg, ot.W(i, j, k)[1]) <= REL_TOL, ("W", i, j, k)
+        assert _rel(Zg, ot.Z(i, j, k)[1]) <= REL_TOL, ("Z", i, j, k)
+        assert _rel(Yg, ot.Y(i, j, k)[1]) <= REL_TOL, ("Y", i, j, k)
+    gc.close()
+
+
+@pytest.mark.parametrize("cfg,scale", [("cfg0", 0.2), ("ragged", 0.05), ("ragged_even", 0.05)])
+def test_triples_energies_match_oracle(gpu, cfg, scale):
+    from oracle.ccsd_oracle import unpack_t2
+    from oracle.triples_oracle import OracleTriples
+    inp, oc = _pair(cfg)
+    o, v = inp.nocc, inp.nvir
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    # (a) seeded random amplitudes, (b) the CCSD iterate after three oracle iterations
+    t1, t2p = ci.random_amplitudes(o, v, 34, scale)
+    cases = [(t1, unpack_t2(t2p, o, v), t2p)]
+    for _ in range(3):
+        oc.iterate()
+    from oracle.ccsd_oracle import pack_t2
+    cases.append((oc.t1.copy(), oc.t2.copy(), pack_t2(oc.t2)))
+    for a1, a2, a2p in cases:
+        ref = OracleTriples(oc, t1=a1, t2=a2).energies(restricted=True)
+        gc.set_amplitudes(a1, a2p)
+        got = gc.triples()
+        for key in ("+T", "(T)", "-T"):
+            assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
+        assert abs(ref["+T"]) > 1e-9
+    gc.close()
+
+
+def test_triples_energies_cfg1_against_oracle_golden(gpu):
+    """cfg1 (16/96): 560 occupied triples; the oracle needs minutes, so its energies at the seeded amplitudes
+    CN(0, 0.01^2) (seed 35) are stored by tests/golden/make_oracle_triples.py (oracle/ only)."""
+    path = os.path.join(GOLDEN, "oracle_triples_cfg1.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated")
+    ref = {}
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            key, re, im = line.split()
+            ref[key] = complex(float(re), float(im))
+    inp = ci.make_config("cfg1")
+    o, v = inp.nocc, inp.nvir
+    t1, t2p = ci.random_amplitudes(o, v, 35, 0.01)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc.set_amplitudes(t1, t2p)
+    got = gc.triples()
+    for key in ("+T", "(T)", "-T"):
+        assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
+    gc.close()
