@@ -263,6 +263,39 @@ def cc2_bench(torch, pkg, inp, o, v, steps=5, warmup=3):
             "note": "eq 34 evaluated as eq 32 at t2 = 0 plus the two Fock terms; singles by eq 33"}
 
 
+def triples_bench(torch, pkg, inp, o, v, peak_tflops):
+    """NEXT-3 row of SURVEY 8(f): +T / (T) / -T at the amplitudes after two CCSD iterations.
+    One timed call without per-launch events (wall clock around a synchronising call), one with (kernel split)."""
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    for _ in range(2):
+        solver.iterate()
+    solver.triples()                                   # warm-up: function attributes, L2
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    en = solver.triples()
+    e1.record()
+    torch.cuda.synchronize()
+    total_ms = e0.elapsed_time(e1)
+    solver.enable_step_timing(True)
+    solver.triples()
+    tm = solver.triples_times()
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    vv, nt = ci.pair_count(v), o * (o - 1) * (o - 2) // 6
+    cmac = nt * vv * v * 3 * (v + o)                   # unique i<j<k, rows a<b, K = 3v + 3o
+    rf = pkg.real_flops_per_cmac()
+    tf8 = 8.0 * cmac / (tm["w_gemm_ms"] * 1e-3) * 1e-12
+    return {"seconds": round(total_ms * 1e-3, 4), "occupied_triples": nt, "w_gemm_ms": round(tm["w_gemm_ms"], 2),
+            "energy_kernels_ms": round(tm["energy_ms"], 2), "w_gemm_tflops": round(tf8, 2),
+            "w_gemm_frac_fp64_peak": round(tf8 * rf / 8.0 / peak_tflops, 4),
+            "E(+T)": [en["+T"].real, en["+T"].imag], "E((T))": [en["(T)"].real, en["(T)"].imag],
+            "E(-T)": [en["-T"].real, en["-T"].imag],
+            "note": "one K-segmented DMMA GEMM (vv x v x (3v+3o)) per occupied triple i<j<k; fraction of peak on the "
+                    "executed (3M) flops"}
+
+
 def max_over_ranks(value: float, dist, device="cuda") -> float:
     """Multi-GPU numbers are the MAX over ranks (replicas-only path: no data-path collective exists)."""
     import torch
@@ -423,6 +456,7 @@ def run_ours(args) -> None:
     del solver
     torch.cuda.empty_cache()
     cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
+    triples = triples_bench(torch, pkg, inp, o, v, peak) if not args.no_sweep else None
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
     cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
@@ -446,7 +480,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "cc2": cc2, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "triples": triples, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:

@@ -81,3 +81,50 @@ class OracleTriples:
         lib().oracle_triples_energies(self.o, v, int(bool(restricted)), _p(self.eps), _p(self.fov), _p(self.t1),
                                       _p(self.t2), _p(self.vvov), _p(self.vooo), _p(self.vvoo), _p(work), _p(out))
         return {"+T": complex(out[0]), "(T)": complex(out[0] + out[1]), "-T": complex(out[0] + out[2])}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# single-element evaluator straight from the factorised integrals (full-size spot checks at cfg2 / cfg3, where the
+# plain-loop oracle would need hours): eq 40 + the cyclic sum written out for one (i,j,k,a,b,c).
+# ---------------------------------------------------------------------------------------------------------------
+def _g(B, p, q, r, s):
+    """<pq||rs> = (pr|qs) - (ps|qr), (pq|rs) = sum_L B[L,p,q] B[L,r,s]; any of p,q,r,s may be an index array."""
+    return np.einsum("l...,l...->...", B[:, p, r], B[:, q, s]) - np.einsum("l...,l...->...", B[:, p, s], B[:, q, r])
+
+
+def _t2(t2p, o, v, i, j, a, b):
+    """signed lookup t2[i,j,a,b] in the packed array [(i<j)][(a<b)]; a or b may be arrays (the other scalar)."""
+    if i == j:
+        return np.zeros(np.broadcast(a, b).shape, dtype=C128)
+    sg = 1.0
+    if i > j:
+        i, j, sg = j, i, -sg
+    row = t2p[i * o - i * (i + 1) // 2 + (j - i - 1)]
+    a, b = np.broadcast_arrays(np.asarray(a), np.asarray(b))
+    lo, hi = np.minimum(a, b), np.maximum(a, b)
+    idx = lo * v - lo * (lo + 1) // 2 + (hi - lo - 1)
+    val = np.where(a == b, 0.0, row[np.where(a == b, 0, idx)])
+    return sg * np.where(a < b, 1.0, -1.0) * val
+
+
+def w_element_from_B(B, nocc, t2p, i, j, k, a, b, c):
+    """W[i,j,k,a,b,c] of eq 40 (reading G22) for one index sextuple."""
+    o, v = nocc, B.shape[1] - nocc
+    e = np.arange(v)
+    m = np.arange(o)
+    s = 0.0
+    for (x, y, z) in ((i, j, k), (j, k, i), (k, i, j)):
+        s += np.sum(_g(B, o + a, o + b, x, o + e) * _t2(t2p, o, v, y, z, e, c))          # <ab||xe> t2[y,z,e,c]
+        gm = _g(B, o + a, m, x, y)                                                       # <am||xy>
+        tm = np.array([_t2(t2p, o, v, z, mm, b, c) for mm in range(o)]).reshape(o)       # t2[z,m,b,c]
+        s += np.sum(gm * tm)
+    return s
+
+
+def wbar_samples_from_B(B, nocc, t2p, ijk, abc):
+    """Wbar = W^abc + W^bca + W^cab at sampled (i,j,k), (a,b,c)."""
+    out = np.zeros(len(ijk), dtype=C128)
+    for n, ((i, j, k), (a, b, c)) in enumerate(zip(ijk, abc)):
+        out[n] = (w_element_from_B(B, nocc, t2p, i, j, k, a, b, c) + w_element_from_B(B, nocc, t2p, i, j, k, b, c, a) +
+                  w_element_from_B(B, nocc, t2p, i, j, k, c, a, b))
+    return out

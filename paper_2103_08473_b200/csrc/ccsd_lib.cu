@@ -1298,7 +1298,7 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
 
 // ---- perturbative triples (Appendix 7.3; kernels in triples.cuh) ------------------------------
 struct TripWs {
-    c128 *t2u, *t2T, *Uo, *Mbuf;
+    c128 *t2u, *t2T, *Uo, *Mcbuf;
     double *t2us, *t2Ts, *Uos, *Vs, *partials, *acc;
     int4* ijk;
     int nb, op;
@@ -1311,7 +1311,7 @@ static void trip_carve(const ccsd_ctx* c, char* base, TripWs* w, size_t* total)
     const int64_t o = c->o, v = c->v, vv = c->vv;
     w->op = (int)round_up(o, 2);
     w->ntrip = o * (o - 1) * (o - 2) / 6;
-    int64_t nb = ((int64_t)1 << 30) / (vv * v * 16 > 0 ? vv * v * 16 : 1);
+    int64_t nb = ((int64_t)1 << 30) / (vv * v * 16 > 0 ? vv * v * 16 : 1);   // Mc of a batch: <= 1 GiB
     if (nb < 1) nb = 1;
     if (nb > 256) nb = 256;
     if (nb > w->ntrip) nb = w->ntrip > 0 ? w->ntrip : 1;
@@ -1320,7 +1320,7 @@ static void trip_carve(const ccsd_ctx* c, char* base, TripWs* w, size_t* total)
     w->t2u = cv.take<c128>(o * o * v * v);
     w->t2T = cv.take<c128>(o * vv * w->op);
     w->Uo = cv.take<c128>(o * o * v * w->op);
-    w->Mbuf = cv.take<c128>(nb * vv * v);
+    w->Mcbuf = cv.take<c128>(nb * vv * v);
     w->t2us = cv.take<double>(o * o * v * v);
     w->t2Ts = cv.take<double>(o * vv * w->op);
     w->Uos = cv.take<double>(o * o * v * w->op);
@@ -1415,7 +1415,7 @@ static int trip_gemm(ccsd_ctx* c, const TripWs& w, const TripLoader& ld0, const 
     DmmaArgs a;
     memset(&a, 0, sizeof(a));
     a.M = c->vv; a.N = c->v; a.K = 3 * ((int64_t)c->v + c->o);
-    a.C = w.Mbuf; a.csm = c->v; a.csn = 1; a.bsC = c->vv * c->v;
+    a.C = w.Mcbuf; a.csm = 1; a.csn = c->vv; a.bsC = c->vv * c->v;          // stored transposed: Mc[c][(a<b)]
     a.alpha = mk(1.0, 0.0); a.accumulate = 0;
     a.batchA = a.batchB = 1; a.ksplit = 1; a.kchunk = a.K; a.partial = nullptr;
     dim3 grid((unsigned)((c->v + V.bn - 1) / V.bn), (unsigned)((c->vv + V.bm - 1) / V.bm), (unsigned)count);
@@ -1474,8 +1474,9 @@ int ccsd_triples(ccsd_ctx* c, double e_plus_t[2], double e_par_t[2], double e_mi
         if (c->timing) cudaEventRecord(e0, st);
         CCSD_TRY(trip_gemm(c, w, ld, V, first, count));
         if (c->timing) cudaEventRecord(e1, st);
-        trip_energy_kernel<<<dim3((unsigned)v, (unsigned)count), TRIP_THREADS, 0, st>>>(d, w.Mbuf, c->vv * v, w.ijk + first, w.partials);
-        trip_reduce_kernel<<<1, 256, 0, st>>>(w.partials, (int64_t)count * v, w.acc);
+        trip_energy_kernel<<<dim3((unsigned)(v - 2), (unsigned)count), TRIP_THREADS, 0, st>>>(d, w.Mcbuf, c->vv * v, w.ijk + first,
+                                                                                           c->pv, w.partials);
+        trip_reduce_kernel<<<1, 256, 0, st>>>(w.partials, (int64_t)count * (v - 2), w.acc);
         g_launches += 2;
         if (c->timing) {
             cudaEventRecord(e2, st);
@@ -1522,7 +1523,7 @@ int ccsd_triples_block(ccsd_ctx* c, int i, int j, int k, ccsd_c128* Wbar, ccsd_c
     if (Wbar) CCSD_CUDA_TRY(cudaMemsetAsync(Wbar, 0, bytes, st));
     if (Zbar) CCSD_CUDA_TRY(cudaMemsetAsync(Zbar, 0, bytes, st));
     if (Ybar) CCSD_CUDA_TRY(cudaMemsetAsync(Ybar, 0, bytes, st));
-    trip_dense_kernel<<<(unsigned)c->v, TRIP_THREADS, 0, st>>>(trip_data(c), w.Mbuf, i, j, k, reinterpret_cast<c128*>(Wbar),
+    trip_dense_kernel<<<(unsigned)(c->v - 2), TRIP_THREADS, 0, st>>>(trip_data(c), w.Mcbuf, c->pv, i, j, k, reinterpret_cast<c128*>(Wbar),
                                                             reinterpret_cast<c128*>(Zbar), reinterpret_cast<c128*>(Ybar));
     g_launches++;
     CCSD_CUDA_TRY(cudaGetLastError());

@@ -6,7 +6,7 @@
 //                  + sum_m ( <cm||ij> t2[k,m,a,b] + <cm||jk> t2[i,m,a,b] + <cm||ki> t2[j,m,a,b] )          3 x o
 // (the hole terms of eq 40, sum_m <am||ij> t2[k,m,b,c], are antisymmetric in (b,c) instead of (a,b); stored with
 // their lone index last they share the layout of the particle terms), so that for a<b<c
-//     Wbar[a,b,c] = W^abc + W^bca + W^cab = Mt[(ab)][c] + Mt[(bc)][a] - Mt[(ac)][b].
+//     Wbar[a,b,c] = W^abc + W^bca + W^cab = Mt[(ab)][c] + Mt[(bc)][a] - Mt[(ac)][b]      (Mt is stored transposed).
 // Zbar (eq 42) and Ybar (eq 44) have the same cyclic structure with rank-3 "matrices" formed on the fly.  A batch of
 // triples is one launch (grid.z); the three energies are reduced deterministically (per-block partials, fixed order).
 // The paper blocks the occupied space to bound the n_red^3 v^3 working set; here the batch of triples
@@ -125,13 +125,16 @@ __device__ __forceinline__ void trip_zy(const TripData& d, const TripPairs& tp, 
         cfma(Y, T, t);
     }
 }
-// Wbar, Zbar, Ybar of one (i<j<k, a<b<c)
-__device__ __forceinline__ void trip_element(const TripData& d, const TripPairs& tp, const c128* __restrict__ Mt, int i, int j,
-                                             int k, int a, int b, int c, c128& W, c128& Z, c128& Y)
+// Wbar, Zbar, Ybar of one (i<j<k, a<b<c).  The GEMM writes its result transposed, Mc[c][(a<b)] = Mt[(a<b)][c], so that
+// for consecutive (b<c) pairs at fixed a two of the three reads (and every read of the pair-indexed tensors) are
+// contiguous; a second, row-major copy for the third read costs more in the GEMM epilogue than it saves here.
+__device__ __forceinline__ void trip_element(const TripData& d, const TripPairs& tp,
+                                             const c128* __restrict__ Mc, int i, int j, int k, int a, int b, int c,
+                                             int64_t AB, int64_t BC, c128& W, c128& Z, c128& Y)
 {
     const int v = d.v;
-    const int64_t AB = pair_idx(a, b, v), BC = pair_idx(b, c, v), AC = pair_idx(a, c, v);
-    W = csub(cadd(Mt[AB * v + c], Mt[BC * v + a]), Mt[AC * v + b]);
+    const int64_t AC = pair_idx(a, c, v);
+    W = csub(cadd(Mc[c * d.vv + AB], Mc[a * d.vv + BC]), Mc[b * d.vv + AC]);
     c128 z1 = mk(0, 0), y1 = mk(0, 0), z2 = mk(0, 0), y2 = mk(0, 0), z3 = mk(0, 0), y3 = mk(0, 0);
     trip_zy(d, tp, AB, c, z1, y1);
     trip_zy(d, tp, BC, a, z2, y2);
@@ -148,31 +151,31 @@ __device__ __forceinline__ void trip_element(const TripData& d, const TripPairs&
     Y = cadd(Y, det);
 }
 
-constexpr int TRIP_THREADS = 128;
-// grid (v, nb): block (a, batch entry); partials[(bz*v + a)*5 + {0..4}] = sums over b, c of
+constexpr int TRIP_THREADS = 256;
+// grid (v - 2, nb): block (a, batch entry); the threads walk the packed pairs (b<c) with b > a, which are the
+// contiguous tail [pair_idx(a+1, a+2), vv) of the pair table.  partials[(bz*gridDim.x + a)*5 + {0..4}] = sums of
 //   |Wbar|^2/D, Re/Im conj(Zbar) Wbar / D, Re/Im conj(Ybar) Wbar        (eqs 39, 41, 43 over a<b<c)
-__global__ void __launch_bounds__(TRIP_THREADS) trip_energy_kernel(TripData d, const c128* __restrict__ Mbuf, int64_t bsM,
-                                                                   const int4* __restrict__ ijk, double* __restrict__ partials)
+__global__ void __launch_bounds__(TRIP_THREADS) trip_energy_kernel(TripData d, const c128* __restrict__ Mcbuf, int64_t bsM,
+                                                                   const int4* __restrict__ ijk, const int2* __restrict__ pv,
+                                                                   double* __restrict__ partials)
 {
     const int a = blockIdx.x, bz = blockIdx.y, v = d.v, o = d.o;
     const int4 t = ijk[bz];
     const int i = t.x, j = t.y, k = t.z;
-    const c128* Mt = Mbuf + (int64_t)bz * bsM;
+    const c128* Mc = Mcbuf + (int64_t)bz * bsM;
     const TripPairs tp = trip_pairs(i, j, k, o);
-    const double eo = d.eps[i] + d.eps[j] + d.eps[k];
+    const double eoa = d.eps[i] + d.eps[j] + d.eps[k] - d.eps[o + a];
     double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    for (int b = a + 1; b < v - 1; b++) {
-        const double eab = eo - d.eps[o + a] - d.eps[o + b];
-        for (int c = b + 1 + threadIdx.x; c < v; c += TRIP_THREADS) {
-            c128 W, Z, Y;
-            trip_element(d, tp, Mt, i, j, k, a, b, c, W, Z, Y);
-            const double rD = 1.0 / (eab - d.eps[o + c]);
-            acc[0] += (W.x * W.x + W.y * W.y) * rD;
-            acc[1] += (Z.x * W.x + Z.y * W.y) * rD;     // Re conj(Z) W
-            acc[2] += (Z.x * W.y - Z.y * W.x) * rD;     // Im conj(Z) W
-            acc[3] += Y.x * W.x + Y.y * W.y;
-            acc[4] += Y.x * W.y - Y.y * W.x;
-        }
+    for (int64_t BC = pair_idx(a + 1, a + 2, v) + threadIdx.x; BC < d.vv; BC += TRIP_THREADS) {
+        const int2 bc = pv[BC];
+        c128 W, Z, Y;
+        trip_element(d, tp, Mc, i, j, k, a, bc.x, bc.y, pair_idx(a, bc.x, v), BC, W, Z, Y);
+        const double rD = 1.0 / (eoa - d.eps[o + bc.x] - d.eps[o + bc.y]);
+        acc[0] += (W.x * W.x + W.y * W.y) * rD;
+        acc[1] += (Z.x * W.x + Z.y * W.y) * rD;     // Re conj(Z) W
+        acc[2] += (Z.x * W.y - Z.y * W.x) * rD;     // Im conj(Z) W
+        acc[3] += Y.x * W.x + Y.y * W.y;
+        acc[4] += Y.x * W.y - Y.y * W.x;
     }
     __shared__ double sh[TRIP_THREADS / 32][5];
 #pragma unroll
@@ -186,7 +189,7 @@ __global__ void __launch_bounds__(TRIP_THREADS) trip_energy_kernel(TripData d, c
     if (threadIdx.x < 5) {
         double x = 0.0;
         for (int w = 0; w < TRIP_THREADS / 32; w++) x += sh[w][threadIdx.x];
-        partials[((int64_t)bz * v + a) * 5 + threadIdx.x] = x;
+        partials[((int64_t)bz * gridDim.x + a) * 5 + threadIdx.x] = x;
     }
 }
 // acc[q] += sum over `count` blocks of partials[.][q], in a fixed order (one block, deterministic)
@@ -213,23 +216,24 @@ __global__ void __launch_bounds__(256) trip_reduce_kernel(const double* __restri
 }
 
 // parity hook: dense, fully antisymmetric Wbar/Zbar/Ybar[a][b][c] of ONE triple (buffers zeroed by the caller)
-__global__ void __launch_bounds__(TRIP_THREADS) trip_dense_kernel(TripData d, const c128* __restrict__ Mt, int i, int j, int k,
+__global__ void __launch_bounds__(TRIP_THREADS) trip_dense_kernel(TripData d, const c128* __restrict__ Mc,
+                                                                  const int2* __restrict__ pv, int i, int j, int k,
                                                                   c128* __restrict__ Wd, c128* __restrict__ Zd, c128* __restrict__ Yd)
 {
     const int a = blockIdx.x, v = d.v;
     const TripPairs tp = trip_pairs(i, j, k, d.o);
-    for (int b = a + 1; b < v - 1; b++)
-        for (int c = b + 1 + threadIdx.x; c < v; c += TRIP_THREADS) {
-            c128 W, Z, Y;
-            trip_element(d, tp, Mt, i, j, k, a, b, c, W, Z, Y);
-            const int64_t idx[6] = {((int64_t)a * v + b) * v + c, ((int64_t)b * v + c) * v + a, ((int64_t)c * v + a) * v + b,
-                                    ((int64_t)b * v + a) * v + c, ((int64_t)a * v + c) * v + b, ((int64_t)c * v + b) * v + a};
+    for (int64_t BC = pair_idx(a + 1, a + 2, v) + threadIdx.x; BC < d.vv; BC += TRIP_THREADS) {
+        const int b = pv[BC].x, c = pv[BC].y;
+        c128 W, Z, Y;
+        trip_element(d, tp, Mc, i, j, k, a, b, c, pair_idx(a, b, v), BC, W, Z, Y);
+        const int64_t idx[6] = {((int64_t)a * v + b) * v + c, ((int64_t)b * v + c) * v + a, ((int64_t)c * v + a) * v + b,
+                                ((int64_t)b * v + a) * v + c, ((int64_t)a * v + c) * v + b, ((int64_t)c * v + b) * v + a};
 #pragma unroll
-            for (int q = 0; q < 6; q++) {
-                const double sg = q < 3 ? 1.0 : -1.0;
-                if (Wd) Wd[idx[q]] = cscale(sg, W);
-                if (Zd) Zd[idx[q]] = cscale(sg, Z);
-                if (Yd) Yd[idx[q]] = cscale(sg, Y);
-            }
+        for (int q = 0; q < 6; q++) {
+            const double sg = q < 3 ? 1.0 : -1.0;
+            if (Wd) Wd[idx[q]] = cscale(sg, W);
+            if (Zd) Zd[idx[q]] = cscale(sg, Z);
+            if (Yd) Yd[idx[q]] = cscale(sg, Y);
         }
+    }
 }

@@ -162,3 +162,27 @@ def test_cfg4_isolated_ladder_sampled(gpu, k):
     if vv <= 20000:
         R4 = gpu.contract("pp_ladder", o, v, [tau, W], gemm_mode=2)
         assert float((R4 - R).abs().max()) <= REL_TOL * float(R.abs().max())
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg3"])
+def test_fullsize_triples_driver_sampled(gpu, cfg):
+    """Perturbative triples at full size: sampled elements of Wbar (eq 40 + cyclic sum) of three
+    occupied triples against the oracle's single-element evaluator from B (pinned to the plain-loop oracle on CPU)."""
+    from oracle.triples_oracle import wbar_samples_from_B
+    inp = ci.make_config(cfg)
+    o, v = inp.nocc, inp.nvir
+    t1, t2p = ci.random_amplitudes(o, v, 36, 0.01)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc.set_amplitudes(t1, t2p)
+    rng = np.random.default_rng(99)
+    for (i, j, k) in [(0, 1, 2), (o - 3, o - 2, o - 1), tuple(sorted(rng.choice(o, 3, replace=False)))]:
+        W = gc.triples_block(int(i), int(j), int(k))[0]
+        abc = [(0, 1, 2), (v - 3, v - 2, v - 1), (0, v // 2, v - 1), (v - 1, 0, 5)] + \
+              [tuple(int(x) for x in rng.choice(v, 3, replace=False)) for _ in range(8)]
+        ref = wbar_samples_from_B(inp.B, o, t2p, [(int(i), int(j), int(k))] * len(abc), abc)
+        got = np.array([complex(W[a, b, c]) for (a, b, c) in abc])
+        assert np.abs(got - ref).max() <= REL_TOL * float(W.abs().max())
+        del W
+    e = gc.triples()
+    assert e["+T"].real < 0 and e["+T"].imag == 0.0
+    gc.close()

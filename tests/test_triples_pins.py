@@ -125,3 +125,18 @@ def test_q5_real_under_kramers_symmetry_complex_otherwise():
     oc.run(6)
     e = OracleTriples(oc).energies()
     assert abs(e["+T"].imag) < 1e-17 and abs(e["(T)"].imag) > 1e-12
+
+
+def test_q6_single_element_evaluator_equals_plain_loop_oracle():
+    """The from-B evaluator used for the full-size GPU spot checks equals the plain-loop oracle on a ragged system."""
+    from oracle.ccsd_oracle import pack_t2
+    from oracle.triples_oracle import wbar_samples_from_B
+    o, v = 5, 7
+    inp, oc, t1, t2 = _setup(o, v, 77)
+    ot = OracleTriples(oc)
+    rng = np.random.default_rng(3)
+    ijk = [(0, 1, 2), (1, 3, 4), (0, 2, 4)]
+    abc = [tuple(rng.permutation(v)[:3]) for _ in ijk]
+    got = wbar_samples_from_B(inp.B, o, pack_t2(t2), ijk, abc)
+    ref = np.array([ot.W(*t)[1][x] for t, x in zip(ijk, abc)])
+    assert np.abs(got - ref).max() < 1e-13 * np.abs(ref).max() + 1e-15
