@@ -349,6 +349,13 @@ def run_ours(args) -> None:
         return
     inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
     pkg.load_library()
+    if args.only_triples:
+        # profiling aid: ccsd_init, one iteration, then the perturbative triples of this workload (same launches as
+        # the "triples" leg of the default run)
+        peak = pkg.measure_fp64_peak(4)
+        print(json.dumps({"metric": "triples_seconds", "unit": "s", "config": {"workload": f"{cfg} +T/(T)/-T"},
+                          **triples_bench(torch, pkg, inp, o, v, peak)}))
+        return
     pkg.launch_count(reset=True)
     t0 = time.perf_counter()
     solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
@@ -496,6 +503,7 @@ def main():
     ap.add_argument("--config", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
+    ap.add_argument("--only-triples", action="store_true", help="time only the perturbative triples of --config")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -18,6 +18,7 @@
 // Out-of-range rows / k are zero-filled by TMA, so ragged M, N, K need no special code in the main loop.
 #pragma once
 #include <cuda.h>
+#include <cstdlib>
 #include "gemm_simple.cuh"
 
 constexpr int DMMA_BKG = 4;         // k-groups (of 4 complex) per pipeline stage -> BK = 16 complex
@@ -89,6 +90,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
         ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
 {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -107,6 +114,12 @@ __device__ __forceinline__ double dsignflip(double x, unsigned mask)
 //   TMA copies of k-iteration L (exactly Cfg::STAGE bytes; out-of-range rows / k are zero-filled by TMA).
 struct PlainLoader {   // C = A B^T with both operands K-contiguous, optional batch coordinate, split-K
     CUtensorMap mapA, mapB, mapAs, mapBs;
+    // wide = 1: the maps are 4-d views {4 complex k, row, k-group, batch} (k-group stride 64 bytes), so that ONE copy per
+    // operand fills a whole stage in the [k-group][row][64 B] layout (4 instead of 16 TMA instructions per k-iteration:
+    // the issuing warp issues no DMMA meanwhile, and that time is lost to its SM sub-partition).  Needs K % 4 == 0,
+    // because a partial last k-group cannot be zero-filled through the bounds of such a view; wide = 0: 3-d maps
+    // {k, row, batch} with one copy per k-group.
+    int wide;
     struct State { int64_t kbeg; int cA, cB; };
     __device__ __forceinline__ int setup(const DmmaArgs& p, int bz, int split, State& st) const
     {
@@ -121,6 +134,17 @@ struct PlainLoader {   // C = A B^T with both operands K-contiguous, optional ba
     {
         unsigned char* sb = sa + Cfg::A_STAGE;
         const int64_t k0 = st.kbeg + (int64_t)L * 4 * DMMA_BKG;
+        if (wide) {
+            const int gk = (int)(k0 / 4);
+            tma_load_4d(sa, &mapA, 0, m0, gk, st.cA, bar);
+            tma_load_4d(sb, &mapB, 0, n0, gk, st.cB, bar);
+            if constexpr (Cfg::PL) {
+                unsigned char* sp = sb + Cfg::B_STAGE;
+                tma_load_4d(sp, &mapAs, 0, m0, gk, st.cA, bar);
+                tma_load_4d(sp + DMMA_BKG * Cfg::AS_KG, &mapBs, 0, n0, gk, st.cB, bar);
+            }
+            return;
+        }
 #pragma unroll
         for (int kg = 0; kg < DMMA_BKG; kg++) {
             const int cd = (int)((k0 + 4 * kg) * 2);   // coordinate in doubles
@@ -346,6 +370,29 @@ static int make_operand_map(CUtensorMap* map, const c128* base, int64_t rows, in
     return CCSD_OK;
 }
 
+// 4-d "wide" view of the same operand: {4 complex k (8 doubles), rows, K/4 k-groups, batches}; a box {8, box_rows, 4, 1}
+// lands in shared memory as [k-group][row][64 B].  elem_doubles = 2 (complex operand) or 1 (real sum plane, box {4,..}).
+static int make_wide_map(CUtensorMap* map, const void* base, int64_t rows, int64_t K, int64_t ld, int nb, int64_t bs, int box_rows,
+                         int elem_doubles)
+{
+    PFN_encodeTiled enc = get_encode_fn();
+    if (!enc) { snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled unavailable"); return CCSD_ECUDA; }
+    const cuuint64_t eb = 8ull * elem_doubles;   // bytes per element
+    cuuint64_t dims[4] = {(cuuint64_t)(4 * elem_doubles), (cuuint64_t)rows, (cuuint64_t)(K / 4), (cuuint64_t)(nb > 0 ? nb : 1)};
+    cuuint64_t strides[3] = {(cuuint64_t)ld * eb, 4 * eb, (cuuint64_t)((nb > 1 && bs > 0) ? bs : ld) * eb};
+    cuuint32_t box[4] = {(cuuint32_t)(4 * elem_doubles), (cuuint32_t)box_rows, DMMA_BKG, 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled (wide) failed (%d): rows=%lld K=%lld ld=%lld nb=%d", (int)r,
+                 (long long)rows, (long long)K, (long long)ld, nb);
+        return CCSD_ECUDA;
+    }
+    return CCSD_OK;
+}
+
 // rows x K real sum plane (same leading dimension / batch stride, in elements, as the complex operand it belongs to)
 static int make_plane_map(CUtensorMap* map, const double* base, int64_t rows, int64_t K, int64_t ld, int nb, int64_t bs,
                           int box_rows)
@@ -387,7 +434,7 @@ static inline bool dmma_worthwhile(const GemmParams& p)
 
 template <class Cfg>
 static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const CUtensorMap& mAs,
-                           const CUtensorMap& mBs, const DmmaArgs& a, dim3 grid)
+                           const CUtensorMap& mBs, int wide, const DmmaArgs& a, dim3 grid)
 {
     static bool configured = false;
     if (!configured) {
@@ -396,6 +443,7 @@ static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtenso
     }
     PlainLoader ld;
     ld.mapA = mA; ld.mapB = mB; ld.mapAs = mAs; ld.mapBs = mBs;
+    ld.wide = wide;
     gemm_dmma_kernel<Cfg, PlainLoader><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(ld, a);
     g_launches++;
     return CCSD_OK;
@@ -406,7 +454,7 @@ static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtenso
 struct DmmaVariant {
     int bm, bn;
     bool m3, planes;
-    int (*launch)(cudaStream_t, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&,
+    int (*launch)(cudaStream_t, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&, int,
                   const DmmaArgs&, dim3);
 };
 #define DMMA_V(nwm, nwn, mi, nj, m3, ...) \
@@ -449,13 +497,26 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     if (variant < 0 || variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
     const DmmaVariant& V = k_dmma_variants[variant];
     CUtensorMap mA, mB;
-    CCSD_TRY(make_operand_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
-    CCSD_TRY(make_operand_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
-    CUtensorMap mAs = mA, mBs = mB;   // unused unless the variant stages sum planes
-    if (V.planes) {
-        if (!p.As || !p.Bs) return CCSD_EINVAL;
-        CCSD_TRY(make_plane_map(&mAs, p.As, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
-        CCSD_TRY(make_plane_map(&mBs, p.Bs, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
+    static const bool no_wide = getenv("CCSD_NO_WIDE_TMA") != nullptr;   // tuning / A-B switch
+    const int wide = (!no_wide && p.K % 4 == 0 && p.K >= 4) ? 1 : 0;
+    if (V.planes && (!p.As || !p.Bs)) return CCSD_EINVAL;
+    CUtensorMap mAs, mBs;
+    if (wide) {
+        CCSD_TRY(make_wide_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, V.bm, 2));
+        CCSD_TRY(make_wide_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn, 2));
+        mAs = mA; mBs = mB;           // unused unless the variant stages sum planes
+        if (V.planes) {
+            CCSD_TRY(make_wide_map(&mAs, p.As, p.M, p.K, p.sam, p.batch, p.bsA, V.bm, 1));
+            CCSD_TRY(make_wide_map(&mBs, p.Bs, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn, 1));
+        }
+    } else {
+        CCSD_TRY(make_operand_map(&mA, p.A, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
+        CCSD_TRY(make_operand_map(&mB, p.B, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
+        mAs = mA; mBs = mB;
+        if (V.planes) {
+            CCSD_TRY(make_plane_map(&mAs, p.As, p.M, p.K, p.sam, p.batch, p.bsA, V.bm));
+            CCSD_TRY(make_plane_map(&mBs, p.Bs, p.N, p.K, p.sbn, p.batch, p.bsB, V.bn));
+        }
     }
     DmmaArgs a;
     a.M = p.M; a.N = p.N; a.K = p.K;
@@ -465,5 +526,5 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     a.batchB = (p.batch > 1 && p.bsB != 0) ? 1 : 0;
     a.ksplit = p.ksplit; a.kchunk = p.kchunk; a.partial = p.partial;
     dim3 grid((unsigned)((p.N + V.bn - 1) / V.bn), (unsigned)((p.M + V.bm - 1) / V.bm), (unsigned)(p.batch * p.ksplit));
-    return V.launch(st, mA, mB, mAs, mBs, a, grid);
+    return V.launch(st, mA, mB, mAs, mBs, wide, a, grid);
 }
