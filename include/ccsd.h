@@ -83,6 +83,10 @@ int ccsd_iterate(ccsd_ctx* ctx, double* e_re, double* e_im, double* step_norm);
 /* E_corr = sum f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij} of the current amplitudes (eq 9).  HOST outputs. */
 int ccsd_energy(ccsd_ctx* ctx, double* e_re, double* e_im);
 
+/* T1 diagnostic of the current amplitudes, sqrt(sum_ia |t^a_i|^2 / nocc) (the paper tabulates it, PAPER.md:346-379 and
+ * 506-522, without defining it; this is the usual definition with nocc correlated spinors).  HOST output. */
+int ccsd_t1_diagnostic(ccsd_ctx* ctx, double* t1_diag);
+
 /* Evaluate eqs 23-33 at the current amplitudes WITHOUT updating them (fills the tensors ccsd_get_tensor returns). */
 int ccsd_residual(ccsd_ctx* ctx);
 

@@ -22,7 +22,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
-           "ccsd_triples_block"]
+           "ccsd_triples_block", "ccsd_t1_diagnostic"]
 
 
 class CCSDError(RuntimeError):
@@ -61,6 +61,7 @@ def load_library():
         lib.ccsd_iterate.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_energy.argtypes = [vp] + [ctypes.POINTER(dbl)] * 2
         lib.ccsd_residual.argtypes = [vp]
+        lib.ccsd_t1_diagnostic.argtypes = [vp, ctypes.POINTER(dbl)]
         lib.ccsd_get_amplitudes.argtypes = [vp, vp, vp]
         lib.ccsd_set_amplitudes.argtypes = [vp, vp, vp, ctypes.c_int]
         lib.ccsd_tensor_elems.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_size_t)]
@@ -216,6 +217,11 @@ class CCSD:
         er, ei = ctypes.c_double(), ctypes.c_double()
         _check(self._lib.ccsd_energy(self._ctx, ctypes.byref(er), ctypes.byref(ei)), "ccsd_energy")
         return complex(er.value, ei.value)
+
+    def t1_diagnostic(self) -> float:
+        out = ctypes.c_double()
+        _check(self._lib.ccsd_t1_diagnostic(self._ctx, ctypes.byref(out)), "ccsd_t1_diagnostic")
+        return out.value
 
     def residual(self):
         _check(self._lib.ccsd_residual(self._ctx), "ccsd_residual")

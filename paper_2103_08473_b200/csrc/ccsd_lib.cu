@@ -1066,6 +1066,17 @@ int ccsd_energy(ccsd_ctx* c, double* e_re, double* e_im)
     return CCSD_OK;
 }
 
+int ccsd_t1_diagnostic(ccsd_ctx* c, double* t1_diag)
+{   // sqrt(sum |t1|^2 / nocc): tabulated by the paper (Tables 3, 8), not defined there; reading G18 of DESIGN.md
+    if (!c || !t1_diag) return CCSD_ESTATE;
+    CCSD_CUDA_TRY(cudaMemsetAsync(c->red + 48, 0, sizeof(double), c->st));
+    launch_redot(c->st, c->t1, c->t1, c->ov, c->red + 48);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 48, c->red + 48, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    *t1_diag = sqrt(c->red_host[48] / (double)c->o);
+    return CCSD_OK;
+}
+
 int ccsd_residual(ccsd_ctx* c)
 {
     if (!c) return CCSD_ESTATE;

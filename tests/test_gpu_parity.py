@@ -258,3 +258,15 @@ def test_error_paths(gpu):
     assert lib.ccsd_iterate(None, None, None, None) == 4  # CCSD_ESTATE
     n = ctypes.c_size_t(0)
     assert lib.ccsd_contract_workspace_bytes(99, 4, 4, ctypes.byref(n)) == 1
+
+
+def test_t1_diagnostic(gpu):
+    """sqrt(sum |t1|^2 / nocc) of the amplitudes held by the library (reading G18)."""
+    inp = ci.make_config("cfg0")
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+    for _ in range(3):
+        gc.iterate()
+    t1 = gc.get_amplitudes()[0].cpu().numpy()
+    ref = np.sqrt((np.abs(t1) ** 2).sum() / inp.nocc)
+    assert abs(gc.t1_diagnostic() - ref) <= 1e-15 + 1e-13 * ref
+    gc.close()
