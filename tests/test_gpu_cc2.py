@@ -91,3 +91,17 @@ def test_cc2_and_ccsd_modes_differ(gpu):
     eb, _ = b.iterate()
     assert abs(ea - eb) > 1e-8
     a.close(); b.close()
+
+
+def test_cc2_minimal_size_and_level_shift(gpu):
+    """nocc = nvir = 2 (one occupied pair, one virtual pair) and shifted denominators, lock-step against the oracle."""
+    from oracle.cc2_oracle import OracleCC2
+    for (o, v, shift) in ((2, 2, 0.0), (3, 5, 0.25)):
+        inp = ci.make_inputs(o, v, 6, seed=50 + o, b_scale=0.1, f_offdiag=0.05)
+        oc = OracleCC2(inp.h, inp.B, o, v, ndiis=3, level_shift=shift)
+        gc = gpu.CCSD(inp.h, inp.B, o, v, ndiis=3, level_shift=shift, cc2=True)
+        for _ in range(6):
+            eo, so = oc.iterate()
+            eg, sg = gc.iterate()
+            assert abs(eg - eo) < E_TOL and abs(sg - so) < 1e-9 * max(1.0, so)
+        gc.close()

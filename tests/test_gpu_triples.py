@@ -115,3 +115,36 @@ def test_triples_energies_cfg1_against_oracle_golden(gpu):
     for key in ("+T", "(T)", "-T"):
         assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
     gc.close()
+
+
+def test_triples_edge_cases(gpu):
+    """Degenerate sizes: fewer than three occupied spinors -> CCSD_EINVAL; exactly three occupied and three virtual
+    spinors (ONE occupied triple, ONE virtual triple); level-shifted denominators; the call leaves the amplitudes and a
+    following iteration untouched."""
+    from paper_2103_08473_b200.binding import CCSDError
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2
+    from oracle.triples_oracle import OracleTriples
+    inp = ci.make_config("cfg0_2e")
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+    with pytest.raises(CCSDError):
+        gc.triples()
+    gc.close()
+    inp = ci.make_inputs(3, 3, 5, seed=31, b_scale=0.2, f_offdiag=0.1)
+    oc = OracleCCSD(inp.h, inp.B, 3, 3)
+    gc = gpu.CCSD(inp.h, inp.B, 3, 3)
+    oc.iterate(); gc.iterate()
+    ref, got = OracleTriples(oc).energies(), gc.triples()
+    for key in ("+T", "(T)", "-T"):
+        assert abs(got[key] - ref[key]) < E_TOL and abs(ref[key]) > 1e-8, (key, got[key], ref[key])
+    e_o, e_g = oc.iterate()[0], gc.iterate()[0]          # the triples call did not disturb the solver state
+    assert abs(e_o - e_g) < E_TOL
+    gc.close()
+    inp = ci.make_inputs(5, 12, 20, seed=32)
+    oc = OracleCCSD(inp.h, inp.B, 5, 12, level_shift=0.3)
+    gc = gpu.CCSD(inp.h, inp.B, 5, 12, level_shift=0.3)
+    for _ in range(2):
+        oc.iterate(); gc.iterate()
+    ref, got = OracleTriples(oc).energies(restricted=True), gc.triples()
+    for key in ("+T", "(T)", "-T"):
+        assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
+    gc.close()
