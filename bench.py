@@ -260,7 +260,8 @@ def cc2_bench(torch, pkg, inp, o, v, steps=5, warmup=3):
     return {"s_per_iteration": round(statistics.median(ts) * 1e-3, 6), "steps": steps, "warmup": warmup,
             "pp_ladder_ms": round(st["pp_ladder"], 3), "C_ovoo_ms": round(st["C_ovoo"], 3),
             "E_last": [e.real, e.imag], "step_norm_last": sn,
-            "note": "eq 34 evaluated as eq 32 at t2 = 0 plus the two Fock terms; singles by eq 33"}
+            "note": "eq 34 evaluated as eq 32 at t2 = 0 plus the two Fock terms, the <ab||cd> and <bk||cd> terms factorised "
+                    "through the auxiliary index (K = naux GEMMs); singles by eq 33"}
 
 
 def triples_bench(torch, pkg, inp, o, v, peak_tflops):

@@ -156,6 +156,9 @@ struct ccsd_ctx {
     c128 *t1, *t2p, *t1T, *S1, *S2p, *taup, *TT, *AG, *Xm, *T2r, *tauc, *tauou, *t2hu;
     c128 *Hvv, *Gvv, *Hoo, *Goo, *Hov, *HovT, *HF, *inner, *Hm, *Cm, *Cm2, *Am, *tmp_ov;
     c128 *Xr, *P, *Qm, *Rr, *Y, *Z;
+    // CC2 only: B blocks with the contracted virtual index fastest and the t1-dressed factors X (cc2_dressed_factors)
+    c128 *BvvT, *BovT, *Xv, *Xo;
+    double* Xvs;
     c128* partial;
     int64_t partial_elems;
     // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
@@ -282,6 +285,15 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
         c->Xms = w.take<double>(ov * ov);
         c->T2rs = w.take<double>(ov * ov);
         c->Hms = w.take<double>(ov * ov);
+    }
+    c->BvvT = c->BovT = c->Xv = c->Xo = nullptr;
+    c->Xvs = nullptr;
+    if (c->opt.cc2) {
+        c->BvvT = w.take<c128>(v * Lp * v);
+        c->BovT = w.take<c128>(o * Lp * v);
+        c->Xv = w.take<c128>(ov * Lp);
+        c->Xo = w.take<c128>(o * o * Lp);
+        c->Xvs = w.take<double>(ov * Lp);
     }
     c->nvec = ov + oo * vv;
     int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
@@ -515,6 +527,12 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
         launch_sum_plane(st, c->Voovv_p, c->Voovv_ps, oo * vv);
         launch_sum_plane(st, c->G1, c->G1s, ov * ov);
     }
+    if (c->opt.cc2) {   // BvvT[a][l][e] = B[l][a][e], BovT[k][l][d] = B[l][k][d]: K-contiguous operands of cc2_dressed_factors
+        const int64_t dv[4] = {v, v, Lp, 1}, dk[4] = {o, v, Lp, 1};
+        const int perm[4] = {0, 2, 1, 3};
+        CCSD_TRY(launch_transpose4d(st, c->Bvv, c->BvvT, dv, perm, 0));
+        CCSD_TRY(launch_transpose4d(st, c->Bov, c->BovT, dk, perm, 0));
+    }
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -673,6 +691,30 @@ static int build_Hvovo(ccsd_ctx* c)
     return CCSD_OK;
 }
 
+// CC2 only.  With t2 = 0 the two quadratic terms that need <ab||cd> and <bk||cd> factorise through the auxiliary index of
+// (pq|rs) = sum_L B^L_pq B^L_rs (Cholesky vectors), with the t1-dressed factors
+//     Xv[(a,i)][L] = sum_e B^L_ae t1[i,e],      Xo[(k,j)][L] = sum_d B^L_kd t1[j,d]:
+//     sum_{e<f} <ab||ef> tau0^{ef}_{ij} = sum_ef <ab||ef> t_i^e t_j^f = sum_L ( Xv_ai Xv_bj - Xv_aj Xv_bi )        (K = L)
+//     sum_{c<d} <bk||cd> tau0^{cd}_{ij}                               = sum_L ( Xv_bi Xo_kj - Xv_bj Xo_ki )
+// i.e. (ov)^2 L and ov o^2 L work instead of oo vv^2 and ov oo vv: the doubles equations of CC2 drop from O(o^2 v^4) to
+// O(o^2 v^2 L), which is what makes CC2 an N^5 method.
+static int cc2_dressed_factors(ccsd_ctx* c)
+{
+    const int o = c->o, v = c->v, Lp = c->Lp;
+    {
+        GemmParams p = gp(Lp, o, v, c->BvvT, v, c->t1, v, c->Xv, 1, Lp, 1.0, 0);      // per a: C_a[L][i]
+        p.batch = v; p.bsA = (int64_t)Lp * v; p.bsB = 0; p.bsC = (int64_t)o * Lp;
+        CCSD_TRY(run_gemm(c->env, p));
+    }
+    {
+        GemmParams p = gp(Lp, o, v, c->BovT, v, c->t1, v, c->Xo, 1, Lp, 1.0, 0);      // per k: C_k[L][j]
+        p.batch = o; p.bsA = (int64_t)Lp * v; p.bsB = 0; p.bsC = (int64_t)o * Lp;
+        CCSD_TRY(run_gemm(c->env, p));
+    }
+    if (c->planes) launch_sum_plane(c->st, c->Xv, c->Xvs, c->ov * Lp);
+    return CCSD_OK;
+}
+
 static int build_C(ccsd_ctx* c)
 {
     cudaStream_t st = c->st;
@@ -688,6 +730,16 @@ static int build_C(ccsd_ctx* c)
         int2 ij = po[IJ];
         return csub(Y[(bk * o + ij.x) * o + ij.y], Y[(bk * o + ij.y) * o + ij.x]);
     });
+    if (c->opt.cc2) {   // - sum_L ( Xv_bi Xo_kj - Xv_bj Xo_ki ): Q[(b,i)][(k,j)] in the buffer the linear term just released
+        c128* Q = c->Y;
+        CCSD_TRY(run_gemm(env, gp(ov, (int64_t)o * o, c->Lp, c->Xv, c->Lp, c->Xo, c->Lp, Q, (int64_t)o * o, 1, 1.0, 0)));
+        launch_fill(st, c->Cm, ov, oo, oo, 1, [=] __device__(int64_t bk, int64_t IJ) {
+            int2 ij = po[IJ];
+            const int64_t b = bk / o, k = bk % o;
+            return csub(Q[((b * o + ij.y) * o + k) * o + ij.x], Q[((b * o + ij.x) * o + k) * o + ij.y]);
+        });
+        return CCSD_OK;
+    }
     CCSD_TRY(run_gemm(env, with_planes(gp(ov, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), c->Vvovv_ps, c->taups)));
     return CCSD_OK;
 }
@@ -721,6 +773,19 @@ static int s2_driver(ccsd_ctx* c, c128* S)
 }
 static int s2_pp_ladder(ccsd_ctx* c, c128* S)
 {   // sum_{c<d} <ab||cd> tau[i,j,c,d]      M = (a<b), N = (i<j), K = (c<d)
+    if (c->opt.cc2) {   // tau = P-(t1 t1): sum_L ( Xv_ai Xv_bj - Xv_aj Xv_bi ), R2[(a,i)][(b,j)] = sum_L Xv_ai Xv_bj
+        const int o = c->o;
+        const int64_t ov = c->ov, vv = c->vv;
+        c128* R2 = c->Xr;
+        CCSD_TRY(run_gemm(c->env, with_planes(gp(ov, ov, c->Lp, c->Xv, c->Lp, c->Xv, c->Lp, R2, ov, 1, 1.0, 0), c->Xvs, c->Xvs)));
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+            int2 ij = po[IJ], ab = pv[AB];
+            const int64_t a = ab.x, b = ab.y;
+            return csub(R2[(a * o + ij.x) * ov + b * o + ij.y], R2[(a * o + ij.y) * ov + b * o + ij.x]);
+        });
+        return CCSD_OK;
+    }
     return run_gemm(c->env, with_planes(gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
 static void fill_AG_hh(ccsd_ctx* c)
@@ -898,6 +963,7 @@ static int residual(ccsd_ctx* c)
 // S1 is eq 33 at the full (t1, t2).  The doubles equation 34 is <Phi_ij^ab| exp(-T1) H exp(T1) + [F, T2] |Phi_0>, i.e.
 // eq 32 evaluated with t2 -> 0 in every operand (tau -> P-(t1 t1); the ring, G.t2 terms vanish; H^{ak}_{ci} is not
 // needed) plus the two Fock terms, which have the form of the G.t2 terms of eq 32 with G^a_c -> f_ac, G^k_i -> -f_ki:
+//   (the pp-ladder and the <bk||cd> part of C at tau0 run factorised through the auxiliary index: cc2_dressed_factors)
 //   W^{ab}_{ef}CC2 (x) t1 t1  = pp-ladder(tau0) + the <bk||cd> tau0 part of C;  W^{mn}_{ij}CC2 = A(tau0) of eq 31 (up to the
 //   factor of the quartic term shared between eqs 35 and 36);  W^{ab}_{ej}, W^{mb}_{ij} = V-dagger.t1 and the rest of C.t1.
 // The oracle evaluates eqs 34-38 literally; the two agree to rounding (tests/test_gpu_cc2.py).
@@ -914,6 +980,7 @@ static int residual_cc2(ccsd_ctx* c)
     CCSD_TRY(build_S1(c));                      // eq 33, full tau (timed under "Hvovo_quad"'s slot: see ccsd_step_name)
     tick(c, 4);
     // doubles: operands with t2 = 0
+    CCSD_TRY(cc2_dressed_factors(c));
     build_tau(st, c->taup, c->t1, nullptr, o, v, c->po, c->pv, c->taups);
     CCSD_TRY(launch_transpose2d_ld(st, c->taup, c->vv, c->TT, 2 * c->oop, c->oo, c->vv, 0));
     const c128* f = c->f;

@@ -1,6 +1,6 @@
 """Write tests/golden/oracle_lockstep_<cfg>.txt: lock-step energies of the CPU ORACLE (and nothing else).
 
-    python tests/golden/make_oracle_energies.py cfg2 10
+    python tests/golden/make_oracle_energies.py cfg2 10 [output file]
 
 Calls only oracle/ and the shared input generator.  The file lists E (Re, Im) and ||S/D||_2 of the MP2 start and of
 every iteration with DIIS(6) (reading G13), to be compared with the CUDA library's ccsd_iterate by the GPU tests.
@@ -26,7 +26,8 @@ def main():
              "# written by tests/golden/make_oracle_energies.py (oracle/ only, restricted-sum mode, DIIS(6))",
              f"# host threads: {num_threads()}",
              "# iteration  Re(E)  Im(E)  ||S/D||_2 of the residual evaluated in that iteration (nan for the MP2 start)"]
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"oracle_lockstep_{cfg}.txt")
+    path = sys.argv[3] if len(sys.argv) > 3 else \
+        os.path.join(os.path.dirname(os.path.abspath(__file__)), f"oracle_lockstep_{cfg}.txt")
 
     def flush():   # rewritten after every iteration: a long run that is cut short still leaves its finished lines
         with open(path, "w") as fh:
