@@ -333,6 +333,10 @@ def run_ours(args) -> None:
     cfg = args.config
     o, v, L, seed = ci.CONFIGS[cfg]
     oo, vv, ov = ci.pair_count(o), ci.pair_count(v), o * v
+    if args.only_ladder and args.ladder_shape:
+        o, v = (int(x) for x in args.ladder_shape.split(","))
+        oo, vv = ci.pair_count(o), ci.pair_count(v)
+        cfg = f"nocc={o} nvir={v}"
     if args.only_ladder:
         # profiling aid: just the pp-ladder launch of this workload's shape (same kernel, same launch configuration
         # as inside ccsd_iterate), W warm-ups + K timed launches
@@ -504,6 +508,7 @@ def main():
     ap.add_argument("--config", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
+    ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-triples", action="store_true", help="time only the perturbative triples of --config")
     args = ap.parse_args()
     if args.impl == "reference":

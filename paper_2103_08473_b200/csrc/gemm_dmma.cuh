@@ -485,7 +485,7 @@ static inline int dmma_pick(int64_t N, bool m3, bool planes = false)
     double bestcost = 0.0;
     for (int v = hi; v >= lo; v--) {
         const int bn = k_dmma_variants[v].bn;
-        const double rel = planes ? (bn == 32 ? 1.019 : 1.0) : m3 ? (bn == 32 ? 1.037 : 1.0) : 1.0 + 0.01 * (64 - bn) / 8.0;
+        const double rel = planes ? (bn == 32 ? 1.026 : 1.0) : m3 ? (bn == 32 ? 1.037 : 1.0) : 1.0 + 0.01 * (64 - bn) / 8.0;
         const double cost = (double)round_up(N, bn) * rel;
         if (best < 0 || cost < bestcost) { best = v; bestcost = cost; }
     }
@@ -498,7 +498,9 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     const DmmaVariant& V = k_dmma_variants[variant];
     CUtensorMap mA, mB;
     static const bool no_wide = getenv("CCSD_NO_WIDE_TMA") != nullptr;   // tuning / A-B switch
-    const int wide = (!no_wide && p.K % 4 == 0 && p.K >= 4) ? 1 : 0;
+    // measured: the wide maps help the 48-column tiles (pp-ladder 0.928 -> 0.935 of peak) but cost the 32-column ones, which
+    // move more bytes per flop, 10-15 % (config-4 sweep at nocc = 40: 0.90 -> 0.78; triples GEMM 5.06 -> 5.36 s)
+    const int wide = (!no_wide && p.K % 4 == 0 && p.K >= 4 && V.bn >= 48) ? 1 : 0;
     if (V.planes && (!p.As || !p.Bs)) return CCSD_EINVAL;
     CUtensorMap mAs, mBs;
     if (wide) {
