@@ -38,7 +38,8 @@ extern "C" {
 typedef struct ccsd_ctx ccsd_ctx; /* opaque, host-side handle */
 typedef struct { double re, im; } ccsd_c128;
 
-enum { CCSD_OK = 0, CCSD_EINVAL = 1, CCSD_ENOMEM = 2, CCSD_ECUDA = 3, CCSD_ESTATE = 4, CCSD_ESINGULAR = 5 };
+enum { CCSD_OK = 0, CCSD_EINVAL = 1, CCSD_ENOMEM = 2, CCSD_ECUDA = 3, CCSD_ESTATE = 4, CCSD_ESINGULAR = 5,
+       CCSD_ENOTCONVERGED = 6 };
 
 typedef struct {
     int ndiis;          /* DIIS subspace size; 0 = plain Jacobi; default 6 (reading G13) */
@@ -79,6 +80,14 @@ int ccsd_init(ccsd_ctx** ctx, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
  * Errors: CCSD_ESTATE (no context), CCSD_ESINGULAR (DIIS system singular even with one vector), CCSD_ECUDA.
  */
 int ccsd_iterate(ccsd_ctx* ctx, double* e_re, double* e_im, double* step_norm);
+
+/*
+ * ccsd_iterate until ||S/D||_2 < tol and |E - E_previous| < tol, or max_iterations (the paper's .TCONVERG 1e-9 and
+ * .NCYCLES 30 keywords; which quantity .TCONVERG tests is not stated: reading G14).  HOST outputs:
+ * iterations done, energy of the last amplitudes, last ||S/D||_2.  Returns CCSD_ENOTCONVERGED if the limit was hit.
+ */
+int ccsd_solve(ccsd_ctx* ctx, double tol, int max_iterations, int* iterations, double* e_re, double* e_im,
+               double* step_norm);
 
 /* E_corr = sum f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij} of the current amplitudes (eq 9).  HOST outputs. */
 int ccsd_energy(ccsd_ctx* ctx, double* e_re, double* e_im);

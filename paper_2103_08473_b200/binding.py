@@ -7,7 +7,8 @@ import os
 HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
-STATUS = {0: "CCSD_OK", 1: "CCSD_EINVAL", 2: "CCSD_ENOMEM", 3: "CCSD_ECUDA", 4: "CCSD_ESTATE", 5: "CCSD_ESINGULAR"}
+STATUS = {0: "CCSD_OK", 1: "CCSD_EINVAL", 2: "CCSD_ENOMEM", 3: "CCSD_ECUDA", 4: "CCSD_ESTATE", 5: "CCSD_ESINGULAR",
+          6: "CCSD_ENOTCONVERGED"}
 TENSOR_IDS = {"fock": 0, "vvvv": 1, "vovv": 2, "vovo": 3, "oovv": 4, "ooov": 5, "oooo": 6, "tau": 10, "Hvv": 11,
               "Gvv": 12, "Hoo": 13, "Goo": 14, "Hov": 15, "Hvovo": 16, "C": 17, "A": 18, "S1": 19, "S2": 20,
               "S2_ring": 30, "S2_goo": 31, "S2_vdag_t1": 32, "S2_gvv": 33, "S2_c_t1": 34, "S2_hh_ladder": 35,
@@ -22,7 +23,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
-           "ccsd_triples_block", "ccsd_t1_diagnostic"]
+           "ccsd_triples_block", "ccsd_t1_diagnostic", "ccsd_solve"]
 
 
 class CCSDError(RuntimeError):
@@ -61,6 +62,7 @@ def load_library():
         lib.ccsd_iterate.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_energy.argtypes = [vp] + [ctypes.POINTER(dbl)] * 2
         lib.ccsd_residual.argtypes = [vp]
+        lib.ccsd_solve.argtypes = [vp, dbl, ctypes.c_int, ctypes.POINTER(ctypes.c_int)] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_t1_diagnostic.argtypes = [vp, ctypes.POINTER(dbl)]
         lib.ccsd_get_amplitudes.argtypes = [vp, vp, vp]
         lib.ccsd_set_amplitudes.argtypes = [vp, vp, vp, ctypes.c_int]
@@ -217,6 +219,15 @@ class CCSD:
         er, ei = ctypes.c_double(), ctypes.c_double()
         _check(self._lib.ccsd_energy(self._ctx, ctypes.byref(er), ctypes.byref(ei)), "ccsd_energy")
         return complex(er.value, ei.value)
+
+    def solve(self, tol: float = 1e-9, max_iterations: int = 30):
+        """ccsd_solve -> (converged, iterations, complex E_corr, ||S/D||_2); defaults = the paper's .TCONVERG / .NCYCLES."""
+        it, er, ei, sn = ctypes.c_int(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        st = self._lib.ccsd_solve(self._ctx, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(er),
+                                  ctypes.byref(ei), ctypes.byref(sn))
+        if st not in (0, 6):
+            _check(st, "ccsd_solve")
+        return st == 0, it.value, complex(er.value, ei.value), sn.value
 
     def t1_diagnostic(self) -> float:
         out = ctypes.c_double()

@@ -1252,6 +1252,28 @@ int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
     return status;
 }
 
+int ccsd_solve(ccsd_ctx* c, double tol, int max_iterations, int* iterations, double* e_re, double* e_im, double* step_norm)
+{   // .TCONVERG / .NCYCLES of the paper's input (reading G14): both ||S/D||_2 and |Delta E| below tol
+    if (!c) return CCSD_ESTATE;
+    if (!(tol > 0.0) || max_iterations < 1) return CCSD_EINVAL;
+    double er = 0.0, ei = 0.0, sn = 0.0, er_old = 0.0, ei_old = 0.0;
+    CCSD_TRY(ccsd_energy(c, &er_old, &ei_old));
+    int it = 0, status = CCSD_OK;
+    bool converged = false;
+    while (it < max_iterations && !converged) {
+        status = ccsd_iterate(c, &er, &ei, &sn);
+        if (status != CCSD_OK && status != CCSD_ESINGULAR) return status;
+        it++;
+        converged = sn < tol && hypot(er - er_old, ei - ei_old) < tol;
+        er_old = er; ei_old = ei;
+    }
+    if (iterations) *iterations = it;
+    if (e_re) *e_re = er;
+    if (e_im) *e_im = ei;
+    if (step_norm) *step_norm = sn;
+    return converged ? CCSD_OK : CCSD_ENOTCONVERGED;
+}
+
 int ccsd_get_amplitudes(ccsd_ctx* c, ccsd_c128* t1, ccsd_c128* t2p)
 {
     if (!c) return CCSD_ESTATE;
@@ -1846,6 +1868,7 @@ const char* ccsd_strerror(int s)
     case CCSD_ECUDA: return "CUDA error";
     case CCSD_ESTATE: return "invalid state or handle";
     case CCSD_ESINGULAR: return "singular DIIS system";
+    case CCSD_ENOTCONVERGED: return "not converged within the iteration limit";
     default: return "unknown status";
     }
 }

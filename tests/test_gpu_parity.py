@@ -270,3 +270,20 @@ def test_t1_diagnostic(gpu):
     ref = np.sqrt((np.abs(t1) ** 2).sum() / inp.nocc)
     assert abs(gc.t1_diagnostic() - ref) <= 1e-15 + 1e-13 * ref
     gc.close()
+
+
+def test_solve_to_convergence(gpu):
+    """ccsd_solve (.TCONVERG / .NCYCLES): stops when ||S/D|| and |dE| < tol; the converged energy
+    equals the oracle's converged energy (independent of the DIIS details); the iteration limit is reported."""
+    from oracle.ccsd_oracle import OracleCCSD
+    inp = ci.make_config("cfg0")
+    oc = OracleCCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+    e_ref = oc.run(60, tol=1e-13)[-1][0]
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+    ok, nit, e, sn = gc.solve(1e-11, 40)
+    assert ok and nit < 40 and sn < 1e-11 and abs(e - e_ref) < E_TOL
+    gc.close()
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+    ok, nit, e, sn = gc.solve(1e-13, 2)
+    assert not ok and nit == 2
+    gc.close()
