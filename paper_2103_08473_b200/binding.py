@@ -50,8 +50,13 @@ def load_library():
     if _LIB is None:
         path = lib_path()
         if not os.path.exists(path):
-            raise ImportError(f"{path} is missing: run `python -m paper_2103_08473_b200.build` (needs nvcc); "
-                              "there is no CPU fallback")
+            # a fresh checkout has no built artefact (*.so is git-ignored): compile it once, in-tree, if nvcc is there
+            try:
+                from . import build as _build
+                _build.build()
+            except Exception as exc:                                   # noqa: BLE001
+                raise ImportError(f"{path} is missing and could not be built ({exc}): run "
+                                  "`python -m paper_2103_08473_b200.build` (needs nvcc); there is no CPU fallback")
         lib = ctypes.CDLL(path)
         vp, i64, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double
         lib.ccsd_default_options.argtypes = [ctypes.POINTER(Options)]
