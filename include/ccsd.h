@@ -141,6 +141,33 @@ int ccsd_triples_workspace_bytes(ccsd_ctx* ctx, size_t* bytes);
 int ccsd_triples(ccsd_ctx* ctx, double e_plus_t[2], double e_par_t[2], double e_minus_t[2], void* workspace,
                  size_t workspace_bytes);
 int ccsd_get_triples_times(ccsd_ctx* ctx, float ms[2]);
+/*
+ * CCSD Lambda equations and Lagrange one-body density matrix (Appendix 7.4-7.5, eqs 45-61; PAPER.md:109-126,
+ * 238), at the CURRENT amplitudes, which should be converged (ccsd_solve): the equations are
+ * <0|(1+Lambda)(Hbar - E)|mu> = 0 up to terms proportional to the amplitude residual.  Reading of the incomplete
+ * printed equations: DESIGN.md G23, G24.  Not available in CC2 mode (CCSD_EINVAL).
+ *   ccsd_lambda_init      builds the elements of Hbar = exp(-T) H exp(T) once (it runs one residual evaluation: the
+ *                         tensors of ccsd_get_tensor are refreshed) and sets lambda = conj(t).  workspace: device,
+ *                         256-byte aligned, ccsd_lambda_workspace_bytes() bytes; it must stay alive while the Lambda
+ *                         entry points are used (until the next ccsd_lambda_init or ccsd_destroy).  Synchronises.
+ *   ccsd_lambda_iterate   one iteration: right-hand sides of eqs 52-56, lambda <- lambda + R/D with the CCSD
+ *                         denominators, DIIS as for the amplitudes.  HOST output ||R/D||_2 over the unique multipliers.
+ *   ccsd_lambda_residual  evaluates the right-hand sides only (ccsd_get_lambda_residual returns them).
+ *   ccsd_get/set_lambda   multipliers lambda^i_a [i][a], lambda^{ij}_{ab} [(i<j)][(a<b)] (device, asynchronous).
+ *   ccsd_density          D[p][q] = <0|(1+Lambda) exp(-T) a+_p a_q exp(T)|0> - delta_pq (p occupied), [n][n] (device),
+ *                         occupied spinors first, assembled from eqs 58-61, unsymmetrised (the paper symmetrises it
+ *                         before use).  Uses the residual buffers: call it between iterations.
+ * Errors: CCSD_ESTATE without ccsd_lambda_init, CCSD_EINVAL (workspace), CCSD_ESINGULAR (DIIS), CCSD_ECUDA.
+ */
+int ccsd_lambda_workspace_bytes(ccsd_ctx* ctx, size_t* bytes);
+int ccsd_lambda_init(ccsd_ctx* ctx, void* workspace, size_t workspace_bytes);
+int ccsd_lambda_iterate(ccsd_ctx* ctx, double* step_norm);
+int ccsd_lambda_residual(ccsd_ctx* ctx);
+int ccsd_get_lambda(ccsd_ctx* ctx, ccsd_c128* l1, ccsd_c128* l2p);
+int ccsd_set_lambda(ccsd_ctx* ctx, const ccsd_c128* l1, const ccsd_c128* l2p, int reset_diis);
+int ccsd_get_lambda_residual(ccsd_ctx* ctx, ccsd_c128* r1, ccsd_c128* r2p);
+int ccsd_density(ccsd_ctx* ctx, ccsd_c128* D);
+
 /* Per-term parity hook: the dense, fully antisymmetric blocks Wbar, Zbar, Ybar [a][b][c] (nvir^3 elements each, device;
  * NULL = skip) of one occupied triple i<j<k.  Asynchronous on the stream after an initial synchronisation. */
 int ccsd_triples_block(ccsd_ctx* ctx, int i, int j, int k, ccsd_c128* Wbar, ccsd_c128* Zbar, ccsd_c128* Ybar,

@@ -23,7 +23,9 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
-           "ccsd_triples_block", "ccsd_t1_diagnostic", "ccsd_solve"]
+           "ccsd_triples_block", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
+           "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
+           "ccsd_get_lambda_residual", "ccsd_density"]
 
 
 class CCSDError(RuntimeError):
@@ -67,6 +69,14 @@ def load_library():
         lib.ccsd_iterate.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_energy.argtypes = [vp] + [ctypes.POINTER(dbl)] * 2
         lib.ccsd_residual.argtypes = [vp]
+        lib.ccsd_lambda_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_lambda_init.argtypes = [vp, vp, ctypes.c_size_t]
+        lib.ccsd_lambda_iterate.argtypes = [vp, ctypes.POINTER(dbl)]
+        lib.ccsd_lambda_residual.argtypes = [vp]
+        lib.ccsd_get_lambda.argtypes = [vp, vp, vp]
+        lib.ccsd_set_lambda.argtypes = [vp, vp, vp, ctypes.c_int]
+        lib.ccsd_get_lambda_residual.argtypes = [vp, vp, vp]
+        lib.ccsd_density.argtypes = [vp, vp]
         lib.ccsd_solve.argtypes = [vp, dbl, ctypes.c_int, ctypes.POINTER(ctypes.c_int)] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_t1_diagnostic.argtypes = [vp, ctypes.POINTER(dbl)]
         lib.ccsd_get_amplitudes.argtypes = [vp, vp, vp]
@@ -205,6 +215,7 @@ class CCSD:
             self._lib.ccsd_destroy(self._ctx)
             self._ctx = ctypes.c_void_p(None)
             self._ws = None
+            self._lam_ws = None
 
     def __del__(self):
         try:
@@ -297,6 +308,53 @@ class CCSD:
         torch.cuda.current_stream().synchronize()
         del ws
         return out
+
+    # ---- Lambda equations / density (Appendix 7.4-7.5) ----
+    def lambda_init(self):
+        torch = self._torch
+        nbytes = ctypes.c_size_t(0)
+        _check(self._lib.ccsd_lambda_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_lambda_workspace_bytes")
+        self._lam_ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")   # lives with the solver
+        base = (self._lam_ws.data_ptr() + 255) // 256 * 256
+        _check(self._lib.ccsd_lambda_init(self._ctx, base, int(nbytes.value)), "ccsd_lambda_init")
+
+    def lambda_iterate(self) -> float:
+        sn = ctypes.c_double()
+        st = self._lib.ccsd_lambda_iterate(self._ctx, ctypes.byref(sn))
+        if st not in (0, 5):
+            _check(st, "ccsd_lambda_iterate")
+        return sn.value
+
+    def lambda_residual(self):
+        torch = self._torch
+        _check(self._lib.ccsd_lambda_residual(self._ctx), "ccsd_lambda_residual")
+        r1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
+        r2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
+        _check(self._lib.ccsd_get_lambda_residual(self._ctx, r1.data_ptr(), r2p.data_ptr()), "ccsd_get_lambda_residual")
+        torch.cuda.current_stream().synchronize()
+        return r1, r2p
+
+    def get_lambda(self):
+        torch = self._torch
+        l1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
+        l2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
+        _check(self._lib.ccsd_get_lambda(self._ctx, l1.data_ptr(), l2p.data_ptr()), "ccsd_get_lambda")
+        torch.cuda.current_stream().synchronize()
+        return l1, l2p
+
+    def set_lambda(self, l1, l2p, reset_diis: bool = True):
+        torch = self._torch
+        a, b = _dev_c128(torch, l1), _dev_c128(torch, l2p)
+        assert tuple(a.shape) == (self.nocc, self.nvir) and tuple(b.shape) == (self.oo, self.vv)
+        _check(self._lib.ccsd_set_lambda(self._ctx, a.data_ptr(), b.data_ptr(), int(reset_diis)), "ccsd_set_lambda")
+        torch.cuda.current_stream().synchronize()
+
+    def density(self):
+        torch = self._torch
+        D = torch.empty((self.n, self.n), dtype=torch.complex128, device="cuda")
+        _check(self._lib.ccsd_density(self._ctx, D.data_ptr()), "ccsd_density")
+        torch.cuda.current_stream().synchronize()
+        return D
 
     def enable_step_timing(self, enable: bool = True):
         _check(self._lib.ccsd_enable_step_timing(self._ctx, int(enable)), "ccsd_enable_step_timing")

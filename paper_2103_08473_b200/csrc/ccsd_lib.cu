@@ -137,7 +137,9 @@ static const char* k_step_names[CCSD_NSTEPS] = {"prep_permute", "fock_like", "Hv
                                                 "A_oooo", "pp_ladder", "hh_ladder+Goo", "ring_gemm", "ring_antisym",
                                                 "Vdag_t1", "Gvv_t2", "C_t1", "S1", "update_diis", "energy"};
 
+struct LambdaState;
 struct ccsd_ctx {
+    LambdaState* lam;       // Lambda solve in progress (ccsd_lambda_init), or null
     int o, v, n, L, Lp;
     int64_t oo, vv, ov, oop, nvec;
     ccsd_options opt;
@@ -1050,6 +1052,8 @@ static int solve_small(std::vector<double>& A, std::vector<double>& b, int m)
     return 0;
 }
 
+#include "lambda.cuh"
+
 extern "C" {
 
 void ccsd_default_options(ccsd_options* opts)
@@ -1085,6 +1089,7 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     }
     ccsd_ctx* c = new (std::nothrow) ccsd_ctx();
     if (!c) return CCSD_ENOMEM;
+    c->lam = nullptr;
     setup_dims(c, nocc, nvir, naux, opts);
     size_t need = 0;
     carve(c, nullptr, &need);
@@ -1118,6 +1123,7 @@ int ccsd_destroy(ccsd_ctx* c)
     for (int k = 0; k <= CCSD_NSTEPS; k++)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->red_host) cudaFreeHost(c->red_host);
+    delete c->lam;
     delete c;
     return CCSD_OK;
 }
@@ -1636,6 +1642,91 @@ int ccsd_get_triples_times(ccsd_ctx* c, float ms[2])
     if (!c || !ms) return CCSD_ESTATE;
     ms[0] = c->trip_ms[0]; ms[1] = c->trip_ms[1];
     return CCSD_OK;
+}
+
+// ---- Lambda equations and one-body density (Appendix 7.4-7.5; lambda.cuh / tensor_ops.cuh) ---------------------------
+int ccsd_lambda_workspace_bytes(ccsd_ctx* c, size_t* bytes)
+{
+    if (!c || !bytes) return CCSD_ESTATE;
+    LambdaState tmp;
+    lambda_carve(c, nullptr, &tmp, bytes);
+    return CCSD_OK;
+}
+
+int ccsd_lambda_init(ccsd_ctx* c, void* workspace, size_t workspace_bytes)
+{
+    if (!c) return CCSD_ESTATE;
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || c->opt.cc2) return CCSD_EINVAL;
+    size_t need = 0;
+    LambdaState tmp;
+    lambda_carve(c, nullptr, &tmp, &need);
+    if (workspace_bytes < need) return CCSD_EINVAL;
+    delete c->lam;
+    c->lam = new (std::nothrow) LambdaState();
+    if (!c->lam) return CCSD_ENOMEM;
+    LambdaState* L = c->lam;
+    lambda_carve(c, static_cast<char*>(workspace), L, &need);
+    L->ready = false;
+    L->diis_count = L->diis_next = L->norder = 0;
+    memset(L->gram, 0, sizeof(L->gram));
+    CCSD_TRY(lambda_build_hbar(c, L));
+    {   // start: lambda = conj(t) (first order: lambda^{ij}_{ab} = <ij||ab>/D = conj t^{ab}_{ij}; reading G23)
+        const c128 *t1 = c->t1, *t2p = c->t2p;
+        const int v = c->v;
+        const int64_t vv = c->vv;
+        launch_fill(c->st, L->l1, c->o, v, v, 0, [=] __device__(int64_t i, int64_t a) { return cconj(t1[i * v + a]); });
+        launch_fill(c->st, L->l2p, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) { return cconj(t2p[IJ * vv + AB]); });
+    }
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    CCSD_CUDA_TRY(cudaGetLastError());
+    L->ready = true;
+    return CCSD_OK;
+}
+
+int ccsd_lambda_iterate(ccsd_ctx* c, double* step_norm)
+{
+    if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
+    return lambda_iterate(c, c->lam, step_norm);
+}
+
+int ccsd_lambda_residual(ccsd_ctx* c)
+{
+    if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
+    return lambda_residual(c, c->lam);
+}
+
+int ccsd_get_lambda(ccsd_ctx* c, ccsd_c128* l1, ccsd_c128* l2p)
+{
+    if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
+    if (l1) dcopy(c->st, reinterpret_cast<c128*>(l1), c->lam->l1, c->ov);
+    if (l2p) dcopy(c->st, reinterpret_cast<c128*>(l2p), c->lam->l2p, c->oo * c->vv);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_set_lambda(ccsd_ctx* c, const ccsd_c128* l1, const ccsd_c128* l2p, int reset_diis)
+{
+    if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
+    if (l1) dcopy(c->st, c->lam->l1, reinterpret_cast<const c128*>(l1), c->ov);
+    if (l2p) dcopy(c->st, c->lam->l2p, reinterpret_cast<const c128*>(l2p), c->oo * c->vv);
+    if (reset_diis) { c->lam->diis_count = c->lam->diis_next = c->lam->norder = 0; }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_get_lambda_residual(ccsd_ctx* c, ccsd_c128* r1, ccsd_c128* r2p)
+{
+    if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
+    if (r1) dcopy(c->st, reinterpret_cast<c128*>(r1), c->lam->R1, c->ov);
+    if (r2p) dcopy(c->st, reinterpret_cast<c128*>(r2p), c->lam->R2p, c->oo * c->vv);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+int ccsd_density(ccsd_ctx* c, ccsd_c128* D)
+{
+    if (!c || !c->lam || !c->lam->ready || !D) return CCSD_ESTATE;
+    return lambda_density(c, c->lam, reinterpret_cast<c128*>(D));
 }
 
 // ---- standalone contractions ----------------------------------------------------------------------------------

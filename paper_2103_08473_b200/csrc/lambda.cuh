@@ -1,0 +1,421 @@
+// CCSD Lambda equations and one-body density (arXiv 2103.08473 Appendix 7.4-7.5, eqs 45-61).
+// Included by ccsd_lib.cu after the iteration driver.  First CUDA path of this row: every term of the working equations
+// (reading G23 of DESIGN.md) is one tensor_contract call on dense unpacked tensors, the GEMM of each
+// call running on the DMMA kernel; the elements of Hbar are built once per solve, an iteration contracts the multipliers
+// with them.  The pp-ladder term runs on the packed, dressed <ef||ab> with the DMMA ladder launch of the CCSD iteration.
+#pragma once
+#include "tensor_ops.cuh"
+
+// C[out index orders] += sign * alpha * sum_k A B   (see tensor_ops.cuh).  Extents are taken from the operands.
+static int tensor_contract(const Env& env, const TcScratch& sc, double alpha, const TView& A, const TView& B, c128* C, int nout,
+                           const TcOut* outs)
+{
+    char K[5] = {0}, MA[5] = {0}, NB[5] = {0};
+    int64_t dimOf[128];
+    for (int q = 0; q < A.rank; q++) dimOf[(int)A.idx[q]] = A.dim[q];
+    for (int q = 0; q < B.rank; q++) {
+        if (strchr(A.idx, B.idx[q]) && dimOf[(int)B.idx[q]] != B.dim[q]) return CCSD_EINVAL;
+        dimOf[(int)B.idx[q]] = B.dim[q];
+    }
+    int nk = 0, nm = 0, nn = 0;
+    for (int q = 0; q < A.rank; q++) {
+        if (strchr(B.idx, A.idx[q])) K[nk++] = A.idx[q]; else MA[nm++] = A.idx[q];
+    }
+    for (int q = 0; q < B.rank; q++)
+        if (!strchr(A.idx, B.idx[q])) NB[nn++] = B.idx[q];
+    if (nm + nn > 4 || nm + nn != (int)strlen(outs[0].idx)) return CCSD_EINVAL;
+    int64_t M = 1, N = 1, Kk = 1;
+    for (int q = 0; q < nm; q++) M *= dimOf[(int)MA[q]];
+    for (int q = 0; q < nn; q++) N *= dimOf[(int)NB[q]];
+    for (int q = 0; q < nk; q++) Kk *= dimOf[(int)K[q]];
+    if (M * Kk > sc.elems || N * Kk > sc.elems || M * N > sc.elems) return CCSD_EINVAL;
+    if (M == 0 || N == 0) return CCSD_OK;
+    char ap[9] = {0}, bp[9] = {0}, cp[9] = {0};
+    strcpy(ap, MA); strcat(ap, K);
+    strcpy(bp, NB); strcat(bp, K);
+    strcpy(cp, MA); strcat(cp, NB);
+    const c128 *Ap = A.p, *Bp = B.p;
+    if (strcmp(ap, A.idx) != 0) { CCSD_TRY(permute_into(env.st, sc.a, ap, A, 1.0, 0)); Ap = sc.a; }
+    if (strcmp(bp, B.idx) != 0) { CCSD_TRY(permute_into(env.st, sc.b, bp, B, 1.0, 0)); Bp = sc.b; }
+    CCSD_TRY(run_gemm(env, gp(M, N, Kk, Ap, Kk, Bp, Kk, sc.c, N, 1, 1.0, 0)));
+    TView R;
+    R.p = sc.c; R.rank = nm + nn;
+    memset(R.idx, 0, sizeof(R.idx));
+    strcpy(R.idx, cp);
+    for (int q = 0; q < 4; q++) R.dim[q] = q < R.rank ? dimOf[(int)cp[q]] : 1;
+    for (int k = 0; k < nout; k++) CCSD_TRY(permute_into(env.st, C, outs[k].idx, R, alpha * outs[k].sign, 1));
+    return CCSD_OK;
+}
+// the common output patterns
+static int tc1(const Env& env, const TcScratch& sc, double alpha, const TView& A, const TView& B, c128* C, const char* o0)
+{
+    const TcOut outs[1] = {{o0, 1.0}};
+    return tensor_contract(env, sc, alpha, A, B, C, 1, outs);
+}
+// C += alpha (X - X with two labels exchanged): o0 and its exchanged twin o1
+static int tc2(const Env& env, const TcScratch& sc, double alpha, const TView& A, const TView& B, c128* C, const char* o0,
+               const char* o1)
+{
+    const TcOut outs[2] = {{o0, 1.0}, {o1, -1.0}};
+    return tensor_contract(env, sc, alpha, A, B, C, 2, outs);
+}
+static int tc4(const Env& env, const TcScratch& sc, double alpha, const TView& A, const TView& B, c128* C, const char* o0,
+               const char* o1, const char* o2, const char* o3)
+{   // P-(ij) P-(ab): + o0 - o1 - o2 + o3
+    const TcOut outs[4] = {{o0, 1.0}, {o1, -1.0}, {o2, -1.0}, {o3, 1.0}};
+    return tensor_contract(env, sc, alpha, A, B, C, 4, outs);
+}
+
+// ---- state of one Lambda solve (all pointers into the caller's Lambda workspace) --------------------------------------
+struct LambdaState {
+    bool ready;
+    TcScratch sc;
+    // unpacked copies of what the CCSD context holds packed
+    c128 *T2, *TAU, *OOVV, *OOOV, *WOOOO;          // [i][j][a][b], [m][n][e][f], [m][n][i][e], [m][n][i][j]
+    // elements of Hbar (constant during the solve)
+    c128 *Fov, *Foo, *Fvv;                         // [m][e], [m][i], [a][e]
+    c128 *Wvovv, *Wooov, *Wovvo, *Wovoo, *Wvvvo;   // [a][m][e][f], [m][n][i][e], [m][b][e][j], [m][b][i][j], [a][b][e][i]
+    c128 *inner, *X3, *Ypk;                        // build temporaries
+    // multipliers, residuals, per-iteration temporaries
+    c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
+    double* cl2s;                                  // 3M sum plane of conj(l2p)
+    // DIIS (as for the amplitudes: reading G13)
+    c128 *diis_u, *diis_e;
+    int nd, diis_count, diis_next;
+    int order[12], norder;
+    double gram[13 * 13];
+};
+
+static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* total)
+{
+    Carver w{base, 0};
+    const int64_t o = c->o, v = c->v, oo = c->oo, vv = c->vv, ov = c->ov;
+    const int64_t o2v2 = o * o * v * v, ov3 = o * v * v * v, o3v = o * o * o * v;
+    L->sc.elems = ov3 > o2v2 ? ov3 : o2v2;
+    if (L->sc.elems < o3v) L->sc.elems = o3v;
+    L->sc.a = w.take<c128>(L->sc.elems);
+    L->sc.b = w.take<c128>(L->sc.elems);
+    L->sc.c = w.take<c128>(L->sc.elems);
+    L->T2 = w.take<c128>(o2v2); L->TAU = w.take<c128>(o2v2); L->OOVV = w.take<c128>(o2v2);
+    L->OOOV = w.take<c128>(o3v); L->WOOOO = w.take<c128>(o * o * o * o);
+    L->Fov = w.take<c128>(ov); L->Foo = w.take<c128>(o * o); L->Fvv = w.take<c128>(v * v);
+    L->Wvovv = w.take<c128>(ov3); L->Wooov = w.take<c128>(o3v); L->Wovvo = w.take<c128>(o2v2);
+    L->Wovoo = w.take<c128>(o3v); L->Wvvvo = w.take<c128>(ov3);
+    L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v); L->Ypk = w.take<c128>(vv * v * o);
+    L->l1 = w.take<c128>(ov); L->l2p = w.take<c128>(oo * vv); L->L2 = w.take<c128>(o2v2);
+    L->R1 = w.take<c128>(ov); L->R2 = w.take<c128>(o2v2); L->R2p = w.take<c128>(oo * vv);
+    L->Gvv = w.take<c128>(v * v); L->Goo = w.take<c128>(o * o);
+    L->Lt = w.take<c128>(o3v); L->LT = w.take<c128>(o * o * o * o);
+    L->cl2p = w.take<c128>(oo * vv); L->P2 = w.take<c128>(oo * vv);
+    L->cl2s = w.take<double>(oo * vv);
+    L->nd = c->opt.ndiis;
+    const int nd = L->nd > 0 ? L->nd : 1;
+    L->diis_u = w.take<c128>((int64_t)nd * c->nvec);
+    L->diis_e = w.take<c128>((int64_t)nd * c->nvec);
+    *total = w.off;
+}
+
+// dense [x][y][p][q] from a tensor packed in its first pair (x<y, extent m1; pk1 = 0: that pair is stored unpacked) and
+// in its second pair (p<q, extent m2; pk2 = 0: unpacked): antisymmetric fill
+static void unpack_pairs(cudaStream_t st, c128* out, const c128* in, int m1, int pk1, int m2, int pk2, int64_t ncols = 0)
+{   // ncols: number of (opaque) columns when the second pair is not packed and is not an m2 x m2 pair
+    const int64_t n1 = (int64_t)m1 * m1, n2 = (!pk2 && ncols > 0) ? ncols : (int64_t)m2 * m2;
+    const int64_t ld = pk2 ? (int64_t)m2 * (m2 - 1) / 2 : n2;
+    launch_fill(st, out, n1, n2, n2, 0, [=] __device__(int64_t xy, int64_t pq) {
+        int x = (int)(xy / m1), y = (int)(xy % m1), p = (int)(pq / m2), q = (int)(pq % m2);
+        double sg = 1.0;
+        int64_t row = xy, col = pq;
+        if (pk1) {
+            if (x == y) return mk(0.0, 0.0);
+            if (x > y) { int t = x; x = y; y = t; sg = -sg; }
+            row = pair_idx(x, y, m1);
+        }
+        if (pk2) {
+            if (p == q) return mk(0.0, 0.0);
+            if (p > q) { int t = p; p = q; q = t; sg = -sg; }
+            col = pair_idx(p, q, m2);
+        }
+        return cscale(sg, in[row * ld + col]);
+    });
+}
+
+#define LV(ptr, idx, ...) tview(ptr, idx, __VA_ARGS__)
+
+// Elements of Hbar (eqs 45-49, 57 and the list of the paper's ref. 39; reading G23), once per solve.  Needs the
+// intermediates of a CCSD residual evaluation at the current amplitudes (tau, H^k_c, G^a_c, G^k_i, A^{kl}_{ij}).
+static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const TcScratch& sc = L->sc;
+    const int o = c->o, v = c->v;
+    const int64_t O = o, V = v, vv = c->vv;
+    CCSD_TRY(residual(c));                                    // tau, Hov, Gvv, Goo, Am of eqs 23-31 at the current (t1, t2)
+    unpack_pairs(st, L->T2, c->t2p, o, 1, v, 1);
+    unpack_pairs(st, L->TAU, c->taup, o, 1, v, 1);
+    unpack_pairs(st, L->OOVV, c->Voovv_p, o, 1, v, 1);
+    unpack_pairs(st, L->OOOV, c->Vooov_p, o, 1, 0, 0, O * V);
+    unpack_pairs(st, L->WOOOO, c->Am, o, 1, o, 1);             // eq 45 = eq 31
+    // Fbar^m_e = H^k_c (eq 28), Fbar^a_e = G^a_c (eq 57 = eq 25), Fbar^m_i = -G^k_i (eq 27)
+    dcopy(st, L->Fov, c->Hov, O * V);
+    dcopy(st, L->Fvv, c->Gvv, V * V);
+    CCSD_TRY(permute_into(st, L->Foo, "mi", LV(c->Goo, "mi", O, O), -1.0, 0));
+    const c128 *T1 = c->t1, *VOVV = c->Vvovv_u /* <ak||cd> stored [a][c][k][d] */, *VOVO = c->Vvovo_m /* <ak||ci> [a][i][c][k] */;
+    // W^{am}_{ef} = <am||ef> - t^a_n <nm||ef>
+    CCSD_TRY(permute_into(st, L->Wvovv, "amef", LV(VOVV, "aemf", V, V, O, V), 1.0, 0));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "na", O, V), LV(L->OOVV, "nmef", O, O, V, V), L->Wvovv, "amef"));
+    // W^{mn}_{ie} = <mn||ie> + t^f_i <mn||fe>
+    dcopy(st, L->Wooov, L->OOOV, O * O * O * V);
+    CCSD_TRY(tc1(env, sc, 1.0, LV(T1, "if", O, V), LV(L->OOVV, "mnfe", O, O, V, V), L->Wooov, "mnie"));
+    // eqs 46-47: W^{mb}_{ej} = <mb||ej> + t^f_j <mb||ef> - t^b_n <mn||ej> - (t^{fb}_{jn} + t^f_j t^b_n) <mn||ef>
+    CCSD_TRY(permute_into(st, L->Wovvo, "mbej", LV(VOVO, "bjem", V, O, V, O), -1.0, 0));                 // <mb||ej> = -<bm||ej>
+    dcopy(st, L->inner, L->Wovvo, O * O * V * V);
+    CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "jf", O, V), LV(VOVV, "bemf", V, V, O, V), L->Wovvo, "mbej"));      // <mb||ef> = -<bm||ef>
+    CCSD_TRY(tc1(env, sc, 1.0, LV(T1, "nb", O, V), LV(L->OOOV, "mnje", O, O, O, V), L->Wovvo, "mbej"));    // <mn||ej> = -<mn||je>
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->T2, "jnfb", O, O, V, V), LV(L->OOVV, "mnef", O, O, V, V), L->Wovvo, "mbej"));
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->X3, 0, (size_t)(O * O * O * V) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(T1, "jf", O, V), LV(L->OOVV, "mnef", O, O, V, V), L->X3, "jmne"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "nb", O, V), LV(L->X3, "jmne", O, O, O, V), L->Wovvo, "mbej"));
+    // inner^{mb}_{ej} = <mb||ej> - t^{bf}_{nj} <mn||ef>
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->T2, "njbf", O, O, V, V), LV(L->OOVV, "mnef", O, O, V, V), L->inner, "mbej"));
+    // W^{mb}_{ij}
+    CCSD_TRY(permute_into(st, L->Wovoo, "mbij", LV(L->OOOV, "ijmb", O, O, O, V), 1.0, 0, 1));               // conj <ij||mb>
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Fov, "me", O, V), LV(L->T2, "ijbe", O, O, V, V), L->Wovoo, "mbij"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "nb", O, V), LV(L->WOOOO, "mnij", O, O, O, O), L->Wovoo, "mbij"));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->TAU, "ijef", O, O, V, V), LV(VOVV, "bemf", V, V, O, V), L->Wovoo, "mbij"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->T2, "jnbe", O, O, V, V), LV(L->OOOV, "mnie", O, O, O, V), L->Wovoo, "mbij", "mbji"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(T1, "ie", O, V), LV(L->inner, "mbej", O, V, V, O), L->Wovoo, "mbij", "mbji"));
+    // eqs 48-49: W^{ab}_{ei}
+    CCSD_TRY(permute_into(st, L->Wvvvo, "abei", LV(VOVV, "eaib", V, V, O, V), 1.0, 0, 1));                  // conj <ei||ab>
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Fov, "me", O, V), LV(L->T2, "miab", O, O, V, V), L->Wvvvo, "abei"));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->TAU, "mnab", O, O, V, V), LV(L->OOOV, "mnie", O, O, O, V), L->Wvvvo, "abei"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->T2, "miaf", O, O, V, V), LV(VOVV, "bemf", V, V, O, V), L->Wvvvo, "abei", "baei"));
+    CCSD_TRY(tc2(env, sc, -1.0, LV(T1, "ma", O, V), LV(L->inner, "mbei", O, V, V, O), L->Wvvvo, "abei", "baei"));
+    // + t^f_i W^{ab}_{ef}, W^{ab}_{ef} = <ab||ef> - P(ab) t^b_m <am||ef> + 1/2 tau^{ab}_{mn} <mn||ef>, never stored:
+    //   (ii) -P(ab) t^b_m ( sum_f <am||ef> t^f_i )        (iii) 1/2 tau^{ab}_{mn} ( sum_f <mn||ef> t^f_i )
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->X3, 0, (size_t)(O * O * V * V) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(VOVV, "aemf", V, V, O, V), LV(T1, "if", O, V), L->X3, "amei"));
+    CCSD_TRY(tc2(env, sc, -1.0, LV(T1, "mb", O, V), LV(L->X3, "amei", V, O, V, O), L->Wvvvo, "abei", "baei"));
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->X3, 0, (size_t)(O * O * O * V) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->OOVV, "mnef", O, O, V, V), LV(T1, "if", O, V), L->X3, "mnei"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->TAU, "mnab", O, O, V, V), LV(L->X3, "mnei", O, O, V, O), L->Wvvvo, "abei"));
+    //   (i) sum_f <ab||ef> t^f_i from the packed <ab||cd>: rows (a<b) in slabs, unpacked in (e,f), times t1
+    {
+        const c128* W = c->W;
+        const int64_t slab_rows = (sc.elems / (V * V)) > 0 ? (sc.elems / (V * V)) : 1;
+        for (int64_t r0 = 0; r0 < vv; r0 += slab_rows) {
+            const int64_t nr = (vv - r0 < slab_rows) ? vv - r0 : slab_rows;
+            launch_fill(st, sc.a, nr * V, V, V, 0, [=] __device__(int64_t row, int64_t ff) {
+                const int64_t AB = r0 + row / v;
+                const int e = (int)(row % v);
+                return asym_col(W, AB, vv, e, (int)ff, v);
+            });
+            // Ypk[(a<b)][e][i] = sum_f U[(ab),e][f] t1[i][f]
+            CCSD_TRY(run_gemm(env, gp(nr * V, O, V, sc.a, V, T1, V, L->Ypk + r0 * V * O, O, 1, 1.0, 0)));
+        }
+        const c128* Y = L->Ypk;
+        c128* Wv = L->Wvvvo;
+        launch_fill(st, Wv, V * V, V * O, V * O, 1, [=] __device__(int64_t ab, int64_t ei) {
+            const int a = (int)(ab / v), b = (int)(ab % v);
+            if (a == b) return mk(0.0, 0.0);
+            return a < b ? Y[pair_idx(a, b, v) * ((int64_t)v * o) + ei] : cneg(Y[pair_idx(b, a, v) * ((int64_t)v * o) + ei]);
+        });
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// Right-hand sides of eqs 52-56 at the current multipliers: R1[i][a], R2p[(i<j)][(a<b)].
+static int lambda_residual(ccsd_ctx* c, LambdaState* L)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const TcScratch& sc = L->sc;
+    const int o = c->o, v = c->v, n = c->n;
+    const int64_t O = o, V = v, oo = c->oo, vv = c->vv;
+    const c128 *VOVV = c->Vvovv_u;
+    unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
+    // eqs 50-51
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->Gvv, 0, (size_t)(V * V) * sizeof(c128), st));
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->Goo, 0, (size_t)(O * O) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->T2, "mnef", O, O, V, V), LV(L->L2, "mnaf", O, O, V, V), L->Gvv, "ae"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->T2, "mnef", O, O, V, V), LV(L->L2, "inef", O, O, V, V), L->Goo, "mi"));
+    // eqs 55-56
+    dcopy(st, L->R1, L->Fov, O * V);
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Fvv, "ea", V, V), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Foo, "im", O, O), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Goo, "mn", O, O), LV(L->Wooov, "mina", O, O, O, V), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Gvv, "ef", V, V), LV(L->Wvovv, "eifa", V, O, V, V), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->Wovvo, "ieam", O, V, V, O), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->L2, "mnae", O, O, V, V), LV(L->Wovoo, "iemn", O, V, O, O), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "imef", O, O, V, V), LV(L->Wvvvo, "efam", V, V, V, O), L->R1, "ia"));
+    // eqs 52-54, unpacked [i][j][a][b]
+    dcopy(st, L->R2, L->OOVV, O * O * V * V);
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->L2, "ijae", O, O, V, V), LV(L->Fvv, "eb", V, V), L->R2, "ijab", "ijba"));
+    CCSD_TRY(tc2(env, sc, -1.0, LV(L->L2, "imab", O, O, V, V), LV(L->Foo, "jm", O, O), L->R2, "ijab", "jiab"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "mnab", O, O, V, V), LV(L->WOOOO, "ijmn", O, O, O, O), L->R2, "ijab"));
+    CCSD_TRY(tc4(env, sc, 1.0, LV(L->L2, "imae", O, O, V, V), LV(L->Wovvo, "jebm", O, V, V, O), L->R2, "ijab", "jiab", "ijba", "jiba"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->OOVV, "ijae", O, O, V, V), LV(L->Gvv, "be", V, V), L->R2, "ijab", "ijba"));
+    CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
+    CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Wvovv, "ejab", V, O, V, V), L->R2, "ijab", "jiab"));
+    CCSD_TRY(tc4(env, sc, 1.0, LV(L->l1, "ia", O, V), LV(L->Fov, "jb", O, V), L->R2, "ijab", "jiab", "ijba", "jiba"));
+    // 1/2 lambda^{ij}_{ef} W^{ef}_{ab}, W^{ef}_{ab} = <ef||ab> - P(ef) t^f_m <em||ab> + 1/2 tau^{ef}_{mn} <mn||ab>, never stored:
+    //   (ii) - ( sum_f lambda^{ij}_{ef} t^f_m ) <em||ab>      (iii) 1/4 ( sum_ef lambda^{ij}_{ef} tau^{ef}_{mn} ) <mn||ab>
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->Lt, 0, (size_t)(O * O * O * V) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "ijef", O, O, V, V), LV(c->t1, "mf", O, V), L->Lt, "ijem"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Lt, "ijem", O, O, V, O), LV(VOVV, "eamb", V, V, O, V), L->R2, "ijab"));
+    CCSD_CUDA_TRY(cudaMemsetAsync(L->LT, 0, (size_t)(O * O * O * O) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "ijef", O, O, V, V), LV(L->TAU, "mnef", O, O, V, V), L->LT, "ijmn"));
+    CCSD_TRY(tc1(env, sc, 0.25, LV(L->LT, "ijmn", O, O, O, O), LV(L->OOVV, "mnab", O, O, V, V), L->R2, "ijab"));
+    //   (i) sum_{e<f} lambda^{ij}_{ef} <ef||ab> = conj( sum_{e<f} conj(lambda) <ab||ef> ): the pp-ladder launch of the CCSD
+    //       iteration (packed, Hermitian <ab||cd>, 3M with sum planes) on the conjugated multipliers
+    {
+        const c128* l2p = L->l2p;
+        double* plane = c->planes ? L->cl2s : nullptr;
+        launch_fill(st, L->cl2p, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t EF) {
+            c128 x = cconj(l2p[IJ * vv + EF]);
+            if (plane) plane[IJ * vv + EF] = x.x + x.y;
+            return x;
+        });
+        CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
+    }
+    {   // pack: R2p[(i<j)][(a<b)] = R2[i][j][a][b] + conj(P2)
+        const c128 *R2 = L->R2, *P2 = L->P2;
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(st, L->R2p, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            return cadd(R2[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(P2[IJ * vv + AB]));
+        });
+    }
+    (void)n;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// One Lambda iteration: residual, Jacobi step lambda <- lambda + R/D with the CCSD denominators, DIIS as for the
+// amplitudes (readings G12, G13, G23).  Returns ||R/D||_2 over the unique multipliers through *step_norm (host).
+static int lambda_iterate(ccsd_ctx* c, LambdaState* L, double* step_norm)
+{
+    CCSD_TRY(lambda_residual(c, L));
+    cudaStream_t st = c->st;
+    const int o = c->o, v = c->v;
+    const int64_t vv = c->vv, ov = c->ov, nvec = c->nvec;
+    const int nd = L->nd;
+    const int slot = nd > 0 ? L->diis_next : 0;
+    c128* U = L->diis_u + (int64_t)slot * nvec;
+    c128* Ev = L->diis_e + (int64_t)slot * nvec;
+    {
+        const c128 *R1 = L->R1, *R2p = L->R2p, *l1 = L->l1, *l2p = L->l2p;
+        const double* eps = c->eps;
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(st, Ev, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
+            const double d = eps[i] - eps[o + a];
+            const c128 e = mk(R1[i * v + a].x / d, R1[i * v + a].y / d);
+            U[i * v + a] = cadd(l1[i * v + a], e);
+            return e;
+        });
+        c128 *E2 = Ev + ov, *U2 = U + ov;
+        launch_fill(st, E2, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            const double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
+            const c128 s = R2p[IJ * vv + AB];
+            const c128 e = mk(s.x / d, s.y / d);
+            U2[IJ * vv + AB] = cadd(l2p[IJ * vv + AB], e);
+            return e;
+        });
+    }
+    int order[13], m = 0;
+    if (nd > 0) {
+        for (int k = 0; k < L->norder; k++)
+            if (L->order[k] != slot) order[m++] = L->order[k];
+        order[m++] = slot;
+    } else {
+        order[m++] = 0;
+    }
+    CCSD_CUDA_TRY(cudaMemsetAsync(c->red, 0, 16 * sizeof(double), st));
+    for (int k = 0; k < m; k++) launch_redot(st, Ev, L->diis_e + (int64_t)order[k] * nvec, nvec, c->red + k);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host, c->red, 16 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(st));
+    for (int k = 0; k < m; k++) {
+        L->gram[slot * 13 + order[k]] = c->red_host[k];
+        L->gram[order[k] * 13 + slot] = c->red_host[k];
+    }
+    const double snorm = sqrt(c->red_host[m - 1] > 0 ? c->red_host[m - 1] : 0.0);
+    std::vector<double> coef(m, 0.0);
+    int status = CCSD_OK;
+    if (nd > 0 && m >= 2) {
+        int mm = m;
+        for (;;) {
+            const int dim = mm + 1;
+            std::vector<double> A(dim * dim, 0.0), rhs(dim, 0.0);
+            for (int a = 0; a < mm; a++)
+                for (int b = 0; b < mm; b++) A[a * dim + b] = L->gram[order[m - mm + a] * 13 + order[m - mm + b]];
+            for (int a = 0; a < mm; a++) { A[a * dim + mm] = -1.0; A[mm * dim + a] = -1.0; }
+            rhs[mm] = -1.0;
+            if (solve_small(A, rhs, dim) == 0) {
+                for (int a = 0; a < mm; a++) coef[m - mm + a] = rhs[a];
+                break;
+            }
+            if (--mm < 1) { status = CCSD_ESINGULAR; coef.assign(m, 0.0); coef[m - 1] = 1.0; break; }
+        }
+    } else {
+        coef[m - 1] = 1.0;
+    }
+    DiisCombo combo;
+    combo.m = m;
+    for (int k = 0; k < m; k++) { combo.c[k] = coef[k]; combo.u[k] = L->diis_u + (int64_t)order[k] * nvec; }
+    launch_combine(st, combo, L->l1, L->l2p, ov, nvec);
+    if (nd > 0) {
+        for (int k = 0; k < m; k++) L->order[k] = order[k];
+        L->norder = m;
+        L->diis_next = (slot + 1) % nd;
+        if (L->diis_count < nd) L->diis_count++;
+    }
+    if (step_norm) *step_norm = snorm;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return status;
+}
+
+// eqs 58-61: D[p][q] = <0|(1+Lambda) exp(-T) a+_p a_q exp(T)|0> - delta_pq(occ), [n][n] (device), unsymmetrised (reading G24)
+static int lambda_density(ccsd_ctx* c, LambdaState* L, c128* D)
+{
+    cudaStream_t st = c->st;
+    const Env& env = c->env;
+    const TcScratch& sc = L->sc;
+    const int o = c->o, v = c->v, n = c->n;
+    const int64_t O = o, V = v;
+    unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
+    // temporaries: the residual buffers of the solver are free between iterations
+    c128 *goo = L->Goo, *gab = L->Gvv, *gai = L->R1, *x_oo = L->LT, *x_ea = L->X3;
+    CCSD_CUDA_TRY(cudaMemsetAsync(goo, 0, (size_t)(O * O) * sizeof(c128), st));
+    CCSD_CUDA_TRY(cudaMemsetAsync(gab, 0, (size_t)(V * V) * sizeof(c128), st));
+    // eq 58: gamma_ij = -1/2 t^{ef}_{im} lambda^{jm}_{ef} - t^e_i lambda^j_e
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->T2, "imef", O, O, V, V), LV(L->L2, "jmef", O, O, V, V), goo, "ij"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(c->t1, "ie", O, V), LV(L->l1, "je", O, V), goo, "ij"));
+    // eq 61: gamma_ab = 1/2 t^{ae}_{mn} lambda^{mn}_{be} + t^a_m lambda^m_b
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->T2, "mnae", O, O, V, V), LV(L->L2, "mnbe", O, O, V, V), gab, "ab"));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(c->t1, "ma", O, V), LV(L->l1, "mb", O, V), gab, "ab"));
+    // eq 60 as [i][a]: t + lambda^m_e (t^{ae}_{im} - t^e_i t^a_m) - 1/2 lambda^{mn}_{ef} (t^{ef}_{in} t^a_m + t^e_i t^{af}_{mn})
+    dcopy(st, gai, c->t1, O * V);
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->T2, "imae", O, O, V, V), gai, "ia"));
+    //   - ( sum_e lambda^m_e t^e_i + 1/2 sum_nef lambda^{mn}_{ef} t^{ef}_{in} ) t^a_m
+    CCSD_CUDA_TRY(cudaMemsetAsync(x_oo, 0, (size_t)(O * O) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(c->t1, "ie", O, V), x_oo, "mi"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "mnef", O, O, V, V), LV(L->T2, "inef", O, O, V, V), x_oo, "mi"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(x_oo, "mi", O, O), LV(c->t1, "ma", O, V), gai, "ia"));
+    //   - 1/2 t^e_i ( sum_mnf lambda^{mn}_{ef} t^{af}_{mn} )
+    CCSD_CUDA_TRY(cudaMemsetAsync(x_ea, 0, (size_t)(V * V) * sizeof(c128), st));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "mnef", O, O, V, V), LV(L->T2, "mnaf", O, O, V, V), x_ea, "ea"));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(c->t1, "ie", O, V), LV(x_ea, "ea", V, V), gai, "ia"));
+    const c128* l1 = L->l1;
+    launch_fill(st, D, n, n, n, 0, [=] __device__(int64_t p, int64_t q) {
+        if (p < o && q < o) return goo[p * o + q];                       // gamma_ij = <a+_i a_j>
+        if (p >= o && q >= o) return gab[(q - o) * v + (p - o)];         // gamma_ab = <a+_b a_a>
+        if (p < o) return gai[p * v + (q - o)];                          // <a+_i a_a> = gamma_ai
+        return l1[q * v + (p - o)];                                      // <a+_a a_i> = gamma_ia = lambda^i_a
+    });
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+#undef LV

@@ -95,7 +95,8 @@ def test_product_does_not_import_oracle():
                 assert "oracle" not in text.replace("shares nothing with oracle/", "").replace(
                     "no code shared with oracle/", "") or f in ("ccsd_lib.cu", "common.cuh"), f
                 assert "import oracle" not in text and "from oracle" not in text, f
-    for f in ("ccsd_oracle.py", "ccsd_oracle.c"):
+    for f in ("ccsd_oracle.py", "ccsd_oracle.c", "cc2_oracle.py", "cc2_oracle.c", "triples_oracle.py", "triples_oracle.c",
+              "lambda_oracle.py"):
         text = open(os.path.join(ROOT, "oracle", f)).read()
         assert not re.search(r"^\s*(import|from)\s+paper_2103_08473_b200", text, flags=re.M), f
         assert not re.search(r"#\s*include\s*[<\"].*ccsd\.h", text), f

@@ -1,0 +1,107 @@
+"""GPU parity of the Lambda equations and the one-body density (Appendix 7.4-7.5) against the
+Lambda oracle (oracle/lambda_oracle.py, pinned by tests/test_lambda_pins.py).
+
+Compared element by element (1e-12 relative max-abs): the right-hand sides of eqs 52-56 at seeded RANDOM multipliers
+(every element of Hbar and every term enters) and at lambda = conj(t); the density matrix of eqs 58-61; lock-step
+||R/D||_2 and multipliers over the iterations with DIIS(6).  Both sides start from their own converged amplitudes.
+"""
+import numpy as np
+import pytest
+
+import ccsd_inputs as ci
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2103_08473_b200 as lib
+    lib.load_library()
+    return lib
+
+
+def _rel(a, b):
+    scale = np.abs(b).max()
+    return np.abs(np.asarray(a) - np.asarray(b)).max() / (scale if scale > 0 else 1.0)
+
+
+def _pair(gpu, name):
+    from oracle.ccsd_oracle import OracleCCSD
+    from oracle.lambda_oracle import OracleLambda
+    if name == "ragged":
+        inp = ci.make_inputs(5, 13, 21, seed=4713, b_scale=0.06, f_offdiag=0.03)
+    elif name == "ragged2":
+        inp = ci.make_inputs(7, 18, 30, seed=4714)
+    else:
+        inp = ci.make_config(name)
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    oc.run(80, tol=1e-13)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    ok, _, _, _ = gc.solve(1e-13, 80)
+    assert ok
+    return inp, oc, OracleLambda(oc), gc
+
+
+@pytest.mark.parametrize("name", ["cfg0_2e", "cfg0", "ragged", "ragged2"])
+def test_lambda_residual_and_density_match_oracle(gpu, name):
+    from oracle.ccsd_oracle import pack_t2, unpack_t2
+    inp, oc, ol, gc = _pair(gpu, name)
+    o, v = inp.nocc, inp.nvir
+    gc.lambda_init()
+    # (a) at the start multipliers conj(t)
+    R1, R2 = ol.residual()
+    r1, r2p = gc.lambda_residual()
+    assert _rel(r1.cpu().numpy(), R1) <= 1e-10 and _rel(r2p.cpu().numpy(), pack_t2(R2)) <= 1e-10   # t differs by ~1e-13
+    # (b) at seeded random multipliers, same on both sides
+    l1, l2p = ci.random_amplitudes(o, v, 44, 0.2)
+    gc.set_lambda(l1, l2p)
+    R1, R2 = ol.residual(l1, unpack_t2(l2p, o, v))
+    r1, r2p = gc.lambda_residual()
+    assert _rel(r1.cpu().numpy(), R1) <= 1e-10
+    assert _rel(r2p.cpu().numpy(), pack_t2(R2)) <= 1e-10
+    D = gc.density().cpu().numpy()
+    assert _rel(D, ol.density(l1, unpack_t2(l2p, o, v))) <= 1e-10
+    gc.close()
+
+
+def test_lambda_exact_parity_at_identical_amplitudes(gpu):
+    """Same amplitudes on both sides (the oracle's converged ones are handed to the library): 1e-12."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
+    from oracle.lambda_oracle import OracleLambda
+    inp = ci.make_inputs(6, 15, 24, seed=4715)
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    oc.run(80, tol=1e-13)
+    ol = OracleLambda(oc)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+    gc.lambda_init()
+    l1, l2p = ci.random_amplitudes(o, v, 45, 0.2)
+    gc.set_lambda(l1, l2p)
+    R1, R2 = ol.residual(l1, unpack_t2(l2p, o, v))
+    r1, r2p = gc.lambda_residual()
+    assert _rel(r1.cpu().numpy(), R1) <= REL_TOL
+    assert _rel(r2p.cpu().numpy(), pack_t2(R2)) <= REL_TOL
+    assert _rel(gc.density().cpu().numpy(), ol.density(l1, unpack_t2(l2p, o, v))) <= REL_TOL
+    gc.close()
+
+
+@pytest.mark.parametrize("name,nit", [("cfg0", 14), ("ragged", 10)])
+def test_lambda_lockstep_iterations(gpu, name, nit):
+    from oracle.ccsd_oracle import pack_t2
+    inp, oc, ol, gc = _pair(gpu, name)
+    gc.lambda_init()
+    for _ in range(nit):
+        so = ol.iterate()
+        sg = gc.lambda_iterate()
+        assert abs(sg - so) <= 1e-9 * max(1.0, so) + 1e-12
+    l1, l2p = gc.get_lambda()
+    assert _rel(l1.cpu().numpy(), ol.l1) <= 1e-9 and _rel(l2p.cpu().numpy(), pack_t2(ol.l2)) <= 1e-9
+    assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-9
+    gc.close()
