@@ -297,6 +297,34 @@ def triples_bench(torch, pkg, inp, o, v, peak_tflops):
                     "executed (3M) flops"}
 
 
+def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
+    """NEXT-2 row of SURVEY 8(f): Lambda equations at the amplitudes after three CCSD iterations
+    (the cost of a Lambda iteration does not depend on the convergence of T): Hbar build once, then timed iterations."""
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    for _ in range(3):
+        solver.iterate()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    solver.lambda_init()
+    e1.record()
+    torch.cuda.synchronize()
+    init_ms = e0.elapsed_time(e1)
+    ts = time_events(torch, solver.lambda_iterate, steps, warmup)
+    sn = solver.lambda_iterate()
+    D = solver.density()
+    tr = complex(torch.trace(D).item())
+    ws = solver._lam_ws.numel()
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    return {"s_per_iteration": round(statistics.median(ts) * 1e-3, 5), "hbar_build_s": round(init_ms * 1e-3, 4),
+            "steps": steps, "warmup": warmup, "step_norm_last": sn, "density_trace_abs": abs(tr),
+            "workspace_gib": round(ws / 2 ** 30, 1),
+            "note": "first CUDA path: one permute + DMMA GEMM + signed permuted add per term; pp-ladder term on the packed "
+                    "<ab||cd> with conjugated multipliers"}
+
+
 def max_over_ranks(value: float, dist, device="cuda") -> float:
     """Multi-GPU numbers are the MAX over ranks (replicas-only path: no data-path collective exists)."""
     import torch
@@ -354,6 +382,10 @@ def run_ours(args) -> None:
         return
     inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
     pkg.load_library()
+    if args.only_lambda:
+        print(json.dumps({"metric": "lambda_seconds_per_iteration", "unit": "s", "config": {"workload": f"{cfg} Lambda"},
+                          **lambda_bench(torch, pkg, inp, o, v)}))
+        return
     if args.only_triples:
         # profiling aid: ccsd_init, one iteration, then the perturbative triples of this workload (same launches as
         # the "triples" leg of the default run)
@@ -469,6 +501,7 @@ def run_ours(args) -> None:
     torch.cuda.empty_cache()
     cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     triples = triples_bench(torch, pkg, inp, o, v, peak) if not args.no_sweep else None
+    lam = lambda_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
     cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
@@ -492,7 +525,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "cc2": cc2, "triples": triples, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "triples": triples, "lambda": lam, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:
@@ -509,6 +542,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
+    ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")
     ap.add_argument("--only-triples", action="store_true", help="time only the perturbative triples of --config")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -24,7 +24,12 @@ import numpy as np
 
 from oracle.ccsd_oracle import C128, pack_t2, unpack_t2
 
-E = np.einsum
+
+
+def E(subscripts, *operands):
+    """One printed term = one einsum; optimize=True lets numpy hand the two-operand products to its matmul."""
+    return np.einsum(subscripts, *operands, optimize=True)
+
 
 
 def _p_ij(x):

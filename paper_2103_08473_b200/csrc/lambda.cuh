@@ -78,6 +78,8 @@ struct LambdaState {
     c128 *inner, *X3, *Ypk;                        // build temporaries
     // multipliers, residuals, per-iteration temporaries
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
+    // packed (i<j, a<b) route of the terms whose output is antisymmetric and whose contraction runs over a packable pair
+    c128 *Pacc, *l2pT, *LTp, *L2hu, *Ltp, *Amc, *TAUp, *VoovvT, *VT2;
     double* cl2s;                                  // 3M sum plane of conj(l2p)
     // DIIS (as for the amplitudes: reading G13)
     c128 *diis_u, *diis_e;
@@ -108,6 +110,9 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Lt = w.take<c128>(o3v); L->LT = w.take<c128>(o * o * o * o);
     L->cl2p = w.take<c128>(oo * vv); L->P2 = w.take<c128>(oo * vv);
     L->cl2s = w.take<double>(oo * vv);
+    L->Pacc = w.take<c128>(oo * vv); L->l2pT = w.take<c128>(vv * oo); L->LTp = w.take<c128>(oo * oo);
+    L->L2hu = w.take<c128>(oo * v * v); L->Ltp = w.take<c128>(oo * ov); L->Amc = w.take<c128>(oo * oo);
+    L->TAUp = w.take<c128>(oo * vv); L->VoovvT = w.take<c128>(vv * oo); L->VT2 = w.take<c128>(vv * ov);
     L->nd = c->opt.ndiis;
     const int nd = L->nd > 0 ? L->nd : 1;
     L->diis_u = w.take<c128>((int64_t)nd * c->nvec);
@@ -221,6 +226,11 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
             return a < b ? Y[pair_idx(a, b, v) * ((int64_t)v * o) + ei] : cneg(Y[pair_idx(b, a, v) * ((int64_t)v * o) + ei]);
         });
     }
+    // packed operands of the iteration: A^{kl}_{ij} and tau as they are now, <mn||ab> and <em||ab> with the (a<b) pair as row
+    dcopy(st, L->Amc, c->Am, c->oo * c->oo);
+    dcopy(st, L->TAUp, c->taup, c->oo * vv);
+    CCSD_TRY(launch_transpose2d(st, c->Voovv_p, L->VoovvT, c->oo, vv, 0));
+    CCSD_TRY(launch_transpose2d(st, c->Vvovv_p, L->VT2, c->ov, vv, 0));
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -253,21 +263,29 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     dcopy(st, L->R2, L->OOVV, O * O * V * V);
     CCSD_TRY(tc2(env, sc, 1.0, LV(L->L2, "ijae", O, O, V, V), LV(L->Fvv, "eb", V, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->L2, "imab", O, O, V, V), LV(L->Foo, "jm", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "mnab", O, O, V, V), LV(L->WOOOO, "ijmn", O, O, O, O), L->R2, "ijab"));
     CCSD_TRY(tc4(env, sc, 1.0, LV(L->L2, "imae", O, O, V, V), LV(L->Wovvo, "jebm", O, V, V, O), L->R2, "ijab", "jiab", "ijba", "jiba"));
     CCSD_TRY(tc2(env, sc, 1.0, LV(L->OOVV, "ijae", O, O, V, V), LV(L->Gvv, "be", V, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
     CCSD_TRY(tc2(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Wvovv, "ejab", V, O, V, V), L->R2, "ijab", "jiab"));
     CCSD_TRY(tc4(env, sc, 1.0, LV(L->l1, "ia", O, V), LV(L->Fov, "jb", O, V), L->R2, "ijab", "jiab", "ijba", "jiba"));
+    // The terms with an antisymmetric (i<j, a<b) output and a pair-wise contraction run packed, into Pacc[(i<j)][(a<b)]:
+    //   sum_{m<n} lambda^{mn}_{ab} W^{ij}_{mn}   (W^{ij}_{mn} = A^{kl}_{ij} of eq 31, packed in both pairs)
+    CCSD_TRY(launch_transpose2d(st, L->l2p, L->l2pT, oo, vv, 0));
+    CCSD_TRY(run_gemm(env, gp(vv, oo, oo, L->l2pT, oo, L->Amc, oo, L->Pacc, 1, vv, 1.0, 0)));
     // 1/2 lambda^{ij}_{ef} W^{ef}_{ab}, W^{ef}_{ab} = <ef||ab> - P(ef) t^f_m <em||ab> + 1/2 tau^{ef}_{mn} <mn||ab>, never stored:
-    //   (ii) - ( sum_f lambda^{ij}_{ef} t^f_m ) <em||ab>      (iii) 1/4 ( sum_ef lambda^{ij}_{ef} tau^{ef}_{mn} ) <mn||ab>
-    CCSD_CUDA_TRY(cudaMemsetAsync(L->Lt, 0, (size_t)(O * O * O * V) * sizeof(c128), st));
-    CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "ijef", O, O, V, V), LV(c->t1, "mf", O, V), L->Lt, "ijem"));
-    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Lt, "ijem", O, O, V, O), LV(VOVV, "eamb", V, V, O, V), L->R2, "ijab"));
-    CCSD_CUDA_TRY(cudaMemsetAsync(L->LT, 0, (size_t)(O * O * O * O) * sizeof(c128), st));
-    CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "ijef", O, O, V, V), LV(L->TAU, "mnef", O, O, V, V), L->LT, "ijmn"));
-    CCSD_TRY(tc1(env, sc, 0.25, LV(L->LT, "ijmn", O, O, O, O), LV(L->OOVV, "mnab", O, O, V, V), L->R2, "ijab"));
+    //   (iii) sum_{m<n} ( sum_{e<f} lambda^{ij}_{ef} tau^{ef}_{mn} ) <mn||ab>
+    CCSD_TRY(run_gemm(env, gp(oo, oo, vv, L->l2p, vv, L->TAUp, vv, L->LTp, oo, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(env, gp(vv, oo, oo, L->VoovvT, oo, L->LTp, oo, L->Pacc, 1, vv, 1.0, 1)));
+    //   (ii) - sum_{em} ( sum_f lambda^{ij}_{ef} t^f_m ) <em||ab>
+    {
+        const c128* l2p = L->l2p;
+        launch_fill(st, L->L2hu, oo * V, V, V, 0, [=] __device__(int64_t row, int64_t ff) {
+            return asym_col(l2p, row / v, vv, (int)(row % v), (int)ff, v);
+        });
+        CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, c->t1, V, L->Ltp, O, 1, 1.0, 0)));
+        CCSD_TRY(run_gemm(env, gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1)));
+    }
     //   (i) sum_{e<f} lambda^{ij}_{ef} <ef||ab> = conj( sum_{e<f} conj(lambda) <ab||ef> ): the pp-ladder launch of the CCSD
     //       iteration (packed, Hermitian <ab||cd>, 3M with sum planes) on the conjugated multipliers
     {
@@ -280,12 +298,12 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         });
         CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
     }
-    {   // pack: R2p[(i<j)][(a<b)] = R2[i][j][a][b] + conj(P2)
-        const c128 *R2 = L->R2, *P2 = L->P2;
+    {   // pack: R2p[(i<j)][(a<b)] = R2[i][j][a][b] + conj(P2) + Pacc
+        const c128 *R2 = L->R2, *P2 = L->P2, *Pacc = L->Pacc;
         const int2 *po = c->po, *pv = c->pv;
         launch_fill(st, L->R2p, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
             const int2 ij = po[IJ], ab = pv[AB];
-            return cadd(R2[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(P2[IJ * vv + AB]));
+            return cadd(cadd(R2[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(P2[IJ * vv + AB])), Pacc[IJ * vv + AB]);
         });
     }
     (void)n;

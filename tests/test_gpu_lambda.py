@@ -105,3 +105,32 @@ def test_lambda_lockstep_iterations(gpu, name, nit):
     assert _rel(l1.cpu().numpy(), ol.l1) <= 1e-9 and _rel(l2p.cpu().numpy(), pack_t2(ol.l2)) <= 1e-9
     assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-9
     gc.close()
+
+
+def test_lambda_cfg1_identical_amplitudes(gpu):
+    """cfg1 (16/96): several DMMA tiles in every GEMM of the Lambda path.  The oracle's amplitudes after two CCSD
+    iterations are handed to the library (the working equations are compared term for term; convergence of T is not
+    needed for that); residuals at random multipliers, density, two lock-step iterations."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
+    from oracle.lambda_oracle import OracleLambda
+    inp = ci.make_config("cfg1")
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v, restricted=True)
+    for _ in range(2):
+        oc.iterate()
+    ol = OracleLambda(oc)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+    gc.lambda_init()
+    l1, l2p = ci.random_amplitudes(o, v, 46, 0.05)
+    gc.set_lambda(l1, l2p)
+    R1, R2 = ol.residual(l1, unpack_t2(l2p, o, v))
+    r1, r2p = gc.lambda_residual()
+    assert _rel(r1.cpu().numpy(), R1) <= REL_TOL
+    assert _rel(r2p.cpu().numpy(), pack_t2(R2)) <= REL_TOL
+    assert _rel(gc.density().cpu().numpy(), ol.density(l1, unpack_t2(l2p, o, v))) <= REL_TOL
+    gc.set_lambda(np.conj(oc.t1), np.conj(pack_t2(oc.t2)))
+    for _ in range(2):
+        so, sg = ol.iterate(), gc.lambda_iterate()
+        assert abs(sg - so) <= 1e-10 * max(1.0, so)
+    gc.close()
