@@ -8,7 +8,7 @@
 
 // C[out index orders] += sign * alpha * sum_k A B   (see tensor_ops.cuh).  Extents are taken from the operands.
 static int tensor_contract(const Env& env, const TcScratch& sc, double alpha, const TView& A, const TView& B, c128* C, int nout,
-                           const TcOut* outs)
+                           const TcOut* outs, bool may_swap = true)
 {
     char K[5] = {0}, MA[5] = {0}, NB[5] = {0};
     int64_t dimOf[128];
@@ -30,6 +30,9 @@ static int tensor_contract(const Env& env, const TcScratch& sc, double alpha, co
     for (int q = 0; q < nk; q++) Kk *= dimOf[(int)K[q]];
     if (M * Kk > sc.elems || N * Kk > sc.elems || M * N > sc.elems) return CCSD_EINVAL;
     if (M == 0 || N == 0) return CCSD_OK;
+    // the DMMA tiles are 128 rows x 48 columns: put the operand whose free extent pads less into the row position
+    if (may_swap && N > 1 && (M == 1 || round_up(N, 128) * round_up(M, 48) < round_up(M, 128) * round_up(N, 48)))
+        return tensor_contract(env, sc, alpha, B, A, C, nout, outs, false);
     char ap[9] = {0}, bp[9] = {0}, cp[9] = {0};
     strcpy(ap, MA); strcat(ap, K);
     strcpy(bp, NB); strcat(bp, K);
@@ -37,7 +40,11 @@ static int tensor_contract(const Env& env, const TcScratch& sc, double alpha, co
     const c128 *Ap = A.p, *Bp = B.p;
     if (strcmp(ap, A.idx) != 0) { CCSD_TRY(permute_into(env.st, sc.a, ap, A, 1.0, 0)); Ap = sc.a; }
     if (strcmp(bp, B.idx) != 0) { CCSD_TRY(permute_into(env.st, sc.b, bp, B, 1.0, 0)); Bp = sc.b; }
-    CCSD_TRY(run_gemm(env, gp(M, N, Kk, Ap, Kk, Bp, Kk, sc.c, N, 1, 1.0, 0)));
+    if (N == 1) {   // matrix-vector product: one pass over the matrix at HBM speed
+        CCSD_TRY(run_gemv(env, M, Kk, Ap, Kk, Bp, sc.c, 1, 1.0, 0));
+    } else {
+        CCSD_TRY(run_gemm(env, gp(M, N, Kk, Ap, Kk, Bp, Kk, sc.c, N, 1, 1.0, 0)));
+    }
     TView R;
     R.p = sc.c; R.rank = nm + nn;
     memset(R.idx, 0, sizeof(R.idx));
@@ -76,6 +83,7 @@ struct LambdaState {
     c128 *Fov, *Foo, *Fvv;                         // [m][e], [m][i], [a][e]
     c128 *Wvovv, *Wooov, *Wovvo, *Wovoo, *Wvvvo;   // [a][m][e][f], [m][n][i][e], [m][b][e][j], [m][b][i][j], [a][b][e][i]
     c128 *inner, *X3, *Ypk;                        // build temporaries
+    c128 *Wvovv_iaef, *Wvovv_jabe, *Wvvvo_amef;    // the o v^3 elements in the operand layouts of the iteration (no per-iteration permute)
     // multipliers, residuals, per-iteration temporaries
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
     // packed (i<j, a<b) route of the terms whose output is antisymmetric and whose contraction runs over a packable pair
@@ -103,6 +111,7 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Fov = w.take<c128>(ov); L->Foo = w.take<c128>(o * o); L->Fvv = w.take<c128>(v * v);
     L->Wvovv = w.take<c128>(ov3); L->Wooov = w.take<c128>(o3v); L->Wovvo = w.take<c128>(o2v2);
     L->Wovoo = w.take<c128>(o3v); L->Wvvvo = w.take<c128>(ov3);
+    L->Wvovv_iaef = w.take<c128>(ov3); L->Wvovv_jabe = w.take<c128>(ov3); L->Wvvvo_amef = w.take<c128>(ov3);
     L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v); L->Ypk = w.take<c128>(vv * v * o);
     L->l1 = w.take<c128>(ov); L->l2p = w.take<c128>(oo * vv); L->L2 = w.take<c128>(o2v2);
     L->R1 = w.take<c128>(ov); L->R2 = w.take<c128>(o2v2); L->R2p = w.take<c128>(oo * vv);
@@ -226,6 +235,10 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
             return a < b ? Y[pair_idx(a, b, v) * ((int64_t)v * o) + ei] : cneg(Y[pair_idx(b, a, v) * ((int64_t)v * o) + ei]);
         });
     }
+    // the o v^3 elements in the [free][contracted] layouts the iteration contracts them in
+    CCSD_TRY(permute_into(st, L->Wvovv_iaef, "iaef", LV(L->Wvovv, "eifa", V, O, V, V), 1.0, 0));
+    CCSD_TRY(permute_into(st, L->Wvovv_jabe, "jabe", LV(L->Wvovv, "ejab", V, O, V, V), 1.0, 0));
+    CCSD_TRY(permute_into(st, L->Wvvvo_amef, "amef", LV(L->Wvvvo, "efam", V, V, V, O), 1.0, 0));
     // packed operands of the iteration: A^{kl}_{ij} and tau as they are now, <mn||ab> and <em||ab> with the (a<b) pair as row
     dcopy(st, L->Amc, c->Am, c->oo * c->oo);
     dcopy(st, L->TAUp, c->taup, c->oo * vv);
@@ -255,10 +268,10 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Fvv, "ea", V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Foo, "im", O, O), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->Goo, "mn", O, O), LV(L->Wooov, "mina", O, O, O, V), L->R1, "ia"));
-    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Gvv, "ef", V, V), LV(L->Wvovv, "eifa", V, O, V, V), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->Gvv, "ef", V, V), LV(L->Wvovv_iaef, "iaef", O, V, V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->Wovvo, "ieam", O, V, V, O), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -0.5, LV(L->L2, "mnae", O, O, V, V), LV(L->Wovoo, "iemn", O, V, O, O), L->R1, "ia"));
-    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "imef", O, O, V, V), LV(L->Wvvvo, "efam", V, V, V, O), L->R1, "ia"));
+    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "imef", O, O, V, V), LV(L->Wvvvo_amef, "amef", V, O, V, V), L->R1, "ia"));
     // eqs 52-54, unpacked [i][j][a][b]
     dcopy(st, L->R2, L->OOVV, O * O * V * V);
     CCSD_TRY(tc2(env, sc, 1.0, LV(L->L2, "ijae", O, O, V, V), LV(L->Fvv, "eb", V, V), L->R2, "ijab", "ijba"));
@@ -267,7 +280,7 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     CCSD_TRY(tc2(env, sc, 1.0, LV(L->OOVV, "ijae", O, O, V, V), LV(L->Gvv, "be", V, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc2(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Wvovv, "ejab", V, O, V, V), L->R2, "ijab", "jiab"));
+    CCSD_TRY(tc2(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Wvovv_jabe, "jabe", O, V, V, V), L->R2, "ijab", "jiab"));
     CCSD_TRY(tc4(env, sc, 1.0, LV(L->l1, "ia", O, V), LV(L->Fov, "jb", O, V), L->R2, "ijab", "jiab", "ijba", "jiba"));
     // The terms with an antisymmetric (i<j, a<b) output and a pair-wise contraction run packed, into Pacc[(i<j)][(a<b)]:
     //   sum_{m<n} lambda^{mn}_{ab} W^{ij}_{mn}   (W^{ij}_{mn} = A^{kl}_{ij} of eq 31, packed in both pairs)
