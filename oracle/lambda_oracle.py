@@ -2,8 +2,8 @@
 
 CCSD Lambda equations and the Lagrange one-body density matrix (arXiv 2103.08473 Appendix 7.4-7.5, PAPER.md:674-730,
 eqs 45-61; eqs 12-16) in plain numpy, one ``einsum`` per printed term, on top of the
-amplitudes and integral classes of the plain CPU CCSD oracle.  NO CUDA PATH EXISTS FOR THIS YET:
-the oracle and its pins are committed first, as the protocol demands; the CUDA Lambda solver is the next row to build.
+amplitudes and integral classes of the plain CPU CCSD oracle.  It is the reference the CUDA Lambda solver
+(ccsd_lambda_* / ccsd_density) is compared with and shares no code with it.
 
 The paper prints the two Lambda equations (eqs 52-56), G (eqs 50-51), three of the similarity-transformed-Hamiltonian
 elements (eqs 45-49: W^{ij}_{mn}, W^{mb}_{ej}, W^{ef}_{am}) and Fbar^e_a (eq 57), and refers to its ref. 39 for "the
