@@ -134,3 +134,43 @@ def test_lambda_cfg1_identical_amplitudes(gpu):
         so, sg = ol.iterate(), gc.lambda_iterate()
         assert abs(sg - so) <= 1e-10 * max(1.0, so)
     gc.close()
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2"])
+def test_fullsize_density_is_the_energy_derivative(gpu, cfg):
+    """A property that holds at any size (eqs 15-16): with the converged Lambda, Tr(P D) equals
+    dE_CCSD/d(eps) for h -> h + eps P.  The derivative is taken by central differences (Richardson) of CCSD energies
+    the library converges itself (their parity with the oracle is tested elsewhere); the oracle-side version of this
+    pin is tests/test_lambda_pins.py::test_l4."""
+    inp = ci.make_config(cfg)
+    o, v = inp.nocc, inp.nvir
+    n = o + v
+    rng = np.random.default_rng(7)
+    X = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    P = 0.5 * (X + X.conj().T)
+
+    def e_corr(eps):
+        g = gpu.CCSD(inp.h + eps * P, inp.B, o, v)
+        ok, _, e, _ = g.solve(1e-12, 120)
+        g.close()
+        assert ok
+        return e
+
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    ok, _, _, _ = gc.solve(1e-12, 120)
+    assert ok
+    gc.lambda_init()
+    for it in range(150):
+        if gc.lambda_iterate() < 1e-12:
+            break
+    else:
+        raise AssertionError("Lambda iteration did not converge")
+    D = gc.density().cpu().numpy()
+    gc.close()
+    assert abs(np.trace(D)) < 1e-12
+    h1, h2 = 2.5e-4, 5e-4             # eps |P| stays small against the orbital-energy gaps: truncation ~1e-10, round-off ~3e-9
+    d1 = (e_corr(h1) - e_corr(-h1)) / (2 * h1)
+    d2 = (e_corr(h2) - e_corr(-h2)) / (2 * h2)
+    deriv = (4 * d1 - d2) / 3
+    got = np.sum(P * D)
+    assert abs(deriv - got) < 2e-8 * max(1.0, abs(deriv)), (deriv, got)
