@@ -43,7 +43,14 @@ static int tensor_contract(const Env& env, const TcScratch& sc, double alpha, co
     if (N == 1) {   // matrix-vector product: one pass over the matrix at HBM speed
         CCSD_TRY(run_gemv(env, M, Kk, Ap, Kk, Bp, sc.c, 1, 1.0, 0));
     } else {
-        CCSD_TRY(run_gemm(env, gp(M, N, Kk, Ap, Kk, Bp, Kk, sc.c, N, 1, 1.0, 0)));
+        GemmParams g = gp(M, N, Kk, Ap, Kk, Bp, Kk, sc.c, N, 1, 1.0, 0);
+        if (sc.as && (double)M * (double)N * (double)Kk >= 2.0e10 && M * Kk <= sc.plane_elems && N * Kk <= sc.plane_elems &&
+            Kk % 2 == 0) {   // large product: stage the 3M sums through planes (gemm_dmma.cuh), two streaming passes
+            launch_sum_plane(env.st, Ap, sc.as, M * Kk);
+            launch_sum_plane(env.st, Bp, sc.bs, N * Kk);
+            g = with_planes(g, sc.as, sc.bs);
+        }
+        CCSD_TRY(run_gemm(env, g));
     }
     TView R;
     R.p = sc.c; R.rank = nm + nn;
@@ -88,6 +95,7 @@ struct LambdaState {
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
     // packed (i<j, a<b) route of the terms whose output is antisymmetric and whose contraction runs over a packable pair
     c128 *Pacc, *l2pT, *LTp, *L2hu, *Ltp, *Amc, *TAUp, *VoovvT, *VT2;
+    double *VT2s, *Ltps;                           // sum planes of the (vv x oo x ov) product's operands
     double* cl2s;                                  // 3M sum plane of conj(l2p)
     // DIIS (as for the amplitudes: reading G13)
     c128 *diis_u, *diis_e;
@@ -106,6 +114,9 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->sc.a = w.take<c128>(L->sc.elems);
     L->sc.b = w.take<c128>(L->sc.elems);
     L->sc.c = w.take<c128>(L->sc.elems);
+    L->sc.plane_elems = o2v2;
+    L->sc.as = c->planes ? w.take<double>(o2v2) : nullptr;
+    L->sc.bs = c->planes ? w.take<double>(o2v2) : nullptr;
     L->T2 = w.take<c128>(o2v2); L->TAU = w.take<c128>(o2v2); L->OOVV = w.take<c128>(o2v2);
     L->OOOV = w.take<c128>(o3v); L->WOOOO = w.take<c128>(o * o * o * o);
     L->Fov = w.take<c128>(ov); L->Foo = w.take<c128>(o * o); L->Fvv = w.take<c128>(v * v);
@@ -122,6 +133,8 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Pacc = w.take<c128>(oo * vv); L->l2pT = w.take<c128>(vv * oo); L->LTp = w.take<c128>(oo * oo);
     L->L2hu = w.take<c128>(oo * v * v); L->Ltp = w.take<c128>(oo * ov); L->Amc = w.take<c128>(oo * oo);
     L->TAUp = w.take<c128>(oo * vv); L->VoovvT = w.take<c128>(vv * oo); L->VT2 = w.take<c128>(vv * ov);
+    L->VT2s = c->planes ? w.take<double>(vv * ov) : nullptr;
+    L->Ltps = c->planes ? w.take<double>(oo * ov) : nullptr;
     L->nd = c->opt.ndiis;
     const int nd = L->nd > 0 ? L->nd : 1;
     L->diis_u = w.take<c128>((int64_t)nd * c->nvec);
@@ -244,6 +257,7 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     dcopy(st, L->TAUp, c->taup, c->oo * vv);
     CCSD_TRY(launch_transpose2d(st, c->Voovv_p, L->VoovvT, c->oo, vv, 0));
     CCSD_TRY(launch_transpose2d(st, c->Vvovv_p, L->VT2, c->ov, vv, 0));
+    if (L->VT2s) launch_sum_plane(st, L->VT2, L->VT2s, vv * c->ov);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -297,7 +311,8 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             return asym_col(l2p, row / v, vv, (int)(row % v), (int)ff, v);
         });
         CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, c->t1, V, L->Ltp, O, 1, 1.0, 0)));
-        CCSD_TRY(run_gemm(env, gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1)));
+        if (L->Ltps) launch_sum_plane(st, L->Ltp, L->Ltps, oo * c->ov);
+        CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1), L->VT2s, L->Ltps)));
     }
     //   (i) sum_{e<f} lambda^{ij}_{ef} <ef||ab> = conj( sum_{e<f} conj(lambda) <ab||ef> ): the pp-ladder launch of the CCSD
     //       iteration (packed, Hermitian <ab||cd>, 3M with sum planes) on the conjugated multipliers

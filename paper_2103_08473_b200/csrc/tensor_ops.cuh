@@ -84,6 +84,8 @@ static int permute_into(cudaStream_t st, c128* out, const char* oidx, const TVie
 struct TcScratch {
     c128 *a, *b, *c;      // permuted operands and the raw GEMM result
     int64_t elems;        // capacity of each
+    double *as, *bs;      // 3M sum planes of the operands of the large products (null: the kernel forms the sums itself)
+    int64_t plane_elems;  // capacity of each plane
 };
 struct TcOut {
     const char* idx;      // index order under which the result is added into C
