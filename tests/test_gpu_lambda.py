@@ -136,7 +136,7 @@ def test_lambda_cfg1_identical_amplitudes(gpu):
     gc.close()
 
 
-@pytest.mark.parametrize("cfg", ["cfg1", "cfg2"])
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2", "cfg3"])
 def test_fullsize_density_is_the_energy_derivative(gpu, cfg):
     """A property that holds at any size (eqs 15-16): with the converged Lambda, Tr(P D) equals
     dE_CCSD/d(eps) for h -> h + eps P.  The derivative is taken by central differences (Richardson) of CCSD energies
@@ -151,16 +151,16 @@ def test_fullsize_density_is_the_energy_derivative(gpu, cfg):
 
     def e_corr(eps):
         g = gpu.CCSD(inp.h + eps * P, inp.B, o, v)
-        ok, _, e, _ = g.solve(1e-12, 120)
+        ok, _, e, _ = g.solve(1e-12, 200)
         g.close()
         assert ok
         return e
 
     gc = gpu.CCSD(inp.h, inp.B, o, v)
-    ok, _, _, _ = gc.solve(1e-12, 120)
+    ok, _, _, _ = gc.solve(1e-12, 200)
     assert ok
     gc.lambda_init()
-    for it in range(150):
+    for it in range(300):
         if gc.lambda_iterate() < 1e-12:
             break
     else:
