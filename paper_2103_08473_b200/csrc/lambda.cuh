@@ -85,7 +85,7 @@ struct LambdaState {
     bool ready;
     TcScratch sc;
     // unpacked copies of what the CCSD context holds packed
-    c128 *T2, *TAU, *OOVV, *OOOV, *WOOOO;          // [i][j][a][b], [m][n][e][f], [m][n][i][e], [m][n][i][j]
+    c128 *T1, *T2, *TAU, *OOVV, *OOOV, *WOOOO;     // [i][a] (copy: the solve stays consistent if the amplitudes move), [i][j][a][b], [m][n][e][f], [m][n][i][e], [m][n][i][j]
     // elements of Hbar (constant during the solve)
     c128 *Fov, *Foo, *Fvv;                         // [m][e], [m][i], [a][e]
     c128 *Wvovv, *Wooov, *Wovvo, *Wovoo, *Wvvvo;   // [a][m][e][f], [m][n][i][e], [m][b][e][j], [m][b][i][j], [a][b][e][i]
@@ -117,7 +117,7 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->sc.plane_elems = o2v2;
     L->sc.as = c->planes ? w.take<double>(o2v2) : nullptr;
     L->sc.bs = c->planes ? w.take<double>(o2v2) : nullptr;
-    L->T2 = w.take<c128>(o2v2); L->TAU = w.take<c128>(o2v2); L->OOVV = w.take<c128>(o2v2);
+    L->T1 = w.take<c128>(ov); L->T2 = w.take<c128>(o2v2); L->TAU = w.take<c128>(o2v2); L->OOVV = w.take<c128>(o2v2);
     L->OOOV = w.take<c128>(o3v); L->WOOOO = w.take<c128>(o * o * o * o);
     L->Fov = w.take<c128>(ov); L->Foo = w.take<c128>(o * o); L->Fvv = w.take<c128>(v * v);
     L->Wvovv = w.take<c128>(ov3); L->Wooov = w.take<c128>(o3v); L->Wovvo = w.take<c128>(o2v2);
@@ -178,6 +178,7 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     const int o = c->o, v = c->v;
     const int64_t O = o, V = v, vv = c->vv;
     CCSD_TRY(residual(c));                                    // tau, Hov, Gvv, Goo, Am of eqs 23-31 at the current (t1, t2)
+    dcopy(st, L->T1, c->t1, O * V);
     unpack_pairs(st, L->T2, c->t2p, o, 1, v, 1);
     unpack_pairs(st, L->TAU, c->taup, o, 1, v, 1);
     unpack_pairs(st, L->OOVV, c->Voovv_p, o, 1, v, 1);
@@ -187,7 +188,7 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     dcopy(st, L->Fov, c->Hov, O * V);
     dcopy(st, L->Fvv, c->Gvv, V * V);
     CCSD_TRY(permute_into(st, L->Foo, "mi", LV(c->Goo, "mi", O, O), -1.0, 0));
-    const c128 *T1 = c->t1, *VOVV = c->Vvovv_u /* <ak||cd> stored [a][c][k][d] */, *VOVO = c->Vvovo_m /* <ak||ci> [a][i][c][k] */;
+    const c128 *T1 = L->T1, *VOVV = c->Vvovv_u /* <ak||cd> stored [a][c][k][d] */, *VOVO = c->Vvovo_m /* <ak||ci> [a][i][c][k] */;
     // W^{am}_{ef} = <am||ef> - t^a_n <nm||ef>
     CCSD_TRY(permute_into(st, L->Wvovv, "amef", LV(VOVV, "aemf", V, V, O, V), 1.0, 0));
     CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "na", O, V), LV(L->OOVV, "nmef", O, O, V, V), L->Wvovv, "amef"));
@@ -268,9 +269,8 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     cudaStream_t st = c->st;
     const Env& env = c->env;
     const TcScratch& sc = L->sc;
-    const int o = c->o, v = c->v, n = c->n;
+    const int o = c->o, v = c->v;
     const int64_t O = o, V = v, oo = c->oo, vv = c->vv;
-    const c128 *VOVV = c->Vvovv_u;
     unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
     // eqs 50-51
     CCSD_CUDA_TRY(cudaMemsetAsync(L->Gvv, 0, (size_t)(V * V) * sizeof(c128), st));
@@ -310,7 +310,7 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         launch_fill(st, L->L2hu, oo * V, V, V, 0, [=] __device__(int64_t row, int64_t ff) {
             return asym_col(l2p, row / v, vv, (int)(row % v), (int)ff, v);
         });
-        CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, c->t1, V, L->Ltp, O, 1, 1.0, 0)));
+        CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, L->T1, V, L->Ltp, O, 1, 1.0, 0)));
         if (L->Ltps) launch_sum_plane(st, L->Ltp, L->Ltps, oo * c->ov);
         CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1), L->VT2s, L->Ltps)));
     }
@@ -334,7 +334,6 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             return cadd(cadd(R2[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(P2[IJ * vv + AB])), Pacc[IJ * vv + AB]);
         });
     }
-    (void)n;
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -438,22 +437,22 @@ static int lambda_density(ccsd_ctx* c, LambdaState* L, c128* D)
     CCSD_CUDA_TRY(cudaMemsetAsync(gab, 0, (size_t)(V * V) * sizeof(c128), st));
     // eq 58: gamma_ij = -1/2 t^{ef}_{im} lambda^{jm}_{ef} - t^e_i lambda^j_e
     CCSD_TRY(tc1(env, sc, -0.5, LV(L->T2, "imef", O, O, V, V), LV(L->L2, "jmef", O, O, V, V), goo, "ij"));
-    CCSD_TRY(tc1(env, sc, -1.0, LV(c->t1, "ie", O, V), LV(L->l1, "je", O, V), goo, "ij"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(L->T1, "ie", O, V), LV(L->l1, "je", O, V), goo, "ij"));
     // eq 61: gamma_ab = 1/2 t^{ae}_{mn} lambda^{mn}_{be} + t^a_m lambda^m_b
     CCSD_TRY(tc1(env, sc, 0.5, LV(L->T2, "mnae", O, O, V, V), LV(L->L2, "mnbe", O, O, V, V), gab, "ab"));
-    CCSD_TRY(tc1(env, sc, 1.0, LV(c->t1, "ma", O, V), LV(L->l1, "mb", O, V), gab, "ab"));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->T1, "ma", O, V), LV(L->l1, "mb", O, V), gab, "ab"));
     // eq 60 as [i][a]: t + lambda^m_e (t^{ae}_{im} - t^e_i t^a_m) - 1/2 lambda^{mn}_{ef} (t^{ef}_{in} t^a_m + t^e_i t^{af}_{mn})
-    dcopy(st, gai, c->t1, O * V);
+    dcopy(st, gai, L->T1, O * V);
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->T2, "imae", O, O, V, V), gai, "ia"));
     //   - ( sum_e lambda^m_e t^e_i + 1/2 sum_nef lambda^{mn}_{ef} t^{ef}_{in} ) t^a_m
     CCSD_CUDA_TRY(cudaMemsetAsync(x_oo, 0, (size_t)(O * O) * sizeof(c128), st));
-    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(c->t1, "ie", O, V), x_oo, "mi"));
+    CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->T1, "ie", O, V), x_oo, "mi"));
     CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "mnef", O, O, V, V), LV(L->T2, "inef", O, O, V, V), x_oo, "mi"));
-    CCSD_TRY(tc1(env, sc, -1.0, LV(x_oo, "mi", O, O), LV(c->t1, "ma", O, V), gai, "ia"));
+    CCSD_TRY(tc1(env, sc, -1.0, LV(x_oo, "mi", O, O), LV(L->T1, "ma", O, V), gai, "ia"));
     //   - 1/2 t^e_i ( sum_mnf lambda^{mn}_{ef} t^{af}_{mn} )
     CCSD_CUDA_TRY(cudaMemsetAsync(x_ea, 0, (size_t)(V * V) * sizeof(c128), st));
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->L2, "mnef", O, O, V, V), LV(L->T2, "mnaf", O, O, V, V), x_ea, "ea"));
-    CCSD_TRY(tc1(env, sc, -0.5, LV(c->t1, "ie", O, V), LV(x_ea, "ea", V, V), gai, "ia"));
+    CCSD_TRY(tc1(env, sc, -0.5, LV(L->T1, "ie", O, V), LV(x_ea, "ea", V, V), gai, "ia"));
     const c128* l1 = L->l1;
     launch_fill(st, D, n, n, n, 0, [=] __device__(int64_t p, int64_t q) {
         if (p < o && q < o) return goo[p * o + q];                       // gamma_ij = <a+_i a_j>
