@@ -174,3 +174,32 @@ def test_fullsize_density_is_the_energy_derivative(gpu, cfg):
     deriv = (4 * d1 - d2) / 3
     got = np.sum(P * D)
     assert abs(deriv - got) < 2e-8 * max(1.0, abs(deriv)), (deriv, got)
+
+
+def test_lambda_edge_cases(gpu):
+    """Minimal system (two occupied, two virtual spinors: one pair each), plain Jacobi (ndiis = 0) with shifted
+    denominators, CC2 mode rejected, calls before ccsd_lambda_init rejected."""
+    from paper_2103_08473_b200.binding import CCSDError
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2
+    from oracle.lambda_oracle import OracleLambda
+    for (o, v, nd, shift) in ((2, 2, 6, 0.0), (3, 5, 0, 0.3), (2, 7, 3, 0.0)):
+        inp = ci.make_inputs(o, v, 6, seed=60 + o + v, b_scale=0.1, f_offdiag=0.05)
+        oc = OracleCCSD(inp.h, inp.B, o, v, ndiis=nd, level_shift=shift)
+        for _ in range(4):
+            oc.iterate()
+        ol = OracleLambda(oc, ndiis=nd)
+        gc = gpu.CCSD(inp.h, inp.B, o, v, ndiis=nd, level_shift=shift)
+        with pytest.raises(CCSDError):
+            gc.lambda_iterate()
+        gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+        gc.lambda_init()
+        for _ in range(5):
+            so, sg = ol.iterate(), gc.lambda_iterate()
+            assert abs(sg - so) <= 1e-11 * max(1.0, so) + 1e-14
+        assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-11
+        gc.close()
+    inp = ci.make_config("cfg0")
+    gc = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, cc2=True)
+    with pytest.raises(CCSDError):
+        gc.lambda_init()
+    gc.close()
