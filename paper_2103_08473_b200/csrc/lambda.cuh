@@ -121,9 +121,12 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->OOOV = w.take<c128>(o3v); L->WOOOO = w.take<c128>(o * o * o * o);
     L->Fov = w.take<c128>(ov); L->Foo = w.take<c128>(o * o); L->Fvv = w.take<c128>(v * v);
     L->Wvovv = w.take<c128>(ov3); L->Wooov = w.take<c128>(o3v); L->Wovvo = w.take<c128>(o2v2);
-    L->Wovoo = w.take<c128>(o3v); L->Wvvvo = w.take<c128>(ov3);
-    L->Wvovv_iaef = w.take<c128>(ov3); L->Wvovv_jabe = w.take<c128>(ov3); L->Wvvvo_amef = w.take<c128>(ov3);
-    L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v); L->Ypk = w.take<c128>(vv * v * o);
+    L->Wovoo = w.take<c128>(o3v);
+    L->Wvvvo = L->Wvovv;   // build order: W^{am}_{ef} is re-laid-out and dead before W^{ab}_{ei} is assembled in the same buffer
+    L->Wvovv_iaef = w.take<c128>(ov3); L->Wvovv_jabe = w.take<c128>(ov3);
+    L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v);
+    L->Wvvvo_amef = L->X3;   // the build temporary is free when the finished W^{ab}_{ei} is re-laid-out into it
+    L->Ypk = w.take<c128>(vv * v * o);
     L->l1 = w.take<c128>(ov); L->l2p = w.take<c128>(oo * vv); L->L2 = w.take<c128>(o2v2);
     L->R1 = w.take<c128>(ov); L->R2 = w.take<c128>(o2v2); L->R2p = w.take<c128>(oo * vv);
     L->Gvv = w.take<c128>(v * v); L->Goo = w.take<c128>(o * o);
@@ -192,6 +195,9 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     // W^{am}_{ef} = <am||ef> - t^a_n <nm||ef>
     CCSD_TRY(permute_into(st, L->Wvovv, "amef", LV(VOVV, "aemf", V, V, O, V), 1.0, 0));
     CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "na", O, V), LV(L->OOVV, "nmef", O, O, V, V), L->Wvovv, "amef"));
+    //   ... kept only in the two [free][contracted] layouts the iteration contracts it in
+    CCSD_TRY(permute_into(st, L->Wvovv_iaef, "iaef", LV(L->Wvovv, "eifa", V, O, V, V), 1.0, 0));
+    CCSD_TRY(permute_into(st, L->Wvovv_jabe, "jabe", LV(L->Wvovv, "ejab", V, O, V, V), 1.0, 0));
     // W^{mn}_{ie} = <mn||ie> + t^f_i <mn||fe>
     dcopy(st, L->Wooov, L->OOOV, O * O * O * V);
     CCSD_TRY(tc1(env, sc, 1.0, LV(T1, "if", O, V), LV(L->OOVV, "mnfe", O, O, V, V), L->Wooov, "mnie"));
@@ -249,9 +255,7 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
             return a < b ? Y[pair_idx(a, b, v) * ((int64_t)v * o) + ei] : cneg(Y[pair_idx(b, a, v) * ((int64_t)v * o) + ei]);
         });
     }
-    // the o v^3 elements in the [free][contracted] layouts the iteration contracts them in
-    CCSD_TRY(permute_into(st, L->Wvovv_iaef, "iaef", LV(L->Wvovv, "eifa", V, O, V, V), 1.0, 0));
-    CCSD_TRY(permute_into(st, L->Wvovv_jabe, "jabe", LV(L->Wvovv, "ejab", V, O, V, V), 1.0, 0));
+    // W^{ab}_{ei} in the [free][contracted] layout the iteration contracts it in (into the build temporary, now free)
     CCSD_TRY(permute_into(st, L->Wvvvo_amef, "amef", LV(L->Wvvvo, "efam", V, V, V, O), 1.0, 0));
     // packed operands of the iteration: A^{kl}_{ij} and tau as they are now, <mn||ab> and <em||ab> with the (a<b) pair as row
     dcopy(st, L->Amc, c->Am, c->oo * c->oo);
@@ -432,7 +436,7 @@ static int lambda_density(ccsd_ctx* c, LambdaState* L, c128* D)
     const int64_t O = o, V = v;
     unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
     // temporaries: the residual buffers of the solver are free between iterations
-    c128 *goo = L->Goo, *gab = L->Gvv, *gai = L->R1, *x_oo = L->LT, *x_ea = L->X3;
+    c128 *goo = L->Goo, *gab = L->Gvv, *gai = L->R1, *x_oo = L->LT, *x_ea = L->R2;
     CCSD_CUDA_TRY(cudaMemsetAsync(goo, 0, (size_t)(O * O) * sizeof(c128), st));
     CCSD_CUDA_TRY(cudaMemsetAsync(gab, 0, (size_t)(V * V) * sizeof(c128), st));
     // eq 58: gamma_ij = -1/2 t^{ef}_{im} lambda^{jm}_{ef} - t^e_i lambda^j_e
