@@ -167,6 +167,9 @@ int ccsd_get_lambda(ccsd_ctx* ctx, ccsd_c128* l1, ccsd_c128* l2p);
 int ccsd_set_lambda(ccsd_ctx* ctx, const ccsd_c128* l1, const ccsd_c128* l2p, int reset_diis);
 int ccsd_get_lambda_residual(ccsd_ctx* ctx, ccsd_c128* r1, ccsd_c128* r2p);
 int ccsd_density(ccsd_ctx* ctx, ccsd_c128* D);
+/* eq 16: expectation value of a one-body operator, sum_pq O[p][q] D[p][q] with D as ccsd_density returns it
+ * (correlation part; the reference determinant contributes sum_i O[i][i]).  D, O: device [n][n].  HOST outputs. */
+int ccsd_expectation(ccsd_ctx* ctx, const ccsd_c128* D, const ccsd_c128* O, double* re, double* im);
 
 /* Per-term parity hook: the dense, fully antisymmetric blocks Wbar, Zbar, Ybar [a][b][c] (nvir^3 elements each, device;
  * NULL = skip) of one occupied triple i<j<k.  Asynchronous on the stream after an initial synchronisation. */

@@ -25,7 +25,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
            "ccsd_triples_block", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
-           "ccsd_get_lambda_residual", "ccsd_density"]
+           "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation"]
 
 
 class CCSDError(RuntimeError):
@@ -77,6 +77,7 @@ def load_library():
         lib.ccsd_set_lambda.argtypes = [vp, vp, vp, ctypes.c_int]
         lib.ccsd_get_lambda_residual.argtypes = [vp, vp, vp]
         lib.ccsd_density.argtypes = [vp, vp]
+        lib.ccsd_expectation.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
         lib.ccsd_solve.argtypes = [vp, dbl, ctypes.c_int, ctypes.POINTER(ctypes.c_int)] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_t1_diagnostic.argtypes = [vp, ctypes.POINTER(dbl)]
         lib.ccsd_get_amplitudes.argtypes = [vp, vp, vp]
@@ -355,6 +356,16 @@ class CCSD:
         _check(self._lib.ccsd_density(self._ctx, D.data_ptr()), "ccsd_density")
         torch.cuda.current_stream().synchronize()
         return D
+
+    def expectation(self, D, O) -> complex:
+        """eq 16: sum_pq O[p][q] D[p][q] (ccsd_expectation); D from density(), O any [n][n] operator matrix."""
+        torch = self._torch
+        D_d, O_d = _dev_c128(torch, D), _dev_c128(torch, O)
+        assert tuple(D_d.shape) == (self.n, self.n) and tuple(O_d.shape) == (self.n, self.n)
+        re, im = ctypes.c_double(), ctypes.c_double()
+        _check(self._lib.ccsd_expectation(self._ctx, D_d.data_ptr(), O_d.data_ptr(), ctypes.byref(re), ctypes.byref(im)),
+               "ccsd_expectation")
+        return complex(re.value, im.value)
 
     def enable_step_timing(self, enable: bool = True):
         _check(self._lib.ccsd_enable_step_timing(self._ctx, int(enable)), "ccsd_enable_step_timing")

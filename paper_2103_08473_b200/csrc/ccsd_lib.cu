@@ -1723,6 +1723,19 @@ int ccsd_get_lambda_residual(ccsd_ctx* c, ccsd_c128* r1, ccsd_c128* r2p)
     return CCSD_OK;
 }
 
+int ccsd_expectation(ccsd_ctx* c, const ccsd_c128* D_, const ccsd_c128* O_, double* re, double* im)
+{   // eq 16: <O> = sum_pq o_pq D[p][q], D[p][q] = <a+_p a_q> as ccsd_density returns it
+    if (!c || !D_ || !O_) return CCSD_ESTATE;
+    const c128 *D = reinterpret_cast<const c128*>(D_), *O = reinterpret_cast<const c128*>(O_);
+    CCSD_CUDA_TRY(cudaMemsetAsync(c->red + 50, 0, 2 * sizeof(double), c->st));
+    launch_reduce(c->st, (int64_t)c->n * c->n, c->red + 50, 1, [=] __device__(int64_t x) { return cmul(O[x], D[x]); });
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 50, c->red + 50, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
+    if (re) *re = c->red_host[50];
+    if (im) *im = c->red_host[51];
+    return CCSD_OK;
+}
+
 int ccsd_density(ccsd_ctx* c, ccsd_c128* D)
 {
     if (!c || !c->lam || !c->lam->ready || !D) return CCSD_ESTATE;

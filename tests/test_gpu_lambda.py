@@ -165,7 +165,9 @@ def test_fullsize_density_is_the_energy_derivative(gpu, cfg):
             break
     else:
         raise AssertionError("Lambda iteration did not converge")
-    D = gc.density().cpu().numpy()
+    D_dev = gc.density()
+    D = D_dev.cpu().numpy()
+    assert abs(gc.expectation(D_dev, P) - np.sum(P * D)) < 1e-13 * max(1.0, abs(np.sum(P * D)))     # eq 16 on the device
     gc.close()
     assert abs(np.trace(D)) < 1e-12
     h1, h2 = 2.5e-4, 5e-4             # eps |P| stays small against the orbital-energy gaps: truncation ~1e-10, round-off ~3e-9
