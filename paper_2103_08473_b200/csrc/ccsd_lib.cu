@@ -72,7 +72,10 @@ static int run_gemm(const Env& env, GemmParams p)
     else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p))
         variant = dmma_pick(p.N, CCSD_DEFAULT_3M != 0, CCSD_DEFAULT_3M != 0 && planes_ok);
     if (variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
-    if (variant >= 0 && !dmma_ok) return CCSD_EINVAL;
+    if (variant >= 0 && !dmma_ok) {   // strided operands: an explicitly requested tile variant is an error, a forced family is not
+        if (env.gemm_mode >= 100) return CCSD_EINVAL;
+        variant = -1;
+    }
     const bool use_dmma = variant >= 0;
     // split-K chosen against wave quantisation on the 148 SMs: minimise  waves(ks) * (K/ks + pipeline overhead)
     const int bm = use_dmma ? k_dmma_variants[variant].bm : SG_BM, bn = use_dmma ? k_dmma_variants[variant].bn : SG_BN;

@@ -205,3 +205,24 @@ def test_lambda_edge_cases(gpu):
     with pytest.raises(CCSDError):
         gc.lambda_init()
     gc.close()
+
+
+@pytest.mark.parametrize("gemm_mode", [1, 2, 3])
+def test_lambda_under_every_gemm_mode(gpu, gemm_mode):
+    """The Lambda path on the simple FMA kernels (1), the 4M DMMA kernels (2, no sum planes) and forced 3M (3)."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2
+    from oracle.lambda_oracle import OracleLambda
+    inp = ci.make_inputs(6, 14, 20, seed=4716)
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    for _ in range(5):
+        oc.iterate()
+    ol = OracleLambda(oc)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, gemm_mode=gemm_mode)
+    gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+    gc.lambda_init()
+    for _ in range(3):
+        so, sg = ol.iterate(), gc.lambda_iterate()
+        assert abs(sg - so) <= 1e-11 * max(1.0, so)
+    assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-11
+    gc.close()

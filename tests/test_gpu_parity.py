@@ -74,7 +74,8 @@ def compare_all(oc, gc, names=None, tol=REL_TOL):
     return worst
 
 
-@pytest.mark.parametrize("o,v,L,gemm_mode", [(5, 11, 20, 1), (5, 11, 20, 0), (6, 16, 30, 0), (3, 9, 10, 0)])
+@pytest.mark.parametrize("o,v,L,gemm_mode", [(5, 11, 20, 1), (5, 11, 20, 0), (6, 16, 30, 0), (3, 9, 10, 0), (6, 16, 30, 2),
+                                            (6, 16, 30, 3)])
 def test_every_tensor_matches_oracle(gpu, o, v, L, gemm_mode):
     """All integral classes, all intermediates of eqs 24-31, all eight terms of eq 32, S1, S2: ragged sizes."""
     from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
