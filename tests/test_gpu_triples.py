@@ -148,3 +148,29 @@ def test_triples_edge_cases(gpu):
     for key in ("+T", "(T)", "-T"):
         assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
     gc.close()
+
+
+@pytest.mark.parametrize("gemm_mode", [1, 2, 3])
+def test_triples_and_cc2_under_every_gemm_mode(gpu, gemm_mode):
+    """Triples (the K-segmented GEMM always runs on the DMMA kernel; without sum planes when they are switched off) and
+    one CC2 iteration with the GEMM family forced."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2
+    from oracle.cc2_oracle import OracleCC2
+    from oracle.triples_oracle import OracleTriples
+    inp = ci.make_inputs(5, 12, 20, seed=4720)
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    for _ in range(3):
+        oc.iterate()
+    gc = gpu.CCSD(inp.h, inp.B, o, v, gemm_mode=gemm_mode)
+    gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+    ref, got = OracleTriples(oc).energies(restricted=True), gc.triples()
+    for key in ("+T", "(T)", "-T"):
+        assert abs(got[key] - ref[key]) < E_TOL, (key, got[key], ref[key])
+    gc.close()
+    o2 = OracleCC2(inp.h, inp.B, o, v)
+    g2 = gpu.CCSD(inp.h, inp.B, o, v, gemm_mode=gemm_mode, cc2=True)
+    for _ in range(3):
+        eo, eg = o2.iterate()[0], g2.iterate()[0]
+        assert abs(eo - eg) < E_TOL
+    g2.close()
