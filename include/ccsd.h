@@ -157,6 +157,7 @@ int ccsd_get_triples_times(ccsd_ctx* ctx, float ms[2]);
  *   ccsd_density          D[p][q] = <0|(1+Lambda) exp(-T) a+_p a_q exp(T)|0> - delta_pq (p occupied), [n][n] (device),
  *                         occupied spinors first, assembled from eqs 58-61, unsymmetrised (the paper symmetrises it
  *                         before use).  Uses the residual buffers: call it between iterations.
+ * In CCD mode (opts.ccd) the Lagrangian has no singles constraint: lambda^i_a stays zero.
  * Errors: CCSD_ESTATE without ccsd_lambda_init, CCSD_EINVAL (workspace), CCSD_ESINGULAR (DIIS), CCSD_ECUDA.
  */
 int ccsd_lambda_workspace_bytes(ccsd_ctx* ctx, size_t* bytes);

@@ -358,7 +358,9 @@ static int lambda_iterate(ccsd_ctx* c, LambdaState* L, double* step_norm)
         const c128 *R1 = L->R1, *R2p = L->R2p, *l1 = L->l1, *l2p = L->l2p;
         const double* eps = c->eps;
         const int2 *po = c->po, *pv = c->pv;
+        const int ccd = c->opt.ccd;                      // CCD: the Lagrangian has no singles constraint, lambda^i_a stays zero
         launch_fill(st, Ev, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
+            if (ccd) { U[i * v + a] = mk(0.0, 0.0); return mk(0.0, 0.0); }
             const double d = eps[i] - eps[o + a];
             const c128 e = mk(R1[i * v + a].x / d, R1[i * v + a].y / d);
             U[i * v + a] = cadd(l1[i * v + a], e);

@@ -226,3 +226,30 @@ def test_lambda_under_every_gemm_mode(gpu, gemm_mode):
         assert abs(sg - so) <= 1e-11 * max(1.0, so)
     assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-11
     gc.close()
+
+
+def test_lambda_in_ccd_mode_keeps_singles_multipliers_zero(gpu):
+    """CCD: t1 = 0 and no singles constraint in the Lagrangian, so lambda^i_a = 0 throughout; the
+    doubles multipliers follow eqs 52-54 with t1 = lambda1 = 0 (oracle: the same equations with both zeroed)."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2
+    from oracle.lambda_oracle import OracleLambda
+    inp = ci.make_inputs(4, 10, 24, seed=79, b_scale=0.08, f_offdiag=0.03)
+    o, v = inp.nocc, inp.nvir
+    oc = OracleCCSD(inp.h, inp.B, o, v, ndiis=0)
+    oc.set_amplitudes(np.zeros_like(oc.t1), oc.t2)
+    for _ in range(6):                                   # plain Jacobi CCD on the oracle side (as in the CCD parity test)
+        _, S2 = oc.residual()
+        oc.set_amplitudes(np.zeros_like(oc.t1), oc.t2 + S2 / oc.D2)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, ccd=True, ndiis=0)
+    gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
+    ol = OracleLambda(oc, ndiis=0)
+    ol.l1[:] = 0.0
+    gc.lambda_init()
+    for _ in range(4):
+        so = ol.iterate()
+        ol.l1[:] = 0.0
+        gc.lambda_iterate()
+    l1, l2p = gc.get_lambda()
+    assert float(l1.abs().max()) == 0.0
+    assert _rel(l2p.cpu().numpy(), pack_t2(ol.l2)) <= 1e-11
+    gc.close()
