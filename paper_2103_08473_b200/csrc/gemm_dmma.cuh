@@ -18,7 +18,6 @@
 // Out-of-range rows / k are zero-filled by TMA, so ragged M, N, K need no special code in the main loop.
 #pragma once
 #include <cuda.h>
-#include <cstdlib>
 #include "gemm_simple.cuh"
 
 constexpr int DMMA_BKG = 4;         // k-groups (of 4 complex) per pipeline stage -> BK = 16 complex
@@ -497,10 +496,9 @@ static int launch_gemm_dmma(cudaStream_t st, const GemmParams& p, int variant)
     if (variant < 0 || variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
     const DmmaVariant& V = k_dmma_variants[variant];
     CUtensorMap mA, mB;
-    static const bool no_wide = getenv("CCSD_NO_WIDE_TMA") != nullptr;   // tuning / A-B switch
     // measured: the wide maps help the 48-column tiles (pp-ladder 0.928 -> 0.935 of peak) but cost the 32-column ones, which
     // move more bytes per flop, 10-15 % (config-4 sweep at nocc = 40: 0.90 -> 0.78; triples GEMM 5.06 -> 5.36 s)
-    const int wide = (!no_wide && p.K % 4 == 0 && p.K >= 4 && V.bn >= 48) ? 1 : 0;
+    const int wide = (p.K % 4 == 0 && p.K >= 4 && V.bn >= 48) ? 1 : 0;
     if (V.planes && (!p.As || !p.Bs)) return CCSD_EINVAL;
     CUtensorMap mAs, mBs;
     if (wide) {
