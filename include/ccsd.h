@@ -52,6 +52,11 @@ typedef struct {
     int cc2;            /* 1 = CC2 (Appendix 7.2 eqs 34-38): singles equations of CCSD,
                            doubles equations <Phi_ij^ab| exp(-T1) H exp(T1) + [F, T2] |Phi_0>; ccsd_get_tensor then returns
                            tau, C, A at t2 = 0, GVV = f_vv, GOO = -f_oo, and S2_GVV / S2_GOO the two Fock terms */
+    int direct_ladder;  /* 1 = integral-direct pp-ladder: the packed <ab||cd>
+                           (vv^2 elements, the largest tensor) is never stored; every iteration rebuilds its rows slab by
+                           slab from the factor B and contracts them.  Trades 8 v^4 naux flops per iteration for
+                           24 vv^2 bytes of HBM; ccsd_get_tensor(CCSD_T_VVVV) and the Lambda entry points then return
+                           CCSD_EINVAL.  Default 0 */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */

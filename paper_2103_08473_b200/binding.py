@@ -39,7 +39,7 @@ class CCSDError(RuntimeError):
 
 class Options(ctypes.Structure):
     _fields_ = [("ndiis", ctypes.c_int), ("level_shift", ctypes.c_double), ("gemm_mode", ctypes.c_int),
-                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int)]
+                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -179,8 +179,8 @@ def measure_fp64_peak(launches: int = 10) -> float:
     return float(out.value)
 
 
-def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False) -> Options:
-    return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)))
+def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False) -> Options:
+    return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)))
 
 
 class CCSD:
@@ -190,7 +190,7 @@ class CCSD:
     """
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
-                 ccd: bool = False, cc2: bool = False):
+                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False):
         torch = _torch()
         lib = load_library()
         self._lib, self._torch = lib, torch
@@ -200,7 +200,7 @@ class CCSD:
         h_d, B_d = _dev_c128(torch, h), _dev_c128(torch, B)
         self.naux = int(B_d.shape[0])
         assert tuple(h_d.shape) == (self.n, self.n) and tuple(B_d.shape) == (self.naux, self.n, self.n)
-        self._opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2)
+        self._opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder)
         nbytes = ctypes.c_size_t(0)
         _check(lib.ccsd_workspace_bytes(self.nocc, self.nvir, self.naux, ctypes.byref(self._opts),
                                         ctypes.byref(nbytes)), "ccsd_workspace_bytes")

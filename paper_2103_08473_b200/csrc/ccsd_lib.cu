@@ -157,6 +157,8 @@ struct ccsd_ctx {
     // init temporaries
     c128 *Boo, *Bov, *Bvo, *Bvv, *Jovov, *Jvoov, *Jvvoo, *Jvvov, *Jooov, *Joooo, *Jslab, *JslabT;
     int na_slab;
+    c128* Wslab;            // direct_ladder: rows of <ab||cd> of one slab of the first virtual index, rebuilt every iteration
+    double* Wslabs;         // ... and their 3M sum plane
     // amplitudes and per-iteration tensors
     c128 *t1, *t2p, *t1T, *S1, *S2p, *taup, *TT, *AG, *Xm, *T2r, *tauc, *tauou, *t2hu;
     c128 *Hvv, *Gvv, *Hoo, *Goo, *Hov, *HovT, *HF, *inner, *Hm, *Cm, *Cm2, *Am, *tmp_ov;
@@ -206,7 +208,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->pv = w.take<int2>(vv);
     c->eps = w.take<double>(n);
     c->f = w.take<c128>(n * n);
-    c->W = w.take<c128>(vv * vv);
+    c->W = c->opt.direct_ladder ? nullptr : w.take<c128>(vv * vv);   // direct_ladder: <ab||cd> is never stored
     c->Vvovv_p = w.take<c128>(v * o * vv);
     c->Vvovv_u = w.take<c128>(v * v * o * v);
     c->VvovvT = w.take<c128>(o * vv * v);
@@ -235,12 +237,27 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Joooo = w.take<c128>(o * o * o * o);
     {
         double per_a = (double)v * v * v * 16.0;
-        int na = (int)(1.5e9 / (per_a > 1 ? per_a : 1));
+        // direct_ladder: slabs grow with the tensor they replace (a sixth of its bytes, 1.5 - 6 GB), so that the ladder GEMM
+        // on one slab of rows fills several waves of the 148 SMs once the problem is large enough to need this mode
+        double budget = 1.5e9;
+        if (c->opt.direct_ladder) {
+            budget = (double)vv * (double)vv * 16.0 / 6.0;
+            if (budget < 1.5e9) budget = 1.5e9;
+            if (budget > 6.0e9) budget = 6.0e9;
+        }
+        int na = (int)(budget / (per_a > 1 ? per_a : 1));
         if (na < 1) na = 1;
         if (na > v) na = (int)v;
         c->na_slab = na;
         c->Jslab = w.take<c128>((int64_t)na * v * v * v);
         c->JslabT = w.take<c128>((int64_t)na * v * v * v);
+        c->Wslab = nullptr;
+        c->Wslabs = nullptr;
+        if (c->opt.direct_ladder) {
+            const int64_t max_rows = (int64_t)na * (v - 1);        // pairs (a,b), b > a, of na values of a: at most na (v-1)
+            c->Wslab = w.take<c128>(max_rows * vv);
+            c->Wslabs = w.take<double>(max_rows * vv);
+        }
     }
     // amplitudes, residuals, operands
     c->t1 = w.take<c128>(ov);
@@ -282,7 +299,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
     if (c->planes) {
-        c->Ws = w.take<double>(vv * vv);
+        c->Ws = c->opt.direct_ladder ? nullptr : w.take<double>(vv * vv);
         c->Vvovv_ps = w.take<double>(ov * vv);
         c->Voovv_ps = w.take<double>(oo * vv);
         c->G1s = w.take<double>(ov * ov);
@@ -385,6 +402,38 @@ static void bblock(cudaStream_t st, c128* out, const c128* B, int n, int L, int 
         int64_t p = p0 + row / nq, q = q0 + row % nq;
         return B[l * (int64_t)n * n + p * n + q];
     });
+}
+
+// Rows of the packed <ab||cd> = (ac|bd) - (ad|bc) owned by the slab a in [a0, a0 + na_slab) of the first virtual index
+// (pairs (a,b), b > a: a contiguous range [r0, r0 + nrows) of packed rows), from the factor B; the v^4 staging tensor is
+// never materialised:
+//   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
+//   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
+//   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
+// absolute = true: dst is the whole matrix (row r0 of the slab goes to dst + r0 vv); false: dst holds the slab only.
+static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* r0_out, int64_t* nrows_out)
+{
+    cudaStream_t st = c->st;
+    const int v = c->v, Lp = c->Lp;
+    const int64_t vv = c->vv, v2 = (int64_t)v * v;
+    const int2* pv = c->pv;
+    const int na = (a0 + c->na_slab <= v) ? c->na_slab : v - a0;
+    const int64_t rows = (int64_t)na * v;
+    CCSD_TRY(run_gemm(c->env, gp(rows, v2, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv, Lp, c->Jslab, v2, 1, 1.0, 0)));
+    CCSD_TRY(launch_transpose2d(st, c->Jslab, c->JslabT, rows, v2, 0));
+    const int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
+    const int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
+    const c128 *J = c->Jslab, *JT = c->JslabT;
+    launch_fill(st, dst + (absolute ? r0 * vv : 0), r1 - r0, vv, vv, 0, [=] __device__(int64_t r, int64_t CD) {
+        int2 ab = pv[r0 + r], cd = pv[CD];
+        int64_t al = ab.x - a0;
+        c128 x = J[(al * v + cd.x) * v2 + (int64_t)ab.y * v + cd.y];
+        c128 y = JT[((int64_t)ab.y * v + cd.x) * rows + al * v + cd.y];
+        return csub(x, y);
+    });
+    *r0_out = r0;
+    *nrows_out = r1 - r0;
+    return CCSD_OK;
 }
 
 static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
@@ -507,27 +556,14 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     //   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
     //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
     //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
-    const int64_t v2 = (int64_t)v * v;
-    for (int a0 = 0; a0 < v && vv > 0; a0 += c->na_slab) {
-        if (a0 > v - 2) break;
-        int na = (a0 + c->na_slab <= v) ? c->na_slab : v - a0;
-        int64_t rows = (int64_t)na * v;
-        CCSD_TRY(run_gemm(env, gp(rows, v2, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv, Lp, c->Jslab, v2, 1, 1.0, 0)));
-        CCSD_TRY(launch_transpose2d(st, c->Jslab, c->JslabT, rows, v2, 0));
-        // rows of W owned by this slab: pairs (a,b), a in [a0, a0+na), b > a -> a contiguous packed range
-        int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
-        int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
-        const c128 *J = c->Jslab, *JT = c->JslabT;
-        launch_fill(st, c->W + r0 * vv, r1 - r0, vv, vv, 0, [=] __device__(int64_t r, int64_t CD) {
-            int2 ab = pv[r0 + r], cd = pv[CD];
-            int64_t al = ab.x - a0;
-            c128 x = J[(al * v + cd.x) * v2 + (int64_t)ab.y * v + cd.y];
-            c128 y = JT[((int64_t)ab.y * v + cd.x) * rows + al * v + cd.y];
-            return csub(x, y);
-        });
+    if (!c->opt.direct_ladder) {
+        for (int a0 = 0; a0 < v - 1 && vv > 0; a0 += c->na_slab) {
+            int64_t r0 = 0, nrows = 0;
+            CCSD_TRY(build_W_slab(c, a0, c->W, true, &r0, &nrows));
+        }
     }
     if (c->planes) {   // sum planes of the constant operands of the large GEMMs (3M, gemm_dmma.cuh)
-        launch_sum_plane(st, c->W, c->Ws, vv * vv);
+        if (c->W) launch_sum_plane(st, c->W, c->Ws, vv * vv);
         launch_sum_plane(st, c->Vvovv_p, c->Vvovv_ps, ov * vv);
         launch_sum_plane(st, c->Voovv_p, c->Voovv_ps, oo * vv);
         launch_sum_plane(st, c->G1, c->G1s, ov * ov);
@@ -789,6 +825,16 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
             const int64_t a = ab.x, b = ab.y;
             return csub(R2[(a * o + ij.x) * ov + b * o + ij.y], R2[(a * o + ij.y) * ov + b * o + ij.x]);
         });
+        return CCSD_OK;
+    }
+    if (c->opt.direct_ladder) {   // integral-direct: rebuild the rows of <ab||cd> slab by slab from the factor B and contract them
+        for (int a0 = 0; a0 < c->v - 1; a0 += c->na_slab) {
+            int64_t r0 = 0, nrows = 0;
+            CCSD_TRY(build_W_slab(c, a0, c->Wslab, false, &r0, &nrows));
+            if (c->planes) launch_sum_plane(c->st, c->Wslab, c->Wslabs, nrows * c->vv);
+            CCSD_TRY(run_gemm(c->env, with_planes(gp(nrows, c->oo, c->vv, c->Wslab, c->vv, c->taup, c->vv, S + r0, 1, c->vv, 1.0, 1),
+                                                  c->planes ? c->Wslabs : nullptr, c->taups)));
+        }
         return CCSD_OK;
     }
     return run_gemm(c->env, with_planes(gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), c->Ws, c->taups));
@@ -1067,6 +1113,7 @@ void ccsd_default_options(ccsd_options* opts)
     opts->gemm_mode = 0;
     opts->ccd = 0;
     opts->cc2 = 0;
+    opts->direct_ladder = 0;
 }
 
 int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
@@ -1343,7 +1390,10 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
     if (id >= CCSD_T_TAU && !c->have_residual) return CCSD_ESTATE;
     switch (id) {
     case CCSD_T_FOCK: dcopy(st, out, c->f, (int64_t)c->n * c->n); break;
-    case CCSD_T_VVVV: dcopy(st, out, c->W, vv * vv); break;
+    case CCSD_T_VVVV:
+        if (!c->W) return CCSD_EINVAL;   // direct_ladder: not stored
+        dcopy(st, out, c->W, vv * vv);
+        break;
     case CCSD_T_VOVV: dcopy(st, out, c->Vvovv_p, ov * vv); break;
     case CCSD_T_VOVO: {
         const c128* V = c->Vvovo_m;  // [(a,i)][(c,k)] -> [a][k][c][i]
@@ -1659,7 +1709,7 @@ int ccsd_lambda_workspace_bytes(ccsd_ctx* c, size_t* bytes)
 int ccsd_lambda_init(ccsd_ctx* c, void* workspace, size_t workspace_bytes)
 {
     if (!c) return CCSD_ESTATE;
-    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || c->opt.cc2) return CCSD_EINVAL;
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || c->opt.cc2 || c->opt.direct_ladder) return CCSD_EINVAL;
     size_t need = 0;
     LambdaState tmp;
     lambda_carve(c, nullptr, &tmp, &need);

@@ -186,3 +186,30 @@ def test_fullsize_triples_driver_sampled(gpu, cfg):
     e = gc.triples()
     assert e["+T"].real < 0 and e["+T"].imag == 0.0
     gc.close()
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg3"])
+def test_fullsize_direct_ladder_sampled(gpu, cfg):
+    """Integral-direct pp-ladder at full size (several slabs of the first virtual index): sampled outputs of the term,
+    including the first and last rows of every slab boundary region, against the oracle's evaluator from B."""
+    import torch
+    from oracle import ccsd_oracle as orc
+    inp = ci.make_config(cfg)
+    o, v = inp.nocc, inp.nvir
+    oo, vv = ci.pair_count(o), ci.pair_count(v)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, direct_ladder=True)
+    t1, t2p = ci.random_amplitudes(o, v, 8, 0.01)
+    gc.set_amplitudes(t1, t2p)
+    gc.residual()
+    R = gc.get_tensor("S2_pp_ladder").view(oo, vv)
+    rng = np.random.default_rng(4)
+    nl = 40
+    IJ, AB = rng.integers(0, oo, nl), rng.integers(0, vv, nl)
+    IJ[:4] = [0, oo - 1, 0, oo - 1]; AB[:4] = [0, vv - 1, vv - 1, 0]
+    AB[4:12] = np.linspace(1, vv - 2, 8).astype(int)          # spread over the slabs
+    got = R[torch.from_numpy(IJ).cuda(), torch.from_numpy(AB).cuda()].cpu().numpy()
+    ref = orc.pp_ladder_samples_from_B(inp.B, o, t1, t2p, IJ, AB)
+    assert np.abs(got - ref).max() <= REL_TOL * float(R.abs().max())
+    e, sn = gc.iterate()
+    assert np.isfinite(sn)
+    gc.close()
