@@ -407,7 +407,7 @@ static void bblock(cudaStream_t st, c128* out, const c128* B, int n, int L, int 
 // Rows of the packed <ab||cd> = (ac|bd) - (ad|bc) owned by the slab a in [a0, a0 + na_slab) of the first virtual index
 // (pairs (a,b), b > a: a contiguous range [r0, r0 + nrows) of packed rows), from the factor B; the v^4 staging tensor is
 // never materialised:
-//   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
+//   Jslab[(a,c)][(b,d)] = (ac|bd), b > a0               (GEMM over the auxiliary index)
 //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
 //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
 // absolute = true: dst is the whole matrix (row r0 of the slab goes to dst + r0 vv); false: dst holds the slab only.
@@ -419,8 +419,10 @@ static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* 
     const int2* pv = c->pv;
     const int na = (a0 + c->na_slab <= v) ? c->na_slab : v - a0;
     const int64_t rows = (int64_t)na * v;
-    CCSD_TRY(run_gemm(c->env, gp(rows, v2, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv, Lp, c->Jslab, v2, 1, 1.0, 0)));
-    CCSD_TRY(launch_transpose2d(st, c->Jslab, c->JslabT, rows, v2, 0));
+    // only b > a is needed, i.e. the columns (b,d) with b >= a0 + 1 of the slab (half the columns on average)
+    const int64_t col0 = (int64_t)(a0 + 1) * v, ncol = v2 - col0;
+    CCSD_TRY(run_gemm(c->env, gp(rows, ncol, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv + col0 * Lp, Lp, c->Jslab + col0, v2, 1, 1.0, 0)));
+    CCSD_TRY(launch_transpose2d_ld(st, c->Jslab + col0, v2, c->JslabT + col0 * rows, rows, rows, ncol, 0));
     const int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
     const int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
     const c128 *J = c->Jslab, *JT = c->JslabT;
