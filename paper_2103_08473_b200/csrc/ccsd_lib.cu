@@ -208,7 +208,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->pv = w.take<int2>(vv);
     c->eps = w.take<double>(n);
     c->f = w.take<c128>(n * n);
-    c->W = c->opt.direct_ladder ? nullptr : w.take<c128>(vv * vv);   // direct_ladder: <ab||cd> is never stored
+    // <ab||cd> is not stored in direct_ladder mode (rebuilt every iteration) nor in CC2 mode (its only use factorises)
+    c->W = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<c128>(vv * vv);
     c->Vvovv_p = w.take<c128>(v * o * vv);
     c->Vvovv_u = w.take<c128>(v * v * o * v);
     c->VvovvT = w.take<c128>(o * vv * v);
@@ -299,7 +300,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
     if (c->planes) {
-        c->Ws = c->opt.direct_ladder ? nullptr : w.take<double>(vv * vv);
+        c->Ws = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<double>(vv * vv);
         c->Vvovv_ps = w.take<double>(ov * vv);
         c->Voovv_ps = w.take<double>(oo * vv);
         c->G1s = w.take<double>(ov * ov);
@@ -558,7 +559,7 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     //   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
     //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
     //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
-    if (!c->opt.direct_ladder) {
+    if (c->W) {
         for (int a0 = 0; a0 < v - 1 && vv > 0; a0 += c->na_slab) {
             int64_t r0 = 0, nrows = 0;
             CCSD_TRY(build_W_slab(c, a0, c->W, true, &r0, &nrows));
