@@ -297,6 +297,21 @@ def triples_bench(torch, pkg, inp, o, v, peak_tflops):
                     "executed (3M) flops"}
 
 
+def direct_ladder_bench(torch, pkg, inp, o, v, steps=3, warmup=2):
+    """Rank 4 of SURVEY 8(f), first half: the CCSD iteration with the integral-direct pp-ladder (<ab||cd> rebuilt from B
+    every iteration, never stored)."""
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, direct_ladder=True)
+    solver.enable_step_timing(True)
+    ts = time_events(torch, solver.iterate, steps, warmup)
+    st = solver.step_times()
+    ws = solver.workspace_bytes
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    return {"s_per_iteration": round(statistics.median(ts) * 1e-3, 5), "pp_ladder_ms": round(st["pp_ladder"], 2),
+            "workspace_gib": round(ws / 2 ** 30, 1), "steps": steps, "warmup": warmup}
+
+
 def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
     """NEXT-2 row of SURVEY 8(f): Lambda equations at the amplitudes after three CCSD iterations
     (the cost of a Lambda iteration does not depend on the convergence of T): Hbar build once, then timed iterations."""
@@ -502,6 +517,7 @@ def run_ours(args) -> None:
     cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     triples = triples_bench(torch, pkg, inp, o, v, peak) if not args.no_sweep else None
     lam = lambda_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
+    direct = direct_ladder_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
     cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
@@ -525,7 +541,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "cc2": cc2, "triples": triples, "lambda": lam, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "triples": triples, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:
