@@ -198,7 +198,18 @@ int ccsd_triples_block(ccsd_ctx* ctx, int i, int j, int k, ccsd_c128* Wbar, ccsd
  * accumulate != 0 adds into out.  workspace: ccsd_contract_workspace_bytes() bytes.  Asynchronous on the stream.
  */
 enum { CCSD_TERM_PP_LADDER = 0, CCSD_TERM_HH_LADDER = 1, CCSD_TERM_RING = 2, CCSD_TERM_TAU = 3,
-       CCSD_TERM_PP_LADDER_PLANES = 4 };
+       CCSD_TERM_PP_LADDER_PLANES = 4,
+       /* The intermediates of eqs 24-31 (BASELINE north_star names: F_me, F_ae, F_mi, W_mnij, W_mbej; DESIGN.md relates them to
+        * the paper's H^k_c, G^a_c, G^k_i, A^{kl}_{ij}, H^{ak}_{ci}, C^{kb}_{ij}).  Inputs in the canonical layouts listed at the
+        * top of this file, f = the Fock matrix [n][n]; accumulate must be 0:
+        *   F_OV   (eq 28)      in = { f, <kl||cd>, t1 }                                  out H^k_c [k][c]
+        *   F_VV   (eqs 24-25)  in = { f, <kl||cd>, <ak||cd>, t1, t2 }                    out G^a_c [a][c]
+        *   F_OO   (eqs 26-27)  in = { f, <kl||cd>, <kl||ic>, t1, t2 }                    out G^k_i [k][i]
+        *   W_OOOO (eq 31)      in = { <kl||ij>, <kl||ic>, <kl||cd>, t1, t2 }             out A [(k<l)][(i<j)]
+        *   W_OVVO (eq 29)      in = { <ak||ci>, <ak||cd>, <kl||ic>, <kl||cd>, t1, t2 }   out H^{ak}_{ci} [a][k][c][i]
+        *   C_OVOO (eq 30)      in = { <kl||ic>, <ak||ci>, <ak||cd>, t1, t2 }             out C [k][b][(i<j)]                    */
+       CCSD_TERM_F_OV = 5, CCSD_TERM_F_VV = 6, CCSD_TERM_F_OO = 7, CCSD_TERM_W_OOOO = 8, CCSD_TERM_W_OVVO = 9,
+       CCSD_TERM_C_OVOO = 10 };
 int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes);
 int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd_c128* out, int accumulate,
                   const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);

@@ -13,7 +13,8 @@ TENSOR_IDS = {"fock": 0, "vvvv": 1, "vovv": 2, "vovo": 3, "oovv": 4, "ooov": 5, 
               "Gvv": 12, "Hoo": 13, "Goo": 14, "Hov": 15, "Hvovo": 16, "C": 17, "A": 18, "S1": 19, "S2": 20,
               "S2_ring": 30, "S2_goo": 31, "S2_vdag_t1": 32, "S2_gvv": 33, "S2_c_t1": 34, "S2_hh_ladder": 35,
               "S2_pp_ladder": 36, "S2_driver": 37}
-TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3, "pp_ladder_planes": 4}
+TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3, "pp_ladder_planes": 4,
+            "f_ov": 5, "f_vv": 6, "f_oo": 7, "w_oooo": 8, "w_ovvo": 9, "c_ovoo": 10}
 NSTEPS = 16
 
 # every symbol include/ccsd.h declares
@@ -377,13 +378,20 @@ class CCSD:
 
 
 def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool = False, gemm_mode: int = 0):
-    """ccsd_contract on CUDA tensors; returns out [(i<j)][(a<b)]."""
+    """ccsd_contract on CUDA tensors; returns out ([(i<j)][(a<b)] for the ladder/ring/tau terms, the layouts of
+    include/ccsd.h for the intermediates f_ov ... c_ovoo)."""
     torch = _torch()
     lib = load_library()
     tid = TERM_IDS[term]
     oo, vv = nocc * (nocc - 1) // 2, nvir * (nvir - 1) // 2
     # the sum planes of "pp_ladder_planes" (inputs[2:]) are real float64 CUDA tensors made by sum_plane()
     ins = [_dev_c128(torch, x) for x in inputs[:2]] + list(inputs[2:])
+    if tid >= TERM_IDS["f_ov"]:   # the intermediates of eqs 24-31: every input complex128, output shape per term
+        ins = [_dev_c128(torch, x) for x in inputs]
+        shape = {"f_ov": (nocc, nvir), "f_vv": (nvir, nvir), "f_oo": (nocc, nocc), "w_oooo": (oo, oo),
+                 "w_ovvo": (nvir, nocc, nvir, nocc), "c_ovoo": (nocc, nvir, oo)}[term]
+        if out is None:
+            out = torch.zeros(shape, dtype=torch.complex128, device="cuda")
     if out is None:
         out = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
     nbytes = ctypes.c_size_t(0)

@@ -1105,6 +1105,7 @@ static int solve_small(std::vector<double>& A, std::vector<double>& b, int m)
 }
 
 #include "lambda.cuh"
+#include "contract_terms.cuh"
 
 extern "C" {
 
@@ -1809,6 +1810,11 @@ int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
 {
     if (!bytes || nocc < 1 || nvir < 1) return CCSD_EINVAL;
     const int64_t o = nocc, v = nvir, oo = o * (o - 1) / 2, vv = v * (v - 1) / 2, ov = o * v, oop = round_up(oo > 0 ? oo : 1, 4);
+    if (term >= CCSD_TERM_F_OV && term <= CCSD_TERM_C_OVOO) {
+        TermWs tw;
+        term_carve(nocc, nvir, nullptr, &tw, bytes);
+        return CCSD_OK;
+    }
     Carver w{nullptr, 0};
     w.take<int2>(oo); w.take<int2>(vv);
     switch (term) {
@@ -1839,6 +1845,13 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const int o = nocc, v = nvir;
     const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2, ov = (int64_t)o * v, oop = round_up(oo > 0 ? oo : 1, 4);
+    if (term >= CCSD_TERM_F_OV && term <= CCSD_TERM_C_OVOO) {   // intermediates of eqs 24-31 (contract_terms.cuh)
+        if (accumulate || nocc < 2 || nvir < 2) return CCSD_EINVAL;
+        static const int k_nin[] = {3, 5, 5, 5, 6, 5};
+        Env env2{st, opts ? opts->gemm_mode : 0, nullptr, 0};
+        return contract_intermediate(term, nocc, nvir, reinterpret_cast<const c128* const*>(in_), k_nin[term - CCSD_TERM_F_OV],
+                                     reinterpret_cast<c128*>(out_), env2, static_cast<char*>(workspace));
+    }
     Env env{st, opts ? opts->gemm_mode : 0, nullptr, 0};
     {   // split-K partials live at the end of the workspace (same carving order as ccsd_contract_workspace_bytes)
         size_t all = 0;

@@ -151,8 +151,9 @@ static void unpack_pairs(cudaStream_t st, c128* out, const c128* in, int m1, int
 {   // ncols: number of (opaque) columns when the second pair is not packed and is not an m2 x m2 pair
     const int64_t n1 = (int64_t)m1 * m1, n2 = (!pk2 && ncols > 0) ? ncols : (int64_t)m2 * m2;
     const int64_t ld = pk2 ? (int64_t)m2 * (m2 - 1) / 2 : n2;
+    const int m2d = m2 > 0 ? m2 : 1;
     launch_fill(st, out, n1, n2, n2, 0, [=] __device__(int64_t xy, int64_t pq) {
-        int x = (int)(xy / m1), y = (int)(xy % m1), p = (int)(pq / m2), q = (int)(pq % m2);
+        int x = (int)(xy / m1), y = (int)(xy % m1), p = (int)(pq / m2d), q = (int)(pq % m2d);
         double sg = 1.0;
         int64_t row = xy, col = pq;
         if (pk1) {

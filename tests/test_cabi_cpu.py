@@ -55,7 +55,8 @@ def test_workspace_bytes_scales_and_validates(lib):
     assert lib.ccsd_workspace_bytes(4, 16, 0, None, ctypes.byref(n)) == 1
     assert lib.ccsd_workspace_bytes(4, 16, 60, None, None) == 1
     assert lib.ccsd_contract_workspace_bytes(0, 4, 16, ctypes.byref(n)) == 0
-    assert lib.ccsd_contract_workspace_bytes(7, 4, 16, ctypes.byref(n)) == 1
+    assert lib.ccsd_contract_workspace_bytes(7, 4, 16, ctypes.byref(n)) == 0      # F_OO
+    assert lib.ccsd_contract_workspace_bytes(11, 4, 16, ctypes.byref(n)) == 1
 
 
 def test_null_handles_are_rejected(lib):
