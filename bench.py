@@ -297,6 +297,32 @@ def triples_bench(torch, pkg, inp, o, v, peak_tflops):
                     "executed (3M) flops"}
 
 
+def triples_sharded_bench(torch, pkg, inp, o, v, dist):
+    """N > 1 only: the triples correction shared among the ranks (CCSD.triples_sharded: contiguous ranges of the
+    occupied triples i<j<k, one all-reduce of six doubles).  Total work fixed -> strong scaling; seconds = max over ranks."""
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    for _ in range(2):
+        solver.iterate()
+    solver.triples_sharded()                           # warm-up
+    torch.cuda.synchronize()
+    dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    en = solver.triples_sharded()
+    e1.record()
+    torch.cuda.synchronize()
+    sec = max_over_ranks(e0.elapsed_time(e1) * 1e-3, dist)
+    nt = solver.triples_count()
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    return {"seconds": round(sec, 4), "ranks": dist.get_world_size(), "occupied_triples": nt, "scaling": "strong",
+            "E(+T)": [en["+T"].real, en["+T"].imag], "E((T))": [en["(T)"].real, en["(T)"].imag],
+            "E(-T)": [en["-T"].real, en["-T"].imag],
+            "note": "each rank evaluates a contiguous range of the occupied triples (ccsd_triples_range); no data-path "
+                    "collective, one all-reduce of six doubles"}
+
+
 def direct_ladder_bench(torch, pkg, inp, o, v, steps=3, warmup=2):
     """Rank 4 of SURVEY 8(f), first half: the CCSD iteration with the integral-direct pp-ladder (<ab||cd> rebuilt from B
     every iteration, never stored)."""
@@ -473,6 +499,8 @@ def run_ours(args) -> None:
     e2e_s = max_over_ranks(e2e_s, dist if world > 1 else None)
     nvec_bytes = (ov + oo * vv) * 16
 
+    trip_sharded = triples_sharded_bench(torch, pkg, inp, o, v, dist) if (world > 1 and not args.no_sweep) else None
+
     if not is_reporting_rank():
         if world > 1:
             dist.destroy_process_group()
@@ -541,7 +569,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "cc2": cc2, "triples": triples, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "triples": triples, "triples_sharded": trip_sharded, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:

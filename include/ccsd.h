@@ -147,6 +147,17 @@ int ccsd_triples(ccsd_ctx* ctx, double e_plus_t[2], double e_par_t[2], double e_
                  size_t workspace_bytes);
 int ccsd_get_triples_times(ccsd_ctx* ctx, float ms[2]);
 /*
+ * The same energies restricted to the occupied triples number first_triple .. first_triple + ntriples - 1 of the
+ * lexicographic list of i<j<k (ccsd_triples_count() entries; "only the unique blocks" of the three nested
+ * occupied loops).  The outputs are the partial sums of eq 39/42/44 over those triples: summed over a partition of the
+ * list they give the values of ccsd_triples, which is how the correction is shared among GPUs (one context per GPU on
+ * the same amplitudes, one range each, one sum of six doubles at the end; binding: CCSD.triples_sharded).
+ * ntriples == 0 returns zeros.  CCSD_EINVAL when the range leaves the list.
+ */
+int ccsd_triples_count(ccsd_ctx* ctx, int64_t* ntriples);
+int ccsd_triples_range(ccsd_ctx* ctx, int64_t first_triple, int64_t ntriples, double e_plus_t[2], double e_par_t[2],
+                       double e_minus_t[2], void* workspace, size_t workspace_bytes);
+/*
  * CCSD Lambda equations and Lagrange one-body density matrix (Appendix 7.4-7.5, eqs 45-61; PAPER.md:109-126,
  * 238), at the CURRENT amplitudes, which should be converged (ccsd_solve): the equations are
  * <0|(1+Lambda)(Hbar - E)|mu> = 0 up to terms proportional to the amplitude residual.  Reading of the incomplete

@@ -144,3 +144,36 @@ void oracle_triples_energies(int o, int v, int restricted, const double *eps, co
     const double w = restricted ? 1.0 / 6.0 : 1.0 / 36.0;
     out[0] = w * e4; out[1] = w * e5; out[2] = w * ey;
 }
+
+/*
+ * The same sums restricted to a LIST of unique occupied triples i<j<k (ijk: ntrip x 3 ints): the partial sums of the
+ * restricted form of eqs 39, 41, 43 (weight 1/6 over a<b<c-unrestricted virtual sums), i.e. what one rank of a
+ * multi-GPU split evaluates ("only the unique blocks").  Over the full list this is
+ * oracle_triples_energies(restricted = 1).  out as there.  work: 6 * v^3 elements.
+ */
+void oracle_triples_energies_list(int o, int v, int ntrip, const int *ijk, const double *eps, const zc *fov, const zc *t1,
+                                  const zc *t2, const zc *vvov, const zc *vooo, const zc *vvoo, zc *work, zc *out)
+{
+    const size_t v3 = (size_t)v * v * v;
+    zc *W = work, *Wb = work + v3, *Z = work + 2 * v3, *Zb = work + 3 * v3, *Y = work + 4 * v3, *Yb = work + 5 * v3;
+    zc e4 = 0.0, e5 = 0.0, ey = 0.0;
+    for (int q = 0; q < ntrip; q++) {
+        const int i = ijk[3 * q], j = ijk[3 * q + 1], k = ijk[3 * q + 2];
+        oracle_triples_W(o, v, t2, vvov, vooo, i, j, k, W);
+        oracle_triples_cyclic(v, W, Wb);
+        oracle_triples_Z(o, v, fov, t1, t2, vvoo, i, j, k, Z);
+        oracle_triples_cyclic(v, Z, Zb);
+        oracle_triples_Y(o, v, t1, t2, i, j, k, Y);
+        oracle_triples_cyclic(v, Y, Yb);
+        for (int a = 0; a < v; a++)
+            for (int b = 0; b < v; b++)
+                for (int c = 0; c < v; c++) {
+                    const double D = eps[i] + eps[j] + eps[k] - eps[o + a] - eps[o + b] - eps[o + c];
+                    const zc w = Wb[IDX3(a, b, c, v, v)];
+                    e4 += conj(w) * w / D;
+                    e5 += conj(Zb[IDX3(a, b, c, v, v)]) * w / D;
+                    ey += conj(Yb[IDX3(a, b, c, v, v)]) * w;
+                }
+    }
+    out[0] = e4 / 6.0; out[1] = e5 / 6.0; out[2] = ey / 6.0;
+}

@@ -82,6 +82,19 @@ class OracleTriples:
                                       _p(self.t2), _p(self.vvov), _p(self.vooo), _p(self.vvoo), _p(work), _p(out))
         return {"+T": complex(out[0]), "(T)": complex(out[0] + out[1]), "-T": complex(out[0] + out[2])}
 
+    def energies_of(self, triples) -> dict:
+        """Partial sums of the same three energies over a list of unique occupied triples (i<j<k): what one rank of a
+        multi-GPU split evaluates ("only the unique blocks").  Over all C(o,3) triples = energies()."""
+        v = self.v
+        ijk = np.ascontiguousarray(np.asarray(list(triples), dtype=np.int32).reshape(-1, 3))
+        assert all(0 <= a < b < c < self.o for a, b, c in ijk)
+        work = np.zeros(6 * v ** 3, dtype=C128)
+        out = np.zeros(3, dtype=C128)
+        lib().oracle_triples_energies_list(self.o, v, int(ijk.shape[0]), ijk.ctypes.data_as(ctypes.c_void_p), _p(self.eps),
+                                           _p(self.fov), _p(self.t1), _p(self.t2), _p(self.vvov), _p(self.vooo),
+                                           _p(self.vvoo), _p(work), _p(out))
+        return {"+T": complex(out[0]), "(T)": complex(out[0] + out[1]), "-T": complex(out[0] + out[2])}
+
 
 # ---------------------------------------------------------------------------------------------------------------
 # single-element evaluator straight from the factorised integrals (full-size spot checks at cfg2 / cfg3, where the

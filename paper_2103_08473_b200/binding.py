@@ -24,7 +24,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
-           "ccsd_triples_block", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
+           "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
            "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation"]
 
@@ -109,6 +109,8 @@ def load_library():
         lib.ccsd_triples_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_triples.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3 + [vp, ctypes.c_size_t]
         lib.ccsd_get_triples_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+        lib.ccsd_triples_count.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+        lib.ccsd_triples_range.argtypes = [vp, ctypes.c_int64, ctypes.c_int64] + [ctypes.POINTER(dbl)] * 3 + [vp, ctypes.c_size_t]
         lib.ccsd_triples_block.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, ctypes.c_size_t]
         _LIB = lib
     return _LIB
@@ -293,6 +295,31 @@ class CCSD:
         _check(self._lib.ccsd_triples(self._ctx, a, b, c, base, nbytes), "ccsd_triples")
         del ws
         return {"+T": complex(a[0], a[1]), "(T)": complex(b[0], b[1]), "-T": complex(c[0], c[1])}
+
+    def triples_count(self) -> int:
+        n = ctypes.c_int64(0)
+        _check(self._lib.ccsd_triples_count(self._ctx, ctypes.byref(n)), "ccsd_triples_count")
+        return int(n.value)
+
+    def triples_range(self, first: int, count: int) -> dict:
+        """Partial sums of +T / (T) / -T over the occupied triples first .. first+count-1 (ccsd_triples_range)."""
+        ws, base, nbytes = self._triples_workspace()
+        a, b, c = (ctypes.c_double * 2)(), (ctypes.c_double * 2)(), (ctypes.c_double * 2)()
+        _check(self._lib.ccsd_triples_range(self._ctx, int(first), int(count), a, b, c, base, nbytes), "ccsd_triples_range")
+        del ws
+        return {"+T": complex(a[0], a[1]), "(T)": complex(b[0], b[1]), "-T": complex(c[0], c[1])}
+
+    def triples_sharded(self, group=None) -> dict:
+        """The triples corrections shared among the ranks of a torch.distributed group (every rank holds the same
+        amplitudes): each rank evaluates its contiguous range of the occupied triples i<j<k, the six doubles are summed
+        with one all-reduce (NCCL: on the device).  Without an initialised process group this is triples()."""
+        import torch.distributed as dist
+        from .sharding import shard_range, allreduce_energies
+        if not (dist.is_available() and dist.is_initialized()):
+            return self.triples()
+        rank, world = dist.get_rank(group), dist.get_world_size(group)
+        first, count = shard_range(self.triples_count(), rank, world)
+        return allreduce_energies(self.triples_range(first, count), group=group, device="cuda")
 
     def triples_times(self) -> dict:
         arr = (ctypes.c_float * 2)()

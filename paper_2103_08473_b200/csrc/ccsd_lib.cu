@@ -1602,12 +1602,32 @@ int ccsd_triples_workspace_bytes(ccsd_ctx* c, size_t* bytes)
     return CCSD_OK;
 }
 
+int ccsd_triples_count(ccsd_ctx* c, int64_t* ntriples)
+{
+    if (!c || !ntriples) return CCSD_ESTATE;
+    const int64_t o = c->o;
+    *ntriples = o >= 3 ? o * (o - 1) * (o - 2) / 6 : 0;
+    return CCSD_OK;
+}
+
 int ccsd_triples(ccsd_ctx* c, double e_plus_t[2], double e_par_t[2], double e_minus_t[2], void* workspace,
                  size_t workspace_bytes)
 {
     if (!c) return CCSD_ESTATE;
+    const int64_t o = c->o;
+    return ccsd_triples_range(c, 0, o * (o - 1) * (o - 2) / 6, e_plus_t, e_par_t, e_minus_t, workspace, workspace_bytes);
+}
+
+int ccsd_triples_range(ccsd_ctx* c, int64_t first_triple, int64_t ntriples, double e_plus_t[2], double e_par_t[2],
+                       double e_minus_t[2], void* workspace, size_t workspace_bytes)
+{
+    if (!c) return CCSD_ESTATE;
     if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0) return CCSD_EINVAL;
     if (c->o < 3 || c->v < 3) return CCSD_EINVAL;
+    {
+        const int64_t all = (int64_t)c->o * (c->o - 1) * (c->o - 2) / 6;
+        if (first_triple < 0 || ntriples < 0 || first_triple > all || ntriples > all - first_triple) return CCSD_EINVAL;
+    }
     TripWs w;
     size_t need = 0;
     trip_carve(c, nullptr, &w, &need);
@@ -1633,8 +1653,9 @@ int ccsd_triples(ccsd_ctx* c, double e_plus_t[2], double e_par_t[2], double e_mi
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     float gemm_ms = 0.f, energy_ms = 0.f;
     if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
-    for (int64_t first = 0; first < w.ntrip; first += w.nb) {
-        const int count = (int)((w.ntrip - first < w.nb) ? w.ntrip - first : w.nb);
+    const int64_t range_end = first_triple + ntriples;
+    for (int64_t first = first_triple; first < range_end; first += w.nb) {
+        const int count = (int)((range_end - first < w.nb) ? range_end - first : w.nb);
         if (c->timing) cudaEventRecord(e0, st);
         CCSD_TRY(trip_gemm(c, w, ld, V, first, count));
         if (c->timing) cudaEventRecord(e1, st);

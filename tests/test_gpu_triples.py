@@ -174,3 +174,41 @@ def test_triples_and_cc2_under_every_gemm_mode(gpu, gemm_mode):
         eo, eg = o2.iterate()[0], g2.iterate()[0]
         assert abs(eo - eg) < E_TOL
     g2.close()
+
+
+def test_triples_ranges_match_oracle_partial_sums(gpu):
+    """ccsd_triples_range (the unit of the multi-GPU split): partial sums over ranges of the lexicographic list of i<j<k
+    against the oracle's partial sums over the same triples; the pieces of every partition add up to ccsd_triples."""
+    import itertools
+    from paper_2103_08473_b200.binding import CCSDError
+    from paper_2103_08473_b200.sharding import shard_range
+    from oracle.ccsd_oracle import OracleCCSD
+    from oracle.triples_oracle import OracleTriples
+    o, v = 6, 9
+    inp = ci.make_inputs(o, v, 14, seed=61, b_scale=0.15, f_offdiag=0.05)
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    for _ in range(2):
+        oc.iterate(); gc.iterate()
+    ot = OracleTriples(oc)
+    triples = list(itertools.combinations(range(o), 3))
+    assert gc.triples_count() == len(triples) == 20
+    full = gc.triples()
+    for world in (1, 2, 3, 7):
+        tot = {"+T": 0.0, "(T)": 0.0, "-T": 0.0}
+        for rank in range(world):
+            first, count = shard_range(len(triples), rank, world)
+            got = gc.triples_range(first, count)
+            ref = ot.energies_of(triples[first:first + count])
+            for key in tot:
+                assert abs(got[key] - ref[key]) < E_TOL, (world, rank, key, got[key], ref[key])
+                tot[key] += got[key]
+        for key in tot:
+            assert abs(tot[key] - full[key]) < 1e-13, (world, key)
+    empty = gc.triples_range(20, 0)
+    assert all(empty[key] == 0 for key in empty)
+    assert gc.triples_sharded() == full                  # no process group: the whole list on this GPU
+    for first, count in ((-1, 2), (0, 21), (20, 1), (3, -1)):
+        with pytest.raises(CCSDError):
+            gc.triples_range(first, count)
+    gc.close()

@@ -140,3 +140,34 @@ def test_q6_single_element_evaluator_equals_plain_loop_oracle():
     got = wbar_samples_from_B(inp.B, o, pack_t2(t2), ijk, abc)
     ref = np.array([ot.W(*t)[1][x] for t, x in zip(ijk, abc)])
     assert np.abs(got - ref).max() < 1e-13 * np.abs(ref).max() + 1e-15
+
+
+def test_q7_partial_sums_over_occupied_triples_equal_determinant_space():
+    """energies_of(list of i<j<k) = the determinant-space sums restricted to the triply excited determinants with those
+    three holes (the unit of the multi-GPU split); the pieces of a partition add up to energies()."""
+    o, v = 4, 4
+    inp, oc, t1, t2 = _setup(o, v, 577)
+    ds, x, z, y = _detspace(inp, oc, t1, t2)
+    eps = oc.eps
+    ot = OracleTriples(oc)
+    all_triples = list(itertools.combinations(range(o), 3))
+    parts = [all_triples[:1], all_triples[1:3], all_triples[3:], []]
+    tot = {"+T": 0.0, "(T)": 0.0, "-T": 0.0}
+    for part in parts:
+        e4 = e5 = ey = 0.0
+        for i, j, k, a, b, c, idx, s in _triples_index(ds, o, v):
+            if tuple(sorted((i, j, k))) not in part:
+                continue
+            D = eps[i] + eps[j] + eps[k] - eps[o + a] - eps[o + b] - eps[o + c]
+            e4 += np.conj(x[idx]) * x[idx] / D
+            e5 += np.conj(z[idx]) * x[idx] / D
+            ey += np.conj(y[idx]) * x[idx]
+        e = ot.energies_of(part)
+        assert abs(e["+T"] - e4) < 1e-13 and abs(e["(T)"] - (e4 + e5)) < 1e-13 and abs(e["-T"] - (e4 + ey)) < 1e-13
+        if part:
+            assert abs(e4) > 1e-5
+        for key in tot:
+            tot[key] += e[key]
+    full = ot.energies(restricted=True)
+    for key in tot:
+        assert abs(tot[key] - full[key]) < 1e-13
