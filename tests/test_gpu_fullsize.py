@@ -65,9 +65,21 @@ def test_lockstep_energies_against_oracle_golden(gpu, cfg):
 def test_fullsize_sampled_integrals_ladder_and_properties(gpu, cfg):
     """Sampled <ab||cd>, <ak||cd>, <kl||cd>, H^k_c and pp-ladder outputs against the oracle's single-element
     evaluators, at seeded random amplitudes CN(0, 0.01^2); plus Hermiticity of <ab||cd> across the whole tensor."""
+    _sampled_checks(gpu, ci.make_config(cfg))
+
+
+def test_index_range_beyond_2_to_32_elements(gpu):
+    """Maximum-size edge case: nvir = 364 makes the packed <ab||cd> 66066 x 66066 = 4.36e9 elements (70 GB), beyond
+    both 2^31 and 2^32, so every flat index of the build and of the pp-ladder has to be 64-bit.  Same sampled checks
+    (the copy-out of the whole <ab||cd> is skipped: a second 70 GB buffer does not fit beside the 115 GiB workspace)."""
+    inp = ci.make_inputs(6, 364, 256, seed=2021030811)
+    assert ci.pair_count(inp.nvir) ** 2 > 2 ** 32
+    _sampled_checks(gpu, inp, check_w=False)
+
+
+def _sampled_checks(gpu, inp, check_w=True):
     import torch
     from oracle import ccsd_oracle as orc
-    inp = ci.make_config(cfg)
     o, v = inp.nocc, inp.nvir
     oo, vv = ci.pair_count(o), ci.pair_count(v)
     gc = gpu.CCSD(inp.h, inp.B, o, v)
@@ -75,23 +87,24 @@ def test_fullsize_sampled_integrals_ladder_and_properties(gpu, cfg):
     av, bv = np.triu_indices(v, 1)
     io, jo = np.triu_indices(o, 1)
     ns = 48
-    # ---- integral classes (step I2) ----
-    W = gc.get_tensor("vvvv").view(vv, vv)
     AB, CD = rng.integers(0, vv, ns), rng.integers(0, vv, ns)
     AB[:4] = [0, vv - 1, 0, vv - 1]; CD[:4] = [0, vv - 1, vv - 1, 0]          # corners of the packed matrix
-    got = W[torch.from_numpy(AB).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
-    ref = orc.g_samples(inp.B, o + av[AB], o + bv[AB], o + av[CD], o + bv[CD])
-    scale = np.abs(ref).max()
-    assert np.abs(got - ref).max() <= REL_TOL * scale
-    # Hermiticity <ab||cd> = conj <cd||ab> over the whole tensor, slab by slab (a property at any size)
-    worst = 0.0
-    step = 2048
-    for r0 in range(0, vv, step):
-        blk = W[r0:r0 + step, :]
-        blkT = W[:, r0:r0 + step].transpose(0, 1).conj()
-        worst = max(worst, float((blk - blkT).abs().max()))
-    assert worst <= 1e-15 * 10 + REL_TOL * scale
-    del W
+    # ---- integral classes (step I2) ----
+    if check_w:
+        W = gc.get_tensor("vvvv").view(vv, vv)
+        got = W[torch.from_numpy(AB).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
+        ref = orc.g_samples(inp.B, o + av[AB], o + bv[AB], o + av[CD], o + bv[CD])
+        scale = np.abs(ref).max()
+        assert np.abs(got - ref).max() <= REL_TOL * scale
+        # Hermiticity <ab||cd> = conj <cd||ab> over the whole tensor, slab by slab (a property at any size)
+        worst = 0.0
+        step = 2048
+        for r0 in range(0, vv, step):
+            blk = W[r0:r0 + step, :]
+            blkT = W[:, r0:r0 + step].transpose(0, 1).conj()
+            worst = max(worst, float((blk - blkT).abs().max()))
+        assert worst <= 1e-15 * 10 + REL_TOL * scale
+        del W
     X = gc.get_tensor("vovv").view(v, o, vv)
     a, k = rng.integers(0, v, ns), rng.integers(0, o, ns)
     got = X[torch.from_numpy(a).cuda(), torch.from_numpy(k).cuda(), torch.from_numpy(CD).cuda()].cpu().numpy()
