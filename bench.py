@@ -427,6 +427,15 @@ def run_ours(args) -> None:
         print(json.dumps({"metric": "lambda_seconds_per_iteration", "unit": "s", "config": {"workload": f"{cfg} Lambda"},
                           **lambda_bench(torch, pkg, inp, o, v)}))
         return
+    if args.only_cc2:
+        print(json.dumps({"metric": "cc2_seconds_per_iteration", "unit": "s", "config": {"workload": f"{cfg} CC2"},
+                          **cc2_bench(torch, pkg, inp, o, v)}))
+        return
+    if args.only_direct:
+        print(json.dumps({"metric": "direct_ladder_seconds_per_iteration", "unit": "s",
+                          "config": {"workload": f"{cfg} CCSD, integral-direct pp-ladder"},
+                          **direct_ladder_bench(torch, pkg, inp, o, v)}))
+        return
     if args.only_triples:
         # profiling aid: ccsd_init, one iteration, then the perturbative triples of this workload (same launches as
         # the "triples" leg of the default run)
@@ -588,6 +597,8 @@ def main():
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")
     ap.add_argument("--only-triples", action="store_true", help="time only the perturbative triples of --config")
+    ap.add_argument("--only-cc2", action="store_true", help="time only the CC2 iteration of --config")
+    ap.add_argument("--only-direct", action="store_true", help="time only the CCSD iteration with the integral-direct pp-ladder")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -166,6 +166,7 @@ struct ccsd_ctx {
     // CC2 only: B blocks with the contracted virtual index fastest and the t1-dressed factors X (cc2_dressed_factors)
     c128 *BvvT, *BovT, *Xv, *Xo;
     double* Xvs;
+    double* Bvvs;           // 3M sum plane of Bvv (the <ab||cd> slab GEMM over the auxiliary index)
     c128* partial;
     int64_t partial_elems;
     // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
@@ -309,6 +310,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
         c->T2rs = w.take<double>(ov * ov);
         c->Hms = w.take<double>(ov * ov);
     }
+    c->Bvvs = (c->planes && !c->opt.cc2) ? w.take<double>(v * v * Lp) : nullptr;
     c->BvvT = c->BovT = c->Xv = c->Xo = nullptr;
     c->Xvs = nullptr;
     if (c->opt.cc2) {
@@ -422,7 +424,9 @@ static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* 
     const int64_t rows = (int64_t)na * v;
     // only b > a is needed, i.e. the columns (b,d) with b >= a0 + 1 of the slab (half the columns on average)
     const int64_t col0 = (int64_t)(a0 + 1) * v, ncol = v2 - col0;
-    CCSD_TRY(run_gemm(c->env, gp(rows, ncol, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv + col0 * Lp, Lp, c->Jslab + col0, v2, 1, 1.0, 0)));
+    GemmParams g = gp(rows, ncol, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv + col0 * Lp, Lp, c->Jslab + col0, v2, 1, 1.0, 0);
+    if (c->Bvvs) g = with_planes(g, c->Bvvs + (int64_t)a0 * v * Lp, c->Bvvs + col0 * Lp);
+    CCSD_TRY(run_gemm(c->env, g));
     CCSD_TRY(launch_transpose2d_ld(st, c->Jslab + col0, v2, c->JslabT + col0 * rows, rows, rows, ncol, 0));
     const int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
     const int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
@@ -473,6 +477,7 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     bblock(st, c->Bov, B, n, L, Lp, 0, o, o, v);
     bblock(st, c->Bvo, B, n, L, Lp, o, v, 0, o);
     bblock(st, c->Bvv, B, n, L, Lp, o, v, o, v);
+    if (c->Bvvs) launch_sum_plane(st, c->Bvv, c->Bvvs, (int64_t)v * v * Lp);
 
     // chemists' blocks (pq|rs) = sum_L B[L,p,q] B[L,r,s]  as NT GEMMs over the auxiliary index
     CCSD_TRY(run_gemm(env, gp(ov, ov, Lp, c->Bov, Lp, c->Bov, Lp, c->Jovov, ov, 1, 1.0, 0)));
