@@ -233,7 +233,10 @@ def test_zgemm_nt_with_sum_planes(gpu, M, N, K, mode):
     assert _rel(C, ref) < REL_TOL
 
 
-@pytest.mark.parametrize("dims", [(3, 5, 7, 9), (34, 33, 2, 65), (1, 1, 40, 40), (8, 8, 8, 8)])
+# the later shapes walk the tile variants of transpose.cuh: one 40-, 48- or 64-row tile for 32 < ny <= 64, merged y groups
+# (two and three sub-dims) longer than one tile, ragged x, unit dims
+@pytest.mark.parametrize("dims", [(3, 5, 7, 9), (34, 33, 2, 65), (1, 1, 40, 40), (8, 8, 8, 8), (5, 7, 33, 37),
+                                  (34, 3, 70, 65), (66, 2, 2, 31), (3, 129, 5, 2), (64, 33, 9, 1), (47, 2, 41, 3)])
 def test_transpose_all_permutations(gpu, dims):
     import itertools
     import torch
