@@ -168,6 +168,9 @@ int ccsd_triples_range(ccsd_ctx* ctx, int64_t first_triple, int64_t ntriples, do
  *                         entry points are used (until the next ccsd_lambda_init or ccsd_destroy).  Synchronises.
  *   ccsd_lambda_iterate   one iteration: right-hand sides of eqs 52-56, lambda <- lambda + R/D with the CCSD
  *                         denominators, DIIS as for the amplitudes.  HOST output ||R/D||_2 over the unique multipliers.
+ *   ccsd_lambda_solve     ccsd_lambda_iterate until ||R/D||_2 < tol or max_iterations (as ccsd_solve; the multipliers have
+ *                         no energy of their own to test).  HOST outputs: iterations done, last ||R/D||_2.  Returns
+ *                         CCSD_ENOTCONVERGED if the limit was hit.
  *   ccsd_lambda_residual  evaluates the right-hand sides only (ccsd_get_lambda_residual returns them).
  *   ccsd_get/set_lambda   multipliers lambda^i_a [i][a], lambda^{ij}_{ab} [(i<j)][(a<b)] (device, asynchronous).
  *   ccsd_density          D[p][q] = <0|(1+Lambda) exp(-T) a+_p a_q exp(T)|0> - delta_pq (p occupied), [n][n] (device),
@@ -179,6 +182,7 @@ int ccsd_triples_range(ccsd_ctx* ctx, int64_t first_triple, int64_t ntriples, do
 int ccsd_lambda_workspace_bytes(ccsd_ctx* ctx, size_t* bytes);
 int ccsd_lambda_init(ccsd_ctx* ctx, void* workspace, size_t workspace_bytes);
 int ccsd_lambda_iterate(ccsd_ctx* ctx, double* step_norm);
+int ccsd_lambda_solve(ccsd_ctx* ctx, double tol, int max_iterations, int* iterations, double* step_norm);
 int ccsd_lambda_residual(ccsd_ctx* ctx);
 int ccsd_get_lambda(ccsd_ctx* ctx, ccsd_c128* l1, ccsd_c128* l2p);
 int ccsd_set_lambda(ccsd_ctx* ctx, const ccsd_c128* l1, const ccsd_c128* l2p, int reset_diis);

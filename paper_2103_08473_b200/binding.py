@@ -25,7 +25,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
-           "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
+           "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_solve", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
            "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation"]
 
 
@@ -73,6 +73,7 @@ def load_library():
         lib.ccsd_lambda_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_lambda_init.argtypes = [vp, vp, ctypes.c_size_t]
         lib.ccsd_lambda_iterate.argtypes = [vp, ctypes.POINTER(dbl)]
+        lib.ccsd_lambda_solve.argtypes = [vp, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(dbl)]
         lib.ccsd_lambda_residual.argtypes = [vp]
         lib.ccsd_get_lambda.argtypes = [vp, vp, vp]
         lib.ccsd_set_lambda.argtypes = [vp, vp, vp, ctypes.c_int]
@@ -353,6 +354,14 @@ class CCSD:
         if st not in (0, 5):
             _check(st, "ccsd_lambda_iterate")
         return sn.value
+
+    def lambda_solve(self, tol: float = 1e-9, max_iterations: int = 30):
+        """ccsd_lambda_solve -> (converged, iterations, ||R/D||_2)."""
+        it, sn = ctypes.c_int(), ctypes.c_double()
+        st = self._lib.ccsd_lambda_solve(self._ctx, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(sn))
+        if st not in (0, 6):
+            _check(st, "ccsd_lambda_solve")
+        return st == 0, it.value, sn.value
 
     def lambda_residual(self):
         torch = self._torch

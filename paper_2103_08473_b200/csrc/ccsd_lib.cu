@@ -1772,6 +1772,24 @@ int ccsd_lambda_iterate(ccsd_ctx* c, double* step_norm)
     return lambda_iterate(c, c->lam, step_norm);
 }
 
+int ccsd_lambda_solve(ccsd_ctx* c, double tol, int max_iterations, int* iterations, double* step_norm)
+{
+    if (!c || !c->lam) return CCSD_ESTATE;
+    if (!(tol > 0.0) || max_iterations < 1) return CCSD_EINVAL;
+    int it = 0;
+    double sn = 0.0;
+    bool converged = false;
+    while (it < max_iterations && !converged) {
+        const int status = ccsd_lambda_iterate(c, &sn);
+        if (status != CCSD_OK && status != CCSD_ESINGULAR) return status;
+        it++;
+        converged = sn < tol;
+    }
+    if (iterations) *iterations = it;
+    if (step_norm) *step_norm = sn;
+    return converged ? CCSD_OK : CCSD_ENOTCONVERGED;
+}
+
 int ccsd_lambda_residual(ccsd_ctx* c)
 {
     if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;

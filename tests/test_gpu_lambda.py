@@ -253,3 +253,30 @@ def test_lambda_in_ccd_mode_keeps_singles_multipliers_zero(gpu):
     assert float(l1.abs().max()) == 0.0
     assert _rel(l2p.cpu().numpy(), pack_t2(ol.l2)) <= 1e-11
     gc.close()
+
+
+def test_lambda_solve_converges_like_the_oracle_loop(gpu):
+    """ccsd_lambda_solve: the same number of iterations to ||R/D||_2 < tol as the oracle's loop with the same test, the
+    same converged multipliers and density; the iteration limit reports CCSD_ENOTCONVERGED (binding: converged False)."""
+    from oracle.ccsd_oracle import pack_t2
+    from paper_2103_08473_b200.binding import CCSDError
+    inp, oc, ol, gc = _pair(gpu, "ragged")
+    with pytest.raises(CCSDError):
+        gc.lambda_solve(1e-10, 50)                       # before ccsd_lambda_init
+    gc.lambda_init()
+    tol, it_o = 1e-10, 0
+    while it_o < 60:
+        it_o += 1
+        if ol.iterate() < tol:
+            break
+    ok, it_g, sn = gc.lambda_solve(tol, 60)
+    assert ok and it_g == it_o and sn < tol
+    l1, l2p = gc.get_lambda()
+    assert _rel(l1.cpu().numpy(), ol.l1) <= 1e-9 and _rel(l2p.cpu().numpy(), pack_t2(ol.l2)) <= 1e-9
+    assert _rel(gc.density().cpu().numpy(), ol.density()) <= 1e-9
+    gc.lambda_init()
+    ok, it_g, sn = gc.lambda_solve(1e-14, 2)
+    assert not ok and it_g == 2 and sn > 1e-14
+    with pytest.raises(CCSDError):
+        gc.lambda_solve(0.0, 5)
+    gc.close()
