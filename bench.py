@@ -430,8 +430,13 @@ def run_ours(args) -> None:
         print(json.dumps({"metric": "pp_ladder_tflops", "value": 8.0 * oo * vv * vv / (t * 1e-3) * 1e-12, "unit": "TFLOP/s",
                           "ms_per_launch": t, "config": {"workload": f"{cfg} pp-ladder {vv}x{oo}x{vv}"}}))
         return
-    inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
     pkg.load_library()
+    if args.only_transposes:
+        # profiling aid: the transposes leg alone (o^2 v^2-shaped tensor of --config)
+        print(json.dumps({"metric": "transpose_gbs", "unit": "GB/s", "config": {"workload": f"{cfg} o^2 v^2 complex128"},
+                          "hbm_peak": measured_peaks(), "transposes": transpose_bench(torch, pkg, measured_peaks()["hbm_gbs"], o, v)}))
+        return
+    inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
     if args.only_lambda:
         print(json.dumps({"metric": "lambda_seconds_per_iteration", "unit": "s", "config": {"workload": f"{cfg} Lambda"},
                           **lambda_bench(torch, pkg, inp, o, v)}))
@@ -606,6 +611,7 @@ def main():
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")
     ap.add_argument("--only-triples", action="store_true", help="time only the perturbative triples of --config")
+    ap.add_argument("--only-transposes", action="store_true", help="time only the 4-index transpositions")
     ap.add_argument("--only-cc2", action="store_true", help="time only the CC2 iteration of --config")
     ap.add_argument("--only-direct", action="store_true", help="time only the CCSD iteration with the integral-direct pp-ladder")
     args = ap.parse_args()
