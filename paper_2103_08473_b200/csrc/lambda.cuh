@@ -90,11 +90,14 @@ struct LambdaState {
     c128 *Fov, *Foo, *Fvv;                         // [m][e], [m][i], [a][e]
     c128 *Wvovv, *Wooov, *Wovvo, *Wovoo, *Wvvvo;   // [a][m][e][f], [m][n][i][e], [m][b][e][j], [m][b][i][j], [a][b][e][i]
     c128 *inner, *X3, *Ypk;                        // build temporaries
-    c128 *Wvovv_iaef, *Wvovv_jabe, *Wvvvo_amef;    // the o v^3 elements in the operand layouts of the iteration (no per-iteration permute)
+    c128 *Wvovv_iaef, *Wvvvo_amef;                 // o v^3 elements in the operand layout of the iteration / of the build
+    c128 *Wjp, *Wq;                                // W^{ej}_{ab} as [j][(a<b)][e] and W^{ef}_{am} as [a][m][(e<f)]: the packed pair halves the product
+    c128 *FvvT, *OOVVhu;                           // Fbar^e_b as [b][e]; <ij||ae> as [(i<j)][a][e]
     // multipliers, residuals, per-iteration temporaries
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
     // packed (i<j, a<b) route of the terms whose output is antisymmetric and whose contraction runs over a packable pair
     c128 *Pacc, *l2pT, *LTp, *L2hu, *Ltp, *Amc, *TAUp, *VoovvT, *VT2;
+    c128 *T2huT, *T2ou;                            // t2 as [e][(m<n)][f] and [m][n][(e<f)]: eqs 50-51 over the packed pair
     double *VT2s, *Ltps;                           // sum planes of the (vv x oo x ov) product's operands
     double* cl2s;                                  // 3M sum plane of conj(l2p)
     // DIIS (as for the amplitudes: reading G13)
@@ -123,7 +126,9 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Wvovv = w.take<c128>(ov3); L->Wooov = w.take<c128>(o3v); L->Wovvo = w.take<c128>(o2v2);
     L->Wovoo = w.take<c128>(o3v);
     L->Wvvvo = L->Wvovv;   // build order: W^{am}_{ef} is re-laid-out and dead before W^{ab}_{ei} is assembled in the same buffer
-    L->Wvovv_iaef = w.take<c128>(ov3); L->Wvovv_jabe = w.take<c128>(ov3);
+    L->Wvovv_iaef = w.take<c128>(ov3);
+    L->Wjp = w.take<c128>(o * vv * v); L->Wq = w.take<c128>(v * o * vv);
+    L->FvvT = w.take<c128>(v * v); L->OOVVhu = w.take<c128>(oo * v * v);
     L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v);
     L->Wvvvo_amef = L->X3;   // the build temporary is free when the finished W^{ab}_{ei} is re-laid-out into it
     L->Ypk = w.take<c128>(vv * v * o);
@@ -136,6 +141,7 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Pacc = w.take<c128>(oo * vv); L->l2pT = w.take<c128>(vv * oo); L->LTp = w.take<c128>(oo * oo);
     L->L2hu = w.take<c128>(oo * v * v); L->Ltp = w.take<c128>(oo * ov); L->Amc = w.take<c128>(oo * oo);
     L->TAUp = w.take<c128>(oo * vv); L->VoovvT = w.take<c128>(vv * oo); L->VT2 = w.take<c128>(vv * ov);
+    L->T2huT = w.take<c128>(v * oo * v); L->T2ou = w.take<c128>(o * o * vv);
     L->VT2s = c->planes ? w.take<double>(vv * ov) : nullptr;
     L->Ltps = c->planes ? w.take<double>(oo * ov) : nullptr;
     L->nd = c->opt.ndiis;
@@ -188,6 +194,14 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     unpack_pairs(st, L->OOVV, c->Voovv_p, o, 1, v, 1);
     unpack_pairs(st, L->OOOV, c->Vooov_p, o, 1, 0, 0, O * V);
     unpack_pairs(st, L->WOOOO, c->Am, o, 1, o, 1);             // eq 45 = eq 31
+    {   // t2 in the two half-packed operand layouts of eqs 50-51
+        const c128* t2p = c->t2p;
+        const int64_t oo = c->oo;
+        launch_fill(st, L->T2huT, V, oo * V, oo * V, 0, [=] __device__(int64_t e, int64_t col) {
+            return asym_col(t2p, col / v, vv, (int)e, (int)(col % v), v);
+        });
+        unpack_pairs(st, L->T2ou, c->t2p, o, 1, 0, 0, vv);
+    }
     // Fbar^m_e = H^k_c (eq 28), Fbar^a_e = G^a_c (eq 57 = eq 25), Fbar^m_i = -G^k_i (eq 27)
     dcopy(st, L->Fov, c->Hov, O * V);
     dcopy(st, L->Fvv, c->Gvv, V * V);
@@ -198,7 +212,19 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     CCSD_TRY(tc1(env, sc, -1.0, LV(T1, "na", O, V), LV(L->OOVV, "nmef", O, O, V, V), L->Wvovv, "amef"));
     //   ... kept only in the two [free][contracted] layouts the iteration contracts it in
     CCSD_TRY(permute_into(st, L->Wvovv_iaef, "iaef", LV(L->Wvovv, "eifa", V, O, V, V), 1.0, 0));
-    CCSD_TRY(permute_into(st, L->Wvovv_jabe, "jabe", LV(L->Wvovv, "ejab", V, O, V, V), 1.0, 0));
+    {   // [j][(a<b)][e] = W^{ej}_{ab} (antisymmetric in ab); Fbar^e_b transposed; <ij||ae> with the occupied pair packed
+        const c128 *Wv = L->Wvovv, *Voovv = c->Voovv_p;
+        const int2* pv = c->pv;
+        launch_fill(st, L->Wjp, O * vv, V, V, 0, [=] __device__(int64_t row, int64_t e) {
+            const int64_t j = row / vv;
+            const int2 ab = pv[row % vv];
+            return Wv[((e * o + j) * v + ab.x) * v + ab.y];
+        });
+        CCSD_TRY(permute_into(st, L->FvvT, "be", LV(L->Fvv, "eb", V, V), 1.0, 0));
+        launch_fill(st, L->OOVVhu, c->oo * V, V, V, 0, [=] __device__(int64_t row, int64_t e) {
+            return asym_col(Voovv, row / v, vv, (int)(row % v), (int)e, v);
+        });
+    }
     // W^{mn}_{ie} = <mn||ie> + t^f_i <mn||fe>
     dcopy(st, L->Wooov, L->OOOV, O * O * O * V);
     CCSD_TRY(tc1(env, sc, 1.0, LV(T1, "if", O, V), LV(L->OOVV, "mnfe", O, O, V, V), L->Wooov, "mnie"));
@@ -258,6 +284,14 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     }
     // W^{ab}_{ei} in the [free][contracted] layout the iteration contracts it in (into the build temporary, now free)
     CCSD_TRY(permute_into(st, L->Wvvvo_amef, "amef", LV(L->Wvvvo, "efam", V, V, V, O), 1.0, 0));
+    {   // ... and packed in its antisymmetric pair: [a][m][(e<f)]
+        const c128* Wam = L->Wvvvo_amef;
+        const int2* pv = c->pv;
+        launch_fill(st, L->Wq, V * O, vv, vv, 0, [=] __device__(int64_t am, int64_t EF) {
+            const int2 ef = pv[EF];
+            return Wam[(am * v + ef.x) * v + ef.y];
+        });
+    }
     // packed operands of the iteration: A^{kl}_{ij} and tau as they are now, <mn||ab> and <em||ab> with the (a<b) pair as row
     dcopy(st, L->Amc, c->Am, c->oo * c->oo);
     dcopy(st, L->TAUp, c->taup, c->oo * vv);
@@ -277,29 +311,33 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     const int o = c->o, v = c->v;
     const int64_t O = o, V = v, oo = c->oo, vv = c->vv;
     unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
-    // eqs 50-51
-    CCSD_CUDA_TRY(cudaMemsetAsync(L->Gvv, 0, (size_t)(V * V) * sizeof(c128), st));
-    CCSD_CUDA_TRY(cudaMemsetAsync(L->Goo, 0, (size_t)(O * O) * sizeof(c128), st));
-    CCSD_TRY(tc1(env, sc, -0.5, LV(L->T2, "mnef", O, O, V, V), LV(L->L2, "mnaf", O, O, V, V), L->Gvv, "ae"));
-    CCSD_TRY(tc1(env, sc, 0.5, LV(L->T2, "mnef", O, O, V, V), LV(L->L2, "inef", O, O, V, V), L->Goo, "mi"));
-    // eqs 55-56
-    dcopy(st, L->R1, L->Fov, O * V);
+    // eqs 50-51 over the packed pair of each product (both factors are antisymmetric in it, so the full sum is twice the
+    // packed one):  G^a_e = -1/2 sum_{mnf} t^{ef}_{mn} lambda^{mn}_{af} = -sum_{m<n,f};  G^m_i = 1/2 sum_{nef} t^{ef}_{mn}
+    // lambda^{in}_{ef} = sum_{n,e<f}.  The lambda operands go to the contraction scratch, the t operands were laid out once.
+    {
+        const c128* l2p = L->l2p;
+        launch_fill(st, sc.a, V, oo * V, oo * V, 0, [=] __device__(int64_t a, int64_t col) {   // [a][(m<n)][f]
+            return asym_col(l2p, col / v, vv, (int)a, (int)(col % v), v);
+        });
+        CCSD_TRY(run_gemm(env, gp(V, V, oo * V, sc.a, oo * V, L->T2huT, oo * V, L->Gvv, V, 1, -1.0, 0)));
+        unpack_pairs(st, sc.b, L->l2p, o, 1, 0, 0, vv);                                        // [i][n][(e<f)]
+        CCSD_TRY(run_gemm(env, gp(O, O, O * vv, L->T2ou, O * vv, sc.b, O * vv, L->Goo, O, 1, 1.0, 0)));
+        // eqs 55-56 start here, while [i][m][(e<f)] is in the scratch: 1/2 sum_{mef} lambda^{im}_{ef} W^{ef}_{am} = sum_{m,e<f}
+        dcopy(st, L->R1, L->Fov, O * V);
+        CCSD_TRY(run_gemm(env, gp(V, O, O * vv, L->Wq, O * vv, sc.b, O * vv, L->R1, 1, V, 1.0, 1)));
+    }
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Fvv, "ea", V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Foo, "im", O, O), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->Goo, "mn", O, O), LV(L->Wooov, "mina", O, O, O, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->Gvv, "ef", V, V), LV(L->Wvovv_iaef, "iaef", O, V, V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->Wovvo, "ieam", O, V, V, O), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -0.5, LV(L->L2, "mnae", O, O, V, V), LV(L->Wovoo, "iemn", O, V, O, O), L->R1, "ia"));
-    CCSD_TRY(tc1(env, sc, 0.5, LV(L->L2, "imef", O, O, V, V), LV(L->Wvvvo_amef, "amef", V, O, V, V), L->R1, "ia"));
     // eqs 52-54, unpacked [i][j][a][b]
     dcopy(st, L->R2, L->OOVV, O * O * V * V);
-    CCSD_TRY(tc2(env, sc, 1.0, LV(L->L2, "ijae", O, O, V, V), LV(L->Fvv, "eb", V, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->L2, "imab", O, O, V, V), LV(L->Foo, "jm", O, O), L->R2, "ijab", "jiab"));
     CCSD_TRY(tc4(env, sc, 1.0, LV(L->L2, "imae", O, O, V, V), LV(L->Wovvo, "jebm", O, V, V, O), L->R2, "ijab", "jiab", "ijba", "jiba"));
-    CCSD_TRY(tc2(env, sc, 1.0, LV(L->OOVV, "ijae", O, O, V, V), LV(L->Gvv, "be", V, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc2(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Wvovv_jabe, "jabe", O, V, V, V), L->R2, "ijab", "jiab"));
     CCSD_TRY(tc4(env, sc, 1.0, LV(L->l1, "ia", O, V), LV(L->Fov, "jb", O, V), L->R2, "ijab", "jiab", "ijba", "jiba"));
     // The terms with an antisymmetric (i<j, a<b) output and a pair-wise contraction run packed, into Pacc[(i<j)][(a<b)]:
     //   sum_{m<n} lambda^{mn}_{ab} W^{ij}_{mn}   (W^{ij}_{mn} = A^{kl}_{ij} of eq 31, packed in both pairs)
@@ -318,6 +356,21 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, L->T1, V, L->Ltp, O, 1, 1.0, 0)));
         if (L->Ltps) launch_sum_plane(st, L->Ltp, L->Ltps, oo * c->ov);
         CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1), L->VT2s, L->Ltps)));
+    }
+    // P-_ab sum_e ( lambda^{ij}_{ae} Fbar^e_b + <ij||ae> G^b_e ) and P-_ij sum_e lambda^i_e W^{ej}_{ab}: the products run over the
+    // packed output pair ((i<j) rows, resp. (a<b) rows), the P- of the other pair is applied when they are added into Pacc
+    {
+        c128 *Y = sc.c, *Z = sc.a;                       // Y[(i<j)][a][b], Z[j][(a<b)][i]
+        CCSD_TRY(run_gemm(env, gp(oo * V, V, V, L->L2hu, V, L->FvvT, V, Y, V, 1, 1.0, 0)));
+        CCSD_TRY(run_gemm(env, gp(oo * V, V, V, L->OOVVhu, V, L->Gvv, V, Y, V, 1, 1.0, 1)));
+        CCSD_TRY(run_gemm(env, gp(O * vv, O, V, L->Wjp, V, L->l1, V, Z, O, 1, 1.0, 0)));
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(st, L->Pacc, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            const c128 y = csub(Y[(IJ * v + ab.x) * v + ab.y], Y[(IJ * v + ab.y) * v + ab.x]);
+            const c128 z = csub(Z[((int64_t)ij.y * vv + AB) * o + ij.x], Z[((int64_t)ij.x * vv + AB) * o + ij.y]);
+            return cadd(y, z);
+        });
     }
     //   (i) sum_{e<f} lambda^{ij}_{ef} <ef||ab> = conj( sum_{e<f} conj(lambda) <ab||ef> ): the pp-ladder launch of the CCSD
     //       iteration (packed, Hermitian <ab||cd>, 3M with sum planes) on the conjugated multipliers
