@@ -371,7 +371,7 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
     return {"s_per_iteration": round(statistics.median(ts) * 1e-3, 5), "hbar_build_s": round(init_ms * 1e-3, 4),
             "steps": steps, "warmup": warmup, "step_norm_last": sn, "density_trace_abs": abs(tr),
             "workspace_gib": round(ws / 2 ** 30, 1),
-            "note": "first CUDA path: one permute + DMMA GEMM + signed permuted add per term; pp-ladder term on the packed "
+            "note": "one permute + DMMA GEMM + signed permuted add per small term, packed-pair routes for the o^2 v^3 products; pp-ladder term on the packed "
                     "<ab||cd> with conjugated multipliers"}
 
 
