@@ -93,6 +93,8 @@ struct LambdaState {
     c128 *Wvovv_iaef, *Wvvvo_amef;                 // o v^3 elements in the operand layout of the iteration / of the build
     c128 *Wjp, *Wq;                                // W^{ej}_{ab} as [j][(a<b)][e] and W^{ef}_{am} as [a][m][(e<f)]: the packed pair halves the product
     c128 *FvvT, *OOVVhu;                           // Fbar^e_b as [b][e]; <ij||ae> as [(i<j)][a][e]
+    c128* Wr;                                      // W^{je}_{bm} as [(j,b)][(m,e)]: operand of the ring-like term
+    double* Wrs;                                   // ... and its 3M sum plane
     // multipliers, residuals, per-iteration temporaries
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
     // packed (i<j, a<b) route of the terms whose output is antisymmetric and whose contraction runs over a packable pair
@@ -129,6 +131,8 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Wvovv_iaef = w.take<c128>(ov3);
     L->Wjp = w.take<c128>(o * vv * v); L->Wq = w.take<c128>(v * o * vv);
     L->FvvT = w.take<c128>(v * v); L->OOVVhu = w.take<c128>(oo * v * v);
+    L->Wr = w.take<c128>(o2v2);
+    L->Wrs = c->planes ? w.take<double>(o2v2) : nullptr;
     L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v);
     L->Wvvvo_amef = L->X3;   // the build temporary is free when the finished W^{ab}_{ei} is re-laid-out into it
     L->Ypk = w.take<c128>(vv * v * o);
@@ -284,6 +288,9 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     }
     // W^{ab}_{ei} in the [free][contracted] layout the iteration contracts it in (into the build temporary, now free)
     CCSD_TRY(permute_into(st, L->Wvvvo_amef, "amef", LV(L->Wvvvo, "efam", V, V, V, O), 1.0, 0));
+    // W^{je}_{bm} (finished above) in the [free][contracted] layout of the ring-like term, with its sum plane
+    CCSD_TRY(permute_into(st, L->Wr, "jbme", LV(L->Wovvo, "jebm", O, V, V, O), 1.0, 0));
+    if (L->Wrs) launch_sum_plane(st, L->Wr, L->Wrs, O * V * O * V);
     {   // ... and packed in its antisymmetric pair: [a][m][(e<f)]
         const c128* Wam = L->Wvvvo_amef;
         const int2* pv = c->pv;
@@ -335,10 +342,8 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     // eqs 52-54, unpacked [i][j][a][b]
     dcopy(st, L->R2, L->OOVV, O * O * V * V);
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->L2, "imab", O, O, V, V), LV(L->Foo, "jm", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc4(env, sc, 1.0, LV(L->L2, "imae", O, O, V, V), LV(L->Wovvo, "jebm", O, V, V, O), L->R2, "ijab", "jiab", "ijba", "jiba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
     CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc4(env, sc, 1.0, LV(L->l1, "ia", O, V), LV(L->Fov, "jb", O, V), L->R2, "ijab", "jiab", "ijba", "jiba"));
     // The terms with an antisymmetric (i<j, a<b) output and a pair-wise contraction run packed, into Pacc[(i<j)][(a<b)]:
     //   sum_{m<n} lambda^{mn}_{ab} W^{ij}_{mn}   (W^{ij}_{mn} = A^{kl}_{ij} of eq 31, packed in both pairs)
     CCSD_TRY(launch_transpose2d(st, L->l2p, L->l2pT, oo, vv, 0));
@@ -356,6 +361,35 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         CCSD_TRY(run_gemm(env, gp(oo * V, O, V, L->L2hu, V, L->T1, V, L->Ltp, O, 1, 1.0, 0)));
         if (L->Ltps) launch_sum_plane(st, L->Ltp, L->Ltps, oo * c->ov);
         CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, c->ov, L->VT2, c->ov, L->Ltp, c->ov, L->Pacc, 1, vv, -1.0, 1), L->VT2s, L->Ltps)));
+    }
+    // P-_ij P-_ab ( sum_{me} lambda^{im}_{ae} W^{je}_{bm} + lambda^i_a Fbar^j_b ): the (ov)^3 GEMM as the ring of the CCSD iteration
+    // runs it (operand laid out from the packed multipliers with its sum plane, the constant operand and plane laid out
+    // once), both P- applied when the result is added into Pacc
+    {
+        const c128 *l2p = L->l2p, *l1 = L->l1, *Fov = L->Fov;
+        const int64_t ov = c->ov;
+        c128 *L2r = sc.a, *X = sc.c;
+        double* L2rs = L->Wrs ? sc.as : nullptr;
+        launch_fill(st, L2r, ov, ov, ov, 0, [=] __device__(int64_t ia, int64_t me) {      // [(i,a)][(m,e)] = lambda^{im}_{ae}
+            const c128 x = t2_at(l2p, (int)(ia / v), (int)(me / v), (int)(ia % v), (int)(me % v), o, v, vv);
+            if (L2rs) L2rs[ia * ov + me] = x.x + x.y;
+            return x;
+        });
+        CCSD_TRY(run_gemm(env, with_planes(gp(ov, ov, ov, L2r, ov, L->Wr, ov, X, ov, 1, 1.0, 0), L2rs, L->Wrs)));
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(st, L->Pacc, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            const int64_t i = ij.x, j = ij.y, a = ab.x, b = ab.y;
+            c128 r = X[((i * v + a) * o + j) * v + b];
+            r = csub(r, X[((j * v + a) * o + i) * v + b]);
+            r = csub(r, X[((i * v + b) * o + j) * v + a]);
+            r = cadd(r, X[((j * v + b) * o + i) * v + a]);
+            cfma(r, l1[i * v + a], Fov[j * v + b]);
+            cfma(r, cneg(l1[j * v + a]), Fov[i * v + b]);
+            cfma(r, cneg(l1[i * v + b]), Fov[j * v + a]);
+            cfma(r, l1[j * v + b], Fov[i * v + a]);
+            return r;
+        });
     }
     // P-_ab sum_e ( lambda^{ij}_{ae} Fbar^e_b + <ij||ae> G^b_e ) and P-_ij sum_e lambda^i_e W^{ej}_{ab}: the products run over the
     // packed output pair ((i<j) rows, resp. (a<b) rows), the P- of the other pair is applied when they are added into Pacc
