@@ -94,6 +94,7 @@ struct LambdaState {
     c128 *Wjp, *Wq;                                // W^{ej}_{ab} as [j][(a<b)][e] and W^{ef}_{am} as [a][m][(e<f)]: the packed pair halves the product
     c128 *FvvT, *OOVVhu;                           // Fbar^e_b as [b][e]; <ij||ae> as [(i<j)][a][e]
     c128* Wr;                                      // W^{je}_{bm} as [(j,b)][(m,e)]: operand of the ring-like term
+    c128 *Wovoo_r, *OOVVr, *Wooov_r, *GooT, *l1T;  // W^{ie}_{mn} as [i][(m<n)][e]; <im||ab> as [(a<b)][i][m]; W^{ij}_{mb} as [(i<j)][b][m]; transposes
     double* Wrs;                                   // ... and its 3M sum plane
     // multipliers, residuals, per-iteration temporaries
     c128 *l1, *l2p, *L2, *R1, *R2, *R2p, *Gvv, *Goo, *Lt, *LT, *cl2p, *P2;
@@ -132,6 +133,8 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->Wjp = w.take<c128>(o * vv * v); L->Wq = w.take<c128>(v * o * vv);
     L->FvvT = w.take<c128>(v * v); L->OOVVhu = w.take<c128>(oo * v * v);
     L->Wr = w.take<c128>(o2v2);
+    L->Wovoo_r = w.take<c128>(o * oo * v); L->OOVVr = w.take<c128>(vv * o * o); L->Wooov_r = w.take<c128>(oo * v * o);
+    L->GooT = w.take<c128>(o * o); L->l1T = w.take<c128>(ov);
     L->Wrs = c->planes ? w.take<double>(o2v2) : nullptr;
     L->inner = w.take<c128>(o2v2); L->X3 = w.take<c128>(ov3 > o3v ? ov3 : o3v);
     L->Wvvvo_amef = L->X3;   // the build temporary is free when the finished W^{ab}_{ei} is re-laid-out into it
@@ -288,6 +291,24 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     }
     // W^{ab}_{ei} in the [free][contracted] layout the iteration contracts it in (into the build temporary, now free)
     CCSD_TRY(permute_into(st, L->Wvvvo_amef, "amef", LV(L->Wvvvo, "efam", V, V, V, O), 1.0, 0));
+    {   // operands of the o^3 v^2-class terms with the pair they leave alone packed: W^{ie}_{mn}, <im||ab>, W^{ij}_{mb}
+        const c128 *Wovoo = L->Wovoo, *Voovv = c->Voovv_p, *Wooov = L->Wooov;
+        const int2 *po = c->po;
+        const int64_t oo = c->oo;
+        launch_fill(st, L->Wovoo_r, O, oo * V, oo * V, 0, [=] __device__(int64_t i, int64_t col) {   // [i][(m<n)][e] = W[i][e][m][n]
+            const int2 mn = po[col / v];
+            return Wovoo[((i * v + col % v) * o + mn.x) * o + mn.y];
+        });
+        launch_fill(st, L->OOVVr, vv, O * O, O * O, 0, [=] __device__(int64_t AB, int64_t im) {      // [(a<b)][i][m] = <im||ab>
+            const int i = (int)(im / o), m = (int)(im % o);
+            if (i == m) return mk(0.0, 0.0);
+            return i < m ? Voovv[pair_idx(i, m, o) * vv + AB] : cneg(Voovv[pair_idx(m, i, o) * vv + AB]);
+        });
+        launch_fill(st, L->Wooov_r, oo * V, O, O, 0, [=] __device__(int64_t row, int64_t m) {        // [(i<j)][b][m] = W[i][j][m][b]
+            const int2 ij = po[row / v];
+            return Wooov[(((int64_t)ij.x * o + ij.y) * o + m) * v + row % v];
+        });
+    }
     // W^{je}_{bm} (finished above) in the [free][contracted] layout of the ring-like term, with its sum plane
     CCSD_TRY(permute_into(st, L->Wr, "jbme", LV(L->Wovvo, "jebm", O, V, V, O), 1.0, 0));
     if (L->Wrs) launch_sum_plane(st, L->Wr, L->Wrs, O * V * O * V);
@@ -317,7 +338,6 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
     const TcScratch& sc = L->sc;
     const int o = c->o, v = c->v;
     const int64_t O = o, V = v, oo = c->oo, vv = c->vv;
-    unpack_pairs(st, L->L2, L->l2p, o, 1, v, 1);
     // eqs 50-51 over the packed pair of each product (both factors are antisymmetric in it, so the full sum is twice the
     // packed one):  G^a_e = -1/2 sum_{mnf} t^{ef}_{mn} lambda^{mn}_{af} = -sum_{m<n,f};  G^m_i = 1/2 sum_{nef} t^{ef}_{mn}
     // lambda^{in}_{ef} = sum_{n,e<f}.  The lambda operands go to the contraction scratch, the t operands were laid out once.
@@ -332,18 +352,15 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         // eqs 55-56 start here, while [i][m][(e<f)] is in the scratch: 1/2 sum_{mef} lambda^{im}_{ef} W^{ef}_{am} = sum_{m,e<f}
         dcopy(st, L->R1, L->Fov, O * V);
         CCSD_TRY(run_gemm(env, gp(V, O, O * vv, L->Wq, O * vv, sc.b, O * vv, L->R1, 1, V, 1.0, 1)));
+        // ... and -1/2 sum_{mne} lambda^{mn}_{ae} W^{ie}_{mn} = -sum_{m<n,e}, with [a][(m<n)][e] still in the scratch
+        CCSD_TRY(run_gemm(env, gp(V, O, oo * V, sc.a, oo * V, L->Wovoo_r, oo * V, L->R1, 1, V, -1.0, 1)));
     }
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "ie", O, V), LV(L->Fvv, "ea", V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Foo, "im", O, O), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->Goo, "mn", O, O), LV(L->Wooov, "mina", O, O, O, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, -1.0, LV(L->Gvv, "ef", V, V), LV(L->Wvovv_iaef, "iaef", O, V, V, V), L->R1, "ia"));
     CCSD_TRY(tc1(env, sc, 1.0, LV(L->l1, "me", O, V), LV(L->Wovvo, "ieam", O, V, V, O), L->R1, "ia"));
-    CCSD_TRY(tc1(env, sc, -0.5, LV(L->L2, "mnae", O, O, V, V), LV(L->Wovoo, "iemn", O, V, O, O), L->R1, "ia"));
-    // eqs 52-54, unpacked [i][j][a][b]
-    dcopy(st, L->R2, L->OOVV, O * O * V * V);
-    CCSD_TRY(tc2(env, sc, -1.0, LV(L->L2, "imab", O, O, V, V), LV(L->Foo, "jm", O, O), L->R2, "ijab", "jiab"));
-    CCSD_TRY(tc2(env, sc, -1.0, LV(L->l1, "ma", O, V), LV(L->Wooov, "ijmb", O, O, O, V), L->R2, "ijab", "ijba"));
-    CCSD_TRY(tc2(env, sc, -1.0, LV(L->OOVV, "imab", O, O, V, V), LV(L->Goo, "mj", O, O), L->R2, "ijab", "jiab"));
+    // eqs 52-54: every term goes into the packed accumulator Pacc[(i<j)][(a<b)] (the driver <ij||ab> is added by the final fill).
     // The terms with an antisymmetric (i<j, a<b) output and a pair-wise contraction run packed, into Pacc[(i<j)][(a<b)]:
     //   sum_{m<n} lambda^{mn}_{ab} W^{ij}_{mn}   (W^{ij}_{mn} = A^{kl}_{ij} of eq 31, packed in both pairs)
     CCSD_TRY(launch_transpose2d(st, L->l2p, L->l2pT, oo, vv, 0));
@@ -391,6 +408,28 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             return r;
         });
     }
+    // -P-_ij sum_m ( lambda^{im}_{ab} Fbar^j_m + <im||ab> G^m_j ) on (a<b) rows and -P-_ab sum_m lambda^m_a W^{ij}_{mb} on (i<j) rows
+    {
+        const c128 *l2pT = L->l2pT;
+        c128 *L2r2 = sc.b, *U = sc.a, *Vb = sc.c;        // [(a<b)][i][m], U[(a<b)][i][j], Vb[(i<j)][b][a]
+        launch_fill(st, L2r2, vv, O * O, O * O, 0, [=] __device__(int64_t AB, int64_t im) {
+            const int i = (int)(im / o), m = (int)(im % o);
+            if (i == m) return mk(0.0, 0.0);
+            return i < m ? l2pT[AB * oo + pair_idx(i, m, o)] : cneg(l2pT[AB * oo + pair_idx(m, i, o)]);
+        });
+        CCSD_TRY(permute_into(st, L->GooT, "jm", LV(L->Goo, "mj", O, O), 1.0, 0));
+        CCSD_TRY(permute_into(st, L->l1T, "am", LV(L->l1, "ma", O, V), 1.0, 0));
+        CCSD_TRY(run_gemm(env, gp(vv * O, O, O, L2r2, O, L->Foo, O, U, O, 1, 1.0, 0)));
+        CCSD_TRY(run_gemm(env, gp(vv * O, O, O, L->OOVVr, O, L->GooT, O, U, O, 1, 1.0, 1)));
+        CCSD_TRY(run_gemm(env, gp(oo * V, V, O, L->Wooov_r, O, L->l1T, O, Vb, V, 1, 1.0, 0)));
+        const int2 *po = c->po, *pv = c->pv;
+        launch_fill(st, L->Pacc, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            const c128 u = csub(U[(AB * o + ij.y) * o + ij.x], U[(AB * o + ij.x) * o + ij.y]);
+            const c128 w = csub(Vb[(IJ * v + ab.x) * v + ab.y], Vb[(IJ * v + ab.y) * v + ab.x]);
+            return cadd(u, w);
+        });
+    }
     // P-_ab sum_e ( lambda^{ij}_{ae} Fbar^e_b + <ij||ae> G^b_e ) and P-_ij sum_e lambda^i_e W^{ej}_{ab}: the products run over the
     // packed output pair ((i<j) rows, resp. (a<b) rows), the P- of the other pair is applied when they are added into Pacc
     {
@@ -418,12 +457,10 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
         });
         CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
     }
-    {   // pack: R2p[(i<j)][(a<b)] = R2[i][j][a][b] + conj(P2) + Pacc
-        const c128 *R2 = L->R2, *P2 = L->P2, *Pacc = L->Pacc;
-        const int2 *po = c->po, *pv = c->pv;
+    {   // R2p[(i<j)][(a<b)] = <ij||ab> + conj(P2) + Pacc
+        const c128 *Voovv = c->Voovv_p, *P2 = L->P2, *Pacc = L->Pacc;
         launch_fill(st, L->R2p, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
-            const int2 ij = po[IJ], ab = pv[AB];
-            return cadd(cadd(R2[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(P2[IJ * vv + AB])), Pacc[IJ * vv + AB]);
+            return cadd(cadd(Voovv[IJ * vv + AB], cconj(P2[IJ * vv + AB])), Pacc[IJ * vv + AB]);
         });
     }
     CCSD_CUDA_TRY(cudaGetLastError());
