@@ -144,6 +144,16 @@ def _check(status: int, where: str):
         raise CCSDError(status, where)
 
 
+def _workspace(torch, nbytes: int):
+    """A device workspace of nbytes (+ alignment slack).  The workspaces are tens of GB: when torch's caching allocator
+    holds freed blocks that are too small to serve the request, hand them back to the driver once and retry."""
+    try:
+        return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device="cuda")
+    except torch.OutOfMemoryError:
+        torch.cuda.empty_cache()
+        return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device="cuda")
+
+
 def _torch():
     import torch
     if not torch.cuda.is_available():
@@ -209,7 +219,7 @@ class CCSD:
         _check(lib.ccsd_workspace_bytes(self.nocc, self.nvir, self.naux, ctypes.byref(self._opts),
                                         ctypes.byref(nbytes)), "ccsd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)
-        self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device="cuda")
+        self._ws = _workspace(torch, self.workspace_bytes)
         base = (self._ws.data_ptr() + 255) // 256 * 256
         self._ctx = ctypes.c_void_p(None)
         _check(lib.ccsd_init(ctypes.byref(self._ctx), h_d.data_ptr(), B_d.data_ptr(), self.nocc, self.nvir, self.naux,
@@ -286,7 +296,7 @@ class CCSD:
         torch = self._torch
         nbytes = ctypes.c_size_t(0)
         _check(self._lib.ccsd_triples_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_triples_workspace_bytes")
-        ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")
+        ws = _workspace(torch, nbytes.value)
         return ws, (ws.data_ptr() + 255) // 256 * 256, int(nbytes.value)
 
     def triples(self) -> dict:
@@ -344,7 +354,8 @@ class CCSD:
         torch = self._torch
         nbytes = ctypes.c_size_t(0)
         _check(self._lib.ccsd_lambda_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_lambda_workspace_bytes")
-        self._lam_ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")   # lives with the solver
+        self._lam_ws = None                                # a previous Lambda workspace is released first
+        self._lam_ws = _workspace(torch, nbytes.value)    # lives with the solver
         base = (self._lam_ws.data_ptr() + 255) // 256 * 256
         _check(self._lib.ccsd_lambda_init(self._ctx, base, int(nbytes.value)), "ccsd_lambda_init")
 
@@ -432,7 +443,7 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
         out = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
     nbytes = ctypes.c_size_t(0)
     _check(lib.ccsd_contract_workspace_bytes(tid, nocc, nvir, ctypes.byref(nbytes)), "ccsd_contract_workspace_bytes")
-    ws = torch.empty(int(nbytes.value) + 256, dtype=torch.uint8, device="cuda")
+    ws = _workspace(torch, nbytes.value)
     base = (ws.data_ptr() + 255) // 256 * 256
     arr = (ctypes.c_void_p * len(ins))(*[x.data_ptr() for x in ins])
     opts = _options(gemm_mode=gemm_mode)
