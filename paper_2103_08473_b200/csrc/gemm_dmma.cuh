@@ -224,6 +224,21 @@ gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
         }
     };
 
+    // accumulate: the lines of C this thread will read-modify-write are pulled into L2 now, so that the epilogue's
+    // loads do not pay a DRAM latency each (it matters for the short-K products, whose main loop is a few microseconds)
+    if (p.accumulate && p.ksplit <= 1) {
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++) {
+            const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++) {
+                const int64_t n = Cfg::M3 ? n0 + wn * NJ * 8 + nj * 8 + 2 * q : n0 + wn * NJ * 4 + nj * 4 + q;
+                if (m < p.M && n < p.N)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn));
+            }
+        }
+    }
+
     // accumulators: 4M: (Re, Im) of C[row g][col q] per fragment pair;  3M: P1, P2, P3 of C[row g][cols 2q, 2q+1]
     constexpr int NACC = Cfg::M3 ? 3 : 1;
     double acc[NACC][MI][NJ][2];
@@ -300,6 +315,19 @@ gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
     for (int mi = 0; mi < MI; mi++) {
         const int64_t m = m0 + wm * MI * 8 + mi * 8 + g;
         if (m >= p.M) continue;
+        // accumulate: all the old values of this fragment row are loaded first (NJ x NE independent loads in flight); one
+        // load-add-store after the other costs a DRAM latency each, 20 us per CTA for the short-K products of the iteration
+        c128 prev[NJ][NE];
+        const bool rmw = p.accumulate && p.ksplit <= 1;
+        if (rmw) {
+#pragma unroll
+            for (int nj = 0; nj < NJ; nj++)
+#pragma unroll
+                for (int e = 0; e < NE; e++) {
+                    const int64_t n = Cfg::M3 ? n0 + wn * NJ * 8 + nj * 8 + 2 * q + e : n0 + wn * NJ * 4 + nj * 4 + q;
+                    prev[nj][e] = n < p.N ? p.C[(int64_t)bz * p.bsC + m * p.csm + n * p.csn] : mk(0.0, 0.0);
+                }
+        }
 #pragma unroll
         for (int nj = 0; nj < NJ; nj++)
 #pragma unroll
@@ -320,7 +348,7 @@ gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
                 } else {
                     c128* c = p.C + (int64_t)bz * p.bsC + m * p.csm + n * p.csn;
                     r = cmul(p.alpha, r);
-                    *c = p.accumulate ? cadd(*c, r) : r;
+                    *c = rmw ? cadd(prev[nj][e], r) : r;
                 }
             }
     }
