@@ -145,8 +145,11 @@ def _check(status: int, where: str):
 
 
 def _workspace(torch, nbytes: int):
-    """A device workspace of nbytes (+ alignment slack).  The workspaces are tens of GB: when torch's caching allocator
-    holds freed blocks that are too small to serve the request, hand them back to the driver once and retry."""
+    """A device workspace of nbytes (+ alignment slack).  The large ones (tens of GB) get a segment of their own: torch's
+    caching allocator would otherwise carve them out of a bigger cached segment (say the 115 GiB one a previous solver
+    left), whose remainder can then neither serve the next large request nor go back to the driver while this one lives."""
+    if nbytes >= (4 << 30):
+        torch.cuda.empty_cache()
     try:
         return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device="cuda")
     except torch.OutOfMemoryError:
@@ -211,15 +214,18 @@ class CCSD:
         self.nocc, self.nvir, self.n = int(nocc), int(nvir), int(nocc + nvir)
         self.oo = self.nocc * (self.nocc - 1) // 2
         self.vv = self.nvir * (self.nvir - 1) // 2
-        h_d, B_d = _dev_c128(torch, h), _dev_c128(torch, B)
-        self.naux = int(B_d.shape[0])
-        assert tuple(h_d.shape) == (self.n, self.n) and tuple(B_d.shape) == (self.naux, self.n, self.n)
+        self.naux = int(B.shape[0])
+        assert tuple(h.shape) == (self.n, self.n) and tuple(B.shape) == (self.naux, self.n, self.n)
         self._opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder)
         nbytes = ctypes.c_size_t(0)
         _check(lib.ccsd_workspace_bytes(self.nocc, self.nvir, self.naux, ctypes.byref(self._opts),
                                         ctypes.byref(nbytes)), "ccsd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)
+        self._lam_ws = None
+        # the workspace first: the (much smaller) device copies of h and B would otherwise be carved out of whatever large
+        # cached segment a previous solver left and pin it while the workspace is allocated (see _workspace)
         self._ws = _workspace(torch, self.workspace_bytes)
+        h_d, B_d = _dev_c128(torch, h), _dev_c128(torch, B)
         base = (self._ws.data_ptr() + 255) // 256 * 256
         self._ctx = ctypes.c_void_p(None)
         _check(lib.ccsd_init(ctypes.byref(self._ctx), h_d.data_ptr(), B_d.data_ptr(), self.nocc, self.nvir, self.naux,
@@ -231,6 +237,8 @@ class CCSD:
             self._ctx = ctypes.c_void_p(None)
             self._ws = None
             self._lam_ws = None
+            if self.workspace_bytes >= (4 << 30):     # hand tens of GB back to the driver rather than to torch's cache
+                self._torch.cuda.empty_cache()
 
     def __del__(self):
         try:
