@@ -19,6 +19,7 @@ static void term_carve(int o_, int v_, char* base, TermWs* W, size_t* total)
     const int64_t o2v2 = o * o * v * v, ov3 = o * v * v * v, o3v = o * o * o * v;
     W->sc.elems = ov3 > o2v2 ? ov3 : o2v2;
     if (W->sc.elems < o3v) W->sc.elems = o3v;
+    if (W->sc.elems < o * o * o * o) W->sc.elems = o * o * o * o;
     W->sc.a = w.take<c128>(W->sc.elems);
     W->sc.b = w.take<c128>(W->sc.elems);
     W->sc.c = w.take<c128>(W->sc.elems);

@@ -115,8 +115,9 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     Carver w{base, 0};
     const int64_t o = c->o, v = c->v, oo = c->oo, vv = c->vv, ov = c->ov;
     const int64_t o2v2 = o * o * v * v, ov3 = o * v * v * v, o3v = o * o * o * v;
-    L->sc.elems = ov3 > o2v2 ? ov3 : o2v2;
-    if (L->sc.elems < o3v) L->sc.elems = o3v;
+    L->sc.elems = ov3 > o2v2 ? ov3 : o2v2;                       // largest operand / result of any product: o v^3, o^2 v^2,
+    if (L->sc.elems < o3v) L->sc.elems = o3v;                     // o^3 v or (more occupied than virtual spinors) o^4
+    if (L->sc.elems < o * o * o * o) L->sc.elems = o * o * o * o;
     L->sc.a = w.take<c128>(L->sc.elems);
     L->sc.b = w.take<c128>(L->sc.elems);
     L->sc.c = w.take<c128>(L->sc.elems);

@@ -74,8 +74,9 @@ def compare_all(oc, gc, names=None, tol=REL_TOL):
     return worst
 
 
+# the last two shapes have more occupied spinors than one 48-column GEMM tile and more occupied than virtual spinors
 @pytest.mark.parametrize("o,v,L,gemm_mode", [(5, 11, 20, 1), (5, 11, 20, 0), (6, 16, 30, 0), (3, 9, 10, 0), (6, 16, 30, 2),
-                                            (6, 16, 30, 3)])
+                                            (6, 16, 30, 3), (50, 20, 30, 0), (52, 7, 12, 0)])
 def test_every_tensor_matches_oracle(gpu, o, v, L, gemm_mode):
     """All integral classes, all intermediates of eqs 24-31, all eight terms of eq 32, S1, S2: ragged sizes."""
     from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
@@ -89,7 +90,7 @@ def test_every_tensor_matches_oracle(gpu, o, v, L, gemm_mode):
     oc.residual()
     gc.residual()
     compare_all(oc, gc)
-    assert abs(gc.energy() - oc.energy()) < 1e-13
+    assert abs(gc.energy() - oc.energy()) < 1e-13 * max(1.0, abs(oc.energy()))
     # seeded random antisymmetric amplitudes, CN(0, 0.01^2) and larger
     for seed, scale in ((1, 0.01), (2, 0.2)):
         t1, t2p = ci.random_amplitudes(o, v, seed, scale)
