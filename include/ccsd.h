@@ -224,7 +224,19 @@ enum { CCSD_TERM_PP_LADDER = 0, CCSD_TERM_HH_LADDER = 1, CCSD_TERM_RING = 2, CCS
         *   W_OVVO (eq 29)      in = { <ak||ci>, <ak||cd>, <kl||ic>, <kl||cd>, t1, t2 }   out H^{ak}_{ci} [a][k][c][i]
         *   C_OVOO (eq 30)      in = { <kl||ic>, <ak||ci>, <ak||cd>, t1, t2 }             out C [k][b][(i<j)]                    */
        CCSD_TERM_F_OV = 5, CCSD_TERM_F_VV = 6, CCSD_TERM_F_OO = 7, CCSD_TERM_W_OOOO = 8, CCSD_TERM_W_OVVO = 9,
-       CCSD_TERM_C_OVOO = 10 };
+       CCSD_TERM_C_OVOO = 10,
+       /* The remaining rows of one iteration; nocc, nvir >= 2, accumulate must be 0:
+        *   S1_RESIDUAL    (eq 33)  in = { f, H^a_c [a][c], H^k_i [k][i], H^k_c [k][c], <ak||cd>, <kl||ic>,
+        *                   <ak||ci>, t1, t2 }                                              out S1 [i][a]
+        *   S2_SMALL_TERMS (eq 32: the G_oo, V^dagger t1, G_vv, C t1 lines and the driver conj <ij||ab>)
+        *                   in = { G^a_c [a][c], G^k_i [k][i], C [k][b][(i<j)], <ak||cd>, <kl||cd>, t1, t2 }
+        *                                                                                   out [(i<j)][(a<b)]
+        *   ENERGY         (eq 9)        in = { f, <kl||cd>, t1, t2 }          out one ccsd_c128 (device)
+        *   JACOBI_UPDATE  (DESIGN reading G12)  in = { f, t1, t2, S1 [i][a], S2 [(i<j)][(a<b)] }
+        *                   out [nocc*nvir + oo*vv]: u1 = t1 + S1/D^a_i followed by u2 = t2 + S2/D^{ab}_{ij} (the layout of the
+        *                   DIIS vectors), D from eps_p = Re f_pp, opts->level_shift added to the virtual eps; opts->ccd
+        *                   keeps u1 = 0 */
+       CCSD_TERM_S1_RESIDUAL = 11, CCSD_TERM_S2_SMALL_TERMS = 12, CCSD_TERM_ENERGY = 13, CCSD_TERM_JACOBI_UPDATE = 14 };
 int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes);
 int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd_c128* out, int accumulate,
                   const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);

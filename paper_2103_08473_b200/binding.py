@@ -14,7 +14,8 @@ TENSOR_IDS = {"fock": 0, "vvvv": 1, "vovv": 2, "vovo": 3, "oovv": 4, "ooov": 5, 
               "S2_ring": 30, "S2_goo": 31, "S2_vdag_t1": 32, "S2_gvv": 33, "S2_c_t1": 34, "S2_hh_ladder": 35,
               "S2_pp_ladder": 36, "S2_driver": 37}
 TERM_IDS = {"pp_ladder": 0, "hh_ladder": 1, "ring": 2, "tau": 3, "pp_ladder_planes": 4,
-            "f_ov": 5, "f_vv": 6, "f_oo": 7, "w_oooo": 8, "w_ovvo": 9, "c_ovoo": 10}
+            "f_ov": 5, "f_vv": 6, "f_oo": 7, "w_oooo": 8, "w_ovvo": 9, "c_ovoo": 10,
+            "s1_residual": 11, "s2_small_terms": 12, "energy": 13, "jacobi_update": 14}
 NSTEPS = 16
 
 # every symbol include/ccsd.h declares
@@ -432,9 +433,11 @@ class CCSD:
         return {n: float(arr[k]) for k, n in enumerate(STEP_NAMES)}
 
 
-def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool = False, gemm_mode: int = 0):
+def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool = False, gemm_mode: int = 0,
+             level_shift: float = 0.0, ccd: bool = False):
     """ccsd_contract on CUDA tensors; returns out ([(i<j)][(a<b)] for the ladder/ring/tau terms, the layouts of
-    include/ccsd.h for the intermediates f_ov ... c_ovoo)."""
+    include/ccsd.h for the intermediates f_ov ... c_ovoo and for s1_residual, s2_small_terms, energy (one element) and
+    jacobi_update (u1 followed by packed u2; level_shift and ccd apply to it only))."""
     torch = _torch()
     lib = load_library()
     tid = TERM_IDS[term]
@@ -444,7 +447,9 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
     if tid >= TERM_IDS["f_ov"]:   # the intermediates of eqs 24-31: every input complex128, output shape per term
         ins = [_dev_c128(torch, x) for x in inputs]
         shape = {"f_ov": (nocc, nvir), "f_vv": (nvir, nvir), "f_oo": (nocc, nocc), "w_oooo": (oo, oo),
-                 "w_ovvo": (nvir, nocc, nvir, nocc), "c_ovoo": (nocc, nvir, oo)}[term]
+                 "w_ovvo": (nvir, nocc, nvir, nocc), "c_ovoo": (nocc, nvir, oo),
+                 "s1_residual": (nocc, nvir), "s2_small_terms": (oo, vv), "energy": (1,),
+                 "jacobi_update": (nocc * nvir + oo * vv,)}[term]
         if out is None:
             out = torch.zeros(shape, dtype=torch.complex128, device="cuda")
     if out is None:
@@ -454,7 +459,7 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
     ws = _workspace(torch, nbytes.value)
     base = (ws.data_ptr() + 255) // 256 * 256
     arr = (ctypes.c_void_p * len(ins))(*[x.data_ptr() for x in ins])
-    opts = _options(gemm_mode=gemm_mode)
+    opts = _options(gemm_mode=gemm_mode, level_shift=level_shift, ccd=ccd)
     _check(lib.ccsd_contract(tid, nocc, nvir, arr, out.data_ptr(), int(accumulate), ctypes.byref(opts), base,
                              int(nbytes.value), _stream_ptr(torch)), f"ccsd_contract({term})")
     torch.cuda.current_stream().synchronize()   # ws / ins must outlive the enqueued kernels

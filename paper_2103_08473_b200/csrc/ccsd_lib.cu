@@ -1859,6 +1859,16 @@ int ccsd_contract_workspace_bytes(int term, int nocc, int nvir, size_t* bytes)
         term_carve(nocc, nvir, nullptr, &tw, bytes);
         return CCSD_OK;
     }
+    if (term == CCSD_TERM_S1_RESIDUAL || term == CCSD_TERM_S2_SMALL_TERMS) {
+        TermWs tw;
+        term_carve(nocc, nvir, nullptr, &tw, bytes);
+        return CCSD_OK;
+    }
+    if (term == CCSD_TERM_ENERGY || term == CCSD_TERM_JACOBI_UPDATE) {
+        StreamWs sw;
+        stream_carve(nocc, nvir, nullptr, &sw, bytes);
+        return CCSD_OK;
+    }
     Carver w{nullptr, 0};
     w.take<int2>(oo); w.take<int2>(vv);
     switch (term) {
@@ -1895,6 +1905,17 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
         Env env2{st, opts ? opts->gemm_mode : 0, nullptr, 0};
         return contract_intermediate(term, nocc, nvir, reinterpret_cast<const c128* const*>(in_), k_nin[term - CCSD_TERM_F_OV],
                                      reinterpret_cast<c128*>(out_), env2, static_cast<char*>(workspace));
+    }
+    if (term >= CCSD_TERM_S1_RESIDUAL && term <= CCSD_TERM_JACOBI_UPDATE) {   // the remaining rows of one iteration
+        if (accumulate || nocc < 2 || nvir < 2) return CCSD_EINVAL;
+        static const int k_nin2[] = {9, 7, 4, 5};
+        const int nin = k_nin2[term - CCSD_TERM_S1_RESIDUAL];
+        if (term == CCSD_TERM_ENERGY || term == CCSD_TERM_JACOBI_UPDATE)
+            return contract_stream_term(term, nocc, nvir, reinterpret_cast<const c128* const*>(in_), nin, reinterpret_cast<c128*>(out_),
+                                        st, static_cast<char*>(workspace), opts ? opts->level_shift : 0.0, opts ? opts->ccd : 0);
+        Env env2{st, opts ? opts->gemm_mode : 0, nullptr, 0};
+        return contract_residual_term(term, nocc, nvir, reinterpret_cast<const c128* const*>(in_), nin, reinterpret_cast<c128*>(out_),
+                                      env2, static_cast<char*>(workspace));
     }
     Env env{st, opts ? opts->gemm_mode : 0, nullptr, 0};
     {   // split-K partials live at the end of the workspace (same carving order as ccsd_contract_workspace_bytes)

@@ -135,4 +135,136 @@ static int contract_intermediate(int term, int o, int v, const c128* const* in, 
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
+// ---------------------------------------------------------------------------------------------------------------
+// The remaining rows of the iteration as standalone terms: S1_RESIDUAL (eq 33),
+// S2_SMALL_TERMS (the G_oo, V^dagger t1, G_vv, C t1 and driver lines of eq 32), ENERGY (eq 9,
+// PAPER.md:97) and JACOBI_UPDATE (reading G12).  Same per-term parity role as the intermediates above.
+// ---------------------------------------------------------------------------------------------------------------
+static int contract_residual_term(int term, int o, int v, const c128* const* in, int nin, c128* out, const Env& env, char* workspace)
+{
+    cudaStream_t st = env.st;
+    TermWs W;
+    size_t total = 0;
+    term_carve(o, v, workspace, &W, &total);
+    const TcScratch& sc = W.sc;
+    const int n = o + v;
+    const int64_t O = o, V = v, oo = O * (O - 1) / 2, vv = V * (V - 1) / 2;
+    for (int q = 0; q < nin; q++)
+        if (!in[q]) return CCSD_EINVAL;
+    pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o);
+    pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v);
+    g_launches += 2;
+    if (term == CCSD_TERM_S1_RESIDUAL) {
+        const c128 *f = in[0], *Hvv = in[1], *Hoo = in[2], *Hov = in[3], *vovv = in[4], *ooov = in[5], *vovo = in[6], *t1 = in[7], *t2p = in[8];
+        build_tau(st, W.taup, t1, t2p, o, v, W.po, W.pv, nullptr);                 // eq 23
+        unpack_pairs(st, W.T2, t2p, o, 1, v, 1);
+        unpack_pairs(st, W.TAU, W.taup, o, 1, v, 1);
+        unpack_pairs(st, W.OOOV, ooov, o, 1, 0, 0, O * V);
+        c128* VOVV = W.VOVV;
+        launch_fill(st, VOVV, V * O * V, V, V, 0, [=] __device__(int64_t row, int64_t d) {
+            return asym_col(vovv, row / v, vv, (int)(row % v), (int)d, v);
+        });
+        // conj f_ia (= f_ai) + sum_c H^a_c t^c_i + sum_k H^k_i t^a_k + sum_kc H^k_c t^{ac}_{ik}
+        launch_fill(st, out, O, V, V, 0, [=] __device__(int64_t i, int64_t a) { return cconj(f[i * n + o + a]); });
+        CCSD_TRY(tc1(env, sc, 1.0, TV(Hvv, "ac", V, V), TV(t1, "ic", O, V), out, "ia"));
+        CCSD_TRY(tc1(env, sc, 1.0, TV(Hoo, "ki", O, O), TV(t1, "ka", O, V), out, "ia"));
+        CCSD_TRY(tc1(env, sc, 1.0, TV(Hov, "kc", O, V), TV(W.T2, "ikac", O, O, V, V), out, "ia"));
+        // sum_k ( sum_c (H^k_c - 2 f_kc) t^c_i ) t^a_k
+        launch_fill(st, W.Fov, O, V, V, 0, [=] __device__(int64_t k, int64_t c) {
+            return csub(Hov[k * v + c], cscale(2.0, f[k * n + o + c]));
+        });
+        CCSD_CUDA_TRY(cudaMemsetAsync(W.Foo, 0, (size_t)(O * O) * sizeof(c128), st));
+        CCSD_TRY(tc1(env, sc, 1.0, TV(W.Fov, "kc", O, V), TV(t1, "ic", O, V), W.Foo, "ki"));
+        CCSD_TRY(tc1(env, sc, 1.0, TV(W.Foo, "ki", O, O), TV(t1, "ka", O, V), out, "ia"));
+        // 1/2 sum_kcd <ak||cd> tau^{cd}_{ik} + 1/2 sum_klc <kl||ic> tau^{ca}_{kl} - sum_kc <ak||ci> t^c_k
+        CCSD_TRY(tc1(env, sc, 0.5, TV(W.VOVV, "akcd", V, O, V, V), TV(W.TAU, "ikcd", O, O, V, V), out, "ia"));
+        CCSD_TRY(tc1(env, sc, 0.5, TV(W.OOOV, "klic", O, O, O, V), TV(W.TAU, "klca", O, O, V, V), out, "ia"));
+        CCSD_TRY(tc1(env, sc, -1.0, TV(vovo, "akci", V, O, V, O), TV(t1, "kc", O, V), out, "ia"));
+    } else if (term == CCSD_TERM_S2_SMALL_TERMS) {
+        const c128 *Gvv = in[0], *Goo = in[1], *Cp = in[2], *vovv = in[3], *oovv = in[4], *t1 = in[5], *t2p = in[6];
+        unpack_pairs(st, W.T2, t2p, o, 1, v, 1);
+        c128* VOVVc = W.VOVV;                       // conj <cj||ab> as [c][j][a][b]
+        launch_fill(st, VOVVc, V * O * V, V, V, 0, [=] __device__(int64_t row, int64_t b) {
+            return cconj(asym_col(vovv, row / v, vv, (int)(row % v), (int)b, v));
+        });
+        c128* Cu = W.tmp;                           // C [k][a][i][j]
+        launch_fill(st, Cu, O * V * O, O, O, 0, [=] __device__(int64_t row, int64_t j) {
+            return asym_col(Cp, row / o, oo, (int)(row % o), (int)j, o);
+        });
+        c128* S = W.X;
+        CCSD_CUDA_TRY(cudaMemsetAsync(S, 0, (size_t)(O * O * V * V) * sizeof(c128), st));
+        CCSD_TRY(tc2(env, sc, 1.0, TV(Goo, "kj", O, O), TV(W.T2, "ikab", O, O, V, V), S, "ijab", "jiab"));     // P-_ji sum_k G^k_j t^{ab}_{ik}
+        CCSD_TRY(tc2(env, sc, 1.0, TV(VOVVc, "cjab", V, O, V, V), TV(t1, "ic", O, V), S, "ijab", "jiab"));     // P-_ij sum_c conj<cj||ab> t^c_i
+        CCSD_TRY(tc2(env, sc, 1.0, TV(Gvv, "ac", V, V), TV(W.T2, "ijcb", O, O, V, V), S, "ijab", "ijba"));     // P-_ab sum_c G^a_c t^{cb}_{ij}
+        CCSD_TRY(tc2(env, sc, 1.0, TV(Cu, "kaij", O, V, O, O), TV(t1, "kb", O, V), S, "ijab", "ijba"));        // P-_ab sum_k C^{ka}_{ij} t^b_k
+        const int2 *po = W.po, *pv = W.pv;
+        launch_fill(st, out, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {                           // + conj <ij||ab>, packed
+            const int2 ij = po[IJ], ab = pv[AB];
+            return cadd(S[(((int64_t)ij.x * o + ij.y) * v + ab.x) * v + ab.y], cconj(oovv[IJ * vv + AB]));
+        });
+    } else {
+        return CCSD_EINVAL;
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
+// ENERGY and JACOBI_UPDATE stream over the packed amplitudes; their workspace is the pair tables, tau and eps only.
+struct StreamWs {
+    int2 *po, *pv;
+    c128* taup;
+    double* eps;
+};
+static void stream_carve(int o_, int v_, char* base, StreamWs* W, size_t* total)
+{
+    Carver w{base, 0};
+    const int64_t o = o_, v = v_, oo = o * (o - 1) / 2, vv = v * (v - 1) / 2;
+    W->po = w.take<int2>(oo);
+    W->pv = w.take<int2>(vv);
+    W->taup = w.take<c128>(oo * vv);
+    W->eps = w.take<double>(o + v);
+    *total = w.off;
+}
+static int contract_stream_term(int term, int o, int v, const c128* const* in, int nin, c128* out, cudaStream_t st, char* workspace,
+                                double level_shift, int ccd)
+{
+    StreamWs W;
+    size_t total = 0;
+    stream_carve(o, v, workspace, &W, &total);
+    const int n = o + v;
+    const int64_t O = o, V = v, oo = O * (O - 1) / 2, vv = V * (V - 1) / 2;
+    for (int q = 0; q < nin; q++)
+        if (!in[q]) return CCSD_EINVAL;
+    pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o);
+    pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v);
+    g_launches += 2;
+    if (term == CCSD_TERM_ENERGY) {          // E = sum_ia f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij}
+        const c128 *f = in[0], *oovv = in[1], *t1 = in[2], *t2p = in[3];
+        build_tau(st, W.taup, t1, t2p, o, v, W.po, W.pv, nullptr);
+        CCSD_CUDA_TRY(cudaMemsetAsync(out, 0, sizeof(c128), st));
+        launch_energy(st, f, n, o, v, t1, oovv, W.taup, oo * vv, reinterpret_cast<double*>(out));
+    } else if (term == CCSD_TERM_JACOBI_UPDATE) {   // u = t + S / D, D from eps_p = Re f_pp (+ level shift on the virtuals)
+        const c128 *f = in[0], *t1 = in[1], *t2p = in[2], *S1 = in[3], *S2 = in[4];
+        double* eps = W.eps;
+        eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(f, eps, n, o, level_shift);
+        g_launches++;
+        const int2 *po = W.po, *pv = W.pv;
+        launch_fill(st, out, O, V, V, 0, [=] __device__(int64_t i, int64_t a) {
+            if (ccd) return mk(0.0, 0.0);
+            const double d = eps[i] - eps[o + a];
+            const c128 s = S1[i * v + a];
+            return cadd(t1[i * v + a], mk(s.x / d, s.y / d));
+        });
+        launch_fill(st, out + O * V, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
+            const int2 ij = po[IJ], ab = pv[AB];
+            const double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
+            const c128 s = S2[IJ * vv + AB];
+            return cadd(t2p[IJ * vv + AB], mk(s.x / d, s.y / d));
+        });
+    } else {
+        return CCSD_EINVAL;
+    }
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
 #undef TV

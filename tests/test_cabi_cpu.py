@@ -56,7 +56,12 @@ def test_workspace_bytes_scales_and_validates(lib):
     assert lib.ccsd_workspace_bytes(4, 16, 60, None, None) == 1
     assert lib.ccsd_contract_workspace_bytes(0, 4, 16, ctypes.byref(n)) == 0
     assert lib.ccsd_contract_workspace_bytes(7, 4, 16, ctypes.byref(n)) == 0      # F_OO
-    assert lib.ccsd_contract_workspace_bytes(11, 4, 16, ctypes.byref(n)) == 1
+    assert lib.ccsd_contract_workspace_bytes(11, 4, 16, ctypes.byref(n)) == 0     # S1_RESIDUAL
+    big_term = n.value
+    assert lib.ccsd_contract_workspace_bytes(13, 4, 16, ctypes.byref(n)) == 0     # ENERGY: pair tables, tau, eps only
+    assert 120 * 6 * 16 <= n.value < big_term
+    assert lib.ccsd_contract_workspace_bytes(14, 4, 16, ctypes.byref(n)) == 0     # JACOBI_UPDATE
+    assert lib.ccsd_contract_workspace_bytes(15, 4, 16, ctypes.byref(n)) == 1
 
 
 def test_null_handles_are_rejected(lib):

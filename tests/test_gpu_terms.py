@@ -106,3 +106,90 @@ def test_intermediate_terms_errors(gpu):
         gpu.contract("f_ov", 4, 6, [can[k] for k in INPUTS["f_ov"]], accumulate=True)
     with pytest.raises(RuntimeError):
         gpu.contract("f_ov", 1, 6, [can["f"], can["oovv"], can["t1"]])
+
+
+# ---- the remaining rows of one iteration as standalone terms: S1 (eq 33), the small S2 terms (eq 32), energy, update ----
+def _setup_residual(o, v, naux, seed, level_shift=0.0):
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
+    can, _ = _setup(o, v, naux, seed)
+    inp = ci.make_inputs(o, v, naux, seed, b_scale=0.1, f_offdiag=0.05)
+    oc = OracleCCSD(inp.h, inp.B, o, v, ndiis=0, level_shift=level_shift)
+    oc.set_amplitudes(can["t1"], unpack_t2(can["t2"], o, v))
+    S1, S2 = oc.residual()
+    io, jo = np.triu_indices(o, 1)
+    can.update({"hvv": oc.Hvv, "hoo": oc.Hoo, "hov": oc.Hov, "gvv": oc.Gvv, "goo": oc.Goo,
+                "c": oc.C[:, :, io, jo], "s1": S1, "s2": pack_t2(S2)})
+    can = {k: np.ascontiguousarray(x) for k, x in can.items()}
+    return can, oc
+
+
+RESIDUAL_INPUTS = {
+    "s1_residual": ("f", "hvv", "hoo", "hov", "vovv", "ooov", "vovo", "t1", "t2"),
+    "s2_small_terms": ("gvv", "goo", "c", "vovv", "oovv", "t1", "t2"),
+    "energy": ("f", "oovv", "t1", "t2"),
+    "jacobi_update": ("f", "t1", "t2", "s1", "s2"),
+}
+
+
+@pytest.mark.parametrize("o,v,naux,seed", [(4, 6, 10, 61), (5, 11, 17, 62), (2, 2, 3, 63), (7, 13, 20, 64), (3, 30, 25, 65),
+                                           (9, 4, 12, 66)])
+def test_residual_terms(gpu, o, v, naux, seed):
+    from oracle.ccsd_oracle import pack_t2
+    can, oc = _setup_residual(o, v, naux, seed)
+    got = gpu.contract("s1_residual", o, v, [can[k] for k in RESIDUAL_INPUTS["s1_residual"]]).cpu().numpy()
+    assert _rel(got, oc.S1) < REL_TOL, ("s1", _rel(got, oc.S1))
+    small = sum(oc.s2_term(name) for name in ("goo", "vdag_t1", "gvv", "c_t1", "driver"))
+    got = gpu.contract("s2_small_terms", o, v, [can[k] for k in RESIDUAL_INPUTS["s2_small_terms"]]).cpu().numpy()
+    assert _rel(got, pack_t2(small)) < REL_TOL, ("s2_small", _rel(got, pack_t2(small)))
+    e = gpu.contract("energy", o, v, [can[k] for k in RESIDUAL_INPUTS["energy"]]).cpu().numpy()[0]
+    want = oc.energy()
+    assert abs(e - want) < 1e-12 * max(1.0, abs(want)), (e, want)
+
+
+def test_small_terms_complete_the_residual(gpu):
+    """Standalone intermediates -> ring + hh-ladder + pp-ladder + small terms = the oracle's full S2 (eq 32)."""
+    from oracle.ccsd_oracle import pack_t2
+    o, v = 5, 9
+    can, oc = _setup_residual(o, v, 14, 71)
+    av, bv = np.triu_indices(v, 1)
+    Wp = np.ascontiguousarray(oc.vvvv[av[:, None], bv[:, None], av[None, :], bv[None, :]])
+    tau = gpu.contract("tau", o, v, [can["t1"], can["t2"]])
+    A = gpu.contract("w_oooo", o, v, [can[k] for k in INPUTS["w_oooo"]])
+    H = gpu.contract("w_ovvo", o, v, [can[k] for k in INPUTS["w_ovvo"]])
+    S2 = gpu.contract("s2_small_terms", o, v, [can[k] for k in RESIDUAL_INPUTS["s2_small_terms"]])
+    gpu.contract("ring", o, v, [H, can["t2"]], out=S2, accumulate=True)
+    gpu.contract("hh_ladder", o, v, [A, tau], out=S2, accumulate=True)
+    gpu.contract("pp_ladder", o, v, [tau, Wp], out=S2, accumulate=True)
+    assert _rel(S2.cpu().numpy(), can["s2"]) < REL_TOL
+
+
+@pytest.mark.parametrize("shift,ccd", [(0.0, False), (0.35, False), (0.0, True)])
+def test_jacobi_update_term(gpu, shift, ccd):
+    """u = t + S/D (reading G12) against the oracle's plain-Jacobi step (ndiis = 0), with the level shift
+    of PAPER.md:1062 and the CCD switch."""
+    from oracle.ccsd_oracle import pack_t2
+    o, v = 6, 11
+    can, oc = _setup_residual(o, v, 16, 81, level_shift=shift)
+    got = gpu.contract("jacobi_update", o, v, [can[k] for k in RESIDUAL_INPUTS["jacobi_update"]], level_shift=shift,
+                       ccd=ccd).cpu().numpy()
+    oc.iterate()   # ndiis = 0: t <- t + S/D
+    want1 = np.zeros_like(oc.t1) if ccd else oc.t1
+    assert _rel(got[: o * v].reshape(o, v), want1) < REL_TOL
+    assert _rel(got[o * v:], pack_t2(oc.t2).ravel()) < REL_TOL
+
+
+def test_residual_terms_gemm_modes_and_errors(gpu):
+    from oracle.ccsd_oracle import pack_t2
+    o, v = 6, 14
+    can, oc = _setup_residual(o, v, 18, 91)
+    small = pack_t2(sum(oc.s2_term(name) for name in ("goo", "vdag_t1", "gvv", "c_t1", "driver")))
+    for mode in (1, 2, 3):
+        got = gpu.contract("s1_residual", o, v, [can[k] for k in RESIDUAL_INPUTS["s1_residual"]], gemm_mode=mode).cpu().numpy()
+        assert _rel(got, oc.S1) < REL_TOL, mode
+        got = gpu.contract("s2_small_terms", o, v, [can[k] for k in RESIDUAL_INPUTS["s2_small_terms"]], gemm_mode=mode).cpu().numpy()
+        assert _rel(got, small) < REL_TOL, mode
+    for term, names in RESIDUAL_INPUTS.items():
+        with pytest.raises(RuntimeError):
+            gpu.contract(term, o, v, [can[k] for k in names], accumulate=True)
+        with pytest.raises(RuntimeError):
+            gpu.contract(term, 1, v, [can[k] for k in names])
