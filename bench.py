@@ -256,6 +256,42 @@ def transpose_bench(torch, pkg, hbm_gbs, o, v):
     return res
 
 
+def library_yardstick(torch, pkg, o, v, peak):
+    """SURVEY 8(d) yardstick (b): the library FP64 GEMMs (cuBLAS through torch.matmul) timed beside this repo's kernel --
+    DGEMM 8192^3, and ZGEMM on the workload's pp-ladder shape (oo x vv x vv, both operands K-contiguous) against
+    ccsd_contract(PP_LADDER) on the very same tensors.  A comparison only: nothing on the product path calls a library GEMM."""
+    torch.cuda.empty_cache()
+    oo, vv = o * (o - 1) // 2, v * (v - 1) // 2
+    a = torch.randn((8192, 8192), device="cuda", dtype=torch.float64)
+    b = torch.randn((8192, 8192), device="cuda", dtype=torch.float64)
+    c = torch.empty((8192, 8192), device="cuda", dtype=torch.float64)
+    ts = time_events(torch, lambda: torch.matmul(a, b, out=c), 5, 2)
+    dgemm_tflops = 2 * 8192 ** 3 / (statistics.median(ts) * 1e-3) * 1e-12
+    del a, b, c
+    gen = torch.Generator(device="cuda").manual_seed(2021030899)
+    W = torch.view_as_complex(torch.randn((vv, vv, 2), generator=gen, device="cuda", dtype=torch.float64)) * 5e-3
+    tau = torch.view_as_complex(torch.randn((oo, vv, 2), generator=gen, device="cuda", dtype=torch.float64)) * 1e-2
+    out_lib = torch.empty((oo, vv), device="cuda", dtype=torch.complex128)
+    Wt = W.t()
+    ts = time_events(torch, lambda: torch.matmul(tau, Wt, out=out_lib), 5, 2)
+    lib_ms = statistics.median(ts)
+    out_own = torch.zeros((oo, vv), device="cuda", dtype=torch.complex128)
+    ts = time_events(torch, lambda: pkg.contract("pp_ladder", o, v, [tau, W], out=out_own), 5, 2)
+    own_ms = statistics.median(ts)
+    diff = float((out_own - out_lib).abs().max() / out_lib.abs().max())
+    fl8 = 8.0 * oo * vv * vv
+    res = {"dgemm_8192_tflops": round(dgemm_tflops, 2), "dgemm_8192_frac_fp64_peak": round(dgemm_tflops / peak, 4),
+           "pp_ladder_shape": [oo, vv, vv],
+           "library_zgemm_ms": round(lib_ms, 3), "library_zgemm_tflops_8flop": round(fl8 / (lib_ms * 1e-3) * 1e-12, 2),
+           "own_pp_ladder_ms": round(own_ms, 3), "own_pp_ladder_tflops_8flop": round(fl8 / (own_ms * 1e-3) * 1e-12, 2),
+           "own_over_library": round(lib_ms / own_ms, 3), "max_rel_diff_own_vs_library": diff,
+           "note": "library = cuBLAS via torch.matmul (complex128 ZGEMM, 4 real products per complex MAC); own = "
+                   "ccsd_contract(PP_LADDER) without caller-held sum planes (3M, 3 real products)"}
+    del W, Wt, tau, out_lib, out_own
+    torch.cuda.empty_cache()
+    return res
+
+
 def cc2_bench(torch, pkg, inp, o, v, steps=5, warmup=3):
     """NEXT-1 row of SURVEY 8(f): the CC2 iteration on the same workload, device-resident."""
     solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, cc2=True)
@@ -494,6 +530,7 @@ def run_ours(args) -> None:
     clocks = sampler.stop(t_wall0, t_wall1)
     ms_total = max_over_ranks(ms_total, dist if world > 1 else None)
     ms_per_step = ms_total / args.steps
+    iter_ms = [sum(step_acc[k][q] for k in step_acc) for q in range(args.steps)] if step_acc else []
 
     # ---- end to end: amplitudes travel host(pinned) -> device -> host every step ----------------------------------
     t1_d, t2_d = solver.get_amplitudes()
@@ -570,6 +607,7 @@ def run_ours(args) -> None:
     lam = lambda_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     direct = direct_ladder_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
+    yard = library_yardstick(torch, pkg, o, v, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
     cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
 
@@ -586,13 +624,15 @@ def run_ours(args) -> None:
         "iteration_frac_fp64_peak": round(fl["total"] * ex / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
         "pp_ladder_tflops": round(pp_tflops, 2), "pp_ladder_frac_fp64_peak": round(pp_exec / peak, 4),
         "tflops_convention": f"8 real flop per complex MAC (ZGEMM); fractions of peak use the {rf} executed",
+        "iteration_ms_from_step_events": ({"median": round(statistics.median(iter_ms), 3), "min": round(min(iter_ms), 3),
+                                           "max": round(max(iter_ms), 3)} if iter_ms else None),
         "roofline": roofline, "terms": terms,
         "e2e": {"value": e2e_s, "unit": "s/iteration", "h2d_bytes_per_step": nvec_bytes,
                 "d2h_bytes_per_step": nvec_bytes + 24},
         "gpu_launches": launches, "clocks": clocks,
         "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
                      "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "cc2": cc2, "triples": triples, "triples_sharded": trip_sharded, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "cc2": cc2, "triples": triples, "triples_sharded": trip_sharded, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "library_yardstick": yard, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:
