@@ -226,3 +226,39 @@ def test_fullsize_direct_ladder_sampled(gpu, cfg):
     e, sn = gc.iterate()
     assert np.isfinite(sn)
     gc.close()
+
+
+_SLOW = pytest.mark.skipif(os.environ.get("CCSD_SLOW_TESTS") != "1",
+                           reason="cfg3: several minutes of oracle loops and ~60 GB of host memory; set CCSD_SLOW_TESTS=1")
+
+
+@pytest.mark.parametrize("cfg,continue_oracle", [("cfg1", True), ("cfg2", False),
+                                                 pytest.param("cfg3", False, marks=_SLOW)])
+def test_converged_energy_certified_by_oracle(gpu, cfg, continue_oracle):
+    """Certification at convergence (SURVEY 8(c) parity protocol; BASELINE north_star: converged energies within 1e-10 Eh):
+    the library iterates to ||S/D||_2 < 1e-11; the ORACLE then evaluates its own residual (eqs 23-33) and energy at those
+    amplitudes.  A wrong solution cannot satisfy the oracle's equations, so max|S_oracle/D| < 1e-11 and
+    |E_oracle(t) - E_library| < 1e-10 certify the converged energy without a cold oracle run (50-100 residual builds).
+    For cfg1 the oracle also continues with its own iteration from there: its energy stays within 1e-10."""
+    from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
+    inp = ci.make_config(cfg)
+    o, v = inp.nocc, inp.nvir
+    gc = gpu.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    ok, nit, e_gpu, sn = gc.solve(1e-11, 400)
+    print(f"{cfg}: library converged={ok} after {nit} iterations, E = {e_gpu!r}, ||S/D|| = {sn:.3e}")
+    assert ok and sn < 1e-11, (cfg, nit, sn)
+    t1, t2p = gc.get_amplitudes()
+    t1, t2p = t1.cpu().numpy(), t2p.cpu().numpy()
+    gc.close()
+    oc = OracleCCSD(inp.h, inp.B, o, v, ndiis=6, restricted=True)
+    oc.set_amplitudes(t1, unpack_t2(t2p, o, v))
+    e_at = oc.energy()
+    assert abs(e_at - e_gpu) < E_TOL, (cfg, e_at, e_gpu)
+    S1, S2 = oc.residual()
+    print(f"{cfg}: oracle at the library's amplitudes: E = {e_at!r}, max|S1/D| = {np.abs(S1 / oc.D1).max():.3e}, "
+          f"max|S2/D| = {np.abs(S2 / oc.D2).max():.3e}")
+    assert np.abs(S1 / oc.D1).max() < 1e-11, (cfg, np.abs(S1 / oc.D1).max())
+    assert np.abs(pack_t2(S2 / oc.D2)).max() < 1e-11, (cfg, np.abs(pack_t2(S2 / oc.D2)).max())
+    if continue_oracle:
+        e_next, sn_o = oc.iterate()
+        assert sn_o < 1e-10 and abs(e_next - e_gpu) < E_TOL, (cfg, e_next, e_gpu, sn_o)
