@@ -495,6 +495,7 @@ static const DmmaVariant k_dmma_variants[] = {
     DMMA_V(4, 3, 4, 2, true),                                        // 9: 3M 128 x 48, 12 warps
     DMMA_V(4, 3, 4, 5, false),                                       // 10: 4M 128 x 60, 12 warps
     DMMA_V(4, 2, 4, 2, true, true), DMMA_V(4, 2, 4, 3, true, true),  // 11-12: 3M with sum planes, 128 x {32,48}
+    DMMA_V(8, 1, 2, 5, true),                                        // 13: 3M 128 x 40, 8 warps in a column (N = nocc products)
 };
 #undef DMMA_V
 constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_variants[0]));
@@ -516,6 +517,10 @@ static inline int dmma_pick(int64_t N, bool m3, bool planes = false)
         const double cost = (double)round_up(N, bn) * rel;
         if (best < 0 || cost < bestcost) { best = v; bestcost = cost; }
     }
+    // 3M 128 x 40 (variant 13, one column of eight warps): N = nocc products with 32 < nocc <= 40 (cfg3: 34) waste 15 %
+    // of a 40-column tile instead of 29 % of a 48-column one; measured 0.875 of the 128 x 48 time per tile (N = 34, K = 224
+    // and K = 7616), i.e. 1.05 per column
+    if (m3 && !planes && (double)round_up(N, 40) * 1.05 < bestcost) best = 13;
     return best;
 }
 
