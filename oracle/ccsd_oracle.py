@@ -108,7 +108,11 @@ class OracleCCSD:
         # Fock matrix
         self.f = np.zeros((n, n), dtype=C128)
         L.oracle_fock(n, o, self.naux, _p(h), _p(B), _p(self.f))
-        self.eps = self.f.diagonal().real.copy()
+        # eps_fock = Re f_pp, the spinor energies themselves: what the triples denominators of eqs 39/41 are made of
+        # (PAPER.md:645-663).  The level shift (.LSHIFT) is a convergence aid of the amplitude iterations
+        # only: eps = eps_fock + shift on the virtuals feeds D1 / D2 of the Jacobi step and of the MP2 start.
+        self.eps_fock = self.f.diagonal().real.copy()
+        self.eps = self.eps_fock.copy()
         self.eps[o:] += level_shift
         # the six integral classes, each by the definition <pq||rs> = (pr|qs) - (ps|qr)
         self.Bt = np.zeros((n, n, self.naux), dtype=C128)

@@ -41,12 +41,14 @@ def lib():
 
 class OracleTriples:
     """+T / (T) / -T at the amplitudes (t1[i][a], t2[i][j][a][b]) of an OracleCCSD-like object `oc`
-    (uses oc.f, oc.eps, oc.vovv, oc.ooov, oc.oovv)."""
+    (uses oc.f, oc.eps_fock, oc.vovv, oc.ooov, oc.oovv).  The denominators D^{abc}_{ijk} of eqs 39/41
+    are built from the spinor energies Re f_pp WITHOUT the level shift of the amplitude iterations: the
+    converged amplitudes do not depend on the shift, so neither may the triples corrections."""
 
     def __init__(self, oc, t1=None, t2=None):
         self.o, self.v = oc.o, oc.v
         o = self.o
-        self.eps = np.ascontiguousarray(oc.eps, dtype=np.float64)
+        self.eps = np.ascontiguousarray(oc.eps_fock, dtype=np.float64)
         self.fov = np.ascontiguousarray(oc.f[:o, o:], dtype=C128)
         self.t1 = np.ascontiguousarray(oc.t1 if t1 is None else t1, dtype=C128)
         self.t2 = np.ascontiguousarray(oc.t2 if t2 is None else t2, dtype=C128)
