@@ -34,6 +34,8 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of the 3M + sum-plane DMMA GEMM at cfg3, from
 # profiles/r01d_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
 NCU_TRAFFIC_BYTES = {"cfg3": 22.144e9 + 0.219e9}
+NCU_TRAFFIC_SOURCE = ("recorded constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of one "
+                      "pp-ladder launch from the ncu --set full capture summarised in profiles/r01d_ncu_pp_ladder_cfg3.md")
 
 
 def flops_per_iteration(o: int, v: int) -> dict:
@@ -115,64 +117,229 @@ def measured_peaks() -> dict:
 
 # -------------------------------------------------------------------------------------------------------------------
 # CPU oracle arm (cpu_baseline leg and --impl reference)
+#
+# What is timed is always the oracle's OWN loop nests (oracle/ccsd_oracle.c), as they stand:
+#   cfg0 / cfg1   real OracleCCSD.iterate() calls (restricted-sum mode), plus each term on its own;
+#   cfg2 / cfg3   a whole oracle iteration takes minutes to tens of minutes (recorded once by
+#                 tests/golden/make_oracle_energies.py: tests/golden/oracle_iteration_seconds.txt), so every term of
+#                 the iteration is timed on a SLAB of its outermost output indices (oracle_*_range / _part: the same
+#                 loop nests, true shapes, synthetic values) and scaled by the exact fraction of loop iterations the
+#                 slab covers.  The sum is reported as s/iteration and marked "extrapolated": true;
+#   cfg4          the pp-ladder evaluator the cfg4 parity tests use, on a bounded number of W rows per shape.
 # -------------------------------------------------------------------------------------------------------------------
-def oracle_sample_seconds_per_iteration(cfg: str, budget_s: float = 12.0) -> dict:
-    """Time the oracle, as it stands, on a bounded sample of the workload and scale to s/iteration.
+def workload_string(cfg: str) -> str:
+    o, v, L, _ = ci.CONFIGS[cfg]
+    vv = ci.pair_count(v)
+    return f"{cfg}: nocc={o} nvir={v} naux={L} complex128, DIIS(6), antisymmetry-packed <ab||cd> {vv}x{vv}"
 
-    cfg0 / cfg1: one real oracle iteration (restricted-sum mode).  cfg2 / cfg3: the oracle's explicit pp-ladder loop
-    (oracle_pp_ladder_samples) on `nrow` rows of a synthetic W[(a<b)][(c<d)] against every row of tau[(i<j)][(c<d)]
-    of the real shape; the measured complex-MAC rate is scaled to the algorithmic work of the whole iteration.
-    """
+
+def _timed(fn) -> float:
+    t0 = time.perf_counter()
+    fn()
+    return time.perf_counter() - t0
+
+
+def _pairs_below(n_first: int, extent: int) -> int:
+    """number of pairs x<y with x < n_first in a dimension of size extent"""
+    return sum(extent - 1 - x for x in range(min(n_first, extent)))
+
+
+def _grow_and_time(run, frac, limits, budget_s):
+    """run(*sizes) evaluates a slab, frac(*sizes) is the fraction of the term's loop iterations it covers.  Start from the
+    smallest slab and grow (last index first) until one evaluation takes about budget_s or the term is complete.  Returns
+    (estimated seconds of the complete term, seconds of the largest slab timed, its fraction, its sizes): complete terms
+    are measured; otherwise the two largest slabs give a fixed cost (buffers cleared, antisymmetric fill) plus a cost per
+    loop iteration, and the term is  t2 + (t2 - t1) / (f2 - f1) * (1 - f2)."""
+    sizes = [1] * len(limits)
+    hist = []
+    while True:
+        dt = _timed(lambda: run(*sizes))
+        f = frac(*sizes)
+        hist.append((dt, f))
+        done = dt >= 0.4 * budget_s or f >= 1.0
+        if not done:
+            want = min(16.0, 0.8 * budget_s / max(dt, 1e-4))
+            for k in reversed(range(len(limits))):
+                if sizes[k] < limits[k] and want > 1.0:
+                    new = int(min(limits[k], max(sizes[k] + 1, sizes[k] * want)))
+                    want /= new / sizes[k]
+                    sizes[k] = new
+            done = frac(*sizes) == f
+        if done:
+            if f >= 1.0:
+                return dt, dt, f, list(sizes)
+            if len(hist) < 2 or hist[-2][1] >= f:        # no second point yet: one more slab, twice the size
+                for k in reversed(range(len(limits))):
+                    if sizes[k] < limits[k]:
+                        sizes[k] = min(limits[k], 2 * sizes[k])
+                        break
+                hist.append((_timed(lambda: run(*sizes)), frac(*sizes)))
+                dt, f = hist[-1]
+            (t1, f1), (t2, f2) = hist[-2], hist[-1]
+            if f2 <= f1:
+                return dt / f, dt, f, list(sizes)
+            return t2 + max(t2 - t1, 0.0) / (f2 - f1) * (1.0 - f2), dt, f, list(sizes)
+
+
+def oracle_term_seconds(oc, budget_s: float) -> dict:
+    """Seconds per term of one residual evaluation + energy on the oracle object `oc` (tau current), every term by its own
+    loop nest; terms that would take longer than budget_s are timed on a slab and scaled (entry "fraction" < 1)."""
+    o, v, R = oc.o, oc.v, oc.restricted
+    oo, vv = ci.pair_count(o), ci.pair_count(v)
+    out = {}
+
+    def rec(name, full, dt, f, slab):
+        out[name] = {"seconds": full, "timed_seconds": dt, "fraction": f, "slab": slab}
+
+    dt = _timed(oc.build_tau)
+    rec("tau", dt, dt, 1.0, "all")
+    for name, extent in zip(oc.PARTS, (v, o, o, v, o, o)):
+        full, dt, f, sz = _grow_and_time(lambda n: oc.intermediates_part(name, 0, n), lambda n: n / extent, [extent], budget_s)
+        rec(name, full, dt, f, f"outer index [0,{sz[0]}) of {extent}")
+    fi = (lambda ni: _pairs_below(ni, o) / oo) if R else (lambda ni: ni / o)
+    fa = (lambda na: _pairs_below(na, v) / vv) if R else (lambda na: na / v)
+    a_cap = v if oc.vvvv is None or oc.vvvv.shape[0] == v else oc.vvvv_range[1]
+    for name in oc.TERMS:
+        if name == "ring":      # all j, all b for the slab of (i, a)
+            frac = lambda ni, na: (ni / o) * (na / v)
+        else:
+            frac = lambda ni, na: fi(ni) * fa(na)
+        lim_a = a_cap if name == "pp_ladder" else v
+        full, dt, f, sz = _grow_and_time(lambda ni, na: oc.s2_term_range(name, 0, ni, 0, na), frac, [o, lim_a], budget_s)
+        rec("S2_" + name, full, dt, f, f"i in [0,{sz[0]}) of {o}, a in [0,{sz[1]}) of {v}")
+    full, dt, f, sz = _grow_and_time(lambda ni: oc.s1_range(0, ni), lambda ni: ni / o, [o], budget_s)
+    rec("S1", full, dt, f, f"i in [0,{sz[0]}) of {o}")
+    dt = _timed(oc.energy)
+    rec("energy", dt, dt, 1.0, "all")
+    return out
+
+
+def _synthetic_oracle(o: int, v: int, seed: int, vvvv_rows: int):
+    """An oracle object of the true shapes on synthetic-valued blocks (timing only): every block is a random row
+    broadcast over the leading indices, which costs a memory pass instead of the oracle's own integral build."""
+    from oracle import ccsd_oracle as orc
+    rng = np.random.default_rng(seed)
+
+    def block(*shape, scale):
+        a = np.empty(shape, dtype=np.complex128)
+        a[...] = (rng.standard_normal(shape[-1]) + 1j * rng.standard_normal(shape[-1])) * scale
+        return a
+
+    n = o + v
+    f = block(n, n, scale=0.01)
+    f[np.arange(n), np.arange(n)] = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.3, 5.0, v)])
+    oc = orc.OracleCCSD.from_blocks(o, v, f, block(o, o, o, o, scale=5e-3), block(o, o, o, v, scale=5e-3),
+                                    block(o, o, v, v, scale=5e-3), block(v, o, v, o, scale=5e-3),
+                                    block(v, o, v, v, scale=5e-3), block(vvvv_rows, v, v, v, scale=5e-3), 0, restricted=True)
+    oc.set_amplitudes(block(o, v, scale=0.01), block(o, o, v, v, scale=0.01))
+    for a in (oc.tau, oc.Hvovo, oc.C, oc.A, oc.S2, oc._scratch):
+        a.fill(0.0)                                  # touch the pages outside the timed region
+    return oc
+
+
+def oracle_baseline(cfg: str, budget_s: float = 20.0, iterations: int = 1) -> dict:
+    """The oracle on the host cores for workload `cfg`: s/iteration (measured for cfg0/cfg1, slab-scaled for cfg2/cfg3)
+    and seconds per term."""
     from oracle import ccsd_oracle as orc
     o, v, L, seed = ci.CONFIGS[cfg]
     cores = orc.num_threads()
+    recorded = recorded_oracle_seconds()
     if cfg in ("cfg0", "cfg0_2e", "cfg1"):
         inp = ci.make_config(cfg)
         oc = orc.OracleCCSD(inp.h, inp.B, o, v, restricted=True)
-        t0 = time.perf_counter()
-        oc.iterate()
-        dt = time.perf_counter() - t0
-        return {"value": dt, "unit": "s/iteration", "cores": cores, "kind": "oracle",
-                "sample": f"one full oracle iteration of {cfg} (restricted-sum loops)"}
-    oo, vv = ci.pair_count(o), ci.pair_count(v)
-    rng = np.random.default_rng(seed)
-    tau = (rng.standard_normal((oo, vv)) + 1j * rng.standard_normal((oo, vv))) * 0.01 / np.sqrt(2)
-    rate = None
-    nrow = 64
-    while True:
-        W = (rng.standard_normal((nrow, vv)) + 1j * rng.standard_normal((nrow, vv))) * 5e-3 / np.sqrt(2)
-        ij, ab = np.meshgrid(np.arange(oo), np.arange(nrow), indexing="ij")
-        t0 = time.perf_counter()
-        orc.pp_ladder_samples(tau, W, ij.ravel(), ab.ravel())
-        dt = time.perf_counter() - t0
-        rate = oo * nrow * vv / dt            # complex MAC / s
-        if dt > budget_s / 3 or nrow >= 8192:
-            break
-        nrow = int(min(8192, nrow * 8, max(nrow * 2, nrow * (budget_s * 0.6) / max(dt, 1e-3))))
-    total_cmac = flops_per_iteration(o, v)["total"] / 8.0
-    return {"value": total_cmac / rate, "unit": "s/iteration", "cores": cores, "kind": "oracle",
-            "sample": f"oracle pp-ladder loop on {nrow} of {vv} W rows x all {oo} tau rows ({dt:.1f} s, "
-                      f"{8 * rate * 1e-9:.1f} GFLOP/s), scaled to the {total_cmac * 8e-12:.2f} TFLOP of one {cfg} iteration"}
+        ts = [_timed(oc.iterate) for _ in range(max(1, iterations))]
+        terms = oracle_term_seconds(oc, 1e9)
+        return {"value": statistics.median(ts), "unit": "s/iteration", "cores": cores, "kind": "oracle",
+                "extrapolated": False, "timed_iterations": len(ts), "timed_seconds": sum(ts),
+                "sample": f"{len(ts)} full OracleCCSD.iterate() of {cfg} (restricted-sum loops, DIIS in numpy)",
+                "per_term_seconds": {k: round(x["seconds"], 4) for k, x in terms.items()},
+                "recorded_full_iterations": recorded.get(cfg)}
+    t0 = time.perf_counter()
+    oc = _synthetic_oracle(o, v, seed, vvvv_rows=min(v, 8))
+    setup = time.perf_counter() - t0
+    nterms = 2 + len(oc.PARTS) + len(oc.TERMS) + 1
+    t0 = time.perf_counter()
+    terms = oracle_term_seconds(oc, max(0.3, budget_s / nterms))
+    timed = time.perf_counter() - t0
+    total = sum(x["seconds"] for x in terms.values())
+    return {"value": total, "unit": "s/iteration", "cores": cores, "kind": "oracle", "extrapolated": True,
+            "timed_iterations": 0, "timed_seconds": round(timed, 2), "setup_seconds": round(setup, 2),
+            "scale_factor": round(total / max(sum(x["timed_seconds"] for x in terms.values()), 1e-9), 2),
+            "sample": f"every term of one {cfg} residual + energy timed with the oracle's own loop nests on a slab of its "
+                      "outermost output indices (true shapes, synthetic values); a term's time = largest slab + cost per loop "
+                      "iteration (from the two largest slabs) x the iterations left; sum over terms (Jacobi/DIIS in numpy "
+                      "not included)",
+            "per_term_seconds": {k: round(x["seconds"], 3) for k, x in terms.items()},
+            "per_term_fraction_timed": {k: round(x["fraction"], 6) for k, x in terms.items()},
+            "recorded_full_iterations": recorded.get(cfg)}
+
+
+def recorded_oracle_seconds() -> dict:
+    """Wall seconds of REAL full oracle iterations at cfg2 / cfg3, recorded by tests/golden/make_oracle_energies.py
+    (context for the slab-scaled numbers; another machine, its core count is in the file)."""
+    path = os.path.join(ROOT, "tests", "golden", "oracle_iteration_seconds.txt")
+    out = {}
+    if not os.path.exists(path):
+        return out
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            cfg, threads, nit, sec = line.split()[:4]
+            out[cfg] = {"seconds_per_iteration": float(sec), "iterations": int(nit), "threads": int(threads),
+                        "source": "tests/golden/oracle_iteration_seconds.txt"}
+    return out
+
+
+def oracle_ladder_sweep(budget_s: float = 6.0) -> list:
+    """BASELINE config 4 on the host cores: the oracle's pp-ladder evaluator (the one the cfg4 parity tests use) on a
+    bounded number of W rows per shape against every tau row, scaled to the whole contraction."""
+    from oracle import ccsd_oracle as orc
+    out = []
+    per = budget_s / len(ci.LADDER_SWEEP)
+    for k, (o, v) in enumerate(ci.LADDER_SWEEP):
+        oo, vv = ci.pair_count(o), ci.pair_count(v)
+        rng = np.random.default_rng(ci.LADDER_SEED0 + k)
+        tau = (rng.standard_normal((oo, vv)) + 1j * rng.standard_normal((oo, vv))) * 0.01 / np.sqrt(2)
+        nrow, dt = 4, 0.0
+        while True:
+            W = (rng.standard_normal((nrow, vv)) + 1j * rng.standard_normal((nrow, vv))) * 5e-3 / np.sqrt(2)
+            ij, ab = np.meshgrid(np.arange(oo), np.arange(nrow), indexing="ij")
+            dt = _timed(lambda: orc.pp_ladder_samples(tau, W, ij.ravel(), ab.ravel()))
+            if dt > 0.4 * per or nrow >= vv:
+                break
+            nrow = int(min(vv, max(nrow * 2, nrow * 0.8 * per / max(dt, 1e-4))))
+        sec = dt * vv / nrow
+        out.append({"nocc": o, "nvir": v, "seconds": round(sec, 2), "gflops": round(8.0 * oo * vv * vv / sec * 1e-9, 2),
+                    "rows_timed": nrow, "of_rows": vv, "timed_seconds": round(dt, 3), "extrapolated": nrow < vv})
+    return out
 
 
 def run_reference(args) -> None:
+    """--impl reference: the CPU oracle on this arm's config, metric and unit.  A "step" is one bounded sample of the
+    workload (cfg0/cfg1: one real iteration; cfg2/cfg3: one pass of per-term slab timings); `steps` is the number of
+    samples actually timed, `ms_per_step` their measured wall time, so that steps x ms_per_step fits the run."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    vals = []
-    info = None
-    for _ in range(max(1, args.warmup if args.warmup < 2 else 1)):
-        oracle_sample_seconds_per_iteration(args.config, budget_s=3.0)
-    for _ in range(max(1, min(args.steps, 3))):
-        info = oracle_sample_seconds_per_iteration(args.config, budget_s=8.0)
-        vals.append(info["value"])
-    v = statistics.median(vals)
-    o, vv_, L, _ = ci.CONFIGS[args.config]
-    info["value"] = v
+    cfg = args.config
+    small = cfg in ("cfg0", "cfg1")
+    nsamp = max(1, min(args.steps, 3 if small else 2))
+    for _ in range(1 if args.warmup > 0 else 0):
+        oracle_baseline(cfg, budget_s=4.0)
+    t0 = time.perf_counter()
+    infos = [oracle_baseline(cfg, budget_s=20.0) for _ in range(nsamp)]
+    wall = time.perf_counter() - t0
+    info = sorted(infos, key=lambda d: d["value"])[len(infos) // 2]
+    v = info["value"]
     line = {"impl": "reference", "metric": "ccsd_seconds_per_iteration", "value": v, "unit": "s/iteration",
-            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": v * 1e3,
+            "n_gpus": args.gpus, "steps": nsamp, "warmup": 1 if args.warmup > 0 else 0, "ms_per_step": wall / nsamp * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
-            "data": "synthetic", "config": {"workload": f"{args.config}: nocc={o} nvir={vv_} naux={L}"},
+            "data": "synthetic", "config": {"workload": workload_string(cfg)},
+            "extrapolated": bool(info["extrapolated"]),
+            "value_note": ("measured: median of real oracle iterations" if not info["extrapolated"] else
+                           "extrapolated: sum over terms of slab seconds / slab fraction (see cpu_baseline.sample); "
+                           "ms_per_step is the measured wall time of one sampling pass, not value x 1000"),
             "cpu_baseline": info,
             "e2e": {"value": v, "unit": "s/iteration", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -182,14 +349,17 @@ def run_reference(args) -> None:
 # -------------------------------------------------------------------------------------------------------------------
 # GPU arm
 # -------------------------------------------------------------------------------------------------------------------
-def time_events(torch, fn, reps, warmup):
+def time_events(torch, fn, reps, warmup, stream=None):
+    """CUDA-event times (ms) of fn(), one pair of events per repetition, recorded on the stream fn launches on
+    (torch.cuda.Event.record() without a stream sees only torch's current stream)."""
+    stream = stream or torch.cuda.current_stream()
     for _ in range(warmup):
         fn()
     torch.cuda.synchronize()
     ts = []
     for _ in range(reps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); fn(); e1.record()
+        e0.record(stream); fn(); e1.record(stream)
         torch.cuda.synchronize()
         ts.append(e0.elapsed_time(e1))
     return ts
@@ -315,7 +485,7 @@ def cc2_bench(torch, pkg, inp, o, v, steps=5, warmup=3):
     """NEXT-1 row of SURVEY 8(f): the CC2 iteration on the same workload, device-resident."""
     solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, cc2=True)
     solver.enable_step_timing(True)
-    ts = time_events(torch, solver.iterate, steps, warmup)
+    ts = time_events(torch, solver.iterate, steps, warmup, solver.stream)
     st = solver.step_times()
     e, sn = solver.iterate()
     solver.close()
@@ -337,9 +507,9 @@ def triples_bench(torch, pkg, inp, o, v, peak_tflops):
     solver.triples()                                   # warm-up: function attributes, L2
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    e0.record(solver.stream)
     en = solver.triples()
-    e1.record()
+    e1.record(solver.stream)
     torch.cuda.synchronize()
     total_ms = e0.elapsed_time(e1)
     solver.enable_step_timing(True)
@@ -371,9 +541,9 @@ def triples_sharded_bench(torch, pkg, inp, o, v, dist):
     torch.cuda.synchronize()
     dist.barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    e0.record(solver.stream)
     en = solver.triples_sharded()
-    e1.record()
+    e1.record(solver.stream)
     torch.cuda.synchronize()
     sec = max_over_ranks(e0.elapsed_time(e1) * 1e-3, dist)
     nt = solver.triples_count()
@@ -392,7 +562,7 @@ def direct_ladder_bench(torch, pkg, inp, o, v, steps=3, warmup=2):
     every iteration, never stored)."""
     solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, direct_ladder=True)
     solver.enable_step_timing(True)
-    ts = time_events(torch, solver.iterate, steps, warmup)
+    ts = time_events(torch, solver.iterate, steps, warmup, solver.stream)
     st = solver.step_times()
     ws = solver.workspace_bytes
     solver.close()
@@ -410,12 +580,12 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
         solver.iterate()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    e0.record(solver.stream)
     solver.lambda_init()
-    e1.record()
+    e1.record(solver.stream)
     torch.cuda.synchronize()
     init_ms = e0.elapsed_time(e1)
-    ts = time_events(torch, solver.lambda_iterate, steps, warmup)
+    ts = time_events(torch, solver.lambda_iterate, steps, warmup, solver.stream)
     sn = solver.lambda_iterate()
     D = solver.density()
     tr = complex(torch.trace(D).item())
@@ -428,6 +598,147 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
             "workspace_gib": round(ws / 2 ** 30, 1),
             "note": "one permute + DMMA GEMM + signed permuted add per small term, packed-pair routes for the o^2 v^3 products; pp-ladder term on the packed "
                     "<ab||cd> with conjugated multipliers"}
+
+
+def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True) -> dict:
+    """Algorithmic bytes of the HBM-bound steps of one iteration (16 B read + 16 B written per element a
+    permutation moves; the update streams (2 + 2m) vectors at the least; m = pairs in the DIIS subspace)."""
+    oo, vv, ov = o * (o - 1) // 2, v * (v - 1) // 2, o * v
+    nvec = ov + oo * vv
+    moved = ov + 2 * oo * vv + 2 * ov * ov + v * oo * v + o * o * vv + oo * v * v      # t1T, tau^T, t2^T, Xm, T2r, tauc, tauou, t2hu
+    return {"prep_permute": moved * 32 + (2 * ov * ov * 8 if planes else 0),
+            # Jacobi + Gram row in one pass (S, t and m-1 stored e read; e, u written), then sum_l c_l u_l (m read, 1 written)
+            "update_diis": (2 * m + 4) * nvec * 16,
+            "update_diis_floor": (2 * m + 2) * nvec * 16,
+            # tau + its plane + energy in one pass: t2 and <ij||ab> read, tau (16 B) and plane (8 B) written
+            "energy": oo * vv * (16 + 16 + 16 + (8 if planes else 0)) + ov * 32}
+
+
+def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=None, clock_index=None, e2e=False,
+                    max_ranks=None) -> dict:
+    """W warm-up + exactly K timed ccsd_iterate of workload `cfg` the way a user runs them (residual replayed as a CUDA
+    graph, no events inside), CUDA events on the solver's stream around the K steps; then a second pass of K iterations
+    with the library's per-step events (direct launches) for the per-term table and the roofline launch."""
+    o, v, L, _ = ci.CONFIGS[cfg]
+    oo, vv, ov = ci.pair_count(o), ci.pair_count(v), o * v
+    barrier = barrier or torch.cuda.synchronize
+    pkg.launch_count(reset=True)
+    t0 = time.perf_counter()
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    torch.cuda.synchronize()
+    init_s = time.perf_counter() - t0
+    init = solver.init_stats()
+    e_mp2 = solver.energy()
+    st = solver.stream
+    for _ in range(warmup):
+        solver.iterate()
+    barrier()
+    launches0 = pkg.launch_count()
+    sampler = ClockSampler(clock_index) if clock_index is not None else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.25)
+    t_wall0 = time.time()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(st)
+    energies = []
+    for _ in range(steps):
+        energies.append(solver.iterate())
+    e1.record(st)
+    barrier()
+    t_wall1 = time.time()
+    ms_total = e0.elapsed_time(e1)
+    launches = pkg.launch_count() - launches0
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms_total = max_over_ranks(ms_total, max_ranks)
+    ms_per_step = ms_total / steps
+
+    # ---- per-term pass: the library's own events between the steps (this switches the graph replay off) ----------
+    solver.enable_step_timing(True)
+    solver.iterate()
+    step_acc, m_hist = {}, []
+    done = warmup + steps + 1
+    e0.record(st)
+    for q in range(steps):
+        solver.iterate()
+        m_hist.append(min(6, done + q + 1))
+        for k, x in solver.step_times().items():
+            step_acc.setdefault(k, []).append(x)
+    e1.record(st)
+    torch.cuda.synchronize()
+    ms_events = e0.elapsed_time(e1) / steps
+    solver.enable_step_timing(False)
+    fl = flops_per_iteration(o, v)
+    ex = pkg.real_flops_per_cmac() / 8.0
+    terms = {}
+    for k, xs in step_acc.items():
+        ms = statistics.median(xs)
+        ent = {"ms": round(ms, 4)}
+        if k in fl and ms > 0:
+            ent["tflops"] = round(fl[k] / (ms * 1e-3) * 1e-12, 2)
+            ent["frac_fp64_peak"] = round(fl[k] * ex / (ms * 1e-3) * 1e-12 / peak, 4)
+        terms[k] = ent
+    for k in ("prep_permute", "update_diis", "energy"):       # HBM-bound steps: algorithmic bytes / time
+        gbs = [hbm_step_bytes(o, v, m)[k] / (x * 1e-3) * 1e-9 for x, m in zip(step_acc[k], m_hist) if x > 0]
+        if gbs:
+            terms[k]["gbs"] = round(statistics.median(gbs), 1)
+            terms[k]["frac_hbm"] = round(statistics.median(gbs) / hbm_gbs, 3)
+    b = hbm_step_bytes(o, v, 6)
+    terms["update_diis"]["vector_passes"] = 16
+    terms["update_diis"]["vector_passes_floor"] = 14
+    init_pack = None
+    if init["pack_ms"] > 0:
+        init_pack = {"pack_ms": round(init["pack_ms"], 3), "pack_gbs": round(init["packed_elems"] * 48 / (init["pack_ms"] * 1e-3) * 1e-9, 1),
+                     "transpose_ms": round(init["transpose_ms"], 3),
+                     "transpose_gbs": round(init["transposed_elems"] * 32 / (init["transpose_ms"] * 1e-3) * 1e-9, 1),
+                     "gemm_ms": round(init["gemm_ms"], 3),
+                     "note": "ccsd_init's build of the packed <ab||cd> (SURVEY 8(a) I2): slab GEMMs (ac|bd) over the auxiliary index, "
+                             "slab transpositions (32 B per element), antisymmetrise-and-pack fills (two 16 B reads + one 16 B "
+                             "write per packed element); device ms summed over the slabs"}
+        init_pack["pack_frac_hbm"] = round(init_pack["pack_gbs"] / hbm_gbs, 3)
+        init_pack["transpose_frac_hbm"] = round(init_pack["transpose_gbs"] / hbm_gbs, 3)
+    out = {"workload": workload_string(cfg), "ms_per_step": ms_per_step, "s_per_iteration": round(ms_per_step * 1e-3, 6),
+           "ms_per_step_with_step_events": round(ms_events, 4), "steps": steps, "warmup": warmup,
+           "ideal_ms_at_peak": round(fl["total"] * ex / peak * 1e-9, 4),
+           "frac_of_ideal": round(fl["total"] * ex / peak * 1e-9 / ms_per_step, 4),
+           "gpu_launches": launches, "gpu_launches_per_step": round(launches / steps, 1),
+           "graph_replay": bool(st.cuda_stream != 0), "terms": terms, "init_seconds": round(init_s, 3), "init_pack": init_pack,
+           "clocks": clocks,
+           "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag], "E_last": [energies[-1][0].real, energies[-1][0].imag],
+                        "step_norm_last": energies[-1][1]}}
+    if e2e:
+        # ---- end to end: amplitudes travel host(pinned) -> device -> host every step ------------------------------
+        t1_d, t2_d = solver.get_amplitudes()
+        t1_h = torch.empty(t1_d.shape, dtype=torch.complex128).pin_memory()
+        t2_h = torch.empty(t2_d.shape, dtype=torch.complex128).pin_memory()
+        t1_h.copy_(t1_d); t2_h.copy_(t2_d)
+
+        def e2e_step():
+            t1_d.copy_(t1_h, non_blocking=True)
+            t2_d.copy_(t2_h, non_blocking=True)
+            solver.set_amplitudes(t1_d, t2_d, reset_diis=False)
+            solver.iterate()
+            a1, a2 = solver.get_amplitudes()
+            t1_h.copy_(a1, non_blocking=True)
+            t2_h.copy_(a2, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+
+        e2e_step()
+        barrier()
+        tw = time.perf_counter()
+        nsteps_e2e = max(1, min(steps, 5))
+        for _ in range(nsteps_e2e):
+            e2e_step()
+        barrier()
+        e2e_s = max_over_ranks((time.perf_counter() - tw) / nsteps_e2e, max_ranks)
+        nvec_bytes = (ov + oo * vv) * 16
+        out["e2e"] = {"value": e2e_s, "unit": "s/iteration", "h2d_bytes_per_step": nvec_bytes,
+                      "d2h_bytes_per_step": nvec_bytes + 32, "steps": nsteps_e2e}
+    solver.close()
+    del solver
+    torch.cuda.empty_cache()
+    return out
 
 
 def max_over_ranks(value: float, dist, device="cuda") -> float:
@@ -512,72 +823,12 @@ def run_ours(args) -> None:
         print(json.dumps({"metric": "triples_seconds", "unit": "s", "config": {"workload": f"{cfg} +T/(T)/-T"},
                           **triples_bench(torch, pkg, inp, o, v, peak)}))
         return
-    pkg.launch_count(reset=True)
-    t0 = time.perf_counter()
-    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
-    torch.cuda.synchronize()
-    init_s = time.perf_counter() - t0
-    e_mp2 = solver.energy()
     peak = pkg.measure_fp64_peak(8) if rank == 0 else FP64_NOMINAL_TFLOPS
     peaks = measured_peaks()
-    solver.enable_step_timing(True)
-
-    # ---- device-resident timing: W warm-up iterations, then exactly K timed iterations --------------------------
-    for _ in range(args.warmup):
-        solver.iterate()
-    barrier()
-    launches0 = pkg.launch_count()
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.25)
-    step_acc = {}
-    t_wall0 = time.time()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    energies = []
-    for _ in range(args.steps):
-        e, sn = solver.iterate()
-        energies.append((e, sn))
-        for k, x in solver.step_times().items():
-            step_acc.setdefault(k, []).append(x)
-    e1.record()
-    barrier()
-    t_wall1 = time.time()
-    ms_total = e0.elapsed_time(e1)
-    launches = pkg.launch_count() - launches0
-    clocks = sampler.stop(t_wall0, t_wall1)
-    ms_total = max_over_ranks(ms_total, dist if world > 1 else None)
-    ms_per_step = ms_total / args.steps
-    iter_ms = [sum(step_acc[k][q] for k in step_acc) for q in range(args.steps)] if step_acc else []
-
-    # ---- end to end: amplitudes travel host(pinned) -> device -> host every step ----------------------------------
-    t1_d, t2_d = solver.get_amplitudes()
-    t1_h = torch.empty(t1_d.shape, dtype=torch.complex128).pin_memory()
-    t2_h = torch.empty(t2_d.shape, dtype=torch.complex128).pin_memory()
-    t1_h.copy_(t1_d); t2_h.copy_(t2_d)
-
-    def e2e_step():
-        t1_d.copy_(t1_h, non_blocking=True)
-        t2_d.copy_(t2_h, non_blocking=True)
-        solver.set_amplitudes(t1_d, t2_d, reset_diis=False)
-        e, sn = solver.iterate()
-        a1, a2 = solver.get_amplitudes()
-        t1_h.copy_(a1, non_blocking=True)
-        t2_h.copy_(a2, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
-
-    e2e_step()
-    barrier()
-    tw = time.perf_counter()
-    nsteps_e2e = max(1, min(args.steps, 5))
-    for _ in range(nsteps_e2e):
-        e2e_step()
-    barrier()
-    e2e_s = (time.perf_counter() - tw) / nsteps_e2e
-    e2e_s = max_over_ranks(e2e_s, dist if world > 1 else None)
-    nvec_bytes = (ov + oo * vv) * 16
-
+    rf = pkg.real_flops_per_cmac()                                  # 6: the 3M kernels execute 3 real FMAs per complex MAC
+    ex = rf / 8.0
+    main = iteration_bench(torch, pkg, cfg, inp, args.steps, args.warmup, peak, peaks["hbm_gbs"], barrier=barrier,
+                           clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None))
     trip_sharded = triples_sharded_bench(torch, pkg, inp, o, v, dist) if (world > 1 and not args.no_sweep) else None
 
     if not is_reporting_rank():
@@ -587,40 +838,44 @@ def run_ours(args) -> None:
 
     # ---- roofline of the dominant kernel (the DMMA GEMM, measured on the pp-ladder launch) ------------------------
     fl = flops_per_iteration(o, v)
-    steps_med = {k: statistics.median(x) for k, x in step_acc.items()}
-    pp_ms = steps_med["pp_ladder"]
+    ms_per_step = main["ms_per_step"]
+    pp_ms = main["terms"]["pp_ladder"]["ms"]
     pp_tflops = fl["pp_ladder"] / (pp_ms * 1e-3) * 1e-12          # 8-flop (ZGEMM) convention
-    rf = pkg.real_flops_per_cmac()                                  # 6: the 3M kernels execute 3 real FMAs per complex MAC
-    ex = rf / 8.0
     pp_exec = pp_tflops * ex
-    terms = {}
-    for k, ms in steps_med.items():
-        ent = {"ms": round(ms, 3)}
-        if k in fl and ms > 0:
-            ent["tflops"] = round(fl[k] / (ms * 1e-3) * 1e-12, 2)
-        terms[k] = ent
     gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
-    gemm_ms = sum(steps_med[k] for k in gemm_steps)
+    gemm_ms = sum(main["terms"][k]["ms"] for k in gemm_steps)
+    traffic = NCU_TRAFFIC_BYTES.get(cfg)
     roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch",
                 "achieved": round(pp_exec, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
-                "frac": round(pp_exec / peak, 4), "traffic": NCU_TRAFFIC_BYTES.get(cfg),
+                "frac": round(pp_exec / peak, 4), "traffic": traffic,
+                "traffic_source": (NCU_TRAFFIC_SOURCE if traffic is not None else
+                                   "no ncu --set full capture of this workload's launch on record"),
                 "real_flops_per_complex_mac": rf,
                 "achieved_8flop_convention": round(pp_tflops, 3),
                 "note": "unit = complex MAC over the packed ranges (oo*vv*vv per launch); achieved counts the real "
                         "flops the kernel EXECUTES per unit (6 with 3M) so that frac <= 1; on the ZGEMM 8-flop "
-                        "convention the same launch is achieved_8flop_convention",
+                        "convention the same launch is achieved_8flop_convention.  launch_ms = median CUDA-event time of "
+                        "the launch over the K iterations of the step-timed pass (direct launches, events between the "
+                        "steps on the launching stream); `value` is timed without those events (graph replay)",
                 "peak_source": "DMMA.8x8x4 issue-rate microbenchmark measured in this run (ccsd_measure_fp64_peak); "
                                f"nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = {FP64_NOMINAL_TFLOPS:.1f}; "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "flops_per_launch": int(fl["pp_ladder"] * ex), "flops_per_launch_8flop": fl["pp_ladder"],
                 "launch_ms": round(pp_ms, 3),
-                "share_of_step": round(pp_ms / ms_per_step, 4),
-                "three_big_gemms": {"ms": round(gemm_ms, 3), "share_of_step": round(gemm_ms / ms_per_step, 4),
+                "share_of_step": round(pp_ms / main["ms_per_step_with_step_events"], 4),
+                "three_big_gemms": {"ms": round(gemm_ms, 3),
+                                    "share_of_step": round(gemm_ms / main["ms_per_step_with_step_events"], 4),
                                     "tflops": round(sum(fl[k] for k in gemm_steps) / (gemm_ms * 1e-3) * 1e-12, 2)}}
 
-    solver.close()
-    del solver
     torch.cuda.empty_cache()
+    # the other BASELINE configs ride along (they cost milliseconds): s/iteration and the same per-term table
+    others = {}
+    if not args.no_sweep:
+        for other in ("cfg1", "cfg2"):
+            if other != cfg:
+                r = iteration_bench(torch, pkg, other, ci.make_config(other), 10, 6, peak, peaks["hbm_gbs"])
+                others[other] = {k: r[k] for k in ("workload", "s_per_iteration", "ms_per_step_with_step_events", "ideal_ms_at_peak",
+                                                   "frac_of_ideal", "gpu_launches_per_step", "graph_replay", "terms", "energies")}
     conv = converge_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     triples = triples_bench(torch, pkg, inp, o, v, peak) if not args.no_sweep else None
@@ -629,30 +884,33 @@ def run_ours(args) -> None:
     sweep = ladder_sweep(torch, pkg, peak) if not args.no_sweep else None
     yard = library_yardstick(torch, pkg, o, v, peak) if not args.no_sweep else None
     transposes = transpose_bench(torch, pkg, peaks["hbm_gbs"], o, v)
-    cpu = oracle_sample_seconds_per_iteration(cfg) if world == 1 else None
+    cpu = oracle_baseline(cfg) if world == 1 else None
+    cpu_sweep = oracle_ladder_sweep() if (world == 1 and not args.no_sweep) else None
+    if sweep and cpu_sweep:
+        for g, c in zip(sweep, cpu_sweep):
+            g["cpu_oracle_seconds"] = c["seconds"]
+            g["cpu_oracle"] = c
 
     line = {
         "metric": "ccsd_seconds_per_iteration", "value": ms_per_step * 1e-3, "unit": "s/iteration",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
         "data": "synthetic",
-        "config": {"workload": f"{cfg}: nocc={o} nvir={v} naux={L} complex128, DIIS(6), antisymmetry-packed "
-                               f"<ab||cd> {vv}x{vv}", "replicas": world, "l2": "inputs larger than L2 (packed <ab||cd> "
-                               f"= {vv * vv * 16 / 2 ** 30:.2f} GiB vs 126 MB L2); no flush needed",
-                   "init_seconds": round(init_s, 3)},
+        "config": {"workload": workload_string(cfg), "replicas": world,
+                   "l2": f"inputs larger than L2 (packed <ab||cd> = {vv * vv * 16 / 2 ** 30:.2f} GiB vs 126 MB L2); no flush needed",
+                   "init_seconds": main["init_seconds"], "graph_replay": main["graph_replay"]},
         "iteration_tflops": round(fl["total"] / (ms_per_step * 1e-3) * 1e-12, 2),
         "iteration_frac_fp64_peak": round(fl["total"] * ex / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
         "pp_ladder_tflops": round(pp_tflops, 2), "pp_ladder_frac_fp64_peak": round(pp_exec / peak, 4),
         "tflops_convention": f"8 real flop per complex MAC (ZGEMM); fractions of peak use the {rf} executed",
-        "iteration_ms_from_step_events": ({"median": round(statistics.median(iter_ms), 3), "min": round(min(iter_ms), 3),
-                                           "max": round(max(iter_ms), 3)} if iter_ms else None),
-        "roofline": roofline, "terms": terms,
-        "e2e": {"value": e2e_s, "unit": "s/iteration", "h2d_bytes_per_step": nvec_bytes,
-                "d2h_bytes_per_step": nvec_bytes + 24},
-        "gpu_launches": launches, "clocks": clocks,
-        "energies": {"E_mp2_start": [e_mp2.real, e_mp2.imag],
-                     "E_last": [energies[-1][0].real, energies[-1][0].imag], "step_norm_last": energies[-1][1]},
-        "solve_to_convergence": conv, "cc2": cc2, "triples": triples, "triples_sharded": trip_sharded, "lambda": lam, "direct_ladder": direct, "ladder_sweep": sweep, "library_yardstick": yard, "transposes": transposes, "hbm_peak": peaks, "cpu_baseline": cpu,
+        "ms_per_step_with_step_events": main["ms_per_step_with_step_events"],
+        "roofline": roofline, "terms": main["terms"], "init_pack": main["init_pack"],
+        "e2e": main["e2e"],
+        "gpu_launches": main["gpu_launches"], "clocks": main["clocks"],
+        "energies": main["energies"], "other_configs": others,
+        "solve_to_convergence": conv, "cc2": cc2, "triples": triples, "triples_sharded": trip_sharded, "lambda": lam,
+        "direct_ladder": direct, "ladder_sweep": sweep, "library_yardstick": yard, "transposes": transposes,
+        "hbm_peak": peaks, "cpu_baseline": cpu,
     }
     print(json.dumps(line))
     if world > 1:

@@ -57,6 +57,11 @@ typedef struct {
                            slab from the factor B and contracts them.  Trades 8 v^4 naux flops per iteration for
                            24 vv^2 bytes of HBM; ccsd_get_tensor(CCSD_T_VVVV) and the Lambda entry points then return
                            CCSD_EINVAL.  Default 0 */
+    int graph;          /* 1 (default) = the residual evaluation inside ccsd_iterate / ccsd_residual (~70 kernel launches that
+                           depend on nothing but the context) is captured into a CUDA graph on its second use and replayed
+                           afterwards; 0 = always launch directly.  Capture needs a stream created by the caller: on the
+                           legacy / per-thread default streams (cuda_stream = 0, 1 or 2), and while step timing is enabled,
+                           the launches are issued directly whatever this says */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */
@@ -279,6 +284,12 @@ enum { CCSD_NSTEPS = 16 };
 int ccsd_enable_step_timing(ccsd_ctx* ctx, int enable);
 int ccsd_get_step_times(ccsd_ctx* ctx, float ms[CCSD_NSTEPS]);
 const char* ccsd_step_name(int step);
+/* How ccsd_init built the packed <ab||cd> (the "transposes" metric; zeros in cc2 / direct_ladder mode):
+ * stats[0..2] = summed device ms of {the slab GEMMs (ac|bd) over the auxiliary index, the slab transpositions, the
+ * antisymmetrise-and-pack fills}, stats[3] = complex elements the transpositions moved (16 B read + 16 B written each),
+ * stats[4] = packed elements written (two 16 B reads + one 16 B write each).  HOST out-pointer. */
+enum { CCSD_NINIT_STATS = 5 };
+int ccsd_get_init_stats(ccsd_ctx* ctx, double stats[CCSD_NINIT_STATS]);
 /* Kernel launches issued by the library since the last reset (all contexts, this process). */
 long long ccsd_launch_count(int reset);
 

@@ -160,19 +160,27 @@ void oracle_tau(int o, int v, const zc *t1, const zc *t2, zc *tau)
 
 /* ------------------------------------------------------------------------------------------------------------
  * Intermediates, eqs 24-31.  `in->tau` must already hold eq 23.
+ * oracle_intermediates_part evaluates ONE group of equations (`which`: 0 = eqs 24-25, 1 = eqs 26-27, 2 = eq 28,
+ * 3 = eq 29, 4 = eq 30, 5 = eq 31; -1 = all) for the outermost output index in [lo, hi) (ignored for which = -1):
+ * the same loop nests, so that bench.py can time a slab of a BASELINE-size term without running all of it.
+ * oracle_intermediates is the whole thing.
  * ---------------------------------------------------------------------------------------------------------- */
-void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, oracle_inter *in)
+void oracle_intermediates_part(const oracle_sys *sys, const zc *t1, const zc *t2, oracle_inter *in, int which, int lo, int hi)
 {
     UNPACK_SYS
     const zc *tau = in->tau;
     zc *Hvv = in->Hvv, *Gvv = in->Gvv, *Hoo = in->Hoo, *Goo = in->Goo, *Hov = in->Hov, *Hvovo = in->Hvovo,
        *Cint = in->C, *Aint = in->A;
     const double half = R ? 1.0 : 0.5;
+#define PART(k) (which < 0 || which == (k))
+#define LO(k) (which == (k) ? lo : 0)
+#define HI(k, full) (which == (k) ? hi : (full))
 
     /* eq 24: Hvv[a,c] = f[a,c] + 1/2 sum_{k,l,d} <kl||cd> tau[k,l,d,a]
      * eq 25: Gvv[a,c] = Hvv[a,c] + sum_{k,d} <ak||cd> t1[k,d] - sum_k f[k,c] t1[k,a] */
+    if (PART(0))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int a = 0; a < v; a++)
+    for (int a = LO(0); a < HI(0, v); a++)
         for (int c = 0; c < v; c++) {
             zc s = 0.0;
             for (int k = 0; k < o; k++)
@@ -190,8 +198,9 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
 
     /* eq 26: Hoo[k,i] = -f[k,i] + 1/2 sum_{l,c,d} <kl||cd> tau[l,i,c,d]
      * eq 27: Goo[k,i] = Hoo[k,i] - sum_{l,c} <kl||ic> t1[l,c] - sum_c f[k,c] t1[i,c] */
+    if (PART(1))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int k = 0; k < o; k++)
+    for (int k = LO(1); k < HI(1, o); k++)
         for (int i = 0; i < o; i++) {
             zc s = 0.0;
             for (int l = 0; l < o; l++)
@@ -208,8 +217,9 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
         }
 
     /* eq 28: Hov[k,c] = f[k,c] + sum_{l,d} <kl||cd> t1[l,d] */
+    if (PART(2))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int k = 0; k < o; k++)
+    for (int k = LO(2); k < HI(2, o); k++)
         for (int c = 0; c < v; c++) {
             zc s = F_(k, o + c);
             for (int l = 0; l < o; l++)
@@ -219,8 +229,9 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
 
     /* eq 29: Hvovo[a,k,c,i] = <ak||ci> + sum_d <ak||cd> t1[i,d] - sum_l <kl||ic> t1[l,a]
      *                         + sum_{l,d} <kl||cd> ( 1/2 t2[l,i,a,d] + t1[l,a] t1[i,d] ) */
+    if (PART(3))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int a = 0; a < v; a++)
+    for (int a = LO(3); a < HI(3, v); a++)
         for (int k = 0; k < o; k++)
             for (int c = 0; c < v; c++)
                 for (int i = 0; i < o; i++) {
@@ -235,8 +246,9 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
 
     /* eq 30: C[k,b,i,j] = conj(<ij||kb>) + sum_c ( <bk||ci> t1[j,c] - <bk||cj> t1[i,c] )
      *                     - 1/2 sum_{c,d} <bk||cd> tau[i,j,c,d] */
+    if (PART(4))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int k = 0; k < o; k++)
+    for (int k = LO(4); k < HI(4, o); k++)
         for (int b = 0; b < v; b++)
             for (int i = 0; i < o; i++)
                 for (int j = R ? i + 1 : 0; j < o; j++) {
@@ -249,14 +261,15 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
                     CI(k, b, i, j) = s;
                     if (R) CI(k, b, j, i) = -s;
                 }
-    if (R)
-        for (int k = 0; k < o; k++)
+    if (R && PART(4))
+        for (int k = LO(4); k < HI(4, o); k++)
             for (int b = 0; b < v; b++)
                 for (int i = 0; i < o; i++) CI(k, b, i, i) = 0.0;
 
     /* eq 31: A[k,l,i,j] = <kl||ij> + sum_c ( <kl||ic> t1[j,c] - <kl||jc> t1[i,c] ) + 1/2 sum_{c,d} <kl||cd> tau[i,j,c,d] */
+    if (PART(5))
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int k = 0; k < o; k++)
+    for (int k = LO(5); k < HI(5, o); k++)
         for (int l = 0; l < o; l++)
             for (int i = 0; i < o; i++)
                 for (int j = 0; j < o; j++) {
@@ -267,6 +280,14 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
                         for (int d = R ? c + 1 : 0; d < v; d++) q += OOVV(k, l, c, d) * TAU(i, j, c, d);
                     AI(k, l, i, j) = s + half * q;
                 }
+#undef PART
+#undef LO
+#undef HI
+}
+
+void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, oracle_inter *in)
+{
+    oracle_intermediates_part(sys, t1, t2, in, -1, 0, 0);
 }
 
 /* ------------------------------------------------------------------------------------------------------------
@@ -279,8 +300,14 @@ void oracle_intermediates(const oracle_sys *sys, const zc *t1, const zc *t2, ora
  *   5 hh-ladder 1/2 sum_{k,l} A[k,l,i,j] tau[k,l,a,b]
  *   6 pp-ladder 1/2 sum_{c,d} <ab||cd> tau[i,j,c,d]
  *   7 driver    conj(<ij||ab>)
+ * oracle_s2_term_range restricts the outermost output index i to [i_lo, i_hi) and the virtual output index a to
+ * [a_lo, a_hi) (the same loop nests; the antisymmetric images of those elements are filled as usual, the rest of out is
+ * left untouched): bench.py times slabs of the BASELINE-size terms with it.  For the a-range only the rows
+ * vvvv[a_lo .. a_hi) of <ab||cd> are read by the pp-ladder, so sys->vvvv may point a_lo * v^3 elements BEFORE a buffer
+ * that holds just those rows.  oracle_s2_term is the full range.
  * ---------------------------------------------------------------------------------------------------------- */
-void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, int term, zc *out)
+void oracle_s2_term_range(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, int term, int i_lo,
+                          int i_hi, int a_lo, int a_hi, zc *out)
 {
     UNPACK_SYS
     const zc *tau = in->tau, *Gvv = in->Gvv, *Goo = in->Goo, *Hvovo = in->Hvovo, *Cint = in->C, *Aint = in->A;
@@ -292,10 +319,11 @@ void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const ora
         zc *X = out; /* build X in place in a scratch copy: need all four permutations, so use a second pass */
         size_t tot = (size_t)o * o * v * v;
         zc *tmp = (zc *)malloc(tot * sizeof(zc));
+        if (i_lo > 0 || i_hi < o || a_lo > 0 || a_hi < v) memset(tmp, 0, tot * sizeof(zc));
 #pragma omp parallel for schedule(static) collapse(2)
-        for (int i = 0; i < o; i++)
+        for (int i = i_lo; i < i_hi; i++)
             for (int j = 0; j < o; j++)
-                for (int a = 0; a < v; a++)
+                for (int a = a_lo; a < a_hi; a++)
                     for (int b = 0; b < v; b++) {
                         zc s = 0.0;
                         for (int k = 0; k < o; k++)
@@ -315,10 +343,10 @@ void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const ora
     }
 
 #pragma omp parallel for schedule(dynamic) collapse(2)
-    for (int i = 0; i < o; i++)
+    for (int i = i_lo; i < i_hi; i++)
         for (int j = 0; j < o; j++) {
             if (R && j <= i) continue;
-            for (int a = 0; a < v; a++)
+            for (int a = a_lo; a < a_hi; a++)
                 for (int b = R ? a + 1 : 0; b < v; b++) {
                     zc s = 0.0;
                     switch (term) {
@@ -361,7 +389,7 @@ void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const ora
                     }
                 }
         }
-    if (R) {
+    if (R && i_lo == 0 && i_hi == o && a_lo == 0 && a_hi == v) {
         for (int i = 0; i < o; i++)
             for (int j = 0; j < o; j++)
                 for (int a = 0; a < v; a++)
@@ -369,6 +397,11 @@ void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const ora
                         if (i == j || a == b) OUT(i, j, a, b) = 0.0;
     }
 #undef OUT
+}
+
+void oracle_s2_term(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, int term, zc *out)
+{
+    oracle_s2_term_range(sys, t1, t2, in, term, 0, sys->o, 0, sys->v, out);
 }
 
 /* eq 32: S2 = sum of the eight terms above.  scratch[o][o][v][v]. */
@@ -386,13 +419,13 @@ void oracle_s2(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_i
  * S1[i,a] = conj(f[i,a]) + sum_c Hvv[a,c] t1[i,c] + sum_k Hoo[k,i] t1[k,a] + sum_{k,c} Hov[k,c] t2[i,k,a,c]
  *         + sum_k ( sum_c (Hov[k,c] - 2 f[k,c]) t1[i,c] ) t1[k,a]
  *         + 1/2 sum_{k,c,d} <ak||cd> tau[i,k,c,d] + 1/2 sum_{k,l,c} <kl||ic> tau[k,l,c,a] - sum_{k,c} <ak||ci> t1[k,c] */
-void oracle_s1(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, zc *S1)
-{
+void oracle_s1_range(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, int i_lo, int i_hi, zc *S1)
+{   /* rows i in [i_lo, i_hi) of S1 (the same loop nest; bench.py times a slab of it) */
     UNPACK_SYS
     const zc *tau = in->tau, *Hvv = in->Hvv, *Hoo = in->Hoo, *Hov = in->Hov;
     const double half = R ? 1.0 : 0.5;
 #pragma omp parallel for schedule(static) collapse(2)
-    for (int i = 0; i < o; i++)
+    for (int i = i_lo; i < i_hi; i++)
         for (int a = 0; a < v; a++) {
             zc s = conj(F_(i, o + a));
             for (int c = 0; c < v; c++) s += Hvv[IDX2(a, c, v)] * T1(i, c);
@@ -418,6 +451,11 @@ void oracle_s1(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_i
                 for (int c = 0; c < v; c++) s -= VOVO(a, k, c, i) * T1(k, c);
             S1[IDX2(i, a, v)] = s;
         }
+}
+
+void oracle_s1(const oracle_sys *sys, const zc *t1, const zc *t2, const oracle_inter *in, zc *S1)
+{
+    oracle_s1_range(sys, t1, t2, in, 0, sys->o, S1);
 }
 
 /* Correlation energy (eq 9 PAPER.md:97 evaluated for CCSD; string form PAPER.md:178-182; reading G11):

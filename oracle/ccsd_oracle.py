@@ -130,7 +130,45 @@ class OracleCCSD:
         eo, ev = self.eps[:o], self.eps[o:]
         self.D1 = eo[:, None] - ev[None, :]
         self.D2 = eo[:, None, None, None] + eo[None, :, None, None] - ev[None, None, :, None] - ev[None, None, None, :]
-        # intermediates
+        self._alloc_work()      # intermediates, residuals
+        self.mp2_guess()
+
+    @classmethod
+    def from_blocks(cls, nocc: int, nvir: int, f, oooo, ooov, oovv, vovo, vovv, vvvv_rows=None, vvvv_row0: int = 0,
+                    restricted: bool = True, ndiis: int = 6):
+        """An oracle object on CALLER-SUPPLIED Fock matrix and integral blocks (no Fock / integral build, amplitudes zero):
+        bench.py's cpu_baseline leg times slabs of the BASELINE-size terms with it, on synthetic-valued blocks of the true
+        shapes (building the real v^4 block takes the oracle tens of minutes at cfg3).  `vvvv_rows` holds rows
+        [vvvv_row0, vvvv_row0 + len) of <ab||cd> [a][b][c][d] only; s2_term_range must then stay inside that a-range."""
+        self = cls.__new__(cls)
+        o, v = int(nocc), int(nvir)
+        self.o, self.v, self.n, self.naux = o, v, o + v, 0
+        self.restricted, self.ndiis = bool(restricted), ndiis
+        self.f, self.oooo, self.ooov, self.oovv, self.vovo, self.vovv = f, oooo, ooov, oovv, vovo, vovv
+        self.vvvv = vvvv_rows
+        for a, shp in ((f, (o + v, o + v)), (oooo, (o, o, o, o)), (ooov, (o, o, o, v)), (oovv, (o, o, v, v)),
+                       (vovo, (v, o, v, o)), (vovv, (v, o, v, v))):
+            assert a.dtype == C128 and a.shape == shp and a.flags["C_CONTIGUOUS"]
+        vvvv_ptr = 0
+        if vvvv_rows is not None:
+            assert vvvv_rows.dtype == C128 and vvvv_rows.shape[1:] == (v, v, v) and vvvv_rows.flags["C_CONTIGUOUS"]
+            vvvv_ptr = vvvv_rows.ctypes.data - int(vvvv_row0) * v ** 3 * 16
+        self.vvvv_range = (int(vvvv_row0), int(vvvv_row0) + (0 if vvvv_rows is None else vvvv_rows.shape[0]))
+        self.sys = _Sys(o, v, int(self.restricted), f.ctypes.data, oooo.ctypes.data, ooov.ctypes.data, oovv.ctypes.data,
+                        vovo.ctypes.data, vovv.ctypes.data, vvvv_ptr)
+        self.eps_fock = f.diagonal().real.copy()
+        self.eps = self.eps_fock.copy()
+        eo, ev = self.eps[:o], self.eps[o:]
+        self.D1 = eo[:, None] - ev[None, :]
+        self.D2 = None
+        self._alloc_work()
+        self.t1 = np.zeros((o, v), dtype=C128)
+        self.t2 = np.zeros((o, o, v, v), dtype=C128)
+        self._diis_u, self._diis_e = [], []
+        return self
+
+    def _alloc_work(self):
+        o, v = self.o, self.v
         self.tau = np.zeros((o, o, v, v), dtype=C128)
         self.Hvv = np.zeros((v, v), dtype=C128); self.Gvv = np.zeros((v, v), dtype=C128)
         self.Hoo = np.zeros((o, o), dtype=C128); self.Goo = np.zeros((o, o), dtype=C128)
@@ -143,7 +181,6 @@ class OracleCCSD:
         self.S1 = np.zeros((o, v), dtype=C128)
         self.S2 = np.zeros((o, o, v, v), dtype=C128)
         self._scratch = np.zeros((o, o, v, v), dtype=C128)
-        self.mp2_guess()
 
     def _g(self, P, Q, Rr, S, apq, ars):
         out = np.zeros((P[1], Q[1], Rr[1], S[1]), dtype=C128)
@@ -177,6 +214,29 @@ class OracleCCSD:
         lib().oracle_s2_term(ctypes.byref(self.sys), _p(self.t1), _p(self.t2), ctypes.byref(self.inter),
                              self.TERMS.index(name), _p(out))
         return out
+
+    # --- slabs of the same loop nests (timing of BASELINE-size terms in bench.py; results land in the usual arrays) ------
+    PARTS = ("Hvv_Gvv", "Hoo_Goo", "Hov", "Hvovo", "C", "A")          # eqs 24-25, 26-27, 28, 29, 30, 31
+
+    def build_tau(self):
+        lib().oracle_tau(self.o, self.v, _p(self.t1), _p(self.t2), _p(self.tau))
+
+    def intermediates_part(self, name: str, lo: int, hi: int):
+        """One group of eqs 24-31 for its outermost output index in [lo, hi) (tau must be current)."""
+        lib().oracle_intermediates_part(ctypes.byref(self.sys), _p(self.t1), _p(self.t2), ctypes.byref(self.inter),
+                                        self.PARTS.index(name), int(lo), int(hi))
+
+    def s2_term_range(self, name: str, i_lo: int, i_hi: int, a_lo: int, a_hi: int, out=None) -> np.ndarray:
+        """One term of eq 32 for i in [i_lo, i_hi) and a in [a_lo, a_hi) (other elements of `out` untouched)."""
+        out = self._scratch if out is None else out
+        lib().oracle_s2_term_range(ctypes.byref(self.sys), _p(self.t1), _p(self.t2), ctypes.byref(self.inter),
+                                   self.TERMS.index(name), int(i_lo), int(i_hi), int(a_lo), int(a_hi), _p(out))
+        return out
+
+    def s1_range(self, i_lo: int, i_hi: int) -> np.ndarray:
+        lib().oracle_s1_range(ctypes.byref(self.sys), _p(self.t1), _p(self.t2), ctypes.byref(self.inter), int(i_lo),
+                              int(i_hi), _p(self.S1))
+        return self.S1
 
     def residual(self):
         """eqs 23-33 at the current amplitudes -> (S1[i][a], S2[i][j][a][b])."""

@@ -1,6 +1,7 @@
 """ctypes binding of include/ccsd.h (argument marshalling only; same names as the C entry points)."""
 from __future__ import annotations
 
+import contextlib
 import ctypes
 import os
 
@@ -22,7 +23,7 @@ NSTEPS = 16
 EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_iterate", "ccsd_energy", "ccsd_residual",
            "ccsd_get_amplitudes", "ccsd_set_amplitudes", "ccsd_tensor_elems", "ccsd_get_tensor", "ccsd_destroy",
            "ccsd_contract_workspace_bytes", "ccsd_contract", "ccsd_zgemm_nt", "ccsd_zgemm_nt_planes", "ccsd_sum_plane", "ccsd_transpose",
-           "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_step_name", "ccsd_launch_count",
+           "ccsd_enable_step_timing", "ccsd_get_step_times", "ccsd_get_init_stats", "ccsd_step_name", "ccsd_launch_count",
            "ccsd_measure_fp64_peak", "ccsd_real_flops_per_cmac", "ccsd_strerror",
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
@@ -41,7 +42,7 @@ class CCSDError(RuntimeError):
 
 class Options(ctypes.Structure):
     _fields_ = [("ndiis", ctypes.c_int), ("level_shift", ctypes.c_double), ("gemm_mode", ctypes.c_int),
-                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int)]
+                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int), ("graph", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -99,6 +100,7 @@ def load_library():
         lib.ccsd_transpose.argtypes = [vp, vp, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_int), ctypes.c_int, vp]
         lib.ccsd_enable_step_timing.argtypes = [vp, ctypes.c_int]
         lib.ccsd_get_step_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+        lib.ccsd_get_init_stats.argtypes = [vp, ctypes.POINTER(dbl)]
         lib.ccsd_step_name.argtypes = [ctypes.c_int]
         lib.ccsd_step_name.restype = ctypes.c_char_p
         lib.ccsd_launch_count.argtypes = [ctypes.c_int]
@@ -197,27 +199,39 @@ def measure_fp64_peak(launches: int = 10) -> float:
     return float(out.value)
 
 
-def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False) -> Options:
-    return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)))
+def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True) -> Options:
+    return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)),
+                   int(bool(graph)))
 
 
 class CCSD:
     """ccsd_init / ccsd_iterate / ccsd_energy / ccsd_get_* on device tensors.
 
     h [n][n] and B [naux][n][n] may be numpy arrays (copied host->device here) or CUDA complex128 tensors.
+    Every context works on ONE stream, `self.stream`: the caller's current stream at construction, unless that is the
+    default stream -- CUDA graphs cannot be captured there -- in which case the context gets a torch stream of its own
+    (pass `stream=` to choose).  Methods may be called from any current stream: every library call is bracketed by
+    device-side stream waits (_on_stream), tensors are allocated on the caller's stream.
     """
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
-                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False):
+                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: bool = True, stream=None):
         torch = _torch()
         lib = load_library()
         self._lib, self._torch = lib, torch
+        if stream is None:
+            stream = torch.cuda.current_stream()
+            if stream.cuda_stream == torch.cuda.default_stream().cuda_stream:
+                stream = torch.cuda.Stream()
+        self.stream = stream
+        self._ctx = ctypes.c_void_p(None)
+        opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder, graph)
         self.nocc, self.nvir, self.n = int(nocc), int(nvir), int(nocc + nvir)
         self.oo = self.nocc * (self.nocc - 1) // 2
         self.vv = self.nvir * (self.nvir - 1) // 2
         self.naux = int(B.shape[0])
         assert tuple(h.shape) == (self.n, self.n) and tuple(B.shape) == (self.naux, self.n, self.n)
-        self._opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder)
+        self._opts = opts
         nbytes = ctypes.c_size_t(0)
         _check(lib.ccsd_workspace_bytes(self.nocc, self.nvir, self.naux, ctypes.byref(self._opts),
                                         ctypes.byref(nbytes)), "ccsd_workspace_bytes")
@@ -229,11 +243,37 @@ class CCSD:
         h_d, B_d = _dev_c128(torch, h), _dev_c128(torch, B)
         base = (self._ws.data_ptr() + 255) // 256 * 256
         self._ctx = ctypes.c_void_p(None)
-        _check(lib.ccsd_init(ctypes.byref(self._ctx), h_d.data_ptr(), B_d.data_ptr(), self.nocc, self.nvir, self.naux,
-                             ctypes.byref(self._opts), base, self.workspace_bytes, _stream_ptr(torch)), "ccsd_init")
+        with self._on_stream():
+            _check(lib.ccsd_init(ctypes.byref(self._ctx), h_d.data_ptr(), B_d.data_ptr(), self.nocc, self.nvir, self.naux,
+                                 ctypes.byref(self._opts), base, self.workspace_bytes,
+                                 ctypes.c_void_p(self.stream.cuda_stream)), "ccsd_init")
+
+    @contextlib.contextmanager
+    def _on_stream(self):
+        """Bracket library calls: the context's stream first waits for the caller's current stream (inputs made there are
+        ready); afterwards the caller's stream waits for it (results are ready for whatever the caller enqueues next).
+        Device-side ordering only."""
+        torch = self._torch
+        caller = torch.cuda.current_stream()
+        if caller.cuda_stream == self.stream.cuda_stream:
+            yield
+            return
+        self.stream.wait_stream(caller)
+        try:
+            yield
+        finally:
+            caller.wait_stream(self.stream)
+
+    def _call(self, fn, *args, where=None, ok=(0,)):
+        with self._on_stream():
+            st = fn(self._ctx, *args)
+        if st not in ok:
+            _check(st, where or fn.__name__)
+        return st
 
     def close(self):
         if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.stream.synchronize()                 # nothing of this context is in flight when its memory goes back
             self._lib.ccsd_destroy(self._ctx)
             self._ctx = ctypes.c_void_p(None)
             self._ws = None
@@ -250,61 +290,56 @@ class CCSD:
     def iterate(self):
         """One CCSD iteration -> (complex E_corr of the new amplitudes, ||S/D||_2)."""
         er, ei, sn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
-        st = self._lib.ccsd_iterate(self._ctx, ctypes.byref(er), ctypes.byref(ei), ctypes.byref(sn))
-        if st not in (0, 5):
-            _check(st, "ccsd_iterate")
+        self._call(self._lib.ccsd_iterate, ctypes.byref(er), ctypes.byref(ei), ctypes.byref(sn), where="ccsd_iterate", ok=(0, 5))
         return complex(er.value, ei.value), sn.value
 
     def energy(self) -> complex:
         er, ei = ctypes.c_double(), ctypes.c_double()
-        _check(self._lib.ccsd_energy(self._ctx, ctypes.byref(er), ctypes.byref(ei)), "ccsd_energy")
+        self._call(self._lib.ccsd_energy, ctypes.byref(er), ctypes.byref(ei), where="ccsd_energy")
         return complex(er.value, ei.value)
 
     def solve(self, tol: float = 1e-9, max_iterations: int = 30):
         """ccsd_solve -> (converged, iterations, complex E_corr, ||S/D||_2); defaults = the paper's .TCONVERG / .NCYCLES."""
         it, er, ei, sn = ctypes.c_int(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
-        st = self._lib.ccsd_solve(self._ctx, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(er),
-                                  ctypes.byref(ei), ctypes.byref(sn))
-        if st not in (0, 6):
-            _check(st, "ccsd_solve")
+        st = self._call(self._lib.ccsd_solve, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(er),
+                        ctypes.byref(ei), ctypes.byref(sn), where="ccsd_solve", ok=(0, 6))
         return st == 0, it.value, complex(er.value, ei.value), sn.value
 
     def t1_diagnostic(self) -> float:
         out = ctypes.c_double()
-        _check(self._lib.ccsd_t1_diagnostic(self._ctx, ctypes.byref(out)), "ccsd_t1_diagnostic")
+        self._call(self._lib.ccsd_t1_diagnostic, ctypes.byref(out), where="ccsd_t1_diagnostic")
         return out.value
 
     def residual(self):
-        _check(self._lib.ccsd_residual(self._ctx), "ccsd_residual")
+        self._call(self._lib.ccsd_residual, where="ccsd_residual")
 
     def get_amplitudes(self):
         torch = self._torch
         t1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
         t2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
-        _check(self._lib.ccsd_get_amplitudes(self._ctx, t1.data_ptr(), t2p.data_ptr()), "ccsd_get_amplitudes")
+        self._call(self._lib.ccsd_get_amplitudes, t1.data_ptr(), t2p.data_ptr(), where="ccsd_get_amplitudes")
         return t1, t2p
 
     def set_amplitudes(self, t1, t2p, reset_diis: bool = True):
         torch = self._torch
         t1_d, t2_d = _dev_c128(torch, t1), _dev_c128(torch, t2p)
         assert tuple(t1_d.shape) == (self.nocc, self.nvir) and tuple(t2_d.shape) == (self.oo, self.vv)
-        _check(self._lib.ccsd_set_amplitudes(self._ctx, t1_d.data_ptr(), t2_d.data_ptr(), int(reset_diis)),
-               "ccsd_set_amplitudes")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_set_amplitudes, t1_d.data_ptr(), t2_d.data_ptr(), int(reset_diis), where="ccsd_set_amplitudes")
+        self.stream.synchronize()
 
     def get_tensor(self, name: str):
         torch = self._torch
         tid = TENSOR_IDS[name]
         ne = ctypes.c_size_t(0)
-        _check(self._lib.ccsd_tensor_elems(self._ctx, tid, ctypes.byref(ne)), "ccsd_tensor_elems")
+        self._call(self._lib.ccsd_tensor_elems, tid, ctypes.byref(ne), where="ccsd_tensor_elems")
         out = torch.empty(int(ne.value), dtype=torch.complex128, device="cuda")
-        _check(self._lib.ccsd_get_tensor(self._ctx, tid, out.data_ptr()), f"ccsd_get_tensor({name})")
+        self._call(self._lib.ccsd_get_tensor, tid, out.data_ptr(), where=f"ccsd_get_tensor({name})")
         return out
 
     def _triples_workspace(self):
         torch = self._torch
         nbytes = ctypes.c_size_t(0)
-        _check(self._lib.ccsd_triples_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_triples_workspace_bytes")
+        self._call(self._lib.ccsd_triples_workspace_bytes, ctypes.byref(nbytes), where="ccsd_triples_workspace_bytes")
         ws = _workspace(torch, nbytes.value)
         return ws, (ws.data_ptr() + 255) // 256 * 256, int(nbytes.value)
 
@@ -312,20 +347,20 @@ class CCSD:
         """+T / (T) / -T corrections at the current amplitudes (ccsd_triples): {"+T": E, "(T)": E, "-T": E} (complex)."""
         ws, base, nbytes = self._triples_workspace()
         a, b, c = (ctypes.c_double * 2)(), (ctypes.c_double * 2)(), (ctypes.c_double * 2)()
-        _check(self._lib.ccsd_triples(self._ctx, a, b, c, base, nbytes), "ccsd_triples")
+        self._call(self._lib.ccsd_triples, a, b, c, base, nbytes, where="ccsd_triples")
         del ws
         return {"+T": complex(a[0], a[1]), "(T)": complex(b[0], b[1]), "-T": complex(c[0], c[1])}
 
     def triples_count(self) -> int:
         n = ctypes.c_int64(0)
-        _check(self._lib.ccsd_triples_count(self._ctx, ctypes.byref(n)), "ccsd_triples_count")
+        self._call(self._lib.ccsd_triples_count, ctypes.byref(n), where="ccsd_triples_count")
         return int(n.value)
 
     def triples_range(self, first: int, count: int) -> dict:
         """Partial sums of +T / (T) / -T over the occupied triples first .. first+count-1 (ccsd_triples_range)."""
         ws, base, nbytes = self._triples_workspace()
         a, b, c = (ctypes.c_double * 2)(), (ctypes.c_double * 2)(), (ctypes.c_double * 2)()
-        _check(self._lib.ccsd_triples_range(self._ctx, int(first), int(count), a, b, c, base, nbytes), "ccsd_triples_range")
+        self._call(self._lib.ccsd_triples_range, int(first), int(count), a, b, c, base, nbytes, where="ccsd_triples_range")
         del ws
         return {"+T": complex(a[0], a[1]), "(T)": complex(b[0], b[1]), "-T": complex(c[0], c[1])}
 
@@ -343,7 +378,7 @@ class CCSD:
 
     def triples_times(self) -> dict:
         arr = (ctypes.c_float * 2)()
-        _check(self._lib.ccsd_get_triples_times(self._ctx, arr), "ccsd_get_triples_times")
+        self._call(self._lib.ccsd_get_triples_times, arr, where="ccsd_get_triples_times")
         return {"w_gemm_ms": float(arr[0]), "energy_ms": float(arr[1])}
 
     def triples_block(self, i: int, j: int, k: int):
@@ -352,9 +387,8 @@ class CCSD:
         ws, base, nbytes = self._triples_workspace()
         v = self.nvir
         out = [torch.empty((v, v, v), dtype=torch.complex128, device="cuda") for _ in range(3)]
-        _check(self._lib.ccsd_triples_block(self._ctx, int(i), int(j), int(k), out[0].data_ptr(), out[1].data_ptr(),
-                                            out[2].data_ptr(), base, nbytes), "ccsd_triples_block")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_triples_block, int(i), int(j), int(k), out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), base, nbytes, where="ccsd_triples_block")
+        self.stream.synchronize()
         del ws
         return out
 
@@ -362,56 +396,53 @@ class CCSD:
     def lambda_init(self):
         torch = self._torch
         nbytes = ctypes.c_size_t(0)
-        _check(self._lib.ccsd_lambda_workspace_bytes(self._ctx, ctypes.byref(nbytes)), "ccsd_lambda_workspace_bytes")
+        self._call(self._lib.ccsd_lambda_workspace_bytes, ctypes.byref(nbytes), where="ccsd_lambda_workspace_bytes")
         self._lam_ws = None                                # a previous Lambda workspace is released first
         self._lam_ws = _workspace(torch, nbytes.value)    # lives with the solver
         base = (self._lam_ws.data_ptr() + 255) // 256 * 256
-        _check(self._lib.ccsd_lambda_init(self._ctx, base, int(nbytes.value)), "ccsd_lambda_init")
+        self._call(self._lib.ccsd_lambda_init, base, int(nbytes.value), where="ccsd_lambda_init")
 
     def lambda_iterate(self) -> float:
         sn = ctypes.c_double()
-        st = self._lib.ccsd_lambda_iterate(self._ctx, ctypes.byref(sn))
-        if st not in (0, 5):
-            _check(st, "ccsd_lambda_iterate")
+        self._call(self._lib.ccsd_lambda_iterate, ctypes.byref(sn), where="ccsd_lambda_iterate", ok=(0, 5))
         return sn.value
 
     def lambda_solve(self, tol: float = 1e-9, max_iterations: int = 30):
         """ccsd_lambda_solve -> (converged, iterations, ||R/D||_2)."""
         it, sn = ctypes.c_int(), ctypes.c_double()
-        st = self._lib.ccsd_lambda_solve(self._ctx, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(sn))
-        if st not in (0, 6):
-            _check(st, "ccsd_lambda_solve")
+        st = self._call(self._lib.ccsd_lambda_solve, float(tol), int(max_iterations), ctypes.byref(it), ctypes.byref(sn),
+                        where="ccsd_lambda_solve", ok=(0, 6))
         return st == 0, it.value, sn.value
 
     def lambda_residual(self):
         torch = self._torch
-        _check(self._lib.ccsd_lambda_residual(self._ctx), "ccsd_lambda_residual")
+        self._call(self._lib.ccsd_lambda_residual, where="ccsd_lambda_residual")
         r1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
         r2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
-        _check(self._lib.ccsd_get_lambda_residual(self._ctx, r1.data_ptr(), r2p.data_ptr()), "ccsd_get_lambda_residual")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_get_lambda_residual, r1.data_ptr(), r2p.data_ptr(), where="ccsd_get_lambda_residual")
+        self.stream.synchronize()
         return r1, r2p
 
     def get_lambda(self):
         torch = self._torch
         l1 = torch.empty((self.nocc, self.nvir), dtype=torch.complex128, device="cuda")
         l2p = torch.empty((self.oo, self.vv), dtype=torch.complex128, device="cuda")
-        _check(self._lib.ccsd_get_lambda(self._ctx, l1.data_ptr(), l2p.data_ptr()), "ccsd_get_lambda")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_get_lambda, l1.data_ptr(), l2p.data_ptr(), where="ccsd_get_lambda")
+        self.stream.synchronize()
         return l1, l2p
 
     def set_lambda(self, l1, l2p, reset_diis: bool = True):
         torch = self._torch
         a, b = _dev_c128(torch, l1), _dev_c128(torch, l2p)
         assert tuple(a.shape) == (self.nocc, self.nvir) and tuple(b.shape) == (self.oo, self.vv)
-        _check(self._lib.ccsd_set_lambda(self._ctx, a.data_ptr(), b.data_ptr(), int(reset_diis)), "ccsd_set_lambda")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_set_lambda, a.data_ptr(), b.data_ptr(), int(reset_diis), where="ccsd_set_lambda")
+        self.stream.synchronize()
 
     def density(self):
         torch = self._torch
         D = torch.empty((self.n, self.n), dtype=torch.complex128, device="cuda")
-        _check(self._lib.ccsd_density(self._ctx, D.data_ptr()), "ccsd_density")
-        torch.cuda.current_stream().synchronize()
+        self._call(self._lib.ccsd_density, D.data_ptr(), where="ccsd_density")
+        self.stream.synchronize()
         return D
 
     def expectation(self, D, O) -> complex:
@@ -420,16 +451,21 @@ class CCSD:
         D_d, O_d = _dev_c128(torch, D), _dev_c128(torch, O)
         assert tuple(D_d.shape) == (self.n, self.n) and tuple(O_d.shape) == (self.n, self.n)
         re, im = ctypes.c_double(), ctypes.c_double()
-        _check(self._lib.ccsd_expectation(self._ctx, D_d.data_ptr(), O_d.data_ptr(), ctypes.byref(re), ctypes.byref(im)),
-               "ccsd_expectation")
+        self._call(self._lib.ccsd_expectation, D_d.data_ptr(), O_d.data_ptr(), ctypes.byref(re), ctypes.byref(im), where="ccsd_expectation")
         return complex(re.value, im.value)
 
     def enable_step_timing(self, enable: bool = True):
-        _check(self._lib.ccsd_enable_step_timing(self._ctx, int(enable)), "ccsd_enable_step_timing")
+        self._call(self._lib.ccsd_enable_step_timing, int(enable), where="ccsd_enable_step_timing")
+
+    def init_stats(self) -> dict:
+        """How ccsd_init built the packed <ab||cd> (ccsd_get_init_stats): device ms and elements moved."""
+        arr = (ctypes.c_double * 5)()
+        self._call(self._lib.ccsd_get_init_stats, arr, where="ccsd_get_init_stats")
+        return {"gemm_ms": arr[0], "transpose_ms": arr[1], "pack_ms": arr[2], "transposed_elems": arr[3], "packed_elems": arr[4]}
 
     def step_times(self):
         arr = (ctypes.c_float * NSTEPS)()
-        _check(self._lib.ccsd_get_step_times(self._ctx, arr), "ccsd_get_step_times")
+        self._call(self._lib.ccsd_get_step_times, arr, where="ccsd_get_step_times")
         return {n: float(arr[k]) for k, n in enumerate(STEP_NAMES)}
 
 

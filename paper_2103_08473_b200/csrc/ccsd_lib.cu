@@ -24,7 +24,8 @@
 #include <vector>
 
 thread_local char g_cuda_err[256] = "";
-long long g_launches = 0;
+std::atomic<long long> g_launches{0};
+thread_local long long t_launch_tally = 0;
 
 // ---------------------------------------------------------------------------------------------------------------
 // GEMM front end
@@ -107,12 +108,12 @@ static int run_gemm(const Env& env, GemmParams p)
     } else {
         dim3 grid((unsigned)((p.N + SG_BN - 1) / SG_BN), (unsigned)((p.M + SG_BM - 1) / SG_BM), (unsigned)(p.batch * p.ksplit));
         gemm_simple_kernel<<<grid, SG_T * SG_T, 0, env.st>>>(p);
-        g_launches++;
+        count_launches(1);
     }
     if (p.ksplit > 1) {
         int64_t tot = p.M * p.N * p.batch;
         splitk_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, env.st>>>(p);
-        g_launches++;
+        count_launches(1);
     }
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
@@ -123,7 +124,7 @@ static int run_gemv(const Env& env, int64_t M, int64_t K, const c128* A, int64_t
 {
     if (M <= 0) return CCSD_OK;
     gemv_kernel<<<(unsigned)((M + 7) / 8), 256, 0, env.st>>>(M, K, A, lda, x, y, sy, mk(alpha, 0.0), acc);
-    g_launches++;
+    count_launches(1);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -150,7 +151,8 @@ struct ccsd_ctx {
     Env env;
     // tables
     int2 *po, *pv;
-    double* eps;
+    double* eps;            // Re f_pp + level shift on the virtuals: denominators of the Jacobi step and of the MP2 start
+    double* eps0;           // Re f_pp: denominators of the perturbative triples (the shift is a convergence aid only)
     // constants
     c128 *f, *W, *Vvovv_p, *Vvovv_u, *VvovvT, *Voovv_p, *G1, *Voovv_c, *Voovv_ou, *Vvovo_m, *Vvovo_c, *Vooov_p,
         *Vooov_b, *Vooov_cc, *Vooov_d, *Vooov_e, *Voooo_p;
@@ -172,14 +174,19 @@ struct ccsd_ctx {
     // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
     bool planes;
     double *Ws, *Vvovv_ps, *Voovv_ps, *G1s, *taups, *Xms, *T2rs, *Hms;
-    // DIIS
-    c128 *diis_u, *diis_e;  // [ndiis][nvec]
-    double* red;            // device reduction outputs (>= 16 doubles)
+    // DIIS ring (reduce.cuh): stored pairs, device-side Gram matrix / coefficients / reduction scratch
+    DiisRing diis;
+    double* red;            // device reduction outputs (64 doubles)
     double* red_host;       // pinned host mirror
-    int diis_count;         // vectors stored so far (<= ndiis)
-    int diis_next;          // slot to overwrite next
-    std::vector<int> diis_order;       // slots, oldest first
-    std::vector<double> gram;          // [ndiis][ndiis] by slot
+    bool tau_valid;         // taup (and its plane) belong to the current (t1, t2p)
+    // the residual evaluation as a CUDA graph (captured on its second use; opts.graph, a capturable stream, timing off)
+    cudaGraphExec_t res_graph;
+    long long graph_kernels;   // kernel launches one replay stands for
+    bool graph_warm, graph_failed;
+    // ccsd_init's build of the packed <ab||cd> (the "transposes" metric): device ms of the slab GEMMs over the
+    // auxiliary index, of the slab transpositions and of the antisymmetrise-and-pack fills, and the elements the last two moved
+    double init_stats[CCSD_NINIT_STATS];
+    std::vector<cudaEvent_t>* init_events;   // 4 per slab, alive only during ccsd_init
     // timing
     int timing;
     cudaEvent_t ev[CCSD_NSTEPS + 1];
@@ -208,6 +215,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->po = w.take<int2>(oo);
     c->pv = w.take<int2>(vv);
     c->eps = w.take<double>(n);
+    c->eps0 = w.take<double>(n);
     c->f = w.take<c128>(n * n);
     // <ab||cd> is not stored in direct_ladder mode (rebuilt every iteration) nor in CC2 mode (its only use factorises)
     c->W = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<c128>(vv * vv);
@@ -322,8 +330,13 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     }
     c->nvec = ov + oo * vv;
     int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
-    c->diis_u = w.take<c128>((int64_t)nd * c->nvec);
-    c->diis_e = w.take<c128>((int64_t)nd * c->nvec);
+    c->diis.nd = c->opt.ndiis;
+    c->diis.u = w.take<c128>((int64_t)nd * c->nvec);
+    c->diis.e = w.take<c128>((int64_t)nd * c->nvec);
+    c->diis.gram = w.take<double>(13 * 13);
+    c->diis.coef = w.take<double>(16);
+    c->diis.info = w.take<double>(4);
+    c->diis.scratch = w.take<double>(RED_SCRATCH_DOUBLES);
     c->red = w.take<double>(64);
     *total = w.off;
 }
@@ -344,7 +357,7 @@ static void setup_dims(ccsd_ctx* c, int nocc, int nvir, int naux, const ccsd_opt
     c->oop = round_up(c->oo > 0 ? c->oo : 1, 4);
     if (opts) c->opt = *opts; else ccsd_default_options(&c->opt);
     if (c->opt.ndiis < 0) c->opt.ndiis = 0;
-    if (c->opt.ndiis > 12) c->opt.ndiis = 12;
+    if (c->opt.ndiis > DIIS_MAX) c->opt.ndiis = DIIS_MAX;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -391,10 +404,14 @@ struct GOooo {  // <kl||ij> = (ki|lj) - (kj|li)
     }
 };
 
-__global__ void eps_kernel(const c128* f, double* eps, int n, int o, double shift)
+// eps[p] = Re f_pp (+ shift on the virtuals, .LSHIFT PAPER.md:1062); eps0[p] = Re f_pp (may be null)
+__global__ void eps_kernel(const c128* f, double* eps, double* eps0, int n, int o, double shift)
 {
     int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p < n) eps[p] = f[(int64_t)p * n + p].x + (p >= o ? shift : 0.0);
+    if (p >= n) return;
+    const double e = f[(int64_t)p * n + p].x;
+    eps[p] = e + (p >= o ? shift : 0.0);
+    if (eps0) eps0[p] = e;
 }
 
 // Bxy[(p,q)][l] = B[l][p][q], auxiliary index fastest and zero-padded to Lp
@@ -424,10 +441,18 @@ static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* 
     const int64_t rows = (int64_t)na * v;
     // only b > a is needed, i.e. the columns (b,d) with b >= a0 + 1 of the slab (half the columns on average)
     const int64_t col0 = (int64_t)(a0 + 1) * v, ncol = v2 - col0;
+    auto mark = [&]() {
+        if (!c->init_events) return;
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); c->init_events->push_back(e); }
+    };
+    mark();
     GemmParams g = gp(rows, ncol, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv + col0 * Lp, Lp, c->Jslab + col0, v2, 1, 1.0, 0);
     if (c->Bvvs) g = with_planes(g, c->Bvvs + (int64_t)a0 * v * Lp, c->Bvvs + col0 * Lp);
     CCSD_TRY(run_gemm(c->env, g));
+    mark();
     CCSD_TRY(launch_transpose2d_ld(st, c->Jslab + col0, v2, c->JslabT + col0 * rows, rows, rows, ncol, 0));
+    mark();
     const int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
     const int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
     const c128 *J = c->Jslab, *JT = c->JslabT;
@@ -438,6 +463,11 @@ static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* 
         c128 y = JT[((int64_t)ab.y * v + cd.x) * rows + al * v + cd.y];
         return csub(x, y);
     });
+    mark();
+    if (c->init_events) {
+        c->init_stats[3] += (double)rows * (double)ncol;       // elements transposed
+        c->init_stats[4] += (double)(r1 - r0) * (double)vv;    // elements packed
+    }
     *r0_out = r0;
     *nrows_out = r1 - r0;
     return CCSD_OK;
@@ -451,8 +481,8 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
     const int2 *po = c->po, *pv = c->pv;
 
-    if (oo > 0) { pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(c->po, o); g_launches++; }
-    if (vv > 0) { pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(c->pv, v); g_launches++; }
+    if (oo > 0) { pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(c->po, o); count_launches(1); }
+    if (vv > 0) { pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(c->pv, v); count_launches(1); }
 
     // Fock matrix f = h + sum_i <pi||qi>
     launch_fill(st, c->f, n, n, n, 0, [=] __device__(int64_t p, int64_t q) {
@@ -469,8 +499,8 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
         }
         return s;
     });
-    eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(c->f, c->eps, n, o, c->opt.level_shift);
-    g_launches++;
+    eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(c->f, c->eps, c->eps0, n, o, c->opt.level_shift);
+    count_launches(1);
 
     // B blocks with the auxiliary index fastest (zero-padded to a multiple of 4): Bxy[(p,q)][l] = B[l][p][q]
     bblock(st, c->Boo, B, n, L, Lp, 0, o, 0, o);
@@ -565,10 +595,23 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
     //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
     if (c->W) {
-        for (int a0 = 0; a0 < v - 1 && vv > 0; a0 += c->na_slab) {
+        std::vector<cudaEvent_t> events;
+        c->init_events = &events;
+        int s = CCSD_OK;
+        for (int a0 = 0; a0 < v - 1 && vv > 0 && s == CCSD_OK; a0 += c->na_slab) {
             int64_t r0 = 0, nrows = 0;
-            CCSD_TRY(build_W_slab(c, a0, c->W, true, &r0, &nrows));
+            s = build_W_slab(c, a0, c->W, true, &r0, &nrows);
         }
+        c->init_events = nullptr;
+        if (s == CCSD_OK && !events.empty() && cudaStreamSynchronize(st) == cudaSuccess) {
+            for (size_t q = 0; q + 3 < events.size(); q += 4)
+                for (int k = 0; k < 3; k++) {
+                    float ms = 0.f;
+                    if (cudaEventElapsedTime(&ms, events[q + k], events[q + k + 1]) == cudaSuccess) c->init_stats[k] += ms;
+                }
+        }
+        for (cudaEvent_t e : events) cudaEventDestroy(e);
+        CCSD_TRY(s);
     }
     if (c->planes) {   // sum planes of the constant operands of the large GEMMs (3M, gemm_dmma.cuh)
         if (c->W) launch_sum_plane(st, c->W, c->Ws, vv * vv);
@@ -607,8 +650,9 @@ static void mp2_guess(ccsd_ctx* c)
         c128 x = cconj(V[IJ * vv + AB]);
         return mk(x.x / d, x.y / d);
     });
-    c->diis_count = 0; c->diis_next = 0; c->diis_order.clear();
+    c->diis.reset();
     c->have_residual = false;
+    c->tau_valid = false;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -636,14 +680,20 @@ static void build_tau(cudaStream_t st, c128* taup, const c128* t1, const c128* t
     });
 }
 
+// tau of the current amplitudes (eq 23) is usually there already: the energy kernel that closed the previous iteration
+// built it (energy_async).  Kept out of the residual proper, so that the captured graph is the same every time.
+static void ensure_tau(ccsd_ctx* c)
+{
+    if (!c->tau_valid) build_tau(c->st, c->taup, c->t1, c->t2p, c->o, c->v, c->po, c->pv, c->taups);
+    c->tau_valid = true;
+}
+
 static int prep_operands(ccsd_ctx* c)
 {
     cudaStream_t st = c->st;
     const int o = c->o, v = c->v;
     const int64_t oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
-    const int2 *po = c->po, *pv = c->pv;
     const c128 *t1 = c->t1, *t2p = c->t2p, *taup = c->taup;
-    build_tau(st, c->taup, t1, t2p, o, v, po, pv, c->taups);
     double *Xms = c->Xms, *T2rs = c->T2rs;
     launch_fill(st, c->t1T, v, o, o, 0, [=] __device__(int64_t a, int64_t i) { return t1[i * v + a]; });
     // TT[(a<b)][0:oo) = tau^T, TT[(a<b)][oop:oop+oo) = t2^T   (K-contiguous operands of the hh-ladder and Goo terms)
@@ -1041,6 +1091,7 @@ static int residual_cc2(ccsd_ctx* c)
     // doubles: operands with t2 = 0
     CCSD_TRY(cc2_dressed_factors(c));
     build_tau(st, c->taup, c->t1, nullptr, o, v, c->po, c->pv, c->taups);
+    c->tau_valid = false;                       // taup now holds tau0 = P-(t1 t1)
     CCSD_TRY(launch_transpose2d_ld(st, c->taup, c->vv, c->TT, 2 * c->oop, c->oo, c->vv, 0));
     const c128* f = c->f;
     launch_fill(st, c->Gvv, v, v, v, 0, [=] __device__(int64_t a, int64_t cc) { return f[(o + a) * n + o + cc]; });
@@ -1069,44 +1120,66 @@ static int residual_cc2(ccsd_ctx* c)
     return CCSD_OK;
 }
 
-static int residual_any(ccsd_ctx* c) { return c->opt.cc2 ? residual_cc2(c) : residual(c); }
+static int residual_body(ccsd_ctx* c) { return c->opt.cc2 ? residual_cc2(c) : residual(c); }
+
+// The ~70 launches of one residual evaluation depend on nothing but the context (shapes, options, resident pointers), so
+// they are captured once into a CUDA graph and replayed: the small configurations are launch-bound otherwise (cfg1: a 3.6 ms
+// iteration of 1.8 ms of kernels).  Capture is not permitted on the legacy / per-thread default streams; there, with step
+// timing on (events between the steps) or after any capture failure the launches are issued directly.
+static bool graph_usable(const ccsd_ctx* c)
+{
+    return c->opt.graph && !c->timing && !c->graph_failed && c->st != nullptr && c->st != cudaStreamLegacy &&
+           c->st != cudaStreamPerThread;
+}
+static int residual_any(ccsd_ctx* c)
+{
+    ensure_tau(c);
+    if (!graph_usable(c)) return residual_body(c);
+    if (!c->res_graph) {
+        if (!c->graph_warm) {   // first use: direct launches (function attributes get set, errors surface at their source)
+            c->graph_warm = true;
+            return residual_body(c);
+        }
+        const long long tally0 = t_launch_tally;
+        if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+            cudaGetLastError();
+            c->graph_failed = true;
+            return residual_body(c);
+        }
+        const int s = residual_body(c);
+        cudaGraph_t g = nullptr;
+        cudaError_t e = cudaStreamEndCapture(c->st, &g);
+        const long long captured = t_launch_tally - tally0;
+        count_launches(-captured);                       // nothing ran yet: replays are counted below
+        if (s == CCSD_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&c->res_graph, g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (s != CCSD_OK || e != cudaSuccess || !c->res_graph) {
+            cudaGetLastError();
+            c->res_graph = nullptr;
+            c->graph_failed = true;
+            return s != CCSD_OK ? s : residual_body(c);
+        }
+        c->graph_kernels = captured;
+    }
+    CCSD_CUDA_TRY(cudaGraphLaunch(c->res_graph, c->st));
+    count_launches(c->graph_kernels);
+    c->have_residual = true;
+    if (c->opt.cc2) c->tau_valid = false;               // as residual_cc2 leaves it: taup holds tau0
+    return CCSD_OK;
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // energy, update, DIIS
 // ---------------------------------------------------------------------------------------------------------------
 static int energy_async(ccsd_ctx* c, double* red_out /* device, 2 doubles */)
 {
-    build_tau(c->st, c->taup, c->t1, c->t2p, c->o, c->v, c->po, c->pv, c->taups);
-    CCSD_CUDA_TRY(cudaMemsetAsync(red_out, 0, 2 * sizeof(double), c->st));
-    // E = sum_ia f[i,a] t1[i,a] + sum_{i<j,a<b} <ij||ab> tau   (eq 9; reading G11)
-    launch_energy(c->st, c->f, c->n, c->o, c->v, c->t1, c->Voovv_p, c->taup, c->oo * c->vv, red_out);
+    // E = sum_ia f[i,a] t1[i,a] + sum_{i<j,a<b} <ij||ab> tau   (eq 9; reading G11), in one pass that also leaves tau (eq 23)
+    // and its sum plane behind as the next residual's operand.  The intermediates of the last residual (Hm, Am, ...) belong
+    // to the amplitudes that residual was evaluated at; whoever moves the amplitudes clears have_residual.
+    launch_energy_tau(c->st, c->diis.scratch, c->f, c->n, c->o, c->v, c->t1, c->t2p, c->Voovv_p, c->taup, c->taups, c->po, c->pv,
+                      red_out);
+    c->tau_valid = true;
     return CCSD_OK;
-}
-
-static int solve_small(std::vector<double>& A, std::vector<double>& b, int m)
-{   // Gaussian elimination with partial pivoting, in place; returns non-zero if singular
-    for (int col = 0; col < m; col++) {
-        int piv = col;
-        for (int r = col + 1; r < m; r++)
-            if (fabs(A[r * m + col]) > fabs(A[piv * m + col])) piv = r;
-        if (fabs(A[piv * m + col]) < 1e-300 || !std::isfinite(A[piv * m + col])) return 1;
-        if (piv != col) {
-            for (int k = 0; k < m; k++) std::swap(A[col * m + k], A[piv * m + k]);
-            std::swap(b[col], b[piv]);
-        }
-        for (int r = col + 1; r < m; r++) {
-            double fct = A[r * m + col] / A[col * m + col];
-            for (int k = col; k < m; k++) A[r * m + k] -= fct * A[col * m + k];
-            b[r] -= fct * b[col];
-        }
-    }
-    for (int r = m - 1; r >= 0; r--) {
-        double s = b[r];
-        for (int k = r + 1; k < m; k++) s -= A[r * m + k] * b[k];
-        b[r] = s / A[r * m + r];
-        if (!std::isfinite(b[r])) return 1;
-    }
-    return 0;
 }
 
 #include "lambda.cuh"
@@ -1123,6 +1196,7 @@ void ccsd_default_options(ccsd_options* opts)
     opts->ccd = 0;
     opts->cc2 = 0;
     opts->direct_ladder = 0;
+    opts->graph = 1;
 }
 
 int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
@@ -1158,7 +1232,11 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     c->env = Env{c->st, c->opt.gemm_mode, c->partial, c->partial_elems};
     c->timing = 0;
     c->red_host = nullptr;
-    c->gram.assign(13 * 13, 0.0);
+    c->res_graph = nullptr;
+    c->init_events = nullptr;
+    for (double& x : c->init_stats) x = 0.0;
+    c->graph_kernels = 0;
+    c->graph_warm = c->graph_failed = false;
     for (int k = 0; k <= CCSD_NSTEPS; k++) c->ev[k] = nullptr;
     if (cudaMallocHost(&c->red_host, 64 * sizeof(double)) != cudaSuccess) { delete c; return CCSD_ECUDA; }
     // zero the padded operand buffers once (pads must stay zero)
@@ -1182,6 +1260,7 @@ int ccsd_destroy(ccsd_ctx* c)
     for (int k = 0; k <= CCSD_NSTEPS; k++)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->red_host) cudaFreeHost(c->red_host);
+    if (c->res_graph) cudaGraphExecDestroy(c->res_graph);
     delete c->lam;
     delete c;
     return CCSD_OK;
@@ -1202,7 +1281,7 @@ int ccsd_t1_diagnostic(ccsd_ctx* c, double* t1_diag)
 {   // sqrt(sum |t1|^2 / nocc): tabulated by the paper (Tables 3, 8), not defined there; reading G18 of DESIGN.md
     if (!c || !t1_diag) return CCSD_ESTATE;
     CCSD_CUDA_TRY(cudaMemsetAsync(c->red + 48, 0, sizeof(double), c->st));
-    launch_redot(c->st, c->t1, c->t1, c->ov, c->red + 48);
+    launch_redot(c->st, c->diis.scratch, c->t1, c->t1, c->ov, c->red + 48);
     CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 48, c->red + 48, sizeof(double), cudaMemcpyDeviceToHost, c->st));
     CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
     *t1_diag = sqrt(c->red_host[48] / (double)c->o);
@@ -1219,102 +1298,26 @@ int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
 {
     if (!c) return CCSD_ESTATE;
     CCSD_TRY(residual_any(c));
-    const int o = c->o, v = c->v;
-    const int64_t vv = c->vv, ov = c->ov, nvec = c->nvec;
-    const int nd = c->opt.ndiis;
-    const int slot = nd > 0 ? c->diis_next : 0;
-    c128* U = c->diis_u + (int64_t)slot * nvec;
-    c128* E = c->diis_e + (int64_t)slot * nvec;
-    {   // Jacobi step (reading G12): e = S/D, u = t + e
-        const c128 *S1 = c->S1, *S2 = c->S2p, *t1 = c->t1, *t2p = c->t2p;
-        const double* eps = c->eps;
-        const int2 *po = c->po, *pv = c->pv;
-        const int ccd = c->opt.ccd;
-        launch_fill(c->st, E, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
-            if (ccd) { U[i * v + a] = mk(0.0, 0.0); return mk(0.0, 0.0); }
-            double d = eps[i] - eps[o + a];
-            c128 e = mk(S1[i * v + a].x / d, S1[i * v + a].y / d);
-            U[i * v + a] = cadd(t1[i * v + a], e);
-            return e;
-        });
-        c128 *E2 = E + ov, *U2 = U + ov;
-        launch_fill(c->st, E2, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
-            int2 ij = po[IJ], ab = pv[AB];
-            double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
-            c128 s = S2[IJ * vv + AB];
-            c128 e = mk(s.x / d, s.y / d);
-            U2[IJ * vv + AB] = cadd(t2p[IJ * vv + AB], e);
-            return e;
-        });
-    }
-    // Gram row of the new error vector against every stored one: Re <e_new | e_l>
-    std::vector<int> order = c->diis_order;
-    if (nd > 0) {
-        // the slot being overwritten leaves the subspace
-        for (size_t k = 0; k < order.size(); k++)
-            if (order[k] == slot) { order.erase(order.begin() + k); break; }
-        order.push_back(slot);
-    } else {
-        order.assign(1, 0);
-    }
-    const int m = (int)order.size();
-    CCSD_CUDA_TRY(cudaMemsetAsync(c->red, 0, 16 * sizeof(double), c->st));
-    for (int k = 0; k < m; k++)
-        launch_redot(c->st, E, c->diis_e + (int64_t)order[k] * nvec, nvec, c->red + k);
-    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host, c->red, 16 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
-    CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
-    for (int k = 0; k < m; k++) {
-        c->gram[slot * 13 + order[k]] = c->red_host[k];
-        c->gram[order[k] * 13 + slot] = c->red_host[k];
-    }
-    double snorm = sqrt(c->red_host[m - 1] > 0 ? c->red_host[m - 1] : 0.0);
-    int status = CCSD_OK;
-    // DIIS (reading G13): bordered Pulay system on the last m pairs, real coefficients
-    std::vector<double> coef(m, 0.0);
-    int mm = m;
-    if (nd > 0 && m >= 2) {
-        for (;;) {
-            int dim = mm + 1;
-            std::vector<double> A(dim * dim, 0.0), rhs(dim, 0.0);
-            for (int a = 0; a < mm; a++)
-                for (int b = 0; b < mm; b++) A[a * dim + b] = c->gram[order[m - mm + a] * 13 + order[m - mm + b]];
-            for (int a = 0; a < mm; a++) { A[a * dim + mm] = -1.0; A[mm * dim + a] = -1.0; }
-            rhs[mm] = -1.0;
-            if (solve_small(A, rhs, dim) == 0) {
-                for (int a = 0; a < mm; a++) coef[m - mm + a] = rhs[a];
-                break;
-            }
-            mm--;
-            if (mm < 1) { status = CCSD_ESINGULAR; coef.assign(m, 0.0); coef[m - 1] = 1.0; break; }
-        }
-    } else {
-        coef[m - 1] = 1.0;
-    }
-    // t = sum_l coef_l u_l
-    {
-        DiisCombo combo;
-        combo.m = m;
-        for (int k = 0; k < m; k++) { combo.c[k] = coef[k]; combo.u[k] = c->diis_u + (int64_t)order[k] * nvec; }
-        launch_combine(c->st, combo, c->t1, c->t2p, ov, nvec);
-    }
-    if (nd > 0) {
-        c->diis_order = order;
-        c->diis_next = (slot + 1) % nd;
-        if (c->diis_count < nd) c->diis_count++;
-    }
+    // Jacobi step (reading G12) + DIIS (reading G13), all on the device: the Gram row is reduced, the bordered
+    // Pulay system solved and the amplitudes recombined without a host round trip (reduce.cuh)
+    launch_jacobi_diis(c->st, c->diis, c->o, c->v, c->S1, c->S2p, c->t1, c->t2p, c->eps, c->po, c->pv, c->opt.ccd);
+    c->have_residual = false;       // the intermediates of this residual belong to the amplitudes before the update
+    c->tau_valid = false;
     tick(c, 15);
     CCSD_TRY(energy_async(c, c->red + 32));
     tick(c, 16);
+    // the iteration's only read-back: E (2 doubles) and ||S/D||^2, singular flag (2 doubles)
     CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 32, c->red + 32, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 34, c->diis.info, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
     CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
     if (e_re) *e_re = c->red_host[32];
     if (e_im) *e_im = c->red_host[33];
-    if (step_norm) *step_norm = snorm;
+    if (step_norm) *step_norm = sqrt(c->red_host[34] > 0 ? c->red_host[34] : 0.0);
     if (c->timing) {
         for (int k = 0; k < CCSD_NSTEPS; k++) cudaEventElapsedTime(&c->step_ms[k], c->ev[k], c->ev[k + 1]);
     }
     CCSD_CUDA_TRY(cudaGetLastError());
-    return status;
+    return c->red_host[35] != 0.0 ? CCSD_ESINGULAR : CCSD_OK;
 }
 
 int ccsd_solve(ccsd_ctx* c, double tol, int max_iterations, int* iterations, double* e_re, double* e_im, double* step_norm)
@@ -1353,8 +1356,9 @@ int ccsd_set_amplitudes(ccsd_ctx* c, const ccsd_c128* t1, const ccsd_c128* t2p, 
     if (!c) return CCSD_ESTATE;
     if (t1) dcopy(c->st, c->t1, reinterpret_cast<const c128*>(t1), c->ov);
     if (t2p) dcopy(c->st, c->t2p, reinterpret_cast<const c128*>(t2p), c->oo * c->vv);
-    if (reset_diis) { c->diis_count = 0; c->diis_next = 0; c->diis_order.clear(); }
+    if (reset_diis) c->diis.reset();
     c->have_residual = false;
+    c->tau_valid = false;
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -1594,7 +1598,7 @@ static int trip_gemm(ccsd_ctx* c, const TripWs& w, const TripLoader& ld0, const 
 static TripData trip_data(const ccsd_ctx* c)
 {
     TripData d;
-    d.t1 = c->t1; d.t2p = c->t2p; d.Voovv_p = c->Voovv_p; d.f = c->f; d.eps = c->eps;
+    d.t1 = c->t1; d.t2p = c->t2p; d.Voovv_p = c->Voovv_p; d.f = c->f; d.eps = c->eps0;   // unshifted
     d.o = c->o; d.v = c->v; d.n = c->n; d.vv = c->vv;
     return d;
 }
@@ -1667,7 +1671,7 @@ int ccsd_triples_range(ccsd_ctx* c, int64_t first_triple, int64_t ntriples, doub
         trip_energy_kernel<<<dim3((unsigned)(v - 2), (unsigned)count), TRIP_THREADS, 0, st>>>(d, w.Mcbuf, c->vv * v, w.ijk + first,
                                                                                            c->pv, w.partials);
         trip_reduce_kernel<<<1, 256, 0, st>>>(w.partials, (int64_t)count * (v - 2), w.acc);
-        g_launches += 2;
+        count_launches(2);
         if (c->timing) {
             cudaEventRecord(e2, st);
             CCSD_CUDA_TRY(cudaEventSynchronize(e2));
@@ -1715,7 +1719,7 @@ int ccsd_triples_block(ccsd_ctx* c, int i, int j, int k, ccsd_c128* Wbar, ccsd_c
     if (Ybar) CCSD_CUDA_TRY(cudaMemsetAsync(Ybar, 0, bytes, st));
     trip_dense_kernel<<<(unsigned)(c->v - 2), TRIP_THREADS, 0, st>>>(trip_data(c), w.Mcbuf, c->pv, i, j, k, reinterpret_cast<c128*>(Wbar),
                                                             reinterpret_cast<c128*>(Zbar), reinterpret_cast<c128*>(Ybar));
-    g_launches++;
+    count_launches(1);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -1750,8 +1754,7 @@ int ccsd_lambda_init(ccsd_ctx* c, void* workspace, size_t workspace_bytes)
     LambdaState* L = c->lam;
     lambda_carve(c, static_cast<char*>(workspace), L, &need);
     L->ready = false;
-    L->diis_count = L->diis_next = L->norder = 0;
-    memset(L->gram, 0, sizeof(L->gram));
+    L->diis.reset();
     CCSD_TRY(lambda_build_hbar(c, L));
     {   // start: lambda = conj(t) (first order: lambda^{ij}_{ab} = <ij||ab>/D = conj t^{ab}_{ij}; reading G23)
         const c128 *t1 = c->t1, *t2p = c->t2p;
@@ -1810,7 +1813,7 @@ int ccsd_set_lambda(ccsd_ctx* c, const ccsd_c128* l1, const ccsd_c128* l2p, int 
     if (!c || !c->lam || !c->lam->ready) return CCSD_ESTATE;
     if (l1) dcopy(c->st, c->lam->l1, reinterpret_cast<const c128*>(l1), c->ov);
     if (l2p) dcopy(c->st, c->lam->l2p, reinterpret_cast<const c128*>(l2p), c->oo * c->vv);
-    if (reset_diis) { c->lam->diis_count = c->lam->diis_next = c->lam->norder = 0; }
+    if (reset_diis) c->lam->diis.reset();
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -1829,7 +1832,7 @@ int ccsd_expectation(ccsd_ctx* c, const ccsd_c128* D_, const ccsd_c128* O_, doub
     if (!c || !D_ || !O_) return CCSD_ESTATE;
     const c128 *D = reinterpret_cast<const c128*>(D_), *O = reinterpret_cast<const c128*>(O_);
     CCSD_CUDA_TRY(cudaMemsetAsync(c->red + 50, 0, 2 * sizeof(double), c->st));
-    launch_reduce(c->st, (int64_t)c->n * c->n, c->red + 50, 1, [=] __device__(int64_t x) { return cmul(O[x], D[x]); });
+    launch_reduce(c->st, c->diis.scratch, (int64_t)c->n * c->n, c->red + 50, 1, [=] __device__(int64_t x) { return cmul(O[x], D[x]); });
     CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 50, c->red + 50, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
     CCSD_CUDA_TRY(cudaStreamSynchronize(c->st));
     if (re) *re = c->red_host[50];
@@ -1946,7 +1949,7 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
     case CCSD_TERM_TAU: {
         pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(po, o);
         pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(pv, v);
-        g_launches += 2;
+        count_launches(2);
         if (accumulate) return CCSD_EINVAL;
         build_tau(st, out, in0, in1, o, v, po, pv, nullptr);
         CCSD_CUDA_TRY(cudaGetLastError());
@@ -1964,7 +1967,7 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in_, ccs
     case CCSD_TERM_RING: {
         pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(po, o);
         pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(pv, v);
-        g_launches += 2;
+        count_launches(2);
         c128* Hm = w.take<c128>(ov * ov);
         c128* T2r = w.take<c128>(ov * ov);
         c128* Xr = w.take<c128>(ov * ov);
@@ -2059,6 +2062,13 @@ int ccsd_enable_step_timing(ccsd_ctx* c, int enable)
     if (enable && !c->ev[0])
         for (int k = 0; k <= CCSD_NSTEPS; k++) CCSD_CUDA_TRY(cudaEventCreate(&c->ev[k]));
     c->timing = enable ? 1 : 0;
+    return CCSD_OK;
+}
+
+int ccsd_get_init_stats(ccsd_ctx* c, double stats[CCSD_NINIT_STATS])
+{
+    if (!c || !stats) return CCSD_ESTATE;
+    for (int k = 0; k < CCSD_NINIT_STATS; k++) stats[k] = c->init_stats[k];
     return CCSD_OK;
 }
 

@@ -1,13 +1,22 @@
 // Shared device/host helpers of the CCSD library (product code; shares nothing with oracle/).
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <cstdint>
 #include <cstdio>
+
+constexpr int CCSD_MAX_DEVICES = 64;   // per-device caches of function attributes
 
 typedef double2 c128;  // (re, im) == ccsd_c128 == torch.complex128
 
 extern thread_local char g_cuda_err[256];
-extern long long g_launches;
+extern std::atomic<long long> g_launches;   // kernels launched by this library (all contexts, all host threads)
+extern thread_local long long t_launch_tally;   // ... by this host thread (counts the kernel nodes of a stream capture)
+static inline void count_launches(long long n)
+{
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+    t_launch_tally += n;
+}
 
 #define CCSD_CUDA_TRY(expr)                                                                      \
     do {                                                                                         \

@@ -46,8 +46,8 @@ static int contract_intermediate(int term, int o, int v, const c128* const* in, 
     const TcScratch& sc = W.sc;
     const int n = o + v;
     const int64_t O = o, V = v, oo = O * (O - 1) / 2, vv = V * (V - 1) / 2;
-    if (oo > 0) { pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o); g_launches++; }
-    if (vv > 0) { pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v); g_launches++; }
+    if (oo > 0) { pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o); count_launches(1); }
+    if (vv > 0) { pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v); count_launches(1); }
     // which inputs are which (see include/ccsd.h)
     const c128 *f = nullptr, *oovv = nullptr, *vovv = nullptr, *ooov = nullptr, *oooo = nullptr, *vovo = nullptr, *t1 = nullptr, *t2p = nullptr;
     switch (term) {
@@ -153,7 +153,7 @@ static int contract_residual_term(int term, int o, int v, const c128* const* in,
         if (!in[q]) return CCSD_EINVAL;
     pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o);
     pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v);
-    g_launches += 2;
+    count_launches(2);
     if (term == CCSD_TERM_S1_RESIDUAL) {
         const c128 *f = in[0], *Hvv = in[1], *Hoo = in[2], *Hov = in[3], *vovv = in[4], *ooov = in[5], *vovo = in[6], *t1 = in[7], *t2p = in[8];
         build_tau(st, W.taup, t1, t2p, o, v, W.po, W.pv, nullptr);                 // eq 23
@@ -212,8 +212,8 @@ static int contract_residual_term(int term, int o, int v, const c128* const* in,
 // ENERGY and JACOBI_UPDATE stream over the packed amplitudes; their workspace is the pair tables, tau and eps only.
 struct StreamWs {
     int2 *po, *pv;
-    c128* taup;
-    double* eps;
+    c128 *taup, *evec;
+    double *eps, *scratch;
 };
 static void stream_carve(int o_, int v_, char* base, StreamWs* W, size_t* total)
 {
@@ -222,7 +222,9 @@ static void stream_carve(int o_, int v_, char* base, StreamWs* W, size_t* total)
     W->po = w.take<int2>(oo);
     W->pv = w.take<int2>(vv);
     W->taup = w.take<c128>(oo * vv);
+    W->evec = w.take<c128>(o * v + oo * vv);
     W->eps = w.take<double>(o + v);
+    W->scratch = w.take<double>(RED_SCRATCH_DOUBLES);
     *total = w.off;
 }
 static int contract_stream_term(int term, int o, int v, const c128* const* in, int nin, c128* out, cudaStream_t st, char* workspace,
@@ -237,30 +239,21 @@ static int contract_stream_term(int term, int o, int v, const c128* const* in, i
         if (!in[q]) return CCSD_EINVAL;
     pair_table_kernel<<<(unsigned)((oo + 255) / 256), 256, 0, st>>>(W.po, o);
     pair_table_kernel<<<(unsigned)((vv + 255) / 256), 256, 0, st>>>(W.pv, v);
-    g_launches += 2;
-    if (term == CCSD_TERM_ENERGY) {          // E = sum_ia f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij}
+    count_launches(2);
+    if (term == CCSD_TERM_ENERGY) {          // E = sum_ia f_ia t^a_i + sum_{i<j,a<b} <ij||ab> tau^{ab}_{ij}: the kernel ccsd_iterate uses
         const c128 *f = in[0], *oovv = in[1], *t1 = in[2], *t2p = in[3];
-        build_tau(st, W.taup, t1, t2p, o, v, W.po, W.pv, nullptr);
-        CCSD_CUDA_TRY(cudaMemsetAsync(out, 0, sizeof(c128), st));
-        launch_energy(st, f, n, o, v, t1, oovv, W.taup, oo * vv, reinterpret_cast<double*>(out));
-    } else if (term == CCSD_TERM_JACOBI_UPDATE) {   // u = t + S / D, D from eps_p = Re f_pp (+ level shift on the virtuals)
-        const c128 *f = in[0], *t1 = in[1], *t2p = in[2], *S1 = in[3], *S2 = in[4];
-        double* eps = W.eps;
-        eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(f, eps, n, o, level_shift);
-        g_launches++;
-        const int2 *po = W.po, *pv = W.pv;
-        launch_fill(st, out, O, V, V, 0, [=] __device__(int64_t i, int64_t a) {
-            if (ccd) return mk(0.0, 0.0);
-            const double d = eps[i] - eps[o + a];
-            const c128 s = S1[i * v + a];
-            return cadd(t1[i * v + a], mk(s.x / d, s.y / d));
-        });
-        launch_fill(st, out + O * V, oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
-            const int2 ij = po[IJ], ab = pv[AB];
-            const double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
-            const c128 s = S2[IJ * vv + AB];
-            return cadd(t2p[IJ * vv + AB], mk(s.x / d, s.y / d));
-        });
+        launch_energy_tau(st, W.scratch, f, n, o, v, t1, t2p, oovv, W.taup, nullptr, W.po, W.pv, reinterpret_cast<double*>(out));
+    } else if (term == CCSD_TERM_JACOBI_UPDATE) {   // u = t + S / D, D from eps_p = Re f_pp (+ level shift on the virtuals):
+        const c128 *f = in[0], *t1 = in[1], *t2p = in[2], *S1 = in[3], *S2 = in[4];     // the kernel ccsd_iterate uses, no DIIS
+        eps_kernel<<<(n + 127) / 128, 128, 0, st>>>(f, W.eps, nullptr, n, o, level_shift);
+        count_launches(1);
+        const VecTiles T = vec_tiles(o, v);
+        JacobiArgs ja;
+        ja.T = T; ja.S1 = S1; ja.S2 = S2; ja.t1 = t1; ja.t2p = t2p; ja.E = W.evec; ja.U = out;
+        for (int k = 0; k < DIIS_MAX; k++) ja.Eold[k] = nullptr;
+        ja.m = 1; ja.eps = W.eps; ja.po = W.po; ja.pv = W.pv; ja.ccd = ccd; ja.partials = W.scratch;
+        jacobi_multidot_kernel<<<tile_blocks(T), RED_THREADS, 0, st>>>(ja);
+        count_launches(1);
     } else {
         return CCSD_EINVAL;
     }

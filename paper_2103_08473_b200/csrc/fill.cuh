@@ -32,7 +32,7 @@ static inline void launch_fill(cudaStream_t st, c128* out, int64_t rows, int64_t
     dim3 block(bx, by);
     dim3 grid((unsigned)((rows + by - 1) / by), (unsigned)((cols + (int64_t)bx * 4 - 1) / ((int64_t)bx * 4)));
     fill_kernel<<<grid, block, 0, st>>>(out, rows, cols, ld, add, f);
-    g_launches++;
+    count_launches(1);
 }
 
 // 3M "sum plane" of a complex buffer: out[i] = Re in[i] + Im in[i]  (gemm_dmma.cuh, DmmaCfg::PL).  Streaming:
@@ -57,7 +57,7 @@ static inline void launch_sum_plane(cudaStream_t st, const c128* in, double* out
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (blocks < 1) blocks = 1;
     sum_plane_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, n);
-    g_launches++;
+    count_launches(1);
 }
 
 // pair table: tab[p] = (x, y) with x<y, p = pair_idx(x, y, m)

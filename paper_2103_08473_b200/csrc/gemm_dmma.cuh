@@ -11,11 +11,17 @@
 //     the complex element C[m0+g][n0+q]: the epilogue stores double2 directly.
 //   Two DMMAs = 8 rows x 4 complex columns x 4 complex k = 128 complex MACs = 512 real FMAs: no wasted lanes.
 //
-// Data movement: operands are staged by TMA (cp.async.bulk.tensor) into a 4-stage shared-memory ring guarded by
-// full/empty mbarriers; one producer warp issues the copies, eight consumer warps issue DMMA.  The shared-memory
-// layout is [k-group of 4 complex][row][64 bytes]: the 16-byte fragment loads of a quarter-warp cover one contiguous
-// 128-byte line, so they are bank-conflict free without swizzling; each TMA box is {4 complex} x {rows}.
-// Out-of-range rows / k are zero-filled by TMA, so ragged M, N, K need no special code in the main loop.
+// A second scheme, 3M (Karatsuba: three real products per complex product, DmmaCfg::M3), is the default; its operand
+// sums Re + Im come from TMA-staged "sum planes" where the caller provides them (DmmaCfg::PL).
+//
+// Data movement: operands are staged by TMA (cp.async.bulk.tensor) into a 3-6 stage shared-memory ring (DmmaCfg::STAGES,
+// as many 16-complex-k stages as fit 220 KB) guarded by full/empty mbarriers.  There is NO producer warp: all eight warps
+// issue DMMA, and the TMA issue for k-iteration it + STAGES - 2 is done by lane 0 of warp it % 8 (a ninth warp would cap
+// the register budget at 168 per thread and spill the 3M tiles).  The shared-memory layout is
+// [k-group of 4 complex][row][64 bytes]: the 16-byte fragment loads of a quarter-warp cover one contiguous 128-byte
+// line, so they are bank-conflict free without swizzling; each TMA box is {4 complex} x {rows} (or, with the 4-d
+// "wide" maps, one box per operand and stage).  Out-of-range rows / k are zero-filled by TMA, so ragged M, N, K need
+// no special code in the main loop.
 #pragma once
 #include <cuda.h>
 #include "gemm_simple.cuh"
@@ -463,16 +469,19 @@ template <class Cfg>
 static int launch_dmma_cfg(cudaStream_t st, const CUtensorMap& mA, const CUtensorMap& mB, const CUtensorMap& mAs,
                            const CUtensorMap& mBs, int wide, const DmmaArgs& a, dim3 grid)
 {
-    static bool configured = false;
-    if (!configured) {
+    // the dynamic shared-memory limit is a per-device attribute of the function: set once per device
+    static std::atomic<bool> configured[CCSD_MAX_DEVICES];
+    int dev = 0;
+    CCSD_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= CCSD_MAX_DEVICES || !configured[dev].load(std::memory_order_acquire)) {
         CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg, PlainLoader>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
-        configured = true;
+        if (dev >= 0 && dev < CCSD_MAX_DEVICES) configured[dev].store(true, std::memory_order_release);
     }
     PlainLoader ld;
     ld.mapA = mA; ld.mapB = mB; ld.mapAs = mAs; ld.mapBs = mBs;
     ld.wide = wide;
     gemm_dmma_kernel<Cfg, PlainLoader><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(ld, a);
-    g_launches++;
+    count_launches(1);
     return CCSD_OK;
 }
 

@@ -104,10 +104,7 @@ struct LambdaState {
     double *VT2s, *Ltps;                           // sum planes of the (vv x oo x ov) product's operands
     double* cl2s;                                  // 3M sum plane of conj(l2p)
     // DIIS (as for the amplitudes: reading G13)
-    c128 *diis_u, *diis_e;
-    int nd, diis_count, diis_next;
-    int order[12], norder;
-    double gram[13 * 13];
+    DiisRing diis;
 };
 
 static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* total)
@@ -152,10 +149,14 @@ static void lambda_carve(const ccsd_ctx* c, char* base, LambdaState* L, size_t* 
     L->T2huT = w.take<c128>(v * oo * v); L->T2ou = w.take<c128>(o * o * vv);
     L->VT2s = c->planes ? w.take<double>(vv * ov) : nullptr;
     L->Ltps = c->planes ? w.take<double>(oo * ov) : nullptr;
-    L->nd = c->opt.ndiis;
-    const int nd = L->nd > 0 ? L->nd : 1;
-    L->diis_u = w.take<c128>((int64_t)nd * c->nvec);
-    L->diis_e = w.take<c128>((int64_t)nd * c->nvec);
+    L->diis.nd = c->opt.ndiis;
+    const int nd = L->diis.nd > 0 ? L->diis.nd : 1;
+    L->diis.u = w.take<c128>((int64_t)nd * c->nvec);
+    L->diis.e = w.take<c128>((int64_t)nd * c->nvec);
+    L->diis.gram = w.take<double>(13 * 13);
+    L->diis.coef = w.take<double>(16);
+    L->diis.info = w.take<double>(4);
+    L->diis.scratch = w.take<double>(RED_SCRATCH_DOUBLES);
     *total = w.off;
 }
 
@@ -195,7 +196,7 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     const TcScratch& sc = L->sc;
     const int o = c->o, v = c->v;
     const int64_t O = o, V = v, vv = c->vv;
-    CCSD_TRY(residual(c));                                    // tau, Hov, Gvv, Goo, Am of eqs 23-31 at the current (t1, t2)
+    CCSD_TRY(residual_any(c));                                // tau, Hov, Gvv, Goo, Am of eqs 23-31 at the current (t1, t2)
     dcopy(st, L->T1, c->t1, O * V);
     unpack_pairs(st, L->T2, c->t2p, o, 1, v, 1);
     unpack_pairs(st, L->TAU, c->taup, o, 1, v, 1);
@@ -474,84 +475,13 @@ static int lambda_iterate(ccsd_ctx* c, LambdaState* L, double* step_norm)
 {
     CCSD_TRY(lambda_residual(c, L));
     cudaStream_t st = c->st;
-    const int o = c->o, v = c->v;
-    const int64_t vv = c->vv, ov = c->ov, nvec = c->nvec;
-    const int nd = L->nd;
-    const int slot = nd > 0 ? L->diis_next : 0;
-    c128* U = L->diis_u + (int64_t)slot * nvec;
-    c128* Ev = L->diis_e + (int64_t)slot * nvec;
-    {
-        const c128 *R1 = L->R1, *R2p = L->R2p, *l1 = L->l1, *l2p = L->l2p;
-        const double* eps = c->eps;
-        const int2 *po = c->po, *pv = c->pv;
-        const int ccd = c->opt.ccd;                      // CCD: the Lagrangian has no singles constraint, lambda^i_a stays zero
-        launch_fill(st, Ev, o, v, v, 0, [=] __device__(int64_t i, int64_t a) {
-            if (ccd) { U[i * v + a] = mk(0.0, 0.0); return mk(0.0, 0.0); }
-            const double d = eps[i] - eps[o + a];
-            const c128 e = mk(R1[i * v + a].x / d, R1[i * v + a].y / d);
-            U[i * v + a] = cadd(l1[i * v + a], e);
-            return e;
-        });
-        c128 *E2 = Ev + ov, *U2 = U + ov;
-        launch_fill(st, E2, c->oo, vv, vv, 0, [=] __device__(int64_t IJ, int64_t AB) {
-            const int2 ij = po[IJ], ab = pv[AB];
-            const double d = eps[ij.x] + eps[ij.y] - eps[o + ab.x] - eps[o + ab.y];
-            const c128 s = R2p[IJ * vv + AB];
-            const c128 e = mk(s.x / d, s.y / d);
-            U2[IJ * vv + AB] = cadd(l2p[IJ * vv + AB], e);
-            return e;
-        });
-    }
-    int order[13], m = 0;
-    if (nd > 0) {
-        for (int k = 0; k < L->norder; k++)
-            if (L->order[k] != slot) order[m++] = L->order[k];
-        order[m++] = slot;
-    } else {
-        order[m++] = 0;
-    }
-    CCSD_CUDA_TRY(cudaMemsetAsync(c->red, 0, 16 * sizeof(double), st));
-    for (int k = 0; k < m; k++) launch_redot(st, Ev, L->diis_e + (int64_t)order[k] * nvec, nvec, c->red + k);
-    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host, c->red, 16 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    // CCD: the Lagrangian has no singles constraint, lambda^i_a stays zero (the ccd flag of the update kernel)
+    launch_jacobi_diis(st, L->diis, c->o, c->v, L->R1, L->R2p, L->l1, L->l2p, c->eps, c->po, c->pv, c->opt.ccd);
+    CCSD_CUDA_TRY(cudaMemcpyAsync(c->red_host + 36, L->diis.info, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CCSD_CUDA_TRY(cudaStreamSynchronize(st));
-    for (int k = 0; k < m; k++) {
-        L->gram[slot * 13 + order[k]] = c->red_host[k];
-        L->gram[order[k] * 13 + slot] = c->red_host[k];
-    }
-    const double snorm = sqrt(c->red_host[m - 1] > 0 ? c->red_host[m - 1] : 0.0);
-    std::vector<double> coef(m, 0.0);
-    int status = CCSD_OK;
-    if (nd > 0 && m >= 2) {
-        int mm = m;
-        for (;;) {
-            const int dim = mm + 1;
-            std::vector<double> A(dim * dim, 0.0), rhs(dim, 0.0);
-            for (int a = 0; a < mm; a++)
-                for (int b = 0; b < mm; b++) A[a * dim + b] = L->gram[order[m - mm + a] * 13 + order[m - mm + b]];
-            for (int a = 0; a < mm; a++) { A[a * dim + mm] = -1.0; A[mm * dim + a] = -1.0; }
-            rhs[mm] = -1.0;
-            if (solve_small(A, rhs, dim) == 0) {
-                for (int a = 0; a < mm; a++) coef[m - mm + a] = rhs[a];
-                break;
-            }
-            if (--mm < 1) { status = CCSD_ESINGULAR; coef.assign(m, 0.0); coef[m - 1] = 1.0; break; }
-        }
-    } else {
-        coef[m - 1] = 1.0;
-    }
-    DiisCombo combo;
-    combo.m = m;
-    for (int k = 0; k < m; k++) { combo.c[k] = coef[k]; combo.u[k] = L->diis_u + (int64_t)order[k] * nvec; }
-    launch_combine(st, combo, L->l1, L->l2p, ov, nvec);
-    if (nd > 0) {
-        for (int k = 0; k < m; k++) L->order[k] = order[k];
-        L->norder = m;
-        L->diis_next = (slot + 1) % nd;
-        if (L->diis_count < nd) L->diis_count++;
-    }
-    if (step_norm) *step_norm = snorm;
+    if (step_norm) *step_norm = sqrt(c->red_host[36] > 0 ? c->red_host[36] : 0.0);
     CCSD_CUDA_TRY(cudaGetLastError());
-    return status;
+    return c->red_host[37] != 0.0 ? CCSD_ESINGULAR : CCSD_OK;
 }
 
 // eqs 58-61: D[p][q] = <0|(1+Lambda) exp(-T) a+_p a_q exp(T)|0> - delta_pq(occ), [n][n] (device), unsymmetrised (reading G24)

@@ -40,7 +40,7 @@ static int measure_fp64_peak(cudaStream_t st, double* scratch, int launches, dou
         cudaEventElapsedTime(&ms, e0, e1);
         double tf = 16.0 * 8 * (double)iters * 512.0 * nsm / (ms * 1e-3) * 1e-12;
         if (tf > best) best = tf;
-        g_launches++;
+        count_launches(1);
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);

@@ -76,7 +76,7 @@ static int permute_into(cudaStream_t st, c128* out, const char* oidx, const TVie
     int64_t blocks = (a.total + 255) / 256;
     if (blocks > 148 * 32) blocks = 148 * 32;
     permute_kernel<<<(unsigned)blocks, 256, 0, st>>>(out, in.p, a, alpha, add, conj);
-    g_launches++;
+    count_launches(1);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }

@@ -155,7 +155,7 @@ static inline int launch_transpose2d_ld(cudaStream_t st, const c128* in, int64_t
     t.ox = ld_out; t.o1 = 0; t.o2 = 0;
     t.conj = conj;
     CCSD_TRY(launch_tr4(st, in, out, t));
-    g_launches++;
+    count_launches(1);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -247,7 +247,7 @@ static inline int launch_transpose4d(cudaStream_t st, const c128* in, c128* out,
         t.conj = conj;
         CCSD_TRY(launch_tr4(st, in, out, t));
     }
-    g_launches++;
+    count_launches(1);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }

@@ -63,13 +63,15 @@ struct TripLoader {
 template <class Cfg>
 static int launch_trip_cfg(cudaStream_t st, const TripLoader& ld, const DmmaArgs& a, dim3 grid)
 {
-    static bool configured = false;
-    if (!configured) {
+    static std::atomic<bool> configured[CCSD_MAX_DEVICES];   // per device, as in launch_dmma_cfg
+    int dev = 0;
+    CCSD_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= CCSD_MAX_DEVICES || !configured[dev].load(std::memory_order_acquire)) {
         CCSD_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg, TripLoader>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
-        configured = true;
+        if (dev >= 0 && dev < CCSD_MAX_DEVICES) configured[dev].store(true, std::memory_order_release);
     }
     gemm_dmma_kernel<Cfg, TripLoader><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(ld, a);
-    g_launches++;
+    count_launches(1);
     return CCSD_OK;
 }
 

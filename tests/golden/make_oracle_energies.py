@@ -4,6 +4,8 @@
 
 Calls only oracle/ and the shared input generator.  The file lists E (Re, Im) and ||S/D||_2 of the MP2 start and of
 every iteration with DIIS(6) (reading G13), to be compared with the CUDA library's ccsd_iterate by the GPU tests.
+The wall seconds of every REAL oracle iteration are appended to tests/golden/oracle_iteration_seconds.txt (the
+genuine full-iteration CPU times bench.py quotes beside its slab-scaled cpu_baseline numbers).
 """
 import os
 import sys
@@ -37,12 +39,24 @@ def main():
     lines.append(f"0 {e.real!r} {e.imag!r} nan")
     print(lines[-1], f"(setup {time.time() - t0:.0f} s)", flush=True)
     flush()
+    setup_s = time.time() - t0
+    secs = []
     for it in range(1, niter + 1):
         t1 = time.time()
         e, sn = oc.iterate()
+        secs.append(time.time() - t1)
         lines.append(f"{it} {e.real!r} {e.imag!r} {sn!r}")
-        print(lines[-1], f"({time.time() - t1:.0f} s)", flush=True)
+        print(lines[-1], f"({secs[-1]:.0f} s)", flush=True)
         flush()
+    if secs:
+        rec = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_iteration_seconds.txt")
+        new = not os.path.exists(rec)
+        with open(rec, "a") as fh:
+            if new:
+                fh.write("# wall seconds of real full oracle iterations (OracleCCSD.iterate, restricted-sum mode), written by\n"
+                         "# tests/golden/make_oracle_energies.py; columns: config  host_threads  iterations  median_seconds_per_iteration"
+                         "  setup_seconds(Fock + six integral classes)  host\n")
+            fh.write(f"{cfg} {num_threads()} {len(secs)} {sorted(secs)[len(secs) // 2]:.1f} {setup_s:.1f} {os.uname().nodename}\n")
 
 
 if __name__ == "__main__":

@@ -36,7 +36,7 @@ def test_defaults_and_strerror(lib):
     from paper_2103_08473_b200.binding import Options
     o = Options()
     lib.ccsd_default_options(ctypes.byref(o))
-    assert (o.ndiis, o.level_shift, o.gemm_mode, o.ccd, o.cc2, o.direct_ladder) == (6, 0.0, 0, 0, 0, 0)
+    assert (o.ndiis, o.level_shift, o.gemm_mode, o.ccd, o.cc2, o.direct_ladder, o.graph) == (6, 0.0, 0, 0, 0, 0, 1)
     assert lib.ccsd_strerror(0) == b"ok"
     assert b"CUDA" in lib.ccsd_strerror(3)
     assert lib.ccsd_step_name(6) == b"pp_ladder" and lib.ccsd_step_name(99) == b""

@@ -256,3 +256,50 @@ def test_sampled_evaluators_from_B_equal_the_plain_loop_oracle():
     k, l = rng.integers(0, o, (2, 30))
     assert np.abs(orc.g_samples(inp.B, k, l, o + c, o + d) - oc.oovv[k, l, c, d]).max() < 1e-15
     assert np.abs(orc.g_samples(inp.B, o + a, k, o + c, o + d) - oc.vovv[a, k, c, d]).max() < 1e-15
+
+
+def test_slab_entry_points_tile_the_full_evaluation():
+    """The range / part entry points bench.py times (slabs of the BASELINE-size terms) are the same loop nests: evaluated
+    slab by slab they reproduce the full evaluation bit for bit, in both sum modes, also through from_blocks with only a
+    row block of <ab||cd> resident."""
+    o, v = 4, 7
+    inp = ci.make_inputs(o, v, 9, seed=71, b_scale=0.2, f_offdiag=0.1)
+    t1, t2 = _random_unpacked_amplitudes(o, v, 72, 0.2)
+    for restricted in (False, True):
+        full = OracleCCSD(inp.h, inp.B, o, v, restricted=restricted)
+        full.set_amplitudes(t1, t2)
+        S1, S2 = full.residual()
+        S1, S2 = S1.copy(), S2.copy()
+        terms = {name: full.s2_term(name).copy() for name in full.TERMS}
+        part = OracleCCSD(inp.h, inp.B, o, v, restricted=restricted)
+        part.set_amplitudes(t1, t2)
+        part.build_tau()
+        for name, extent in zip(part.PARTS, (v, o, o, v, o, o)):
+            for lo in range(0, extent, 3):
+                part.intermediates_part(name, lo, min(extent, lo + 3))
+        for name in ("Hvv", "Gvv", "Hoo", "Goo", "Hov", "Hvovo", "C", "A"):
+            assert np.array_equal(getattr(part, name), getattr(full, name)), name
+        for name in part.TERMS:
+            out = np.zeros_like(S2)
+            for i0 in range(0, o, 2):
+                for a0 in range(0, v, 3):
+                    part.s2_term_range(name, i0, min(o, i0 + 2), a0, min(v, a0 + 3), out=out)
+            if name == "ring":      # the ring antisymmetrises a buffer that holds the slab only: slabs ADD up
+                out = np.zeros_like(S2)
+                for i0 in range(0, o, 2):
+                    for a0 in range(0, v, 3):
+                        out += part.s2_term_range(name, i0, min(o, i0 + 2), a0, min(v, a0 + 3), out=np.zeros_like(S2))
+                assert np.abs(out - terms[name]).max() < 1e-14
+            else:
+                assert np.array_equal(out, terms[name]), name
+        for i0 in range(0, o, 3):
+            part.s1_range(i0, min(o, i0 + 3))
+        assert np.array_equal(part.S1, S1)
+    # from_blocks with rows [2, 5) of <ab||cd> only: the pp-ladder slab of those rows
+    rows = np.ascontiguousarray(full.vvvv[2:5])
+    fb = OracleCCSD.from_blocks(o, v, full.f, full.oooo, full.ooov, full.oovv, full.vovo, full.vovv, rows, 2, restricted=True)
+    fb.set_amplitudes(t1, t2)
+    fb.build_tau()
+    out = fb.s2_term_range("pp_ladder", 0, o, 2, 5, out=np.zeros_like(S2))
+    ref = terms["pp_ladder"]
+    assert np.array_equal(out[:, :, 2:5, :][:, :, :, 3:], ref[:, :, 2:5, :][:, :, :, 3:])
