@@ -62,6 +62,16 @@ typedef struct {
                            afterwards; 0 = always launch directly.  Capture needs a stream created by the caller: on the
                            legacy / per-thread default streams (cuda_stream = 0, 1 or 2), and while step timing is enabled,
                            the launches are issued directly whatever this says */
+    int shard_rank;     /* slab sharding of the iteration over several GPUs (one process and one context per GPU, */
+    int shard_world;    /* every rank gets the same h, B and holds the same amplitudes): with shard_world = P > 1 the context
+                           of rank r builds and stores only its 1/P of the rows of the packed <ab||cd>, and ccsd_residual
+                           evaluates only its slab of every large contraction of eqs 29-32 (disjoint output rows: the (a<b)
+                           rows of the pp-ladder, the (a,i) rows of H^{ak}_{ci} and of the ring product, the (b,k) rows of C),
+                           adding them into an S2 that is zero elsewhere.  The caller sums S2 over the ranks (ONE all-reduce of
+                           the packed S2 per iteration; ccsd_shard_info locates the buffer) and then calls ccsd_update, which
+                           is replicated.  S1 and the small intermediates are replicated too.  The library issues no
+                           collective itself.  Defaults 0, 1.  Not with cc2; ccsd_iterate / ccsd_solve, CCSD_T_VVVV and the
+                           Lambda entry points return CCSD_EINVAL in a sharded context */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */
@@ -90,6 +100,27 @@ int ccsd_init(ccsd_ctx** ctx, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
  * Errors: CCSD_ESTATE (no context), CCSD_ESINGULAR (DIIS system singular even with one vector), CCSD_ECUDA.
  */
 int ccsd_iterate(ccsd_ctx* ctx, double* e_re, double* e_im, double* step_norm);
+
+/*
+ * The second half of ccsd_iterate on its own: Jacobi step + DIIS + energy from the residuals (S1, S2) held by the context
+ * (those of the last ccsd_residual, after the caller's all-reduce of S2 in a sharded run: ccsd_residual; all-reduce;
+ * ccsd_update is one iteration).  HOST outputs as ccsd_iterate.  CCSD_ESTATE without a residual of the current amplitudes.
+ */
+int ccsd_update(ccsd_ctx* ctx, double* e_re, double* e_im, double* step_norm);
+/*
+ * Where this context's slab lies and where the caller's collective has to act.  HOST out-pointer, info[] =
+ * { shard_rank, shard_world, a_lo, a_hi (virtual-index slab of the (ov)^3 / C rows), w_lo, w_hi (packed (a<b) rows of
+ *   <ab||cd> this rank stores and contracts), ij_lo, ij_hi (packed (i<j) rows of the row-wise small terms),
+ *   byte offset of S2 [(i<j)][(a<b)] in the workspace handed to ccsd_init, its ccsd_c128 element count,
+ *   byte offset of S1 [i][a], its element count }.
+ */
+enum { CCSD_NSHARD_INFO = 12 };
+int ccsd_shard_info(ccsd_ctx* ctx, int64_t info[CCSD_NSHARD_INFO]);
+/* The same ranges without a context (host arithmetic only, no CUDA device needed): ranges[] = { a_lo, a_hi, w_lo, w_hi,
+ * ij_lo, ij_hi, wa_lo, wa_hi } of rank `rank` of `world`; [wa_lo, wa_hi) is the range of the first virtual index whose
+ * pairs (a, b > a) are the packed rows [w_lo, w_hi).  Over rank = 0..world-1 each family of ranges tiles its index range
+ * exactly once.  CCSD_EINVAL for world > nvir. */
+int ccsd_shard_ranges(int nocc, int nvir, int rank, int world, int64_t ranges[8]);
 
 /*
  * ccsd_iterate until ||S/D||_2 < tol and |E - E_previous| < tol, or max_iterations (the paper's .TCONVERG 1e-9 and

@@ -19,9 +19,10 @@ from __future__ import annotations
 
 import ctypes
 import os
-import subprocess
 
 import numpy as np
+
+from oracle._build import compile_oracle
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
@@ -33,10 +34,7 @@ C128 = np.complex128
 
 def build(force: bool = False) -> str:
     """Compile ccsd_oracle.c -> liboracle.so (gcc -O2 -fopenmp, no -ffast-math)."""
-    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < os.path.getmtime(_SRC_PATH):
-        cmd = ["gcc", "-O2", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC", "-o", _LIB_PATH, _SRC_PATH]
-        subprocess.check_call(cmd)
-    return _LIB_PATH
+    return compile_oracle(_SRC_PATH, _LIB_PATH, force)
 
 
 class _Sys(ctypes.Structure):
@@ -53,8 +51,7 @@ class _Inter(ctypes.Structure):
 def lib():
     global _lib
     if _lib is None:
-        build()
-        _lib = ctypes.CDLL(_LIB_PATH)
+        _lib = ctypes.CDLL(build())
         _lib.oracle_num_threads.restype = ctypes.c_int
     return _lib
 

@@ -12,9 +12,10 @@ from __future__ import annotations
 
 import ctypes
 import os
-import subprocess
 
 import numpy as np
+
+from oracle._build import compile_oracle
 
 from oracle.ccsd_oracle import C128, _p
 
@@ -25,17 +26,13 @@ _lib = None
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < os.path.getmtime(_SRC_PATH):
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC", "-o", _LIB_PATH,
-                               _SRC_PATH])
-    return _LIB_PATH
+    return compile_oracle(_SRC_PATH, _LIB_PATH, force)
 
 
 def lib():
     global _lib
     if _lib is None:
-        build()
-        _lib = ctypes.CDLL(_LIB_PATH)
+        _lib = ctypes.CDLL(build())
     return _lib
 
 

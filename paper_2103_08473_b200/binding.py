@@ -28,7 +28,8 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_last_cuda_error", "ccsd_triples_workspace_bytes", "ccsd_triples", "ccsd_get_triples_times",
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_solve", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
-           "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation"]
+           "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation", "ccsd_update", "ccsd_shard_info",
+           "ccsd_shard_ranges"]
 
 
 class CCSDError(RuntimeError):
@@ -42,7 +43,8 @@ class CCSDError(RuntimeError):
 
 class Options(ctypes.Structure):
     _fields_ = [("ndiis", ctypes.c_int), ("level_shift", ctypes.c_double), ("gemm_mode", ctypes.c_int),
-                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int), ("graph", ctypes.c_int)]
+                ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int), ("graph", ctypes.c_int),
+                ("shard_rank", ctypes.c_int), ("shard_world", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -72,6 +74,9 @@ def load_library():
         lib.ccsd_iterate.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_energy.argtypes = [vp] + [ctypes.POINTER(dbl)] * 2
         lib.ccsd_residual.argtypes = [vp]
+        lib.ccsd_update.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
+        lib.ccsd_shard_info.argtypes = [vp, ctypes.POINTER(i64)]
+        lib.ccsd_shard_ranges.argtypes = [ctypes.c_int] * 4 + [ctypes.POINTER(i64)]
         lib.ccsd_lambda_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_lambda_init.argtypes = [vp, vp, ctypes.c_size_t]
         lib.ccsd_lambda_iterate.argtypes = [vp, ctypes.POINTER(dbl)]
@@ -178,6 +183,13 @@ def _dev_c128(torch, x):
     return x.to(device="cuda", dtype=torch.complex128).contiguous()
 
 
+def shard_ranges(nocc: int, nvir: int, rank: int, world: int) -> dict:
+    """ccsd_shard_ranges (host arithmetic only): the slab of rank `rank` of `world`."""
+    arr = (ctypes.c_int64 * 8)()
+    _check(load_library().ccsd_shard_ranges(int(nocc), int(nvir), int(rank), int(world), arr), "ccsd_shard_ranges")
+    return dict(zip(("a_lo", "a_hi", "w_lo", "w_hi", "ij_lo", "ij_hi", "wa_lo", "wa_hi"), (int(x) for x in arr)))
+
+
 def launch_count(reset: bool = False) -> int:
     return int(load_library().ccsd_launch_count(1 if reset else 0))
 
@@ -199,9 +211,10 @@ def measure_fp64_peak(launches: int = 10) -> float:
     return float(out.value)
 
 
-def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True) -> Options:
+def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True,
+             shard=(0, 1)) -> Options:
     return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)),
-                   int(bool(graph)))
+                   int(bool(graph)), int(shard[0]), int(shard[1]))
 
 
 class CCSD:
@@ -215,7 +228,8 @@ class CCSD:
     """
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
-                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: bool = True, stream=None):
+                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: bool = True, stream=None,
+                 shard=None, group=None):
         torch = _torch()
         lib = load_library()
         self._lib, self._torch = lib, torch
@@ -225,7 +239,12 @@ class CCSD:
                 stream = torch.cuda.Stream()
         self.stream = stream
         self._ctx = ctypes.c_void_p(None)
-        opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder, graph)
+        # shard = (rank, world): this context evaluates rank's slab of the iteration (ccsd_options.shard_rank / shard_world);
+        # iterate() then sums the packed S2 over `group` (torch.distributed; None = the default group) between ccsd_residual
+        # and ccsd_update.  shard=None: one GPU does everything.
+        self.shard = (0, 1) if shard is None else (int(shard[0]), int(shard[1]))
+        self.group = group
+        opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder, graph, self.shard)
         self.nocc, self.nvir, self.n = int(nocc), int(nvir), int(nocc + nvir)
         self.oo = self.nocc * (self.nocc - 1) // 2
         self.vv = self.nvir * (self.nvir - 1) // 2
@@ -287,8 +306,36 @@ class CCSD:
         except Exception:
             pass
 
+    def shard_info(self) -> dict:
+        arr = (ctypes.c_int64 * 12)()
+        self._call(self._lib.ccsd_shard_info, arr, where="ccsd_shard_info")
+        keys = ("rank", "world", "a_lo", "a_hi", "w_lo", "w_hi", "ij_lo", "ij_hi", "s2_offset", "s2_elems", "s1_offset", "s1_elems")
+        return dict(zip(keys, (int(x) for x in arr)))
+
+    def s2_view(self):
+        """The context's S2 buffer [(i<j)][(a<b)] as a torch view of the workspace (no copy): what the all-reduce of a sharded
+        iteration acts on."""
+        torch = self._torch
+        info = self.shard_info()
+        off = info["s2_offset"] + ((self._ws.data_ptr() + 255) // 256 * 256 - self._ws.data_ptr())
+        return self._ws[off:off + info["s2_elems"] * 16].view(torch.complex128).view(self.oo, self.vv)
+
+    def update(self):
+        """ccsd_update: Jacobi + DIIS + energy from the residuals the context holds -> (E_corr, ||S/D||_2)."""
+        er, ei, sn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        self._call(self._lib.ccsd_update, ctypes.byref(er), ctypes.byref(ei), ctypes.byref(sn), where="ccsd_update", ok=(0, 5))
+        return complex(er.value, ei.value), sn.value
+
     def iterate(self):
-        """One CCSD iteration -> (complex E_corr of the new amplitudes, ||S/D||_2)."""
+        """One CCSD iteration -> (complex E_corr of the new amplitudes, ||S/D||_2).  In a sharded context: this rank's slab
+        of the residual, ONE all-reduce of the packed S2 over the group (on the context's stream), the replicated update."""
+        if self.shard[1] > 1:
+            from .sharding import allreduce_complex_
+            self.residual()
+            s2 = self.s2_view()
+            with self._on_stream(), self._torch.cuda.stream(self.stream):
+                allreduce_complex_(s2, self.group)
+            return self.update()
         er, ei, sn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
         self._call(self._lib.ccsd_iterate, ctypes.byref(er), ctypes.byref(ei), ctypes.byref(sn), where="ccsd_iterate", ok=(0, 5))
         return complex(er.value, ei.value), sn.value

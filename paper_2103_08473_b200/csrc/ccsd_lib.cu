@@ -141,8 +141,48 @@ static const char* k_step_names[CCSD_NSTEPS] = {"prep_permute", "fock_like", "Hv
                                                 "A_oooo", "pp_ladder", "hh_ladder+Goo", "ring_gemm", "ring_antisym",
                                                 "Vdag_t1", "Gvv_t2", "C_t1", "S1", "update_diis", "energy"};
 
+// Slab of the iteration this context evaluates (opts.shard_rank / shard_world, DESIGN "Multi-GPU"): every
+// large contraction has disjoint output rows, so rank r computes
+//   rows (a<b) in [w_lo, w_hi) of <ab||cd> x tau (pp-ladder), of the hh-ladder / G_oo term and of the V^dagger t1 term;
+//   rows (a, .) with a in [a_lo, a_hi) of H^{ak}_{ci} (eq 29) and of the ring product (eq 32), of C (eq 30) and of C.t1;
+//   rows (i<j) in [ij_lo, ij_hi) of the G_vv.t2 term and of the driver;
+// and adds them into ITS S2 buffer, which is zero elsewhere: the sum over the ranks (one all-reduce of the packed S2, issued
+// by the caller) is the S2 of eq 32.  S1, the small intermediates (Fock-like, A) and the update are replicated.
+// Only the rows [w_lo, w_hi) of the packed <ab||cd> are built and stored.  world = 1: the full ranges.
+struct Shard {
+    int rank, world;
+    int a_lo, a_hi;
+    int wa_lo, wa_hi;          // first-virtual-index range whose pairs (a, b > a) are the packed rows [w_lo, w_hi)
+    int64_t w_lo, w_hi, ij_lo, ij_hi;
+};
+static Shard make_shard(int rank, int world, int o, int v)
+{
+    Shard s;
+    s.rank = rank; s.world = world;
+    const int64_t oo = (int64_t)o * (o - 1) / 2, vv = (int64_t)v * (v - 1) / 2;
+    auto split = [&](int64_t n, int r) { return n * r / world; };
+    s.a_lo = (int)split(v, rank); s.a_hi = (int)split(v, rank + 1);
+    s.ij_lo = split(oo, rank); s.ij_hi = split(oo, rank + 1);
+    // boundary k: the smallest a whose pairs start at or beyond row vv k / world (pairs before a: a v - a (a + 1) / 2)
+    auto bound = [&](int k) {
+        if (k >= world) return v - 1 > 0 ? v - 1 : 0;
+        const int64_t target = split(vv, k);
+        int a = 0;
+        while (a < v - 1 && (int64_t)a * v - (int64_t)a * (a + 1) / 2 < target) a++;
+        return a;
+    };
+    s.wa_lo = bound(rank); s.wa_hi = bound(rank + 1);
+    s.w_lo = (int64_t)s.wa_lo * v - (int64_t)s.wa_lo * (s.wa_lo + 1) / 2;
+    s.w_hi = (int64_t)s.wa_hi * v - (int64_t)s.wa_hi * (s.wa_hi + 1) / 2;
+    if (s.w_hi > vv) s.w_hi = vv;
+    if (s.w_lo > s.w_hi) s.w_lo = s.w_hi;
+    return s;
+}
+
 struct LambdaState;
 struct ccsd_ctx {
+    Shard sh;
+    char* ws_base;          // the caller's workspace (ccsd_shard_info reports offsets into it)
     LambdaState* lam;       // Lambda solve in progress (ccsd_lambda_init), or null
     int o, v, n, L, Lp;
     int64_t oo, vv, ov, oop, nvec;
@@ -218,7 +258,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->eps0 = w.take<double>(n);
     c->f = w.take<c128>(n * n);
     // <ab||cd> is not stored in direct_ladder mode (rebuilt every iteration) nor in CC2 mode (its only use factorises)
-    c->W = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<c128>(vv * vv);
+    c->W = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<c128>((c->sh.w_hi - c->sh.w_lo) * vv);   // this rank's rows
     c->Vvovv_p = w.take<c128>(v * o * vv);
     c->Vvovv_u = w.take<c128>(v * v * o * v);
     c->VvovvT = w.take<c128>(o * vv * v);
@@ -309,7 +349,7 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
     if (c->planes) {
-        c->Ws = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<double>(vv * vv);
+        c->Ws = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<double>((c->sh.w_hi - c->sh.w_lo) * vv);
         c->Vvovv_ps = w.take<double>(ov * vv);
         c->Voovv_ps = w.take<double>(oo * vv);
         c->G1s = w.take<double>(ov * ov);
@@ -358,6 +398,8 @@ static void setup_dims(ccsd_ctx* c, int nocc, int nvir, int naux, const ccsd_opt
     if (opts) c->opt = *opts; else ccsd_default_options(&c->opt);
     if (c->opt.ndiis < 0) c->opt.ndiis = 0;
     if (c->opt.ndiis > DIIS_MAX) c->opt.ndiis = DIIS_MAX;
+    if (c->opt.shard_world < 1) { c->opt.shard_world = 1; c->opt.shard_rank = 0; }
+    c->sh = make_shard(c->opt.shard_rank, c->opt.shard_world, nocc, nvir);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -431,13 +473,13 @@ static void bblock(cudaStream_t st, c128* out, const c128* B, int n, int L, int 
 //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
 //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
 // absolute = true: dst is the whole matrix (row r0 of the slab goes to dst + r0 vv); false: dst holds the slab only.
-static int build_W_slab(ccsd_ctx* c, int a0, c128* dst, bool absolute, int64_t* r0_out, int64_t* nrows_out)
+static int build_W_slab(ccsd_ctx* c, int a0, int a_end, c128* dst, bool absolute, int64_t* r0_out, int64_t* nrows_out)
 {
     cudaStream_t st = c->st;
     const int v = c->v, Lp = c->Lp;
     const int64_t vv = c->vv, v2 = (int64_t)v * v;
     const int2* pv = c->pv;
-    const int na = (a0 + c->na_slab <= v) ? c->na_slab : v - a0;
+    const int na = (a0 + c->na_slab <= a_end) ? c->na_slab : a_end - a0;
     const int64_t rows = (int64_t)na * v;
     // only b > a is needed, i.e. the columns (b,d) with b >= a0 + 1 of the slab (half the columns on average)
     const int64_t col0 = (int64_t)(a0 + 1) * v, ncol = v2 - col0;
@@ -598,9 +640,9 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
         std::vector<cudaEvent_t> events;
         c->init_events = &events;
         int s = CCSD_OK;
-        for (int a0 = 0; a0 < v - 1 && vv > 0 && s == CCSD_OK; a0 += c->na_slab) {
-            int64_t r0 = 0, nrows = 0;
-            s = build_W_slab(c, a0, c->W, true, &r0, &nrows);
+        for (int a0 = c->sh.wa_lo; a0 < c->sh.wa_hi && vv > 0 && s == CCSD_OK; a0 += c->na_slab) {
+            int64_t r0 = 0, nrows = 0;      // "absolute" rows, relative to this rank's first row
+            s = build_W_slab(c, a0, c->sh.wa_hi, c->W - c->sh.w_lo * vv, true, &r0, &nrows);
         }
         c->init_events = nullptr;
         if (s == CCSD_OK && !events.empty() && cudaStreamSynchronize(st) == cudaSuccess) {
@@ -614,7 +656,7 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
         CCSD_TRY(s);
     }
     if (c->planes) {   // sum planes of the constant operands of the large GEMMs (3M, gemm_dmma.cuh)
-        if (c->W) launch_sum_plane(st, c->W, c->Ws, vv * vv);
+        if (c->W) launch_sum_plane(st, c->W, c->Ws, (c->sh.w_hi - c->sh.w_lo) * vv);
         launch_sum_plane(st, c->Vvovv_p, c->Vvovv_ps, ov * vv);
         launch_sum_plane(st, c->Voovv_p, c->Voovv_ps, oo * vv);
         launch_sum_plane(st, c->G1, c->G1s, ov * ov);
@@ -700,7 +742,9 @@ static int prep_operands(ccsd_ctx* c)
     CCSD_TRY(launch_transpose2d_ld(st, c->taup, vv, c->TT, 2 * oop, oo, vv, 0));
     CCSD_TRY(launch_transpose2d_ld(st, c->t2p, vv, c->TT + oop, 2 * oop, oo, vv, 0));
     // Xm[(a,i)][(l,d)] = 1/2 t2[l,i,a,d] + t1[l,a] t1[i,d]      (eq 29 operand)
-    launch_fill(st, c->Xm, ov, ov, ov, 0, [=] __device__(int64_t ai, int64_t ld) {
+    const int64_t xrow0 = (int64_t)c->sh.a_lo * o, xrows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;   // this rank's rows (a, i)
+    launch_fill(st, c->Xm + xrow0 * ov, xrows, ov, ov, 0, [=] __device__(int64_t row, int64_t ld) {
+        const int64_t ai = xrow0 + row;
         int a = ai / o, i = ai % o, l = ld / v, d = ld % v;
         c128 x = cscale(0.5, t2_at(t2p, l, i, a, d, o, v, vv));
         cfma(x, t1[l * v + a], t1[i * v + d]);
@@ -774,19 +818,23 @@ static int build_Hvovo(ccsd_ctx* c)
     const Env& env = c->env;
     const int o = c->o, v = c->v;
     const int64_t ov = c->ov;
-    // eq 29, stored as Hm[(a,i)][(c,k)]
-    dcopy(c->st, c->Hm, c->Vvovo_m, ov * ov);
+    // eq 29, stored as Hm[(a,i)][(c,k)]; this rank's rows: a in [a_lo, a_hi)
+    const int a0 = c->sh.a_lo, na = c->sh.a_hi - c->sh.a_lo;
+    const int64_t off = (int64_t)a0 * o * ov, rows = (int64_t)na * o;
+    if (na <= 0) { tick(c, 3); return CCSD_OK; }
+    dcopy(c->st, c->Hm + off, c->Vvovo_m + off, rows * ov);
     {   // + sum_d <ak||cd> t1[i,d]        batched over a: C_a[(c,k)][i]
-        GemmParams p = gp(ov, o, v, c->Vvovv_u, v, c->t1, v, c->Hm, 1, ov, 1.0, 1);
-        p.batch = v; p.bsA = ov * v; p.bsB = 0; p.bsC = (int64_t)o * ov;
+        GemmParams p = gp(ov, o, v, c->Vvovv_u + (int64_t)a0 * ov * v, v, c->t1, v, c->Hm + off, 1, ov, 1.0, 1);
+        p.batch = na; p.bsA = ov * v; p.bsB = 0; p.bsC = (int64_t)o * ov;
         CCSD_TRY(run_gemm(env, p));
     }
     // - sum_l <kl||ic> t1[l,a]            C[a][(i,c,k)]
-    CCSD_TRY(run_gemm(env, gp(v, (int64_t)o * ov, o, c->t1T, o, c->Vooov_b, o, c->Hm, (int64_t)o * ov, 1, -1.0, 1)));
+    CCSD_TRY(run_gemm(env, gp(na, (int64_t)o * ov, o, c->t1T + (int64_t)a0 * o, o, c->Vooov_b, o, c->Hm + off, (int64_t)o * ov, 1, -1.0, 1)));
     tick(c, 3);
     // + sum_{ld} <kl||cd> (1/2 t2[l,i,a,d] + t1[l,a] t1[i,d])       (ov x ov x ov)
-    CCSD_TRY(run_gemm(env, with_planes(gp(ov, ov, ov, c->Xm, ov, c->G1, ov, c->Hm, ov, 1, 1.0, 1), c->Xms, c->G1s)));
-    if (c->planes) launch_sum_plane(c->st, c->Hm, c->Hms, ov * ov);   // operand of the ring GEMM
+    CCSD_TRY(run_gemm(env, with_planes(gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1),
+                                       c->Xms ? c->Xms + off : nullptr, c->G1s)));
+    if (c->planes) launch_sum_plane(c->st, c->Hm + off, c->Hms + off, rows * ov);   // operand of the ring GEMM
     return CCSD_OK;
 }
 
@@ -819,27 +867,31 @@ static int build_C(ccsd_ctx* c)
     cudaStream_t st = c->st;
     const Env& env = c->env;
     const int o = c->o, v = c->v;
-    const int64_t oo = c->oo, vv = c->vv, ov = c->ov;
+    const int64_t oo = c->oo, vv = c->vv;
     const int2* po = c->po;
-    // eq 30, stored as Cm[(b,k)][(i<j)]
-    dcopy(st, c->Cm, c->Vooov_cc, ov * oo);
-    CCSD_TRY(run_gemm(env, gp(ov * o, o, v, c->Vvovo_c, v, c->t1, v, c->Y, o, 1, 1.0, 0)));
+    // eq 30, stored as Cm[(b,k)][(i<j)]; this rank's rows: b in [a_lo, a_hi)
+    const int64_t row0 = (int64_t)c->sh.a_lo * o, rows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;
+    if (rows <= 0) return CCSD_OK;
+    dcopy(st, c->Cm + row0 * oo, c->Vooov_cc + row0 * oo, rows * oo);
+    CCSD_TRY(run_gemm(env, gp(rows * o, o, v, c->Vvovo_c + row0 * o * v, v, c->t1, v, c->Y + row0 * o * o, o, 1, 1.0, 0)));
     const c128* Y = c->Y;
-    launch_fill(st, c->Cm, ov, oo, oo, 1, [=] __device__(int64_t bk, int64_t IJ) {
+    launch_fill(st, c->Cm + row0 * oo, rows, oo, oo, 1, [=] __device__(int64_t r, int64_t IJ) {
+        const int64_t bk = row0 + r;
         int2 ij = po[IJ];
         return csub(Y[(bk * o + ij.x) * o + ij.y], Y[(bk * o + ij.y) * o + ij.x]);
     });
     if (c->opt.cc2) {   // - sum_L ( Xv_bi Xo_kj - Xv_bj Xo_ki ): Q[(b,i)][(k,j)] in the buffer the linear term just released
         c128* Q = c->Y;
-        CCSD_TRY(run_gemm(env, gp(ov, (int64_t)o * o, c->Lp, c->Xv, c->Lp, c->Xo, c->Lp, Q, (int64_t)o * o, 1, 1.0, 0)));
-        launch_fill(st, c->Cm, ov, oo, oo, 1, [=] __device__(int64_t bk, int64_t IJ) {
+        CCSD_TRY(run_gemm(env, gp(c->ov, (int64_t)o * o, c->Lp, c->Xv, c->Lp, c->Xo, c->Lp, Q, (int64_t)o * o, 1, 1.0, 0)));
+        launch_fill(st, c->Cm, c->ov, oo, oo, 1, [=] __device__(int64_t bk, int64_t IJ) {
             int2 ij = po[IJ];
             const int64_t b = bk / o, k = bk % o;
             return csub(Q[((b * o + ij.y) * o + k) * o + ij.x], Q[((b * o + ij.x) * o + k) * o + ij.y]);
         });
         return CCSD_OK;
     }
-    CCSD_TRY(run_gemm(env, with_planes(gp(ov, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), c->Vvovv_ps, c->taups)));
+    CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, c->Cm + row0 * oo, oo, 1, -1.0, 1),
+                                       c->Vvovv_ps ? c->Vvovv_ps + row0 * vv : nullptr, c->taups)));
     return CCSD_OK;
 }
 
@@ -862,12 +914,13 @@ static int build_A(ccsd_ctx* c)
     return CCSD_OK;
 }
 
-// ---- the eight terms of eq 32; each ADDS into S[(i<j)][(a<b)] ---------------------------------------------------
+// ---- the eight terms of eq 32; each ADDS this rank's slab of the term into S[(i<j)][(a<b)] (struct Shard) --------------
 static int s2_driver(ccsd_ctx* c, c128* S)
 {
     const c128* V = c->Voovv_p;
-    const int64_t vv = c->vv;
-    launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) { return cconj(V[IJ * vv + AB]); });
+    const int64_t vv = c->vv, r0 = c->sh.ij_lo;
+    launch_fill(c->st, S + r0 * vv, c->sh.ij_hi - r0, vv, vv, 1,
+                [=] __device__(int64_t r, int64_t AB) { return cconj(V[(r0 + r) * vv + AB]); });
     return CCSD_OK;
 }
 static int s2_pp_ladder(ccsd_ctx* c, c128* S)
@@ -886,16 +939,17 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
         return CCSD_OK;
     }
     if (c->opt.direct_ladder) {   // integral-direct: rebuild the rows of <ab||cd> slab by slab from the factor B and contract them
-        for (int a0 = 0; a0 < c->v - 1; a0 += c->na_slab) {
+        for (int a0 = c->sh.wa_lo; a0 < c->sh.wa_hi; a0 += c->na_slab) {
             int64_t r0 = 0, nrows = 0;
-            CCSD_TRY(build_W_slab(c, a0, c->Wslab, false, &r0, &nrows));
+            CCSD_TRY(build_W_slab(c, a0, c->sh.wa_hi, c->Wslab, false, &r0, &nrows));
             if (c->planes) launch_sum_plane(c->st, c->Wslab, c->Wslabs, nrows * c->vv);
             CCSD_TRY(run_gemm(c->env, with_planes(gp(nrows, c->oo, c->vv, c->Wslab, c->vv, c->taup, c->vv, S + r0, 1, c->vv, 1.0, 1),
                                                   c->planes ? c->Wslabs : nullptr, c->taups)));
         }
         return CCSD_OK;
     }
-    return run_gemm(c->env, with_planes(gp(c->vv, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), c->Ws, c->taups));
+    const int64_t rows = c->sh.w_hi - c->sh.w_lo;      // this rank's rows of <ab||cd> (all of them for world = 1)
+    return run_gemm(c->env, with_planes(gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S + c->sh.w_lo, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
 static void fill_AG_hh(ccsd_ctx* c)
 {   // AG[(i<j)][(k<l)] = A[k,l,i,j]
@@ -919,37 +973,49 @@ static void fill_AG_goo(ccsd_ctx* c)
         return s;
     });
 }
+// the three products with M = (a<b) rows of TT run on this rank's rows [w_lo, w_hi)
 static int s2_hh_ladder(ccsd_ctx* c, c128* S)
 {   // sum_{k<l} A[k,l,i,j] tau[k,l,a,b]
     fill_AG_hh(c);
-    return run_gemm(c->env, gp(c->vv, c->oo, c->oop, c->TT, 2 * c->oop, c->AG, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+    const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
+    return run_gemm(c->env, gp(rows, c->oo, c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1));
 }
 static int s2_goo(ccsd_ctx* c, c128* S)
 {
     fill_AG_goo(c);
-    return run_gemm(c->env, gp(c->vv, c->oo, c->oop, c->TT + c->oop, 2 * c->oop, c->AG + c->oop, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+    const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
+    return run_gemm(c->env, gp(rows, c->oo, c->oop, c->TT + r0 * ld + c->oop, ld, c->AG + c->oop, ld, S + r0, 1, c->vv, 1.0, 1));
 }
 static int s2_hh_and_goo(ccsd_ctx* c, c128* S)
 {   // both in one GEMM with K = [ (k<l) of tau | (k<l) of t2 ]
     fill_AG_hh(c);
     fill_AG_goo(c);
-    return run_gemm(c->env, gp(c->vv, c->oo, 2 * c->oop, c->TT, 2 * c->oop, c->AG, 2 * c->oop, S, 1, c->vv, 1.0, 1));
+    const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
+    return run_gemm(c->env, gp(rows, c->oo, 2 * c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1));
 }
 static int s2_ring(ccsd_ctx* c, c128* S)
 {   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)];  S += P-_ij P-_ab X
+    // this rank holds the rows a in [a_lo, a_hi) of H and X: it adds the terms of P-_ij P-_ab X whose first index is one of them
     const int o = c->o, v = c->v;
     const int64_t ov = c->ov, vv = c->vv;
-    CCSD_TRY(run_gemm(c->env, with_planes(gp(ov, ov, ov, c->Hm, ov, c->T2r, ov, c->Xr, ov, 1, 1.0, 0), c->Hms, c->T2rs)));
+    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
+    const int64_t off = (int64_t)alo * o * ov, rows = (int64_t)(ahi - alo) * o;
+    if (rows > 0)
+        CCSD_TRY(run_gemm(c->env, with_planes(gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0),
+                                              c->Hms ? c->Hms + off : nullptr, c->T2rs)));
     tick(c, 9);
+    if (rows <= 0) return CCSD_OK;
     const c128* Xr = c->Xr;
     const int2 *po = c->po, *pv = c->pv;
     launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
         int2 ij = po[IJ], ab = pv[AB];
         int64_t i = ij.x, j = ij.y, a = ab.x, b = ab.y;
-        c128 s = Xr[((a * o + i) * o + j) * v + b];
-        s = csub(s, Xr[((a * o + j) * o + i) * v + b]);
-        s = csub(s, Xr[((b * o + i) * o + j) * v + a]);
-        s = cadd(s, Xr[((b * o + j) * o + i) * v + a]);
+        c128 s = mk(0.0, 0.0);
+        if (a >= alo && a < ahi) s = csub(Xr[((a * o + i) * o + j) * v + b], Xr[((a * o + j) * o + i) * v + b]);
+        if (b >= alo && b < ahi) {
+            s = csub(s, Xr[((b * o + i) * o + j) * v + a]);
+            s = cadd(s, Xr[((b * o + j) * o + i) * v + a]);
+        }
         return s;
     });
     return CCSD_OK;
@@ -957,44 +1023,60 @@ static int s2_ring(ccsd_ctx* c, c128* S)
 static int s2_vdag_t1(ccsd_ctx* c, c128* S)
 {   // sum_c conj(<cj||ab>) t1[i,c] - (i<->j):   P[i][(j,a<b)]
     const int o = c->o, v = c->v;
-    const int64_t vv = c->vv;
-    CCSD_TRY(run_gemm(c->env, gp(o * vv, o, v, c->VvovvT, v, c->t1, v, c->P, 1, o * vv, 1.0, 0)));
+    const int64_t vv = c->vv, r0 = c->sh.w_lo, rows = c->sh.w_hi - c->sh.w_lo;
+    if (c->sh.world == 1) {
+        CCSD_TRY(run_gemm(c->env, gp(o * vv, o, v, c->VvovvT, v, c->t1, v, c->P, 1, o * vv, 1.0, 0)));
+    } else {   // this rank's (a<b) columns only: one product per j
+        if (rows <= 0) return CCSD_OK;
+        GemmParams p = gp(rows, o, v, c->VvovvT + r0 * v, v, c->t1, v, c->P + r0, 1, o * vv, 1.0, 0);
+        p.batch = o; p.bsA = vv * v; p.bsB = 0; p.bsC = vv;
+        CCSD_TRY(run_gemm(c->env, p));
+    }
     const c128* P = c->P;
     const int2* po = c->po;
-    launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+    launch_fill(c->st, S + r0, c->oo, rows, vv, 1, [=] __device__(int64_t IJ, int64_t col) {
         int2 ij = po[IJ];
+        const int64_t AB = r0 + col;
         return csub(P[((int64_t)ij.x * o + ij.y) * vv + AB], P[((int64_t)ij.y * o + ij.x) * vv + AB]);
     });
     return CCSD_OK;
 }
 static int s2_gvv(ccsd_ctx* c, c128* S)
-{   // sum_c Gvv[a,c] t2[i,j,c,b] - Gvv[b,c] t2[i,j,c,a];   Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]
+{   // sum_c Gvv[a,c] t2[i,j,c,b] - Gvv[b,c] t2[i,j,c,a];   Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]; rows (i<j) of this rank
     const int v = c->v;
-    const int64_t vv = c->vv, oo = c->oo;
-    CCSD_TRY(run_gemm(c->env, gp(oo * v, v, v, c->t2hu, v, c->Gvv, v, c->Qm, v, 1, 1.0, 0)));
+    const int64_t vv = c->vv, r0 = c->sh.ij_lo, rows = c->sh.ij_hi - c->sh.ij_lo;
+    if (rows <= 0) return CCSD_OK;
+    CCSD_TRY(run_gemm(c->env, gp(rows * v, v, v, c->t2hu + r0 * v * v, v, c->Gvv, v, c->Qm + r0 * v * v, v, 1, 1.0, 0)));
     const c128* Qm = c->Qm;
     const int2* pv = c->pv;
-    launch_fill(c->st, S, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
+    launch_fill(c->st, S + r0 * vv, rows, vv, vv, 1, [=] __device__(int64_t r, int64_t AB) {
+        const int64_t IJ = r0 + r;
         int2 ab = pv[AB];
         return csub(Qm[(IJ * v + ab.x) * v + ab.y], Qm[(IJ * v + ab.y) * v + ab.x]);
     });
     return CCSD_OK;
 }
 static int s2_c_t1(ccsd_ctx* c, c128* S)
-{   // sum_k C[k,a,i,j] t1[k,b] - C[k,b,i,j] t1[k,a];   Rr[(a,i<j)][b] = sum_k C[k,a,i,j] t1[k,b]
+{   // sum_k C[k,a,i,j] t1[k,b] - C[k,b,i,j] t1[k,a];   Rr[(a,i<j)][b] = sum_k C[k,a,i,j] t1[k,b]; rows a of this rank
     const int o = c->o, v = c->v;
     const int64_t vv = c->vv, oo = c->oo;
+    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
+    const int64_t row0 = (int64_t)alo * oo, rows = (int64_t)(ahi - alo) * oo;
+    if (rows <= 0) return CCSD_OK;
     const c128* Cm = c->Cm;
-    launch_fill(c->st, c->Cm2, v * oo, o, o, 0, [=] __device__(int64_t row, int64_t k) {
-        int64_t a = row / oo, IJ = row % oo;
+    launch_fill(c->st, c->Cm2 + row0 * o, rows, o, o, 0, [=] __device__(int64_t r, int64_t k) {
+        const int64_t row = row0 + r, a = row / oo, IJ = row % oo;
         return Cm[(a * o + k) * oo + IJ];
     });
-    CCSD_TRY(run_gemm(c->env, gp(v * oo, v, o, c->Cm2, o, c->t1T, o, c->Rr, v, 1, 1.0, 0)));
+    CCSD_TRY(run_gemm(c->env, gp(rows, v, o, c->Cm2 + row0 * o, o, c->t1T, o, c->Rr + row0 * v, v, 1, 1.0, 0)));
     const c128* Rr = c->Rr;
     const int2* pv = c->pv;
     launch_fill(c->st, S, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
         int2 ab = pv[AB];
-        return csub(Rr[((int64_t)ab.x * oo + IJ) * v + ab.y], Rr[((int64_t)ab.y * oo + IJ) * v + ab.x]);
+        c128 s = mk(0.0, 0.0);
+        if (ab.x >= alo && ab.x < ahi) s = Rr[((int64_t)ab.x * oo + IJ) * v + ab.y];
+        if (ab.y >= alo && ab.y < ahi) s = csub(s, Rr[((int64_t)ab.y * oo + IJ) * v + ab.x]);
+        return s;
     });
     return CCSD_OK;
 }
@@ -1197,6 +1279,8 @@ void ccsd_default_options(ccsd_options* opts)
     opts->cc2 = 0;
     opts->direct_ladder = 0;
     opts->graph = 1;
+    opts->shard_rank = 0;
+    opts->shard_world = 1;
 }
 
 int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
@@ -1220,9 +1304,13 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
         snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
         return CCSD_ECUDA;
     }
+    if (opts && opts->shard_world > 1) {
+        if (opts->shard_rank < 0 || opts->shard_rank >= opts->shard_world || opts->shard_world > nvir || opts->cc2) return CCSD_EINVAL;
+    }
     ccsd_ctx* c = new (std::nothrow) ccsd_ctx();
     if (!c) return CCSD_ENOMEM;
     c->lam = nullptr;
+    c->ws_base = static_cast<char*>(workspace);
     setup_dims(c, nocc, nvir, naux, opts);
     size_t need = 0;
     carve(c, nullptr, &need);
@@ -1294,12 +1382,10 @@ int ccsd_residual(ccsd_ctx* c)
     return residual_any(c);
 }
 
-int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
+// Jacobi step (reading G12) + DIIS (reading G13) + energy of the new amplitudes, all on the device: the Gram row
+// is reduced, the bordered Pulay system solved and the amplitudes recombined without a host round trip (reduce.cuh)
+static int update_from_residual(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
 {
-    if (!c) return CCSD_ESTATE;
-    CCSD_TRY(residual_any(c));
-    // Jacobi step (reading G12) + DIIS (reading G13), all on the device: the Gram row is reduced, the bordered
-    // Pulay system solved and the amplitudes recombined without a host round trip (reduce.cuh)
     launch_jacobi_diis(c->st, c->diis, c->o, c->v, c->S1, c->S2p, c->t1, c->t2p, c->eps, c->po, c->pv, c->opt.ccd);
     c->have_residual = false;       // the intermediates of this residual belong to the amplitudes before the update
     c->tau_valid = false;
@@ -1318,6 +1404,40 @@ int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
     }
     CCSD_CUDA_TRY(cudaGetLastError());
     return c->red_host[35] != 0.0 ? CCSD_ESINGULAR : CCSD_OK;
+}
+
+int ccsd_iterate(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
+{
+    if (!c) return CCSD_ESTATE;
+    if (c->sh.world > 1) return CCSD_EINVAL;   // the slabs of S2 have to be summed over the ranks between the two halves
+    CCSD_TRY(residual_any(c));
+    return update_from_residual(c, e_re, e_im, step_norm);
+}
+
+int ccsd_update(ccsd_ctx* c, double* e_re, double* e_im, double* step_norm)
+{
+    if (!c || !c->have_residual) return CCSD_ESTATE;
+    return update_from_residual(c, e_re, e_im, step_norm);
+}
+
+int ccsd_shard_ranges(int nocc, int nvir, int rank, int world, int64_t ranges[8])
+{   // host only: the slab of rank `rank` of `world` (struct Shard)
+    if (!ranges || nocc < 2 || nvir < 2 || world < 1 || rank < 0 || rank >= world || world > nvir) return CCSD_EINVAL;
+    const Shard s = make_shard(rank, world, nocc, nvir);
+    const int64_t vals[8] = {s.a_lo, s.a_hi, s.w_lo, s.w_hi, s.ij_lo, s.ij_hi, s.wa_lo, s.wa_hi};
+    for (int k = 0; k < 8; k++) ranges[k] = vals[k];
+    return CCSD_OK;
+}
+
+int ccsd_shard_info(ccsd_ctx* c, int64_t info[CCSD_NSHARD_INFO])
+{
+    if (!c || !info) return CCSD_ESTATE;
+    const Shard& s = c->sh;
+    const int64_t vals[CCSD_NSHARD_INFO] = {s.rank, s.world, s.a_lo, s.a_hi, s.w_lo, s.w_hi, s.ij_lo, s.ij_hi,
+                                            (int64_t)(reinterpret_cast<char*>(c->S2p) - c->ws_base), c->oo * c->vv,
+                                            (int64_t)(reinterpret_cast<char*>(c->S1) - c->ws_base), c->ov};
+    for (int k = 0; k < CCSD_NSHARD_INFO; k++) info[k] = vals[k];
+    return CCSD_OK;
 }
 
 int ccsd_solve(ccsd_ctx* c, double tol, int max_iterations, int* iterations, double* e_re, double* e_im, double* step_norm)
@@ -1404,7 +1524,7 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
     switch (id) {
     case CCSD_T_FOCK: dcopy(st, out, c->f, (int64_t)c->n * c->n); break;
     case CCSD_T_VVVV:
-        if (!c->W) return CCSD_EINVAL;   // direct_ladder: not stored
+        if (!c->W || c->sh.world > 1) return CCSD_EINVAL;   // direct_ladder: not stored; sharded: this rank's rows only
         dcopy(st, out, c->W, vv * vv);
         break;
     case CCSD_T_VOVV: dcopy(st, out, c->Vvovv_p, ov * vv); break;
@@ -1743,7 +1863,8 @@ int ccsd_lambda_workspace_bytes(ccsd_ctx* c, size_t* bytes)
 int ccsd_lambda_init(ccsd_ctx* c, void* workspace, size_t workspace_bytes)
 {
     if (!c) return CCSD_ESTATE;
-    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || c->opt.cc2 || c->opt.direct_ladder) return CCSD_EINVAL;
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || c->opt.cc2 || c->opt.direct_ladder || c->sh.world > 1)
+        return CCSD_EINVAL;
     size_t need = 0;
     LambdaState tmp;
     lambda_carve(c, nullptr, &tmp, &need);

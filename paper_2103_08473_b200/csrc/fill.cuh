@@ -37,11 +37,15 @@ static inline void launch_fill(cudaStream_t st, c128* out, int64_t rows, int64_t
 
 // 3M "sum plane" of a complex buffer: out[i] = Re in[i] + Im in[i]  (gemm_dmma.cuh, DmmaCfg::PL).  Streaming:
 // 32 bytes read + 16 bytes written per thread and step.
-__global__ void __launch_bounds__(256) sum_plane_kernel(const c128* __restrict__ in, double* __restrict__ out, int64_t n)
+__global__ void __launch_bounds__(256) sum_plane_kernel(const c128* __restrict__ in, double* __restrict__ out, int64_t n, int pairs)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x * 2;
     for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n; i += stride) {
-        if (i + 1 < n) {
+        if (i + 1 < n && !pairs) {      // out is only 8-byte aligned (a slab that starts at an odd element)
+            const c128 x = in[i], y = in[i + 1];
+            out[i] = x.x + x.y;
+            out[i + 1] = y.x + y.y;
+        } else if (i + 1 < n) {
             const c128 x = in[i], y = in[i + 1];
             *reinterpret_cast<double2*>(out + i) = make_double2(x.x + x.y, y.x + y.y);
         } else {
@@ -56,7 +60,7 @@ static inline void launch_sum_plane(cudaStream_t st, const c128* in, double* out
     int64_t blocks = (n / 2 + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (blocks < 1) blocks = 1;
-    sum_plane_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, n);
+    sum_plane_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, n, (reinterpret_cast<uintptr_t>(out) & 15) == 0 ? 1 : 0);
     count_launches(1);
 }
 

@@ -228,8 +228,23 @@ def test_fullsize_direct_ladder_sampled(gpu, cfg):
     gc.close()
 
 
-_SLOW = pytest.mark.skipif(os.environ.get("CCSD_SLOW_TESTS") != "1",
-                           reason="cfg3: several minutes of oracle loops and ~60 GB of host memory; set CCSD_SLOW_TESTS=1")
+def _host_can_certify_cfg3() -> bool:
+    """The cfg3 certification is one oracle residual at cfg3: ~8 minutes of explicit loops on 16 cores and ~60 GB of host
+    memory (the unpacked <ab||cd>).  It runs wherever the host has that (the B200 boxes do: 16 cores, 196 GB); CCSD_SLOW_TESTS=0
+    switches it off, =1 forces it."""
+    flag = os.environ.get("CCSD_SLOW_TESTS")
+    if flag is not None:
+        return flag == "1"
+    try:
+        with open("/proc/meminfo") as fh:
+            avail = next(int(line.split()[1]) for line in fh if line.startswith("MemAvailable")) / 2 ** 20     # GiB
+    except (OSError, StopIteration):
+        return False
+    return (os.cpu_count() or 1) >= 12 and avail >= 80.0
+
+
+_SLOW = pytest.mark.skipif(not _host_can_certify_cfg3(),
+                           reason="cfg3 certification needs >= 12 host cores and >= 80 GiB of free host memory (or CCSD_SLOW_TESTS=1)")
 
 
 @pytest.mark.parametrize("cfg,continue_oracle", [("cfg1", True), ("cfg2", False),

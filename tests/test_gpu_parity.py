@@ -324,3 +324,70 @@ def test_direct_ladder_matches_oracle(gpu, o, v, L):
         eg, sg = gc.iterate()
         assert abs(eg - eo) < E_TOL and abs(sg - so) < 1e-9 * max(1.0, so)
     gc.close()
+
+
+def test_two_contexts_on_two_streams_concurrently(gpu):
+    """The C ABI takes a stream per context: two contexts iterating at the same time on two streams (from two host threads)
+    share no scratch -- reduction partials, Gram matrix and DIIS coefficients are carved from each context's workspace --
+    and both reproduce the oracle's lock-step energies."""
+    import threading
+    import torch
+    from oracle.ccsd_oracle import OracleCCSD
+    cases = [ci.make_inputs(6, 20, 40, seed=4101, b_scale=0.06), ci.make_inputs(5, 24, 40, seed=4102, b_scale=0.06)]
+    refs = []
+    for inp in cases:
+        oc = OracleCCSD(inp.h, inp.B, inp.nocc, inp.nvir)
+        refs.append([oc.iterate() for _ in range(12)])
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    solvers = [gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=st) for inp, st in zip(cases, streams)]
+    assert solvers[0].stream.cuda_stream != solvers[1].stream.cuda_stream
+    out = [[], []]
+
+    def work(k):
+        torch.cuda.set_device(0)
+        for _ in range(12):
+            out[k].append(solvers[k].iterate())
+
+    for rep in range(3):                       # several rounds: a race would not show every time
+        out[0].clear(); out[1].clear()
+        for k, inp in enumerate(cases):
+            solvers[k].close()
+            solvers[k] = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=streams[k])
+        threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        for k in range(2):
+            for (eg, sg), (eo, so) in zip(out[k], refs[k]):
+                assert abs(eg - eo) < E_TOL and abs(sg - so) < 1e-9 * max(1.0, so), (rep, k, eg, eo)
+    for s_ in solvers:
+        s_.close()
+
+
+def test_graph_replay_equals_direct_launches_and_stale_tensors_are_refused(gpu):
+    """opts.graph: the residual replayed as a CUDA graph gives bit-identical iterates to direct launches (same kernels, same
+    order); after ccsd_iterate the intermediates of the residual no longer belong to the current amplitudes, so
+    ccsd_get_tensor refuses them (CCSD_ESTATE) until the next ccsd_residual."""
+    from paper_2103_08473_b200.binding import CCSDError
+    inp = ci.make_inputs(7, 30, 50, seed=4103, b_scale=0.05)
+    a = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=True)
+    b = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=False)
+    n0 = gpu.launch_count()
+    for it in range(8):
+        ea, eb = a.iterate(), b.iterate()
+        assert ea == eb, (it, ea, eb)
+    assert gpu.launch_count() - n0 > 8 * 2 * 60           # replays are counted kernel by kernel
+    with pytest.raises(CCSDError):
+        a.get_tensor("Hvv")
+    a.get_tensor("oovv")                                   # constants are always there
+    a.residual()
+    b.residual()
+    for name in ("tau", "Hvv", "Hvovo", "S2", "S1"):
+        assert torch_equal(a.get_tensor(name), b.get_tensor(name)), name
+    a.close(); b.close()
+
+
+def torch_equal(x, y):
+    import torch
+    return bool(torch.equal(x, y))

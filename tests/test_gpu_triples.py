@@ -150,6 +150,29 @@ def test_triples_edge_cases(gpu):
     gc.close()
 
 
+def test_triples_do_not_depend_on_the_level_shift(gpu):
+    """Converged with shift 0 and with shift 0.3 the amplitudes agree, so +T / (T) / -T must too: their denominators are the
+    spinor energies Re f_pp, not the shifted ones of the Jacobi step (PAPER.md:1062 vs eqs 39/41).  Against the oracle too."""
+    from oracle.ccsd_oracle import OracleCCSD
+    from oracle.triples_oracle import OracleTriples
+    o, v = 5, 11
+    inp = ci.make_inputs(o, v, 18, seed=882, b_scale=0.1, f_offdiag=0.05)
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    assert oc.run(300, tol=1e-13)[-1][1] < 1e-12
+    ref = OracleTriples(oc).energies(restricted=True)
+    got = {}
+    for shift in (0.0, 0.3):
+        gc = gpu.CCSD(inp.h, inp.B, o, v, level_shift=shift)
+        ok, nit, e, sn = gc.solve(1e-13, 600)
+        assert ok, (shift, nit, sn)
+        got[shift] = gc.triples()
+        gc.close()
+    for key in ("+T", "(T)", "-T"):
+        assert abs(ref[key]) > 1e-7
+        assert abs(got[0.0][key] - got[0.3][key]) < E_TOL, (key, got[0.0][key], got[0.3][key])
+        assert abs(got[0.3][key] - ref[key]) < E_TOL, (key, got[0.3][key], ref[key])
+
+
 @pytest.mark.parametrize("gemm_mode", [1, 2, 3])
 def test_triples_and_cc2_under_every_gemm_mode(gpu, gemm_mode):
     """Triples (the K-segmented GEMM always runs on the DMMA kernel; without sum planes when they are switched off) and

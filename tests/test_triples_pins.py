@@ -171,3 +171,22 @@ def test_q7_partial_sums_over_occupied_triples_equal_determinant_space():
     full = ot.energies(restricted=True)
     for key in tot:
         assert abs(tot[key] - full[key]) < 1e-13
+
+
+def test_q8_triples_corrections_do_not_depend_on_the_level_shift():
+    """The level shift (.LSHIFT) only preconditions the amplitude iterations: the converged amplitudes, and
+    with them +T / (T) / -T (whose denominators are the spinor energies Re f_pp, eqs 39/41), must not depend on it."""
+    o, v = 4, 7
+    inp = ci.make_inputs(o, v, 12, seed=881, b_scale=0.12, f_offdiag=0.08)
+    ref = None
+    for shift in (0.0, 0.3):
+        oc = OracleCCSD(inp.h, inp.B, o, v, level_shift=shift)
+        hist = oc.run(400, tol=1e-13)
+        assert hist[-1][1] < 1e-12
+        e = OracleTriples(oc).energies(restricted=True)
+        assert abs(e["+T"]) > 1e-6
+        if ref is None:
+            ref = e
+        else:
+            for key in ref:
+                assert abs(e[key] - ref[key]) < 1e-10, (key, e[key], ref[key])
