@@ -1694,10 +1694,12 @@ static int trip_loader(ccsd_ctx* c, const TripWs& w, const TripVariant& V, TripL
 
 static const TripVariant& trip_variant(const ccsd_ctx* c, const TripWs& w)
 {
-    // column-tile width by padded columns x relative cost, as dmma_pick
+    // column-tile width by padded columns x relative cost, as dmma_pick (N = nvir)
     const int v = c->v;
-    const double c32 = (double)round_up(v, 32) * (w.planes ? 1.019 : 1.037), c48 = (double)round_up(v, 48);
-    const int idx = (w.planes ? 2 : 0) + (c48 < c32 ? 1 : 0);
+    const double c32 = (double)round_up(v, 32) * (w.planes ? 1.026 : 1.037), c48 = (double)round_up(v, 48),
+                 c56 = (double)round_up(v, 56);
+    int idx = (w.planes ? 2 : 0) + (c48 < c32 ? 1 : 0);
+    if (c56 < (c48 < c32 ? c48 : c32)) idx = w.planes ? 5 : 4;
     return k_trip_variants[idx];
 }
 

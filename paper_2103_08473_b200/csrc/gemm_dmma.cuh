@@ -35,10 +35,13 @@ constexpr int DMMA_BKG = 4;         // k-groups (of 4 complex) per pipeline stag
 // PL (3M only): the sums Ar + Ai / Br + Bi come from precomputed real "sum planes" (TMA-staged beside the complex
 // tiles) instead of DADDs in the main loop: DADD shares the FP64 pipe with DMMA and every DADD between DMMAs costs
 // far more than its two issue cycles (measured: 5 % of the kernel).
-template <int NWM_, int NWN_, int MI_, int NJ_, bool M3_, bool PL_ = false>
+// PF: fragment loads run one k-group ahead of the DMMAs (two register copies of every fragment).  The 128 x 56 tiles have no
+// registers left for that (84 FP64 accumulators x 2 + 9 fragments + planes): they load just in time and rely on the second
+// warp of the SM sub-partition to cover the shared-memory latency.
+template <int NWM_, int NWN_, int MI_, int NJ_, bool M3_, bool PL_ = false, bool PF_ = true>
 struct DmmaCfg {
     static constexpr int NWM = NWM_, NWN = NWN_, MI = MI_, NJ = NJ_;
-    static constexpr bool M3 = M3_, PL = PL_;
+    static constexpr bool M3 = M3_, PL = PL_, PF = PF_;
     static_assert(!PL_ || M3_, "sum planes belong to the 3M scheme");
     static constexpr int NB = M3_ ? 8 : 4;                       // complex columns per B fragment
     static constexpr int BM = NWM_ * MI_ * 8, BN = NWN_ * NJ_ * NB;
@@ -257,7 +260,7 @@ gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
     const bool odd = g & 1;
     const unsigned negmask = odd ? 0u : 0x80000000u;
 
-    if (kt > 0) {
+    if (Cfg::PF && kt > 0) {
         mbar_wait(&full[0], 0);
         load_frags(0, 0);
     }
@@ -271,15 +274,21 @@ gemm_dmma_kernel(const __grid_constant__ Loader ld, DmmaArgs p)
         for (int kg = 0; kg < DMMA_BKG; kg++) {
             double2 a[MI], b[NJ];
             double as[MI], bs[NJ];
+            if constexpr (!Cfg::PF) {
+                if (kg == 0) mbar_wait(&full[s], (it / S) & 1);
+                load_frags(s, kg);
+            }
 #pragma unroll
             for (int mi = 0; mi < MI; mi++) { a[mi] = an[mi]; if constexpr (Cfg::PL) as[mi] = asn[mi]; }
 #pragma unroll
             for (int nj = 0; nj < NJ; nj++) { b[nj] = bn[nj]; if constexpr (Cfg::PL) bs[nj] = bsn[nj]; }
-            if (kg + 1 < DMMA_BKG) {
-                load_frags(s, kg + 1);
-            } else if (it + 1 < kt) {
-                mbar_wait(&full[(it + 1) % S], ((it + 1) / S) & 1);
-                load_frags((it + 1) % S, 0);
+            if constexpr (Cfg::PF) {
+                if (kg + 1 < DMMA_BKG) {
+                    load_frags(s, kg + 1);
+                } else if (it + 1 < kt) {
+                    mbar_wait(&full[(it + 1) % S], ((it + 1) / S) & 1);
+                    load_frags((it + 1) % S, 0);
+                }
             }
             if constexpr (!Cfg::M3) {
                 // 4M: DMMA #1 (Re A) x (Re column: Re B | Im column: Im B); DMMA #2 (Im A) x (-Im B | Re B)
@@ -505,6 +514,7 @@ static const DmmaVariant k_dmma_variants[] = {
     DMMA_V(4, 3, 4, 5, false),                                       // 10: 4M 128 x 60, 12 warps
     DMMA_V(4, 2, 4, 2, true, true), DMMA_V(4, 2, 4, 3, true, true),  // 11-12: 3M with sum planes, 128 x {32,48}
     DMMA_V(8, 1, 2, 5, true),                                        // 13: 3M 128 x 40, 8 warps in a column (N = nocc products)
+    DMMA_V(8, 1, 2, 7, true, false, false), DMMA_V(8, 1, 2, 7, true, true, false),   // 14-15: 3M 128 x 56 (+ planes), one column of warps
 };
 #undef DMMA_V
 constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_variants[0]));
@@ -529,7 +539,11 @@ static inline int dmma_pick(int64_t N, bool m3, bool planes = false)
     // 3M 128 x 40 (variant 13, one column of eight warps): N = nocc products with 32 < nocc <= 40 (cfg3: 34) waste 15 %
     // of a 40-column tile instead of 29 % of a 48-column one; measured 0.875 of the 128 x 48 time per tile (N = 34, K = 224
     // and K = 7616), i.e. 1.05 per column
-    if (m3 && !planes && (double)round_up(N, 40) * 1.05 < bestcost) best = 13;
+    if (m3 && !planes && (double)round_up(N, 40) * 1.05 < bestcost) { best = 13; bestcost = (double)round_up(N, 40) * 1.05; }
+    // 3M 128 x 56 (variants 14 / 15, one column of eight warps, fragments loaded just in time): per column as fast as the
+    // 128 x 48 tile (cfg3 (ov)^3 product 74.66 vs 74.63 ms), so it is taken where it pads less -- N = nvir = 224 is 4 x 56:
+    // 0.890 vs 0.862 (128 x 32) and 0.813 (128 x 48) of the FP64 peak at M = 50000, K = 784
+    if (m3 && (double)round_up(N, 56) < bestcost) best = planes ? 15 : 14;
     return best;
 }
 

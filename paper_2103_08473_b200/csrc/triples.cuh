@@ -85,6 +85,8 @@ static const TripVariant k_trip_variants[] = {
     {128, 48, false, &launch_trip_cfg<DmmaCfg<4, 2, 4, 3, true>>},
     {128, 32, true, &launch_trip_cfg<DmmaCfg<4, 2, 4, 2, true, true>>},
     {128, 48, true, &launch_trip_cfg<DmmaCfg<4, 2, 4, 3, true, true>>},
+    {128, 56, false, &launch_trip_cfg<DmmaCfg<8, 1, 2, 7, true, false, false>>},
+    {128, 56, true, &launch_trip_cfg<DmmaCfg<8, 1, 2, 7, true, true, false>>},
 };
 
 // ---- what the energy kernel needs of one triple --------------------------------------------------------------------
