@@ -286,6 +286,12 @@ int ccsd_zgemm_nt(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t l
                   ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
                   void* cuda_stream);
 
+/* Host arithmetic only (no CUDA device needed): the launch plan of the DMMA GEMM for a shape -- tile variant and split-K depth
+ * chosen together against wave quantisation on the SMs.  mode 0 / 2 / 3 as above; with_planes: the
+ * operands carry 3M sum planes; partial_elems: ccsd_c128 elements of split-K scratch available (0 = no split-K).
+ * plan[] = { variant id, tile rows, tile columns, split-K depth }. */
+int ccsd_gemm_plan(int64_t M, int64_t N, int64_t K, int64_t batch, int mode, int with_planes, int64_t partial_elems, int plan[4]);
+
 /*
  * 3M operand "sum plane": out[i] = Re in[i] + Im in[i], i < n.  The 3M complex GEMM (three real products per complex
  * MAC: Ar Br, Ai Bi, (Ar + Ai)(Br + Bi)) reads these sums through TMA instead of forming them on the FP64 pipe.

@@ -29,7 +29,7 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_solve", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
            "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation", "ccsd_update", "ccsd_shard_info",
-           "ccsd_shard_ranges"]
+           "ccsd_shard_ranges", "ccsd_gemm_plan"]
 
 
 class CCSDError(RuntimeError):
@@ -77,6 +77,7 @@ def load_library():
         lib.ccsd_update.argtypes = [vp] + [ctypes.POINTER(dbl)] * 3
         lib.ccsd_shard_info.argtypes = [vp, ctypes.POINTER(i64)]
         lib.ccsd_shard_ranges.argtypes = [ctypes.c_int] * 4 + [ctypes.POINTER(i64)]
+        lib.ccsd_gemm_plan.argtypes = [i64, i64, i64, i64, ctypes.c_int, ctypes.c_int, i64, ctypes.POINTER(ctypes.c_int)]
         lib.ccsd_lambda_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_lambda_init.argtypes = [vp, vp, ctypes.c_size_t]
         lib.ccsd_lambda_iterate.argtypes = [vp, ctypes.POINTER(dbl)]
@@ -188,6 +189,14 @@ def shard_ranges(nocc: int, nvir: int, rank: int, world: int) -> dict:
     arr = (ctypes.c_int64 * 8)()
     _check(load_library().ccsd_shard_ranges(int(nocc), int(nvir), int(rank), int(world), arr), "ccsd_shard_ranges")
     return dict(zip(("a_lo", "a_hi", "w_lo", "w_hi", "ij_lo", "ij_hi", "wa_lo", "wa_hi"), (int(x) for x in arr)))
+
+
+def gemm_plan(M: int, N: int, K: int, batch: int = 1, mode: int = 0, planes: bool = False, partial_elems: int = 0) -> dict:
+    """ccsd_gemm_plan (host arithmetic only): tile variant and split-K depth the DMMA GEMM would use for this shape."""
+    arr = (ctypes.c_int * 4)()
+    _check(load_library().ccsd_gemm_plan(int(M), int(N), int(K), int(batch), int(mode), int(bool(planes)), int(partial_elems), arr),
+           "ccsd_gemm_plan")
+    return {"variant": arr[0], "bm": arr[1], "bn": arr[2], "ksplit": arr[3]}
 
 
 def launch_count(reset: bool = False) -> int:

@@ -63,26 +63,30 @@ static int run_gemm(const Env& env, GemmParams p)
     if (p.K <= 0) return p.accumulate ? CCSD_OK : CCSD_EINVAL;
     bool dmma_ok = dmma_supported(p);
     // gemm_mode: 0 auto, 1 simple FMA kernel, 2 DMMA 4M, 3 DMMA 3M, 100+v explicit DMMA variant v (tuning)
-    int variant = -1;
     // sum planes are staged by TMA: 16-byte aligned rows, i.e. even leading dimensions
     const bool planes_ok = p.As && p.Bs && p.sam % 2 == 0 && p.sbn % 2 == 0 && (p.batch == 1 || (p.bsA % 2 == 0 && p.bsB % 2 == 0)) &&
                            ((reinterpret_cast<uintptr_t>(p.As) | reinterpret_cast<uintptr_t>(p.Bs)) & 15) == 0;
-    if (env.gemm_mode >= 100) variant = env.gemm_mode - 100;
-    else if (env.gemm_mode == 2) variant = dmma_pick(p.N, false);
-    else if (env.gemm_mode == 3) variant = dmma_pick(p.N, true, planes_ok);
-    else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p))
-        variant = dmma_pick(p.N, CCSD_DEFAULT_3M != 0, CCSD_DEFAULT_3M != 0 && planes_ok);
-    if (variant >= DMMA_NVARIANTS) return CCSD_EINVAL;
-    if (variant >= 0 && !dmma_ok) {   // strided operands: an explicitly requested tile variant is an error, a forced family is not
-        if (env.gemm_mode >= 100) return CCSD_EINVAL;
-        variant = -1;
+    int family = -1;   // -1 simple kernel, 0 4M, 1 3M, 2 3M with planes, 3 one explicit variant
+    if (env.gemm_mode >= 100) family = 3;
+    else if (env.gemm_mode == 2) family = 0;
+    else if (env.gemm_mode == 3) family = planes_ok ? 2 : 1;
+    else if (env.gemm_mode == 0 && dmma_ok && dmma_worthwhile(p)) family = CCSD_DEFAULT_3M != 0 ? (planes_ok ? 2 : 1) : 0;
+    if (family == 3 && env.gemm_mode - 100 >= DMMA_NVARIANTS) return CCSD_EINVAL;
+    if (family >= 0 && !dmma_ok) {   // strided operands: an explicitly requested tile variant is an error, a forced family is not
+        if (family == 3) return CCSD_EINVAL;
+        family = -1;
     }
-    const bool use_dmma = variant >= 0;
-    // split-K chosen against wave quantisation on the 148 SMs: minimise  waves(ks) * (K/ks + pipeline overhead)
-    const int bm = use_dmma ? k_dmma_variants[variant].bm : SG_BM, bn = use_dmma ? k_dmma_variants[variant].bn : SG_BN;
-    const int64_t tiles = ((p.M + bm - 1) / bm) * ((p.N + bn - 1) / bn) * p.batch;
+    const bool use_dmma = family >= 0;
+    int variant = -1;
     p.ksplit = 1; p.kchunk = p.K; p.partial = nullptr;
-    if (env.partial && p.K >= 512) {
+    if (use_dmma) {   // tile variant and split-K depth together, against wave quantisation on the 148 SMs (dmma_plan)
+        const DmmaPlan plan = dmma_plan(p.M, p.N, p.K, p.batch, family != 0, family == 2, env.partial != nullptr, env.partial_elems,
+                                        family == 3 ? env.gemm_mode - 100 : -1);
+        variant = plan.variant;
+        if (plan.ksplit > 1) { p.ksplit = plan.ksplit; p.kchunk = plan.kchunk; p.partial = env.partial; }
+    } else if (env.partial && p.K >= 512) {
+        // simple kernel: split-K chosen against wave quantisation: minimise  waves(ks) * (K/ks + pipeline overhead)
+        const int64_t tiles = ((p.M + SG_BM - 1) / SG_BM) * ((p.N + SG_BN - 1) / SG_BN) * p.batch;
         const int64_t cap = env.partial_elems / (p.M * p.N * p.batch);
         const double overhead = 96.0;   // pipeline fill + epilogue, in units of k
         double best = 1e300;
@@ -2211,6 +2215,16 @@ int ccsd_measure_fp64_peak(double* tflops, double* device_scratch, int launches,
         return CCSD_ECUDA;
     }
     return measure_fp64_peak(static_cast<cudaStream_t>(cuda_stream), device_scratch, launches, tflops);
+}
+
+int ccsd_gemm_plan(int64_t M, int64_t N, int64_t K, int64_t batch, int mode, int with_planes, int64_t partial_elems, int plan[4])
+{   // host only: what ccsd_zgemm_nt / the contractions would launch for this shape (dmma_plan)
+    if (!plan || M < 1 || N < 1 || K < 1 || batch < 1) return CCSD_EINVAL;
+    const bool m3 = mode == 3 || (mode == 0 && CCSD_DEFAULT_3M != 0);
+    if (!(mode == 0 || mode == 2 || mode == 3)) return CCSD_EINVAL;
+    const DmmaPlan pl = dmma_plan(M, N, K, batch, m3, m3 && with_planes, partial_elems > 0, partial_elems);
+    plan[0] = pl.variant; plan[1] = k_dmma_variants[pl.variant].bm; plan[2] = k_dmma_variants[pl.variant].bn; plan[3] = pl.ksplit;
+    return CCSD_OK;
 }
 
 int ccsd_real_flops_per_cmac(const ccsd_options* opts)

@@ -522,28 +522,41 @@ constexpr int DMMA_NVARIANTS = (int)(sizeof(k_dmma_variants) / sizeof(k_dmma_var
 #define CCSD_DEFAULT_3M 1
 #endif
 
-// variant of a family (4M, 3M, 3M with sum planes) with the lowest estimated cost: padded columns x the measured
-// relative cost per column of that tile width (narrow tiles re-read the A tile more often and, for 3M, spend a larger
-// share of the FP64 pipe on the sums; cfg3 (ov)^3 GEMM: 128x32 vs 128x48 = 1.037 without planes, 1.019 with)
-static inline int dmma_pick(int64_t N, bool m3, bool planes = false)
+// Tile variant AND split-K depth of a launch, chosen together against wave quantisation on the SMs: a launch costs
+//     waves(tiles x splits) x (k per split + pipeline overhead) x columns of the tile x relative cost per column
+// (every CTA tile is 128 rows).  The relative cost per column is measured: narrow tiles re-read the A tile more often and,
+// for 3M without planes, spend a larger share of the FP64 pipe on the sums (cfg3 (ov)^3 GEMM: 128x32 vs 128x48 = 1.037
+// without planes, 1.026 with; 128x40 = 1.05; 128x56 = 1.00: 74.66 vs 74.63 ms).  For many waves this is "padded columns x
+// relative cost" (cfg3: N = 561 -> 12 x 48, N = nvir = 224 -> 4 x 56, N = nocc = 34 -> 40); for the smaller configurations
+// the waves decide (cfg2 pp-ladder: 6 x 100 tiles of 48 columns are 4.05 waves, 5 x 100 of 56 columns 3.4).
+struct DmmaPlan { int variant, ksplit; int64_t kchunk; double cost; };
+static inline DmmaPlan dmma_plan(int64_t M, int64_t N, int64_t K, int64_t batch, bool m3, bool planes, bool may_split, int64_t partial_elems,
+                                 int only_variant = -1)
 {
-    const int lo = planes ? 11 : (m3 ? 5 : 0), hi = planes ? 12 : (m3 ? 6 : 4);
-    int best = -1;
-    double bestcost = 0.0;
-    for (int v = hi; v >= lo; v--) {
-        const int bn = k_dmma_variants[v].bn;
-        const double rel = planes ? (bn == 32 ? 1.026 : 1.0) : m3 ? (bn == 32 ? 1.037 : 1.0) : 1.0 + 0.01 * (64 - bn) / 8.0;
-        const double cost = (double)round_up(N, bn) * rel;
-        if (best < 0 || cost < bestcost) { best = v; bestcost = cost; }
+    static const int fam_4m[] = {4, 3, 2, 1, 0}, fam_3m[] = {6, 5, 13, 14}, fam_pl[] = {12, 11, 15};
+    const int* fam = planes ? fam_pl : (m3 ? fam_3m : fam_4m);
+    const int nfam = planes ? 3 : (m3 ? 4 : 5);
+    const double overhead = 96.0;   // pipeline fill + epilogue, in units of k
+    DmmaPlan best{-1, 1, K, 0.0};
+    for (int q = 0; q < (only_variant >= 0 ? 1 : nfam); q++) {
+        const int v = only_variant >= 0 ? only_variant : fam[q];
+        const int bm = k_dmma_variants[v].bm, bn = k_dmma_variants[v].bn;
+        const double rel = !k_dmma_variants[v].m3 ? 1.0 + 0.01 * (64 - bn) / 8.0
+                           : bn == 32 ? (k_dmma_variants[v].planes ? 1.026 : 1.037) : bn == 40 ? 1.05 : 1.0;
+        const int64_t tiles = ((M + bm - 1) / bm) * ((N + bn - 1) / bn) * batch;
+        const int64_t cap = may_split && K >= 512 ? partial_elems / (M * N * batch) : 1;
+        for (int ks = 1; ks <= 592 && (ks == 1 || (ks <= cap && K / ks >= 256)); ks++) {
+            if (ks > 16 && tiles * ks > 2 * 592) break;   // deep splits only for skinny outputs
+            const int64_t chunk = ks == 1 ? K : round_up((K + ks - 1) / ks, 16);
+            const int64_t nsplit = (K + chunk - 1) / chunk;
+            const int64_t waves = (tiles * nsplit + 147) / 148;
+            const double cost = (double)waves * ((double)chunk + overhead) * (ks > 1 ? 1.02 : 1.0) * bn * rel;
+            if (best.variant < 0 || cost < best.cost * (ks > 1 ? 0.97 : 0.999)) {   // a split has to pay for its reduction pass
+                best.variant = v; best.cost = cost;
+                best.ksplit = (int)nsplit; best.kchunk = nsplit > 1 ? chunk : K;
+            }
+        }
     }
-    // 3M 128 x 40 (variant 13, one column of eight warps): N = nocc products with 32 < nocc <= 40 (cfg3: 34) waste 15 %
-    // of a 40-column tile instead of 29 % of a 48-column one; measured 0.875 of the 128 x 48 time per tile (N = 34, K = 224
-    // and K = 7616), i.e. 1.05 per column
-    if (m3 && !planes && (double)round_up(N, 40) * 1.05 < bestcost) { best = 13; bestcost = (double)round_up(N, 40) * 1.05; }
-    // 3M 128 x 56 (variants 14 / 15, one column of eight warps, fragments loaded just in time): per column as fast as the
-    // 128 x 48 tile (cfg3 (ov)^3 product 74.66 vs 74.63 ms), so it is taken where it pads less -- N = nvir = 224 is 4 x 56:
-    // 0.890 vs 0.862 (128 x 32) and 0.813 (128 x 48) of the FP64 peak at M = 50000, K = 784
-    if (m3 && (double)round_up(N, 56) < bestcost) best = planes ? 15 : 14;
     return best;
 }
 

@@ -107,3 +107,22 @@ def test_product_does_not_import_oracle():
         assert not re.search(r"^\s*(import|from)\s+paper_2103_08473_b200", text, flags=re.M), f
         assert not re.search(r"#\s*include\s*[<\"].*ccsd\.h", text), f
         assert "csrc" not in text, f
+
+
+def test_gemm_plan_picks_tiles_against_padding_and_wave_quantisation(lib):
+    """ccsd_gemm_plan (host arithmetic): the documented choices of DESIGN.md's kernel section."""
+    from paper_2103_08473_b200.binding import gemm_plan
+    pe = 16 * 1024 * 1024
+    # cfg3: many waves -> padded columns decide.  N = oo = 561 -> 12 x 48; N = nvir = 224 -> 4 x 56; N = nocc = 34 -> 40
+    assert gemm_plan(24976, 561, 24976, planes=True, partial_elems=pe) == {"variant": 12, "bm": 128, "bn": 48, "ksplit": 1}
+    assert gemm_plan(24976, 224, 816, batch=256, planes=True, partial_elems=pe)["bn"] == 56
+    assert gemm_plan(849184, 34, 224, partial_elems=pe)["bn"] == 40
+    # cfg2 / cfg1: few waves -> the wave count decides (6 x 100 tiles of 48 columns would be 4.05 waves)
+    assert gemm_plan(12720, 276, 12720, planes=True, partial_elems=pe)["bn"] == 56
+    assert gemm_plan(4560, 120, 4560, planes=True, partial_elems=pe)["bn"] == 32
+    # skinny outputs with a huge K are split deep; without scratch there is no split
+    p = gemm_plan(34, 34, 849184, partial_elems=pe)
+    assert p["ksplit"] > 100 and gemm_plan(34, 34, 849184)["ksplit"] == 1
+    # 4M family on request
+    assert gemm_plan(1000, 64, 1000, mode=2)["variant"] in (0, 1, 2, 3, 4)
+    assert lib.ccsd_gemm_plan(0, 1, 1, 1, 0, 0, 0, None) == 1
