@@ -615,7 +615,7 @@ def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True) -> dict:
 
 
 def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=None, clock_index=None, e2e=False,
-                    max_ranks=None) -> dict:
+                    max_ranks=None, graph=1) -> dict:
     """W warm-up + exactly K timed ccsd_iterate of workload `cfg` the way a user runs them (residual replayed as a CUDA
     graph, no events inside), CUDA events on the solver's stream around the K steps; then a second pass of K iterations
     with the library's per-step events (direct launches) for the per-term table and the roofline launch."""
@@ -624,7 +624,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
     barrier = barrier or torch.cuda.synchronize
     pkg.launch_count(reset=True)
     t0 = time.perf_counter()
-    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6)
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, graph=graph)
     torch.cuda.synchronize()
     init_s = time.perf_counter() - t0
     init = solver.init_stats()
@@ -828,7 +828,7 @@ def run_ours(args) -> None:
     rf = pkg.real_flops_per_cmac()                                  # 6: the 3M kernels execute 3 real FMAs per complex MAC
     ex = rf / 8.0
     main = iteration_bench(torch, pkg, cfg, inp, args.steps, args.warmup, peak, peaks["hbm_gbs"], barrier=barrier,
-                           clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None))
+                           clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None), graph=args.graph)
     trip_sharded = triples_sharded_bench(torch, pkg, inp, o, v, dist) if (world > 1 and not args.no_sweep) else None
 
     if not is_reporting_rank():
@@ -925,6 +925,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--graph", type=int, default=1, help="ccsd_options.graph of the main leg: 0 direct launches, 1 graph with parallel "
+                                                          "branches, 3 serial graph (profiling aid)")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")

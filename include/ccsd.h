@@ -61,7 +61,10 @@ typedef struct {
                            depend on nothing but the context) is captured into a CUDA graph on its second use and replayed
                            afterwards; 0 = always launch directly.  Capture needs a stream created by the caller: on the
                            legacy / per-thread default streams (cuda_stream = 0, 1 or 2), and while step timing is enabled,
-                           the launches are issued directly whatever this says */
+                           the launches are issued directly whatever this says.  In the graph the independent parts of the
+                           residual (H^{ak}_{ci} + ring product; Fock-like terms + S1; C; A; driver + pp-ladder) are parallel
+                           branches, so that the small products fill the partial waves of the large ones; 3 = a graph with the
+                           launches in their serial order.  Results are bit-identical in all cases */
     int shard_rank;     /* slab sharding of the iteration over several GPUs (one process and one context per GPU, */
     int shard_world;    /* every rank gets the same h, B and holds the same amplitudes): with shard_world = P > 1 the context
                            of rank r builds and stores only its 1/P of the rows of the packed <ab||cd>, and ccsd_residual

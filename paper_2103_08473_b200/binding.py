@@ -223,7 +223,7 @@ def measure_fp64_peak(launches: int = 10) -> float:
 def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True,
              shard=(0, 1)) -> Options:
     return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)),
-                   int(bool(graph)), int(shard[0]), int(shard[1]))
+                   int(graph), int(shard[0]), int(shard[1]))
 
 
 class CCSD:
@@ -237,7 +237,7 @@ class CCSD:
     """
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
-                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: bool = True, stream=None,
+                 ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: int = 1, stream=None,
                  shard=None, group=None):
         torch = _torch()
         lib = load_library()

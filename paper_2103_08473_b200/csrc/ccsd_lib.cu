@@ -215,6 +215,8 @@ struct ccsd_ctx {
     double* Bvvs;           // 3M sum plane of Bvv (the <ab||cd> slab GEMM over the auxiliary index)
     c128* partial;
     int64_t partial_elems;
+    c128* partial_extra;    // split-K scratch of branches 1..4 of the captured residual
+    int64_t partial_extra_elems;
     // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
     bool planes;
     double *Ws, *Vvovv_ps, *Voovv_ps, *G1s, *taups, *Xms, *T2rs, *Hms;
@@ -350,6 +352,9 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
     if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
     c->partial = w.take<c128>(c->partial_elems);
+    // four more split-K slots, one per parallel branch of the captured residual (residual_forked): 32 Mi elements at most
+    c->partial_extra_elems = c->partial_elems < 32 * 1024 * 1024 ? c->partial_elems : 32 * 1024 * 1024;
+    c->partial_extra = (c->opt.graph && !c->opt.cc2) ? w.take<c128>(4 * c->partial_extra_elems) : nullptr;
     c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
     if (c->planes) {
@@ -997,18 +1002,21 @@ static int s2_hh_and_goo(ccsd_ctx* c, c128* S)
     const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
     return run_gemm(c->env, gp(rows, c->oo, 2 * c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1));
 }
-static int s2_ring(ccsd_ctx* c, c128* S)
-{   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)];  S += P-_ij P-_ab X
-    // this rank holds the rows a in [a_lo, a_hi) of H and X: it adds the terms of P-_ij P-_ab X whose first index is one of them
-    const int o = c->o, v = c->v;
-    const int64_t ov = c->ov, vv = c->vv;
-    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
-    const int64_t off = (int64_t)alo * o * ov, rows = (int64_t)(ahi - alo) * o;
-    if (rows > 0)
-        CCSD_TRY(run_gemm(c->env, with_planes(gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0),
-                                              c->Hms ? c->Hms + off : nullptr, c->T2rs)));
-    tick(c, 9);
+static int ring_gemm(ccsd_ctx* c)
+{   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)]; this rank holds the rows a in [a_lo, a_hi) of H and X
+    const int o = c->o;
+    const int64_t ov = c->ov;
+    const int64_t off = (int64_t)c->sh.a_lo * o * ov, rows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;
     if (rows <= 0) return CCSD_OK;
+    return run_gemm(c->env, with_planes(gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0),
+                                        c->Hms ? c->Hms + off : nullptr, c->T2rs));
+}
+static int ring_add(ccsd_ctx* c, c128* S)
+{   // S += P-_ij P-_ab X: this rank adds the terms whose first index is one of its rows a
+    const int o = c->o, v = c->v;
+    const int64_t vv = c->vv;
+    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
+    if (ahi <= alo) return CCSD_OK;
     const c128* Xr = c->Xr;
     const int2 *po = c->po, *pv = c->pv;
     launch_fill(c->st, S, c->oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
@@ -1024,18 +1032,29 @@ static int s2_ring(ccsd_ctx* c, c128* S)
     });
     return CCSD_OK;
 }
-static int s2_vdag_t1(ccsd_ctx* c, c128* S)
-{   // sum_c conj(<cj||ab>) t1[i,c] - (i<->j):   P[i][(j,a<b)]
+static int s2_ring(ccsd_ctx* c, c128* S)
+{
+    CCSD_TRY(ring_gemm(c));
+    tick(c, 9);
+    return ring_add(c, S);
+}
+// The three remaining small terms, each as its product (into a buffer of its own) and its antisymmetrising add into S:
+// in the captured graph the products run inside the parallel branches, the adds after the join (residual_forked).
+static int vdag_gemm(ccsd_ctx* c)
+{   // P[i][(j,a<b)] = sum_c conj(<cj||ab>) t1[i,c]
     const int o = c->o, v = c->v;
     const int64_t vv = c->vv, r0 = c->sh.w_lo, rows = c->sh.w_hi - c->sh.w_lo;
-    if (c->sh.world == 1) {
-        CCSD_TRY(run_gemm(c->env, gp(o * vv, o, v, c->VvovvT, v, c->t1, v, c->P, 1, o * vv, 1.0, 0)));
-    } else {   // this rank's (a<b) columns only: one product per j
-        if (rows <= 0) return CCSD_OK;
-        GemmParams p = gp(rows, o, v, c->VvovvT + r0 * v, v, c->t1, v, c->P + r0, 1, o * vv, 1.0, 0);
-        p.batch = o; p.bsA = vv * v; p.bsB = 0; p.bsC = vv;
-        CCSD_TRY(run_gemm(c->env, p));
-    }
+    if (c->sh.world == 1) return run_gemm(c->env, gp(o * vv, o, v, c->VvovvT, v, c->t1, v, c->P, 1, o * vv, 1.0, 0));
+    if (rows <= 0) return CCSD_OK;   // this rank's (a<b) columns only: one product per j
+    GemmParams p = gp(rows, o, v, c->VvovvT + r0 * v, v, c->t1, v, c->P + r0, 1, o * vv, 1.0, 0);
+    p.batch = o; p.bsA = vv * v; p.bsB = 0; p.bsC = vv;
+    return run_gemm(c->env, p);
+}
+static int vdag_add(ccsd_ctx* c, c128* S)
+{   // S += P[(i,j)] - P[(j,i)]
+    const int o = c->o;
+    const int64_t vv = c->vv, r0 = c->sh.w_lo, rows = c->sh.w_hi - c->sh.w_lo;
+    if (rows <= 0) return CCSD_OK;
     const c128* P = c->P;
     const int2* po = c->po;
     launch_fill(c->st, S + r0, c->oo, rows, vv, 1, [=] __device__(int64_t IJ, int64_t col) {
@@ -1045,12 +1064,23 @@ static int s2_vdag_t1(ccsd_ctx* c, c128* S)
     });
     return CCSD_OK;
 }
-static int s2_gvv(ccsd_ctx* c, c128* S)
-{   // sum_c Gvv[a,c] t2[i,j,c,b] - Gvv[b,c] t2[i,j,c,a];   Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]; rows (i<j) of this rank
+static int s2_vdag_t1(ccsd_ctx* c, c128* S)
+{   // sum_c conj(<cj||ab>) t1[i,c] - (i<->j)
+    CCSD_TRY(vdag_gemm(c));
+    return vdag_add(c, S);
+}
+static int gvv_gemm(ccsd_ctx* c)
+{   // Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]; rows (i<j) of this rank
+    const int v = c->v;
+    const int64_t r0 = c->sh.ij_lo, rows = c->sh.ij_hi - c->sh.ij_lo;
+    if (rows <= 0) return CCSD_OK;
+    return run_gemm(c->env, gp(rows * v, v, v, c->t2hu + r0 * v * v, v, c->Gvv, v, c->Qm + r0 * v * v, v, 1, 1.0, 0));
+}
+static int gvv_add(ccsd_ctx* c, c128* S)
+{   // S += sum_c Gvv[a,c] t2[i,j,c,b] - Gvv[b,c] t2[i,j,c,a] = Qm[(ij,a)][b] - Qm[(ij,b)][a]
     const int v = c->v;
     const int64_t vv = c->vv, r0 = c->sh.ij_lo, rows = c->sh.ij_hi - c->sh.ij_lo;
     if (rows <= 0) return CCSD_OK;
-    CCSD_TRY(run_gemm(c->env, gp(rows * v, v, v, c->t2hu + r0 * v * v, v, c->Gvv, v, c->Qm + r0 * v * v, v, 1, 1.0, 0)));
     const c128* Qm = c->Qm;
     const int2* pv = c->pv;
     launch_fill(c->st, S + r0 * vv, rows, vv, vv, 1, [=] __device__(int64_t r, int64_t AB) {
@@ -1060,19 +1090,30 @@ static int s2_gvv(ccsd_ctx* c, c128* S)
     });
     return CCSD_OK;
 }
-static int s2_c_t1(ccsd_ctx* c, c128* S)
-{   // sum_k C[k,a,i,j] t1[k,b] - C[k,b,i,j] t1[k,a];   Rr[(a,i<j)][b] = sum_k C[k,a,i,j] t1[k,b]; rows a of this rank
+static int s2_gvv(ccsd_ctx* c, c128* S)
+{
+    CCSD_TRY(gvv_gemm(c));
+    return gvv_add(c, S);
+}
+static int c_t1_gemm(ccsd_ctx* c)
+{   // Rr[(a,i<j)][b] = sum_k C[k,a,i,j] t1[k,b]; rows a of this rank
     const int o = c->o, v = c->v;
-    const int64_t vv = c->vv, oo = c->oo;
-    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
-    const int64_t row0 = (int64_t)alo * oo, rows = (int64_t)(ahi - alo) * oo;
+    const int64_t oo = c->oo;
+    const int64_t row0 = (int64_t)c->sh.a_lo * oo, rows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * oo;
     if (rows <= 0) return CCSD_OK;
     const c128* Cm = c->Cm;
     launch_fill(c->st, c->Cm2 + row0 * o, rows, o, o, 0, [=] __device__(int64_t r, int64_t k) {
         const int64_t row = row0 + r, a = row / oo, IJ = row % oo;
         return Cm[(a * o + k) * oo + IJ];
     });
-    CCSD_TRY(run_gemm(c->env, gp(rows, v, o, c->Cm2 + row0 * o, o, c->t1T, o, c->Rr + row0 * v, v, 1, 1.0, 0)));
+    return run_gemm(c->env, gp(rows, v, o, c->Cm2 + row0 * o, o, c->t1T, o, c->Rr + row0 * v, v, 1, 1.0, 0));
+}
+static int c_t1_add(ccsd_ctx* c, c128* S)
+{   // S += sum_k C[k,a,i,j] t1[k,b] - C[k,b,i,j] t1[k,a], the terms whose C row is one of this rank's
+    const int v = c->v;
+    const int64_t vv = c->vv, oo = c->oo;
+    const int alo = c->sh.a_lo, ahi = c->sh.a_hi;
+    if (ahi <= alo) return CCSD_OK;
     const c128* Rr = c->Rr;
     const int2* pv = c->pv;
     launch_fill(c->st, S, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
@@ -1083,6 +1124,11 @@ static int s2_c_t1(ccsd_ctx* c, c128* S)
         return s;
     });
     return CCSD_OK;
+}
+static int s2_c_t1(ccsd_ctx* c, c128* S)
+{
+    CCSD_TRY(c_t1_gemm(c));
+    return c_t1_add(c, S);
 }
 
 static int build_S1(ccsd_ctx* c)
@@ -1154,6 +1200,106 @@ static int residual(ccsd_ctx* c)
     return CCSD_OK;
 }
 
+// Fork / join inside ONE stream capture, without further streams: the dependency set of the capturing stream is read
+// (cudaStreamGetCaptureInfo) and rewritten (cudaStreamUpdateCaptureDependencies), so that the launches that follow hang off the
+// fork point instead of off the previous branch.  The replayed graph then runs independent parts of the residual side by side.
+struct CaptureFork {
+    cudaStream_t st;
+    std::vector<cudaGraphNode_t> base, tails;
+    bool snapshot(std::vector<cudaGraphNode_t>& out) const
+    {
+        cudaStreamCaptureStatus status = cudaStreamCaptureStatusNone;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t n = 0;
+        if (cudaStreamGetCaptureInfo(st, &status, nullptr, nullptr, &deps, &n) != cudaSuccess || status != cudaStreamCaptureStatusActive)
+            return false;
+        out.assign(deps, deps + n);
+        return true;
+    }
+    bool begin(cudaStream_t s) { st = s; tails.clear(); return snapshot(base); }
+    bool end_branch()
+    {   // what this branch ended on joins the tails; the next branch starts from the fork point again
+        std::vector<cudaGraphNode_t> t;
+        if (!snapshot(t)) return false;
+        tails.insert(tails.end(), t.begin(), t.end());
+        return cudaStreamUpdateCaptureDependencies(st, base.data(), base.size(), cudaStreamSetCaptureDependencies) == cudaSuccess;
+    }
+    bool join()
+    {
+        std::vector<cudaGraphNode_t> u;
+        for (cudaGraphNode_t n : tails) {
+            bool seen = false;
+            for (cudaGraphNode_t m : u) seen = seen || m == n;
+            if (!seen) u.push_back(n);
+        }
+        return cudaStreamUpdateCaptureDependencies(st, u.data(), u.size(), cudaStreamSetCaptureDependencies) == cudaSuccess;
+    }
+};
+
+// The residual with its independent parts as parallel branches of the captured graph (only ever called during capture):
+//   after the operand re-layout:   [ H^{ak}_{ci} -> ring product ]   [ Fock-like intermediates -> G_vv t2 product -> S1 ]
+//                                  [ C -> C t1 product ]   [ A -> V^dagger t1 product ]   [ S2 = driver + pp-ladder ]
+//   joined:                        hh-ladder / G_oo, then the antisymmetrising adds of ring, V^dagger t1, G_vv t2, C t1 into S2
+// The small configurations do not fill 148 SMs with one product at a time (cfg1: 108-384 tiles per large GEMM, a chain of
+// 25 few-microsecond kernels for the Fock-like terms and S1): side by side they fill each other's partial waves.  Every
+// branch writes buffers of its own; split-K scratch comes in one slot per branch.  Same kernels on the same inputs as the
+// serial order, so the results are bit-identical to it.
+static int residual_forked(ccsd_ctx* c)
+{
+    CaptureFork fk;
+    c128* const partial0 = c->env.partial;
+    const int64_t pe0 = c->env.partial_elems;
+    auto slot = [&](int k) {   // split-K scratch of branch k
+        c->env.partial = k == 0 ? partial0 : c->partial_extra + (int64_t)(k - 1) * c->partial_extra_elems;
+        c->env.partial_elems = k == 0 ? pe0 : c->partial_extra_elems;
+    };
+    int s = prep_operands(c);
+    bool ok = s == CCSD_OK && fk.begin(c->st);
+    if (ok) {
+        slot(0);
+        s = build_Hvovo(c);
+        if (s == CCSD_OK) s = ring_gemm(c);
+        ok = s == CCSD_OK && fk.end_branch();
+    }
+    if (ok) {
+        slot(1);
+        s = fock_like(c);
+        if (s == CCSD_OK) s = gvv_gemm(c);
+        if (s == CCSD_OK) s = build_S1(c);
+        ok = s == CCSD_OK && fk.end_branch();
+    }
+    if (ok) {
+        slot(2);
+        s = build_C(c);
+        if (s == CCSD_OK) s = c_t1_gemm(c);
+        ok = s == CCSD_OK && fk.end_branch();
+    }
+    if (ok) {
+        slot(3);
+        s = build_A(c);
+        if (s == CCSD_OK) s = vdag_gemm(c);
+        ok = s == CCSD_OK && fk.end_branch();
+    }
+    if (ok) {
+        slot(4);
+        cudaMemsetAsync(c->S2p, 0, (size_t)(c->oo * c->vv) * sizeof(c128), c->st);
+        s = s2_driver(c, c->S2p);
+        if (s == CCSD_OK) s = s2_pp_ladder(c, c->S2p);
+        ok = s == CCSD_OK && fk.end_branch();
+    }
+    slot(0);
+    if (s != CCSD_OK) return s;
+    if (!ok || !fk.join()) return CCSD_ECUDA;
+    CCSD_TRY(s2_hh_and_goo(c, c->S2p));
+    CCSD_TRY(ring_add(c, c->S2p));
+    CCSD_TRY(vdag_add(c, c->S2p));
+    CCSD_TRY(gvv_add(c, c->S2p));
+    CCSD_TRY(c_t1_add(c, c->S2p));
+    c->have_residual = true;
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
 // CC2 (Appendix 7.2, eqs 34-38).  "The T1 amplitude equations in 7.1 are unchanged":
 // S1 is eq 33 at the full (t1, t2).  The doubles equation 34 is <Phi_ij^ab| exp(-T1) H exp(T1) + [F, T2] |Phi_0>, i.e.
 // eq 32 evaluated with t2 -> 0 in every operand (tau -> P-(t1 t1); the ring, G.t2 terms vanish; H^{ak}_{ci} is not
@@ -1217,6 +1363,12 @@ static bool graph_usable(const ccsd_ctx* c)
     return c->opt.graph && !c->timing && !c->graph_failed && c->st != nullptr && c->st != cudaStreamLegacy &&
            c->st != cudaStreamPerThread;
 }
+// opts.graph: 1 = graph with parallel branches (measured faster at every BASELINE configuration: cfg1 3.17 -> 2.99 ms,
+// cfg2 34.9 -> 34.3 ms, cfg3 252.3 -> 249.4 ms), 3 = graph with the launches in their serial order.
+static bool graph_branches(const ccsd_ctx* c)
+{
+    return !c->opt.cc2 && c->partial_extra && c->opt.graph != 3;
+}
 static int residual_any(ccsd_ctx* c)
 {
     ensure_tau(c);
@@ -1232,7 +1384,7 @@ static int residual_any(ccsd_ctx* c)
             c->graph_failed = true;
             return residual_body(c);
         }
-        const int s = residual_body(c);
+        const int s = graph_branches(c) ? residual_forked(c) : residual_body(c);
         cudaGraph_t g = nullptr;
         cudaError_t e = cudaStreamEndCapture(c->st, &g);
         const long long captured = t_launch_tally - tally0;
