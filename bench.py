@@ -741,6 +741,35 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
     return out
 
 
+def variant_sweep(torch, pkg, peak):
+    """Profiling aid (--only-variants): the 3M tile variants of the DMMA GEMM on the shapes that decide the tile choice
+    (DESIGN.md "The DMMA GEMM"): executed-flop fraction of the FP64 peak of ccsd_zgemm_nt(mode = 100 + variant)."""
+    shapes = [("triples driver, 61 triples batched as rows", 50000, 224, 784, True, (11, 12, 15)),
+              ("one triple", 24976, 224, 816, True, (11, 12, 15)),
+              ("G_vv.t2", 125664, 224, 224, False, (5, 6, 14)),
+              ("N = nocc product", 200000, 34, 224, False, (5, 6, 13)),
+              ("pp-ladder cfg3", 24976, 561, 24976, True, (12, 15)),
+              ("(ov)^3 cfg3", 7616, 7616, 7616, True, (12, 15)),
+              ("pp-ladder cfg2", 12720, 276, 12720, True, (11, 12, 15))]
+    out = []
+    for name, M, N, K, planes, variants in shapes:
+        g = torch.Generator(device="cuda").manual_seed(1)
+        A = torch.view_as_complex(torch.randn((M, K, 2), generator=g, device="cuda", dtype=torch.float64))
+        B = torch.view_as_complex(torch.randn((N, K, 2), generator=g, device="cuda", dtype=torch.float64))
+        C = torch.zeros((M, N), dtype=torch.complex128, device="cuda")
+        pl = (pkg.sum_plane(A), pkg.sum_plane(B)) if planes else None
+        row = {"shape": name, "M": M, "N": N, "K": K, "planes": planes, "variants": {}}
+        for v in variants:
+            ts = time_events(torch, lambda: pkg.zgemm_nt(A, B, C=C, mode=100 + v, planes=pl), 5, 2)
+            t = statistics.median(ts)
+            row["variants"][str(v)] = {"ms": round(t, 3), "frac_fp64_peak": round(6.0 * M * N * K / (t * 1e-3) * 1e-12 / peak, 4)}
+        row["picked"] = pkg.gemm_plan(M, N, K, 1, 0, planes)
+        out.append(row)
+        del A, B, C, pl
+        torch.cuda.empty_cache()
+    return out
+
+
 def max_over_ranks(value: float, dist, device="cuda") -> float:
     """Multi-GPU numbers are the MAX over ranks (replicas-only path: no data-path collective exists)."""
     import torch
@@ -801,6 +830,12 @@ def run_ours(args) -> None:
         # profiling aid: the transposes leg alone (o^2 v^2-shaped tensor of --config)
         print(json.dumps({"metric": "transpose_gbs", "unit": "GB/s", "config": {"workload": f"{cfg} o^2 v^2 complex128"},
                           "hbm_peak": measured_peaks(), "transposes": transpose_bench(torch, pkg, measured_peaks()["hbm_gbs"], o, v)}))
+        return
+    if args.only_variants:
+        peak = pkg.measure_fp64_peak(4)
+        print(json.dumps({"metric": "dmma_tile_variants", "unit": "fraction of FP64 peak (executed 3M flops)", "fp64_peak_tflops": peak,
+                          "variants": {"5/11": "128x32", "6/12": "128x48", "13": "128x40", "14/15": "128x56", "11,12,15": "with sum planes"},
+                          "sweep": variant_sweep(torch, pkg, peak)}))
         return
     inp = ci.make_config(cfg)                      # every replica solves the same synthetic problem
     if args.only_lambda:
@@ -934,6 +969,7 @@ def main():
     ap.add_argument("--only-transposes", action="store_true", help="time only the 4-index transpositions")
     ap.add_argument("--only-cc2", action="store_true", help="time only the CC2 iteration of --config")
     ap.add_argument("--only-direct", action="store_true", help="time only the CCSD iteration with the integral-direct pp-ladder")
+    ap.add_argument("--only-variants", action="store_true", help="time the 3M tile variants of the DMMA GEMM on the deciding shapes")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
