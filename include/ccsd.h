@@ -24,6 +24,13 @@
  *    memory and never creates streams.  All work is enqueued on the caller's `cuda_stream` (a cudaStream_t).
  *  - Errors: every call returns a CCSD_* status; nothing is thrown or printed.  There is no CPU fallback: without
  *    a CUDA device every compute entry point returns CCSD_ECUDA.
+ *  - Threads and streams: contexts are independent -- every buffer a context's kernels touch (reduction scratch, DIIS Gram
+ *    matrix and coefficients, split-K scratch included) lies in ITS workspace, so different contexts may be driven from
+ *    different host threads on different streams at the same time.  ONE context must not be entered from two threads at once
+ *    (its host-side state -- DIIS ring order, graph handle, pinned read-back buffer -- is not locked), and all its calls are
+ *    ordered on the stream given to ccsd_init.  The context-free entry points (ccsd_contract, ccsd_zgemm_nt*, ccsd_transpose,
+ *    ccsd_sum_plane) keep no state between calls.  ccsd_launch_count is one process-wide atomic counter; ccsd_last_cuda_error
+ *    is per host thread.  The current CUDA device must be the one the workspace lives on.
  */
 #ifndef CCSD_B200_H
 #define CCSD_B200_H

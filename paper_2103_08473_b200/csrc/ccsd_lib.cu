@@ -205,6 +205,8 @@ struct ccsd_ctx {
     int na_slab;
     c128* Wslab;            // direct_ladder: rows of <ab||cd> of one slab of the first virtual index, rebuilt every iteration
     double* Wslabs;         // ... and their 3M sum plane
+    c128* WslabT;           // direct_ladder, one GPU: conj-transpose of the slab's columns beyond the slab (Hermitian half, s2_pp_ladder)
+    double* WslabTs;
     // amplitudes and per-iteration tensors
     c128 *t1, *t2p, *t1T, *S1, *S2p, *taup, *TT, *AG, *Xm, *T2r, *tauc, *tauou, *t2hu;
     c128 *Hvv, *Gvv, *Hoo, *Goo, *Hov, *HovT, *HF, *inner, *Hm, *Cm, *Cm2, *Am, *tmp_ov;
@@ -309,10 +311,16 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
         c->JslabT = w.take<c128>((int64_t)na * v * v * v);
         c->Wslab = nullptr;
         c->Wslabs = nullptr;
+        c->WslabT = nullptr;
+        c->WslabTs = nullptr;
         if (c->opt.direct_ladder) {
             const int64_t max_rows = (int64_t)na * (v - 1);        // pairs (a,b), b > a, of na values of a: at most na (v-1)
             c->Wslab = w.take<c128>(max_rows * vv);
             c->Wslabs = w.take<double>(max_rows * vv);
+            if (c->opt.shard_world <= 1) {
+                c->WslabT = w.take<c128>(vv * round_up(max_rows, 2));
+                c->WslabTs = w.take<double>(vv * round_up(max_rows, 2));
+            }
         }
     }
     // amplitudes, residuals, operands
@@ -482,7 +490,11 @@ static void bblock(cudaStream_t st, c128* out, const c128* B, int n, int L, int 
 //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
 //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
 // absolute = true: dst is the whole matrix (row r0 of the slab goes to dst + r0 vv); false: dst holds the slab only.
-static int build_W_slab(ccsd_ctx* c, int a0, int a_end, c128* dst, bool absolute, int64_t* r0_out, int64_t* nrows_out)
+// upper = true (integral-direct ladder on one GPU): only the columns (c<d) with c >= a0, i.e. the packed columns CD >= r0, are
+// built (the rest follows from <ab||cd> = conj <cd||ab> and is never needed, s2_pp_ladder) -- half the flops of the slab GEMM
+// summed over the slabs -- and the 3M sum plane is written along into `plane` (may be null).
+static int build_W_slab(ccsd_ctx* c, int a0, int a_end, c128* dst, bool absolute, int64_t* r0_out, int64_t* nrows_out,
+                        bool upper = false, double* plane = nullptr)
 {
     cudaStream_t st = c->st;
     const int v = c->v, Lp = c->Lp;
@@ -498,21 +510,34 @@ static int build_W_slab(ccsd_ctx* c, int a0, int a_end, c128* dst, bool absolute
         if (cudaEventCreate(&e) == cudaSuccess) { cudaEventRecord(e, st); c->init_events->push_back(e); }
     };
     mark();
+    const int cfrom = upper ? a0 : 0;          // rows (a, c) with c >= cfrom: one product per a when that is not all of them
     GemmParams g = gp(rows, ncol, Lp, c->Bvv + (int64_t)a0 * v * Lp, Lp, c->Bvv + col0 * Lp, Lp, c->Jslab + col0, v2, 1, 1.0, 0);
     if (c->Bvvs) g = with_planes(g, c->Bvvs + (int64_t)a0 * v * Lp, c->Bvvs + col0 * Lp);
+    if (cfrom > 0) {
+        // the restricted index goes into the COLUMN position of the product (tiles of 32-56 columns pad v - a0 <= nvir far less
+        // than 128-row tiles would): Jslab^T, one product per a with the (b,d) operand shared, stored through csm = 1
+        const int64_t off = ((int64_t)a0 * v + cfrom) * Lp;
+        g = gp(ncol, v - cfrom, Lp, c->Bvv + col0 * Lp, Lp, c->Bvv + off, Lp, c->Jslab + (int64_t)cfrom * v2 + col0, 1, v2, 1.0, 0);
+        g.batch = na; g.bsA = 0; g.bsB = (int64_t)v * Lp; g.bsC = (int64_t)v * v2;
+        if (c->Bvvs) g = with_planes(g, c->Bvvs + col0 * Lp, c->Bvvs + off);
+    }
     CCSD_TRY(run_gemm(c->env, g));
     mark();
     CCSD_TRY(launch_transpose2d_ld(st, c->Jslab + col0, v2, c->JslabT + col0 * rows, rows, rows, ncol, 0));
     mark();
     const int alast = (a0 + na - 1 < v - 2) ? a0 + na - 1 : v - 2;
     const int64_t r0 = pair_idx(a0, a0 + 1, v), r1 = pair_idx(alast, v - 1, v) + 1;
+    const int64_t cd0 = upper ? r0 : 0;        // first packed column built
     const c128 *J = c->Jslab, *JT = c->JslabT;
-    launch_fill(st, dst + (absolute ? r0 * vv : 0), r1 - r0, vv, vv, 0, [=] __device__(int64_t r, int64_t CD) {
+    launch_fill(st, dst + (absolute ? r0 * vv : 0) + cd0, r1 - r0, vv - cd0, vv, 0, [=] __device__(int64_t r, int64_t col) {
+        const int64_t CD = cd0 + col;
         int2 ab = pv[r0 + r], cd = pv[CD];
         int64_t al = ab.x - a0;
         c128 x = J[(al * v + cd.x) * v2 + (int64_t)ab.y * v + cd.y];
         c128 y = JT[((int64_t)ab.y * v + cd.x) * rows + al * v + cd.y];
-        return csub(x, y);
+        x = csub(x, y);
+        if (plane) plane[r * vv + CD] = x.x + x.y;
+        return x;
     });
     mark();
     if (c->init_events) {
@@ -947,7 +972,31 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
         });
         return CCSD_OK;
     }
-    if (c->opt.direct_ladder) {   // integral-direct: rebuild the rows of <ab||cd> slab by slab from the factor B and contract them
+    if (c->opt.direct_ladder && c->WslabT) {
+        // integral-direct on one GPU, using <ab||cd> = conj <cd||ab>: for the slab of packed rows [r0, r1) only the columns
+        // CD >= r0 are rebuilt from B (half the slab-GEMM flops over all slabs), and the block serves twice:
+        //   (1) S[:, r0:r1) += W[r0:r1, r0:vv) tau[:, r0:vv)^T                      M = slab rows,  K = vv - r0
+        //   (2) S[:, r1:vv) += conj(W[r0:r1, r1:vv))^T tau[:, r0:r1)^T               M = vv - r1,    K = slab rows
+        // (2) is what the later slabs would have computed from their columns CD < their r0.  Its left operand is the
+        // conj-transposed copy of the block (one bandwidth-bound pass), so that both products stay K-contiguous.
+        const int64_t vv = c->vv, oo = c->oo;
+        for (int a0 = 0; a0 < c->v - 1; a0 += c->na_slab) {
+            int64_t r0 = 0, nrows = 0;
+            CCSD_TRY(build_W_slab(c, a0, c->v - 1, c->Wslab, false, &r0, &nrows, true, c->planes ? c->Wslabs : nullptr));
+            const int64_t r1 = r0 + nrows, ldt = round_up(nrows, 2);
+            CCSD_TRY(run_gemm(c->env, with_planes(gp(nrows, oo, vv - r0, c->Wslab + r0, vv, c->taup + r0, vv, S + r0, 1, vv, 1.0, 1),
+                                                  c->planes ? c->Wslabs + r0 : nullptr, c->taups ? c->taups + r0 : nullptr)));
+            if (r1 < vv) {
+                if (ldt > nrows) CCSD_CUDA_TRY(cudaMemsetAsync(c->WslabT, 0, (size_t)((vv - r1) * ldt) * sizeof(c128), c->st));
+                CCSD_TRY(launch_transpose2d_ld(c->st, c->Wslab + r1, vv, c->WslabT, ldt, nrows, vv - r1, 1));
+                if (c->planes) launch_sum_plane(c->st, c->WslabT, c->WslabTs, (vv - r1) * ldt);
+                CCSD_TRY(run_gemm(c->env, with_planes(gp(vv - r1, oo, nrows, c->WslabT, ldt, c->taup + r0, vv, S + r1, 1, vv, 1.0, 1),
+                                                      c->planes ? c->WslabTs : nullptr, c->taups ? c->taups + r0 : nullptr)));
+            }
+        }
+        return CCSD_OK;
+    }
+    if (c->opt.direct_ladder) {   // integral-direct, sharded: rebuild this rank's rows of <ab||cd> slab by slab and contract them
         for (int a0 = c->sh.wa_lo; a0 < c->sh.wa_hi; a0 += c->na_slab) {
             int64_t r0 = 0, nrows = 0;
             CCSD_TRY(build_W_slab(c, a0, c->sh.wa_hi, c->Wslab, false, &r0, &nrows));
