@@ -1892,8 +1892,10 @@ static int trip_loader(ccsd_ctx* c, const TripWs& w, const TripVariant& V, TripL
     }
     ld->ijk = w.ijk;
     ld->o = o;
+    ld->op = op;
     ld->tp = (v + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG);
-    ld->th = (o + 4 * DMMA_BKG - 1) / (4 * DMMA_BKG);
+    ld->ngh = (o + 3) / 4;
+    ld->th = (3 * ld->ngh + DMMA_BKG - 1) / DMMA_BKG;
     return CCSD_OK;
 }
 

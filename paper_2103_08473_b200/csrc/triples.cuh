@@ -22,39 +22,62 @@ struct TripLoader {
     CUtensorMap PA, PB, PAs, PBs;   // particle: A = -<ab||xe> [x][(a<b)][e],  B = t2[z,y,e,c] as [(z,y)][c][e]
     CUtensorMap HA, HB, HAs, HBs;   // hole:     A = t2[z,m,a,b] [z][(a<b)][m],  B = <cm||xy> as [(x,y)][c][m]
     const int4* ijk;
-    int o, tp, th;                  // k-iterations per particle / hole segment
+    int o, op;
+    int tp;                         // k-iterations per particle segment (16 e each)
+    int ngh, th;                    // hole part: k-GROUPS (4 m each) per segment; k-iterations of the three segments together
     struct State { int i, j, k; };
     __device__ __forceinline__ int setup(const DmmaArgs&, int bz, int, State& st) const
     {
         const int4 t = ijk[bz];
         st.i = t.x; st.j = t.y; st.k = t.z;
-        return 3 * (tp + th);
+        return 3 * tp + th;
+    }
+    // (x,y,z) = (i,j,k), (j,k,i), (k,i,j)
+    __device__ __forceinline__ void cyc(const State& st, int seg, int& x, int& y, int& z) const
+    {
+        x = seg == 0 ? st.i : (seg == 1 ? st.j : st.k);
+        y = seg == 0 ? st.j : (seg == 1 ? st.k : st.i);
+        z = seg == 0 ? st.k : (seg == 1 ? st.i : st.j);
     }
     template <class Cfg>
     __device__ __forceinline__ void load(const State& st, int L, unsigned char* sa, uint64_t* bar, int m0, int n0) const
     {
-        const bool hole = L >= 3 * tp;
-        const int Ls = hole ? L - 3 * tp : L, per = hole ? th : tp;
-        const int seg = Ls / per, kk = (Ls - seg * per) * 4 * DMMA_BKG;
-        // (x,y,z) = (i,j,k), (j,k,i), (k,i,j)
-        const int x = seg == 0 ? st.i : (seg == 1 ? st.j : st.k);
-        const int y = seg == 0 ? st.j : (seg == 1 ? st.k : st.i);
-        const int z = seg == 0 ? st.k : (seg == 1 ? st.i : st.j);
-        const int cA = hole ? z : x, cB = hole ? x * o + y : z * o + y;
-        const CUtensorMap* mA = hole ? &HA : &PA;
-        const CUtensorMap* mB = hole ? &HB : &PB;
-        const CUtensorMap* mAs = hole ? &HAs : &PAs;
-        const CUtensorMap* mBs = hole ? &HBs : &PBs;
         unsigned char* sb = sa + Cfg::A_STAGE;
+        unsigned char* sp = sb + Cfg::B_STAGE;
+        if (L < 3 * tp) {   // particle segments: whole k-iterations
+            const int seg = L / tp, kk = (L - seg * tp) * 4 * DMMA_BKG;
+            int x, y, z;
+            cyc(st, seg, x, y, z);
+            const int cA = x, cB = z * o + y;
+#pragma unroll
+            for (int kg = 0; kg < DMMA_BKG; kg++) {
+                const int cd = (kk + 4 * kg) * 2;
+                tma_load_3d(sa + kg * Cfg::A_KG, &PA, cd, m0, cA, bar);
+                tma_load_3d(sb + kg * Cfg::B_KG, &PB, cd, n0, cB, bar);
+                if constexpr (Cfg::PL) {
+                    tma_load_3d(sp + kg * Cfg::AS_KG, &PAs, cd / 2, m0, cA, bar);
+                    tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, &PBs, cd / 2, n0, cB, bar);
+                }
+            }
+            return;
+        }
+        // hole segments: nocc is small (34 at cfg3), so they are packed at k-GROUP granularity -- the three segments follow
+        // each other without rounding each up to a whole k-iteration (3 x 34 -> 7 instead of 9 iterations of 16).  A k-group
+        // is its own TMA copy anyway; k-groups beyond the last segment read out of range and are zero-filled.
+        const int g0 = (L - 3 * tp) * DMMA_BKG;
 #pragma unroll
         for (int kg = 0; kg < DMMA_BKG; kg++) {
-            const int cd = (kk + 4 * kg) * 2;
-            tma_load_3d(sa + kg * Cfg::A_KG, mA, cd, m0, cA, bar);
-            tma_load_3d(sb + kg * Cfg::B_KG, mB, cd, n0, cB, bar);
+            const int G = g0 + kg;
+            const int seg = (G >= ngh) + (G >= 2 * ngh);
+            int x, y, z;
+            cyc(st, seg, x, y, z);
+            const int cA = z, cB = x * o + y;
+            const int cd = G >= 3 * ngh ? 2 * op : (G - seg * ngh) * 8;      // doubles; 2 op = out of range -> zeros
+            tma_load_3d(sa + kg * Cfg::A_KG, &HA, cd, m0, cA, bar);
+            tma_load_3d(sb + kg * Cfg::B_KG, &HB, cd, n0, cB, bar);
             if constexpr (Cfg::PL) {
-                unsigned char* sp = sb + Cfg::B_STAGE;
-                tma_load_3d(sp + kg * Cfg::AS_KG, mAs, cd / 2, m0, cA, bar);
-                tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, mBs, cd / 2, n0, cB, bar);
+                tma_load_3d(sp + kg * Cfg::AS_KG, &HAs, cd / 2, m0, cA, bar);
+                tma_load_3d(sp + DMMA_BKG * Cfg::AS_KG + kg * Cfg::BS_KG, &HBs, cd / 2, n0, cB, bar);
             }
         }
     }
