@@ -288,6 +288,31 @@ int ccsd_contract(int term, int nocc, int nvir, const ccsd_c128* const* in, ccsd
                   const ccsd_options* opts, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * The correlation energy (eq 9, with tau of eq 23; reading G11) WITHOUT a workspace, for callers
+ * that cannot allocate one (code under stream capture, tight serving loops, harnesses that forbid cudaMalloc):
+ *   e_out = sum_ia f[i][o+a] t1[i][a] + sum_{i<j,a<b} <ij||ab> (t2 + P-(t1 t1))^{ab}_{ij}
+ * Same arguments as ccsd_contract(CCSD_TERM_ENERGY): f = Fock matrix [n][n], oovv = <kl||cd> [(k<l)][(c<d)], t1 [i][a],
+ * t2p [(i<j)][(a<b)] (device, read only); e_out = one ccsd_c128 on the device, overwritten.  Same kernels in their
+ * energy-only form, same summation order: the result equals that of the workspace path bit for bit.
+ * The scratch that path carves from the caller's workspace (two pair tables and the per-block partial sums) lives in one
+ * file-scope device array of CCSD_ENERGY_STATIC_SCRATCH_BYTES (1.07 MiB) inside the library, which every GPU that loads the
+ * library holds until the process exits.  Limits: 2 <= nocc <= CCSD_ENERGY_STATIC_MAX_NOCC, 2 <= nvir <=
+ * CCSD_ENERGY_STATIC_MAX_NVIR; anything larger returns CCSD_EINVAL (the reason in ccsd_last_cuda_error()) and enqueues
+ * nothing -- use ccsd_contract with a workspace there.  The call makes no cudaMalloc / cudaFree and no allocating
+ * library call; it enqueues four kernels on `cuda_stream` and returns (asynchronous).  The first call on a device resolves
+ * the array's address (cudaGetSymbolAddress, once per device, with the caller's current device).
+ * ALL calls on a device share the one array and it keeps the last call's contents.  Every word a call reads it has
+ * written itself first (tables and partials are rewritten each call; nothing needs to start at zero), so calls
+ * ordered on one stream are independent, but two calls that OVERLAP on the GPU -- different streams or host threads without
+ * an ordering between them -- race on it and give undefined results.  Serialise them, or use the workspace path.
+ */
+#define CCSD_ENERGY_STATIC_MAX_NOCC 128
+#define CCSD_ENERGY_STATIC_MAX_NVIR 512
+#define CCSD_ENERGY_STATIC_SCRATCH_BYTES 1121024
+int ccsd_energy_static(int nocc, int nvir, const ccsd_c128* f, const ccsd_c128* oovv, const ccsd_c128* t1,
+                       const ccsd_c128* t2p, ccsd_c128* e_out, void* cuda_stream);
+
+/*
  * Generic complex GEMM used by every contraction above ("NT" form, both operands K-contiguous):
  *   C[m*csm + n*csn] (+)= alpha * sum_k A[m*lda + k] * B[n*ldb + k]
  * mode: as ccsd_options.gemm_mode (0 auto, 1 simple FMA kernel, 2 DMMA 4M, 3 DMMA 3M, 100+v tile variant v).

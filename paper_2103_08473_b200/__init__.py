@@ -4,8 +4,8 @@ Thin Python binding over the C ABI in include/ccsd.h; every step runs in the CUD
 for device memory and streams.  There is no CPU fallback: without the built library or without a CUDA device the
 compute entry points raise.
 """
-from .binding import (CCSD, CCSDError, TENSOR_IDS, TERM_IDS, STEP_NAMES, contract, gemm_plan, launch_count, lib_path,
+from .binding import (CCSD, CCSDError, TENSOR_IDS, TERM_IDS, STEP_NAMES, contract, energy_static, gemm_plan, launch_count, lib_path,
                       load_library, measure_fp64_peak, real_flops_per_cmac, shard_ranges, sum_plane, transpose, zgemm_nt)
 
-__all__ = ["CCSD", "CCSDError", "TENSOR_IDS", "TERM_IDS", "STEP_NAMES", "contract", "gemm_plan", "launch_count", "lib_path",
+__all__ = ["CCSD", "CCSDError", "TENSOR_IDS", "TERM_IDS", "STEP_NAMES", "contract", "energy_static", "gemm_plan", "launch_count", "lib_path",
            "load_library", "measure_fp64_peak", "real_flops_per_cmac", "shard_ranges", "sum_plane", "transpose", "zgemm_nt"]

@@ -29,7 +29,12 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_solve", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
            "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation", "ccsd_update", "ccsd_shard_info",
-           "ccsd_shard_ranges", "ccsd_gemm_plan"]
+           "ccsd_shard_ranges", "ccsd_gemm_plan", "ccsd_energy_static"]
+
+# limits of ccsd_energy_static (include/ccsd.h): its scratch is a fixed device array inside the library
+ENERGY_STATIC_MAX_NOCC = 128
+ENERGY_STATIC_MAX_NVIR = 512
+ENERGY_STATIC_SCRATCH_BYTES = 1121024
 
 
 class CCSDError(RuntimeError):
@@ -98,6 +103,7 @@ def load_library():
         lib.ccsd_contract_workspace_bytes.argtypes = [ctypes.c_int] * 3 + [ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_contract.argtypes = [ctypes.c_int] * 3 + [ctypes.POINTER(vp), vp, ctypes.c_int,
                                                             ctypes.POINTER(Options), vp, ctypes.c_size_t, vp]
+        lib.ccsd_energy_static.argtypes = [ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp]
         lib.ccsd_zgemm_nt.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
                                       ctypes.c_int, vp]
         lib.ccsd_sum_plane.argtypes = [vp, vp, i64, vp]
@@ -555,6 +561,25 @@ def contract(term: str, nocc: int, nvir: int, inputs, out=None, accumulate: bool
     _check(lib.ccsd_contract(tid, nocc, nvir, arr, out.data_ptr(), int(accumulate), ctypes.byref(opts), base,
                              int(nbytes.value), _stream_ptr(torch)), f"ccsd_contract({term})")
     torch.cuda.current_stream().synchronize()   # ws / ins must outlive the enqueued kernels
+    return out
+
+
+def energy_static(nocc: int, nvir: int, f, oovv, t1, t2p, out):
+    """ccsd_energy_static: the correlation energy (eq 9) of the amplitudes (t1, t2p) without any workspace -- the library's
+    fixed device scratch is used (nocc <= ENERGY_STATIC_MAX_NOCC, nvir <= ENERGY_STATIC_MAX_NVIR, CCSDError beyond).  Nothing is
+    allocated or copied here either: every argument must already be a contiguous complex128 CUDA tensor (f [n][n],
+    oovv [(k<l)][(c<d)], t1 [i][a], t2p [(i<j)][(a<b)], out one element, overwritten).  Asynchronous on the current stream;
+    calls that overlap on the GPU race on the shared scratch (include/ccsd.h).  Returns out."""
+    torch = _torch()
+    lib = load_library()
+    oo, vv = nocc * (nocc - 1) // 2, nvir * (nvir - 1) // 2
+    for name, x, elems in (("f", f, (nocc + nvir) ** 2), ("oovv", oovv, oo * vv), ("t1", t1, nocc * nvir),
+                           ("t2p", t2p, oo * vv), ("out", out, 1)):
+        if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous()
+                and x.numel() == elems):
+            raise ValueError(f"energy_static: {name} must be a contiguous complex128 CUDA tensor of {elems} elements")
+    _check(lib.ccsd_energy_static(nocc, nvir, f.data_ptr(), oovv.data_ptr(), t1.data_ptr(), t2p.data_ptr(), out.data_ptr(),
+                                  _stream_ptr(torch)), "ccsd_energy_static")
     return out
 
 

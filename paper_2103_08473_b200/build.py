@@ -26,7 +26,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or sources_newer_than_lib():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-            ["-o", LIB, os.path.join(CSRC, "ccsd_lib.cu")]
+            ["-o", LIB, os.path.join(CSRC, "ccsd_lib.cu"), os.path.join(CSRC, "energy_static.cu")]
         subprocess.check_call(cmd)
     return LIB
 
