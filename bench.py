@@ -32,10 +32,10 @@ import ccsd_inputs as ci  # noqa: E402
 
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of the 3M + sum-plane DMMA GEMM at cfg3, from
-# profiles/r01d_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
-NCU_TRAFFIC_BYTES = {"cfg3": 22.144e9 + 0.219e9}
+# profiles/r02_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
+NCU_TRAFFIC_BYTES = {"cfg3": 23.10e9 + 0.220e9}
 NCU_TRAFFIC_SOURCE = ("recorded constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of one "
-                      "pp-ladder launch from the ncu --set full capture summarised in profiles/r01d_ncu_pp_ladder_cfg3.md")
+                      "pp-ladder launch from the ncu --set full capture summarised in profiles/r02_ncu_pp_ladder_cfg3.md")
 
 
 def flops_per_iteration(o: int, v: int) -> dict:
