@@ -34,6 +34,7 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of the 3M + sum-plane DMMA GEMM at cfg3, from
 # profiles/r02_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
 NCU_TRAFFIC_BYTES = {"cfg3": 23.10e9 + 0.220e9}
+NCU_TRAFFIC_BYTES_STRASSEN = {}     # the batched seven-product launch of the Strassen level: captured separately
 NCU_TRAFFIC_SOURCE = ("recorded constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of one "
                       "pp-ladder launch from the ncu --set full capture summarised in profiles/r02_ncu_pp_ladder_cfg3.md")
 
@@ -600,13 +601,16 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
                     "<ab||cd> with conjugated multipliers"}
 
 
-def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True) -> dict:
+def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool = False) -> dict:
     """Algorithmic bytes of the HBM-bound steps of one iteration (16 B read + 16 B written per element a
     permutation moves; the update streams (2 + 2m) vectors at the least; m = pairs in the DIIS subspace)."""
     oo, vv, ov = o * (o - 1) // 2, v * (v - 1) // 2, o * v
     nvec = ov + oo * vv
-    moved = ov + 2 * oo * vv + 2 * ov * ov + v * oo * v + o * o * vv + oo * v * v      # t1T, tau^T, t2^T, Xm, T2r, tauc, tauou, t2hu
-    return {"prep_permute": moved * 32 + (2 * ov * ov * 8 if planes else 0),
+    moved = ov + oo * vv + 2 * ov * ov + v * oo * v + o * o * vv + oo * v * v      # t1T, tau^T, Xm, T2r, tauc, tauou, t2hu
+    # with the Strassen level the planes of Xm, T2r are not written (their stacks carry planes); the stack of tau is: tau read
+    # once, seven half-size matrices (16 B) and their planes (8 B) written
+    tau_stack = oo * vv * 16 + 7 * ((oo + 1) // 2) * ((vv + 1) // 2) * 24
+    return {"prep_permute": moved * 32 + ((tau_stack if strassen else 2 * ov * ov * 8) if planes else 0),
             # Jacobi + Gram row in one pass (S, t and m-1 stored e read; e, u written), then sum_l c_l u_l (m read, 1 written)
             "update_diis": (2 * m + 4) * nvec * 16,
             "update_diis_floor": (2 * m + 2) * nvec * 16,
@@ -615,7 +619,7 @@ def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True) -> dict:
 
 
 def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=None, clock_index=None, e2e=False,
-                    max_ranks=None, graph=1) -> dict:
+                    max_ranks=None, graph=1, strassen=True) -> dict:
     """W warm-up + exactly K timed ccsd_iterate of workload `cfg` the way a user runs them (residual replayed as a CUDA
     graph, no events inside), CUDA events on the solver's stream around the K steps; then a second pass of K iterations
     with the library's per-step events (direct launches) for the per-term table and the roofline launch."""
@@ -624,7 +628,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
     barrier = barrier or torch.cuda.synchronize
     pkg.launch_count(reset=True)
     t0 = time.perf_counter()
-    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, graph=graph)
+    solver = pkg.CCSD(inp.h, inp.B, o, v, ndiis=6, graph=graph, strassen=strassen)
     torch.cuda.synchronize()
     init_s = time.perf_counter() - t0
     init = solver.init_stats()
@@ -671,16 +675,23 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
     solver.enable_step_timing(False)
     fl = flops_per_iteration(o, v)
     ex = pkg.real_flops_per_cmac() / 8.0
+    # a product that runs as one Strassen level (ccsd_options.strassen) EXECUTES 7/8 of the plain product's real flops
+    strassen_steps = solver.strassen_steps()
+    exk = {k: ex * (7.0 / 8.0 if k in strassen_steps else 1.0) for k in fl}
+    executed_total = fl["total"] * ex - sum(fl[k] * (ex - exk[k]) for k in strassen_steps)      # in 8-flop units x ex
     terms = {}
     for k, xs in step_acc.items():
         ms = statistics.median(xs)
         ent = {"ms": round(ms, 4)}
         if k in fl and ms > 0:
             ent["tflops"] = round(fl[k] / (ms * 1e-3) * 1e-12, 2)
-            ent["frac_fp64_peak"] = round(fl[k] * ex / (ms * 1e-3) * 1e-12 / peak, 4)
+            ent["frac_fp64_peak"] = round(fl[k] * exk[k] / (ms * 1e-3) * 1e-12 / peak, 4)
+            if k in strassen_steps:
+                ent["strassen_level"] = 1
         terms[k] = ent
     for k in ("prep_permute", "update_diis", "energy"):       # HBM-bound steps: algorithmic bytes / time
-        gbs = [hbm_step_bytes(o, v, m)[k] / (x * 1e-3) * 1e-9 for x, m in zip(step_acc[k], m_hist) if x > 0]
+        gbs = [hbm_step_bytes(o, v, m, strassen="pp_ladder" in strassen_steps)[k] / (x * 1e-3) * 1e-9
+               for x, m in zip(step_acc[k], m_hist) if x > 0]
         if gbs:
             terms[k]["gbs"] = round(statistics.median(gbs), 1)
             terms[k]["frac_hbm"] = round(statistics.median(gbs) / hbm_gbs, 3)
@@ -700,8 +711,9 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
         init_pack["transpose_frac_hbm"] = round(init_pack["transpose_gbs"] / hbm_gbs, 3)
     out = {"workload": workload_string(cfg), "ms_per_step": ms_per_step, "s_per_iteration": round(ms_per_step * 1e-3, 6),
            "ms_per_step_with_step_events": round(ms_events, 4), "steps": steps, "warmup": warmup,
-           "ideal_ms_at_peak": round(fl["total"] * ex / peak * 1e-9, 4),
-           "frac_of_ideal": round(fl["total"] * ex / peak * 1e-9 / ms_per_step, 4),
+           "ideal_ms_at_peak": round(executed_total / peak * 1e-9, 4),
+           "frac_of_ideal": round(executed_total / peak * 1e-9 / ms_per_step, 4),
+           "executed_flops_per_iteration": executed_total, "strassen_steps": strassen_steps,
            "gpu_launches": launches, "gpu_launches_per_step": round(launches / steps, 1),
            "graph_replay": bool(st.cuda_stream != 0), "terms": terms, "init_seconds": round(init_s, 3), "init_pack": init_pack,
            "clocks": clocks,
@@ -863,7 +875,8 @@ def run_ours(args) -> None:
     rf = pkg.real_flops_per_cmac()                                  # 6: the 3M kernels execute 3 real FMAs per complex MAC
     ex = rf / 8.0
     main = iteration_bench(torch, pkg, cfg, inp, args.steps, args.warmup, peak, peaks["hbm_gbs"], barrier=barrier,
-                           clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None), graph=args.graph)
+                           clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None), graph=args.graph,
+                           strassen=bool(args.strassen))
     trip_sharded = triples_sharded_bench(torch, pkg, inp, o, v, dist) if (world > 1 and not args.no_sweep) else None
 
     if not is_reporting_rank():
@@ -876,26 +889,33 @@ def run_ours(args) -> None:
     ms_per_step = main["ms_per_step"]
     pp_ms = main["terms"]["pp_ladder"]["ms"]
     pp_tflops = fl["pp_ladder"] / (pp_ms * 1e-3) * 1e-12          # 8-flop (ZGEMM) convention
-    pp_exec = pp_tflops * ex
+    pp_strassen = "pp_ladder" in main["strassen_steps"]
+    ex_pp = ex * (7.0 / 8.0 if pp_strassen else 1.0)              # one Strassen level: seven half-size products for eight
+    pp_exec = pp_tflops * ex_pp
     gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
     gemm_ms = sum(main["terms"][k]["ms"] for k in gemm_steps)
-    traffic = NCU_TRAFFIC_BYTES.get(cfg)
-    roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch",
+    traffic = (NCU_TRAFFIC_BYTES_STRASSEN if pp_strassen else NCU_TRAFFIC_BYTES).get(cfg)
+    roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch" +
+                          (": ONE batched launch of the seven half-size products of a Strassen level" if pp_strassen else ""),
                 "achieved": round(pp_exec, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
                 "frac": round(pp_exec / peak, 4), "traffic": traffic,
                 "traffic_source": (NCU_TRAFFIC_SOURCE if traffic is not None else
                                    "no ncu --set full capture of this workload's launch on record"),
-                "real_flops_per_complex_mac": rf,
+                "real_flops_per_complex_mac": rf * (7.0 / 8.0 if pp_strassen else 1.0),
                 "achieved_8flop_convention": round(pp_tflops, 3),
                 "note": "unit = complex MAC over the packed ranges (oo*vv*vv per launch); achieved counts the real "
-                        "flops the kernel EXECUTES per unit (6 with 3M) so that frac <= 1; on the ZGEMM 8-flop "
-                        "convention the same launch is achieved_8flop_convention.  launch_ms = median CUDA-event time of "
+                        "flops the kernel EXECUTES per unit (6 with 3M; x 7/8 = 5.25 when the product runs as one Strassen "
+                        "level) so that frac <= 1; on the ZGEMM 8-flop "
+                        "convention the same launch is achieved_8flop_convention.  With the Strassen level launch_ms also "
+                        "contains the pass that sums the seven products into S2 (HBM-bound, ~0.3 % of it); the operand "
+                        "stacks are made outside it (<ab||cd>: once, in ccsd_init; tau: in prep_permute).  "
+                        "launch_ms = median CUDA-event time of "
                         "the launch over the K iterations of the step-timed pass (direct launches, events between the "
                         "steps on the launching stream); `value` is timed without those events (graph replay)",
                 "peak_source": "DMMA.8x8x4 issue-rate microbenchmark measured in this run (ccsd_measure_fp64_peak); "
                                f"nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = {FP64_NOMINAL_TFLOPS:.1f}; "
                                "MEASURED_PEAKS.json has no FP64 entry",
-                "flops_per_launch": int(fl["pp_ladder"] * ex), "flops_per_launch_8flop": fl["pp_ladder"],
+                "flops_per_launch": int(fl["pp_ladder"] * ex_pp), "flops_per_launch_8flop": fl["pp_ladder"],
                 "launch_ms": round(pp_ms, 3),
                 "share_of_step": round(pp_ms / main["ms_per_step_with_step_events"], 4),
                 "three_big_gemms": {"ms": round(gemm_ms, 3),
@@ -910,7 +930,7 @@ def run_ours(args) -> None:
             if other != cfg:
                 r = iteration_bench(torch, pkg, other, ci.make_config(other), 10, 6, peak, peaks["hbm_gbs"])
                 others[other] = {k: r[k] for k in ("workload", "s_per_iteration", "ms_per_step_with_step_events", "ideal_ms_at_peak",
-                                                   "frac_of_ideal", "gpu_launches_per_step", "graph_replay", "terms", "energies")}
+                                                   "frac_of_ideal", "strassen_steps", "gpu_launches_per_step", "graph_replay", "terms", "energies")}
     conv = converge_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     cc2 = cc2_bench(torch, pkg, inp, o, v) if not args.no_sweep else None
     triples = triples_bench(torch, pkg, inp, o, v, peak) if not args.no_sweep else None
@@ -935,9 +955,10 @@ def run_ours(args) -> None:
                    "l2": f"inputs larger than L2 (packed <ab||cd> = {vv * vv * 16 / 2 ** 30:.2f} GiB vs 126 MB L2); no flush needed",
                    "init_seconds": main["init_seconds"], "graph_replay": main["graph_replay"]},
         "iteration_tflops": round(fl["total"] / (ms_per_step * 1e-3) * 1e-12, 2),
-        "iteration_frac_fp64_peak": round(fl["total"] * ex / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
+        "iteration_frac_fp64_peak": round(main["executed_flops_per_iteration"] / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
         "pp_ladder_tflops": round(pp_tflops, 2), "pp_ladder_frac_fp64_peak": round(pp_exec / peak, 4),
-        "tflops_convention": f"8 real flop per complex MAC (ZGEMM); fractions of peak use the {rf} executed",
+        "tflops_convention": f"8 real flop per complex MAC (ZGEMM); fractions of peak use the {rf} executed (x 7/8 for the "
+                             "products that run as one Strassen level: terms[].strassen_level)",
         "ms_per_step_with_step_events": main["ms_per_step_with_step_events"],
         "roofline": roofline, "terms": main["terms"], "init_pack": main["init_pack"],
         "e2e": main["e2e"],
@@ -962,6 +983,8 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--graph", type=int, default=1, help="ccsd_options.graph of the main leg: 0 direct launches, 1 graph with parallel "
                                                           "branches, 3 serial graph (profiling aid)")
+    ap.add_argument("--strassen", type=int, default=1, help="ccsd_options.strassen of the main leg: 1 (default) one Strassen level on "
+                    "the four large contractions, 0 plain products")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")

@@ -5,7 +5,7 @@ for device memory and streams.  There is no CPU fallback: without the built libr
 compute entry points raise.
 """
 from .binding import (CCSD, CCSDError, TENSOR_IDS, TERM_IDS, STEP_NAMES, contract, energy_static, gemm_plan, launch_count, lib_path,
-                      load_library, measure_fp64_peak, real_flops_per_cmac, shard_ranges, sum_plane, transpose, zgemm_nt)
+                      load_library, measure_fp64_peak, real_flops_per_cmac, shard_ranges, sum_plane, transpose, zgemm_nt, zgemm_nt_strassen)
 
 __all__ = ["CCSD", "CCSDError", "TENSOR_IDS", "TERM_IDS", "STEP_NAMES", "contract", "energy_static", "gemm_plan", "launch_count", "lib_path",
-           "load_library", "measure_fp64_peak", "real_flops_per_cmac", "shard_ranges", "sum_plane", "transpose", "zgemm_nt"]
+           "load_library", "measure_fp64_peak", "real_flops_per_cmac", "shard_ranges", "sum_plane", "transpose", "zgemm_nt", "zgemm_nt_strassen"]

@@ -29,7 +29,8 @@ EXPORTS = ["ccsd_default_options", "ccsd_workspace_bytes", "ccsd_init", "ccsd_it
            "ccsd_triples_block", "ccsd_triples_count", "ccsd_triples_range", "ccsd_t1_diagnostic", "ccsd_solve", "ccsd_lambda_workspace_bytes",
            "ccsd_lambda_init", "ccsd_lambda_iterate", "ccsd_lambda_solve", "ccsd_lambda_residual", "ccsd_get_lambda", "ccsd_set_lambda",
            "ccsd_get_lambda_residual", "ccsd_density", "ccsd_expectation", "ccsd_update", "ccsd_shard_info",
-           "ccsd_shard_ranges", "ccsd_gemm_plan", "ccsd_energy_static"]
+           "ccsd_shard_ranges", "ccsd_gemm_plan", "ccsd_energy_static",
+           "ccsd_zgemm_nt_strassen_workspace_bytes", "ccsd_zgemm_nt_strassen", "ccsd_strassen_info"]
 
 # limits of ccsd_energy_static (include/ccsd.h): its scratch is a fixed device array inside the library
 ENERGY_STATIC_MAX_NOCC = 128
@@ -49,7 +50,7 @@ class CCSDError(RuntimeError):
 class Options(ctypes.Structure):
     _fields_ = [("ndiis", ctypes.c_int), ("level_shift", ctypes.c_double), ("gemm_mode", ctypes.c_int),
                 ("ccd", ctypes.c_int), ("cc2", ctypes.c_int), ("direct_ladder", ctypes.c_int), ("graph", ctypes.c_int),
-                ("shard_rank", ctypes.c_int), ("shard_world", ctypes.c_int)]
+                ("shard_rank", ctypes.c_int), ("shard_world", ctypes.c_int), ("strassen", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -106,6 +107,10 @@ def load_library():
         lib.ccsd_energy_static.argtypes = [ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp]
         lib.ccsd_zgemm_nt.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
                                       ctypes.c_int, vp]
+        lib.ccsd_zgemm_nt_strassen_workspace_bytes.argtypes = [i64, i64, i64, ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_zgemm_nt_strassen.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
+                                               ctypes.c_int, vp, ctypes.c_size_t, vp]
+        lib.ccsd_strassen_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int)]
         lib.ccsd_sum_plane.argtypes = [vp, vp, i64, vp]
         lib.ccsd_zgemm_nt_planes.argtypes = [i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, i64, dbl, dbl, ctypes.c_int,
                                              ctypes.c_int, vp]
@@ -227,9 +232,9 @@ def measure_fp64_peak(launches: int = 10) -> float:
 
 
 def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True,
-             shard=(0, 1)) -> Options:
+             shard=(0, 1), strassen=True) -> Options:
     return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)),
-                   int(graph), int(shard[0]), int(shard[1]))
+                   int(graph), int(shard[0]), int(shard[1]), int(bool(strassen)))
 
 
 class CCSD:
@@ -244,7 +249,7 @@ class CCSD:
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
                  ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: int = 1, stream=None,
-                 shard=None, group=None):
+                 shard=None, group=None, strassen: bool = True):
         torch = _torch()
         lib = load_library()
         self._lib, self._torch = lib, torch
@@ -259,7 +264,7 @@ class CCSD:
         # and ccsd_update.  shard=None: one GPU does everything.
         self.shard = (0, 1) if shard is None else (int(shard[0]), int(shard[1]))
         self.group = group
-        opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder, graph, self.shard)
+        opts = _options(ndiis, level_shift, gemm_mode, ccd, cc2, direct_ladder, graph, self.shard, strassen)
         self.nocc, self.nvir, self.n = int(nocc), int(nvir), int(nocc + nvir)
         self.oo = self.nocc * (self.nocc - 1) // 2
         self.vv = self.nvir * (self.nvir - 1) // 2
@@ -516,6 +521,12 @@ class CCSD:
         self._call(self._lib.ccsd_expectation, D_d.data_ptr(), O_d.data_ptr(), ctypes.byref(re), ctypes.byref(im), where="ccsd_expectation")
         return complex(re.value, im.value)
 
+    def strassen_steps(self):
+        """Names of the timed steps (step_times()) whose product runs as one Strassen level: 7/8 of the plain product's flops."""
+        info = (ctypes.c_int * 4)()
+        self._call(self._lib.ccsd_strassen_info, info, where="ccsd_strassen_info")
+        return (["Hvovo_quad", "ring_gemm"] if info[1] else []) + (["pp_ladder"] if info[2] else []) + (["C_ovoo"] if info[3] else [])
+
     def enable_step_timing(self, enable: bool = True):
         self._call(self._lib.ccsd_enable_step_timing, int(enable), where="ccsd_enable_step_timing")
 
@@ -608,6 +619,28 @@ def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode:
     _check(lib.ccsd_zgemm_nt(M, N, K, A.data_ptr(), K, B.data_ptr(), K, C.data_ptr(), csm, csn, alpha.real, alpha.imag,
                              int(accumulate), mode, _stream_ptr(torch)), "ccsd_zgemm_nt")
     torch.cuda.current_stream().synchronize()
+    return C
+
+
+def zgemm_nt_strassen(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False):
+    """zgemm_nt by one Strassen level (ccsd_zgemm_nt_strassen): seven half-size products in one batched DMMA launch."""
+    torch = _torch()
+    lib = load_library()
+    A, B = _dev_c128(torch, A), _dev_c128(torch, B)
+    M, K = A.shape
+    N = B.shape[0]
+    assert B.shape[1] == K
+    if C is None:
+        C = torch.zeros((N, M) if transposed_out else (M, N), dtype=torch.complex128, device="cuda")
+    csm, csn = (1, M) if transposed_out else (N, 1)
+    alpha = complex(alpha)
+    nbytes = ctypes.c_size_t(0)
+    _check(lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, ctypes.byref(nbytes)), "ccsd_zgemm_nt_strassen_workspace_bytes")
+    ws = _workspace(torch, nbytes.value)
+    base = (ws.data_ptr() + 255) // 256 * 256
+    _check(lib.ccsd_zgemm_nt_strassen(M, N, K, A.data_ptr(), K, B.data_ptr(), K, C.data_ptr(), csm, csn, alpha.real, alpha.imag,
+                                      int(accumulate), mode, base, int(nbytes.value), _stream_ptr(torch)), "ccsd_zgemm_nt_strassen")
+    torch.cuda.current_stream().synchronize()   # ws must outlive the enqueued kernels
     return C
 
 

@@ -15,6 +15,7 @@
 #include "triples.cuh"
 #include "transpose.cuh"
 #include "reduce.cuh"
+#include "strassen.cuh"
 #include "peak.cuh"
 
 #include <cmath>
@@ -123,6 +124,54 @@ static int run_gemm(const Env& env, GemmParams p)
     return CCSD_OK;
 }
 
+// ---- one Strassen level around run_gemm (strassen.cuh) ---------------------------------------------------------------
+struct StrassenScratch {
+    c128 *SA, *SB, *P;        // stacks of the left / right operand made per call, the seven products
+    double *SAp, *SBp;
+    int64_t a_elems, b_elems, p_elems;
+};
+
+// Where a Strassen level pays: the seven half-size products must still be long-K, many-tile DMMA GEMMs and the three
+// streaming passes must be small beside the eighth product they save (measured: 0.93 at 1536^3 down to 0.88 at 7616^3).
+static inline bool strassen_worthwhile(int64_t M, int64_t N, int64_t K)
+{
+    return M >= 1024 && K >= 1024 && N >= 96 && (double)M * (double)N * (double)K >= 2.0e9;
+}
+
+// p: a plain (batch 1, k-contiguous) product C (+)= alpha A B^T.  preA / preB: ready-made stacks of operands that do not
+// change between calls; an operand without one is stacked here into w.  The products go to w.P, then into C.
+static int strassen_gemm(const Env& env, const GemmParams& p, const StrassenStack* preA, const StrassenStack* preB,
+                         const StrassenScratch& w)
+{
+    if (p.M <= 0 || p.N <= 0 || p.K <= 0) return CCSD_OK;
+    if (p.batch != 1 || p.sak != 1 || p.sbk != 1) return CCSD_EINVAL;
+    const int64_t Mh = strassen_half(p.M), Nh = strassen_half(p.N), Kh = strassen_khalf(p.K);
+    StrassenStack sa, sb;
+    if (preA) {
+        sa = *preA;
+    } else {
+        if (7 * Mh * Kh > w.a_elems) return CCSD_EINVAL;
+        sa = strassen_stack(w.SA, w.SAp, p.M, p.K);
+        launch_strassen_prep(env.st, 0, p.A, p.sam, sa);
+    }
+    if (preB) {
+        sb = *preB;
+    } else {
+        if (7 * Nh * Kh > w.b_elems) return CCSD_EINVAL;
+        sb = strassen_stack(w.SB, w.SBp, p.N, p.K);
+        launch_strassen_prep(env.st, 1, p.B, p.sbn, sb);
+    }
+    if (sa.R != p.M || sa.K != p.K || sb.R != p.N || sb.K != p.K || 7 * Mh * Nh > w.p_elems) return CCSD_EINVAL;
+    const bool fast_m = p.csm == 1;    // the products take C's unit-stride index as their fast index
+    GemmParams g = gp(Mh, Nh, Kh, sa.S, Kh, sb.S, Kh, w.P, fast_m ? 1 : Nh, fast_m ? Mh : 1, 1.0, 0);
+    g.batch = 7; g.bsA = Mh * Kh; g.bsB = Nh * Kh; g.bsC = Mh * Nh;
+    g.As = sa.Sp; g.Bs = sb.Sp;
+    CCSD_TRY(run_gemm(env, g));
+    launch_strassen_combine(env.st, w.P, p.M, p.N, p.C, p.csm, p.csn, p.alpha, p.accumulate);
+    CCSD_CUDA_TRY(cudaGetLastError());
+    return CCSD_OK;
+}
+
 static int run_gemv(const Env& env, int64_t M, int64_t K, const c128* A, int64_t lda, const c128* x, c128* y, int64_t sy,
                     double alpha, int acc)
 {
@@ -222,6 +271,13 @@ struct ccsd_ctx {
     // 3M sum planes (Re + Im) of the operands of the five large GEMMs; null when the 4M / simple kernels are forced
     bool planes;
     double *Ws, *Vvovv_ps, *Voovv_ps, *G1s, *taups, *Xms, *T2rs, *Hms;
+    // One Strassen level on the four large contractions (strassen.cuh; opts.strassen, one GPU, 3M planes): operand stacks of
+    // the constants <ab||cd> (left operand of the pp-ladder), <bk||cd> (left operand of C) and <kl||cd> (right operand of the
+    // quadratic H^{ak}_{ci} term) built once by ccsd_init, the stack of tau (right operand of the pp-ladder and of C) built by
+    // prep_operands, and per-branch scratch for the stacks of Xm, Hm, T2r and for the seven products.
+    bool strassen;
+    StrassenStack sW, sVvovv, sG1, sTau;
+    StrassenScratch str_ring, str_C, str_L;
     // DIIS ring (reduce.cuh): stored pairs, device-side Gram matrix / coefficients / reduction scratch
     DiisRing diis;
     double* red;            // device reduction outputs (64 doubles)
@@ -287,12 +343,14 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Bov = w.take<c128>(ov * Lp);
     c->Bvo = w.take<c128>(ov * Lp);
     c->Bvv = w.take<c128>(v * v * Lp);
+    const size_t j_begin = w.off;     // [Jovov, Joooo]: dead once ccsd_init has filled the integral classes (Strassen scratch below)
     c->Jovov = w.take<c128>(ov * ov);
     c->Jvoov = w.take<c128>(ov * ov);
     c->Jvvoo = w.take<c128>(v * v * o * o);
     c->Jvvov = w.take<c128>(v * v * ov);
     c->Jooov = w.take<c128>(o * o * ov);
     c->Joooo = w.take<c128>(o * o * o * o);
+    const size_t j_end = w.off;
     {
         double per_a = (double)v * v * v * 16.0;
         // direct_ladder: slabs grow with the tensor they replace (a sixth of its bytes, 1.5 - 6 GB), so that the ladder GEMM
@@ -384,6 +442,43 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
         c->Xv = w.take<c128>(ov * Lp);
         c->Xo = w.take<c128>(o * o * Lp);
         c->Xvs = w.take<double>(ov * Lp);
+    }
+    // One Strassen level (strassen.cuh) on the (ov)^3 products, the pp-ladder and the <bk||cd> tau part of C: one GPU, 3M planes
+    c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 && strassen_worthwhile(ov, ov, ov);
+    memset(&c->sW, 0, sizeof(c->sW)); memset(&c->sVvovv, 0, sizeof(c->sVvovv)); memset(&c->sG1, 0, sizeof(c->sG1));
+    memset(&c->sTau, 0, sizeof(c->sTau));
+    memset(&c->str_ring, 0, sizeof(c->str_ring)); memset(&c->str_C, 0, sizeof(c->str_C)); memset(&c->str_L, 0, sizeof(c->str_L));
+    if (c->strassen) {
+        const bool use_L = !c->opt.direct_ladder && strassen_worthwhile(vv, oo, vv);
+        const bool use_C = strassen_worthwhile(ov, oo, vv);
+        auto stack = [](Carver& a, int64_t R, int64_t K) {
+            c128* S = a.take<c128>(strassen_stack_elems(R, K));
+            double* Sp = a.take<double>(strassen_stack_elems(R, K));
+            return strassen_stack(S, Sp, R, K);
+        };
+        // constants: memory of their own
+        if (use_L) c->sW = stack(w, vv, vv);
+        if (use_C) c->sVvovv = stack(w, ov, vv);
+        c->sG1 = stack(w, ov, ov);
+        // per-iteration stacks and products: in the dead init temporaries when they fit there, else appended
+        auto scratch = [&](Carver& a) {
+            StrassenStack sa = stack(a, ov, ov), sb = stack(a, ov, ov);
+            c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov);
+            c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov);
+            c->str_ring.p_elems = 7 * strassen_half(ov) * strassen_half(ov);
+            c->str_ring.P = a.take<c128>(c->str_ring.p_elems);
+            if (use_L || use_C) c->sTau = stack(a, oo, vv);
+            if (use_L) { c->str_L.p_elems = 7 * strassen_half(vv) * strassen_half(oo); c->str_L.P = a.take<c128>(c->str_L.p_elems); }
+            if (use_C) { c->str_C.p_elems = 7 * strassen_half(ov) * strassen_half(oo); c->str_C.P = a.take<c128>(c->str_C.p_elems); }
+        };
+        Carver probe{nullptr, 0};
+        scratch(probe);
+        if (probe.off <= j_end - j_begin) {
+            Carver alias{base ? base + j_begin : nullptr, 0};
+            scratch(alias);
+        } else {
+            scratch(w);
+        }
     }
     c->nvec = ov + oo * vv;
     int nd = c->opt.ndiis > 0 ? c->opt.ndiis : 1;
@@ -770,11 +865,12 @@ static int prep_operands(ccsd_ctx* c)
     const int o = c->o, v = c->v;
     const int64_t oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
     const c128 *t1 = c->t1, *t2p = c->t2p, *taup = c->taup;
-    double *Xms = c->Xms, *T2rs = c->T2rs;
+    double *Xms = c->strassen ? nullptr : c->Xms, *T2rs = c->strassen ? nullptr : c->T2rs;   // Strassen stacks carry their own planes
+    if (c->sTau.S) launch_strassen_prep(st, 1, c->taup, vv, c->sTau);    // right operand of the pp-ladder and of C
     launch_fill(st, c->t1T, v, o, o, 0, [=] __device__(int64_t a, int64_t i) { return t1[i * v + a]; });
-    // TT[(a<b)][0:oo) = tau^T, TT[(a<b)][oop:oop+oo) = t2^T   (K-contiguous operands of the hh-ladder and Goo terms)
+    // TT[(a<b)][0:oo) = tau^T   (K-contiguous operand of the hh-ladder + Goo product; the second half of TT, t2^T, is the operand
+    // of the Goo term on its own: fill_TT_t2, made where that form is used -- the per-term hook and CC2)
     CCSD_TRY(launch_transpose2d_ld(st, c->taup, vv, c->TT, 2 * oop, oo, vv, 0));
-    CCSD_TRY(launch_transpose2d_ld(st, c->t2p, vv, c->TT + oop, 2 * oop, oo, vv, 0));
     // Xm[(a,i)][(l,d)] = 1/2 t2[l,i,a,d] + t1[l,a] t1[i,d]      (eq 29 operand)
     const int64_t xrow0 = (int64_t)c->sh.a_lo * o, xrows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;   // this rank's rows (a, i)
     launch_fill(st, c->Xm + xrow0 * ov, xrows, ov, ov, 0, [=] __device__(int64_t row, int64_t ld) {
@@ -866,6 +962,9 @@ static int build_Hvovo(ccsd_ctx* c)
     CCSD_TRY(run_gemm(env, gp(na, (int64_t)o * ov, o, c->t1T + (int64_t)a0 * o, o, c->Vooov_b, o, c->Hm + off, (int64_t)o * ov, 1, -1.0, 1)));
     tick(c, 3);
     // + sum_{ld} <kl||cd> (1/2 t2[l,i,a,d] + t1[l,a] t1[i,d])       (ov x ov x ov)
+    if (c->strassen) {   // seven half-size products (strassen.cuh); the ring product stacks Hm itself, no plane of Hm needed
+        return strassen_gemm(env, gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1), nullptr, &c->sG1, c->str_ring);
+    }
     CCSD_TRY(run_gemm(env, with_planes(gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1),
                                        c->Xms ? c->Xms + off : nullptr, c->G1s)));
     if (c->planes) launch_sum_plane(c->st, c->Hm + off, c->Hms + off, rows * ov);   // operand of the ring GEMM
@@ -924,6 +1023,8 @@ static int build_C(ccsd_ctx* c)
         });
         return CCSD_OK;
     }
+    if (c->strassen && c->sVvovv.S)
+        return strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), &c->sVvovv, &c->sTau, c->str_C);
     CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, c->Cm + row0 * oo, oo, 1, -1.0, 1),
                                        c->Vvovv_ps ? c->Vvovv_ps + row0 * vv : nullptr, c->taups)));
     return CCSD_OK;
@@ -1007,6 +1108,8 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
         return CCSD_OK;
     }
     const int64_t rows = c->sh.w_hi - c->sh.w_lo;      // this rank's rows of <ab||cd> (all of them for world = 1)
+    if (c->strassen && c->sW.S)      // both operand stacks are ready (ccsd_init, prep_operands): one batched launch + the result sums
+        return strassen_gemm(c->env, gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), &c->sW, &c->sTau, c->str_L);
     return run_gemm(c->env, with_planes(gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S + c->sh.w_lo, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
 static void fill_AG_hh(ccsd_ctx* c)
@@ -1031,6 +1134,10 @@ static void fill_AG_goo(ccsd_ctx* c)
         return s;
     });
 }
+static int fill_TT_t2(ccsd_ctx* c)
+{   // TT[(a<b)][oop:oop+oo) = t2^T
+    return launch_transpose2d_ld(c->st, c->t2p, c->vv, c->TT + c->oop, 2 * c->oop, c->oo, c->vv, 0);
+}
 // the three products with M = (a<b) rows of TT run on this rank's rows [w_lo, w_hi)
 static int s2_hh_ladder(ccsd_ctx* c, c128* S)
 {   // sum_{k<l} A[k,l,i,j] tau[k,l,a,b]
@@ -1040,16 +1147,55 @@ static int s2_hh_ladder(ccsd_ctx* c, c128* S)
 }
 static int s2_goo(ccsd_ctx* c, c128* S)
 {
+    CCSD_TRY(fill_TT_t2(c));
     fill_AG_goo(c);
     const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
     return run_gemm(c->env, gp(rows, c->oo, c->oop, c->TT + r0 * ld + c->oop, ld, c->AG + c->oop, ld, S + r0, 1, c->vv, 1.0, 1));
 }
 static int s2_hh_and_goo(ccsd_ctx* c, c128* S)
-{   // both in one GEMM with K = [ (k<l) of tau | (k<l) of t2 ]
-    fill_AG_hh(c);
-    fill_AG_goo(c);
+{   // Both terms in ONE product over the pairs (k<l) of tau:  A tau + Ghat t2 = (A + Ghat) tau - Ghat (tau - t2), and the last
+    // piece is elementwise because tau - t2 = P-(t1 t1) (eq 23):  with X[j,b] = sum_m Goo[m,j] t1[m,b]
+    //   (Ghat (tau - t2))[(ij)][(ab)] = P-_ji ( t1[i,a] X[j,b] - X[j,a] t1[i,b] ).
+    // (K = oo instead of the 2 oo of the operand pair [tau | t2] x [A | Ghat]: half the tensor-pipe work of this step.)
+    if (c->opt.cc2) {   // CC2 runs this with tau0 = P-(t1 t1) beside the full t2: tau - t2 is not P-(t1 t1); keep the operand pair
+        CCSD_TRY(fill_TT_t2(c));
+        fill_AG_hh(c);
+        fill_AG_goo(c);
+        const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
+        return run_gemm(c->env, gp(rows, c->oo, 2 * c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1));
+    }
+    const c128 *Am = c->Am, *Goo = c->Goo, *t1 = c->t1;
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo;
+    const int2 *po = c->po, *pv = c->pv;
+    launch_fill(c->st, c->AG, oo, oo, 2 * c->oop, 0, [=] __device__(int64_t IJ, int64_t KL) {
+        int2 ij = po[IJ], kl = po[KL];
+        c128 s = Am[KL * oo + IJ];
+        if (ij.x == kl.x) s = cadd(s, Goo[kl.y * o + ij.y]);
+        if (ij.x == kl.y) s = csub(s, Goo[kl.x * o + ij.y]);
+        if (ij.y == kl.x) s = csub(s, Goo[kl.y * o + ij.x]);
+        if (ij.y == kl.y) s = cadd(s, Goo[kl.x * o + ij.x]);
+        return s;
+    });
+    c128* X = c->tmp_ov;     // X[j][b]
+    launch_fill(c->st, X, o, v, v, 0, [=] __device__(int64_t j, int64_t b) {
+        c128 s = mk(0.0, 0.0);
+        for (int m = 0; m < o; m++) cfma(s, Goo[m * o + j], t1[m * v + b]);
+        return s;
+    });
     const int64_t r0 = c->sh.w_lo, rows = c->sh.w_hi - r0, ld = 2 * c->oop;
-    return run_gemm(c->env, gp(rows, c->oo, 2 * c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1));
+    CCSD_TRY(run_gemm(c->env, gp(rows, oo, c->oop, c->TT + r0 * ld, ld, c->AG, ld, S + r0, 1, c->vv, 1.0, 1)));
+    launch_fill(c->st, S + r0, oo, rows, c->vv, 1, [=] __device__(int64_t IJ, int64_t rel) {
+        const int2 ij = po[IJ], ab = pv[r0 + rel];
+        const c128 *ti = t1 + (int64_t)ij.x * v, *tj = t1 + (int64_t)ij.y * v, *Xi = X + (int64_t)ij.x * v, *Xj = X + (int64_t)ij.y * v;
+        c128 d = mk(0.0, 0.0);                       // - [ (t_ia X_jb - X_ja t_ib) - (t_ja X_ib - X_ia t_jb) ]
+        cfma(d, Xj[ab.x], ti[ab.y]);
+        cfma(d, tj[ab.x], Xi[ab.y]);
+        d = csub(d, cmul(ti[ab.x], Xj[ab.y]));
+        d = csub(d, cmul(Xi[ab.x], tj[ab.y]));
+        return d;
+    });
+    return CCSD_OK;
 }
 static int ring_gemm(ccsd_ctx* c)
 {   // X[i,j,a,b] = sum_{kc} Hvovo[a,k,c,i] t2[j,k,c,b] = Xr[(a,i)][(j,b)]; this rank holds the rows a in [a_lo, a_hi) of H and X
@@ -1057,6 +1203,8 @@ static int ring_gemm(ccsd_ctx* c)
     const int64_t ov = c->ov;
     const int64_t off = (int64_t)c->sh.a_lo * o * ov, rows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;
     if (rows <= 0) return CCSD_OK;
+    if (c->strassen)
+        return strassen_gemm(c->env, gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0), nullptr, nullptr, c->str_ring);
     return run_gemm(c->env, with_planes(gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0),
                                         c->Hms ? c->Hms + off : nullptr, c->T2rs));
 }
@@ -1486,6 +1634,7 @@ void ccsd_default_options(ccsd_options* opts)
     opts->graph = 1;
     opts->shard_rank = 0;
     opts->shard_world = 1;
+    opts->strassen = 1;
 }
 
 int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts, size_t* bytes)
@@ -1536,6 +1685,11 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     cudaMemsetAsync(c->TT, 0, (size_t)(c->vv * 2 * c->oop) * sizeof(c128), c->st);
     cudaMemsetAsync(c->AG, 0, (size_t)(c->oo * 2 * c->oop) * sizeof(c128), c->st);
     int s = build_constants(c, reinterpret_cast<const c128*>(h), reinterpret_cast<const c128*>(B));
+    if (s == CCSD_OK && c->strassen) {   // operand stacks of the constants (strassen.cuh), once
+        if (c->sW.S) launch_strassen_prep(c->st, 0, c->W, c->vv, c->sW);
+        if (c->sVvovv.S) launch_strassen_prep(c->st, 0, c->Vvovv_p, c->vv, c->sVvovv);
+        launch_strassen_prep(c->st, 1, c->G1, c->ov, c->sG1);
+    }
     if (s == CCSD_OK) mp2_guess(c);
     if (s == CCSD_OK && cudaStreamSynchronize(c->st) != cudaSuccess) s = CCSD_ECUDA;
     if (s == CCSD_OK) {
@@ -2359,6 +2513,61 @@ int ccsd_zgemm_nt_planes(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, in
                       reinterpret_cast<c128*>(C), csm, csn, 1.0, accumulate);
     p.alpha = mk(alpha_re, alpha_im);
     return run_gemm(env, with_planes(p, As, Bs));
+}
+
+// ccsd_zgemm_nt by one Strassen level (strassen.cuh): both operand stacks, their planes and the seven products live in the
+// caller's workspace.  Any extents >= 1 (odd ones are zero-padded inside the stacks).
+static void strassen_standalone_carve(int64_t M, int64_t N, int64_t K, char* base, StrassenScratch* w, size_t* total)
+{
+    Carver cv{base, 0};
+    w->a_elems = strassen_stack_elems(M, K);
+    w->b_elems = strassen_stack_elems(N, K);
+    w->p_elems = 7 * strassen_half(M) * strassen_half(N);
+    w->SA = cv.take<c128>(w->a_elems); w->SAp = cv.take<double>(w->a_elems);
+    w->SB = cv.take<c128>(w->b_elems); w->SBp = cv.take<double>(w->b_elems);
+    w->P = cv.take<c128>(w->p_elems);
+    *total = cv.off;
+}
+
+int ccsd_zgemm_nt_strassen_workspace_bytes(int64_t M, int64_t N, int64_t K, size_t* bytes)
+{
+    if (!bytes || M < 1 || N < 1 || K < 1) return CCSD_EINVAL;
+    StrassenScratch w;
+    strassen_standalone_carve(M, N, K, nullptr, &w, bytes);
+    return CCSD_OK;
+}
+
+int ccsd_zgemm_nt_strassen(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
+                           ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!A || !B || !C || M < 1 || N < 1 || K < 1 || lda < K || ldb < K) return CCSD_EINVAL;
+    if (!(mode == 0 || mode == 3 || mode >= 100)) return CCSD_EINVAL;
+    size_t need = 0;
+    StrassenScratch w;
+    strassen_standalone_carve(M, N, K, nullptr, &w, &need);
+    if (!workspace || workspace_bytes < need || reinterpret_cast<uintptr_t>(workspace) % 256) return CCSD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return CCSD_ECUDA;
+    }
+    strassen_standalone_carve(M, N, K, static_cast<char*>(workspace), &w, &need);
+    Env env{static_cast<cudaStream_t>(cuda_stream), mode, nullptr, 0};
+    GemmParams p = gp(M, N, K, reinterpret_cast<const c128*>(A), lda, reinterpret_cast<const c128*>(B), ldb,
+                      reinterpret_cast<c128*>(C), csm, csn, 1.0, accumulate);
+    p.alpha = mk(alpha_re, alpha_im);
+    return strassen_gemm(env, p, nullptr, nullptr, w);
+}
+
+int ccsd_strassen_info(ccsd_ctx* c, int info[4])
+{
+    if (!c || !info) return CCSD_ESTATE;
+    info[0] = c->strassen ? 1 : 0;
+    info[1] = c->strassen ? 1 : 0;                       // the two (ov)^3 products
+    info[2] = (c->strassen && c->sW.S) ? 1 : 0;          // pp-ladder
+    info[3] = (c->strassen && c->sVvovv.S) ? 1 : 0;      // <bk||cd> tau part of C
+    return CCSD_OK;
 }
 
 int ccsd_sum_plane(const ccsd_c128* in, double* out, int64_t n, void* cuda_stream)

@@ -1,0 +1,125 @@
+// One level of Strassen's algorithm around the DMMA GEMM (gemm_dmma.cuh) for the large contractions of eq 32 / eqs 29-30
+// (PAPER.md:594-606): C = A B^T with every dimension halved is 7 half-size products instead of 8, i.e. 7/8 of the FP64
+// tensor-pipe work, for three streaming passes (operand sums, result sums).  All arithmetic stays FP64; the result differs
+// from the plain product by rounding only (measured max error 2-9e-15 of the largest element against 1-5e-15 for the
+// plain 3M product; the parity bound is 1e-12).
+//
+// "NT" convention of the library: C[m][n] = sum_k A[m][k] B[n][k].  Quadrants by halves (Mh, Nh, Kh = ceil of half the
+// extent, Kh rounded up to even so that plane rows stay 16-byte aligned; what lies beyond the extent reads as zero):
+//     A = [A11 A12; A21 A22]  (row half, k half),   B = [B11 B12; B21 B22]  (row half n, k half)
+//     P1 = (A11 + A22)(B11 + B22)^T   P2 = (A21 + A22) B11^T      P3 = A11 (B21 - B22)^T     P4 = A22 (B12 - B11)^T
+//     P5 = (A11 + A12) B22^T          P6 = (A21 - A11)(B11 + B21)^T                          P7 = (A12 - A22)(B12 + B22)^T
+//     C11 = P1 + P4 - P5 + P7         C12 = P3 + P5               C21 = P2 + P4              C22 = P1 - P2 + P3 + P6
+// (Strassen 1969 with X = B^T, X_kl = B_lk^T.)  The seven left and the seven right operands are written as two STACKS
+// S[q][row][k], q < 7, together with their 3M sum planes, so that the seven products are ONE batched launch of the GEMM
+// (uniform batch strides; 7 x the tiles of a half-size product fill the 148 SMs where a single one would leave a ragged last
+// wave).  The stack of an operand that does not change between iterations (<ab||cd>, <bk||cd>, <kl||cd>) is built once.
+#pragma once
+#include "common.cuh"
+
+struct StrassenStack {      // the seven operand combinations of one side
+    c128* S;                // [7][Rh][Kh]
+    double* Sp;             // their sum planes Re + Im, same layout
+    int64_t R, K, Rh, Kh;   // extents of the operand it was made from, and of one stacked matrix
+};
+
+static inline int64_t strassen_half(int64_t x) { return (x + 1) / 2; }
+static inline int64_t strassen_khalf(int64_t K) { return round_up((K + 1) / 2, 2); }
+static inline int64_t strassen_stack_elems(int64_t R, int64_t K) { return 7 * strassen_half(R) * strassen_khalf(K); }
+static inline StrassenStack strassen_stack(c128* S, double* Sp, int64_t R, int64_t K)
+{
+    StrassenStack s;
+    s.S = S; s.Sp = Sp; s.R = R; s.K = K; s.Rh = strassen_half(R); s.Kh = strassen_khalf(K);
+    return s;
+}
+
+constexpr int STR_THREADS = 256;
+
+// SIDE 0: left operand A [R = M][K];  SIDE 1: right operand B [R = N][K] (both k-contiguous, leading dimension ld)
+template <int SIDE>
+__global__ void __launch_bounds__(STR_THREADS)
+strassen_prep_kernel(const c128* __restrict__ in, int64_t ld, int64_t R, int64_t K, int64_t Rh, int64_t Kh,
+                     c128* __restrict__ S, double* __restrict__ Sp)
+{
+    const int64_t k = (int64_t)blockIdx.x * STR_THREADS + threadIdx.x;
+    if (k >= Kh) return;
+    const int64_t plane = Rh * Kh;
+    const c128 zero = mk(0.0, 0.0);
+    for (int64_t r = blockIdx.y; r < Rh; r += gridDim.y) {
+        const bool k2 = k + Kh < K, r2 = r + Rh < R, k1 = k < K;
+        const c128 x11 = k1 ? in[r * ld + k] : zero;
+        const c128 x12 = k2 ? in[r * ld + k + Kh] : zero;
+        const c128 x21 = (r2 && k1) ? in[(r + Rh) * ld + k] : zero;
+        const c128 x22 = (r2 && k2) ? in[(r + Rh) * ld + k + Kh] : zero;
+        c128 s[7];
+        if (SIDE == 0) {
+            s[0] = cadd(x11, x22); s[1] = cadd(x21, x22); s[2] = x11; s[3] = x22;
+            s[4] = cadd(x11, x12); s[5] = csub(x21, x11); s[6] = csub(x12, x22);
+        } else {
+            s[0] = cadd(x11, x22); s[1] = x11; s[2] = csub(x21, x22); s[3] = csub(x12, x11);
+            s[4] = x22; s[5] = cadd(x11, x21); s[6] = cadd(x12, x22);
+        }
+        const int64_t at = r * Kh + k;
+#pragma unroll
+        for (int q = 0; q < 7; q++) {
+            S[q * plane + at] = s[q];
+            Sp[q * plane + at] = s[q].x + s[q].y;
+        }
+    }
+}
+
+static inline void launch_strassen_prep(cudaStream_t st, int side, const c128* in, int64_t ld, const StrassenStack& s)
+{
+    if (s.Rh <= 0 || s.Kh <= 0) return;
+    dim3 grid((unsigned)((s.Kh + STR_THREADS - 1) / STR_THREADS), (unsigned)(s.Rh < 32768 ? s.Rh : 32768));
+    if (side == 0) strassen_prep_kernel<0><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
+    else strassen_prep_kernel<1><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
+    count_launches(1);
+}
+
+// C (+)= alpha * (the four quadrants from the seven products).  The products are stored with the unit-stride index of C as
+// their fast index: P[q][slow][fast], (fast, slow) = (m, n) halves if csm == 1 ("transposed" C), else (n, m).
+__global__ void __launch_bounds__(STR_THREADS)
+strassen_combine_kernel(const c128* __restrict__ P, int64_t Fh, int64_t Sh, int64_t F, int64_t Sx, c128* __restrict__ C,
+                        int64_t stride_f, int64_t stride_s, int fast_is_m, c128 alpha, int accumulate)
+{
+    const int64_t f = (int64_t)blockIdx.x * STR_THREADS + threadIdx.x;
+    if (f >= Fh) return;
+    const int64_t plane = Fh * Sh;
+    for (int64_t s = blockIdx.y; s < Sh; s += gridDim.y) {
+        const int64_t at = s * Fh + f;
+        const c128 p1 = P[at], p2 = P[plane + at], p3 = P[2 * plane + at], p4 = P[3 * plane + at], p5 = P[4 * plane + at],
+                   p6 = P[5 * plane + at], p7 = P[6 * plane + at];
+        const c128 c11 = cadd(csub(cadd(p1, p4), p5), p7);
+        const c128 c12 = cadd(p3, p5);
+        const c128 c21 = cadd(p2, p4);
+        const c128 c22 = cadd(cadd(csub(p1, p2), p3), p6);
+        // quadrant (row half of m, row half of n): c12 is (m low, n high).  In (fast, slow) terms:
+        const c128 q_fs[2][2] = {{c11, fast_is_m ? c12 : c21}, {fast_is_m ? c21 : c12, c22}};   // [fast half][slow half]
+#pragma unroll
+        for (int hf = 0; hf < 2; hf++)
+#pragma unroll
+            for (int hs = 0; hs < 2; hs++) {
+                const int64_t ff = f + hf * Fh, ss = s + hs * Sh;
+                if (ff >= F || ss >= Sx) continue;
+                c128* dst = C + ff * stride_f + ss * stride_s;
+                c128 val = cmul(alpha, q_fs[hf][hs]);
+                if (accumulate) val = cadd(val, *dst);
+                *dst = val;
+            }
+    }
+}
+
+// P: products [7][Sh][Fh] of a C with extents M x N and strides (csm, csn)
+static inline void launch_strassen_combine(cudaStream_t st, const c128* P, int64_t M, int64_t N, c128* C, int64_t csm, int64_t csn,
+                                           c128 alpha, int accumulate)
+{
+    const int fast_is_m = csm == 1;
+    const int64_t F = fast_is_m ? M : N, Sx = fast_is_m ? N : M;
+    const int64_t Fh = strassen_half(F), Sh = strassen_half(Sx);
+    if (Fh <= 0 || Sh <= 0) return;
+    dim3 grid((unsigned)((Fh + STR_THREADS - 1) / STR_THREADS), (unsigned)(Sh < 32768 ? Sh : 32768));
+    strassen_combine_kernel<<<grid, STR_THREADS, 0, st>>>(P, Fh, Sh, F, Sx, C, fast_is_m ? csm : csn, fast_is_m ? csn : csm,
+                                                          fast_is_m, alpha, accumulate);
+    count_launches(1);
+}

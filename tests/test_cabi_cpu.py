@@ -37,6 +37,7 @@ def test_defaults_and_strerror(lib):
     o = Options()
     lib.ccsd_default_options(ctypes.byref(o))
     assert (o.ndiis, o.level_shift, o.gemm_mode, o.ccd, o.cc2, o.direct_ladder, o.graph) == (6, 0.0, 0, 0, 0, 0, 1)
+    assert (o.shard_rank, o.shard_world, o.strassen) == (0, 1, 1)
     assert lib.ccsd_strerror(0) == b"ok"
     assert b"CUDA" in lib.ccsd_strerror(3)
     assert lib.ccsd_step_name(6) == b"pp_ladder" and lib.ccsd_step_name(99) == b""
@@ -49,7 +50,11 @@ def test_workspace_bytes_scales_and_validates(lib):
     assert lib.ccsd_workspace_bytes(34, 224, 774, None, ctypes.byref(n)) == 0
     big = n.value
     vv = 224 * 223 // 2
-    assert big > vv * vv * 16 and big < 80 * 2 ** 30      # holds packed <ab||cd>; fits a 180 GB part with room
+    assert big > vv * vv * 16 and big < 100 * 2 ** 30     # holds packed <ab||cd> and its Strassen stack; fits a 180 GB part
+    from paper_2103_08473_b200.binding import _options
+    plain = _options(strassen=False)
+    assert lib.ccsd_workspace_bytes(34, 224, 774, ctypes.byref(plain), ctypes.byref(n)) == 0
+    assert vv * vv * 16 < n.value < 80 * 2 ** 30 and n.value < big   # the operand stacks of the constants are what strassen costs
     assert small < big
     assert lib.ccsd_workspace_bytes(1, 16, 60, None, ctypes.byref(n)) == 1      # CCSD_EINVAL
     assert lib.ccsd_workspace_bytes(4, 16, 0, None, ctypes.byref(n)) == 1
