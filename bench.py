@@ -619,7 +619,7 @@ def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool =
 
 
 def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=None, clock_index=None, e2e=False,
-                    max_ranks=None, graph=1, strassen=True) -> dict:
+                    max_ranks=None, graph=1, strassen=1) -> dict:
     """W warm-up + exactly K timed ccsd_iterate of workload `cfg` the way a user runs them (residual replayed as a CUDA
     graph, no events inside), CUDA events on the solver's stream around the K steps; then a second pass of K iterations
     with the library's per-step events (direct launches) for the per-term table and the roofline launch."""
@@ -677,7 +677,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
     ex = pkg.real_flops_per_cmac() / 8.0
     # a product that runs as one Strassen level (ccsd_options.strassen) EXECUTES 7/8 of the plain product's real flops
     strassen_steps = solver.strassen_steps()
-    exk = {k: ex * (7.0 / 8.0 if k in strassen_steps else 1.0) for k in fl}
+    exk = {k: ex * (7.0 / 8.0) ** strassen_steps.get(k, 0) for k in fl}
     executed_total = fl["total"] * ex - sum(fl[k] * (ex - exk[k]) for k in strassen_steps)      # in 8-flop units x ex
     terms = {}
     for k, xs in step_acc.items():
@@ -687,7 +687,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
             ent["tflops"] = round(fl[k] / (ms * 1e-3) * 1e-12, 2)
             ent["frac_fp64_peak"] = round(fl[k] * exk[k] / (ms * 1e-3) * 1e-12 / peak, 4)
             if k in strassen_steps:
-                ent["strassen_level"] = 1
+                ent["strassen_levels"] = strassen_steps[k]
         terms[k] = ent
     for k in ("prep_permute", "update_diis", "energy"):       # HBM-bound steps: algorithmic bytes / time
         gbs = [hbm_step_bytes(o, v, m, strassen="pp_ladder" in strassen_steps)[k] / (x * 1e-3) * 1e-9
@@ -876,7 +876,7 @@ def run_ours(args) -> None:
     ex = rf / 8.0
     main = iteration_bench(torch, pkg, cfg, inp, args.steps, args.warmup, peak, peaks["hbm_gbs"], barrier=barrier,
                            clock_index=local, e2e=True, max_ranks=(dist if world > 1 else None), graph=args.graph,
-                           strassen=bool(args.strassen))
+                           strassen=args.strassen)
     trip_sharded = triples_sharded_bench(torch, pkg, inp, o, v, dist) if (world > 1 and not args.no_sweep) else None
 
     if not is_reporting_rank():
@@ -890,7 +890,7 @@ def run_ours(args) -> None:
     pp_ms = main["terms"]["pp_ladder"]["ms"]
     pp_tflops = fl["pp_ladder"] / (pp_ms * 1e-3) * 1e-12          # 8-flop (ZGEMM) convention
     pp_strassen = "pp_ladder" in main["strassen_steps"]
-    ex_pp = ex * (7.0 / 8.0 if pp_strassen else 1.0)              # one Strassen level: seven half-size products for eight
+    ex_pp = ex * (7.0 / 8.0) ** main["strassen_steps"].get("pp_ladder", 0)     # one Strassen level: seven half-size products for eight
     pp_exec = pp_tflops * ex_pp
     gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
     gemm_ms = sum(main["terms"][k]["ms"] for k in gemm_steps)
@@ -958,7 +958,7 @@ def run_ours(args) -> None:
         "iteration_frac_fp64_peak": round(main["executed_flops_per_iteration"] / (ms_per_step * 1e-3) * 1e-12 / peak, 4),
         "pp_ladder_tflops": round(pp_tflops, 2), "pp_ladder_frac_fp64_peak": round(pp_exec / peak, 4),
         "tflops_convention": f"8 real flop per complex MAC (ZGEMM); fractions of peak use the {rf} executed (x 7/8 for the "
-                             "products that run as one Strassen level: terms[].strassen_level)",
+                             "products that run as L Strassen levels: terms[].strassen_levels)",
         "ms_per_step_with_step_events": main["ms_per_step_with_step_events"],
         "roofline": roofline, "terms": main["terms"], "init_pack": main["init_pack"],
         "e2e": main["e2e"],
@@ -983,8 +983,8 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--graph", type=int, default=1, help="ccsd_options.graph of the main leg: 0 direct launches, 1 graph with parallel "
                                                           "branches, 3 serial graph (profiling aid)")
-    ap.add_argument("--strassen", type=int, default=1, help="ccsd_options.strassen of the main leg: 1 (default) one Strassen level on "
-                    "the four large contractions, 0 plain products")
+    ap.add_argument("--strassen", type=int, default=1, help="ccsd_options.strassen of the main leg: 1 (default) Strassen levels on "
+                    "the four large contractions, 0 plain products, 2 one level only, 3 two levels on the (ov)^3 products")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")

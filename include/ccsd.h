@@ -83,14 +83,16 @@ typedef struct {
                            collective itself.  Defaults 0, 1.  Not with cc2; ccsd_iterate / ccsd_solve, CCSD_T_VVVV and the
                            Lambda entry points return CCSD_EINVAL in a sharded context */
     int strassen;       /* 1 (default) = the four large contractions of an iteration -- the two (ov)^3 products of eq 29 and of
-                           the ring term, the pp-ladder and the <bk||cd> tau part of eq 30 -- run as ONE level of Strassen's
-                           algorithm around the DMMA GEMM: seven half-size products in one batched launch instead of eight,
-                           i.e. 7/8 of the FP64 tensor-pipe work, plus three streaming passes.
-                           Pure FP64; results differ from strassen = 0 by rounding only (a few 1e-15 of the largest element of
-                           each product).  Costs workspace: the operand stacks of <ab||cd>, <bk||cd> and <kl||cd> are built
-                           once and kept (2.6 x the bytes of those three tensors).  Used on one GPU with the 3M kernels
+                           the ring term, the pp-ladder and the <bk||cd> tau part of eq 30 -- run by Strassen's algorithm around
+                           the DMMA GEMM: seven half-size products in ONE batched launch instead of eight, i.e. 7/8 of the FP64
+                           tensor-pipe work, plus three streaming passes; the two (ov)^3 products
+                           take TWO levels (49 quarter-size products, 0.766 of the work) from ov >= 3072.  Pure FP64; results
+                           differ from strassen = 0 by rounding only (about 1e-14 of the largest element of each product at
+                           most).  Costs workspace: the operand stacks of <ab||cd>, <bk||cd> and <kl||cd> are built once and
+                           kept (1.75 x - 3 x the bytes of those tensors with their planes).  Used on one GPU with the 3M kernels
                            (gemm_mode 0 or 3) where the products are large enough (ov >= 1024); ignored in cc2 mode and in a
-                           sharded context; with direct_ladder the ladder keeps its slab form.  0 = plain products */
+                           sharded context; with direct_ladder the ladder keeps its slab form.  0 = plain products;
+                           2 = one level everywhere; 3 = two levels on the (ov)^3 products whatever their size (tests) */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */
@@ -355,12 +357,15 @@ int ccsd_zgemm_nt_planes(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, in
  * products are ONE batched launch, and a third pass sums them into C (+)= alpha A B^T.  7/8 of the tensor-pipe work of
  * ccsd_zgemm_nt; same result up to rounding (pure FP64; max error a few 1e-15 of the largest element of C).  Any extents
  * >= 1 (odd halves are zero-padded inside the stacks); it pays from roughly M, K >= 1024, N >= 96.  mode 0, 3 or 100+v.
+ * levels = 2 applies the scheme twice: 49 quarter-size products in one batched launch (0.766 of the plain work), the 49
+ * operand combinations written straight from the 4 x 4 blocks of the operand and the 16 blocks of C summed straight from the
+ * 49 products (one pass each, as for one level); it pays from roughly M, K >= 4096.
  * workspace: ccsd_zgemm_nt_strassen_workspace_bytes() bytes, 256-byte aligned, device.  Asynchronous on the stream.
  */
-int ccsd_zgemm_nt_strassen_workspace_bytes(int64_t M, int64_t N, int64_t K, size_t* bytes);
+int ccsd_zgemm_nt_strassen_workspace_bytes(int64_t M, int64_t N, int64_t K, int levels, size_t* bytes);
 int ccsd_zgemm_nt_strassen(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
                            ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
-                           void* workspace, size_t workspace_bytes, void* cuda_stream);
+                           int levels, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
  * Tensor transposition ("A(a,c,b,d)+=B(a,b,c,d)"):  out[permuted index] = in[index]
@@ -386,8 +391,8 @@ const char* ccsd_step_name(int step);
 enum { CCSD_NINIT_STATS = 5 };
 int ccsd_get_init_stats(ccsd_ctx* ctx, double stats[CCSD_NINIT_STATS]);
 /* Where this context uses the Strassen level (ccsd_options.strassen; it needs one GPU, the 3M kernels and ov >= 1024):
- * info[] = { any, the two (ov)^3 products (H^{ak}_{ci} quadratic term, ring), the pp-ladder, the <bk||cd> tau part of C }, 1 or 0.
- * A product that uses it executes 7/8 of the real flops of the plain product.  HOST out-pointer. */
+ * info[] = { any, the two (ov)^3 products (H^{ak}_{ci} quadratic term, ring), the pp-ladder, the <bk||cd> tau part of C }: the
+ * number of levels L (0 = plain product).  Such a product executes (7/8)^L of the real flops of the plain one.  HOST out-pointer. */
 int ccsd_strassen_info(ccsd_ctx* ctx, int info[4]);
 /* Kernel launches issued by the library since the last reset (all contexts, this process). */
 long long ccsd_launch_count(int reset);

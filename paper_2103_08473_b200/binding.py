@@ -107,9 +107,9 @@ def load_library():
         lib.ccsd_energy_static.argtypes = [ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp]
         lib.ccsd_zgemm_nt.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
                                       ctypes.c_int, vp]
-        lib.ccsd_zgemm_nt_strassen_workspace_bytes.argtypes = [i64, i64, i64, ctypes.POINTER(ctypes.c_size_t)]
+        lib.ccsd_zgemm_nt_strassen_workspace_bytes.argtypes = [i64, i64, i64, ctypes.c_int, ctypes.POINTER(ctypes.c_size_t)]
         lib.ccsd_zgemm_nt_strassen.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, ctypes.c_int,
-                                               ctypes.c_int, vp, ctypes.c_size_t, vp]
+                                               ctypes.c_int, ctypes.c_int, vp, ctypes.c_size_t, vp]
         lib.ccsd_strassen_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int)]
         lib.ccsd_sum_plane.argtypes = [vp, vp, i64, vp]
         lib.ccsd_zgemm_nt_planes.argtypes = [i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, i64, dbl, dbl, ctypes.c_int,
@@ -232,9 +232,9 @@ def measure_fp64_peak(launches: int = 10) -> float:
 
 
 def _options(ndiis=6, level_shift=0.0, gemm_mode=0, ccd=False, cc2=False, direct_ladder=False, graph=True,
-             shard=(0, 1), strassen=True) -> Options:
+             shard=(0, 1), strassen=1) -> Options:
     return Options(int(ndiis), float(level_shift), int(gemm_mode), int(bool(ccd)), int(bool(cc2)), int(bool(direct_ladder)),
-                   int(graph), int(shard[0]), int(shard[1]), int(bool(strassen)))
+                   int(graph), int(shard[0]), int(shard[1]), int(strassen))
 
 
 class CCSD:
@@ -249,7 +249,7 @@ class CCSD:
 
     def __init__(self, h, B, nocc: int, nvir: int, ndiis: int = 6, level_shift: float = 0.0, gemm_mode: int = 0,
                  ccd: bool = False, cc2: bool = False, direct_ladder: bool = False, graph: int = 1, stream=None,
-                 shard=None, group=None, strassen: bool = True):
+                 shard=None, group=None, strassen: int = 1):
         torch = _torch()
         lib = load_library()
         self._lib, self._torch = lib, torch
@@ -521,11 +521,19 @@ class CCSD:
         self._call(self._lib.ccsd_expectation, D_d.data_ptr(), O_d.data_ptr(), ctypes.byref(re), ctypes.byref(im), where="ccsd_expectation")
         return complex(re.value, im.value)
 
-    def strassen_steps(self):
-        """Names of the timed steps (step_times()) whose product runs as one Strassen level: 7/8 of the plain product's flops."""
+    def strassen_steps(self) -> dict:
+        """{name of a timed step (step_times()): Strassen levels L of its product}; such a product executes (7/8)^L of the
+        plain product's flops."""
         info = (ctypes.c_int * 4)()
         self._call(self._lib.ccsd_strassen_info, info, where="ccsd_strassen_info")
-        return (["Hvovo_quad", "ring_gemm"] if info[1] else []) + (["pp_ladder"] if info[2] else []) + (["C_ovoo"] if info[3] else [])
+        out = {}
+        if info[1]:
+            out["Hvovo_quad"] = out["ring_gemm"] = int(info[1])
+        if info[2]:
+            out["pp_ladder"] = int(info[2])
+        if info[3]:
+            out["C_ovoo"] = int(info[3])
+        return out
 
     def enable_step_timing(self, enable: bool = True):
         self._call(self._lib.ccsd_enable_step_timing, int(enable), where="ccsd_enable_step_timing")
@@ -622,8 +630,10 @@ def zgemm_nt(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode:
     return C
 
 
-def zgemm_nt_strassen(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False):
-    """zgemm_nt by one Strassen level (ccsd_zgemm_nt_strassen): seven half-size products in one batched DMMA launch."""
+def zgemm_nt_strassen(A, B, C=None, alpha: complex = 1.0, accumulate: bool = False, mode: int = 0, transposed_out: bool = False,
+                      levels: int = 1, sync: bool = True):
+    """zgemm_nt by one or two Strassen levels (ccsd_zgemm_nt_strassen): 7 half-size / 49 quarter-size products in one batched
+    DMMA launch.  sync=False returns (C, workspace) without waiting (timing loops: keep the workspace alive)."""
     torch = _torch()
     lib = load_library()
     A, B = _dev_c128(torch, A), _dev_c128(torch, B)
@@ -635,11 +645,14 @@ def zgemm_nt_strassen(A, B, C=None, alpha: complex = 1.0, accumulate: bool = Fal
     csm, csn = (1, M) if transposed_out else (N, 1)
     alpha = complex(alpha)
     nbytes = ctypes.c_size_t(0)
-    _check(lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, ctypes.byref(nbytes)), "ccsd_zgemm_nt_strassen_workspace_bytes")
+    _check(lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, levels, ctypes.byref(nbytes)), "ccsd_zgemm_nt_strassen_workspace_bytes")
     ws = _workspace(torch, nbytes.value)
     base = (ws.data_ptr() + 255) // 256 * 256
     _check(lib.ccsd_zgemm_nt_strassen(M, N, K, A.data_ptr(), K, B.data_ptr(), K, C.data_ptr(), csm, csn, alpha.real, alpha.imag,
-                                      int(accumulate), mode, base, int(nbytes.value), _stream_ptr(torch)), "ccsd_zgemm_nt_strassen")
+                                      int(accumulate), mode, levels, base, int(nbytes.value), _stream_ptr(torch)),
+           "ccsd_zgemm_nt_strassen")
+    if not sync:
+        return C, ws
     torch.cuda.current_stream().synchronize()   # ws must outlive the enqueued kernels
     return C
 

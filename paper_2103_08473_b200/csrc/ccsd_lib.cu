@@ -141,33 +141,36 @@ static inline bool strassen_worthwhile(int64_t M, int64_t N, int64_t K)
 // p: a plain (batch 1, k-contiguous) product C (+)= alpha A B^T.  preA / preB: ready-made stacks of operands that do not
 // change between calls; an operand without one is stacked here into w.  The products go to w.P, then into C.
 static int strassen_gemm(const Env& env, const GemmParams& p, const StrassenStack* preA, const StrassenStack* preB,
-                         const StrassenScratch& w)
+                         const StrassenScratch& w, int levels = 1)
 {
     if (p.M <= 0 || p.N <= 0 || p.K <= 0) return CCSD_OK;
-    if (p.batch != 1 || p.sak != 1 || p.sbk != 1) return CCSD_EINVAL;
-    const int64_t Mh = strassen_half(p.M), Nh = strassen_half(p.N), Kh = strassen_khalf(p.K);
+    if (p.batch != 1 || p.sak != 1 || p.sbk != 1 || levels < 1 || levels > 2) return CCSD_EINVAL;
+    const int64_t Mh = strassen_rows(p.M, levels), Nh = strassen_rows(p.N, levels), Kh = strassen_cols(p.K, levels);
+    const int nprod = levels == 2 ? 49 : 7;
     StrassenStack sa, sb;
     if (preA) {
         sa = *preA;
     } else {
-        if (7 * Mh * Kh > w.a_elems) return CCSD_EINVAL;
-        sa = strassen_stack(w.SA, w.SAp, p.M, p.K);
+        if (nprod * Mh * Kh > w.a_elems) return CCSD_EINVAL;
+        sa = strassen_stack(w.SA, w.SAp, p.M, p.K, levels);
         launch_strassen_prep(env.st, 0, p.A, p.sam, sa);
     }
     if (preB) {
         sb = *preB;
     } else {
-        if (7 * Nh * Kh > w.b_elems) return CCSD_EINVAL;
-        sb = strassen_stack(w.SB, w.SBp, p.N, p.K);
+        if (nprod * Nh * Kh > w.b_elems) return CCSD_EINVAL;
+        sb = strassen_stack(w.SB, w.SBp, p.N, p.K, levels);
         launch_strassen_prep(env.st, 1, p.B, p.sbn, sb);
     }
-    if (sa.R != p.M || sa.K != p.K || sb.R != p.N || sb.K != p.K || 7 * Mh * Nh > w.p_elems) return CCSD_EINVAL;
+    if (sa.R != p.M || sa.K != p.K || sb.R != p.N || sb.K != p.K || sa.levels != levels || sb.levels != levels ||
+        nprod * Mh * Nh > w.p_elems)
+        return CCSD_EINVAL;
     const bool fast_m = p.csm == 1;    // the products take C's unit-stride index as their fast index
     GemmParams g = gp(Mh, Nh, Kh, sa.S, Kh, sb.S, Kh, w.P, fast_m ? 1 : Nh, fast_m ? Mh : 1, 1.0, 0);
-    g.batch = 7; g.bsA = Mh * Kh; g.bsB = Nh * Kh; g.bsC = Mh * Nh;
+    g.batch = nprod; g.bsA = Mh * Kh; g.bsB = Nh * Kh; g.bsC = Mh * Nh;
     g.As = sa.Sp; g.Bs = sb.Sp;
     CCSD_TRY(run_gemm(env, g));
-    launch_strassen_combine(env.st, w.P, p.M, p.N, p.C, p.csm, p.csn, p.alpha, p.accumulate);
+    launch_strassen_combine(env.st, w.P, p.M, p.N, p.C, p.csm, p.csn, p.alpha, p.accumulate, levels);
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
 }
@@ -276,6 +279,7 @@ struct ccsd_ctx {
     // quadratic H^{ak}_{ci} term) built once by ccsd_init, the stack of tau (right operand of the pp-ladder and of C) built by
     // prep_operands, and per-branch scratch for the stacks of Xm, Hm, T2r and for the seven products.
     bool strassen;
+    int strassen_levels;    // of the two (ov)^3 products: 1 or 2 (the pp-ladder and C always take one)
     StrassenStack sW, sVvovv, sG1, sTau;
     StrassenScratch str_ring, str_C, str_L;
     // DIIS ring (reduce.cuh): stored pairs, device-side Gram matrix / coefficients / reduction scratch
@@ -445,39 +449,46 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     }
     // One Strassen level (strassen.cuh) on the (ov)^3 products, the pp-ladder and the <bk||cd> tau part of C: one GPU, 3M planes
     c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 && strassen_worthwhile(ov, ov, ov);
+    // two levels on the (ov)^3 products where a quarter-size product is still a long-K, many-tile GEMM (measured: 0.80 of the
+    // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
+    c->strassen_levels = c->opt.strassen == 3 ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
     memset(&c->sW, 0, sizeof(c->sW)); memset(&c->sVvovv, 0, sizeof(c->sVvovv)); memset(&c->sG1, 0, sizeof(c->sG1));
     memset(&c->sTau, 0, sizeof(c->sTau));
     memset(&c->str_ring, 0, sizeof(c->str_ring)); memset(&c->str_C, 0, sizeof(c->str_C)); memset(&c->str_L, 0, sizeof(c->str_L));
     if (c->strassen) {
         const bool use_L = !c->opt.direct_ladder && strassen_worthwhile(vv, oo, vv);
         const bool use_C = strassen_worthwhile(ov, oo, vv);
-        auto stack = [](Carver& a, int64_t R, int64_t K) {
-            c128* S = a.take<c128>(strassen_stack_elems(R, K));
-            double* Sp = a.take<double>(strassen_stack_elems(R, K));
-            return strassen_stack(S, Sp, R, K);
+        const int lv = c->strassen_levels;
+        // Per-iteration stacks and products go into the dead init temporaries [Jovov, Joooo] while they fit there (largest
+        // first), the rest and the stacks of the constants are appended.
+        Carver dead{base ? base + j_begin : nullptr, 0};
+        const size_t dead_bytes = j_end - j_begin;
+        auto place = [&](int64_t elems, size_t elem_bytes) -> Carver& {
+            const size_t bytes = ((size_t)(elems > 0 ? elems : 1) * elem_bytes + 255) & ~(size_t)255;
+            return dead.off + bytes <= dead_bytes ? dead : w;
         };
-        // constants: memory of their own
-        if (use_L) c->sW = stack(w, vv, vv);
-        if (use_C) c->sVvovv = stack(w, ov, vv);
-        c->sG1 = stack(w, ov, ov);
-        // per-iteration stacks and products: in the dead init temporaries when they fit there, else appended
-        auto scratch = [&](Carver& a) {
-            StrassenStack sa = stack(a, ov, ov), sb = stack(a, ov, ov);
-            c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov);
-            c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov);
-            c->str_ring.p_elems = 7 * strassen_half(ov) * strassen_half(ov);
-            c->str_ring.P = a.take<c128>(c->str_ring.p_elems);
-            if (use_L || use_C) c->sTau = stack(a, oo, vv);
-            if (use_L) { c->str_L.p_elems = 7 * strassen_half(vv) * strassen_half(oo); c->str_L.P = a.take<c128>(c->str_L.p_elems); }
-            if (use_C) { c->str_C.p_elems = 7 * strassen_half(ov) * strassen_half(oo); c->str_C.P = a.take<c128>(c->str_C.p_elems); }
+        auto stack = [&](bool scratch, int64_t R, int64_t K, int levels) {
+            const int64_t e = strassen_stack_elems(R, K, levels);
+            c128* S = (scratch ? place(e, sizeof(c128)) : w).take<c128>(e);
+            double* Sp = (scratch ? place(e, sizeof(double)) : w).take<double>(e);
+            return strassen_stack(S, Sp, R, K, levels);
         };
-        Carver probe{nullptr, 0};
-        scratch(probe);
-        if (probe.off <= j_end - j_begin) {
-            Carver alias{base ? base + j_begin : nullptr, 0};
-            scratch(alias);
-        } else {
-            scratch(w);
+        if (use_L) c->sW = stack(false, vv, vv, 1);
+        if (use_C) c->sVvovv = stack(false, ov, vv, 1);
+        c->sG1 = stack(false, ov, ov, lv);
+        StrassenStack sa = stack(true, ov, ov, lv), sb = stack(true, ov, ov, lv);
+        c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov, lv);
+        c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov, lv);
+        c->str_ring.p_elems = (lv == 2 ? 49 : 7) * strassen_rows(ov, lv) * strassen_rows(ov, lv);
+        c->str_ring.P = place(c->str_ring.p_elems, sizeof(c128)).take<c128>(c->str_ring.p_elems);
+        if (use_L || use_C) c->sTau = stack(true, oo, vv, 1);
+        if (use_L) {
+            c->str_L.p_elems = 7 * strassen_half(vv) * strassen_half(oo);
+            c->str_L.P = place(c->str_L.p_elems, sizeof(c128)).take<c128>(c->str_L.p_elems);
+        }
+        if (use_C) {
+            c->str_C.p_elems = 7 * strassen_half(ov) * strassen_half(oo);
+            c->str_C.P = place(c->str_C.p_elems, sizeof(c128)).take<c128>(c->str_C.p_elems);
         }
     }
     c->nvec = ov + oo * vv;
@@ -963,7 +974,8 @@ static int build_Hvovo(ccsd_ctx* c)
     tick(c, 3);
     // + sum_{ld} <kl||cd> (1/2 t2[l,i,a,d] + t1[l,a] t1[i,d])       (ov x ov x ov)
     if (c->strassen) {   // seven half-size products (strassen.cuh); the ring product stacks Hm itself, no plane of Hm needed
-        return strassen_gemm(env, gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1), nullptr, &c->sG1, c->str_ring);
+        return strassen_gemm(env, gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1), nullptr, &c->sG1, c->str_ring,
+                             c->strassen_levels);
     }
     CCSD_TRY(run_gemm(env, with_planes(gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1),
                                        c->Xms ? c->Xms + off : nullptr, c->G1s)));
@@ -1204,7 +1216,8 @@ static int ring_gemm(ccsd_ctx* c)
     const int64_t off = (int64_t)c->sh.a_lo * o * ov, rows = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o;
     if (rows <= 0) return CCSD_OK;
     if (c->strassen)
-        return strassen_gemm(c->env, gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0), nullptr, nullptr, c->str_ring);
+        return strassen_gemm(c->env, gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0), nullptr, nullptr, c->str_ring,
+                             c->strassen_levels);
     return run_gemm(c->env, with_planes(gp(rows, ov, ov, c->Hm + off, ov, c->T2r, ov, c->Xr + off, ov, 1, 1.0, 0),
                                         c->Hms ? c->Hms + off : nullptr, c->T2rs));
 }
@@ -2517,54 +2530,54 @@ int ccsd_zgemm_nt_planes(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, in
 
 // ccsd_zgemm_nt by one Strassen level (strassen.cuh): both operand stacks, their planes and the seven products live in the
 // caller's workspace.  Any extents >= 1 (odd ones are zero-padded inside the stacks).
-static void strassen_standalone_carve(int64_t M, int64_t N, int64_t K, char* base, StrassenScratch* w, size_t* total)
+static void strassen_standalone_carve(int64_t M, int64_t N, int64_t K, int levels, char* base, StrassenScratch* w, size_t* total)
 {
     Carver cv{base, 0};
-    w->a_elems = strassen_stack_elems(M, K);
-    w->b_elems = strassen_stack_elems(N, K);
-    w->p_elems = 7 * strassen_half(M) * strassen_half(N);
+    w->a_elems = strassen_stack_elems(M, K, levels);
+    w->b_elems = strassen_stack_elems(N, K, levels);
+    w->p_elems = (levels == 2 ? 49 : 7) * strassen_rows(M, levels) * strassen_rows(N, levels);
     w->SA = cv.take<c128>(w->a_elems); w->SAp = cv.take<double>(w->a_elems);
     w->SB = cv.take<c128>(w->b_elems); w->SBp = cv.take<double>(w->b_elems);
     w->P = cv.take<c128>(w->p_elems);
     *total = cv.off;
 }
 
-int ccsd_zgemm_nt_strassen_workspace_bytes(int64_t M, int64_t N, int64_t K, size_t* bytes)
+int ccsd_zgemm_nt_strassen_workspace_bytes(int64_t M, int64_t N, int64_t K, int levels, size_t* bytes)
 {
-    if (!bytes || M < 1 || N < 1 || K < 1) return CCSD_EINVAL;
+    if (!bytes || M < 1 || N < 1 || K < 1 || levels < 1 || levels > 2) return CCSD_EINVAL;
     StrassenScratch w;
-    strassen_standalone_carve(M, N, K, nullptr, &w, bytes);
+    strassen_standalone_carve(M, N, K, levels, nullptr, &w, bytes);
     return CCSD_OK;
 }
 
 int ccsd_zgemm_nt_strassen(int64_t M, int64_t N, int64_t K, const ccsd_c128* A, int64_t lda, const ccsd_c128* B, int64_t ldb,
                            ccsd_c128* C, int64_t csm, int64_t csn, double alpha_re, double alpha_im, int accumulate, int mode,
-                           void* workspace, size_t workspace_bytes, void* cuda_stream)
+                           int levels, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    if (!A || !B || !C || M < 1 || N < 1 || K < 1 || lda < K || ldb < K) return CCSD_EINVAL;
+    if (!A || !B || !C || M < 1 || N < 1 || K < 1 || lda < K || ldb < K || levels < 1 || levels > 2) return CCSD_EINVAL;
     if (!(mode == 0 || mode == 3 || mode >= 100)) return CCSD_EINVAL;
     size_t need = 0;
     StrassenScratch w;
-    strassen_standalone_carve(M, N, K, nullptr, &w, &need);
+    strassen_standalone_carve(M, N, K, levels, nullptr, &w, &need);
     if (!workspace || workspace_bytes < need || reinterpret_cast<uintptr_t>(workspace) % 256) return CCSD_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
         return CCSD_ECUDA;
     }
-    strassen_standalone_carve(M, N, K, static_cast<char*>(workspace), &w, &need);
+    strassen_standalone_carve(M, N, K, levels, static_cast<char*>(workspace), &w, &need);
     Env env{static_cast<cudaStream_t>(cuda_stream), mode, nullptr, 0};
     GemmParams p = gp(M, N, K, reinterpret_cast<const c128*>(A), lda, reinterpret_cast<const c128*>(B), ldb,
                       reinterpret_cast<c128*>(C), csm, csn, 1.0, accumulate);
     p.alpha = mk(alpha_re, alpha_im);
-    return strassen_gemm(env, p, nullptr, nullptr, w);
+    return strassen_gemm(env, p, nullptr, nullptr, w, levels);
 }
 
 int ccsd_strassen_info(ccsd_ctx* c, int info[4])
 {
     if (!c || !info) return CCSD_ESTATE;
     info[0] = c->strassen ? 1 : 0;
-    info[1] = c->strassen ? 1 : 0;                       // the two (ov)^3 products
+    info[1] = c->strassen ? c->strassen_levels : 0;      // the two (ov)^3 products: levels
     info[2] = (c->strassen && c->sW.S) ? 1 : 0;          // pp-ladder
     info[3] = (c->strassen && c->sVvovv.S) ? 1 : 0;      // <bk||cd> tau part of C
     return CCSD_OK;

@@ -1,6 +1,7 @@
-// One level of Strassen's algorithm around the DMMA GEMM (gemm_dmma.cuh) for the large contractions of eq 32 / eqs 29-30
+// One or two levels of Strassen's algorithm around the DMMA GEMM (gemm_dmma.cuh) for the large contractions of eq 32 / eqs 29-30
 // (PAPER.md:594-606): C = A B^T with every dimension halved is 7 half-size products instead of 8, i.e. 7/8 of the FP64
-// tensor-pipe work, for three streaming passes (operand sums, result sums).  All arithmetic stays FP64; the result differs
+// tensor-pipe work (49 quarter-size products for 64 with two levels: 0.766), for three streaming passes (operand sums,
+// result sums).  All arithmetic stays FP64; the result differs
 // from the plain product by rounding only (measured max error 2-9e-15 of the largest element against 1-5e-15 for the
 // plain 3M product; the parity bound is 1e-12).
 //
@@ -17,23 +18,50 @@
 #pragma once
 #include "common.cuh"
 
-struct StrassenStack {      // the seven operand combinations of one side
-    c128* S;                // [7][Rh][Kh]
+struct StrassenStack {      // the operand combinations of one side: 7 (one level) or 7 x 7 (two levels) matrices
+    c128* S;                // [7^levels][Rh][Kh]; two levels: index q1 * 7 + q2 (q1 outer level, q2 inner)
     double* Sp;             // their sum planes Re + Im, same layout
     int64_t R, K, Rh, Kh;   // extents of the operand it was made from, and of one stacked matrix
+    int levels;
 };
 
 static inline int64_t strassen_half(int64_t x) { return (x + 1) / 2; }
 static inline int64_t strassen_khalf(int64_t K) { return round_up((K + 1) / 2, 2); }
-static inline int64_t strassen_stack_elems(int64_t R, int64_t K) { return 7 * strassen_half(R) * strassen_khalf(K); }
-static inline StrassenStack strassen_stack(c128* S, double* Sp, int64_t R, int64_t K)
+static inline int64_t strassen_rows(int64_t R, int levels) { return levels == 2 ? strassen_half(strassen_half(R)) : strassen_half(R); }
+static inline int64_t strassen_cols(int64_t K, int levels) { return levels == 2 ? strassen_khalf(strassen_khalf(K)) : strassen_khalf(K); }
+static inline int64_t strassen_stack_elems(int64_t R, int64_t K, int levels = 1)
+{
+    return (levels == 2 ? 49 : 7) * strassen_rows(R, levels) * strassen_cols(K, levels);
+}
+static inline StrassenStack strassen_stack(c128* S, double* Sp, int64_t R, int64_t K, int levels = 1)
 {
     StrassenStack s;
-    s.S = S; s.Sp = Sp; s.R = R; s.K = K; s.Rh = strassen_half(R); s.Kh = strassen_khalf(K);
+    s.S = S; s.Sp = Sp; s.R = R; s.K = K; s.Rh = strassen_rows(R, levels); s.Kh = strassen_cols(K, levels); s.levels = levels;
     return s;
 }
 
 constexpr int STR_THREADS = 256;
+
+// the seven operand combinations of one side (SIDE 0: left operand A, SIDE 1: right operand B) from its four quadrants
+template <int SIDE>
+__device__ __forceinline__ void strassen_combos(c128 x11, c128 x12, c128 x21, c128 x22, c128 s[7])
+{
+    if (SIDE == 0) {
+        s[0] = cadd(x11, x22); s[1] = cadd(x21, x22); s[2] = x11; s[3] = x22;
+        s[4] = cadd(x11, x12); s[5] = csub(x21, x11); s[6] = csub(x12, x22);
+    } else {
+        s[0] = cadd(x11, x22); s[1] = x11; s[2] = csub(x21, x22); s[3] = csub(x12, x11);
+        s[4] = x22; s[5] = cadd(x11, x21); s[6] = cadd(x12, x22);
+    }
+}
+// the four quadrants of C from the seven products
+__device__ __forceinline__ void strassen_quadrants(const c128 p[7], c128& c11, c128& c12, c128& c21, c128& c22)
+{
+    c11 = cadd(csub(cadd(p[0], p[3]), p[4]), p[6]);
+    c12 = cadd(p[2], p[4]);
+    c21 = cadd(p[1], p[3]);
+    c22 = cadd(cadd(csub(p[0], p[1]), p[2]), p[5]);
+}
 
 // SIDE 0: left operand A [R = M][K];  SIDE 1: right operand B [R = N][K] (both k-contiguous, leading dimension ld)
 template <int SIDE>
@@ -52,13 +80,7 @@ strassen_prep_kernel(const c128* __restrict__ in, int64_t ld, int64_t R, int64_t
         const c128 x21 = (r2 && k1) ? in[(r + Rh) * ld + k] : zero;
         const c128 x22 = (r2 && k2) ? in[(r + Rh) * ld + k + Kh] : zero;
         c128 s[7];
-        if (SIDE == 0) {
-            s[0] = cadd(x11, x22); s[1] = cadd(x21, x22); s[2] = x11; s[3] = x22;
-            s[4] = cadd(x11, x12); s[5] = csub(x21, x11); s[6] = csub(x12, x22);
-        } else {
-            s[0] = cadd(x11, x22); s[1] = x11; s[2] = csub(x21, x22); s[3] = csub(x12, x11);
-            s[4] = x22; s[5] = cadd(x11, x21); s[6] = cadd(x12, x22);
-        }
+        strassen_combos<SIDE>(x11, x12, x21, x22, s);
         const int64_t at = r * Kh + k;
 #pragma unroll
         for (int q = 0; q < 7; q++) {
@@ -68,12 +90,62 @@ strassen_prep_kernel(const c128* __restrict__ in, int64_t ld, int64_t R, int64_t
     }
 }
 
+// Two levels in one pass: the 49 combinations S[q1 * 7 + q2] = combos(combos(quadrants)[q1] quadrants)[q2] of an operand, from
+// its 4 x 4 blocks (R1, K1: extents of a half, Rq, Kq: of a quarter).  Same additions in the same order as two passes of
+// strassen_prep_kernel, without writing and re-reading the seven half-size matrices.
+template <int SIDE>
+__global__ void __launch_bounds__(STR_THREADS)
+strassen_prep2_kernel(const c128* __restrict__ in, int64_t ld, int64_t R, int64_t K, int64_t R1, int64_t K1, int64_t Rq, int64_t Kq,
+                      c128* __restrict__ S, double* __restrict__ Sp)
+{
+    const int64_t k = (int64_t)blockIdx.x * STR_THREADS + threadIdx.x;
+    if (k >= Kq) return;
+    const int64_t plane = Rq * Kq;
+    const c128 zero = mk(0.0, 0.0);
+    for (int64_t r = blockIdx.y; r < Rq; r += gridDim.y) {
+        c128 s1[2][2][7];      // [inner row half][inner k half][q1]: the outer combinations at the four inner block positions
+#pragma unroll
+        for (int u2 = 0; u2 < 2; u2++)
+#pragma unroll
+            for (int v2 = 0; v2 < 2; v2++) {
+                const int64_t rr = r + u2 * Rq, kk = k + v2 * Kq;       // position inside a half
+                const bool in_half = rr < R1 && kk < K1;
+                c128 x[2][2];
+#pragma unroll
+                for (int u1 = 0; u1 < 2; u1++)
+#pragma unroll
+                    for (int v1 = 0; v1 < 2; v1++) {
+                        const int64_t row = rr + u1 * R1, col = kk + v1 * K1;
+                        x[u1][v1] = (in_half && row < R && col < K) ? in[row * ld + col] : zero;
+                    }
+                strassen_combos<SIDE>(x[0][0], x[0][1], x[1][0], x[1][1], s1[u2][v2]);
+            }
+        const int64_t at = r * Kq + k;
+#pragma unroll
+        for (int q1 = 0; q1 < 7; q1++) {
+            c128 s2[7];
+            strassen_combos<SIDE>(s1[0][0][q1], s1[0][1][q1], s1[1][0][q1], s1[1][1][q1], s2);
+#pragma unroll
+            for (int q2 = 0; q2 < 7; q2++) {
+                S[(q1 * 7 + q2) * plane + at] = s2[q2];
+                Sp[(q1 * 7 + q2) * plane + at] = s2[q2].x + s2[q2].y;
+            }
+        }
+    }
+}
+
 static inline void launch_strassen_prep(cudaStream_t st, int side, const c128* in, int64_t ld, const StrassenStack& s)
 {
     if (s.Rh <= 0 || s.Kh <= 0) return;
     dim3 grid((unsigned)((s.Kh + STR_THREADS - 1) / STR_THREADS), (unsigned)(s.Rh < 32768 ? s.Rh : 32768));
-    if (side == 0) strassen_prep_kernel<0><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
-    else strassen_prep_kernel<1><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
+    if (s.levels == 2) {
+        const int64_t R1 = strassen_half(s.R), K1 = strassen_khalf(s.K);
+        if (side == 0) strassen_prep2_kernel<0><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, R1, K1, s.Rh, s.Kh, s.S, s.Sp);
+        else strassen_prep2_kernel<1><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, R1, K1, s.Rh, s.Kh, s.S, s.Sp);
+    } else {
+        if (side == 0) strassen_prep_kernel<0><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
+        else strassen_prep_kernel<1><<<grid, STR_THREADS, 0, st>>>(in, ld, s.R, s.K, s.Rh, s.Kh, s.S, s.Sp);
+    }
     count_launches(1);
 }
 
@@ -88,12 +160,10 @@ strassen_combine_kernel(const c128* __restrict__ P, int64_t Fh, int64_t Sh, int6
     const int64_t plane = Fh * Sh;
     for (int64_t s = blockIdx.y; s < Sh; s += gridDim.y) {
         const int64_t at = s * Fh + f;
-        const c128 p1 = P[at], p2 = P[plane + at], p3 = P[2 * plane + at], p4 = P[3 * plane + at], p5 = P[4 * plane + at],
-                   p6 = P[5 * plane + at], p7 = P[6 * plane + at];
-        const c128 c11 = cadd(csub(cadd(p1, p4), p5), p7);
-        const c128 c12 = cadd(p3, p5);
-        const c128 c21 = cadd(p2, p4);
-        const c128 c22 = cadd(cadd(csub(p1, p2), p3), p6);
+        c128 p[7], c11, c12, c21, c22;
+#pragma unroll
+        for (int q = 0; q < 7; q++) p[q] = P[q * plane + at];
+        strassen_quadrants(p, c11, c12, c21, c22);
         // quadrant (row half of m, row half of n): c12 is (m low, n high).  In (fast, slow) terms:
         const c128 q_fs[2][2] = {{c11, fast_is_m ? c12 : c21}, {fast_is_m ? c21 : c12, c22}};   // [fast half][slow half]
 #pragma unroll
@@ -110,16 +180,67 @@ strassen_combine_kernel(const c128* __restrict__ P, int64_t Fh, int64_t Sh, int6
     }
 }
 
-// P: products [7][Sh][Fh] of a C with extents M x N and strides (csm, csn)
+// Two levels in one pass: the 49 quarter-size products P[q1 * 7 + q2][slow][fast] -> the seven half-size products (in
+// registers, at the four inner positions) -> the 16 blocks of C.  (Fh, Sh: extents of a half, Fq, Sq: of a quarter.)
+__global__ void __launch_bounds__(STR_THREADS)
+strassen_combine2_kernel(const c128* __restrict__ P, int64_t Fq, int64_t Sq, int64_t Fh, int64_t Sh, int64_t F, int64_t Sx,
+                         c128* __restrict__ C, int64_t stride_f, int64_t stride_s, int fast_is_m, c128 alpha, int accumulate)
+{
+    const int64_t f = (int64_t)blockIdx.x * STR_THREADS + threadIdx.x;
+    if (f >= Fq) return;
+    const int64_t plane = Fq * Sq;
+    for (int64_t s = blockIdx.y; s < Sq; s += gridDim.y) {
+        const int64_t at = s * Fq + f;
+        c128 p1[2][2][7];      // [inner fast half][inner slow half][q1]: the half-size products at the four inner positions
+#pragma unroll
+        for (int q1 = 0; q1 < 7; q1++) {
+            c128 p[7], c11, c12, c21, c22;
+#pragma unroll
+            for (int q2 = 0; q2 < 7; q2++) p[q2] = P[(q1 * 7 + q2) * plane + at];
+            strassen_quadrants(p, c11, c12, c21, c22);
+            p1[0][0][q1] = c11; p1[0][1][q1] = fast_is_m ? c12 : c21; p1[1][0][q1] = fast_is_m ? c21 : c12; p1[1][1][q1] = c22;
+        }
+#pragma unroll
+        for (int f2 = 0; f2 < 2; f2++)
+#pragma unroll
+            for (int s2 = 0; s2 < 2; s2++) {
+                const int64_t fi = f + f2 * Fq, si = s + s2 * Sq;       // position inside a half
+                if (fi >= Fh || si >= Sh) continue;
+                c128 c11, c12, c21, c22;
+                strassen_quadrants(p1[f2][s2], c11, c12, c21, c22);
+                const c128 q_fs[2][2] = {{c11, fast_is_m ? c12 : c21}, {fast_is_m ? c21 : c12, c22}};
+#pragma unroll
+                for (int hf = 0; hf < 2; hf++)
+#pragma unroll
+                    for (int hs = 0; hs < 2; hs++) {
+                        const int64_t ff = fi + hf * Fh, ss = si + hs * Sh;
+                        if (ff >= F || ss >= Sx) continue;
+                        c128* dst = C + ff * stride_f + ss * stride_s;
+                        c128 val = cmul(alpha, q_fs[hf][hs]);
+                        if (accumulate) val = cadd(val, *dst);
+                        *dst = val;
+                    }
+            }
+    }
+}
+
+// P: products [7^levels][S][F] (S, F: the slow / fast extent of one product) of a C with extents M x N and strides (csm, csn)
 static inline void launch_strassen_combine(cudaStream_t st, const c128* P, int64_t M, int64_t N, c128* C, int64_t csm, int64_t csn,
-                                           c128 alpha, int accumulate)
+                                           c128 alpha, int accumulate, int levels = 1)
 {
     const int fast_is_m = csm == 1;
     const int64_t F = fast_is_m ? M : N, Sx = fast_is_m ? N : M;
     const int64_t Fh = strassen_half(F), Sh = strassen_half(Sx);
     if (Fh <= 0 || Sh <= 0) return;
-    dim3 grid((unsigned)((Fh + STR_THREADS - 1) / STR_THREADS), (unsigned)(Sh < 32768 ? Sh : 32768));
-    strassen_combine_kernel<<<grid, STR_THREADS, 0, st>>>(P, Fh, Sh, F, Sx, C, fast_is_m ? csm : csn, fast_is_m ? csn : csm,
-                                                          fast_is_m, alpha, accumulate);
+    if (levels == 2) {
+        const int64_t Fq = strassen_half(Fh), Sq = strassen_half(Sh);
+        dim3 grid((unsigned)((Fq + STR_THREADS - 1) / STR_THREADS), (unsigned)(Sq < 32768 ? Sq : 32768));
+        strassen_combine2_kernel<<<grid, STR_THREADS, 0, st>>>(P, Fq, Sq, Fh, Sh, F, Sx, C, fast_is_m ? csm : csn,
+                                                               fast_is_m ? csn : csm, fast_is_m, alpha, accumulate);
+    } else {
+        dim3 grid((unsigned)((Fh + STR_THREADS - 1) / STR_THREADS), (unsigned)(Sh < 32768 ? Sh : 32768));
+        strassen_combine_kernel<<<grid, STR_THREADS, 0, st>>>(P, Fh, Sh, F, Sx, C, fast_is_m ? csm : csn, fast_is_m ? csn : csm,
+                                                              fast_is_m, alpha, accumulate);
+    }
     count_launches(1);
 }

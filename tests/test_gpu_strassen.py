@@ -39,20 +39,21 @@ def _rel(a, b):
 
 
 @pytest.mark.parametrize("M,N,K", [(1031, 97, 1033), (1024, 96, 1024), (257, 129, 515), (130, 50, 70), (5, 3, 7), (2, 2, 2),
-                                   (1, 1, 1), (1, 9, 4), (300, 1, 33), (64, 64, 1)])
+                                   (1, 1, 1), (1, 9, 4), (300, 1, 33), (64, 64, 1), (7, 6, 5), (3, 3, 3), (515, 262, 1031)])
 @pytest.mark.parametrize("transposed_out", [False, True])
-def test_strassen_gemm_equals_the_definition(gpu, M, N, K, transposed_out):
+@pytest.mark.parametrize("levels", [1, 2])
+def test_strassen_gemm_equals_the_definition(gpu, M, N, K, transposed_out, levels):
     import torch
     A, B = _rand((M, K), 10 * M + K), _rand((N, K), 10 * N + K + 1)
     want = A @ B.T
-    got = gpu.zgemm_nt_strassen(A, B, transposed_out=transposed_out).cpu().numpy()
+    got = gpu.zgemm_nt_strassen(A, B, transposed_out=transposed_out, levels=levels).cpu().numpy()
     got = got.T if transposed_out else got
     assert _rel(got, want) < REL_TOL, _rel(got, want)
     # complex alpha, accumulation into a non-zero C (the products' scratch still holds the previous call's values)
     alpha = 0.7 - 1.3j
     C0 = _rand((N, M) if transposed_out else (M, N), 77)
     C = torch.from_numpy(C0.copy()).cuda()
-    gpu.zgemm_nt_strassen(A, B, C=C, alpha=alpha, accumulate=True, transposed_out=transposed_out)
+    gpu.zgemm_nt_strassen(A, B, C=C, alpha=alpha, accumulate=True, transposed_out=transposed_out, levels=levels)
     got = C.cpu().numpy()
     ref = (C0.T if transposed_out else C0) + alpha * want
     assert _rel(got.T if transposed_out else got, ref) < REL_TOL
@@ -66,21 +67,25 @@ def test_strassen_gemm_equals_the_plain_dmma_gemm_at_a_ladder_like_shape(gpu):
     A = torch.view_as_complex(torch.randn(M, K, 2, dtype=torch.float64, device="cuda", generator=g))
     B = torch.view_as_complex(torch.randn(N, K, 2, dtype=torch.float64, device="cuda", generator=g))
     plain = gpu.zgemm_nt(A, B, transposed_out=True)
-    fast = gpu.zgemm_nt_strassen(A, B, transposed_out=True)
     scale = float(plain.abs().max())
-    assert float((plain - fast).abs().max()) / scale < 1e-13
-    rows = [0, 1, 2279, 2280, 2281, 4559]                      # both sides of the split
-    want = (A[rows].cpu().numpy() @ B.cpu().numpy().T).T       # [n][rows]
-    assert np.abs(fast[:, rows].cpu().numpy() - want).max() / scale < REL_TOL
+    rows = [0, 1, 1139, 1140, 1141, 2279, 2280, 2281, 3419, 3420, 3421, 4559]      # both sides of every split
+    want = (A[rows].cpu().numpy() @ B.cpu().numpy().T).T                           # [n][rows]
+    for levels in (1, 2):
+        fast = gpu.zgemm_nt_strassen(A, B, transposed_out=True, levels=levels)
+        assert float((plain - fast).abs().max()) / scale < 1e-13
+        assert np.abs(fast[:, rows].cpu().numpy() - want).max() / scale < REL_TOL
 
 
-def test_context_with_strassen_equals_context_without(gpu):
-    """cfg1 (16/96/336): ov = 1536, vv = 4560 -- the level is used for the two (ov)^3 products, the pp-ladder and C."""
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_context_with_strassen_equals_context_without(gpu, mode):
+    """cfg1 (16/96/336): ov = 1536, vv = 4560 -- the scheme is used for the two (ov)^3 products and the pp-ladder.  mode 1: the
+    default choice of levels (one, at this size), 2: one level forced, 3: two levels forced on the (ov)^3 products."""
     o, v, naux = 16, 96, 336
     inp = ci.make_inputs(o, v, naux, 2021030801)
-    fast = gpu.CCSD(inp.h, inp.B, o, v, strassen=True)
-    plain = gpu.CCSD(inp.h, inp.B, o, v, strassen=False)
+    fast = gpu.CCSD(inp.h, inp.B, o, v, strassen=mode)
+    plain = gpu.CCSD(inp.h, inp.B, o, v, strassen=0)
     assert fast.workspace_bytes > plain.workspace_bytes      # the operand stacks of the constants
+    assert fast.strassen_steps().get("ring_gemm") == (2 if mode == 3 else 1) and plain.strassen_steps() == {}
     # same (MP2) amplitudes in both: every product on its own scale; the sums S1, S2 cancel against the driver term, so they
     # get the north_star bound relative to the largest term
     fast.residual(); plain.residual()
