@@ -830,6 +830,16 @@ def run_ours(args) -> None:
         W = torch.view_as_complex(torch.randn((vv, vv, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(5e-3 / np.sqrt(2))
         tau = torch.view_as_complex(torch.randn((oo, vv, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(0.01 / np.sqrt(2))
         R = torch.zeros((oo, vv), dtype=torch.complex128, device="cuda")
+        if args.strassen:
+            # the form ccsd_iterate runs: one Strassen level.  This standalone call also stacks <ab||cd> (done once, by ccsd_init,
+            # inside the solver), so ms_per_call is NOT the launch time; the batched gemm_dmma_kernel launch inside it is the
+            # launch of the iteration (same kernel, same grid) -- this leg exists to capture that launch with ncu.
+            ts = time_events(torch, lambda: pkg.zgemm_nt_strassen(W, tau, C=R, transposed_out=True), args.steps, args.warmup)
+            t = statistics.median(ts)
+            print(json.dumps({"metric": "pp_ladder_strassen_call_ms", "value": t, "unit": "ms", "ms_per_call": t,
+                              "config": {"workload": f"{cfg} pp-ladder {vv}x{oo}x{vv}, one Strassen level, both operand stacks made "
+                                                     "inside the call"}}))
+            return
         Ws, taus = pkg.sum_plane(W), pkg.sum_plane(tau)
         ts = time_events(torch, lambda: pkg.contract("pp_ladder_planes", o, v, [tau, W, taus, Ws], out=R),
                          args.steps, args.warmup)

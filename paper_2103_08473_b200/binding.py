@@ -317,6 +317,7 @@ class CCSD:
             self._ctx = ctypes.c_void_p(None)
             self._ws = None
             self._lam_ws = None
+            self._trip_ws = None
             if self.workspace_bytes >= (4 << 30):     # hand tens of GB back to the driver rather than to torch's cache
                 self._torch.cuda.empty_cache()
 
@@ -404,11 +405,14 @@ class CCSD:
         return out
 
     def _triples_workspace(self):
-        torch = self._torch
-        nbytes = ctypes.c_size_t(0)
-        self._call(self._lib.ccsd_triples_workspace_bytes, ctypes.byref(nbytes), where="ccsd_triples_workspace_bytes")
-        ws = _workspace(torch, nbytes.value)
-        return ws, (ws.data_ptr() + 255) // 256 * 256, int(nbytes.value)
+        """The triples workspace, allocated on first use and kept until close() (a fresh multi-GiB cudaMalloc per call costs
+        tenths of a second beside a 5 s computation)."""
+        if getattr(self, "_trip_ws", None) is None:
+            nbytes = ctypes.c_size_t(0)
+            self._call(self._lib.ccsd_triples_workspace_bytes, ctypes.byref(nbytes), where="ccsd_triples_workspace_bytes")
+            self._trip_ws = (_workspace(self._torch, nbytes.value), int(nbytes.value))
+        ws, nbytes = self._trip_ws
+        return ws, (ws.data_ptr() + 255) // 256 * 256, nbytes
 
     def triples(self) -> dict:
         """+T / (T) / -T corrections at the current amplitudes (ccsd_triples): {"+T": E, "(T)": E, "-T": E} (complex)."""

@@ -394,7 +394,11 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             if (L2rs) L2rs[ia * ov + me] = x.x + x.y;
             return x;
         });
-        CCSD_TRY(run_gemm(env, with_planes(gp(ov, ov, ov, L2r, ov, L->Wr, ov, X, ov, 1, 1.0, 0), L2rs, L->Wrs)));
+        if (c->strassen)      // the Strassen levels of the CCSD iteration's (ov)^3 products, in the same scratch (strassen.cuh)
+            CCSD_TRY(strassen_gemm(env, gp(ov, ov, ov, L2r, ov, L->Wr, ov, X, ov, 1, 1.0, 0), nullptr, nullptr, c->str_ring,
+                                   c->strassen_levels));
+        else
+            CCSD_TRY(run_gemm(env, with_planes(gp(ov, ov, ov, L2r, ov, L->Wr, ov, X, ov, 1, 1.0, 0), L2rs, L->Wrs)));
         const int2 *po = c->po, *pv = c->pv;
         launch_fill(st, L->Pacc, oo, vv, vv, 1, [=] __device__(int64_t IJ, int64_t AB) {
             const int2 ij = po[IJ], ab = pv[AB];
@@ -457,7 +461,15 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             if (plane) plane[IJ * vv + EF] = x.x + x.y;
             return x;
         });
-        CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
+        if (c->strassen && c->sW.S && strassen_stack_elems(oo, vv, 1) <= c->str_ring.b_elems) {
+            // one Strassen level with the stack of <ab||cd> ccsd_init made; conj(lambda) is stacked in the scratch of the (ov)^3
+            // products (idle here; tau's own stack stays valid for the CCSD residual's per-term hooks)
+            StrassenStack sl = strassen_stack(c->str_ring.SB, c->str_ring.SBp, oo, vv, 1);
+            launch_strassen_prep(st, 1, L->cl2p, vv, sl);
+            CCSD_TRY(strassen_gemm(env, gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), &c->sW, &sl, c->str_L));
+        } else {
+            CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
+        }
     }
     {   // R2p[(i<j)][(a<b)] = <ij||ab> + conj(P2) + Pacc
         const c128 *Voovv = c->Voovv_p, *P2 = L->P2, *Pacc = L->Pacc;

@@ -166,16 +166,21 @@ strassen_combine_kernel(const c128* __restrict__ P, int64_t Fh, int64_t Sh, int6
         strassen_quadrants(p, c11, c12, c21, c22);
         // quadrant (row half of m, row half of n): c12 is (m low, n high).  In (fast, slow) terms:
         const c128 q_fs[2][2] = {{c11, fast_is_m ? c12 : c21}, {fast_is_m ? c21 : c12, c22}};   // [fast half][slow half]
+        c128 old[2][2];        // all reads of C before the first write: the loads are independent of the stores
+#pragma unroll
+        for (int hf = 0; hf < 2; hf++)
+#pragma unroll
+            for (int hs = 0; hs < 2; hs++) {
+                const int64_t ff = f + hf * Fh, ss = s + hs * Sh;
+                old[hf][hs] = (accumulate && ff < F && ss < Sx) ? C[ff * stride_f + ss * stride_s] : mk(0.0, 0.0);
+            }
 #pragma unroll
         for (int hf = 0; hf < 2; hf++)
 #pragma unroll
             for (int hs = 0; hs < 2; hs++) {
                 const int64_t ff = f + hf * Fh, ss = s + hs * Sh;
                 if (ff >= F || ss >= Sx) continue;
-                c128* dst = C + ff * stride_f + ss * stride_s;
-                c128 val = cmul(alpha, q_fs[hf][hs]);
-                if (accumulate) val = cadd(val, *dst);
-                *dst = val;
+                C[ff * stride_f + ss * stride_s] = cadd(cmul(alpha, q_fs[hf][hs]), old[hf][hs]);
             }
     }
 }
@@ -191,6 +196,19 @@ strassen_combine2_kernel(const c128* __restrict__ P, int64_t Fq, int64_t Sq, int
     const int64_t plane = Fq * Sq;
     for (int64_t s = blockIdx.y; s < Sq; s += gridDim.y) {
         const int64_t at = s * Fq + f;
+        c128 old[2][2][2][2];  // all 16 reads of C before the first write (independent of the stores, issued with the P loads)
+#pragma unroll
+        for (int f2 = 0; f2 < 2; f2++)
+#pragma unroll
+            for (int s2 = 0; s2 < 2; s2++)
+#pragma unroll
+                for (int hf = 0; hf < 2; hf++)
+#pragma unroll
+                    for (int hs = 0; hs < 2; hs++) {
+                        const int64_t fi = f + f2 * Fq, si = s + s2 * Sq, ff = fi + hf * Fh, ss = si + hs * Sh;
+                        old[f2][s2][hf][hs] = (accumulate && fi < Fh && si < Sh && ff < F && ss < Sx) ? C[ff * stride_f + ss * stride_s]
+                                                                                                     : mk(0.0, 0.0);
+                    }
         c128 p1[2][2][7];      // [inner fast half][inner slow half][q1]: the half-size products at the four inner positions
 #pragma unroll
         for (int q1 = 0; q1 < 7; q1++) {
@@ -215,10 +233,7 @@ strassen_combine2_kernel(const c128* __restrict__ P, int64_t Fq, int64_t Sq, int
                     for (int hs = 0; hs < 2; hs++) {
                         const int64_t ff = fi + hf * Fh, ss = si + hs * Sh;
                         if (ff >= F || ss >= Sx) continue;
-                        c128* dst = C + ff * stride_f + ss * stride_s;
-                        c128 val = cmul(alpha, q_fs[hf][hs]);
-                        if (accumulate) val = cadd(val, *dst);
-                        *dst = val;
+                        C[ff * stride_f + ss * stride_s] = cadd(cmul(alpha, q_fs[hf][hs]), old[f2][s2][hf][hs]);
                     }
             }
     }
