@@ -187,7 +187,7 @@ strassen_combine_kernel(const c128* __restrict__ P, int64_t Fh, int64_t Sh, int6
 
 // Two levels in one pass: the 49 quarter-size products P[q1 * 7 + q2][slow][fast] -> the seven half-size products (in
 // registers, at the four inner positions) -> the 16 blocks of C.  (Fh, Sh: extents of a half, Fq, Sq: of a quarter.)
-__global__ void __launch_bounds__(STR_THREADS)
+__global__ void __launch_bounds__(STR_THREADS)   // 255 registers: every load of a thread in flight at once (a 128-register cap is 35 % slower)
 strassen_combine2_kernel(const c128* __restrict__ P, int64_t Fq, int64_t Sq, int64_t Fh, int64_t Sh, int64_t F, int64_t Sx,
                          c128* __restrict__ C, int64_t stride_f, int64_t stride_s, int fast_is_m, c128 alpha, int accumulate)
 {
@@ -196,46 +196,50 @@ strassen_combine2_kernel(const c128* __restrict__ P, int64_t Fq, int64_t Sq, int
     const int64_t plane = Fq * Sq;
     for (int64_t s = blockIdx.y; s < Sq; s += gridDim.y) {
         const int64_t at = s * Fq + f;
-        c128 old[2][2][2][2];  // all 16 reads of C before the first write (independent of the stores, issued with the P loads)
-#pragma unroll
-        for (int f2 = 0; f2 < 2; f2++)
-#pragma unroll
-            for (int s2 = 0; s2 < 2; s2++)
-#pragma unroll
-                for (int hf = 0; hf < 2; hf++)
-#pragma unroll
-                    for (int hs = 0; hs < 2; hs++) {
-                        const int64_t fi = f + f2 * Fq, si = s + s2 * Sq, ff = fi + hf * Fh, ss = si + hs * Sh;
-                        old[f2][s2][hf][hs] = (accumulate && fi < Fh && si < Sh && ff < F && ss < Sx) ? C[ff * stride_f + ss * stride_s]
-                                                                                                     : mk(0.0, 0.0);
-                    }
-        c128 p1[2][2][7];      // [inner fast half][inner slow half][q1]: the half-size products at the four inner positions
+        // out[inner position][outer quadrant], quadrants in the order (c11, c12, c21, c22).  The half-size products P1[q1] are
+        // never held together: each is formed at the four inner positions from its seven quarter-size products and added
+        // straight into the outer quadrants it belongs to -- in the order q1 = 0..6, which is the order of
+        // strassen_quadrants (c11 = ((P1 + P4) - P5) + P7, ...), so the sums have the bits of two separate passes.
+        c128 out[4][4];
 #pragma unroll
         for (int q1 = 0; q1 < 7; q1++) {
-            c128 p[7], c11, c12, c21, c22;
+            c128 p[7], sub[4];
 #pragma unroll
             for (int q2 = 0; q2 < 7; q2++) p[q2] = P[(q1 * 7 + q2) * plane + at];
-            strassen_quadrants(p, c11, c12, c21, c22);
-            p1[0][0][q1] = c11; p1[0][1][q1] = fast_is_m ? c12 : c21; p1[1][0][q1] = fast_is_m ? c21 : c12; p1[1][1][q1] = c22;
-        }
+            strassen_quadrants(p, sub[0], sub[1], sub[2], sub[3]);
 #pragma unroll
-        for (int f2 = 0; f2 < 2; f2++)
-#pragma unroll
-            for (int s2 = 0; s2 < 2; s2++) {
-                const int64_t fi = f + f2 * Fq, si = s + s2 * Sq;       // position inside a half
-                if (fi >= Fh || si >= Sh) continue;
-                c128 c11, c12, c21, c22;
-                strassen_quadrants(p1[f2][s2], c11, c12, c21, c22);
-                const c128 q_fs[2][2] = {{c11, fast_is_m ? c12 : c21}, {fast_is_m ? c21 : c12, c22}};
-#pragma unroll
-                for (int hf = 0; hf < 2; hf++)
-#pragma unroll
-                    for (int hs = 0; hs < 2; hs++) {
-                        const int64_t ff = fi + hf * Fh, ss = si + hs * Sh;
-                        if (ff >= F || ss >= Sx) continue;
-                        C[ff * stride_f + ss * stride_s] = cadd(cmul(alpha, q_fs[hf][hs]), old[f2][s2][hf][hs]);
-                    }
+            for (int u = 0; u < 4; u++) {
+                const c128 x = sub[u];
+                if (q1 == 0) { out[u][0] = x; out[u][3] = x; }
+                if (q1 == 1) { out[u][2] = x; out[u][3] = csub(out[u][3], x); }
+                if (q1 == 2) { out[u][1] = x; out[u][3] = cadd(out[u][3], x); }
+                if (q1 == 3) { out[u][0] = cadd(out[u][0], x); out[u][2] = cadd(out[u][2], x); }
+                if (q1 == 4) { out[u][0] = csub(out[u][0], x); out[u][1] = cadd(out[u][1], x); }
+                if (q1 == 5) { out[u][3] = cadd(out[u][3], x); }
+                if (q1 == 6) { out[u][0] = cadd(out[u][0], x); }
             }
+        }
+        // quadrant index (c11, c12, c21, c22) -> (fast half, slow half): c12 is (m low, n high).  One inner position at a time:
+        // its four reads of C are issued together, before its four writes.
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int f2 = fast_is_m ? (u >> 1) : (u & 1), s2 = fast_is_m ? (u & 1) : (u >> 1);
+            const int64_t fi = f + f2 * Fq, si = s + s2 * Sq;
+            if (fi >= Fh || si >= Sh) continue;
+            c128 old[4];
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const int hf = fast_is_m ? (q >> 1) : (q & 1), hs = fast_is_m ? (q & 1) : (q >> 1);
+                const int64_t ff = fi + hf * Fh, ss = si + hs * Sh;
+                old[q] = (accumulate && ff < F && ss < Sx) ? C[ff * stride_f + ss * stride_s] : mk(0.0, 0.0);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const int hf = fast_is_m ? (q >> 1) : (q & 1), hs = fast_is_m ? (q & 1) : (q >> 1);
+                const int64_t ff = fi + hf * Fh, ss = si + hs * Sh;
+                if (ff < F && ss < Sx) C[ff * stride_f + ss * stride_s] = cadd(cmul(alpha, out[u][q]), old[q]);
+            }
+        }
     }
 }
 
