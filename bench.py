@@ -34,7 +34,8 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of the 3M + sum-plane DMMA GEMM at cfg3, from
 # profiles/r02_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
 NCU_TRAFFIC_BYTES = {"cfg3": 23.10e9 + 0.220e9}
-NCU_TRAFFIC_BYTES_STRASSEN = {}     # the batched seven-product launch of the Strassen level: captured separately
+# ... and of the batched seven-product launch the pp-ladder is with one Strassen level (profiles/r02b_ncu_pp_ladder_strassen_cfg3.md)
+NCU_TRAFFIC_BYTES_STRASSEN = {"cfg3": 30.472e9 + 0.389e9}
 NCU_TRAFFIC_SOURCE = ("recorded constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of one "
                       "pp-ladder launch from the ncu --set full capture summarised in profiles/r02_ncu_pp_ladder_cfg3.md")
 
@@ -905,11 +906,12 @@ def run_ours(args) -> None:
     gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
     gemm_ms = sum(main["terms"][k]["ms"] for k in gemm_steps)
     traffic = (NCU_TRAFFIC_BYTES_STRASSEN if pp_strassen else NCU_TRAFFIC_BYTES).get(cfg)
+    traffic_source = NCU_TRAFFIC_SOURCE.replace("r02_ncu_pp_ladder_cfg3.md", "r02b_ncu_pp_ladder_strassen_cfg3.md") if pp_strassen else NCU_TRAFFIC_SOURCE
     roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch" +
                           (": ONE batched launch of the seven half-size products of a Strassen level" if pp_strassen else ""),
                 "achieved": round(pp_exec, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
                 "frac": round(pp_exec / peak, 4), "traffic": traffic,
-                "traffic_source": (NCU_TRAFFIC_SOURCE if traffic is not None else
+                "traffic_source": (traffic_source if traffic is not None else
                                    "no ncu --set full capture of this workload's launch on record"),
                 "real_flops_per_complex_mac": rf * (7.0 / 8.0 if pp_strassen else 1.0),
                 "achieved_8flop_convention": round(pp_tflops, 3),
