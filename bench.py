@@ -602,7 +602,7 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
                     "<ab||cd> with conjugated multipliers"}
 
 
-def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool = False) -> dict:
+def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool = False, c_levels: int = 1) -> dict:
     """Algorithmic bytes of the HBM-bound steps of one iteration (16 B read + 16 B written per element a
     permutation moves; the update streams (2 + 2m) vectors at the least; m = pairs in the DIIS subspace)."""
     oo, vv, ov = o * (o - 1) // 2, v * (v - 1) // 2, o * v
@@ -611,6 +611,8 @@ def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool =
     # with the Strassen level the planes of Xm, T2r are not written (their stacks carry planes); the stack of tau is: tau read
     # once, seven half-size matrices (16 B) and their planes (8 B) written
     tau_stack = oo * vv * 16 + 7 * ((oo + 1) // 2) * ((vv + 1) // 2) * 24
+    if c_levels == 2:       # C takes two levels: tau is stacked a second time, as 49 quarter-size matrices
+        tau_stack += oo * vv * 16 + 49 * ((oo + 3) // 4) * ((vv + 3) // 4) * 24
     return {"prep_permute": moved * 32 + ((tau_stack if strassen else 2 * ov * ov * 8) if planes else 0),
             # Jacobi + Gram row in one pass (S, t and m-1 stored e read; e, u written), then sum_l c_l u_l (m read, 1 written)
             "update_diis": (2 * m + 4) * nvec * 16,
@@ -691,7 +693,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
                 ent["strassen_levels"] = strassen_steps[k]
         terms[k] = ent
     for k in ("prep_permute", "update_diis", "energy"):       # HBM-bound steps: algorithmic bytes / time
-        gbs = [hbm_step_bytes(o, v, m, strassen="pp_ladder" in strassen_steps)[k] / (x * 1e-3) * 1e-9
+        gbs = [hbm_step_bytes(o, v, m, strassen="pp_ladder" in strassen_steps, c_levels=strassen_steps.get("C_ovoo", 1))[k] / (x * 1e-3) * 1e-9
                for x, m in zip(step_acc[k], m_hist) if x > 0]
         if gbs:
             terms[k]["gbs"] = round(statistics.median(gbs), 1)

@@ -279,8 +279,9 @@ struct ccsd_ctx {
     // quadratic H^{ak}_{ci} term) built once by ccsd_init, the stack of tau (right operand of the pp-ladder and of C) built by
     // prep_operands, and per-branch scratch for the stacks of Xm, Hm, T2r and for the seven products.
     bool strassen;
-    int strassen_levels;    // of the two (ov)^3 products: 1 or 2 (the pp-ladder and C always take one)
-    StrassenStack sW, sVvovv, sG1, sTau;
+    int strassen_levels;    // of the two (ov)^3 products: 1 or 2 (the pp-ladder always takes one)
+    int strassen_levels_C;  // of the <bk||cd> tau part of C: 1 or 2
+    StrassenStack sW, sVvovv, sG1, sTau, sTauC;   // sTauC: tau stacked for C when C takes two levels (else C shares sTau)
     StrassenScratch str_ring, str_C, str_L;
     // DIIS ring (reduce.cuh): stored pairs, device-side Gram matrix / coefficients / reduction scratch
     DiisRing diis;
@@ -453,7 +454,9 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
     c->strassen_levels = c->opt.strassen == 3 ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
     memset(&c->sW, 0, sizeof(c->sW)); memset(&c->sVvovv, 0, sizeof(c->sVvovv)); memset(&c->sG1, 0, sizeof(c->sG1));
-    memset(&c->sTau, 0, sizeof(c->sTau));
+    memset(&c->sTau, 0, sizeof(c->sTau)); memset(&c->sTauC, 0, sizeof(c->sTauC));
+    // C: a second level only where a quarter of its (i<j) extent still fills whole 48-column tiles (cfg3: 141 -> 144; cfg2: 69 -> 96 not)
+    c->strassen_levels_C = (c->strassen_levels == 2 && strassen_half(strassen_half(oo)) >= 128) ? 2 : 1;
     memset(&c->str_ring, 0, sizeof(c->str_ring)); memset(&c->str_C, 0, sizeof(c->str_C)); memset(&c->str_L, 0, sizeof(c->str_L));
     if (c->strassen) {
         const bool use_L = !c->opt.direct_ladder && strassen_worthwhile(vv, oo, vv);
@@ -474,20 +477,22 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
             return strassen_stack(S, Sp, R, K, levels);
         };
         if (use_L) c->sW = stack(false, vv, vv, 1);
-        if (use_C) c->sVvovv = stack(false, ov, vv, 1);
+        const int lvC = c->strassen_levels_C;
+        if (use_C) c->sVvovv = stack(false, ov, vv, lvC);
         c->sG1 = stack(false, ov, ov, lv);
         StrassenStack sa = stack(true, ov, ov, lv), sb = stack(true, ov, ov, lv);
         c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov, lv);
         c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov, lv);
         c->str_ring.p_elems = (lv == 2 ? 49 : 7) * strassen_rows(ov, lv) * strassen_rows(ov, lv);
         c->str_ring.P = place(c->str_ring.p_elems, sizeof(c128)).take<c128>(c->str_ring.p_elems);
-        if (use_L || use_C) c->sTau = stack(true, oo, vv, 1);
+        if (use_L || (use_C && lvC == 1)) c->sTau = stack(true, oo, vv, 1);
+        if (use_C && lvC == 2) c->sTauC = stack(true, oo, vv, 2);
         if (use_L) {
             c->str_L.p_elems = 7 * strassen_half(vv) * strassen_half(oo);
             c->str_L.P = place(c->str_L.p_elems, sizeof(c128)).take<c128>(c->str_L.p_elems);
         }
         if (use_C) {
-            c->str_C.p_elems = 7 * strassen_half(ov) * strassen_half(oo);
+            c->str_C.p_elems = (lvC == 2 ? 49 : 7) * strassen_rows(ov, lvC) * strassen_rows(oo, lvC);
             c->str_C.P = place(c->str_C.p_elems, sizeof(c128)).take<c128>(c->str_C.p_elems);
         }
     }
@@ -878,6 +883,7 @@ static int prep_operands(ccsd_ctx* c)
     const c128 *t1 = c->t1, *t2p = c->t2p, *taup = c->taup;
     double *Xms = c->strassen ? nullptr : c->Xms, *T2rs = c->strassen ? nullptr : c->T2rs;   // Strassen stacks carry their own planes
     if (c->sTau.S) launch_strassen_prep(st, 1, c->taup, vv, c->sTau);    // right operand of the pp-ladder and of C
+    if (c->sTauC.S) launch_strassen_prep(st, 1, c->taup, vv, c->sTauC);  // ... of C with two levels
     launch_fill(st, c->t1T, v, o, o, 0, [=] __device__(int64_t a, int64_t i) { return t1[i * v + a]; });
     // TT[(a<b)][0:oo) = tau^T   (K-contiguous operand of the hh-ladder + Goo product; the second half of TT, t2^T, is the operand
     // of the Goo term on its own: fill_TT_t2, made where that form is used -- the per-term hook and CC2)
@@ -1036,7 +1042,8 @@ static int build_C(ccsd_ctx* c)
         return CCSD_OK;
     }
     if (c->strassen && c->sVvovv.S)
-        return strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), &c->sVvovv, &c->sTau, c->str_C);
+        return strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), &c->sVvovv,
+                             c->strassen_levels_C == 2 ? &c->sTauC : &c->sTau, c->str_C, c->strassen_levels_C);
     CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, c->Cm + row0 * oo, oo, 1, -1.0, 1),
                                        c->Vvovv_ps ? c->Vvovv_ps + row0 * vv : nullptr, c->taups)));
     return CCSD_OK;
@@ -2579,7 +2586,7 @@ int ccsd_strassen_info(ccsd_ctx* c, int info[4])
     info[0] = c->strassen ? 1 : 0;
     info[1] = c->strassen ? c->strassen_levels : 0;      // the two (ov)^3 products: levels
     info[2] = (c->strassen && c->sW.S) ? 1 : 0;          // pp-ladder
-    info[3] = (c->strassen && c->sVvovv.S) ? 1 : 0;      // <bk||cd> tau part of C
+    info[3] = (c->strassen && c->sVvovv.S) ? c->strassen_levels_C : 0;      // <bk||cd> tau part of C
     return CCSD_OK;
 }
 
