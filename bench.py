@@ -55,7 +55,9 @@ def flops_per_iteration(o: int, v: int) -> dict:
         "Vdag_t1": 8 * o * vv * o * v,
         "Gvv_t2": 8 * oo * v * v * v,
         "C_t1": 8 * v * oo * v * o,
-        "S1": 8 * (v * o * o * vv + o * v * oo * v + 2 * ov * ov),
+        # S1: its <ak||cd> tau term (v o o vv MACs as a product of its own) is read off the product of C (a partial trace,
+        # ccsd_lib.cu s1_c_trace) on one GPU, so it is not counted as work
+        "S1": 8 * (o * v * oo * v + 2 * ov * ov),
     }
     f["total"] = sum(f.values())
     return f

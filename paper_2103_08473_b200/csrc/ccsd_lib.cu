@@ -263,6 +263,11 @@ struct ccsd_ctx {
     c128 *t1, *t2p, *t1T, *S1, *S2p, *taup, *TT, *AG, *Xm, *T2r, *tauc, *tauou, *t2hu;
     c128 *Hvv, *Gvv, *Hoo, *Goo, *Hov, *HovT, *HF, *inner, *Hm, *Cm, *Cm2, *Am, *tmp_ov;
     c128 *Xr, *P, *Qm, *Rr, *Y, *Z;
+    // The K = (c<d) product of C on its own, Cq[(b,k)][(i<j)] = -sum_{c<d} <bk||cd> tau^{cd}_{ij}: the <ak||cd> tau term of S1
+    // (eq 33) is a partial trace of it, S1[i,a] += sum_k <ak||cd> tau[i,k,c,d] = -+ Cq[(a,k)][(i,k)], so that term needs no product
+    // of its own (one GPU, not CC2: a sharded context holds only a slab of C, CC2 never forms this product)
+    c128* Cq;
+    bool s1_trace;
     // CC2 only: B blocks with the contracted virtual index fastest and the t1-dressed factors X (cc2_dressed_factors)
     c128 *BvvT, *BovT, *Xv, *Xo;
     double* Xvs;
@@ -419,6 +424,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Rr = w.take<c128>(v * oo * v);
     c->Y = w.take<c128>(ov * o * o);
     c->Z = w.take<c128>(oo * o * o);
+    c->s1_trace = !c->opt.cc2 && c->opt.shard_world <= 1;
+    c->Cq = c->s1_trace ? w.take<c128>(ov * oo) : nullptr;
     c->partial_elems = 16 * 1024 * 1024;  // split-K partials: >= 256 MB and >= 4 copies of the largest split-K output
     if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
     if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
@@ -1041,11 +1048,39 @@ static int build_C(ccsd_ctx* c)
         });
         return CCSD_OK;
     }
+    // - sum_{c<d} <bk||cd> tau^{cd}_{ij}: into Cq when S1 takes its <ak||cd> tau term from it (s1_c_trace), then added to Cm
+    c128* dst = c->s1_trace ? c->Cq : c->Cm + row0 * oo;
+    const int acc = c->s1_trace ? 0 : 1;
     if (c->strassen && c->sVvovv.S)
-        return strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, c->Cm, oo, 1, -1.0, 1), &c->sVvovv,
-                             c->strassen_levels_C == 2 ? &c->sTauC : &c->sTau, c->str_C, c->strassen_levels_C);
-    CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, c->Cm + row0 * oo, oo, 1, -1.0, 1),
-                                       c->Vvovv_ps ? c->Vvovv_ps + row0 * vv : nullptr, c->taups)));
+        CCSD_TRY(strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, dst, oo, 1, -1.0, acc), &c->sVvovv,
+                               c->strassen_levels_C == 2 ? &c->sTauC : &c->sTau, c->str_C, c->strassen_levels_C));
+    else
+        CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, dst, oo, 1, -1.0, acc),
+                                           c->Vvovv_ps ? c->Vvovv_ps + row0 * vv : nullptr, c->taups)));
+    if (c->s1_trace) {
+        const c128* Cq = c->Cq;
+        launch_fill(st, c->Cm, rows, oo, oo, 1, [=] __device__(int64_t r, int64_t IJ) { return Cq[r * oo + IJ]; });
+    }
+    return CCSD_OK;
+}
+
+// S1[i,a] += sum_{k, c<d} <ak||cd> tau[i,k,c,d]  (eq 33) read off the product of C: tau[i,k] = +-tau[(min,max)], so the sum over
+// (c<d) is -Cq[(a,k)][(i,k)] for i < k and +Cq[(a,k)][(k,i)] for k < i
+static int s1_c_trace(ccsd_ctx* c)
+{
+    if (!c->s1_trace) return CCSD_OK;
+    const c128* Cq = c->Cq;
+    const int o = c->o, v = c->v;
+    const int64_t oo = c->oo;
+    launch_fill(c->st, c->S1, o, v, v, 1, [=] __device__(int64_t i, int64_t a) {
+        c128 s = mk(0.0, 0.0);
+        for (int k = 0; k < o; k++) {
+            if (k == (int)i) continue;
+            const c128 x = (int)i < k ? cneg(Cq[(a * o + k) * oo + pair_idx((int)i, k, o)]) : Cq[(a * o + k) * oo + pair_idx(k, (int)i, o)];
+            s = cadd(s, x);
+        }
+        return s;
+    });
     return CCSD_OK;
 }
 
@@ -1375,7 +1410,8 @@ static int build_S1(ccsd_ctx* c)
         p.sam = 1; p.sak = o; p.sbn = 1; p.sbk = v;
         CCSD_TRY(run_gemm(env, p));
     }
-    CCSD_TRY(run_gemm(env, gp(v, o, o * vv, c->Vvovv_p, o * vv, c->tauou, o * vv, c->S1, 1, v, 1.0, 1)));  // <ak||cd> tau[i,k,c,d]
+    if (!c->s1_trace)      // else: s1_c_trace, once C's product is there
+        CCSD_TRY(run_gemm(env, gp(v, o, o * vv, c->Vvovv_p, o * vv, c->tauou, o * vv, c->S1, 1, v, 1.0, 1)));  // <ak||cd> tau[i,k,c,d]
     CCSD_TRY(run_gemm(env, gp(o, v, oo * v, c->Vooov_e, oo * v, c->tauc, oo * v, c->S1, v, 1, 1.0, 1)));   // <kl||ic> tau[k,l,c,a]
     CCSD_TRY(run_gemv(env, ov, ov, c->Vvovo_m, ov, c->t1T, c->tmp_ov, 1, 1.0, 0));                         // <ak||ci> t1[k,c]
     const c128* tmp = c->tmp_ov;
@@ -1411,6 +1447,7 @@ static int residual(ccsd_ctx* c)
     CCSD_TRY(s2_c_t1(c, c->S2p));
     tick(c, 13);
     CCSD_TRY(build_S1(c));
+    CCSD_TRY(s1_c_trace(c));
     tick(c, 14);
     c->have_residual = true;
     CCSD_CUDA_TRY(cudaGetLastError());
@@ -1512,6 +1549,7 @@ static int residual_forked(ccsd_ctx* c)
     CCSD_TRY(vdag_add(c, c->S2p));
     CCSD_TRY(gvv_add(c, c->S2p));
     CCSD_TRY(c_t1_add(c, c->S2p));
+    CCSD_TRY(s1_c_trace(c));
     c->have_residual = true;
     CCSD_CUDA_TRY(cudaGetLastError());
     return CCSD_OK;
