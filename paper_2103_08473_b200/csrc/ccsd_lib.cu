@@ -268,6 +268,11 @@ struct ccsd_ctx {
     // of its own (one GPU, not CC2: a sharded context holds only a slab of C, CC2 never forms this product)
     c128* Cq;
     bool s1_trace;
+    // In the same way the <ak||cd> t1 term of G^a_c (eq 25) is a partial trace of the linear term of H^{ak}_{ci} (eq 29):
+    // sum_{kd} <ak||cd> t1[k,d] = sum_k ( sum_d <ak||cd> t1[i,d] ) at i = k.  gvtr[a][c] holds it; it is added to Gvv once both the
+    // Fock-like terms and that product are there (gvv_trace_add), before Gvv's first use (the G_vv t2 product).
+    c128* gvtr;
+    bool gv_trace;
     // CC2 only: B blocks with the contracted virtual index fastest and the t1-dressed factors X (cc2_dressed_factors)
     c128 *BvvT, *BovT, *Xv, *Xo;
     double* Xvs;
@@ -426,6 +431,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Z = w.take<c128>(oo * o * o);
     c->s1_trace = !c->opt.cc2 && c->opt.shard_world <= 1;
     c->Cq = c->s1_trace ? w.take<c128>(ov * oo) : nullptr;
+    c->gv_trace = c->s1_trace;
+    c->gvtr = c->gv_trace ? w.take<c128>(v * v) : nullptr;
     c->partial_elems = 16 * 1024 * 1024;  // split-K partials: >= 256 MB and >= 4 copies of the largest split-K output
     if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
     if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
@@ -951,7 +958,8 @@ static int fock_like(ccsd_ctx* c)
     CCSD_TRY(run_gemm(env, gp(v, v, oo * v, c->tauc, oo * v, c->Voovv_c, oo * v, c->Hvv, v, 1, 1.0, 1)));
     // eq 25: Gvv = Hvv + sum_{kd} <ak||cd> t1[k,d] - sum_k f[k,c] t1[k,a]
     dcopy(st, c->Gvv, c->Hvv, (int64_t)v * v);
-    CCSD_TRY(run_gemv(env, (int64_t)v * v, ov, c->Vvovv_u, ov, c->t1, c->Gvv, 1, 1.0, 1));
+    if (!c->gv_trace)     // else: read off the linear term of H^{ak}_{ci} (build_Hvovo, gvv_trace_add)
+        CCSD_TRY(run_gemv(env, (int64_t)v * v, ov, c->Vvovv_u, ov, c->t1, c->Gvv, 1, 1.0, 1));
     {
         GemmParams p = gp(v, v, o, c->t1T, o, f + o, 1, c->Gvv, v, 1, -1.0, 1);
         p.sbn = 1; p.sbk = n;  // B[c][k] = f[k][o+c]
@@ -981,6 +989,17 @@ static int build_Hvovo(ccsd_ctx* c)
         GemmParams p = gp(ov, o, v, c->Vvovv_u + (int64_t)a0 * ov * v, v, c->t1, v, c->Hm + off, 1, ov, 1.0, 1);
         p.batch = na; p.bsA = ov * v; p.bsB = 0; p.bsC = (int64_t)o * ov;
         CCSD_TRY(run_gemm(env, p));
+    }
+    if (c->gv_trace) {    // gvtr[a][c] = sum_k ( Hm - <ak||ci> )[(a,k)][(c,k)]: the product just added, at i = k
+        const c128 *Hm = c->Hm, *V0 = c->Vvovo_m;
+        launch_fill(c->st, c->gvtr, v, v, v, 0, [=] __device__(int64_t a, int64_t cc) {
+            c128 s = mk(0.0, 0.0);
+            for (int k = 0; k < o; k++) {
+                const int64_t at = (a * o + k) * ov + cc * o + k;
+                s = cadd(s, csub(Hm[at], V0[at]));
+            }
+            return s;
+        });
     }
     // - sum_l <kl||ic> t1[l,a]            C[a][(i,c,k)]
     CCSD_TRY(run_gemm(env, gp(na, (int64_t)o * ov, o, c->t1T + (int64_t)a0 * o, o, c->Vooov_b, o, c->Hm + off, (int64_t)o * ov, 1, -1.0, 1)));
@@ -1321,6 +1340,13 @@ static int s2_vdag_t1(ccsd_ctx* c, c128* S)
     CCSD_TRY(vdag_gemm(c));
     return vdag_add(c, S);
 }
+static void gvv_trace_add(ccsd_ctx* c)
+{   // Gvv += gvtr (see ccsd_ctx::gvtr): after fock_like and the linear term of build_Hvovo, before gvv_gemm
+    if (!c->gv_trace) return;
+    const c128* g = c->gvtr;
+    const int v = c->v;
+    launch_fill(c->st, c->Gvv, v, v, v, 1, [=] __device__(int64_t a, int64_t cc) { return g[a * v + cc]; });
+}
 static int gvv_gemm(ccsd_ctx* c)
 {   // Qm[(i<j,b)][a] = sum_c t2[i,j,b,c] Gvv[a,c]; rows (i<j) of this rank
     const int v = c->v;
@@ -1427,6 +1453,7 @@ static int residual(ccsd_ctx* c)
     CCSD_TRY(fock_like(c));
     tick(c, 2);
     CCSD_TRY(build_Hvovo(c));   // ticks 3 inside
+    gvv_trace_add(c);
     tick(c, 4);
     CCSD_TRY(build_C(c));
     tick(c, 5);
@@ -1518,7 +1545,7 @@ static int residual_forked(ccsd_ctx* c)
     if (ok) {
         slot(1);
         s = fock_like(c);
-        if (s == CCSD_OK) s = gvv_gemm(c);
+        if (s == CCSD_OK && !c->gv_trace) s = gvv_gemm(c);     // with gv_trace Gvv is complete only after the join
         if (s == CCSD_OK) s = build_S1(c);
         ok = s == CCSD_OK && fk.end_branch();
     }
@@ -1544,6 +1571,10 @@ static int residual_forked(ccsd_ctx* c)
     slot(0);
     if (s != CCSD_OK) return s;
     if (!ok || !fk.join()) return CCSD_ECUDA;
+    if (c->gv_trace) {
+        gvv_trace_add(c);
+        CCSD_TRY(gvv_gemm(c));
+    }
     CCSD_TRY(s2_hh_and_goo(c, c->S2p));
     CCSD_TRY(ring_add(c, c->S2p));
     CCSD_TRY(vdag_add(c, c->S2p));
