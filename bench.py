@@ -48,9 +48,11 @@ def flops_per_iteration(o: int, v: int) -> dict:
         "Hvovo_quad": 8 * ov ** 3,
         "ring_gemm": 8 * ov ** 3,
         "C_ovoo": 8 * ov * oo * vv + 8 * ov * o * o * v,
-        "A_oooo": 8 * oo * oo * vv + 8 * oo * o * o * v,
+        # the quartic term of A (oo oo vv MACs) is timed with the Fock-like terms: H^k_i reads ITS quartic term (o o o vv MACs as a
+        # product of its own) off that product as a partial trace, as G^a_c reads its <ak||cd> t1 term off the linear term of H^{ak}_{ci}
+        "A_oooo": 8 * oo * o * o * v,
         "hh_ladder+Goo": 8 * oo * oo * vv,            # algorithmic: hh-ladder oo^2 vv (+ Goo term o*oo*vv*... small)
-        "fock_like": 8 * (v * v * oo * v + o * o * o * vv + 2 * ov * ov),
+        "fock_like": 8 * (v * v * oo * v + oo * oo * vv + ov * ov),
         "Hvovo_linear": 8 * (v * ov * o * v + v * o * ov * o),
         "Vdag_t1": 8 * o * vv * o * v,
         "Gvv_t2": 8 * oo * v * v * v,

@@ -273,6 +273,10 @@ struct ccsd_ctx {
     // Fock-like terms and that product are there (gvv_trace_add), before Gvv's first use (the G_vv t2 product).
     c128* gvtr;
     bool gv_trace;
+    // ... and the <kl||cd> tau term of H^k_i (eq 26) is a partial trace of the quartic term of A (eq 31):
+    // sum_{l, c<d} <kl||cd> tau[l,i,c,d] = sum_l +- Aq[(k,l)][(l,i)], Aq[(k<l)][(i<j)] = sum_{c<d} <kl||cd> tau^{cd}_{ij} (build_Aq)
+    c128* Aq;
+    bool hoo_trace;
     // CC2 only: B blocks with the contracted virtual index fastest and the t1-dressed factors X (cc2_dressed_factors)
     c128 *BvvT, *BovT, *Xv, *Xo;
     double* Xvs;
@@ -433,6 +437,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->Cq = c->s1_trace ? w.take<c128>(ov * oo) : nullptr;
     c->gv_trace = c->s1_trace;
     c->gvtr = c->gv_trace ? w.take<c128>(v * v) : nullptr;
+    c->hoo_trace = c->s1_trace;
+    c->Aq = c->hoo_trace ? w.take<c128>(oo * oo) : nullptr;
     c->partial_elems = 16 * 1024 * 1024;  // split-K partials: >= 256 MB and >= 4 copies of the largest split-K output
     if (c->partial_elems < 4 * oo * vv) c->partial_elems = 4 * oo * vv;
     if (c->partial_elems < 4 * ov * ov) c->partial_elems = 4 * ov * ov;
@@ -925,7 +931,8 @@ static int prep_operands(ccsd_ctx* c)
         int d = col % v;
         return asym_col(taup, KL, vv, d, (int)a, v);
     });
-    // tauou[(i,l)][(c<d)] = tau[i,l,c,d]
+    // tauou[(i,l)][(c<d)] = tau[i,l,c,d]: operand of the quartic terms of H^k_i and S1 where those are products of their own
+    if (!(c->hoo_trace && c->s1_trace))
     launch_fill(st, c->tauou, (int64_t)o * o, vv, vv, 0, [=] __device__(int64_t il, int64_t CD) {
         int i = il / o, l = il % o;
         if (i == l) return mk(0.0, 0.0);
@@ -939,6 +946,15 @@ static int prep_operands(ccsd_ctx* c)
         return asym_col(t2p, IJ, vv, b, (int)cc, v);
     });
     return CCSD_OK;
+}
+
+// Aq[(k<l)][(i<j)] = sum_{c<d} <kl||cd> tau^{cd}_{ij}: the quartic term of A (eq 31), kept on its own because H^k_i (eq 26)
+// reads its own quartic term off it (fock_like); build_A adds it into A.  Runs before fock_like.
+static int build_Aq(ccsd_ctx* c)
+{
+    if (!c->hoo_trace) return CCSD_OK;
+    return run_gemm(c->env, with_planes(gp(c->oo, c->oo, c->vv, c->Voovv_p, c->vv, c->taup, c->vv, c->Aq, c->oo, 1, 1.0, 0),
+                                        c->Voovv_ps, c->taups));
 }
 
 static int fock_like(ccsd_ctx* c)
@@ -966,8 +982,23 @@ static int fock_like(ccsd_ctx* c)
         CCSD_TRY(run_gemm(env, p));
     }
     // eq 26: Hoo[k,i] = -f[k,i] + sum_{l, c<d} <kl||cd> tau[l,i,c,d]   (tau[l,i] = -tauou[(i,l)])
-    launch_fill(st, c->Hoo, o, o, o, 0, [=] __device__(int64_t k, int64_t i) { return cneg(f[k * n + i]); });
-    CCSD_TRY(run_gemm(env, gp(o, o, o * vv, c->Voovv_ou, o * vv, c->tauou, o * vv, c->Hoo, o, 1, -1.0, 1)));
+    if (c->hoo_trace) {   // <kl||cd> = +-V[(k,l)], tau[l,i] = +-tau[(l,i)]: the sum over (c<d) is +-Aq[(k,l)][(l,i)]
+        const c128* Aq = c->Aq;
+        launch_fill(st, c->Hoo, o, o, o, 0, [=] __device__(int64_t k, int64_t i) {
+            c128 s = cneg(f[k * n + i]);
+            for (int l = 0; l < o; l++) {
+                if (l == (int)k || l == (int)i) continue;
+                const int64_t KL = (int)k < l ? pair_idx((int)k, l, o) : pair_idx(l, (int)k, o);
+                const int64_t LI = l < (int)i ? pair_idx(l, (int)i, o) : pair_idx((int)i, l, o);
+                const c128 x = Aq[KL * oo + LI];
+                s = (((int)k < l) == (l < (int)i)) ? cadd(s, x) : csub(s, x);
+            }
+            return s;
+        });
+    } else {
+        launch_fill(st, c->Hoo, o, o, o, 0, [=] __device__(int64_t k, int64_t i) { return cneg(f[k * n + i]); });
+        CCSD_TRY(run_gemm(env, gp(o, o, o * vv, c->Voovv_ou, o * vv, c->tauou, o * vv, c->Hoo, o, 1, -1.0, 1)));
+    }
     // eq 27: Goo = Hoo - sum_{lc} <kl||ic> t1[l,c] - sum_c f[k,c] t1[i,c]
     dcopy(st, c->Goo, c->Hoo, (int64_t)o * o);
     CCSD_TRY(run_gemv(env, (int64_t)o * o, ov, c->Vooov_d, ov, c->t1, c->Goo, 1, -1.0, 1));
@@ -1118,6 +1149,11 @@ static int build_A(ccsd_ctx* c)
         int2 ij = po[IJ];
         return csub(Z[(KL * o + ij.x) * o + ij.y], Z[(KL * o + ij.y) * o + ij.x]);
     });
+    if (c->hoo_trace) {   // the quartic term is there already (build_Aq)
+        const c128* Aq = c->Aq;
+        launch_fill(st, c->Am, oo, oo, oo, 1, [=] __device__(int64_t KL, int64_t IJ) { return Aq[KL * oo + IJ]; });
+        return CCSD_OK;
+    }
     CCSD_TRY(run_gemm(env, with_planes(gp(oo, oo, vv, c->Voovv_p, vv, c->taup, vv, c->Am, oo, 1, 1.0, 1), c->Voovv_ps, c->taups)));
     return CCSD_OK;
 }
@@ -1450,6 +1486,7 @@ static int residual(ccsd_ctx* c)
     tick(c, 0);
     CCSD_TRY(prep_operands(c));
     tick(c, 1);
+    CCSD_TRY(build_Aq(c));      // the quartic term of A: timed with the Fock-like terms, which read H^k_i's quartic term off it
     CCSD_TRY(fock_like(c));
     tick(c, 2);
     CCSD_TRY(build_Hvovo(c));   // ticks 3 inside
@@ -1544,7 +1581,9 @@ static int residual_forked(ccsd_ctx* c)
     }
     if (ok) {
         slot(1);
-        s = fock_like(c);
+        s = build_Aq(c);
+        if (s == CCSD_OK && c->hoo_trace) s = build_A(c);      // A needs Aq: same branch
+        if (s == CCSD_OK) s = fock_like(c);
         if (s == CCSD_OK && !c->gv_trace) s = gvv_gemm(c);     // with gv_trace Gvv is complete only after the join
         if (s == CCSD_OK) s = build_S1(c);
         ok = s == CCSD_OK && fk.end_branch();
@@ -1557,7 +1596,7 @@ static int residual_forked(ccsd_ctx* c)
     }
     if (ok) {
         slot(3);
-        s = build_A(c);
+        s = c->hoo_trace ? CCSD_OK : build_A(c);
         if (s == CCSD_OK) s = vdag_gemm(c);
         ok = s == CCSD_OK && fk.end_branch();
     }
