@@ -914,12 +914,12 @@ def run_ours(args) -> None:
     traffic = (NCU_TRAFFIC_BYTES_STRASSEN if pp_strassen else NCU_TRAFFIC_BYTES).get(cfg)
     traffic_source = NCU_TRAFFIC_SOURCE.replace("r02_ncu_pp_ladder_cfg3.md", "r02b_ncu_pp_ladder_strassen_cfg3.md") if pp_strassen else NCU_TRAFFIC_SOURCE
     roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch" +
-                          (": ONE batched launch of the seven half-size products of a Strassen level" if pp_strassen else ""),
+                          (": ONE batched launch of the 7 half-size / 49 quarter-size products of its Strassen level(s)" if pp_strassen else ""),
                 "achieved": round(pp_exec, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
                 "frac": round(pp_exec / peak, 4), "traffic": traffic,
                 "traffic_source": (traffic_source if traffic is not None else
                                    "no ncu --set full capture of this workload's launch on record"),
-                "real_flops_per_complex_mac": rf * (7.0 / 8.0 if pp_strassen else 1.0),
+                "real_flops_per_complex_mac": 8.0 * ex_pp,
                 "achieved_8flop_convention": round(pp_tflops, 3),
                 "note": "unit = complex MAC over the packed ranges (oo*vv*vv per launch); achieved counts the real "
                         "flops the kernel EXECUTES per unit (6 with 3M; x 7/8 = 5.25 when the product runs as one Strassen "
@@ -1002,7 +1002,7 @@ def main():
     ap.add_argument("--graph", type=int, default=1, help="ccsd_options.graph of the main leg: 0 direct launches, 1 graph with parallel "
                                                           "branches, 3 serial graph (profiling aid)")
     ap.add_argument("--strassen", type=int, default=1, help="ccsd_options.strassen of the main leg: 1 (default) Strassen levels on "
-                    "the four large contractions, 0 plain products, 2 one level only, 3 two levels on the (ov)^3 products")
+                    "the four large contractions, 0 plain products, 2 one level only, 3 two levels everywhere (tests)")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")

@@ -85,14 +85,17 @@ typedef struct {
     int strassen;       /* 1 (default) = the four large contractions of an iteration -- the two (ov)^3 products of eq 29 and of
                            the ring term, the pp-ladder and the <bk||cd> tau part of eq 30 -- run by Strassen's algorithm around
                            the DMMA GEMM: seven half-size products in ONE batched launch instead of eight, i.e. 7/8 of the FP64
-                           tensor-pipe work, plus three streaming passes; the two (ov)^3 products
-                           take TWO levels (49 quarter-size products, 0.766 of the work) from ov >= 3072.  Pure FP64; results
+                           tensor-pipe work, plus three streaming passes; TWO levels (49
+                           quarter-size products, 0.766 of the work) for the (ov)^3 products from ov >= 3072 and for the ladder
+                           and C where a quarter of the (i<j) extent still fills whole tiles (oo >= 510).  Pure FP64; results
                            differ from strassen = 0 by rounding only (about 1e-14 of the largest element of each product at
                            most).  Costs workspace: the operand stacks of <ab||cd>, <bk||cd> and <kl||cd> are built once and
-                           kept (1.75 x - 3 x the bytes of those tensors with their planes).  Used on one GPU with the 3M kernels
+                           kept (1.75 x - 3 x the bytes of those tensors with their planes); where the ladder and C both use
+                           it, the packed <ab||cd> itself is NOT kept beside its stack (ccsd_get_tensor(CCSD_T_VVVV) rebuilds
+                           it from the stack, exact up to one rounding per element).  Used on one GPU with the 3M kernels
                            (gemm_mode 0 or 3) where the products are large enough (ov >= 1024); ignored in cc2 mode and in a
                            sharded context; with direct_ladder the ladder keeps its slab form.  0 = plain products;
-                           2 = one level everywhere; 3 = two levels on the (ov)^3 products whatever their size (tests) */
+                           2 = one level only; 3 = two levels on all four products whatever their size (tests) */
 } ccsd_options;
 
 /* Fill *opts with the defaults above. */

@@ -295,6 +295,9 @@ struct ccsd_ctx {
     bool strassen;
     int strassen_levels;    // of the two (ov)^3 products: 1 or 2 (the pp-ladder always takes one)
     int strassen_levels_C;  // of the <bk||cd> tau part of C: 1 or 2
+    bool W_dropped;         // the packed <ab||cd> is not kept beside its operand stack (c->W = null after ccsd_init)
+    c128* W_init;           // where ccsd_init builds it meanwhile
+    int strassen_levels_L;  // of the pp-ladder: 1, or 2 with opts.strassen = 4 (an 18 GiB larger stack of <ab||cd> at cfg3)
     StrassenStack sW, sVvovv, sG1, sTau, sTauC;   // sTauC: tau stacked for C when C takes two levels (else C shares sTau)
     StrassenScratch str_ring, str_C, str_L;
     // DIIS ring (reduce.cuh): stored pairs, device-side Gram matrix / coefficients / reduction scratch
@@ -335,13 +338,33 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
 {
     Carver w{base, 0};
     const int64_t o = c->o, v = c->v, n = c->n, Lp = c->Lp, oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
+    c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
+    // Strassen levels (strassen.cuh) on the (ov)^3 products, the pp-ladder and the <bk||cd> tau part of C: one GPU, 3M planes.
+    // opts.strassen: 1 = levels chosen by size, 2 = one level wherever it pays, 3 = two levels everywhere whatever the size (tests)
+    const bool force = c->opt.strassen == 3;
+    c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 &&
+                  (force ? (o >= 2 && v >= 2) : strassen_worthwhile(ov, ov, ov));
+    const bool use_L = c->strassen && !c->opt.direct_ladder && (force || strassen_worthwhile(vv, oo, vv));
+    const bool use_C = c->strassen && (force || strassen_worthwhile(ov, oo, vv));
+    // two levels on the (ov)^3 products where a quarter-size product is still a long-K, many-tile GEMM (measured: 0.80 of the
+    // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
+    c->strassen_levels = force ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
+    // C and the ladder: a second level only where a quarter of their (i<j) extent still fills whole 48-column tiles (cfg3: 141 ->
+    // 144; cfg2: 69 -> 96 does not)
+    c->strassen_levels_C = force ? 2 : ((c->strassen_levels == 2 && strassen_half(strassen_half(oo)) >= 128) ? 2 : 1);
+    c->strassen_levels_L = force ? 2 : ((c->strassen_levels_C == 2 && use_C && use_L) ? 2 : 1);
     c->po = w.take<int2>(oo);
     c->pv = w.take<int2>(vv);
     c->eps = w.take<double>(n);
     c->eps0 = w.take<double>(n);
     c->f = w.take<c128>(n * n);
     // <ab||cd> is not stored in direct_ladder mode (rebuilt every iteration) nor in CC2 mode (its only use factorises)
-    c->W = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<c128>((c->sh.w_hi - c->sh.w_lo) * vv);   // this rank's rows
+    // With the Strassen ladder <ab||cd> lives on as its operand stack only (c->sW; single elements: strassen_left_at).  ccsd_init
+    // builds the packed tensor in the memory of C's operand stack, stacks it, and only then fills C's stack (c->W_init).
+    c->W_dropped = use_L && use_C && strassen_stack_elems(ov, vv, c->strassen_levels_C) * (int64_t)(sizeof(c128) + sizeof(double)) >=
+                                         vv * vv * (int64_t)sizeof(c128) + 512;
+    c->W_init = nullptr;
+    c->W = (c->opt.direct_ladder || c->opt.cc2 || c->W_dropped) ? nullptr : w.take<c128>((c->sh.w_hi - c->sh.w_lo) * vv);   // this rank's rows
     c->Vvovv_p = w.take<c128>(v * o * vv);
     c->Vvovv_u = w.take<c128>(v * v * o * v);
     c->VvovvT = w.take<c128>(o * vv * v);
@@ -446,17 +469,18 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     // four more split-K slots, one per parallel branch of the captured residual (residual_forked): 32 Mi elements at most
     c->partial_extra_elems = c->partial_elems < 32 * 1024 * 1024 ? c->partial_elems : 32 * 1024 * 1024;
     c->partial_extra = (c->opt.graph && !c->opt.cc2) ? w.take<c128>(4 * c->partial_extra_elems) : nullptr;
-    c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     c->Ws = c->Vvovv_ps = c->Voovv_ps = c->G1s = c->taups = c->Xms = c->T2rs = c->Hms = nullptr;
-    if (c->planes) {
-        c->Ws = (c->opt.direct_ladder || c->opt.cc2) ? nullptr : w.take<double>((c->sh.w_hi - c->sh.w_lo) * vv);
-        c->Vvovv_ps = w.take<double>(ov * vv);
+    if (c->planes) {   // an operand whose product runs through Strassen stacks needs no plane of its own (the stacks carry theirs)
+        c->Ws = (c->opt.direct_ladder || c->opt.cc2 || use_L) ? nullptr : w.take<double>((c->sh.w_hi - c->sh.w_lo) * vv);
+        c->Vvovv_ps = use_C ? nullptr : w.take<double>(ov * vv);
         c->Voovv_ps = w.take<double>(oo * vv);
-        c->G1s = w.take<double>(ov * ov);
         c->taups = w.take<double>(oo * vv);
-        c->Xms = w.take<double>(ov * ov);
-        c->T2rs = w.take<double>(ov * ov);
-        c->Hms = w.take<double>(ov * ov);
+        if (!c->strassen) {
+            c->G1s = w.take<double>(ov * ov);
+            c->Xms = w.take<double>(ov * ov);
+            c->T2rs = w.take<double>(ov * ov);
+            c->Hms = w.take<double>(ov * ov);
+        }
     }
     c->Bvvs = (c->planes && !c->opt.cc2) ? w.take<double>(v * v * Lp) : nullptr;
     c->BvvT = c->BovT = c->Xv = c->Xo = nullptr;
@@ -468,19 +492,10 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
         c->Xo = w.take<c128>(o * o * Lp);
         c->Xvs = w.take<double>(ov * Lp);
     }
-    // One Strassen level (strassen.cuh) on the (ov)^3 products, the pp-ladder and the <bk||cd> tau part of C: one GPU, 3M planes
-    c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 && strassen_worthwhile(ov, ov, ov);
-    // two levels on the (ov)^3 products where a quarter-size product is still a long-K, many-tile GEMM (measured: 0.80 of the
-    // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
-    c->strassen_levels = c->opt.strassen == 3 ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
     memset(&c->sW, 0, sizeof(c->sW)); memset(&c->sVvovv, 0, sizeof(c->sVvovv)); memset(&c->sG1, 0, sizeof(c->sG1));
     memset(&c->sTau, 0, sizeof(c->sTau)); memset(&c->sTauC, 0, sizeof(c->sTauC));
-    // C: a second level only where a quarter of its (i<j) extent still fills whole 48-column tiles (cfg3: 141 -> 144; cfg2: 69 -> 96 not)
-    c->strassen_levels_C = (c->strassen_levels == 2 && strassen_half(strassen_half(oo)) >= 128) ? 2 : 1;
     memset(&c->str_ring, 0, sizeof(c->str_ring)); memset(&c->str_C, 0, sizeof(c->str_C)); memset(&c->str_L, 0, sizeof(c->str_L));
     if (c->strassen) {
-        const bool use_L = !c->opt.direct_ladder && strassen_worthwhile(vv, oo, vv);
-        const bool use_C = strassen_worthwhile(ov, oo, vv);
         const int lv = c->strassen_levels;
         // Per-iteration stacks and products go into the dead init temporaries [Jovov, Joooo] while they fit there (largest
         // first), the rest and the stacks of the constants are appended.
@@ -496,19 +511,21 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
             double* Sp = (scratch ? place(e, sizeof(double)) : w).take<double>(e);
             return strassen_stack(S, Sp, R, K, levels);
         };
-        if (use_L) c->sW = stack(false, vv, vv, 1);
+        const int lvL = c->strassen_levels_L;
+        if (use_L) c->sW = stack(false, vv, vv, lvL);
         const int lvC = c->strassen_levels_C;
         if (use_C) c->sVvovv = stack(false, ov, vv, lvC);
+        if (c->W_dropped) c->W_init = c->sVvovv.S;      // S and Sp are adjacent: together they hold the packed tensor
         c->sG1 = stack(false, ov, ov, lv);
         StrassenStack sa = stack(true, ov, ov, lv), sb = stack(true, ov, ov, lv);
         c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov, lv);
         c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov, lv);
         c->str_ring.p_elems = (lv == 2 ? 49 : 7) * strassen_rows(ov, lv) * strassen_rows(ov, lv);
         c->str_ring.P = place(c->str_ring.p_elems, sizeof(c128)).take<c128>(c->str_ring.p_elems);
-        if (use_L || (use_C && lvC == 1)) c->sTau = stack(true, oo, vv, 1);
-        if (use_C && lvC == 2) c->sTauC = stack(true, oo, vv, 2);
+        if ((use_L && lvL == 1) || (use_C && lvC == 1)) c->sTau = stack(true, oo, vv, 1);
+        if ((use_L && lvL == 2) || (use_C && lvC == 2)) c->sTauC = stack(true, oo, vv, 2);
         if (use_L) {
-            c->str_L.p_elems = 7 * strassen_half(vv) * strassen_half(oo);
+            c->str_L.p_elems = (lvL == 2 ? 49 : 7) * strassen_rows(vv, lvL) * strassen_rows(oo, lvL);
             c->str_L.P = place(c->str_L.p_elems, sizeof(c128)).take<c128>(c->str_L.p_elems);
         }
         if (use_C) {
@@ -801,13 +818,14 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
     //   Jslab[(a,c)][(b,d)] = (ac|bd)                      (GEMM over the auxiliary index)
     //   JslabT[(b,c)][(a,d)] = Jslab[(a,d)][(b,c)]         (tiled transposition, bandwidth bound)
     //   W[(a<b)][(c<d)] = Jslab[(a,c)][(b,d)] - JslabT[(b,c)][(a,d)]     (both reads contiguous in d)
-    if (c->W) {
+    c128* const Wdst = c->W ? c->W : c->W_init;
+    if (Wdst) {
         std::vector<cudaEvent_t> events;
         c->init_events = &events;
         int s = CCSD_OK;
         for (int a0 = c->sh.wa_lo; a0 < c->sh.wa_hi && vv > 0 && s == CCSD_OK; a0 += c->na_slab) {
             int64_t r0 = 0, nrows = 0;      // "absolute" rows, relative to this rank's first row
-            s = build_W_slab(c, a0, c->sh.wa_hi, c->W - c->sh.w_lo * vv, true, &r0, &nrows);
+            s = build_W_slab(c, a0, c->sh.wa_hi, Wdst - c->sh.w_lo * vv, true, &r0, &nrows);
         }
         c->init_events = nullptr;
         if (s == CCSD_OK && !events.empty() && cudaStreamSynchronize(st) == cudaSuccess) {
@@ -821,10 +839,10 @@ static int build_constants(ccsd_ctx* c, const c128* h, const c128* B)
         CCSD_TRY(s);
     }
     if (c->planes) {   // sum planes of the constant operands of the large GEMMs (3M, gemm_dmma.cuh)
-        if (c->W) launch_sum_plane(st, c->W, c->Ws, (c->sh.w_hi - c->sh.w_lo) * vv);
-        launch_sum_plane(st, c->Vvovv_p, c->Vvovv_ps, ov * vv);
+        if (c->W && c->Ws) launch_sum_plane(st, c->W, c->Ws, (c->sh.w_hi - c->sh.w_lo) * vv);
+        if (c->Vvovv_ps) launch_sum_plane(st, c->Vvovv_p, c->Vvovv_ps, ov * vv);
         launch_sum_plane(st, c->Voovv_p, c->Voovv_ps, oo * vv);
-        launch_sum_plane(st, c->G1, c->G1s, ov * ov);
+        if (c->G1s) launch_sum_plane(st, c->G1, c->G1s, ov * ov);
     }
     if (c->opt.cc2) {   // BvvT[a][l][e] = B[l][a][e], BovT[k][l][d] = B[l][k][d]: K-contiguous operands of cc2_dressed_factors
         const int64_t dv[4] = {v, v, Lp, 1}, dk[4] = {o, v, Lp, 1};
@@ -1042,7 +1060,7 @@ static int build_Hvovo(ccsd_ctx* c)
     }
     CCSD_TRY(run_gemm(env, with_planes(gp(rows, ov, ov, c->Xm + off, ov, c->G1, ov, c->Hm + off, ov, 1, 1.0, 1),
                                        c->Xms ? c->Xms + off : nullptr, c->G1s)));
-    if (c->planes) launch_sum_plane(c->st, c->Hm + off, c->Hms + off, rows * ov);   // operand of the ring GEMM
+    if (c->Hms) launch_sum_plane(c->st, c->Hm + off, c->Hms + off, rows * ov);   // operand of the ring GEMM
     return CCSD_OK;
 }
 
@@ -1218,7 +1236,8 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
     }
     const int64_t rows = c->sh.w_hi - c->sh.w_lo;      // this rank's rows of <ab||cd> (all of them for world = 1)
     if (c->strassen && c->sW.S)      // both operand stacks are ready (ccsd_init, prep_operands): one batched launch + the result sums
-        return strassen_gemm(c->env, gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), &c->sW, &c->sTau, c->str_L);
+        return strassen_gemm(c->env, gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), &c->sW,
+                             c->strassen_levels_L == 2 ? &c->sTauC : &c->sTau, c->str_L, c->strassen_levels_L);
     return run_gemm(c->env, with_planes(gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S + c->sh.w_lo, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
 static void fill_AG_hh(ccsd_ctx* c)
@@ -1814,8 +1833,8 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     cudaMemsetAsync(c->AG, 0, (size_t)(c->oo * 2 * c->oop) * sizeof(c128), c->st);
     int s = build_constants(c, reinterpret_cast<const c128*>(h), reinterpret_cast<const c128*>(B));
     if (s == CCSD_OK && c->strassen) {   // operand stacks of the constants (strassen.cuh), once
-        if (c->sW.S) launch_strassen_prep(c->st, 0, c->W, c->vv, c->sW);
-        if (c->sVvovv.S) launch_strassen_prep(c->st, 0, c->Vvovv_p, c->vv, c->sVvovv);
+        if (c->sW.S) launch_strassen_prep(c->st, 0, c->W ? c->W : c->W_init, c->vv, c->sW);
+        if (c->sVvovv.S) launch_strassen_prep(c->st, 0, c->Vvovv_p, c->vv, c->sVvovv);     // overwrites W_init: after the line above
         launch_strassen_prep(c->st, 1, c->G1, c->ov, c->sG1);
     }
     if (s == CCSD_OK) mp2_guess(c);
@@ -2011,8 +2030,13 @@ int ccsd_get_tensor(ccsd_ctx* c, int id, ccsd_c128* out_)
     switch (id) {
     case CCSD_T_FOCK: dcopy(st, out, c->f, (int64_t)c->n * c->n); break;
     case CCSD_T_VVVV:
-        if (!c->W || c->sh.world > 1) return CCSD_EINVAL;   // direct_ladder: not stored; sharded: this rank's rows only
-        dcopy(st, out, c->W, vv * vv);
+        if (c->sh.world > 1 || (!c->W && !(c->W_dropped && c->sW.S))) return CCSD_EINVAL;   // direct_ladder: not stored; sharded: this rank's rows only
+        if (c->W) {
+            dcopy(st, out, c->W, vv * vv);
+        } else {      // kept as the ladder's operand stack only
+            const StrassenView wv = strassen_view(c->sW);
+            launch_fill(st, out, vv, vv, vv, 0, [=] __device__(int64_t AB, int64_t CD) { return strassen_left_at(wv, AB, CD); });
+        }
         break;
     case CCSD_T_VOVV: dcopy(st, out, c->Vvovv_p, ov * vv); break;
     case CCSD_T_VOVO: {
@@ -2693,7 +2717,7 @@ int ccsd_strassen_info(ccsd_ctx* c, int info[4])
     if (!c || !info) return CCSD_ESTATE;
     info[0] = c->strassen ? 1 : 0;
     info[1] = c->strassen ? c->strassen_levels : 0;      // the two (ov)^3 products: levels
-    info[2] = (c->strassen && c->sW.S) ? 1 : 0;          // pp-ladder
+    info[2] = (c->strassen && c->sW.S) ? c->strassen_levels_L : 0;      // pp-ladder
     info[3] = (c->strassen && c->sVvovv.S) ? c->strassen_levels_C : 0;      // <bk||cd> tau part of C
     return CCSD_OK;
 }

@@ -272,13 +272,16 @@ static int lambda_build_hbar(ccsd_ctx* c, LambdaState* L)
     //   (i) sum_f <ab||ef> t^f_i from the packed <ab||cd>: rows (a<b) in slabs, unpacked in (e,f), times t1
     {
         const c128* W = c->W;
+        const StrassenView wv = strassen_view(c->sW);      // where <ab||cd> is kept as the ladder's operand stack only (c->W null)
         const int64_t slab_rows = (sc.elems / (V * V)) > 0 ? (sc.elems / (V * V)) : 1;
         for (int64_t r0 = 0; r0 < vv; r0 += slab_rows) {
             const int64_t nr = (vv - r0 < slab_rows) ? vv - r0 : slab_rows;
             launch_fill(st, sc.a, nr * V, V, V, 0, [=] __device__(int64_t row, int64_t ff) {
                 const int64_t AB = r0 + row / v;
                 const int e = (int)(row % v);
-                return asym_col(W, AB, vv, e, (int)ff, v);
+                if (W) return asym_col(W, AB, vv, e, (int)ff, v);
+                if (e == (int)ff) return mk(0.0, 0.0);
+                return e < (int)ff ? strassen_left_at(wv, AB, pair_idx(e, (int)ff, v)) : cneg(strassen_left_at(wv, AB, pair_idx((int)ff, e, v)));
             });
             // Ypk[(a<b)][e][i] = sum_f U[(ab),e][f] t1[i][f]
             CCSD_TRY(run_gemm(env, gp(nr * V, O, V, sc.a, V, T1, V, L->Ypk + r0 * V * O, O, 1, 1.0, 0)));
@@ -461,13 +464,15 @@ static int lambda_residual(ccsd_ctx* c, LambdaState* L)
             if (plane) plane[IJ * vv + EF] = x.x + x.y;
             return x;
         });
-        if (c->strassen && c->sW.S && strassen_stack_elems(oo, vv, 1) <= c->str_ring.b_elems) {
+        const int lvL = c->strassen_levels_L;
+        if (c->strassen && c->sW.S && strassen_stack_elems(oo, vv, lvL) <= c->str_ring.b_elems) {
             // one Strassen level with the stack of <ab||cd> ccsd_init made; conj(lambda) is stacked in the scratch of the (ov)^3
             // products (idle here; tau's own stack stays valid for the CCSD residual's per-term hooks)
-            StrassenStack sl = strassen_stack(c->str_ring.SB, c->str_ring.SBp, oo, vv, 1);
+            StrassenStack sl = strassen_stack(c->str_ring.SB, c->str_ring.SBp, oo, vv, lvL);
             launch_strassen_prep(st, 1, L->cl2p, vv, sl);
-            CCSD_TRY(strassen_gemm(env, gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), &c->sW, &sl, c->str_L));
+            CCSD_TRY(strassen_gemm(env, gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), &c->sW, &sl, c->str_L, lvL));
         } else {
+            if (!c->W) return CCSD_ESTATE;
             CCSD_TRY(run_gemm(env, with_planes(gp(vv, oo, vv, c->W, vv, L->cl2p, vv, L->P2, 1, vv, 1.0, 0), c->Ws, plane)));
         }
     }

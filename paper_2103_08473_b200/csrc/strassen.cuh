@@ -42,6 +42,47 @@ static inline StrassenStack strassen_stack(c128* S, double* Sp, int64_t R, int64
 
 constexpr int STR_THREADS = 256;
 
+// Read access to the operand a LEFT stack was made from: the quadrants are x11 = s[2], x22 = s[3], x12 = s[4] - s[2],
+// x21 = s[5] + s[2] (one subtraction: exact up to one rounding of the larger term); with two levels the same rule is applied to the
+// quadrants of the stacked half-size matrices.  Lets the packed <ab||cd> be dropped once its stack exists: the few readers that
+// want single elements (ccsd_get_tensor, the one-time unpacking in the Lambda set-up) pay up to four loads per element.
+struct StrassenView {
+    const c128* S;
+    int64_t R1, K1, Rq, Kq;   // extents of a half; of a quarter (two levels)
+    int levels;
+};
+static inline StrassenView strassen_view(const StrassenStack& s)
+{
+    StrassenView v;
+    v.S = s.S; v.levels = s.levels;
+    v.R1 = strassen_half(s.R); v.K1 = strassen_khalf(s.K);
+    v.Rq = s.levels == 2 ? s.Rh : 0; v.Kq = s.levels == 2 ? s.Kh : 0;
+    return v;
+}
+// value of quadrant (u, v) from the seven combinations, given a reader of combination q at the position in question
+template <class F>
+__device__ __forceinline__ c128 strassen_left_quadrant(int u, int v, F comb)
+{
+    if (u == 0 && v == 0) return comb(2);
+    if (u == 1 && v == 1) return comb(3);
+    if (u == 0) return csub(comb(4), comb(2));
+    return cadd(comb(5), comb(2));
+}
+__device__ __forceinline__ c128 strassen_left_at(const StrassenView& w, int64_t r, int64_t k)
+{
+    const int u1 = r >= w.R1, v1 = k >= w.K1;
+    const int64_t rr = r - u1 * w.R1, kk = k - v1 * w.K1;
+    if (w.levels == 1) {
+        const int64_t plane = w.R1 * w.K1, at = rr * w.K1 + kk;
+        return strassen_left_quadrant(u1, v1, [&](int q) { return w.S[q * plane + at]; });
+    }
+    const int u2 = rr >= w.Rq, v2 = kk >= w.Kq;
+    const int64_t plane = w.Rq * w.Kq, at = (rr - u2 * w.Rq) * w.Kq + (kk - v2 * w.Kq);
+    return strassen_left_quadrant(u1, v1, [&](int q1) {
+        return strassen_left_quadrant(u2, v2, [&](int q2) { return w.S[(q1 * 7 + q2) * plane + at]; });
+    });
+}
+
 // the seven operand combinations of one side (SIDE 0: left operand A, SIDE 1: right operand B) from its four quadrants
 template <int SIDE>
 __device__ __forceinline__ void strassen_combos(c128 x11, c128 x12, c128 x21, c128 x22, c128 s[7])

@@ -70,8 +70,10 @@ def test_lambda_residual_and_density_match_oracle(gpu, name):
     gc.close()
 
 
-def test_lambda_exact_parity_at_identical_amplitudes(gpu):
-    """Same amplitudes on both sides (the oracle's converged ones are handed to the library): 1e-12."""
+@pytest.mark.parametrize("strassen", [1, 3])
+def test_lambda_exact_parity_at_identical_amplitudes(gpu, strassen):
+    """Same amplitudes on both sides (the oracle's converged ones are handed to the library): 1e-12.  strassen = 3: the Lambda
+    iteration's ladder and (ov)^3 product as 49 quarter-size products, <ab||cd> read back from the ladder's operand stack."""
     from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
     from oracle.lambda_oracle import OracleLambda
     inp = ci.make_inputs(6, 15, 24, seed=4715)
@@ -79,7 +81,7 @@ def test_lambda_exact_parity_at_identical_amplitudes(gpu):
     oc = OracleCCSD(inp.h, inp.B, o, v)
     oc.run(80, tol=1e-13)
     ol = OracleLambda(oc)
-    gc = gpu.CCSD(inp.h, inp.B, o, v)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, strassen=strassen)
     gc.set_amplitudes(oc.t1, pack_t2(oc.t2))
     gc.lambda_init()
     l1, l2p = ci.random_amplitudes(o, v, 45, 0.2)

@@ -103,6 +103,35 @@ def test_every_tensor_matches_oracle(gpu, o, v, L, gemm_mode):
     gc.close()
 
 
+@pytest.mark.parametrize("o,v,L", [(6, 16, 30), (5, 11, 20), (7, 13, 18), (9, 8, 12)])
+def test_every_tensor_matches_oracle_with_strassen_levels_forced(gpu, o, v, L):
+    """ccsd_options.strassen = 3: all four large contractions as 49 quarter-size products at sizes the oracle finishes in seconds
+    (odd halves and quarters: every zero-padding path), the packed <ab||cd> kept as the ladder's operand stack only (the "vvvv"
+    entry below is rebuilt from it), S1 / G_vv / H_oo quartic terms read off the products of C, H^{ak}_{ci} and A.  Every tensor
+    against the oracle, then six iterations in lock step."""
+    from oracle.ccsd_oracle import OracleCCSD, unpack_t2
+    inp = ci.make_inputs(o, v, L, seed=300 + o + v, b_scale=0.1, f_offdiag=0.05)
+    oc = OracleCCSD(inp.h, inp.B, o, v)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, strassen=3)
+    assert gc.strassen_steps() == {"Hvovo_quad": 2, "ring_gemm": 2, "pp_ladder": 2, "C_ovoo": 2}
+    oc.residual()
+    gc.residual()
+    compare_all(oc, gc)
+    t1, t2p = ci.random_amplitudes(o, v, 5, 0.2)
+    oc.set_amplitudes(t1, unpack_t2(t2p, o, v))
+    gc.set_amplitudes(t1, t2p)
+    oc.residual()
+    gc.residual()
+    compare_all(oc, gc)
+    assert abs(gc.energy() - oc.energy()) < 1e-12 * max(1.0, abs(oc.energy()))
+    for it in range(6):
+        eo, so = oc.iterate()
+        eg, sg = gc.iterate()
+        assert abs(eg - eo) < 1e-12 * max(1.0, abs(eo)), (it, eg, eo)
+        assert abs(sg - so) < 1e-11 * max(1.0, so), (it, sg, so)
+    gc.close()
+
+
 @pytest.mark.parametrize("cfg,niter", [("cfg0_2e", 8), ("cfg0", 10)])
 def test_lockstep_energies_tiny_configs(gpu, cfg, niter):
     from oracle.ccsd_oracle import OracleCCSD

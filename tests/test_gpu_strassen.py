@@ -79,7 +79,8 @@ def test_strassen_gemm_equals_the_plain_dmma_gemm_at_a_ladder_like_shape(gpu):
 @pytest.mark.parametrize("mode", [1, 2, 3])
 def test_context_with_strassen_equals_context_without(gpu, mode):
     """cfg1 (16/96/336): ov = 1536, vv = 4560 -- the scheme is used for the two (ov)^3 products and the pp-ladder.  mode 1: the
-    default choice of levels (one, at this size), 2: one level forced, 3: two levels forced on the (ov)^3 products."""
+    default choice of levels (one, at this size), 2: one level, 3: two levels forced on all four products (the packed <ab||cd> is
+    then kept as the ladder's operand stack only)."""
     o, v, naux = 16, 96, 336
     inp = ci.make_inputs(o, v, naux, 2021030801)
     fast = gpu.CCSD(inp.h, inp.B, o, v, strassen=mode)
@@ -98,6 +99,8 @@ def test_context_with_strassen_equals_context_without(gpu, mode):
     for name in ["S1", "S2"]:
         a, b = fast.get_tensor(name).cpu().numpy(), plain.get_tensor(name).cpu().numpy()
         assert np.abs(a - b).max() < REL_TOL * max(term_scale, np.abs(b).max()), name
+    a, b = fast.get_tensor("vvvv").cpu().numpy(), plain.get_tensor("vvvv").cpu().numpy()
+    assert _rel(a, b) < 4e-16                  # stored tensor / rebuilt from the ladder's operand stack: one rounding at most
     for it in range(4):
         ef, nf = fast.iterate()
         ep, npl = plain.iterate()
