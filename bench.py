@@ -841,11 +841,16 @@ def run_ours(args) -> None:
             # the form ccsd_iterate runs: one Strassen level.  This standalone call also stacks <ab||cd> (done once, by ccsd_init,
             # inside the solver), so ms_per_call is NOT the launch time; the batched gemm_dmma_kernel launch inside it is the
             # launch of the iteration (same kernel, same grid) -- this leg exists to capture that launch with ncu.
-            ts = time_events(torch, lambda: pkg.zgemm_nt_strassen(W, tau, C=R, transposed_out=True), args.steps, args.warmup)
+            # levels as ccsd_init chooses them for this shape (ccsd_lib.cu carve): two where ov >= 3072 and a quarter of oo >= 128
+            levels = 2 if (o * v >= 3072 and (((oo + 1) // 2) + 1) // 2 >= 128) else 1
+            if args.strassen in (2, 3):
+                levels = args.strassen - 1
+            ts = time_events(torch, lambda: pkg.zgemm_nt_strassen(W, tau, C=R, transposed_out=True, levels=levels),
+                             args.steps, args.warmup)
             t = statistics.median(ts)
-            print(json.dumps({"metric": "pp_ladder_strassen_call_ms", "value": t, "unit": "ms", "ms_per_call": t,
-                              "config": {"workload": f"{cfg} pp-ladder {vv}x{oo}x{vv}, one Strassen level, both operand stacks made "
-                                                     "inside the call"}}))
+            print(json.dumps({"metric": "pp_ladder_strassen_call_ms", "value": t, "unit": "ms", "ms_per_call": t, "levels": levels,
+                              "config": {"workload": f"{cfg} pp-ladder {vv}x{oo}x{vv}, {levels} Strassen level(s), both operand stacks "
+                                                     "made inside the call"}}))
             return
         Ws, taus = pkg.sum_plane(W), pkg.sum_plane(tau)
         ts = time_events(torch, lambda: pkg.contract("pp_ladder_planes", o, v, [tau, W, taus, Ws], out=R),
