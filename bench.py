@@ -34,8 +34,10 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 FMA/clk x 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pp-ladder launch of the 3M + sum-plane DMMA GEMM at cfg3, from
 # profiles/r02_ncu_pp_ladder_cfg3.md (ncu --set full).  None until captured for the workload.
 NCU_TRAFFIC_BYTES = {"cfg3": 23.10e9 + 0.220e9}
-# ... and of the batched seven-product launch the pp-ladder is with one Strassen level (profiles/r02b_ncu_pp_ladder_strassen_cfg3.md)
-NCU_TRAFFIC_BYTES_STRASSEN = {"cfg3": 30.472e9 + 0.389e9}
+# ... and of the batched launch the pp-ladder is with its Strassen levels: {levels: {workload: bytes}}
+# (profiles/r02b_ncu_pp_ladder_strassen_cfg3.md: one level, 7 products; profiles/r02c_ncu_pp_ladder_strassen_cfg3.md: two levels, 49)
+NCU_TRAFFIC_BYTES_STRASSEN = {1: {"cfg3": 30.472e9 + 0.389e9}, 2: {"cfg3": 49.517e9 + 0.687e9}}
+NCU_TRAFFIC_FILE_STRASSEN = {1: "r02b_ncu_pp_ladder_strassen_cfg3.md", 2: "r02c_ncu_pp_ladder_strassen_cfg3.md"}
 NCU_TRAFFIC_SOURCE = ("recorded constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of one "
                       "pp-ladder launch from the ncu --set full capture summarised in profiles/r02_ncu_pp_ladder_cfg3.md")
 
@@ -606,18 +608,26 @@ def lambda_bench(torch, pkg, inp, o, v, steps=3, warmup=1):
                     "<ab||cd> with conjugated multipliers"}
 
 
-def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, strassen: bool = False, c_levels: int = 1) -> dict:
+def hbm_step_bytes(o: int, v: int, m: int, planes: bool = True, levels: dict | None = None) -> dict:
     """Algorithmic bytes of the HBM-bound steps of one iteration (16 B read + 16 B written per element a
-    permutation moves; the update streams (2 + 2m) vectors at the least; m = pairs in the DIIS subspace)."""
+    permutation moves; the update streams (2 + 2m) vectors at the least; m = pairs in the DIIS subspace).  levels: the solver's
+    strassen_steps() (None / {}: plain products)."""
     oo, vv, ov = o * (o - 1) // 2, v * (v - 1) // 2, o * v
     nvec = ov + oo * vv
-    moved = ov + oo * vv + 2 * ov * ov + v * oo * v + o * o * vv + oo * v * v      # t1T, tau^T, Xm, T2r, tauc, tauou, t2hu
-    # with the Strassen level the planes of Xm, T2r are not written (their stacks carry planes); the stack of tau is: tau read
-    # once, seven half-size matrices (16 B) and their planes (8 B) written
-    tau_stack = oo * vv * 16 + 7 * ((oo + 1) // 2) * ((vv + 1) // 2) * 24
-    if c_levels == 2:       # C takes two levels: tau is stacked a second time, as 49 quarter-size matrices
-        tau_stack += oo * vv * 16 + 49 * ((oo + 3) // 4) * ((vv + 3) // 4) * 24
-    return {"prep_permute": moved * 32 + ((tau_stack if strassen else 2 * ov * ov * 8) if planes else 0),
+    levels = levels or {}
+    moved = ov + oo * vv + 2 * ov * ov + v * oo * v + oo * v * v      # t1T, tau^T, Xm, T2r, tauc, t2hu
+    extra = 0
+    if planes:
+        if "ring_gemm" not in levels:
+            extra += 2 * ov * ov * 8                                  # planes of Xm, T2r (Strassen stacks carry their own)
+        # Strassen stacks of tau for the ladder and C: tau read once per stack, 7 half-size / 49 quarter-size matrices (16 B) and
+        # their planes (8 B) written
+        used = {levels.get("pp_ladder", 0), levels.get("C_ovoo", 0)}
+        if 1 in used:
+            extra += oo * vv * 16 + 7 * ((oo + 1) // 2) * ((vv + 1) // 2) * 24
+        if 2 in used:
+            extra += oo * vv * 16 + 49 * ((oo + 3) // 4) * ((vv + 3) // 4) * 24
+    return {"prep_permute": moved * 32 + extra,
             # Jacobi + Gram row in one pass (S, t and m-1 stored e read; e, u written), then sum_l c_l u_l (m read, 1 written)
             "update_diis": (2 * m + 4) * nvec * 16,
             "update_diis_floor": (2 * m + 2) * nvec * 16,
@@ -697,7 +707,7 @@ def iteration_bench(torch, pkg, cfg, inp, steps, warmup, peak, hbm_gbs, barrier=
                 ent["strassen_levels"] = strassen_steps[k]
         terms[k] = ent
     for k in ("prep_permute", "update_diis", "energy"):       # HBM-bound steps: algorithmic bytes / time
-        gbs = [hbm_step_bytes(o, v, m, strassen="pp_ladder" in strassen_steps, c_levels=strassen_steps.get("C_ovoo", 1))[k] / (x * 1e-3) * 1e-9
+        gbs = [hbm_step_bytes(o, v, m, levels=strassen_steps)[k] / (x * 1e-3) * 1e-9
                for x, m in zip(step_acc[k], m_hist) if x > 0]
         if gbs:
             terms[k]["gbs"] = round(statistics.median(gbs), 1)
@@ -916,8 +926,10 @@ def run_ours(args) -> None:
     pp_exec = pp_tflops * ex_pp
     gemm_steps = ("pp_ladder", "Hvovo_quad", "ring_gemm")
     gemm_ms = sum(main["terms"][k]["ms"] for k in gemm_steps)
-    traffic = (NCU_TRAFFIC_BYTES_STRASSEN if pp_strassen else NCU_TRAFFIC_BYTES).get(cfg)
-    traffic_source = NCU_TRAFFIC_SOURCE.replace("r02_ncu_pp_ladder_cfg3.md", "r02b_ncu_pp_ladder_strassen_cfg3.md") if pp_strassen else NCU_TRAFFIC_SOURCE
+    pp_levels = main["strassen_steps"].get("pp_ladder", 0)
+    traffic = (NCU_TRAFFIC_BYTES_STRASSEN.get(pp_levels, {}) if pp_strassen else NCU_TRAFFIC_BYTES).get(cfg)
+    traffic_source = (NCU_TRAFFIC_SOURCE.replace("r02_ncu_pp_ladder_cfg3.md", NCU_TRAFFIC_FILE_STRASSEN.get(pp_levels, "?"))
+                      if pp_strassen else NCU_TRAFFIC_SOURCE)
     roofline = {"bound": "tensor", "kernel": "gemm_dmma_kernel<DmmaCfg<4,2,4,3,3M,planes>> (FP64 DMMA.8x8x4), pp-ladder launch" +
                           (": ONE batched launch of the 7 half-size / 49 quarter-size products of its Strassen level(s)" if pp_strassen else ""),
                 "achieved": round(pp_exec, 3), "peak": round(peak, 3), "unit": "TFLOP/s",
