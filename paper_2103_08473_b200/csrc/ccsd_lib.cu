@@ -334,7 +334,7 @@ struct Carver {
     }
 };
 
-static void carve(ccsd_ctx* c, char* base, size_t* total)
+static void carve(ccsd_ctx* c, char* base, size_t* total, int degrade)
 {
     Carver w{base, 0};
     const int64_t o = c->o, v = c->v, n = c->n, Lp = c->Lp, oo = c->oo, vv = c->vv, ov = c->ov, oop = c->oop;
@@ -344,8 +344,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     const bool force = c->opt.strassen == 3;
     c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 &&
                   (force ? (o >= 2 && v >= 2) : strassen_worthwhile(ov, ov, ov));
-    const bool use_L = c->strassen && !c->opt.direct_ladder && (force || strassen_worthwhile(vv, oo, vv));
-    const bool use_C = c->strassen && (force || strassen_worthwhile(ov, oo, vv));
+    bool use_L = c->strassen && !c->opt.direct_ladder && (force || strassen_worthwhile(vv, oo, vv));
+    bool use_C = c->strassen && (force || strassen_worthwhile(ov, oo, vv));
     // two levels on the (ov)^3 products where a quarter-size product is still a long-K, many-tile GEMM (measured: 0.80 of the
     // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
     c->strassen_levels = force ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
@@ -353,6 +353,16 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     // 144; cfg2: 69 -> 96 does not)
     c->strassen_levels_C = force ? 2 : ((c->strassen_levels == 2 && strassen_half(strassen_half(oo)) >= 128) ? 2 : 1);
     c->strassen_levels_L = force ? 2 : ((c->strassen_levels_C == 2 && use_C && use_L) ? 2 : 1);
+    // The operand stacks of the constants grow like v^4 (the two-level stack of <ab||cd> is 3 x the tensor with planes).  `degrade`
+    // gives up levels one step at a time -- the ladder's first, then C's, then the (ov)^3 products' -- see carve_auto.
+    for (int k = 0; k < degrade && c->strassen && !force; k++) {
+        if (use_L && c->strassen_levels_L == 2) c->strassen_levels_L = 1;
+        else if (use_L) use_L = false;
+        else if (use_C && c->strassen_levels_C == 2) c->strassen_levels_C = 1;
+        else if (use_C) use_C = false;
+        else if (c->strassen_levels == 2) c->strassen_levels = 1;
+        else c->strassen = false;
+    }
     c->po = w.take<int2>(oo);
     c->pv = w.take<int2>(vv);
     c->eps = w.take<double>(n);
@@ -544,6 +554,20 @@ static void carve(ccsd_ctx* c, char* base, size_t* total)
     c->diis.scratch = w.take<double>(RED_SCRATCH_DOUBLES);
     c->red = w.take<double>(64);
     *total = w.off;
+}
+
+// Workspace layout with as many Strassen levels as fit: a workspace beyond 128 GiB (of a 180 GB part; the Lambda and triples
+// workspaces need room beside it) gives levels up step by step, down to plain products, instead of asking for memory no GPU has
+// (cfg3: 107 GiB with everything; plain products need 60 GiB).  Host arithmetic only: ccsd_workspace_bytes and ccsd_init agree.
+static void carve_auto(ccsd_ctx* c, char* base, size_t* total)
+{
+    int degrade = 0;
+    for (; degrade < 6; degrade++) {
+        size_t t = 0;
+        carve(c, nullptr, &t, degrade);
+        if (t <= ((size_t)128 << 30) || !c->strassen || c->opt.strassen == 3) break;
+    }
+    carve(c, base, total, degrade);
 }
 
 static int check_sizes(int nocc, int nvir, int naux)
@@ -1790,7 +1814,7 @@ int ccsd_workspace_bytes(int nocc, int nvir, int naux, const ccsd_options* opts,
     CCSD_TRY(check_sizes(nocc, nvir, naux));
     ccsd_ctx tmp;
     setup_dims(&tmp, nocc, nvir, naux, opts);
-    carve(&tmp, nullptr, bytes);
+    carve_auto(&tmp, nullptr, bytes);
     return CCSD_OK;
 }
 
@@ -1814,9 +1838,9 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     c->ws_base = static_cast<char*>(workspace);
     setup_dims(c, nocc, nvir, naux, opts);
     size_t need = 0;
-    carve(c, nullptr, &need);
+    carve_auto(c, nullptr, &need);
     if (workspace_bytes < need) { delete c; return CCSD_EINVAL; }
-    carve(c, static_cast<char*>(workspace), &need);
+    carve_auto(c, static_cast<char*>(workspace), &need);
     c->st = static_cast<cudaStream_t>(cuda_stream);
     c->env = Env{c->st, c->opt.gemm_mode, c->partial, c->partial_elems};
     c->timing = 0;
