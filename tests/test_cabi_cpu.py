@@ -69,6 +69,32 @@ def test_workspace_bytes_scales_and_validates(lib):
     assert lib.ccsd_contract_workspace_bytes(15, 4, 16, ctypes.byref(n)) == 1
 
 
+def test_strassen_entry_points_validate_on_the_host(lib):
+    """ccsd_zgemm_nt_strassen*: size arithmetic and argument checks need no GPU."""
+    n = ctypes.c_size_t(0)
+    M, N, K = 1031, 97, 1033
+    assert lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, 1, ctypes.byref(n)) == 0
+    one = n.value
+    mh, nh, kh = (M + 1) // 2, (N + 1) // 2, ((K + 1) // 2 + 1) // 2 * 2
+    # two operand stacks (16 B + 8 B plane per element) and seven products, each buffer rounded up to 256 bytes
+    assert 7 * (mh * kh + nh * kh) * 24 + 7 * mh * nh * 16 <= one <= 7 * (mh * kh + nh * kh) * 24 + 7 * mh * nh * 16 + 5 * 256
+    assert lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, 2, ctypes.byref(n)) == 0
+    assert n.value > one                                                       # 49 quarter-size matrices: 49/16 vs 7/4 of the operand
+    for bad in ((0, N, K, 1), (M, 0, K, 1), (M, N, 0, 1), (M, N, K, 0), (M, N, K, 3)):
+        assert lib.ccsd_zgemm_nt_strassen_workspace_bytes(*bad, ctypes.byref(n)) == 1
+    assert lib.ccsd_zgemm_nt_strassen_workspace_bytes(M, N, K, 1, None) == 1
+    buf = ctypes.create_string_buffer(512)
+    p = (ctypes.addressof(buf) + 255) // 256 * 256
+    call = lambda m, nn, k, a, b, c, lda, ldb, lv, ws, wsb: lib.ccsd_zgemm_nt_strassen(  # noqa: E731
+        m, nn, k, a, lda, b, ldb, c, N, 1, 1.0, 0.0, 0, 0, lv, ws, wsb, None)
+    assert call(M, N, K, None, p, p, K, K, 1, p, one) == 1                     # null operand
+    assert call(M, N, K, p, p, p, K - 1, K, 1, p, one) == 1                    # rows overlap
+    assert call(M, N, K, p, p, p, K, K, 3, p, one) == 1                        # levels
+    assert call(M, N, K, p, p, p, K, K, 1, p, one - 1) == 1                    # workspace too small
+    assert call(M, N, K, p, p, p, K, K, 1, p + 8, one) == 1                    # workspace misaligned
+    assert lib.ccsd_strassen_info(None, None) == 4                             # CCSD_ESTATE
+
+
 def test_null_handles_are_rejected(lib):
     assert lib.ccsd_iterate(None, None, None, None) == 4     # CCSD_ESTATE
     assert lib.ccsd_energy(None, None, None) == 4
@@ -88,6 +114,10 @@ def test_no_cpu_fallback(lib):
     ws = ctypes.c_void_p(256 * 1024)
     assert lib.ccsd_init(ctypes.byref(ctx), p, p, 2, 2, 1, None, ws, 1 << 40, None) == 3
     assert not ctx.value
+    n = ctypes.c_size_t(0)
+    assert lib.ccsd_zgemm_nt_strassen_workspace_bytes(2, 2, 2, 1, ctypes.byref(n)) == 0
+    assert lib.ccsd_zgemm_nt_strassen(2, 2, 2, p, 2, p, 2, p, 2, 1, 1.0, 0.0, 0, 0, 1, ws, n.value, None) == 3
+    assert lib.ccsd_energy_static(2, 2, p, p, p, p, p, None) == 3
     import paper_2103_08473_b200 as pkg
     with pytest.raises(RuntimeError):
         pkg.zgemm_nt([[1.0]], [[1.0]])
