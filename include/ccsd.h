@@ -69,7 +69,7 @@ typedef struct {
                            afterwards; 0 = always launch directly.  Capture needs a stream created by the caller: on the
                            legacy / per-thread default streams (cuda_stream = 0, 1 or 2), and while step timing is enabled,
                            the launches are issued directly whatever this says.  In the graph the independent parts of the
-                           residual (H^{ak}_{ci} + ring product; Fock-like terms + S1; C; A; driver + pp-ladder) are parallel
+                           residual (H^{ak}_{ci} + ring product; A + Fock-like terms + S1; C; V^dagger t1; driver + pp-ladder) are parallel
                            branches, so that the small products fill the partial waves of the large ones; 3 = a graph with the
                            launches in their serial order.  Results are bit-identical in all cases */
     int shard_rank;     /* slab sharding of the iteration over several GPUs (one process and one context per GPU, */
