@@ -59,6 +59,34 @@ def test_strassen_gemm_equals_the_definition(gpu, M, N, K, transposed_out, level
     assert _rel(got.T if transposed_out else got, ref) < REL_TOL
 
 
+@pytest.mark.parametrize("M,N,K,transposed_out", [(3840, 3840, 3840, False), (12720, 276, 12720, True)])
+def test_strassen_error_against_extended_precision_sums(gpu, M, N, K, transposed_out):
+    """The error claim of DESIGN.md "Strassen levels" at sizes where the levels are used (cfg2's (ov)^3 and ladder shapes): sampled
+    elements against 80-bit sums formed on the host.  Plain 3M product and one / two levels all stay below 5e-14 of the largest
+    element of C -- a factor 20 inside the 1e-12 parity bound -- and the levels lose at most a factor 4 on the plain product."""
+    import torch
+    g = torch.Generator(device="cuda"); g.manual_seed(M + N)
+    A = torch.view_as_complex(torch.randn(M, K, 2, dtype=torch.float64, device="cuda", generator=g))
+    B = torch.view_as_complex(torch.randn(N, K, 2, dtype=torch.float64, device="cuda", generator=g))
+    rng = np.random.default_rng(3)
+    ms, ns = rng.integers(0, M, 96), rng.integers(0, N, 96)
+    Ah, Bh = A[torch.from_numpy(ms).cuda()].cpu().numpy(), B[torch.from_numpy(ns).cuda()].cpu().numpy()
+    ar, ai, br, bi = [x.astype(np.longdouble) for x in (Ah.real, Ah.imag, Bh.real, Bh.imag)]
+    ex_re, ex_im = (ar * br - ai * bi).sum(1), (ar * bi + ai * br).sum(1)
+
+    def err(C):
+        Cf = C.t() if transposed_out else C
+        x = Cf[torch.from_numpy(ms).cuda(), torch.from_numpy(ns).cuda()].cpu().numpy()
+        scale = float(C.abs().max())
+        return float(max(np.abs(x.real - ex_re).max(), np.abs(x.imag - ex_im).max())) / scale
+
+    e0 = err(gpu.zgemm_nt(A, B, transposed_out=transposed_out))
+    e1 = err(gpu.zgemm_nt_strassen(A, B, transposed_out=transposed_out, levels=1))
+    e2 = err(gpu.zgemm_nt_strassen(A, B, transposed_out=transposed_out, levels=2))
+    assert e0 < 5e-14 and e1 < 5e-14 and e2 < 5e-14, (e0, e1, e2)
+    assert e1 < 4 * e0 + 1e-15 and e2 < 4 * e0 + 1e-15, (e0, e1, e2)
+
+
 def test_strassen_gemm_equals_the_plain_dmma_gemm_at_a_ladder_like_shape(gpu):
     """(a<b) x (i<j) x (c<d) with an odd N, output transposed as the pp-ladder writes it; sampled rows against numpy."""
     import torch
