@@ -161,11 +161,12 @@ def test_lockstep_no_diis_and_level_shift(gpu):
     gc.close()
 
 
-def test_ccd_mode_keeps_t1_zero(gpu):
+@pytest.mark.parametrize("strassen", [1, 3])
+def test_ccd_mode_keeps_t1_zero(gpu, strassen):
     """CCD (PAPER.md:1044 .CCDOUBLES): t1 = 0 throughout; plain Jacobi on both sides."""
     from oracle.ccsd_oracle import OracleCCSD
     inp = ci.make_inputs(4, 10, 24, seed=78, b_scale=0.08, f_offdiag=0.03)
-    gc = gpu.CCSD(inp.h, inp.B, 4, 10, ccd=True, ndiis=0)
+    gc = gpu.CCSD(inp.h, inp.B, 4, 10, ccd=True, ndiis=0, strassen=strassen)
     oc = OracleCCSD(inp.h, inp.B, 4, 10, ndiis=0)
     oc.set_amplitudes(np.zeros_like(oc.t1), oc.t2)
     for it in range(4):
@@ -355,10 +356,11 @@ def test_direct_ladder_matches_oracle(gpu, o, v, L):
     gc.close()
 
 
-def test_two_contexts_on_two_streams_concurrently(gpu):
+@pytest.mark.parametrize("strassen", [1, 3])
+def test_two_contexts_on_two_streams_concurrently(gpu, strassen):
     """The C ABI takes a stream per context: two contexts iterating at the same time on two streams (from two host threads)
-    share no scratch -- reduction partials, Gram matrix and DIIS coefficients are carved from each context's workspace --
-    and both reproduce the oracle's lock-step energies."""
+    share no scratch -- reduction partials, Gram matrix and DIIS coefficients (strassen = 3: the Strassen operand stacks and
+    products too) are carved from each context's workspace -- and both reproduce the oracle's lock-step energies."""
     import threading
     import torch
     from oracle.ccsd_oracle import OracleCCSD
@@ -368,7 +370,7 @@ def test_two_contexts_on_two_streams_concurrently(gpu):
         oc = OracleCCSD(inp.h, inp.B, inp.nocc, inp.nvir)
         refs.append([oc.iterate() for _ in range(12)])
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
-    solvers = [gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=st) for inp, st in zip(cases, streams)]
+    solvers = [gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=st, strassen=strassen) for inp, st in zip(cases, streams)]
     assert solvers[0].stream.cuda_stream != solvers[1].stream.cuda_stream
     out = [[], []]
 
@@ -381,7 +383,7 @@ def test_two_contexts_on_two_streams_concurrently(gpu):
         out[0].clear(); out[1].clear()
         for k, inp in enumerate(cases):
             solvers[k].close()
-            solvers[k] = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=streams[k])
+            solvers[k] = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, stream=streams[k], strassen=strassen)
         threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
         for t in threads:
             t.start()
@@ -394,14 +396,16 @@ def test_two_contexts_on_two_streams_concurrently(gpu):
         s_.close()
 
 
-def test_graph_replay_equals_direct_launches_and_stale_tensors_are_refused(gpu):
+@pytest.mark.parametrize("strassen", [1, 3])
+def test_graph_replay_equals_direct_launches_and_stale_tensors_are_refused(gpu, strassen):
     """opts.graph: the residual replayed as a CUDA graph gives bit-identical iterates to direct launches (same kernels, same
-    order); after ccsd_iterate the intermediates of the residual no longer belong to the current amplitudes, so
-    ccsd_get_tensor refuses them (CCSD_ESTATE) until the next ccsd_residual."""
+    data flow; strassen = 3: with two Strassen levels forced on the four large products); after ccsd_iterate the intermediates
+    of the residual no longer belong to the current amplitudes, so ccsd_get_tensor refuses them (CCSD_ESTATE) until the next
+    ccsd_residual."""
     from paper_2103_08473_b200.binding import CCSDError
     inp = ci.make_inputs(7, 30, 50, seed=4103, b_scale=0.05)
-    a = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=True)
-    b = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=False)
+    a = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=True, strassen=strassen)
+    b = gpu.CCSD(inp.h, inp.B, inp.nocc, inp.nvir, graph=False, strassen=strassen)
     n0 = gpu.launch_count()
     for it in range(8):
         ea, eb = a.iterate(), b.iterate()
