@@ -173,7 +173,8 @@ int ccsd_set_amplitudes(ccsd_ctx* ctx, const ccsd_c128* t1, const ccsd_c128* t2p
 /* Tensor ids for ccsd_get_tensor; canonical layouts as listed at the top.  S2_* are the eight terms of eq 32. */
 enum {
     CCSD_T_FOCK = 0,   /* [n][n] */
-    CCSD_T_VVVV = 1,   /* [(a<b)][(c<d)]; CCSD_EINVAL in cc2 and direct_ladder mode, where it is not stored */
+    CCSD_T_VVVV = 1,   /* [(a<b)][(c<d)]; CCSD_EINVAL in cc2 and direct_ladder mode, where it is not stored; where the ladder runs
+                          through its Strassen operand stack (ccsd_options.strassen) it is rebuilt from that stack */
     CCSD_T_VOVV = 2,   /* [a][k][(c<d)] */
     CCSD_T_VOVO = 3,   /* [a][k][c][i] */
     CCSD_T_OOVV = 4,   /* [(k<l)][(c<d)] */
