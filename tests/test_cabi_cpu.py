@@ -69,6 +69,26 @@ def test_workspace_bytes_scales_and_validates(lib):
     assert lib.ccsd_contract_workspace_bytes(15, 4, 16, ctypes.byref(n)) == 1
 
 
+def test_strassen_levels_are_given_up_where_the_workspace_would_not_fit(lib):
+    """ccsd_options.strassen = 1 keeps the workspace within 128 GiB by giving levels up (down to plain products), so that a large
+    virtual space never asks for more than plain products + what fits (include/ccsd.h)."""
+    from paper_2103_08473_b200.binding import _options
+    n = ctypes.c_size_t(0)
+    limit = 128 * 2 ** 30
+    seen_partial = False
+    for shape in ((34, 224, 774), (40, 256, 900), (40, 320, 1080), (20, 364, 1000), (60, 300, 1080)):
+        sizes = []
+        for mode in (0, 1):
+            o = _options(strassen=mode)
+            assert lib.ccsd_workspace_bytes(*shape, ctypes.byref(o), ctypes.byref(n)) == 0
+            sizes.append(n.value)
+        plain, auto = sizes
+        assert auto >= plain                                   # levels only ever add operand stacks
+        assert auto <= max(limit, plain), (shape, plain, auto)  # and never push the workspace beyond the limit
+        seen_partial |= plain < auto < limit and shape != (34, 224, 774)
+    assert seen_partial                                        # (40, 256, 900): some levels kept, some given up
+
+
 def test_strassen_entry_points_validate_on_the_host(lib):
     """ccsd_zgemm_nt_strassen*: size arithmetic and argument checks need no GPU."""
     n = ctypes.c_size_t(0)
