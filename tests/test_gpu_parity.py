@@ -103,8 +103,8 @@ def test_every_tensor_matches_oracle(gpu, o, v, L, gemm_mode):
     gc.close()
 
 
-@pytest.mark.parametrize("o,v,L", [(6, 16, 30), (5, 11, 20), (7, 13, 18), (9, 8, 12)])
-def test_every_tensor_matches_oracle_with_strassen_levels_forced(gpu, o, v, L):
+@pytest.mark.parametrize("o,v,L,gemm_mode", [(6, 16, 30, 0), (5, 11, 20, 0), (7, 13, 18, 0), (9, 8, 12, 0), (6, 16, 30, 3)])
+def test_every_tensor_matches_oracle_with_strassen_levels_forced(gpu, o, v, L, gemm_mode):
     """ccsd_options.strassen = 3: all four large contractions as 49 quarter-size products at sizes the oracle finishes in seconds
     (odd halves and quarters: every zero-padding path), the packed <ab||cd> kept as the ladder's operand stack only (the "vvvv"
     entry below is rebuilt from it), S1 / G_vv / H_oo quartic terms read off the products of C, H^{ak}_{ci} and A.  Every tensor
@@ -112,8 +112,12 @@ def test_every_tensor_matches_oracle_with_strassen_levels_forced(gpu, o, v, L):
     from oracle.ccsd_oracle import OracleCCSD, unpack_t2
     inp = ci.make_inputs(o, v, L, seed=300 + o + v, b_scale=0.1, f_offdiag=0.05)
     oc = OracleCCSD(inp.h, inp.B, o, v)
-    gc = gpu.CCSD(inp.h, inp.B, o, v, strassen=3)
+    gc = gpu.CCSD(inp.h, inp.B, o, v, strassen=3, gemm_mode=gemm_mode)
     assert gc.strassen_steps() == {"Hvovo_quad": 2, "ring_gemm": 2, "pp_ladder": 2, "C_ovoo": 2}
+    for mode in (1, 2):      # the levels need the 3M kernels with sum planes: forced simple / 4M kernels run plain products
+        other = gpu.CCSD(inp.h, inp.B, o, v, strassen=3, gemm_mode=mode)
+        assert other.strassen_steps() == {}
+        other.close()
     oc.residual()
     gc.residual()
     compare_all(oc, gc)
