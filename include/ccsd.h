@@ -93,8 +93,9 @@ typedef struct {
                            kept (1.75 x - 3 x the bytes of those tensors with their planes); where the ladder and C both use
                            it, the packed <ab||cd> itself is NOT kept beside its stack (ccsd_get_tensor(CCSD_T_VVVV) rebuilds
                            it from the stack, exact up to one rounding per element).  Used on one GPU with the 3M kernels
-                           (gemm_mode 0 or 3) where the products are large enough (ov >= 1024); ignored in cc2 mode and in a
-                           sharded context; with direct_ladder the ladder keeps its slab form.  A workspace that would exceed
+                           (gemm_mode 0 or 3) where the products are large enough (ov >= 1024); ignored in cc2 mode; in a sharded
+                           context the left operands are the rank's row slabs (stacks of this rank's rows only); with
+                           direct_ladder the ladder keeps its slab form.  A workspace that would exceed
                            128 GiB (of a 180 GB part) gives levels up step by step -- the ladder's first, then C's, then the
                            (ov)^3 products' -- down to plain products: ccsd_strassen_info reports what is used.  0 = plain products;
                            2 = one level only; 3 = two levels on all four products whatever their size (tests) */

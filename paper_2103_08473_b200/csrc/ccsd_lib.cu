@@ -341,11 +341,13 @@ static void carve(ccsd_ctx* c, char* base, size_t* total, int degrade)
     c->planes = (c->opt.gemm_mode == 0 && CCSD_DEFAULT_3M != 0) || c->opt.gemm_mode == 3;
     // Strassen levels (strassen.cuh) on the (ov)^3 products, the pp-ladder and the <bk||cd> tau part of C: one GPU, 3M planes.
     // opts.strassen: 1 = levels chosen by size, 2 = one level wherever it pays, 3 = two levels everywhere whatever the size (tests)
+    // In a sharded context the left operands are this rank's row slabs (rov rows of the (ov)^3 products and of C, rw rows of
+    // <ab||cd>); the right operands (G1, T2r, tau) are whole.
     const bool force = c->opt.strassen == 3;
-    c->strassen = c->opt.strassen != 0 && c->planes && c->opt.shard_world <= 1 && !c->opt.cc2 &&
-                  (force ? (o >= 2 && v >= 2) : strassen_worthwhile(ov, ov, ov));
-    bool use_L = c->strassen && !c->opt.direct_ladder && (force || strassen_worthwhile(vv, oo, vv));
-    bool use_C = c->strassen && (force || strassen_worthwhile(ov, oo, vv));
+    const int64_t rov = (int64_t)(c->sh.a_hi - c->sh.a_lo) * o, rw = c->sh.w_hi - c->sh.w_lo;
+    c->strassen = c->opt.strassen != 0 && c->planes && !c->opt.cc2 && (force ? (o >= 2 && v >= 2) : strassen_worthwhile(rov, ov, ov));
+    bool use_L = c->strassen && !c->opt.direct_ladder && (force || strassen_worthwhile(rw, oo, vv));
+    bool use_C = c->strassen && (force || strassen_worthwhile(rov, oo, vv));
     // two levels on the (ov)^3 products where a quarter-size product is still a long-K, many-tile GEMM (measured: 0.80 of the
     // plain product at ov = 7616 against 0.89 for one level; 0.90 against 0.93 at ov = 3840; no gain at 1536)
     c->strassen_levels = force ? 2 : (c->opt.strassen == 2 ? 1 : (ov >= 3072 ? 2 : 1));
@@ -371,8 +373,8 @@ static void carve(ccsd_ctx* c, char* base, size_t* total, int degrade)
     // <ab||cd> is not stored in direct_ladder mode (rebuilt every iteration) nor in CC2 mode (its only use factorises)
     // With the Strassen ladder <ab||cd> lives on as its operand stack only (c->sW; single elements: strassen_left_at).  ccsd_init
     // builds the packed tensor in the memory of C's operand stack, stacks it, and only then fills C's stack (c->W_init).
-    c->W_dropped = use_L && use_C && strassen_stack_elems(ov, vv, c->strassen_levels_C) * (int64_t)(sizeof(c128) + sizeof(double)) >=
-                                         vv * vv * (int64_t)sizeof(c128) + 512;
+    c->W_dropped = use_L && use_C && strassen_stack_elems(rov, vv, c->strassen_levels_C) * (int64_t)(sizeof(c128) + sizeof(double)) >=
+                                         rw * vv * (int64_t)sizeof(c128) + 512;
     c->W_init = nullptr;
     c->W = (c->opt.direct_ladder || c->opt.cc2 || c->W_dropped) ? nullptr : w.take<c128>((c->sh.w_hi - c->sh.w_lo) * vv);   // this rank's rows
     c->Vvovv_p = w.take<c128>(v * o * vv);
@@ -522,24 +524,24 @@ static void carve(ccsd_ctx* c, char* base, size_t* total, int degrade)
             return strassen_stack(S, Sp, R, K, levels);
         };
         const int lvL = c->strassen_levels_L;
-        if (use_L) c->sW = stack(false, vv, vv, lvL);
+        if (use_L) c->sW = stack(false, rw, vv, lvL);
         const int lvC = c->strassen_levels_C;
-        if (use_C) c->sVvovv = stack(false, ov, vv, lvC);
+        if (use_C) c->sVvovv = stack(false, rov, vv, lvC);
         if (c->W_dropped) c->W_init = c->sVvovv.S;      // S and Sp are adjacent: together they hold the packed tensor
         c->sG1 = stack(false, ov, ov, lv);
-        StrassenStack sa = stack(true, ov, ov, lv), sb = stack(true, ov, ov, lv);
-        c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(ov, ov, lv);
+        StrassenStack sa = stack(true, rov, ov, lv), sb = stack(true, ov, ov, lv);
+        c->str_ring.SA = sa.S; c->str_ring.SAp = sa.Sp; c->str_ring.a_elems = strassen_stack_elems(rov, ov, lv);
         c->str_ring.SB = sb.S; c->str_ring.SBp = sb.Sp; c->str_ring.b_elems = strassen_stack_elems(ov, ov, lv);
-        c->str_ring.p_elems = (lv == 2 ? 49 : 7) * strassen_rows(ov, lv) * strassen_rows(ov, lv);
+        c->str_ring.p_elems = (lv == 2 ? 49 : 7) * strassen_rows(rov, lv) * strassen_rows(ov, lv);
         c->str_ring.P = place(c->str_ring.p_elems, sizeof(c128)).take<c128>(c->str_ring.p_elems);
         if ((use_L && lvL == 1) || (use_C && lvC == 1)) c->sTau = stack(true, oo, vv, 1);
         if ((use_L && lvL == 2) || (use_C && lvC == 2)) c->sTauC = stack(true, oo, vv, 2);
         if (use_L) {
-            c->str_L.p_elems = (lvL == 2 ? 49 : 7) * strassen_rows(vv, lvL) * strassen_rows(oo, lvL);
+            c->str_L.p_elems = (lvL == 2 ? 49 : 7) * strassen_rows(rw, lvL) * strassen_rows(oo, lvL);
             c->str_L.P = place(c->str_L.p_elems, sizeof(c128)).take<c128>(c->str_L.p_elems);
         }
         if (use_C) {
-            c->str_C.p_elems = (lvC == 2 ? 49 : 7) * strassen_rows(ov, lvC) * strassen_rows(oo, lvC);
+            c->str_C.p_elems = (lvC == 2 ? 49 : 7) * strassen_rows(rov, lvC) * strassen_rows(oo, lvC);
             c->str_C.P = place(c->str_C.p_elems, sizeof(c128)).take<c128>(c->str_C.p_elems);
         }
     }
@@ -1144,7 +1146,7 @@ static int build_C(ccsd_ctx* c)
     c128* dst = c->s1_trace ? c->Cq : c->Cm + row0 * oo;
     const int acc = c->s1_trace ? 0 : 1;
     if (c->strassen && c->sVvovv.S)
-        CCSD_TRY(strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p, vv, c->taup, vv, dst, oo, 1, -1.0, acc), &c->sVvovv,
+        CCSD_TRY(strassen_gemm(env, gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, dst, oo, 1, -1.0, acc), &c->sVvovv,
                                c->strassen_levels_C == 2 ? &c->sTauC : &c->sTau, c->str_C, c->strassen_levels_C));
     else
         CCSD_TRY(run_gemm(env, with_planes(gp(rows, oo, vv, c->Vvovv_p + row0 * vv, vv, c->taup, vv, dst, oo, 1, -1.0, acc),
@@ -1260,7 +1262,7 @@ static int s2_pp_ladder(ccsd_ctx* c, c128* S)
     }
     const int64_t rows = c->sh.w_hi - c->sh.w_lo;      // this rank's rows of <ab||cd> (all of them for world = 1)
     if (c->strassen && c->sW.S)      // both operand stacks are ready (ccsd_init, prep_operands): one batched launch + the result sums
-        return strassen_gemm(c->env, gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S, 1, c->vv, 1.0, 1), &c->sW,
+        return strassen_gemm(c->env, gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S + c->sh.w_lo, 1, c->vv, 1.0, 1), &c->sW,
                              c->strassen_levels_L == 2 ? &c->sTauC : &c->sTau, c->str_L, c->strassen_levels_L);
     return run_gemm(c->env, with_planes(gp(rows, c->oo, c->vv, c->W, c->vv, c->taup, c->vv, S + c->sh.w_lo, 1, c->vv, 1.0, 1), c->Ws, c->taups));
 }
@@ -1858,7 +1860,8 @@ int ccsd_init(ccsd_ctx** out, const ccsd_c128* h, const ccsd_c128* B, int nocc, 
     int s = build_constants(c, reinterpret_cast<const c128*>(h), reinterpret_cast<const c128*>(B));
     if (s == CCSD_OK && c->strassen) {   // operand stacks of the constants (strassen.cuh), once
         if (c->sW.S) launch_strassen_prep(c->st, 0, c->W ? c->W : c->W_init, c->vv, c->sW);
-        if (c->sVvovv.S) launch_strassen_prep(c->st, 0, c->Vvovv_p, c->vv, c->sVvovv);     // overwrites W_init: after the line above
+        if (c->sVvovv.S)      // this rank's rows (b,k); overwrites W_init: after the line above
+            launch_strassen_prep(c->st, 0, c->Vvovv_p + (int64_t)c->sh.a_lo * c->o * c->vv, c->vv, c->sVvovv);
         launch_strassen_prep(c->st, 1, c->G1, c->ov, c->sG1);
     }
     if (s == CCSD_OK) mp2_guess(c);

@@ -30,8 +30,11 @@ def _rel(a, b):
     return float(np.abs(a - b).max()) / (scale if scale > 0 else 1.0)
 
 
-@pytest.mark.parametrize("o,v,naux,direct", [(6, 21, 30, False), (9, 40, 50, False), (5, 17, 24, True)])
-def test_slabs_tile_the_single_gpu_residual_and_match_the_oracle(gpu, o, v, naux, direct):
+@pytest.mark.parametrize("o,v,naux,direct,strassen", [(6, 21, 30, False, 1), (9, 40, 50, False, 1), (5, 17, 24, True, 1),
+                                                      (6, 21, 30, False, 3), (9, 40, 50, False, 3), (5, 17, 24, True, 3)])
+def test_slabs_tile_the_single_gpu_residual_and_match_the_oracle(gpu, o, v, naux, direct, strassen):
+    """strassen = 3: two Strassen levels forced on every rank's slab products (left operands = the rank's row slabs, odd and empty
+    slabs included), the rank's rows of <ab||cd> kept as their operand stack only."""
     import torch
     from oracle.ccsd_oracle import OracleCCSD, pack_t2, unpack_t2
     inp = ci.make_inputs(o, v, naux, seed=5200 + o + v, b_scale=0.08, f_offdiag=0.05)
@@ -40,7 +43,7 @@ def test_slabs_tile_the_single_gpu_residual_and_match_the_oracle(gpu, o, v, naux
     oc.set_amplitudes(t1, unpack_t2(t2p, o, v))
     S1o, S2o = oc.residual()
     S2o = pack_t2(S2o)
-    one = gpu.CCSD(inp.h, inp.B, o, v, direct_ladder=direct)
+    one = gpu.CCSD(inp.h, inp.B, o, v, direct_ladder=direct, strassen=strassen)
     one.set_amplitudes(t1, t2p)
     one.residual()
     full = {name: one.get_tensor(name).clone() for name in ("S2", "S1", "S2_pp_ladder", "S2_ring", "S2_hh_ladder", "S2_goo",
@@ -51,7 +54,9 @@ def test_slabs_tile_the_single_gpu_residual_and_match_the_oracle(gpu, o, v, naux
         acc = {k: torch.zeros_like(x) for k, x in full.items() if k.startswith("S2")}
         support = torch.zeros_like(full["S2_pp_ladder"], dtype=torch.int32)
         for rank in range(world):
-            gc = gpu.CCSD(inp.h, inp.B, o, v, shard=(rank, world), direct_ladder=direct)
+            gc = gpu.CCSD(inp.h, inp.B, o, v, shard=(rank, world), direct_ladder=direct, strassen=strassen)
+            if strassen == 3 and (info_rows := gc.shard_info()) and info_rows["a_hi"] > info_rows["a_lo"]:
+                assert gc.strassen_steps().get("ring_gemm") == 2
             info = gc.shard_info()
             assert (info["rank"], info["world"]) == (rank, world)
             assert gc.workspace_bytes <= one.workspace_bytes
@@ -87,7 +92,8 @@ def test_slabs_tile_the_single_gpu_residual_and_match_the_oracle(gpu, o, v, naux
         assert _rel(acc["S2"].cpu().numpy().reshape(S2o.shape), S2o) <= REL_TOL, world
 
 
-def test_sharded_iteration_protocol_reproduces_ccsd_iterate(gpu):
+@pytest.mark.parametrize("strassen", [1, 3])
+def test_sharded_iteration_protocol_reproduces_ccsd_iterate(gpu, strassen):
     """residual on every rank -> sum of the S2 slabs written back into every rank's buffer (what the all-reduce does) ->
     ccsd_update on every rank: lock step with the single-GPU ccsd_iterate and with the oracle, DIIS included; every rank ends
     each iteration with identical amplitudes."""
@@ -96,8 +102,8 @@ def test_sharded_iteration_protocol_reproduces_ccsd_iterate(gpu):
     o, v, world = 6, 22, 3
     inp = ci.make_inputs(o, v, 36, seed=5300, b_scale=0.1, f_offdiag=0.05)
     oc = OracleCCSD(inp.h, inp.B, o, v)
-    one = gpu.CCSD(inp.h, inp.B, o, v)
-    ranks = [gpu.CCSD(inp.h, inp.B, o, v, shard=(r, world)) for r in range(world)]
+    one = gpu.CCSD(inp.h, inp.B, o, v, strassen=strassen)
+    ranks = [gpu.CCSD(inp.h, inp.B, o, v, shard=(r, world), strassen=strassen) for r in range(world)]
     for it in range(9):
         eo, so = oc.iterate()
         e1, s1 = one.iterate()
