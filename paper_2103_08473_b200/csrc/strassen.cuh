@@ -1,9 +1,9 @@
 // One or two levels of Strassen's algorithm around the DMMA GEMM (gemm_dmma.cuh) for the large contractions of eq 32 / eqs 29-30
 // (PAPER.md:594-606): C = A B^T with every dimension halved is 7 half-size products instead of 8, i.e. 7/8 of the FP64
 // tensor-pipe work (49 quarter-size products for 64 with two levels: 0.766), for three streaming passes (operand sums,
-// result sums).  All arithmetic stays FP64; the result differs
-// from the plain product by rounding only (measured max error 2-9e-15 of the largest element against 1-5e-15 for the
-// plain 3M product; the parity bound is 1e-12).
+// result sums).  All arithmetic stays FP64; the result differs from the plain product by rounding only (measured max error
+// 2e-15 - 1.2e-14 of the largest element against 1-7e-15 for the plain 3M product; the parity bound
+// is 1e-12).
 //
 // "NT" convention of the library: C[m][n] = sum_k A[m][k] B[n][k].  Quadrants by halves (Mh, Nh, Kh = ceil of half the
 // extent, Kh rounded up to even so that plane rows stay 16-byte aligned; what lies beyond the extent reads as zero):
