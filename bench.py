@@ -839,6 +839,24 @@ def run_ours(args) -> None:
         o, v = (int(x) for x in args.ladder_shape.split(","))
         oo, vv = ci.pair_count(o), ci.pair_count(v)
         cfg = f"nocc={o} nvir={v}"
+    if args.only_ov3:
+        # profiling aid: the (ov)^3 product X[(a,i)][(j,b)] = sum_{(c,k)} H[(a,i)][(c,k)] T[(j,b)][(c,k)] of this workload's shape the
+        # way ccsd_iterate runs it (operand stacks, ONE batched launch of the 7 / 49 products, result sum)
+        pkg.load_library()
+        gen = torch.Generator(device="cuda"); gen.manual_seed(seed)
+        H = torch.view_as_complex(torch.randn((ov, ov, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(0.05)
+        T = torch.view_as_complex(torch.randn((ov, ov, 2), generator=gen, device="cuda", dtype=torch.float64)).mul_(0.01)
+        X = torch.zeros((ov, ov), dtype=torch.complex128, device="cuda")
+        levels = {0: 0, 2: 1, 3: 2}.get(args.strassen, 2 if ov >= 3072 else (1 if ov >= 1024 else 0))
+        if levels:
+            ts = time_events(torch, lambda: pkg.zgemm_nt_strassen(H, T, C=X, levels=levels), args.steps, args.warmup)
+        else:
+            ts = time_events(torch, lambda: pkg.zgemm_nt(H, T, C=X), args.steps, args.warmup)
+        t = statistics.median(ts)
+        print(json.dumps({"metric": "ov3_product_call_ms", "value": t, "unit": "ms", "levels": levels,
+                          "config": {"workload": f"{cfg} (ov)^3 product {ov}x{ov}x{ov}, {levels} Strassen level(s); the call includes "
+                                                 "the binding's workspace allocation"}}))
+        return
     if args.only_ladder:
         # profiling aid: just the pp-ladder launch of this workload's shape (same kernel, same launch configuration
         # as inside ccsd_iterate), W warm-ups + K timed launches
@@ -1020,6 +1038,8 @@ def main():
                                                           "branches, 3 serial graph (profiling aid)")
     ap.add_argument("--strassen", type=int, default=1, help="ccsd_options.strassen of the main leg: 1 (default) Strassen levels on "
                     "the four large contractions, 0 plain products, 2 one level only, 3 two levels everywhere (tests)")
+    ap.add_argument("--only-ov3", action="store_true", help="profiling aid: the (ov)^3 product of --config's shape through "
+                    "ccsd_zgemm_nt_strassen with the level count of the iteration (the batched launch of the ring / H^{ak}_{ci} terms)")
     ap.add_argument("--only-ladder", action="store_true", help="time only the pp-ladder launch of --config's shape")
     ap.add_argument("--ladder-shape", default="", help="with --only-ladder: 'nocc,nvir' of a BASELINE config-4 sweep shape")
     ap.add_argument("--only-lambda", action="store_true", help="time only the Lambda equations of --config")
